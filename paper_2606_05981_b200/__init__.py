@@ -1,0 +1,220 @@
+"""paper_2606_05981_b200 — Python binding of the B200-native batched-prefill text encoder.
+
+Thin ctypes layer over the C ABI in include/te.h (same entry-point names; argument
+marshalling only — every step of the hot path runs in the CUDA kernels of libte_b200.so).
+PyTorch appears only as the owner of device memory / streams handed in by the caller.
+There is no CPU fallback: if the shared library is missing or the device is not sm_100 the
+calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import (POINTER, Structure, byref, c_char_p, c_double, c_float, c_int, c_int32, c_int64,
+                    c_size_t, c_void_p)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libte_b200.so")
+
+TE_OK = 0
+TE_ERR_INVALID_ARG, TE_ERR_NOT_LOADED, TE_ERR_BLOB_SIZE = -1, -2, -3
+TE_ERR_CUDA, TE_ERR_UNSUPPORTED, TE_ERR_DEVICE_CHECK = -4, -5, -6
+TE_OPT_USE_GRAPH = 0
+TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT = range(7)
+
+EXPORTS = [
+    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_host",
+    "te_query_async_error", "te_set_option", "te_kernel_launches", "te_debug_set_range",
+    "te_debug_tap", "te_debug_gemm", "te_destroy", "te_strerror", "te_last_error",
+]
+
+
+class TEConfig(Structure):
+    """Mirror of `te_config` (include/te.h)."""
+    _fields_ = [
+        ("n_layers", c_int32), ("hidden", c_int32), ("n_q_heads", c_int32), ("n_kv_heads", c_int32),
+        ("head_dim", c_int32), ("ffn", c_int32),
+        ("rope_sec_t", c_int32), ("rope_sec_h", c_int32), ("rope_sec_w", c_int32),
+        ("rms_eps", c_float), ("rope_theta", c_double),
+        ("max_frames", c_int32), ("max_tokens", c_int32), ("max_tokens_per_frame", c_int32),
+        ("final_norm", c_int32),
+    ]
+
+
+class TEError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"te error {code}: {msg}")
+        self.code = code
+
+
+_lib_cache = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libte_b200.so (built in-tree by `python -m paper_2606_05981_b200.build`)."""
+    global _lib_cache
+    if _lib_cache is not None:
+        return _lib_cache
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(
+            f"{LIB_PATH} not found: build it with `python -m paper_2606_05981_b200.build` "
+            "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    L.te_blob_bytes.restype = c_size_t
+    L.te_blob_bytes.argtypes = [POINTER(TEConfig)]
+    L.te_create.restype = c_int
+    L.te_create.argtypes = [POINTER(TEConfig), c_int, POINTER(c_void_p)]
+    L.te_load_weights.restype = c_int
+    L.te_load_weights.argtypes = [c_void_p, c_void_p, c_size_t]
+    L.te_encode.restype = c_int
+    L.te_encode.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_int32, c_void_p, c_void_p]
+    L.te_encode_host.restype = c_int
+    L.te_encode_host.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_void_p]
+    L.te_query_async_error.restype = c_int
+    L.te_query_async_error.argtypes = [c_void_p]
+    L.te_set_option.restype = c_int
+    L.te_set_option.argtypes = [c_void_p, c_int, c_int]
+    L.te_kernel_launches.restype = c_int64
+    L.te_kernel_launches.argtypes = [c_void_p]
+    L.te_debug_set_range.restype = c_int
+    L.te_debug_set_range.argtypes = [c_void_p, c_int32, c_int32, c_int32]
+    L.te_debug_tap.restype = c_int
+    L.te_debug_tap.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
+    L.te_debug_gemm.restype = c_int
+    L.te_debug_gemm.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
+    L.te_destroy.restype = None
+    L.te_destroy.argtypes = [c_void_p]
+    L.te_strerror.restype = c_char_p
+    L.te_strerror.argtypes = [c_int]
+    L.te_last_error.restype = c_char_p
+    L.te_last_error.argtypes = [c_void_p]
+    _lib_cache = L
+    return L
+
+
+def _ptr(x) -> int:
+    """Raw address of a torch tensor / numpy array / int."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if hasattr(x, "ctypes"):
+        return int(x.ctypes.data)
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _check(code: int, h=None):
+    if code != TE_OK:
+        L = lib()
+        msg = L.te_strerror(code).decode()
+        if h:
+            extra = L.te_last_error(h).decode()
+            if extra:
+                msg += f" ({extra})"
+        raise TEError(code, msg)
+
+
+def make_config(model, max_frames: int, max_tokens: int, max_tokens_per_frame: int = 256,
+                final_norm: int | None = None) -> TEConfig:
+    """TEConfig from a workloads.TEModelConfig-like object (duck-typed)."""
+    s_t, s_h, s_w = model.rope_sections
+    return TEConfig(model.n_layers, model.hidden, model.n_q_heads, model.n_kv_heads, model.head_dim,
+                    model.ffn, s_t, s_h, s_w, model.rms_eps, model.rope_theta, max_frames, max_tokens,
+                    max_tokens_per_frame, model.final_norm if final_norm is None else final_norm)
+
+
+# ---------------------------------------------------------------- C-ABI names, marshalling only
+def te_blob_bytes(cfg: TEConfig) -> int:
+    return int(lib().te_blob_bytes(byref(cfg)))
+
+
+def te_create(cfg: TEConfig, device: int = 0) -> c_void_p:
+    h = c_void_p()
+    _check(lib().te_create(byref(cfg), device, byref(h)))
+    return h
+
+
+def te_load_weights(h, blob, n_bytes: int | None = None):
+    """blob: numpy uint16 array / torch tensor (host or device) holding bf16 bits."""
+    if n_bytes is None:
+        n_bytes = int(blob.nbytes) if hasattr(blob, "nbytes") else int(blob.numel() * blob.element_size())
+    _check(lib().te_load_weights(h, _ptr(blob), n_bytes), h)
+
+
+def te_encode(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream=None):
+    """embeds/out: DEVICE fp32 [T, d]; text_lens: DEVICE int32 [B]; stream: cudaStream_t as int."""
+    _check(lib().te_encode(h, n_frames, grid_h, grid_w, _ptr(embeds), _ptr(text_lens), total_tokens,
+                           _ptr(out), _ptr(stream)), h)
+
+
+def te_encode_host(h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host):
+    _check(lib().te_encode_host(h, n_frames, grid_h, grid_w, _ptr(embeds_host), _ptr(text_lens_host),
+                                _ptr(out_host)), h)
+
+
+def te_query_async_error(h) -> int:
+    return int(lib().te_query_async_error(h))
+
+
+def te_set_option(h, option: int, value: int):
+    _check(lib().te_set_option(h, option, value), h)
+
+
+def te_kernel_launches(h) -> int:
+    return int(lib().te_kernel_launches(h))
+
+
+def te_debug_set_range(h, layer_begin: int, layer_end: int, stop_after_attn: int = 0):
+    _check(lib().te_debug_set_range(h, layer_begin, layer_end, stop_after_attn), h)
+
+
+def te_debug_tap(h, what: int, dst_host):
+    _check(lib().te_debug_tap(h, what, _ptr(dst_host), int(dst_host.nbytes)), h)
+
+
+def te_debug_gemm(device, a_bf16, b_bf16, c, m, n, k, block_n=256):
+    _check(lib().te_debug_gemm(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n))
+
+
+def te_destroy(h):
+    lib().te_destroy(h)
+
+
+def te_strerror(code: int) -> str:
+    return lib().te_strerror(code).decode()
+
+
+def te_last_error(h) -> str:
+    return lib().te_last_error(h).decode()
+
+
+class TextEncoder:
+    """Convenience owner of a handle (create -> load -> encode -> destroy)."""
+
+    def __init__(self, model, max_frames: int, max_tokens: int, device: int = 0,
+                 max_tokens_per_frame: int = 256, final_norm: int | None = None):
+        self.model = model
+        self.cfg = make_config(model, max_frames, max_tokens, max_tokens_per_frame, final_norm)
+        self.h = te_create(self.cfg, device)
+
+    def load_weights(self, blob):
+        te_load_weights(self.h, blob)
+
+    def encode(self, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream=None):
+        te_encode(self.h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream)
+
+    def encode_host(self, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host):
+        te_encode_host(self.h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host)
+
+    def close(self):
+        if self.h:
+            te_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

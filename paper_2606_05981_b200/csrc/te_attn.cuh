@@ -1,0 +1,219 @@
+// te_attn.cuh — causal GQA flash-attention prefill, varlen-packed across frames (SURVEY.md §8(a)
+// row a2): per frame b and q head a (kv head a / G): P = softmax(q k^T / sqrt(dh) + causal),
+// o = P v, fp32 online softmax, causal by sequence index within the frame.
+//
+// Sequences are short (S_b <= 256) and attention is < 1 % of the stack's FLOPs, so this kernel is
+// latency/occupancy-bound, not tensor-bound: one CTA = 64 query rows of one (frame, q head),
+// 4 warps x 16 rows, K/V streamed through shared memory in 64-key blocks, bf16 mma.sync
+// m16n8k16 with fp32 accumulation, several CTAs resident per SM.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace te {
+
+constexpr int ATT_BQ = 64;
+constexpr int ATT_BKV = 64;
+constexpr int ATT_THREADS = 128;
+
+struct AttnParams {
+  const __nv_bfloat16* qkv;  // [T, ld] : q heads | k heads | v heads
+  __nv_bfloat16* out;        // [T, Hq*DH]
+  const int32_t* cu_seqlens; // [B+1]
+  int ld;
+  int n_q_heads, n_kv_heads;
+  int total_tokens;
+  float scale_log2;  // log2(e) / sqrt(dh)
+};
+
+template <int DH>
+struct AttnCfg {
+  static constexpr int ROW = DH + 8;  // padded row (elements): 16 B pad -> conflict-free ldmatrix
+  static constexpr int SMEM_BYTES = (ATT_BQ + 2 * ATT_BKV) * ROW * 2;
+};
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, bool pred) {
+  const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
+  const int sz = pred ? 16 : 0;  // src-size 0 -> zero fill
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+  asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], const void* p) {
+  const uint32_t a = static_cast<uint32_t>(__cvta_generic_to_shared(p));
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(a));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], const void* p) {
+  const uint32_t a = static_cast<uint32_t>(__cvta_generic_to_shared(p));
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(a));
+}
+__device__ __forceinline__ void mma_bf16_16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack2_bf16(float a, float b) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// grid: (q blocks, Hq, B); block: 128 threads
+template <int DH>
+__global__ void __launch_bounds__(ATT_THREADS, 3) te_attn_kernel(const AttnParams p) {
+  using Cfg = AttnCfg<DH>;
+  constexpr int ROW = Cfg::ROW;
+  extern __shared__ __align__(16) uint8_t att_smem[];
+  __nv_bfloat16* sQ = reinterpret_cast<__nv_bfloat16*>(att_smem);
+  __nv_bfloat16* sK = sQ + ATT_BQ * ROW;
+  __nv_bfloat16* sV = sK + ATT_BKV * ROW;
+
+  const int b = blockIdx.z;
+  const int head = blockIdx.y;
+  const int qb = blockIdx.x;
+  const int seq0 = p.cu_seqlens[b];
+  const int S = min(p.cu_seqlens[b + 1], p.total_tokens) - seq0;
+  const int q0 = qb * ATT_BQ;
+  if (q0 >= S) return;
+  const int kvh = head / (p.n_q_heads / p.n_kv_heads);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, t = lane & 3;
+
+  const __nv_bfloat16* gq = p.qkv + (size_t)seq0 * p.ld + head * DH;
+  const __nv_bfloat16* gk = p.qkv + (size_t)seq0 * p.ld + (p.n_q_heads + kvh) * DH;
+  const __nv_bfloat16* gv = p.qkv + (size_t)seq0 * p.ld + (p.n_q_heads + p.n_kv_heads + kvh) * DH;
+
+  constexpr int CH = DH / 8;  // 16-byte chunks per row
+  for (int i = tid; i < ATT_BQ * CH; i += ATT_THREADS) {
+    const int r = i / CH, c = i % CH;
+    cp_async16(sQ + r * ROW + c * 8, gq + (size_t)(q0 + r) * p.ld + c * 8, q0 + r < S);
+  }
+
+  float o[DH / 8][4];
+#pragma unroll
+  for (int i = 0; i < DH / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+  float m_run[2] = {-INFINITY, -INFINITY};
+  float l_run[2] = {0.f, 0.f};
+  const int qrow0 = q0 + warp * 16 + g;  // this thread's rows: qrow0 and qrow0 + 8 (index within the frame)
+
+  const int n_kv_blocks = qb + 1;  // causal: keys [0, q0 + 64)
+  for (int kb = 0; kb < n_kv_blocks; ++kb) {
+    const int k0 = kb * ATT_BKV;
+    __syncthreads();  // previous block's smem reads are done
+    for (int i = tid; i < ATT_BKV * CH; i += ATT_THREADS) {
+      const int r = i / CH, c = i % CH;
+      const bool ok = k0 + r < S;
+      cp_async16(sK + r * ROW + c * 8, gk + (size_t)(k0 + r) * p.ld + c * 8, ok);
+      cp_async16(sV + r * ROW + c * 8, gv + (size_t)(k0 + r) * p.ld + c * 8, ok);
+    }
+    cp_async_wait_all();
+    __syncthreads();
+
+    // ---- S = Q K^T  (16 x 64 per warp)
+    float s[ATT_BKV / 8][4];
+#pragma unroll
+    for (int i = 0; i < ATT_BKV / 8; ++i) s[i][0] = s[i][1] = s[i][2] = s[i][3] = 0.f;
+#pragma unroll
+    for (int kk = 0; kk < DH / 16; ++kk) {
+      uint32_t a[4];
+      {
+        const int mi = lane >> 3, r = lane & 7;
+        ldsm_x4(a, sQ + (warp * 16 + (mi & 1) * 8 + r) * ROW + kk * 16 + (mi >> 1) * 8);
+      }
+#pragma unroll
+      for (int nt = 0; nt < ATT_BKV / 16; ++nt) {
+        uint32_t bfr[4];
+        const int mi = lane >> 3, r = lane & 7;
+        ldsm_x4(bfr, sK + (nt * 16 + (mi >> 1) * 8 + r) * ROW + kk * 16 + (mi & 1) * 8);
+        mma_bf16_16816(s[2 * nt], a, bfr[0], bfr[1]);
+        mma_bf16_16816(s[2 * nt + 1], a, bfr[2], bfr[3]);
+      }
+    }
+    // ---- causal mask (only the diagonal block needs it) + online softmax
+    if (kb == qb) {
+#pragma unroll
+      for (int nt = 0; nt < ATT_BKV / 8; ++nt) {
+        const int key = k0 + nt * 8 + 2 * t;
+        if (key > qrow0) s[nt][0] = -INFINITY;
+        if (key + 1 > qrow0) s[nt][1] = -INFINITY;
+        if (key > qrow0 + 8) s[nt][2] = -INFINITY;
+        if (key + 1 > qrow0 + 8) s[nt][3] = -INFINITY;
+      }
+    }
+    float mx[2] = {-INFINITY, -INFINITY};
+#pragma unroll
+    for (int nt = 0; nt < ATT_BKV / 8; ++nt) {
+      mx[0] = fmaxf(mx[0], fmaxf(s[nt][0], s[nt][1]));
+      mx[1] = fmaxf(mx[1], fmaxf(s[nt][2], s[nt][3]));
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      mx[i] = fmaxf(mx[i], __shfl_xor_sync(0xffffffffu, mx[i], 1));
+      mx[i] = fmaxf(mx[i], __shfl_xor_sync(0xffffffffu, mx[i], 2));
+    }
+    float corr[2], msc[2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const float m_new = fmaxf(m_run[i], mx[i]);  // key 0 is always visible -> finite from the first block on
+      corr[i] = exp2f((m_run[i] - m_new) * p.scale_log2);
+      m_run[i] = m_new;
+      msc[i] = m_new * p.scale_log2;
+    }
+    float rs[2] = {0.f, 0.f};
+#pragma unroll
+    for (int nt = 0; nt < ATT_BKV / 8; ++nt) {
+      s[nt][0] = exp2f(fmaf(s[nt][0], p.scale_log2, -msc[0]));
+      s[nt][1] = exp2f(fmaf(s[nt][1], p.scale_log2, -msc[0]));
+      s[nt][2] = exp2f(fmaf(s[nt][2], p.scale_log2, -msc[1]));
+      s[nt][3] = exp2f(fmaf(s[nt][3], p.scale_log2, -msc[1]));
+      rs[0] += s[nt][0] + s[nt][1];
+      rs[1] += s[nt][2] + s[nt][3];
+    }
+    l_run[0] = l_run[0] * corr[0] + rs[0];
+    l_run[1] = l_run[1] * corr[1] + rs[1];
+#pragma unroll
+    for (int i = 0; i < DH / 8; ++i) {
+      o[i][0] *= corr[0]; o[i][1] *= corr[0];
+      o[i][2] *= corr[1]; o[i][3] *= corr[1];
+    }
+    // ---- O += P V
+#pragma unroll
+    for (int kk = 0; kk < ATT_BKV / 16; ++kk) {
+      uint32_t a[4];
+      a[0] = pack2_bf16(s[2 * kk][0], s[2 * kk][1]);
+      a[1] = pack2_bf16(s[2 * kk][2], s[2 * kk][3]);
+      a[2] = pack2_bf16(s[2 * kk + 1][0], s[2 * kk + 1][1]);
+      a[3] = pack2_bf16(s[2 * kk + 1][2], s[2 * kk + 1][3]);
+#pragma unroll
+      for (int nt = 0; nt < DH / 16; ++nt) {
+        uint32_t bfr[4];
+        const int mi = lane >> 3, r = lane & 7;
+        ldsm_x4_t(bfr, sV + (kk * 16 + (mi & 1) * 8 + r) * ROW + nt * 16 + (mi >> 1) * 8);
+        mma_bf16_16816(o[2 * nt], a, bfr[0], bfr[1]);
+        mma_bf16_16816(o[2 * nt + 1], a, bfr[2], bfr[3]);
+      }
+    }
+  }
+  // ---- finalize: row sums across the 4 threads of a row, normalise, store
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    l_run[i] += __shfl_xor_sync(0xffffffffu, l_run[i], 1);
+    l_run[i] += __shfl_xor_sync(0xffffffffu, l_run[i], 2);
+  }
+  const float inv0 = 1.0f / l_run[0], inv1 = 1.0f / l_run[1];
+  __nv_bfloat16* out0 = p.out + (size_t)(seq0 + qrow0) * (p.n_q_heads * DH) + head * DH + 2 * t;
+  __nv_bfloat16* out1 = out0 + (size_t)8 * (p.n_q_heads * DH);
+#pragma unroll
+  for (int nt = 0; nt < DH / 8; ++nt) {
+    if (qrow0 < S) *reinterpret_cast<uint32_t*>(out0 + nt * 8) = pack2_bf16(o[nt][0] * inv0, o[nt][1] * inv0);
+    if (qrow0 + 8 < S) *reinterpret_cast<uint32_t*>(out1 + nt * 8) = pack2_bf16(o[nt][2] * inv1, o[nt][3] * inv1);
+  }
+}
+
+}  // namespace te

@@ -1,0 +1,143 @@
+// te_prep.cuh — a0 of SURVEY.md §8(a): packing offsets, 3D M-RoPE position ids and the rotary
+// cos/sin table computed ON THE DEVICE from text_lens (this replaces the `.item()` host
+// round-trip the paper locates in the TE's rotary code), plus the initial
+// copy embeds -> fp32 residual (= out) with the first layer's RMSNorm statistics.
+// Also: final RMSNorm (a6) and the gate/up weight interleave used by te_load_weights.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace te {
+
+enum { FLAG_BAD_LEN = 1, FLAG_BAD_TOTAL = 2, FLAG_TOO_LONG = 4 };
+
+// One block; thread 0 scans (B is at most a few thousand).  cu[b] is clamped to total_tokens so
+// that later kernels never touch rows beyond the caller's buffers even when validation fails.
+__global__ void te_scan_kernel(const int32_t* __restrict__ text_lens, int n_frames, int n_vis, int total_tokens,
+                               int max_tokens_per_frame, int32_t* __restrict__ cu, int32_t* __restrict__ flag) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  long long acc = 0;
+  int f = 0;
+  cu[0] = 0;
+  for (int b = 0; b < n_frames; ++b) {
+    int tl = text_lens[b];
+    if (tl < 0) { f |= FLAG_BAD_LEN; tl = 0; }
+    const int s = n_vis + tl;
+    if (s > max_tokens_per_frame) f |= FLAG_TOO_LONG;
+    acc += s;
+    cu[b + 1] = static_cast<int32_t>(acc < total_tokens ? acc : total_tokens);
+  }
+  if (acc != total_tokens) f |= FLAG_BAD_TOTAL;
+  if (f) atomicOr(flag, f);
+}
+
+struct PrepParams {
+  const float* embeds;  // [T, d]
+  float* out;           // [T, d]  fp32 residual stream
+  const int32_t* cu;    // [B+1]
+  int32_t* pos;         // [3, T]
+  float* cos_t;         // [T, dh/2]
+  float* sin_t;
+  const double* inv_freq;       // [dh/2]  omega_i = theta^(-2i/dh)
+  const __nv_bfloat16* g_first; // gain of the first RMSNorm that will consume the residual
+  __nv_bfloat16* xg;            // [T, d]  bf16(x * g_first)
+  float* ssq;                   // [parts][ssq_stride]
+  int ssq_parts, ssq_stride;
+  int n_frames, total_tokens, d, half_dim;
+  int grid_h, grid_w, sec_t, sec_h;
+};
+
+// One warp per token.
+__global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int tok = blockIdx.x * 8 + warp;
+  if (tok >= p.total_tokens) return;
+  // frame of this token: largest b with cu[b] <= tok
+  int lo = 0, hi = p.n_frames - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (p.cu[mid] <= tok) lo = mid; else hi = mid - 1;
+  }
+  const int n = tok - p.cu[lo];
+  const int n_vis = p.grid_h * p.grid_w;
+  int pt, ph, pw;
+  if (n < n_vis) {
+    pt = 0; ph = n / p.grid_w; pw = n % p.grid_w;     // visual token: row-major grid, t = 0
+  } else {
+    pt = ph = pw = max(p.grid_h, p.grid_w) + (n - n_vis);  // text: continues from max grid id + 1
+  }
+  if (lane == 0) {
+    p.pos[tok] = pt;
+    p.pos[p.total_tokens + tok] = ph;
+    p.pos[2 * p.total_tokens + tok] = pw;
+  }
+  for (int i = lane; i < p.half_dim; i += 32) {
+    const int pid = (i < p.sec_t) ? pt : ((i < p.sec_t + p.sec_h) ? ph : pw);
+    double s, c;
+    sincos(static_cast<double>(pid) * p.inv_freq[i], &s, &c);
+    p.cos_t[(size_t)tok * p.half_dim + i] = static_cast<float>(c);
+    p.sin_t[(size_t)tok * p.half_dim + i] = static_cast<float>(s);
+  }
+  // residual copy + sum of squares + bf16(x * g)
+  const float4* src = reinterpret_cast<const float4*>(p.embeds + (size_t)tok * p.d);
+  float4* dst = reinterpret_cast<float4*>(p.out + (size_t)tok * p.d);
+  float ss = 0.f;
+  for (int c4 = lane; c4 < p.d / 4; c4 += 32) {
+    const float4 v = __ldg(src + c4);
+    dst[c4] = v;
+    ss = fmaf(v.x, v.x, ss); ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
+    const uint2 g = __ldg(reinterpret_cast<const uint2*>(p.g_first) + c4);
+    __nv_bfloat162 o0 = __floats2bfloat162_rn(v.x * __uint_as_float(g.x << 16), v.y * __uint_as_float(g.x & 0xFFFF0000u));
+    __nv_bfloat162 o1 = __floats2bfloat162_rn(v.z * __uint_as_float(g.y << 16), v.w * __uint_as_float(g.y & 0xFFFF0000u));
+    uint2 o;
+    o.x = *reinterpret_cast<uint32_t*>(&o0);
+    o.y = *reinterpret_cast<uint32_t*>(&o1);
+    reinterpret_cast<uint2*>(p.xg + (size_t)tok * p.d)[c4] = o;
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
+  if (lane == 0) {
+    p.ssq[tok] = ss;
+    for (int i = 1; i < p.ssq_parts; ++i) p.ssq[(size_t)i * p.ssq_stride + tok] = 0.f;
+  }
+}
+
+// a6: out <- RMSNorm(out; gf), fp32, one warp per row.
+__global__ void __launch_bounds__(256) te_final_norm_kernel(float* __restrict__ x, const __nv_bfloat16* __restrict__ gf,
+                                                            int total_tokens, int d, float eps) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int tok = blockIdx.x * 8 + warp;
+  if (tok >= total_tokens) return;
+  float4* row = reinterpret_cast<float4*>(x + (size_t)tok * d);
+  float ss = 0.f;
+  for (int c4 = lane; c4 < d / 4; c4 += 32) {
+    const float4 v = row[c4];
+    ss = fmaf(v.x, v.x, ss); ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
+  const float rstd = 1.0f / sqrtf(ss / static_cast<float>(d) + eps);
+  for (int c4 = lane; c4 < d / 4; c4 += 32) {
+    float4 v = row[c4];
+    const uint2 g = __ldg(reinterpret_cast<const uint2*>(gf) + c4);
+    v.x = v.x * rstd * __uint_as_float(g.x << 16);
+    v.y = v.y * rstd * __uint_as_float(g.x & 0xFFFF0000u);
+    v.z = v.z * rstd * __uint_as_float(g.y << 16);
+    v.w = v.w * rstd * __uint_as_float(g.y & 0xFFFF0000u);
+    row[c4] = v;
+  }
+}
+
+// te_load_weights: interleave [Wgate; Wup] per N-tile of `bn` rows so that one GEMM tile holds
+// matching gate (first bn/2 rows) and up (last bn/2 rows) columns.  One block per destination row.
+__global__ void te_interleave_gate_up_kernel(const uint4* __restrict__ gate, const uint4* __restrict__ up,
+                                             uint4* __restrict__ dst, int ffn, int row_vec16, int bn) {
+  const int r = blockIdx.x;  // destination row in [0, 2*ffn)
+  const int tile = r / bn, within = r % bn, half = bn / 2;
+  const uint4* src = (within < half) ? gate + (size_t)(tile * half + within) * row_vec16
+                                     : up + (size_t)(tile * half + within - half) * row_vec16;
+  for (int i = threadIdx.x; i < row_vec16; i += blockDim.x) dst[(size_t)r * row_vec16 + i] = src[i];
+}
+
+}  // namespace te

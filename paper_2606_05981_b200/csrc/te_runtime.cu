@@ -1,0 +1,626 @@
+// te_runtime.cu — host runtime + C ABI (include/te.h): handle, weight repack, workspace,
+// tensor maps, kernel sequencing and the CUDA-graph cache.  One graph launch per te_encode.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/te.h"
+#include "te_attn.cuh"
+#include "te_gemm.cuh"
+#include "te_prep.cuh"
+
+namespace {
+
+using bf16 = __nv_bfloat16;
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+PFN_encodeTiled get_encode_fn() {
+  static PFN_encodeTiled fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_encodeTiled>(p);
+  }
+  return fn;
+}
+
+// 2-D bf16 row-major [rows, cols] tensor, box = [box_rows, 64 cols], 128-byte swizzle.
+bool make_tmap(CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols * sizeof(bf16)};
+  cuuint32_t box[2] = {64, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+struct LayerOff {
+  size_t g1, wqkv, gq, gk, wo, g2, wgu, wd;  // element offsets into the device weight buffer
+};
+
+struct GraphKey {
+  int n_frames, grid_h, grid_w, total_tokens, lb, le, stop;
+  const void *embeds, *lens, *out;
+  bool operator==(const GraphKey& o) const { return memcmp(this, &o, sizeof(GraphKey)) == 0; }
+};
+struct GraphEntry {
+  GraphKey key;
+  cudaGraphExec_t exec;
+  cudaGraph_t graph;
+  int n_kernels;
+  uint64_t stamp;
+};
+
+}  // namespace
+
+struct te_handle {
+  te_config cfg{};
+  int device = 0;
+  int sm_count = 0;
+  bool loaded = false;
+  // tile choices
+  int bn_qkv = 256, bn_gu = 256, bn_res = 256;
+  // weights
+  bf16* w = nullptr;
+  size_t w_elems = 0;
+  std::vector<LayerOff> off;
+  size_t gf_off = 0;
+  std::vector<CUtensorMap> tm_qkv, tm_o, tm_gu, tm_d;
+  // workspace
+  int32_t *cu = nullptr, *pos = nullptr, *flag = nullptr;
+  float *cos_t = nullptr, *sin_t = nullptr, *ssq = nullptr;
+  double* inv_freq = nullptr;
+  bf16 *xg = nullptr, *qkv = nullptr, *attn = nullptr, *act = nullptr;
+  int ssq_parts_cap = 0;
+  // host-path staging
+  float *stg_embeds = nullptr, *stg_out = nullptr;
+  int32_t* stg_lens = nullptr;
+  cudaStream_t own_stream = nullptr;
+  // graphs
+  std::vector<GraphEntry> cache;
+  uint64_t stamp = 0;
+  int use_graph = 1;
+  int dbg_lb = 0, dbg_le = 0, dbg_stop = 0;
+  int last_T = 0, last_B = 0;
+  long long launches = 0;
+  std::string err;
+};
+
+namespace {
+
+#define TE_CUDA(h, expr)                                                                      \
+  do {                                                                                        \
+    cudaError_t _e = (expr);                                                                  \
+    if (_e != cudaSuccess) {                                                                  \
+      (h)->err = std::string(#expr) + ": " + cudaGetErrorString(_e);                          \
+      return TE_ERR_CUDA;                                                                     \
+    }                                                                                         \
+  } while (0)
+
+size_t layer_elems(const te_config& c) {
+  const size_t d = c.hidden, dh = c.head_dim, F = c.ffn;
+  return d + (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * dh * d + 2 * dh + d * (size_t)c.n_q_heads * dh + d +
+         2 * F * d + d * F;
+}
+size_t blob_elems(const te_config& c) { return layer_elems(c) * c.n_layers + c.hidden; }
+
+int validate_config(const te_config& c) {
+  if (c.n_layers < 1 || c.hidden < 1 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.ffn < 1) return TE_ERR_INVALID_ARG;
+  if (c.n_q_heads % c.n_kv_heads != 0) return TE_ERR_INVALID_ARG;
+  if (c.rope_sec_t < 0 || c.rope_sec_h < 0 || c.rope_sec_w < 0) return TE_ERR_INVALID_ARG;
+  if (c.rope_sec_t + c.rope_sec_h + c.rope_sec_w != c.head_dim / 2) return TE_ERR_INVALID_ARG;
+  if (c.max_frames < 1 || c.max_tokens < 1 || c.max_tokens_per_frame < 1) return TE_ERR_INVALID_ARG;
+  if (!(c.rms_eps > 0.f) || !(c.rope_theta > 0.0)) return TE_ERR_INVALID_ARG;
+  if (c.head_dim != 64 && c.head_dim != 128) return TE_ERR_UNSUPPORTED;
+  if (c.hidden % 128 != 0 || c.ffn % 128 != 0) return TE_ERR_UNSUPPORTED;
+  if (((c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim) % 128 != 0) return TE_ERR_UNSUPPORTED;
+  if ((c.n_q_heads * c.head_dim) % 64 != 0) return TE_ERR_UNSUPPORTED;
+  if (c.max_tokens_per_frame > 256) return TE_ERR_UNSUPPORTED;
+  return TE_OK;
+}
+
+template <int BN, int EPI, int DH>
+cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, int sm_count,
+                        cudaStream_t st) {
+  using Cfg = te::GemmCfg<BN>;
+  const int tiles = p.num_m_blk * p.num_n_blk;
+  const int grid = tiles < sm_count ? tiles : sm_count;
+  te::te_gemm_kernel<BN, EPI, DH><<<grid, te::GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, p);
+  return cudaGetLastError();
+}
+
+template <int EPI>
+cudaError_t launch_gemm_bn(int bn, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p, int sms,
+                           cudaStream_t st) {
+  if constexpr (EPI == te::EPI_QKV) {
+    if (bn == 256 && dh == 128) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
+    if (bn == 256 && dh == 64) return launch_gemm<256, EPI, 64>(a, b, p, sms, st);
+    if (bn == 128 && dh == 128) return launch_gemm<128, EPI, 128>(a, b, p, sms, st);
+    return launch_gemm<128, EPI, 64>(a, b, p, sms, st);
+  } else {
+    if (bn == 256) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
+    return launch_gemm<128, EPI, 128>(a, b, p, sms, st);
+  }
+}
+
+template <int DH>
+cudaError_t launch_attn(const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
+  using Cfg = te::AttnCfg<DH>;
+  dim3 grid(q_blocks, p.n_q_heads, n_frames);
+  te::te_attn_kernel<DH><<<grid, te::ATT_THREADS, Cfg::SMEM_BYTES, st>>>(p);
+  return cudaGetLastError();
+}
+
+template <int BN, int EPI, int DH>
+cudaError_t set_gemm_attr() {
+  return cudaFuncSetAttribute(te::te_gemm_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              te::GemmCfg<BN>::SMEM_BYTES);
+}
+// Opt every kernel instantiation into its dynamic shared-memory size (once per process, outside
+// any stream capture).
+cudaError_t init_kernel_attrs() {
+  cudaError_t e;
+#define TE_ATTR(call) if ((e = (call)) != cudaSuccess) return e
+  TE_ATTR((set_gemm_attr<256, te::EPI_QKV, 128>()));
+  TE_ATTR((set_gemm_attr<256, te::EPI_QKV, 64>()));
+  TE_ATTR((set_gemm_attr<128, te::EPI_QKV, 128>()));
+  TE_ATTR((set_gemm_attr<128, te::EPI_QKV, 64>()));
+  TE_ATTR((set_gemm_attr<256, te::EPI_RESID, 128>()));
+  TE_ATTR((set_gemm_attr<128, te::EPI_RESID, 128>()));
+  TE_ATTR((set_gemm_attr<256, te::EPI_SWIGLU, 128>()));
+  TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
+  TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
+  TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
+  TE_ATTR(cudaFuncSetAttribute(te::te_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               te::AttnCfg<128>::SMEM_BYTES));
+  TE_ATTR(cudaFuncSetAttribute(te::te_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               te::AttnCfg<64>::SMEM_BYTES));
+#undef TE_ATTR
+  return cudaSuccess;
+}
+
+// Enqueue the whole stack on `st`.  Returns the number of kernels launched via *n_kernels.
+int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const float* embeds, const int32_t* lens, int T,
+                  float* out, cudaStream_t st, int* n_kernels) {
+  const te_config& c = h->cfg;
+  const int d = c.hidden, dh = c.head_dim, F = c.ffn;
+  const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
+  const int n_q = c.n_q_heads * dh;
+  const int lb = h->dbg_lb, le = h->dbg_le;
+  const int parts = d / h->bn_res;
+  int nk = 0;
+
+  te::te_scan_kernel<<<1, 32, 0, st>>>(lens, n_frames, grid_h * grid_w, T, c.max_tokens_per_frame, h->cu, h->flag);
+  TE_CUDA(h, cudaGetLastError());
+  ++nk;
+  {
+    te::PrepParams pp{};
+    pp.embeds = embeds; pp.out = out; pp.cu = h->cu; pp.pos = h->pos; pp.cos_t = h->cos_t; pp.sin_t = h->sin_t;
+    pp.inv_freq = h->inv_freq; pp.g_first = h->w + h->off[lb].g1; pp.xg = h->xg; pp.ssq = h->ssq;
+    pp.ssq_parts = parts; pp.ssq_stride = c.max_tokens; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
+    pp.half_dim = dh / 2; pp.grid_h = grid_h; pp.grid_w = grid_w; pp.sec_t = c.rope_sec_t; pp.sec_h = c.rope_sec_h;
+    te::te_prep_kernel<<<(T + 7) / 8, 256, 0, st>>>(pp);
+    TE_CUDA(h, cudaGetLastError());
+    ++nk;
+  }
+  CUtensorMap tmA_xg, tmA_attn, tmA_act;
+  if (!make_tmap(&tmA_xg, h->xg, T, d, te::GEMM_BM) || !make_tmap(&tmA_attn, h->attn, T, n_q, te::GEMM_BM) ||
+      !make_tmap(&tmA_act, h->act, T, F, te::GEMM_BM)) {
+    h->err = "cuTensorMapEncodeTiled failed for an activation map";
+    return TE_ERR_CUDA;
+  }
+  const int num_m = (T + te::GEMM_BM - 1) / te::GEMM_BM;
+  te::GemmParams base{};
+  base.M = T; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = parts; base.ssq_stride = c.max_tokens;
+  base.inv_d = 1.0f / static_cast<float>(d); base.eps = c.rms_eps;
+
+  // host-side upper bound of S_b for the attention grid (exact lengths stay on the device)
+  int s_bound = T - (n_frames - 1) * (grid_h * grid_w);
+  if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
+  const int q_blocks = (s_bound + te::ATT_BQ - 1) / te::ATT_BQ;
+
+  for (int l = lb; l < le; ++l) {
+    const LayerOff& o = h->off[l];
+    {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
+      te::GemmParams p = base;
+      p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / h->bn_qkv;
+      p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
+      p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
+      TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(h->bn_qkv, dh, tmA_xg, h->tm_qkv[l], p, h->sm_count, st));
+      ++nk;
+    }
+    {  // a2: causal GQA attention
+      te::AttnParams ap{};
+      ap.qkv = h->qkv; ap.out = h->attn; ap.cu_seqlens = h->cu; ap.ld = n_qkv; ap.n_q_heads = c.n_q_heads;
+      ap.n_kv_heads = c.n_kv_heads; ap.total_tokens = T;
+      ap.scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
+      TE_CUDA(h, dh == 128 ? launch_attn<128>(ap, q_blocks, n_frames, st) : launch_attn<64>(ap, q_blocks, n_frames, st));
+      ++nk;
+    }
+    {  // a3: O projection + residual add (+ next norm's gain / statistics)
+      te::GemmParams p = base;
+      p.N = d; p.K = n_q; p.num_n_blk = d / h->bn_res;
+      p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
+      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm_o[l], p, h->sm_count, st));
+      ++nk;
+    }
+    if (h->dbg_stop && l == le - 1) break;
+    {  // a4: RMSNorm -> gate/up GEMM -> SiLU(gate) * up
+      te::GemmParams p = base;
+      p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / h->bn_gu;
+      p.act = h->act; p.ld_act = F;
+      TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, dh, tmA_xg, h->tm_gu[l], p, h->sm_count, st));
+      ++nk;
+    }
+    {  // a5: down projection + residual add
+      te::GemmParams p = base;
+      p.N = d; p.K = F; p.num_n_blk = d / h->bn_res;
+      p.x = out; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
+      p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
+      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm_d[l], p, h->sm_count, st));
+      ++nk;
+    }
+  }
+  if (c.final_norm && le == c.n_layers && !h->dbg_stop) {  // a6
+    te::te_final_norm_kernel<<<(T + 7) / 8, 256, 0, st>>>(out, h->w + h->gf_off, T, d, c.rms_eps);
+    TE_CUDA(h, cudaGetLastError());
+    ++nk;
+  }
+  *n_kernels = nk;
+  return TE_OK;
+}
+
+void free_graphs(te_handle* h) {
+  for (auto& e : h->cache) {
+    cudaGraphExecDestroy(e.exec);
+    cudaGraphDestroy(e.graph);
+  }
+  h->cache.clear();
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t te_blob_bytes(const te_config* cfg) {
+  if (!cfg || validate_config(*cfg) != TE_OK) return 0;
+  return blob_elems(*cfg) * sizeof(bf16);
+}
+
+int te_create(const te_config* cfg, int device, te_handle** out) {
+  if (!cfg || !out) return TE_ERR_INVALID_ARG;
+  *out = nullptr;
+  int rc = validate_config(*cfg);
+  if (rc != TE_OK) return rc;
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) return TE_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TE_ERR_CUDA;
+  if (prop.major != 10) return TE_ERR_UNSUPPORTED;  // tcgen05 / TMEM: sm_100 family only; no fallback
+  if (!get_encode_fn()) return TE_ERR_CUDA;
+  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
+  if (init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
+
+  te_handle* h = new te_handle();
+  h->cfg = *cfg;
+  h->device = device;
+  h->sm_count = prop.multiProcessorCount;
+  h->dbg_lb = 0;
+  h->dbg_le = cfg->n_layers;
+  const te_config& c = h->cfg;
+  const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim;
+  h->bn_qkv = (n_qkv % 256 == 0) ? 256 : 128;
+  h->bn_gu = ((2 * c.ffn) % 256 == 0) ? 256 : 128;
+  h->bn_res = (c.hidden % 256 == 0) ? 256 : 128;
+  h->ssq_parts_cap = c.hidden / 128;
+
+  auto fail = [&](int code) {
+    te_destroy(h);
+    return code;
+  };
+  const size_t T = c.max_tokens, B = c.max_frames, hd2 = c.head_dim / 2;
+#define TE_ALLOC(ptr, bytes) \
+  if (cudaMalloc(reinterpret_cast<void**>(&(ptr)), (bytes)) != cudaSuccess) return fail(TE_ERR_CUDA)
+  TE_ALLOC(h->cu, (B + 1) * sizeof(int32_t));
+  TE_ALLOC(h->pos, 3 * T * sizeof(int32_t));
+  TE_ALLOC(h->flag, sizeof(int32_t));
+  TE_ALLOC(h->cos_t, T * hd2 * sizeof(float));
+  TE_ALLOC(h->sin_t, T * hd2 * sizeof(float));
+  TE_ALLOC(h->ssq, (size_t)h->ssq_parts_cap * T * sizeof(float));
+  TE_ALLOC(h->inv_freq, hd2 * sizeof(double));
+  TE_ALLOC(h->xg, T * c.hidden * sizeof(bf16));
+  TE_ALLOC(h->qkv, T * n_qkv * sizeof(bf16));
+  TE_ALLOC(h->attn, T * (size_t)c.n_q_heads * c.head_dim * sizeof(bf16));
+  TE_ALLOC(h->act, T * c.ffn * sizeof(bf16));
+#undef TE_ALLOC
+  if (cudaMemset(h->flag, 0, sizeof(int32_t)) != cudaSuccess) return fail(TE_ERR_CUDA);
+  std::vector<double> invf(hd2);
+  for (size_t i = 0; i < hd2; ++i) invf[i] = std::pow(c.rope_theta, -2.0 * (double)i / (double)c.head_dim);
+  if (cudaMemcpy(h->inv_freq, invf.data(), hd2 * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess)
+    return fail(TE_ERR_CUDA);
+  if (cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(TE_ERR_CUDA);
+  *out = h;
+  return TE_OK;
+}
+
+int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
+  if (!h || !blob) return TE_ERR_INVALID_ARG;
+  const te_config& c = h->cfg;
+  const size_t n_el = blob_elems(c);
+  if (n_bytes != n_el * sizeof(bf16)) return TE_ERR_BLOB_SIZE;
+  TE_CUDA(h, cudaSetDevice(h->device));
+  free_graphs(h);
+  h->loaded = false;
+  if (!h->w) TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->w), n_el * sizeof(bf16)));
+  h->w_elems = n_el;
+  // The device copy keeps the canonical layout (so Wq|Wk|Wv are already one fused [Nqkv, d] matrix);
+  // only [Wgate; Wup] is rewritten, interleaved per N-tile, via a per-layer staging buffer.
+  TE_CUDA(h, cudaMemcpy(h->w, blob, n_bytes, cudaMemcpyDefault));
+  const size_t d = c.hidden, dh = c.head_dim, F = c.ffn;
+  const size_t n_qkv = (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * dh, n_q = (size_t)c.n_q_heads * dh;
+  bf16* stage = nullptr;
+  TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&stage), 2 * F * d * sizeof(bf16)));
+  h->off.resize(c.n_layers);
+  h->tm_qkv.resize(c.n_layers); h->tm_o.resize(c.n_layers); h->tm_gu.resize(c.n_layers); h->tm_d.resize(c.n_layers);
+  size_t o = 0;
+  bool ok = true;
+  for (int l = 0; l < c.n_layers; ++l) {
+    LayerOff& L = h->off[l];
+    L.g1 = o; o += d;
+    L.wqkv = o; o += n_qkv * d;
+    L.gq = o; o += dh;
+    L.gk = o; o += dh;
+    L.wo = o; o += d * n_q;
+    L.g2 = o; o += d;
+    L.wgu = o; o += 2 * F * d;
+    L.wd = o; o += d * F;
+    cudaError_t e = cudaMemcpy(stage, h->w + L.wgu, 2 * F * d * sizeof(bf16), cudaMemcpyDeviceToDevice);
+    if (e == cudaSuccess) {
+      te::te_interleave_gate_up_kernel<<<(unsigned)(2 * F), 128>>>(
+          reinterpret_cast<const uint4*>(stage), reinterpret_cast<const uint4*>(stage + F * d),
+          reinterpret_cast<uint4*>(h->w + L.wgu), (int)F, (int)(d / 8), h->bn_gu);
+      e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+      h->err = std::string("gate/up interleave: ") + cudaGetErrorString(e);
+      cudaFree(stage);
+      return TE_ERR_CUDA;
+    }
+    ok = ok && make_tmap(&h->tm_qkv[l], h->w + L.wqkv, n_qkv, d, h->bn_qkv);
+    ok = ok && make_tmap(&h->tm_o[l], h->w + L.wo, d, n_q, h->bn_res);
+    ok = ok && make_tmap(&h->tm_gu[l], h->w + L.wgu, 2 * F, d, h->bn_gu);
+    ok = ok && make_tmap(&h->tm_d[l], h->w + L.wd, d, F, h->bn_res);
+  }
+  h->gf_off = o;
+  cudaError_t e = cudaDeviceSynchronize();
+  cudaFree(stage);
+  if (e != cudaSuccess) {
+    h->err = std::string("te_load_weights: ") + cudaGetErrorString(e);
+    return TE_ERR_CUDA;
+  }
+  if (!ok) {
+    h->err = "cuTensorMapEncodeTiled failed for a weight map";
+    return TE_ERR_CUDA;
+  }
+  h->loaded = true;
+  return TE_OK;
+}
+
+int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds,
+              const int32_t* text_lens, int32_t total_tokens, float* out, void* cuda_stream) {
+  if (!h) return TE_ERR_INVALID_ARG;
+  if (!h->loaded) return TE_ERR_NOT_LOADED;
+  const te_config& c = h->cfg;
+  if (!embeds || !text_lens || !out || embeds == out) return TE_ERR_INVALID_ARG;
+  if (n_frames < 1 || n_frames > c.max_frames || grid_h < 1 || grid_w < 1) return TE_ERR_INVALID_ARG;
+  if (total_tokens < 1 || total_tokens > c.max_tokens) return TE_ERR_INVALID_ARG;
+  if ((long long)grid_h * grid_w > c.max_tokens_per_frame) return TE_ERR_INVALID_ARG;
+  if ((long long)n_frames * grid_h * grid_w > total_tokens) return TE_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  h->last_T = total_tokens;
+  h->last_B = n_frames;
+
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (st != nullptr) TE_CUDA(h, cudaStreamIsCapturing(st, &cap));
+  int nk = 0;
+  if (!h->use_graph || cap != cudaStreamCaptureStatusNone) {
+    int rc = enqueue_stack(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, st, &nk);
+    if (rc == TE_OK) h->launches += nk;
+    return rc;
+  }
+  GraphKey key;
+  memset(&key, 0, sizeof(key));
+  key.n_frames = n_frames; key.grid_h = grid_h; key.grid_w = grid_w; key.total_tokens = total_tokens;
+  key.lb = h->dbg_lb; key.le = h->dbg_le; key.stop = h->dbg_stop;
+  key.embeds = embeds; key.lens = text_lens; key.out = out;
+  GraphEntry* hit = nullptr;
+  for (auto& e : h->cache)
+    if (e.key == key) { hit = &e; break; }
+  if (!hit) {
+    // First call for this (shape, pointers) key: capture the kernel sequence once.
+    TE_CUDA(h, cudaStreamBeginCapture(h->own_stream, cudaStreamCaptureModeThreadLocal));
+    int rc = enqueue_stack(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, h->own_stream, &nk);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(h->own_stream, &g);
+    if (rc != TE_OK) {
+      if (g) cudaGraphDestroy(g);
+      return rc;
+    }
+    if (e != cudaSuccess) {
+      h->err = std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e);
+      return TE_ERR_CUDA;
+    }
+    cudaGraphExec_t ex = nullptr;
+    e = cudaGraphInstantiate(&ex, g, 0);
+    if (e != cudaSuccess) {
+      cudaGraphDestroy(g);
+      h->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e);
+      return TE_ERR_CUDA;
+    }
+    if (h->cache.size() >= 16) {  // evict the least recently used entry
+      size_t victim = 0;
+      for (size_t i = 1; i < h->cache.size(); ++i)
+        if (h->cache[i].stamp < h->cache[victim].stamp) victim = i;
+      cudaGraphExecDestroy(h->cache[victim].exec);
+      cudaGraphDestroy(h->cache[victim].graph);
+      h->cache.erase(h->cache.begin() + victim);
+    }
+    h->cache.push_back(GraphEntry{key, ex, g, nk, 0});
+    hit = &h->cache.back();
+  }
+  hit->stamp = ++h->stamp;
+  TE_CUDA(h, cudaGraphLaunch(hit->exec, st));
+  h->launches += hit->n_kernels;
+  return TE_OK;
+}
+
+int te_encode_host(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds_host,
+                   const int32_t* text_lens_host, float* out_host) {
+  if (!h || !embeds_host || !text_lens_host || !out_host) return TE_ERR_INVALID_ARG;
+  if (!h->loaded) return TE_ERR_NOT_LOADED;
+  const te_config& c = h->cfg;
+  if (n_frames < 1 || n_frames > c.max_frames || grid_h < 1 || grid_w < 1) return TE_ERR_INVALID_ARG;
+  long long T = 0;
+  for (int b = 0; b < n_frames; ++b) {
+    if (text_lens_host[b] < 0) return TE_ERR_INVALID_ARG;
+    T += (long long)grid_h * grid_w + text_lens_host[b];
+  }
+  if (T < 1 || T > c.max_tokens) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaSetDevice(h->device));
+  if (!h->stg_embeds) {
+    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->stg_embeds), (size_t)c.max_tokens * c.hidden * sizeof(float)));
+    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->stg_out), (size_t)c.max_tokens * c.hidden * sizeof(float)));
+    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->stg_lens), (size_t)c.max_frames * sizeof(int32_t)));
+  }
+  const size_t bytes = (size_t)T * c.hidden * sizeof(float);
+  cudaStream_t st = h->own_stream;
+  TE_CUDA(h, cudaMemcpyAsync(h->stg_lens, text_lens_host, n_frames * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  TE_CUDA(h, cudaMemcpyAsync(h->stg_embeds, embeds_host, bytes, cudaMemcpyHostToDevice, st));
+  int rc = te_encode(h, n_frames, grid_h, grid_w, h->stg_embeds, h->stg_lens, (int32_t)T, h->stg_out, st);
+  if (rc != TE_OK) return rc;
+  TE_CUDA(h, cudaMemcpyAsync(out_host, h->stg_out, bytes, cudaMemcpyDeviceToHost, st));
+  TE_CUDA(h, cudaStreamSynchronize(st));
+  return TE_OK;
+}
+
+int te_query_async_error(te_handle* h) {
+  if (!h) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaSetDevice(h->device));
+  TE_CUDA(h, cudaDeviceSynchronize());
+  int32_t f = 0;
+  TE_CUDA(h, cudaMemcpy(&f, h->flag, sizeof(f), cudaMemcpyDeviceToHost));
+  if (f) {
+    TE_CUDA(h, cudaMemset(h->flag, 0, sizeof(int32_t)));
+    char buf[96];
+    snprintf(buf, sizeof(buf), "device validation flag 0x%x (1=negative length, 2=sum!=total_tokens, 4=frame too long)", f);
+    h->err = buf;
+    return TE_ERR_DEVICE_CHECK;
+  }
+  return TE_OK;
+}
+
+int te_set_option(te_handle* h, int option, int value) {
+  if (!h) return TE_ERR_INVALID_ARG;
+  if (option == TE_OPT_USE_GRAPH) {
+    h->use_graph = value ? 1 : 0;
+    return TE_OK;
+  }
+  return TE_ERR_INVALID_ARG;
+}
+
+int64_t te_kernel_launches(te_handle* h) { return h ? h->launches : 0; }
+
+int te_debug_set_range(te_handle* h, int32_t layer_begin, int32_t layer_end, int32_t stop_after_attn) {
+  if (!h) return TE_ERR_INVALID_ARG;
+  if (layer_begin < 0 || layer_end > h->cfg.n_layers || layer_begin >= layer_end) return TE_ERR_INVALID_ARG;
+  h->dbg_lb = layer_begin;
+  h->dbg_le = layer_end;
+  h->dbg_stop = stop_after_attn ? 1 : 0;
+  return TE_OK;
+}
+
+int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
+  if (!h || !dst) return TE_ERR_INVALID_ARG;
+  const te_config& c = h->cfg;
+  const size_t T = h->last_T, B = h->last_B;
+  const void* src = nullptr;
+  size_t need = 0;
+  switch (what) {
+    case TE_TAP_POS: src = h->pos; need = 3 * T * sizeof(int32_t); break;
+    case TE_TAP_CU_SEQLENS: src = h->cu; need = (B + 1) * sizeof(int32_t); break;
+    case TE_TAP_COS: src = h->cos_t; need = T * (c.head_dim / 2) * sizeof(float); break;
+    case TE_TAP_SIN: src = h->sin_t; need = T * (c.head_dim / 2) * sizeof(float); break;
+    case TE_TAP_QKV: src = h->qkv; need = T * (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim * sizeof(bf16); break;
+    case TE_TAP_ATTN: src = h->attn; need = T * (size_t)c.n_q_heads * c.head_dim * sizeof(bf16); break;
+    case TE_TAP_ACT: src = h->act; need = T * (size_t)c.ffn * sizeof(bf16); break;
+    default: return TE_ERR_INVALID_ARG;
+  }
+  if (T == 0 || n_bytes != need) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaSetDevice(h->device));
+  TE_CUDA(h, cudaDeviceSynchronize());
+  TE_CUDA(h, cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost));
+  return TE_OK;
+}
+
+int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                  int32_t block_n) {
+  if (!a || !b || !cmat || m < 1 || n < 1 || k < 1) return TE_ERR_INVALID_ARG;
+  if ((block_n != 128 && block_n != 256) || n % block_n != 0 || k % 64 != 0) return TE_ERR_UNSUPPORTED;
+  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TE_ERR_CUDA;
+  if (prop.major != 10) return TE_ERR_UNSUPPORTED;
+  if (init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
+  CUtensorMap ta, tb;
+  if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, block_n)) return TE_ERR_CUDA;
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
+  p.c = cmat; p.ld_c = n;
+  cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(block_n, 128, ta, tb, p, prop.multiProcessorCount, nullptr);
+  if (e != cudaSuccess) return TE_ERR_CUDA;
+  return cudaDeviceSynchronize() == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+}
+
+void te_destroy(te_handle* h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  cudaDeviceSynchronize();
+  free_graphs(h);
+  void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
+                  h->act, h->stg_embeds, h->stg_out, h->stg_lens};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  delete h;
+}
+
+const char* te_strerror(int code) {
+  switch (code) {
+    case TE_OK: return "ok";
+    case TE_ERR_INVALID_ARG: return "invalid argument";
+    case TE_ERR_NOT_LOADED: return "weights not loaded";
+    case TE_ERR_BLOB_SIZE: return "weight blob has the wrong size";
+    case TE_ERR_CUDA: return "CUDA error";
+    case TE_ERR_UNSUPPORTED: return "unsupported configuration or device";
+    case TE_ERR_DEVICE_CHECK: return "device-side validation failed";
+    default: return "unknown error";
+  }
+}
+
+const char* te_last_error(te_handle* h) { return h ? h->err.c_str() : ""; }
+
+}  // extern "C"

@@ -1,0 +1,79 @@
+"""Helpers for the `-m gpu` parity tests: run the CUDA path through the C-ABI binding and the
+fp64 oracle on the same seeded inputs (workloads/), and return both for comparison."""
+from __future__ import annotations
+
+import functools
+
+import numpy as np
+
+import workloads as W
+
+
+def bf16_bits_to_f64(bits):
+    u = np.ascontiguousarray(bits, dtype=np.uint16).astype(np.uint32) << np.uint32(16)
+    return u.view(np.float32).astype(np.float64)
+
+
+@functools.lru_cache(maxsize=4)
+def cached_blob(model, seed, gains="randn"):
+    return W.make_weight_blob(model, seed, gains=gains)
+
+
+class GpuTE:
+    """Owns one handle; encode() returns numpy arrays."""
+
+    def __init__(self, model, max_frames, max_tokens, blob, final_norm=None):
+        import torch
+        import paper_2606_05981_b200 as te
+        self.te, self.torch, self.model = te, torch, model
+        self.enc = te.TextEncoder(model, max_frames, max_tokens, final_norm=final_norm)
+        self.enc.load_weights(blob)
+
+    def encode(self, embeds, text_lens, gh, gw, layer_range=None, stop_after_attn=0, stream=None,
+               total_tokens=None, use_graph=1):
+        torch, te = self.torch, self.te
+        T = embeds.shape[0] if total_tokens is None else total_tokens
+        e = torch.from_numpy(np.ascontiguousarray(embeds, dtype=np.float32)).cuda()
+        tl = torch.from_numpy(np.asarray(text_lens, dtype=np.int32)).cuda()
+        out = torch.empty_like(e)
+        lb, le = (0, self.model.n_layers) if layer_range is None else layer_range
+        te.te_debug_set_range(self.enc.h, lb, le, stop_after_attn)
+        te.te_set_option(self.enc.h, te.TE_OPT_USE_GRAPH, use_graph)
+        self.enc.encode(len(text_lens), gh, gw, e, tl, T, out, stream)
+        torch.cuda.synchronize()
+        self._keep = (e, tl, out)
+        return out.cpu().numpy()
+
+    def tap(self, what, shape, dtype):
+        buf = np.empty(shape, dtype=dtype)
+        self.te.te_debug_tap(self.enc.h, what, buf)
+        return buf
+
+    def taps(self, T, B):
+        m, te = self.model, self.te
+        nqkv = (m.n_q_heads + 2 * m.n_kv_heads) * m.head_dim
+        nq = m.n_q_heads * m.head_dim
+        nk = m.n_kv_heads * m.head_dim
+        qkv = bf16_bits_to_f64(self.tap(te.TE_TAP_QKV, (T, nqkv), np.uint16))
+        return {
+            "pos": self.tap(te.TE_TAP_POS, (3, T), np.int32),
+            "cu_seqlens": self.tap(te.TE_TAP_CU_SEQLENS, (B + 1,), np.int32),
+            "cos": self.tap(te.TE_TAP_COS, (T, m.head_dim // 2), np.float32),
+            "sin": self.tap(te.TE_TAP_SIN, (T, m.head_dim // 2), np.float32),
+            "q": qkv[:, :nq], "k": qkv[:, nq:nq + nk], "v": qkv[:, nq + nk:],
+            "attn": bf16_bits_to_f64(self.tap(te.TE_TAP_ATTN, (T, nq), np.uint16)),
+            "act": bf16_bits_to_f64(self.tap(te.TE_TAP_ACT, (T, m.ffn), np.uint16)),
+        }
+
+    def close(self):
+        self.enc.close()
+
+
+def workload_inputs(cfg_id, outliers=None):
+    w = W.get_workload(cfg_id)
+    tl = W.make_text_lens(w)
+    T = W.total_tokens(w, tl)
+    emb = W.make_embeddings(w, T, outliers=outliers)
+    blob = cached_blob(w.model, w.seed_weights)
+    ch = W.gen.outlier_channels(w) if (outliers or w.outliers) != "none" else None
+    return w, blob, tl, T, emb, ch
