@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py — TE-prefill throughput on B200 (BASELINE.json:metric).
+
+A "step" is one te_encode call = one pass of the whole hot path
+over one batch of synthetic frames.  Default workload: cfg 4 = BASELINE.json configs[3]
+(28 layers, B=16 frames x (64 visual + 128 text) = 3072 tokens) — the configuration
+north_star's target is quoted on.  Prints ONE JSON line (rank 0).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config {2,3,4,5}] [--impl reference]
+
+N>1 (torchrun): frames are independent, so every rank runs its own replica on its own batch
+(weak scaling, no data-path collective); timing = max over ranks.
+`--impl reference`: times the fp64 CPU oracle (oracle/) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as W  # noqa: E402
+
+METRIC = "te_prefill_frames_per_s"
+UNIT = "frames/s"
+
+
+# ------------------------------------------------------------------ algorithmic work
+def gemm_flops_per_token_layer(m) -> float:
+    nqkv = (m.n_q_heads + 2 * m.n_kv_heads) * m.head_dim
+    params = nqkv * m.hidden + m.hidden * m.n_q_heads * m.head_dim + 3 * m.ffn * m.hidden
+    return 2.0 * params
+
+
+def attn_flops_per_layer(m, seq_lens) -> float:
+    # causal lower triangle only: QK^T + PV = 4 * dh * S(S+1)/2 per q head
+    return sum(4.0 * m.head_dim * m.n_q_heads * s * (s + 1) / 2.0 for s in seq_lens)
+
+
+def stack_work(m, seq_lens):
+    T = sum(seq_lens)
+    flops = m.n_layers * (gemm_flops_per_token_layer(m) * T + attn_flops_per_layer(m, seq_lens))
+    weight_bytes = 2.0 * W.blob_num_elements(m)
+    act_bytes = m.n_layers * T * 98304.0 * (m.hidden / 2048.0) + 16384.0 * T * (m.hidden / 2048.0)
+    return flops, weight_bytes, act_bytes
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "tf_burst": d["bf16_tflops"],
+                "tf_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "tf_burst": 1590.0, "tf_sustained": 1400.0, "src": "fallback"}
+
+
+# ------------------------------------------------------------------------- N>1 helpers (gloo-tested)
+def rank_seed_offset(rank: int) -> int:
+    """Each rank encodes its own batch of frames: embeddings seed = base + 1000 * rank."""
+    return 1000 * rank
+
+
+def max_over_ranks(seconds: float, device="cuda") -> float:
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return seconds
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank: float, world: int, seconds: float) -> float:
+    return units_per_rank * world / seconds
+
+
+# ------------------------------------------------------------------------------- clocks sampling
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------- oracle timing
+def time_oracle(w, blob, tl, emb, budget_s: float, n_frames_sample: int):
+    """Run the fp64 oracle, as it stands, on a bounded sample: `n_frames_sample` frames through as
+    many leading layers as fit the time budget; scaled to the full depth.  Returns a dict."""
+    from oracle import te_oracle as O
+    m = w.model
+    lay = W.blob_layout(m)
+    cu = O.cu_seqlens(tl, w.grid_h, w.grid_w)
+    frames = list(range(min(n_frames_sample, w.n_frames)))
+    sub_tl = [int(tl[b]) for b in frames]
+    sub_emb = np.concatenate([emb[cu[b]:cu[b + 1]] for b in frames])
+    t0 = time.perf_counter()
+    O.encode(blob, lay, m, sub_emb, sub_tl, w.grid_h, w.grid_w, layer_begin=0, layer_end=1)
+    t1 = time.perf_counter() - t0
+    n_layers = int(max(1, min(m.n_layers, budget_s // max(t1, 1e-3))))
+    t0 = time.perf_counter()
+    O.encode(blob, lay, m, sub_emb, sub_tl, w.grid_h, w.grid_w, layer_begin=0, layer_end=n_layers)
+    dt = time.perf_counter() - t0
+    full = dt * m.n_layers / n_layers
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    return {"seconds_sample": dt, "frames": len(frames), "layers_run": n_layers,
+            "frames_per_s": len(frames) / full, "tokens_per_s": float(sum(cu[b + 1] - cu[b] for b in frames)) / full,
+            "cores": int(cores),
+            "sample": f"{len(frames)} of {w.n_frames} frames x first {n_layers} of {m.n_layers} layers "
+                      f"({dt:.1f} s), scaled by {m.n_layers}/{n_layers} to full depth"}
+
+
+# ------------------------------------------------------------------------------------------ main
+def run_reference(args, w, blob, tl, T, emb, rank):
+    if rank != 0:
+        return
+    per_step = max(2.0, 150.0 / max(1, args.steps + args.warmup))
+    for _ in range(args.warmup):
+        time_oracle(w, blob, tl, emb, per_step / 2, 1)
+    vals, samples = [], None
+    t_all = 0.0
+    for _ in range(args.steps):
+        r = time_oracle(w, blob, tl, emb, per_step / 2, 1)
+        vals.append(r["frames_per_s"]); samples = r
+        t_all += r["seconds_sample"]
+    v = statistics.median(vals)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1000.0 * w.n_frames / v,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "n_frames": w.n_frames, "total_tokens": T, "n_layers": w.model.n_layers},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": samples["cores"], "kind": "oracle",
+                         "sample": samples["sample"] + " per step"},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel-timing-steps", type=int, default=3)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    w = W.get_workload(args.config)
+    m = w.model
+    tl = W.make_text_lens(w)
+    T = W.total_tokens(w, tl)
+    seq_lens = [w.grid_h * w.grid_w + int(t) for t in tl]
+
+    if args.impl == "reference":
+        if rank == 0:
+            blob = W.make_weight_blob(m, w.seed_weights)
+            emb = W.make_embeddings(w, T)
+            run_reference(args, w, blob, tl, T, emb, rank)
+        return
+
+    import torch
+    import paper_2606_05981_b200 as te
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    blob = W.make_weight_blob(m, w.seed_weights)
+    import dataclasses
+    w_rank = dataclasses.replace(w, seed_embeds=w.seed_embeds + rank_seed_offset(rank))
+    emb = W.make_embeddings(w_rank, T)
+
+    enc = te.TextEncoder(m, w.n_frames, T, device=local_rank)
+    enc.load_weights(blob)
+    e_dev = torch.from_numpy(emb).cuda()
+    lens_dev = torch.from_numpy(tl).cuda()
+    out_dev = torch.empty_like(e_dev)
+    stream = torch.cuda.Stream()
+    flush_l2 = 2.0 * W.blob_num_elements(m) < 256e6          # weights fit L2 (cfg 1/2): flush between steps
+    flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda") if flush_l2 else None
+
+    def step():
+        enc.encode(w.n_frames, w.grid_h, w.grid_w, e_dev, lens_dev, T, out_dev, stream.cuda_stream)
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            step()
+    torch.cuda.synchronize()
+    assert te.te_query_async_error(enc.h) == te.TE_OK
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    n0 = te.te_kernel_launches(enc.h)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_wall0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        for a, b in evs:
+            if flush_l2:
+                flush_buf.zero_()
+            a.record(stream)
+            step()
+            b.record(stream)
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    if dist is not None:
+        dist.barrier()
+    launches = te.te_kernel_launches(enc.h) - n0
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    t_dev = sum(step_ms) / 1000.0
+    t_dev = max_over_ranks(t_dev)
+    clocks = sampler.stop() if rank == 0 else None
+    ms_per_step = 1000.0 * t_dev / args.steps
+    value = aggregate_value(w.n_frames * args.steps, world, t_dev)
+    tokens_per_s = aggregate_value(T * args.steps, world, t_dev)
+
+    # ---- e2e: host buffers through te_encode_host (H2D + encode + D2H + sync inside the timed region)
+    eh = torch.from_numpy(emb).pin_memory()
+    oh = torch.empty_like(eh).pin_memory()
+    for _ in range(3):
+        enc.encode_host(w.n_frames, w.grid_h, w.grid_w, eh, tl, oh)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        enc.encode_host(w.n_frames, w.grid_h, w.grid_w, eh, tl, oh)
+    t_e2e = max_over_ranks(time.perf_counter() - t0)
+    e2e_value = aggregate_value(w.n_frames * args.steps, world, t_e2e)
+    h2d = int(emb.nbytes + tl.nbytes)
+    d2h = int(emb.nbytes)
+
+    # ---- per-kernel device times (CUDA events on the launching stream, direct launches)
+    te.te_set_option(enc.h, te.TE_OPT_KERNEL_TIMING, 1)
+    with torch.cuda.stream(stream):
+        step()
+    torch.cuda.synchronize()
+    te.te_kernel_times(enc.h)                                # discard the first (cold) pass
+    with torch.cuda.stream(stream):
+        for _ in range(args.kernel_timing_steps):
+            step()
+    torch.cuda.synchronize()
+    ktimes = te.te_kernel_times(enc.h)
+    te.te_set_option(enc.h, te.TE_OPT_KERNEL_TIMING, 0)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks = load_peaks()
+    flops, wbytes, abytes = stack_work(m, seq_lens)
+    t_compute = flops / (peaks["tf_sustained"] * 1e12)
+    t_hbm = (wbytes + abytes) / (peaks["hbm_gbs"] * 1e9)
+    t_roof = max(t_compute, t_hbm)
+    # dominant kernel: gate/up GEMM (50 % of the stack's FLOPs): 2 * T * d * 2F per launch
+    gu_ms, gu_n = ktimes["gateup"]
+    gu_flops = 2.0 * T * m.hidden * 2 * m.ffn
+    ksum = sum(v[0] for v in ktimes.values())
+    kernels = {k: {"ms_per_launch": (v[0] / v[1] if v[1] else None), "launches": v[1],
+                   "share": (v[0] / ksum if ksum else None)} for k, v in ktimes.items() if v[1]}
+    if t_compute >= t_hbm:
+        achieved = gu_flops / (gu_ms / gu_n / 1000.0) / 1e12
+        roofline = {"bound": "tensor", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
+                    "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sustained"],
+                    "peak_kind": f"bf16_tflops_sustained ({peaks['src']}); kernel timed inside a long step",
+                    "frac_of_burst": achieved / peaks["tf_burst"], "traffic": None}
+    else:
+        gu_bytes = 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
+        achieved = gu_bytes / (gu_ms / gu_n / 1000.0) / 1e9
+        roofline = {"bound": "hbm", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+                    "peak_kind": f"hbm_gbs ({peaks['src']})", "traffic": None}
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        r = time_oracle(w, blob, tl, emb, 25.0, 3)
+        cpu_baseline = {"value": r["frames_per_s"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                        "sample": r["sample"], "tokens_per_s": r["tokens_per_s"]}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": w.name, "n_frames_per_gpu": w.n_frames, "total_tokens_per_gpu": T,
+                   "n_layers": m.n_layers, "hidden": m.hidden,
+                   "l2": ("L2 flushed (256 MiB memset) before every timed step" if flush_l2 else
+                          "no flush: per-step working set (2.8 GB weights + activations) exceeds the 126 MB L2"),
+                   "parallelism": f"replica x{world} (frames sharded, no collective)"},
+        "tokens_per_s": tokens_per_s,
+        "ms_per_step_min": min(step_ms), "ms_per_step_median": statistics.median(step_ms),
+        "wall_ms_per_step": 1000.0 * t_wall / args.steps,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": 1000.0 * t_e2e / args.steps},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": roofline,
+        "stack_roofline": {"flops": flops, "weight_bytes": wbytes, "act_bytes": abytes,
+                           "t_compute_ms": 1000 * t_compute, "t_hbm_ms": 1000 * t_hbm,
+                           "bound": "tensor" if t_compute >= t_hbm else "hbm",
+                           "frac_of_sustained": t_roof / (t_dev / args.steps),
+                           "frac_of_burst": max(flops / (peaks["tf_burst"] * 1e12), t_hbm) / (t_dev / args.steps),
+                           "achieved_tflops": flops / (t_dev / args.steps) / 1e12, "peaks": peaks},
+        "kernels": kernels,
+        "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(line), flush=True)
+    enc.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -109,13 +109,24 @@ int te_query_async_error(te_handle* h);
 
 /* Options. */
 enum {
-  TE_OPT_USE_GRAPH = 0 /* 1 (default): te_encode = one cudaGraphLaunch; 0: direct launches */
+  TE_OPT_USE_GRAPH = 0,    /* 1 (default): te_encode = one cudaGraphLaunch; 0: direct launches   */
+  TE_OPT_KERNEL_TIMING = 1 /* 1: direct launches bracketed by CUDA events per kernel (implies no
+                              graph); read with te_kernel_times.  Measurement aid, default 0.     */
 };
 int te_set_option(te_handle* h, int option, int value);
 
 /* Number of kernels the library has launched so far on behalf of te_encode (graph replays
  * count the kernel nodes they contain).  For bench.py's `gpu_launches`. */
 int64_t te_kernel_launches(te_handle* h);
+
+/* Per-kernel-class device time accumulated by calls made under TE_OPT_KERNEL_TIMING, measured with
+ * CUDA events on the launching stream.  Synchronises; fills ms_sum[TE_KCLASS_COUNT] and
+ * n_launches[TE_KCLASS_COUNT] (HOST arrays) and resets the accumulation. */
+enum {
+  TE_KCLASS_SCAN = 0, TE_KCLASS_PREP = 1, TE_KCLASS_QKV = 2, TE_KCLASS_ATTN = 3, TE_KCLASS_OPROJ = 4,
+  TE_KCLASS_GATEUP = 5, TE_KCLASS_DOWN = 6, TE_KCLASS_FINAL_NORM = 7, TE_KCLASS_COUNT = 8
+};
+int te_kernel_times(te_handle* h, float* ms_sum, int32_t* n_launches);
 
 /* ---- test-only taps (SURVEY.md §8b "Debug taps") ------------------------------------------
  * te_debug_set_range restricts subsequent te_encode calls to layers [layer_begin, layer_end)

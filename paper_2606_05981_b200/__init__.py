@@ -20,11 +20,13 @@ TE_OK = 0
 TE_ERR_INVALID_ARG, TE_ERR_NOT_LOADED, TE_ERR_BLOB_SIZE = -1, -2, -3
 TE_ERR_CUDA, TE_ERR_UNSUPPORTED, TE_ERR_DEVICE_CHECK = -4, -5, -6
 TE_OPT_USE_GRAPH = 0
+TE_OPT_KERNEL_TIMING = 1
+TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT = range(7)
 
 EXPORTS = [
     "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_host",
-    "te_query_async_error", "te_set_option", "te_kernel_launches", "te_debug_set_range",
+    "te_query_async_error", "te_set_option", "te_kernel_launches", "te_kernel_times", "te_debug_set_range",
     "te_debug_tap", "te_debug_gemm", "te_destroy", "te_strerror", "te_last_error",
 ]
 
@@ -76,6 +78,8 @@ def lib() -> ctypes.CDLL:
     L.te_set_option.argtypes = [c_void_p, c_int, c_int]
     L.te_kernel_launches.restype = c_int64
     L.te_kernel_launches.argtypes = [c_void_p]
+    L.te_kernel_times.restype = c_int
+    L.te_kernel_times.argtypes = [c_void_p, c_void_p, c_void_p]
     L.te_debug_set_range.restype = c_int
     L.te_debug_set_range.argtypes = [c_void_p, c_int32, c_int32, c_int32]
     L.te_debug_tap.restype = c_int
@@ -164,6 +168,15 @@ def te_set_option(h, option: int, value: int):
 
 def te_kernel_launches(h) -> int:
     return int(lib().te_kernel_launches(h))
+
+
+def te_kernel_times(h) -> dict:
+    """{class name: (ms_sum, n_launches)} accumulated under TE_OPT_KERNEL_TIMING; resets."""
+    n = len(TE_KCLASS_NAMES)
+    ms = (c_float * n)()
+    cnt = (c_int32 * n)()
+    _check(lib().te_kernel_times(h, ms, cnt), h)
+    return {TE_KCLASS_NAMES[i]: (float(ms[i]), int(cnt[i])) for i in range(n)}
 
 
 def te_debug_set_range(h, layer_begin: int, layer_end: int, stop_after_attn: int = 0):

@@ -94,6 +94,9 @@ struct te_handle {
   std::vector<GraphEntry> cache;
   uint64_t stamp = 0;
   int use_graph = 1;
+  int timing = 0;
+  struct TimedLaunch { int kclass; cudaEvent_t a, b; };
+  std::vector<TimedLaunch> timed;
   int dbg_lb = 0, dbg_le = 0, dbg_stop = 0;
   int last_T = 0, last_B = 0;
   long long launches = 0;
@@ -203,9 +206,25 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int lb = h->dbg_lb, le = h->dbg_le;
   const int parts = d / h->bn_res;
   int nk = 0;
+  // Optional per-kernel CUDA-event bracketing (TE_OPT_KERNEL_TIMING; never inside a capture).
+  cudaEvent_t ev_a = nullptr;
+  auto tick = [&]() {
+    if (!h->timing) return;
+    cudaEventCreate(&ev_a);
+    cudaEventRecord(ev_a, st);
+  };
+  auto tock = [&](int kclass) {
+    if (!h->timing) return;
+    cudaEvent_t ev_b;
+    cudaEventCreate(&ev_b);
+    cudaEventRecord(ev_b, st);
+    h->timed.push_back({kclass, ev_a, ev_b});
+  };
 
+  tick();
   te::te_scan_kernel<<<1, 32, 0, st>>>(lens, n_frames, grid_h * grid_w, T, c.max_tokens_per_frame, h->cu, h->flag);
   TE_CUDA(h, cudaGetLastError());
+  tock(TE_KCLASS_SCAN);
   ++nk;
   {
     te::PrepParams pp{};
@@ -213,8 +232,10 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     pp.inv_freq = h->inv_freq; pp.g_first = h->w + h->off[lb].g1; pp.xg = h->xg; pp.ssq = h->ssq;
     pp.ssq_parts = parts; pp.ssq_stride = c.max_tokens; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
     pp.half_dim = dh / 2; pp.grid_h = grid_h; pp.grid_w = grid_w; pp.sec_t = c.rope_sec_t; pp.sec_h = c.rope_sec_h;
+    tick();
     te::te_prep_kernel<<<(T + 7) / 8, 256, 0, st>>>(pp);
     TE_CUDA(h, cudaGetLastError());
+    tock(TE_KCLASS_PREP);
     ++nk;
   }
   CUtensorMap tmA_xg, tmA_attn, tmA_act;
@@ -240,7 +261,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / h->bn_qkv;
       p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
       p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
+      tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(h->bn_qkv, dh, tmA_xg, h->tm_qkv[l], p, h->sm_count, st));
+      tock(TE_KCLASS_QKV);
       ++nk;
     }
     {  // a2: causal GQA attention
@@ -248,14 +271,18 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       ap.qkv = h->qkv; ap.out = h->attn; ap.cu_seqlens = h->cu; ap.ld = n_qkv; ap.n_q_heads = c.n_q_heads;
       ap.n_kv_heads = c.n_kv_heads; ap.total_tokens = T;
       ap.scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
+      tick();
       TE_CUDA(h, dh == 128 ? launch_attn<128>(ap, q_blocks, n_frames, st) : launch_attn<64>(ap, q_blocks, n_frames, st));
+      tock(TE_KCLASS_ATTN);
       ++nk;
     }
     {  // a3: O projection + residual add (+ next norm's gain / statistics)
       te::GemmParams p = base;
       p.N = d; p.K = n_q; p.num_n_blk = d / h->bn_res;
       p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
+      tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm_o[l], p, h->sm_count, st));
+      tock(TE_KCLASS_OPROJ);
       ++nk;
     }
     if (h->dbg_stop && l == le - 1) break;
@@ -263,7 +290,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       te::GemmParams p = base;
       p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / h->bn_gu;
       p.act = h->act; p.ld_act = F;
+      tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, dh, tmA_xg, h->tm_gu[l], p, h->sm_count, st));
+      tock(TE_KCLASS_GATEUP);
       ++nk;
     }
     {  // a5: down projection + residual add
@@ -271,13 +300,17 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.N = d; p.K = F; p.num_n_blk = d / h->bn_res;
       p.x = out; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
       p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
+      tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm_d[l], p, h->sm_count, st));
+      tock(TE_KCLASS_DOWN);
       ++nk;
     }
   }
   if (c.final_norm && le == c.n_layers && !h->dbg_stop) {  // a6
+    tick();
     te::te_final_norm_kernel<<<(T + 7) / 8, 256, 0, st>>>(out, h->w + h->gf_off, T, d, c.rms_eps);
     TE_CUDA(h, cudaGetLastError());
+    tock(TE_KCLASS_FINAL_NORM);
     ++nk;
   }
   *n_kernels = nk;
@@ -437,7 +470,8 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   if (st != nullptr) TE_CUDA(h, cudaStreamIsCapturing(st, &cap));
   int nk = 0;
-  if (!h->use_graph || cap != cudaStreamCaptureStatusNone) {
+  if (h->timing && cap != cudaStreamCaptureStatusNone) return TE_ERR_INVALID_ARG;
+  if (!h->use_graph || h->timing || cap != cudaStreamCaptureStatusNone) {
     int rc = enqueue_stack(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, st, &nk);
     if (rc == TE_OK) h->launches += nk;
     return rc;
@@ -539,10 +573,32 @@ int te_set_option(te_handle* h, int option, int value) {
     h->use_graph = value ? 1 : 0;
     return TE_OK;
   }
+  if (option == TE_OPT_KERNEL_TIMING) {
+    h->timing = value ? 1 : 0;
+    return TE_OK;
+  }
   return TE_ERR_INVALID_ARG;
 }
 
 int64_t te_kernel_launches(te_handle* h) { return h ? h->launches : 0; }
+
+int te_kernel_times(te_handle* h, float* ms_sum, int32_t* n_launches) {
+  if (!h || !ms_sum || !n_launches) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaSetDevice(h->device));
+  TE_CUDA(h, cudaDeviceSynchronize());
+  for (int i = 0; i < TE_KCLASS_COUNT; ++i) { ms_sum[i] = 0.f; n_launches[i] = 0; }
+  for (auto& t : h->timed) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, t.a, t.b) == cudaSuccess) {
+      ms_sum[t.kclass] += ms;
+      n_launches[t.kclass] += 1;
+    }
+    cudaEventDestroy(t.a);
+    cudaEventDestroy(t.b);
+  }
+  h->timed.clear();
+  return TE_OK;
+}
 
 int te_debug_set_range(te_handle* h, int32_t layer_begin, int32_t layer_end, int32_t stop_after_attn) {
   if (!h) return TE_ERR_INVALID_ARG;
@@ -600,6 +656,7 @@ void te_destroy(te_handle* h) {
   cudaSetDevice(h->device);
   cudaDeviceSynchronize();
   free_graphs(h);
+  for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
                   h->act, h->stg_embeds, h->stg_out, h->stg_lens};
   for (void* p : ptrs)

@@ -34,7 +34,7 @@ class GpuTE:
         torch, te = self.torch, self.te
         T = embeds.shape[0] if total_tokens is None else total_tokens
         e = torch.from_numpy(np.ascontiguousarray(embeds, dtype=np.float32)).cuda()
-        tl = torch.from_numpy(np.asarray(text_lens, dtype=np.int32)).cuda()
+        tl = torch.from_numpy(np.ascontiguousarray(text_lens, dtype=np.int32)).cuda()
         out = torch.empty_like(e)
         lb, le = (0, self.model.n_layers) if layer_range is None else layer_range
         te.te_debug_set_range(self.enc.h, lb, le, stop_after_attn)

@@ -1,0 +1,304 @@
+"""`-m gpu` parity tests: the CUDA path, called through the C-ABI binding, against the fp64 oracle
+on the same seeded inputs.  Gates: tests/parity_metrics.py (BASELINE.json:north_star + SURVEY §8c).
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+import parity_metrics as PM
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import te_oracle
+    return te_oracle
+
+
+@pytest.fixture(scope="module")
+def H():
+    import gpu_helpers
+    return gpu_helpers
+
+
+def _assert_final(m, tag=""):
+    assert m["rel_l2"] <= PM.GATE_FINAL_REL_L2, (tag, m)
+    assert m["update_rel_l2"] <= PM.GATE_UPDATE_REL_L2, (tag, m)
+    assert m["nonoutlier_rel_l2"] <= PM.GATE_NONOUTLIER_REL_L2, (tag, m)
+    assert m["outlier_maxabs_rel"] <= PM.GATE_OUTLIER_MAXABS, (tag, m)
+    assert m["cos_sim"] > 0.999, (tag, m)
+
+
+# --------------------------------------------------------------------------- GEMM main loop
+@pytest.mark.parametrize("M,N,K,bn", [(128, 256, 64, 256), (1, 128, 64, 128), (300, 512, 256, 256),
+                                       (300, 512, 256, 128), (517, 768, 832, 256), (3072, 2048, 2048, 256)])
+def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn):
+    """TMA + tcgen05 main loop alone: several tiles, ragged M tail, K spanning >1 pipeline ring."""
+    import torch
+    import paper_2606_05981_b200 as te
+    rng = np.random.default_rng(M * 7 + N)
+    a = W.f32_to_bf16_bits(rng.standard_normal((M, K)).astype(np.float32))
+    b = W.f32_to_bf16_bits(rng.standard_normal((N, K)).astype(np.float32))
+    ref = H.bf16_bits_to_f64(a).reshape(M, K) @ H.bf16_bits_to_f64(b).reshape(N, K).T
+    ad = torch.from_numpy(a.view(np.int16)).cuda()
+    bd = torch.from_numpy(b.view(np.int16)).cuda()
+    c = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
+    te.te_debug_gemm(0, ad, bd, c, M, N, K, bn)
+    out = c.cpu().numpy()
+    assert np.isfinite(out).all()
+    # fp32 accumulation of exact bf16 products: error ~ sqrt(K) * 2^-24 relative to |a||b|
+    assert PM.rel_l2(out, ref) < 1e-5
+    assert np.max(np.abs(out - ref)) < 1e-4 * np.sqrt(K) * 4
+
+
+# ------------------------------------------------------------------- ids / packing / rotary table
+@pytest.mark.parametrize("gh,gw,tl", [(4, 4, [24, 24]), (8, 8, [64]), (4, 16, [3, 0, 17]), (16, 4, [0, 9]),
+                                      (1, 5, [1, 2, 3, 4, 5, 6, 7])])
+def test_position_ids_bit_exact(H, O, gh, gw, tl):
+    m = W.TINY.with_layers(1)
+    blob = H.cached_blob(m, 1)
+    T = len(tl) * gh * gw + sum(tl)
+    g = H.GpuTE(m, len(tl), T, blob)
+    emb = np.random.default_rng(0).standard_normal((T, m.hidden)).astype(np.float32)
+    g.encode(emb, tl, gh, gw)
+    t = g.taps(T, len(tl))
+    assert np.array_equal(t["pos"], O.position_ids(tl, gh, gw))
+    assert np.array_equal(t["cu_seqlens"], O.cu_seqlens(tl, gh, gw))
+    phi = O.mrope_angles(O.position_ids(tl, gh, gw), m.head_dim, m.rope_sections, m.rope_theta)
+    assert np.max(np.abs(t["cos"] - np.cos(phi))) <= PM.GATE_COSSIN_ABS
+    assert np.max(np.abs(t["sin"] - np.sin(phi))) <= PM.GATE_COSSIN_ABS
+    import paper_2606_05981_b200 as te
+    assert te.te_query_async_error(g.enc.h) == 0
+    g.close()
+
+
+# ------------------------------------------------------------ per-layer taps + teacher-forced layers
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_layer_taps_and_teacher_forced_updates(H, O, cfg_id):
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    m = w.model
+    lay = W.blob_layout(m)
+    g = H.GpuTE(m, w.n_frames, T, blob)
+    x_in = emb.astype(np.float64)
+    for l in range(m.n_layers):
+        taps = {}
+        x32 = x_in.astype(np.float32)                      # teacher forcing: the oracle's residual, as fp32
+        ref = O.encode(blob, lay, m, x32, tl, w.grid_h, w.grid_w, layer_begin=l, layer_end=l + 1, taps=taps)
+        out = g.encode(x32, tl, w.grid_h, w.grid_w, layer_range=(l, l + 1))
+        gt = g.taps(T, w.n_frames)
+        for key in ("q", "k", "v", "attn", "act"):
+            assert PM.rel_l2(gt[key], taps[key][0]) <= PM.GATE_TAP_REL_L2, (cfg_id, l, key)
+        assert PM.rel_l2(out, ref) <= PM.GATE_LAYER_REL_L2
+        assert PM.rel_l2(out - x32, ref - x32) <= PM.GATE_LAYER_UPDATE_REL_L2, (cfg_id, l)
+        oa = g.encode(x32, tl, w.grid_h, w.grid_w, layer_range=(l, l + 1), stop_after_attn=1)
+        assert PM.rel_l2(oa - x32, taps["x_attn"][0] - x32) <= PM.GATE_LAYER_UPDATE_REL_L2
+        x_in = ref
+    g.close()
+
+
+# ------------------------------------------------------------------------------- whole stacks
+def test_cfg1_full_stack(H, O):
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4)
+    g = H.GpuTE(w.model, w.n_frames, T, blob)
+    out = g.encode(emb, tl, 4, 4)
+    _assert_final(PM.stack_metrics(out, ref, emb), "cfg1")
+    out_direct = g.encode(emb, tl, 4, 4, use_graph=0)
+    assert np.array_equal(out, out_direct)                 # graph replay == direct launches, bitwise
+    out_again = g.encode(emb, tl, 4, 4)
+    assert np.array_equal(out, out_again)                  # deterministic
+    g.close()
+
+
+def test_cfg1_final_norm(H, O):
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4, final_norm=1)
+    g = H.GpuTE(w.model, w.n_frames, T, blob, final_norm=1)
+    out = g.encode(emb, tl, 4, 4)
+    assert PM.rel_l2(out, ref) <= 3e-3
+    g.close()
+
+
+@pytest.mark.parametrize("gains", ["ones"])
+def test_cfg1_unit_gains(H, O, gains):
+    w = W.get_workload(1)
+    blob = W.make_weight_blob(w.model, 1, gains=gains)
+    tl = W.make_text_lens(w)
+    emb = W.make_embeddings(w, 80)
+    ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4)
+    g = H.GpuTE(w.model, 2, 80, blob)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, 4, 4), ref, emb), "unit gains")
+    g.close()
+
+
+def test_ragged_nonsquare_tiny_stack(H, O):
+    """Ragged frames incl. a zero-length text and a 200-token frame (4 attention q-blocks,
+    2 M tiles with a ragged tail), non-square grid."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    tl = [5, 0, 190, 33]
+    gh, gw = 2, 5
+    T = len(tl) * gh * gw + sum(tl)
+    emb = np.random.default_rng(3).standard_normal((T, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    g = H.GpuTE(m, len(tl), T, blob)
+    out = g.encode(emb, tl, gh, gw)
+    _assert_final(PM.stack_metrics(out, ref, emb), "ragged")
+    g.close()
+
+
+@pytest.mark.parametrize("cfg_id,frames", [(3, None), (4, [0, 7, 15]), (5, [1, 8, 31])])
+def test_full_28_layer_stacks_sampled_frames(H, O, cfg_id, frames):
+    """cfg 3 whole; cfg 4/5 at FULL size in the bench launch configuration, compared on sampled
+    frames the oracle computes one by one (frames are independent)."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    m = w.model
+    g = H.GpuTE(m, w.n_frames, T, blob)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    t = g.taps(T, w.n_frames)
+    assert np.array_equal(t["pos"], O.position_ids(tl, w.grid_h, w.grid_w))
+    assert np.array_equal(t["cu_seqlens"], O.cu_seqlens(tl, w.grid_h, w.grid_w))
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, w.grid_h, w.grid_w, frames=frames)
+    met = PM.stack_metrics(out, ref, emb, ch)
+    print(f"cfg{cfg_id} metrics: {met}  out std={out.std():.2f} min={out.min():.1f} max={out.max():.1f}")
+    _assert_final(met, f"cfg{cfg_id}")
+    assert np.isfinite(out).all()
+    g.close()
+
+
+def test_cfg3_paper_shaped_outliers(H, O):
+    """SURVEY Q16 variant: two near-constant channels at the paper's extremes (+1160 / -854)."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(3, outliers="paper")
+    m = w.model
+    g = H.GpuTE(m, w.n_frames, T, blob)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, w.grid_h, w.grid_w, frames=[0, 3])
+    _assert_final(PM.stack_metrics(out, ref, emb, ch), "cfg3 paper-shaped")
+    g.close()
+
+
+# ------------------------------------------------------------------------ invariants on the GPU
+def test_zero_projections_pass_residual_bitwise(H):
+    """W_o = W_down = 0 => out == embeds BITWISE, outlier channels included (fp32 residual)."""
+    w = W.get_workload(1)
+    m = w.model
+    lay = W.blob_layout(m)
+    blob = H.cached_blob(m, 1).copy()
+    for l in range(m.n_layers):
+        for name in ("Wo", "Wdown"):
+            off, shape = lay[(l, name)]
+            blob[off:off + int(np.prod(shape))] = 0
+    emb = W.make_embeddings(w, 80, outliers="x1000")
+    g = H.GpuTE(m, 2, 80, blob)
+    out = g.encode(emb, [24, 24], 4, 4)
+    assert np.array_equal(out, emb)
+    g.close()
+
+
+def test_frame_independence_permutation_causality_bitwise(H):
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    g = H.GpuTE(w.model, 4, 256, blob)
+    out = g.encode(emb, tl, 4, 4)
+    solo = g.encode(emb[40:], tl[1:], 4, 4)
+    assert np.array_equal(out[40:], solo)
+    perm = g.encode(np.concatenate([emb[40:], emb[:40]]), tl[::-1], 4, 4)
+    assert np.array_equal(perm[:40], out[40:]) and np.array_equal(perm[40:], out[:40])
+    emb2 = emb.copy()
+    emb2[30:40] += 1.0
+    out2 = g.encode(emb2, tl, 4, 4)
+    assert np.array_equal(out[:30], out2[:30]) and np.array_equal(out[40:], out2[40:])
+    assert not np.array_equal(out[30:40], out2[30:40])
+    g.close()
+
+
+def test_single_token_frames(H, O):
+    """Degenerate: 1x1 grid, no text -> S_b = 1 -> attention output == v."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    tl = [0, 0, 0]
+    emb = np.random.default_rng(5).standard_normal((3, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, 1, 1)
+    g = H.GpuTE(m, 3, 3, blob)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, 1, 1), ref, emb), "S=1")
+    g.close()
+
+
+def test_max_tokens_per_frame(H, O):
+    """Maximum frame length (256 tokens): 4 attention q-blocks, all kv blocks used."""
+    m = W.TINY.with_layers(1)
+    blob = H.cached_blob(m, 1)
+    tl = [256 - 16]
+    emb = np.random.default_rng(6).standard_normal((256, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, 4, 4)
+    g = H.GpuTE(m, 1, 256, blob)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, 4, 4), ref, emb), "S=256")
+    g.close()
+
+
+# --------------------------------------------------------------------- boundary / error behaviour
+def test_boundary_errors(H):
+    import torch
+    import paper_2606_05981_b200 as te
+    m = W.TINY
+    cfg = te.make_config(m, 2, 128)
+    h = te.te_create(cfg, 0)
+    e = torch.zeros((80, m.hidden), device="cuda")
+    o = torch.zeros_like(e)
+    tl = torch.tensor([24, 24], dtype=torch.int32, device="cuda")
+    L = te.lib()
+    assert L.te_encode(h, 2, 4, 4, e.data_ptr(), tl.data_ptr(), 80, o.data_ptr(), None) == te.TE_ERR_NOT_LOADED
+    blob = H.cached_blob(m, 1)
+    assert L.te_load_weights(h, blob.ctypes.data, blob.nbytes - 2) == te.TE_ERR_BLOB_SIZE
+    te.te_load_weights(h, blob)
+    assert te.te_blob_bytes(cfg) == blob.nbytes
+    assert L.te_encode(h, 3, 4, 4, e.data_ptr(), tl.data_ptr(), 80, o.data_ptr(), None) == te.TE_ERR_INVALID_ARG
+    assert L.te_encode(h, 2, 4, 4, e.data_ptr(), tl.data_ptr(), 500, o.data_ptr(), None) == te.TE_ERR_INVALID_ARG
+    assert L.te_encode(h, 2, 4, 4, e.data_ptr(), tl.data_ptr(), 80, e.data_ptr(), None) == te.TE_ERR_INVALID_ARG
+    assert L.te_encode(h, 2, 4, 4, None, tl.data_ptr(), 80, o.data_ptr(), None) == te.TE_ERR_INVALID_ARG
+    # device-side validation: total_tokens that disagrees with the lengths raises the sticky flag
+    te.te_encode(h, 2, 4, 4, e, tl, 79, o)
+    assert te.te_query_async_error(h) == te.TE_ERR_DEVICE_CHECK
+    assert te.te_query_async_error(h) == te.TE_OK
+    bad = torch.tensor([-1, 49], dtype=torch.int32, device="cuda")
+    te.te_encode(h, 2, 4, 4, e, bad, 80, o)
+    assert te.te_query_async_error(h) == te.TE_ERR_DEVICE_CHECK
+    te.te_encode(h, 2, 4, 4, e, tl, 80, o)
+    assert te.te_query_async_error(h) == te.TE_OK
+    bad_cfg = te.make_config(W.TEModelConfig(1, 256, 4, 2, 32, 768, (4, 6, 6)), 2, 128)
+    hh = te.c_void_p()
+    assert L.te_create(te.byref(bad_cfg), 0, te.byref(hh)) == te.TE_ERR_UNSUPPORTED
+    te.te_destroy(h)
+
+
+def test_encode_is_async_no_sync_and_counts_launches(H):
+    """te_encode must not synchronise: after the call returns, the stream still has work queued
+    behind a long-running blocker kernel placed before it."""
+    import torch
+    import paper_2606_05981_b200 as te
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    g = H.GpuTE(w.model, 2, 80, blob)
+    g.encode(emb, tl, 4, 4)                                # warm: graph captured
+    e, tld, out = g._keep
+    st = torch.cuda.Stream()
+    n0 = te.te_kernel_launches(g.enc.h)
+    with torch.cuda.stream(st):
+        torch.cuda._sleep(400_000_000)                     # ~0.2 s of device spin ahead of us
+        te.te_encode(g.enc.h, 2, 4, 4, e, tld, 80, out, st.cuda_stream)
+        done_at_return = st.query()
+    st.synchronize()
+    assert not done_at_return
+    assert te.te_kernel_launches(g.enc.h) - n0 == 2 + 5 * w.model.n_layers
+    g.close()
+
+
+def test_host_path_matches_device_path(H):
+    import torch
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    g = H.GpuTE(w.model, 2, 80, blob)
+    out = g.encode(emb, tl, 4, 4)
+    eh = torch.from_numpy(emb).pin_memory()
+    oh = torch.empty_like(eh).pin_memory()
+    g.enc.encode_host(2, 4, 4, eh, np.asarray(tl, dtype=np.int32), oh)
+    assert np.array_equal(oh.numpy(), out)
+    g.close()

@@ -66,23 +66,35 @@ def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
     return r.astype(np.uint16)
 
 
+def _fill_layer(blob: np.ndarray, m: TEModelConfig, seed: int, l: int, off: int, gains: str) -> None:
+    rng = np.random.Generator(np.random.Philox(key=[seed, l]))
+    for _, shape, kind in layer_tensors(m):
+        n = int(np.prod(shape))
+        z = rng.standard_normal(n, dtype=np.float32)
+        if kind == "matrix":
+            w = z * np.float32(0.02)
+        elif gains == "ones":
+            w = np.ones(n, dtype=np.float32)
+        else:
+            w = np.float32(1.0) + np.float32(0.1) * z
+        blob[off:off + n] = f32_to_bf16_bits(w)
+        off += n
+
+
 def make_weight_blob(m: TEModelConfig, seed: int = 1, gains: str = "randn") -> np.ndarray:
-    """uint16[blob_num_elements] of bf16 bits.  gains: "randn" (1+0.1N) or "ones"."""
+    """uint16[blob_num_elements] of bf16 bits.  gains: "randn" (1+0.1N) or "ones".
+    Layers are independent Philox streams, so they are filled by a small thread pool."""
     blob = np.empty(blob_num_elements(m), dtype=np.uint16)
-    off = 0
-    for l in range(m.n_layers):
-        rng = np.random.Generator(np.random.Philox(key=[seed, l]))
-        for _, shape, kind in layer_tensors(m):
-            n = int(np.prod(shape))
-            z = rng.standard_normal(n, dtype=np.float32)
-            if kind == "matrix":
-                w = z * np.float32(0.02)
-            elif gains == "ones":
-                w = np.ones(n, dtype=np.float32)
-            else:
-                w = np.float32(1.0) + np.float32(0.1) * z
-            blob[off:off + n] = f32_to_bf16_bits(w)
-            off += n
+    per_layer = sum(int(np.prod(s)) for _, s, _ in layer_tensors(m))
+    if m.n_layers >= 4:
+        from concurrent.futures import ThreadPoolExecutor
+        import os
+        with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+            list(ex.map(lambda l: _fill_layer(blob, m, seed, l, l * per_layer, gains), range(m.n_layers)))
+    else:
+        for l in range(m.n_layers):
+            _fill_layer(blob, m, seed, l, l * per_layer, gains)
+    off = per_layer * m.n_layers
     rng = np.random.Generator(np.random.Philox(key=[seed, _FINAL_KEY]))
     z = rng.standard_normal(m.hidden, dtype=np.float32)
     gf = np.ones(m.hidden, np.float32) if gains == "ones" else np.float32(1.0) + np.float32(0.1) * z
