@@ -110,8 +110,11 @@ int te_query_async_error(te_handle* h);
 /* Options. */
 enum {
   TE_OPT_USE_GRAPH = 0,    /* 1 (default): te_encode = one cudaGraphLaunch; 0: direct launches   */
-  TE_OPT_KERNEL_TIMING = 1 /* 1: direct launches bracketed by CUDA events per kernel (implies no
+  TE_OPT_KERNEL_TIMING = 1,/* 1: direct launches bracketed by CUDA events per kernel (implies no
                               graph); read with te_kernel_times.  Measurement aid, default 0.     */
+  TE_OPT_CTA_PAIR = 2,     /* GEMM tiling: 0 = one CTA per 128-row tile, 1 = CTA pairs (cta_group::2,
+                              256-row tiles), 2 = auto by token count (default)                    */
+  TE_OPT_RESID_BLOCK_N = 3 /* tile width (128 default, or 256) of the O-proj / down GEMMs          */
 };
 int te_set_option(te_handle* h, int option, int value);
 
@@ -149,9 +152,10 @@ int te_debug_tap(te_handle* h, int what, void* dst_host, size_t n_bytes);
 
 /* Test-only: C[M,N] (DEVICE fp32, row-major) = A[M,K] * B[N,K]^T with A, B DEVICE bf16
  * row-major, through the same TMA + tcgen05 main loop as the stack's GEMMs (plain epilogue).
- * K % 64 == 0, N % 128 == 0.  Synchronous. */
+ * K % 64 == 0, N % block_n == 0, block_n in {128, 256}; cta_pair selects the cta_group::2
+ * kernel (256-row tiles).  Synchronous. */
 int te_debug_gemm(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
-                  int32_t n, int32_t k, int32_t block_n);
+                  int32_t n, int32_t k, int32_t block_n, int32_t cta_pair);
 
 void te_destroy(te_handle* h);
 const char* te_strerror(int code);

@@ -21,6 +21,8 @@ TE_ERR_INVALID_ARG, TE_ERR_NOT_LOADED, TE_ERR_BLOB_SIZE = -1, -2, -3
 TE_ERR_CUDA, TE_ERR_UNSUPPORTED, TE_ERR_DEVICE_CHECK = -4, -5, -6
 TE_OPT_USE_GRAPH = 0
 TE_OPT_KERNEL_TIMING = 1
+TE_OPT_CTA_PAIR = 2
+TE_OPT_RESID_BLOCK_N = 3
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT = range(7)
 
@@ -85,7 +87,7 @@ def lib() -> ctypes.CDLL:
     L.te_debug_tap.restype = c_int
     L.te_debug_tap.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
     L.te_debug_gemm.restype = c_int
-    L.te_debug_gemm.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
+    L.te_debug_gemm.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
     L.te_destroy.restype = None
     L.te_destroy.argtypes = [c_void_p]
     L.te_strerror.restype = c_char_p
@@ -187,8 +189,8 @@ def te_debug_tap(h, what: int, dst_host):
     _check(lib().te_debug_tap(h, what, _ptr(dst_host), int(dst_host.nbytes)), h)
 
 
-def te_debug_gemm(device, a_bf16, b_bf16, c, m, n, k, block_n=256):
-    _check(lib().te_debug_gemm(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n))
+def te_debug_gemm(device, a_bf16, b_bf16, c, m, n, k, block_n=256, cta_pair=0):
+    _check(lib().te_debug_gemm(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, cta_pair))
 
 
 def te_destroy(h):

@@ -65,7 +65,11 @@ struct GemmCfg {
   static constexpr int B_BYTES = BN * GEMM_BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
   static constexpr int BAR_BYTES = 256;
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // +1024: manual alignment
+  // epilogue staging: per epilogue warp two 32-row x 32-float XOR-swizzled fp32 chunks, used to turn
+  // the one-thread-per-row TMEM layout into row-contiguous (coalesced) global accesses
+  static constexpr int STG_WARP_BYTES = 2 * 32 * 32 * 4;
+  static constexpr int STG_BYTES = 4 * STG_WARP_BYTES;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STG_BYTES + 1024;  // +1024: manual alignment
   static constexpr int TMEM_COLS = 2 * BN;
 };
 
@@ -94,47 +98,90 @@ __device__ __forceinline__ void epi_plain(const GemmParams& p, uint32_t t_row, i
   }
 }
 
+// Staging layout shared by the coalesced epilogues.  A warp owns 32 accumulator rows (thread = row
+// after tcgen05.ld 32x32b).  A 32-column fp32 chunk is written to shared memory by rows and read
+// back so that 8 consecutive lanes hold one 128-byte row segment (4 rows per warp instruction).
+// Element (row, col) lives at row*32 + (((col>>2) ^ (row&7))<<2) + (col&3): both the row-wise
+// 16-byte writes and the segment-wise 16-byte reads are bank-conflict free without padding.
+__device__ __forceinline__ void stg_put_row(float* buf, int lane, const float (&v)[32]) {
+#pragma unroll
+  for (int j = 0; j < 8; ++j)
+    *reinterpret_cast<float4*>(buf + lane * 32 + ((j ^ (lane & 7)) << 2)) =
+        make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+}
+__device__ __forceinline__ float4 stg_get(const float* buf, int rr, int cq) {
+  return *reinterpret_cast<const float4*>(buf + rr * 32 + ((cq ^ (rr & 7)) << 2));
+}
+
+// Residual epilogue: x += acc (fp32, in place), xg = bf16(x * g_next), per-row partial sum of squares.
 template <int BN>
-__device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, int row, bool valid, int n_blk) {
-  float ss = 0.f;
+__device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
+                                          float* stg) {
+  const int sub = lane >> 3;  // row within a group of 4
+  const int cq = lane & 7;    // 4-column group inside the 32-column chunk
   const bool has_g = p.g_next != nullptr;
+  float ss[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) ss[i] = 0.f;
 #pragma unroll 1
   for (int c0 = 0; c0 < BN; c0 += 32) {
-    uint32_t r[32];
-    tmem_ld32(t_row + c0, r);
-    tmem_ld_wait();
-    if (valid) {
-      const int col = n_blk * BN + c0;
-      float4* xp = reinterpret_cast<float4*>(p.x + (size_t)row * p.ld_x + col);
-      float xn[32];
+    {
+      uint32_t r[32];
+      tmem_ld32(t_row + c0, r);
+      tmem_ld_wait();
+      float v[32];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        float4 v = xp[j];
-        v.x += __uint_as_float(r[4 * j]);
-        v.y += __uint_as_float(r[4 * j + 1]);
-        v.z += __uint_as_float(r[4 * j + 2]);
-        v.w += __uint_as_float(r[4 * j + 3]);
-        xp[j] = v;
-        xn[4 * j] = v.x; xn[4 * j + 1] = v.y; xn[4 * j + 2] = v.z; xn[4 * j + 3] = v.w;
-        ss = fmaf(v.x, v.x, ss); ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
-      }
-      if (has_g) {
-        const uint4* gp = reinterpret_cast<const uint4*>(p.g_next + col);
-        uint4* op = reinterpret_cast<uint4*>(p.xg + (size_t)row * p.ld_x + col);
+      for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+      stg_put_row(stg, lane, v);
+    }
+    __syncwarp();
+    const int col = n_blk * BN + c0 + cq * 4;
+    float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f;
+    if (has_g) {
+      const uint2 g = __ldg(reinterpret_cast<const uint2*>(p.g_next + col));
+      g0 = bf16_lo(g.x); g1 = bf16_hi(g.x); g2 = bf16_lo(g.y); g3 = bf16_hi(g.y);
+    }
+    float4 xv[8];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint4 g = __ldg(gp + j);
-          uint4 o;
-          o.x = pack_bf16(xn[8 * j + 0] * bf16_lo(g.x), xn[8 * j + 1] * bf16_hi(g.x));
-          o.y = pack_bf16(xn[8 * j + 2] * bf16_lo(g.y), xn[8 * j + 3] * bf16_hi(g.y));
-          o.z = pack_bf16(xn[8 * j + 4] * bf16_lo(g.z), xn[8 * j + 5] * bf16_hi(g.z));
-          o.w = pack_bf16(xn[8 * j + 6] * bf16_lo(g.w), xn[8 * j + 7] * bf16_hi(g.w));
-          op[j] = o;
+    for (int i = 0; i < 8; ++i) {
+      const int row = row_base + sub + 4 * i;
+      if (row < p.M) xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int rr = sub + 4 * i;
+      const int row = row_base + rr;
+      if (row < p.M) {
+        const float4 a = stg_get(stg, rr, cq);
+        float4 v = xv[i];
+        v.x += a.x; v.y += a.y; v.z += a.z; v.w += a.w;
+        *reinterpret_cast<float4*>(p.x + (size_t)row * p.ld_x + col) = v;
+        ss[i] = fmaf(v.x, v.x, ss[i]); ss[i] = fmaf(v.y, v.y, ss[i]);
+        ss[i] = fmaf(v.z, v.z, ss[i]); ss[i] = fmaf(v.w, v.w, ss[i]);
+        if (has_g) {
+          uint2 o;
+          o.x = pack_bf16(v.x * g0, v.y * g1);
+          o.y = pack_bf16(v.z * g2, v.w * g3);
+          *reinterpret_cast<uint2*>(p.xg + (size_t)row * p.ld_x + col) = o;
         }
       }
     }
+    __syncwarp();
   }
-  if (valid && p.ssq_out != nullptr) p.ssq_out[(size_t)n_blk * p.ssq_stride + row] = ss;
+  // per-row sum of squares over this tile's columns: fixed-order reduction over the row's 8 lanes
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 1);
+    ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 2);
+    ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 4);
+  }
+  if (cq == 0 && p.ssq_out != nullptr) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int row = row_base + sub + 4 * i;
+      if (row < p.M) p.ssq_out[(size_t)n_blk * p.ssq_stride + row] = ss[i];
+    }
+  }
 }
 
 __device__ __forceinline__ float row_rstd(const GemmParams& p, int row, bool valid) {
@@ -144,37 +191,66 @@ __device__ __forceinline__ float row_rstd(const GemmParams& p, int row, bool val
   return 1.0f / sqrtf(s * p.inv_d + p.eps);
 }
 
-template <int BN>
-__device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, int row, bool valid, int n_blk) {
-  const float rstd = row_rstd(p, row, valid);
-  constexpr int HALF = BN / 2;  // tile columns [0,HALF) = gate, [HALF,BN) = up (weights interleaved per tile)
-#pragma unroll 1
-  for (int c0 = 0; c0 < HALF; c0 += 16) {
-    uint32_t g[16], u[16];
-    tmem_ld16(t_row + c0, g);
-    tmem_ld16(t_row + HALF + c0, u);
-    tmem_ld_wait();
-    if (valid) {
-      uint32_t o[8];
+// Store a staged 32x32 fp32 chunk as bf16: 8 lanes x 4 columns = 64 B per row, 4 rows per instruction.
+__device__ __forceinline__ void stg_store_bf16(const float* buf, int lane, int row_base, int M, __nv_bfloat16* dst,
+                                               int ld, int col0) {
+  const int sub = lane >> 3, cq = lane & 7;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        float g0 = __uint_as_float(g[2 * j]) * rstd, g1 = __uint_as_float(g[2 * j + 1]) * rstd;
-        float u0 = __uint_as_float(u[2 * j]) * rstd, u1 = __uint_as_float(u[2 * j + 1]) * rstd;
-        float a0 = g0 / (1.0f + __expf(-g0)) * u0;
-        float a1 = g1 / (1.0f + __expf(-g1)) * u1;
-        o[j] = pack_bf16(a0, a1);
-      }
-      uint4* dst = reinterpret_cast<uint4*>(p.act + (size_t)row * p.ld_act + n_blk * HALF + c0);
-      dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
-      dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
+  for (int i = 0; i < 8; ++i) {
+    const int rr = sub + 4 * i;
+    const int row = row_base + rr;
+    if (row < M) {
+      const float4 a = stg_get(buf, rr, cq);
+      uint2 o;
+      o.x = pack_bf16(a.x, a.y);
+      o.y = pack_bf16(a.z, a.w);
+      *reinterpret_cast<uint2*>(dst + (size_t)row * ld + col0 + cq * 4) = o;
     }
   }
 }
 
+// SwiGLU epilogue: tile columns [0,BN/2) = gate, [BN/2,BN) = up (weights interleaved per tile).
+// The arithmetic runs in the thread-per-row domain; only the bf16 store is transposed.
+template <int BN>
+__device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
+                                           float* stg) {
+  const int my_row = row_base + lane;
+  const float rstd = row_rstd(p, my_row, my_row < p.M);
+  constexpr int HALF = BN / 2;
+#pragma unroll 1
+  for (int c0 = 0; c0 < HALF; c0 += 32) {
+    float a[32];
+    {
+      uint32_t g[32], u[32];
+      tmem_ld32(t_row + c0, g);
+      tmem_ld32(t_row + HALF + c0, u);
+      tmem_ld_wait();
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const float gv = __uint_as_float(g[j]) * rstd;
+        const float uv = __uint_as_float(u[j]) * rstd;
+        a[j] = gv / (1.0f + __expf(-gv)) * uv;
+      }
+    }
+    stg_put_row(stg, lane, a);
+    __syncwarp();
+    stg_store_bf16(stg, lane, row_base, p.M, p.act, p.ld_act, n_blk * HALF + c0);
+    __syncwarp();
+  }
+}
+
+// QKV epilogue: y = rstd * acc; v heads are stored; q/k heads get the per-head RMSNorm (pass 1, in the
+// thread-per-row domain) and then gain + M-RoPE rotation of the pairs (i, i + DH/2) in the coalesced
+// domain, where the cos/sin rows are read as whole 128-byte segments.
 template <int BN, int DH>
-__device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int row, bool valid, int n_blk) {
-  const float rstd = row_rstd(p, row, valid);
+__device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
+                                        float* stg) {
+  const int my_row = row_base + lane;
+  const float rstd = row_rstd(p, my_row, my_row < p.M);
   constexpr int HD2 = DH / 2;
+  const int sub = lane >> 3, cq = lane & 7;
+  float* bufA = stg;
+  float* bufB = stg + 32 * 32;
 #pragma unroll 1
   for (int hh = 0; hh < BN / DH; ++hh) {
     const int col0 = n_blk * BN + hh * DH;  // first column of this head in the fused qkv row
@@ -183,25 +259,22 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
       // ---- v head: scale and store
 #pragma unroll 1
       for (int c0 = 0; c0 < DH; c0 += 32) {
-        uint32_t r[32];
-        tmem_ld32(t_head + c0, r);
-        tmem_ld_wait();
-        if (valid) {
-          uint4* dst = reinterpret_cast<uint4*>(p.qkv + (size_t)row * p.ld_qkv + col0 + c0);
+        float v[32];
+        {
+          uint32_t r[32];
+          tmem_ld32(t_head + c0, r);
+          tmem_ld_wait();
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            uint4 o;
-            o.x = pack_bf16(__uint_as_float(r[8 * j + 0]) * rstd, __uint_as_float(r[8 * j + 1]) * rstd);
-            o.y = pack_bf16(__uint_as_float(r[8 * j + 2]) * rstd, __uint_as_float(r[8 * j + 3]) * rstd);
-            o.z = pack_bf16(__uint_as_float(r[8 * j + 4]) * rstd, __uint_as_float(r[8 * j + 5]) * rstd);
-            o.w = pack_bf16(__uint_as_float(r[8 * j + 6]) * rstd, __uint_as_float(r[8 * j + 7]) * rstd);
-            dst[j] = o;
-          }
+          for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) * rstd;
         }
+        stg_put_row(bufA, lane, v);
+        __syncwarp();
+        stg_store_bf16(bufA, lane, row_base, p.M, p.qkv, p.ld_qkv, col0 + c0);
+        __syncwarp();
       }
       continue;
     }
-    // ---- q or k head: per-head RMSNorm (pass 1: sum of squares), then gain + rotation (pass 2)
+    // ---- q or k head.  Pass 1: sum of squares of the head (thread = row, TMEM reads only)
     const __nv_bfloat16* gain = (col0 < p.q_cols_end) ? p.gq : p.gk;
     float ss = 0.f;
 #pragma unroll 1
@@ -216,50 +289,57 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
       }
     }
     const float sc = rstd / sqrtf(ss * (1.0f / DH) + p.eps);
+    // ---- Pass 2: normalised halves a = u[c0..c0+32), b = u[HD2+c0..) -> staging -> rotate -> store
 #pragma unroll 1
-    for (int c0 = 0; c0 < HD2; c0 += 16) {
-      uint32_t a[16], b[16];
-      tmem_ld16(t_head + c0, a);
-      tmem_ld16(t_head + HD2 + c0, b);
-      tmem_ld_wait();
-      if (valid) {
-        const float4* cp = reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + c0);
-        const float4* sp = reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + c0);
-        const uint4* ga = reinterpret_cast<const uint4*>(gain + c0);
-        const uint4* gb = reinterpret_cast<const uint4*>(gain + HD2 + c0);
-        uint32_t o1[8], o2[8];
+    for (int c0 = 0; c0 < HD2; c0 += 32) {
+      {
+        float v[32];
+        uint32_t r[32];
+        tmem_ld32(t_head + c0, r);
+        tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {  // 8 columns per iteration
-          const uint4 g1 = __ldg(ga + j), g2 = __ldg(gb + j);
-          const float4 c_lo = __ldg(cp + 2 * j), c_hi = __ldg(cp + 2 * j + 1);
-          const float4 s_lo = __ldg(sp + 2 * j), s_hi = __ldg(sp + 2 * j + 1);
-          const float cs[8] = {c_lo.x, c_lo.y, c_lo.z, c_lo.w, c_hi.x, c_hi.y, c_hi.z, c_hi.w};
-          const float sn[8] = {s_lo.x, s_lo.y, s_lo.z, s_lo.w, s_hi.x, s_hi.y, s_hi.z, s_hi.w};
-          const float gA[8] = {bf16_lo(g1.x), bf16_hi(g1.x), bf16_lo(g1.y), bf16_hi(g1.y),
-                               bf16_lo(g1.z), bf16_hi(g1.z), bf16_lo(g1.w), bf16_hi(g1.w)};
-          const float gB[8] = {bf16_lo(g2.x), bf16_hi(g2.x), bf16_lo(g2.y), bf16_hi(g2.y),
-                               bf16_lo(g2.z), bf16_hi(g2.z), bf16_lo(g2.w), bf16_hi(g2.w)};
-          float r1[8], r2[8];
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) * sc;
+        stg_put_row(bufA, lane, v);
+        tmem_ld32(t_head + HD2 + c0, r);
+        tmem_ld_wait();
 #pragma unroll
-          for (int e = 0; e < 8; ++e) {
-            const float ua = __uint_as_float(a[8 * j + e]) * sc * gA[e];
-            const float ub = __uint_as_float(b[8 * j + e]) * sc * gB[e];
-            r1[e] = ua * cs[e] - ub * sn[e];
-            r2[e] = ub * cs[e] + ua * sn[e];
-          }
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) * sc;
+        stg_put_row(bufB, lane, v);
+      }
+      __syncwarp();
+      const int cc = c0 + cq * 4;  // this lane's 4 columns inside the half
+      const uint2 ga = __ldg(reinterpret_cast<const uint2*>(gain + cc));
+      const uint2 gb = __ldg(reinterpret_cast<const uint2*>(gain + HD2 + cc));
+      const float gA[4] = {bf16_lo(ga.x), bf16_hi(ga.x), bf16_lo(ga.y), bf16_hi(ga.y)};
+      const float gB[4] = {bf16_lo(gb.x), bf16_hi(gb.x), bf16_lo(gb.y), bf16_hi(gb.y)};
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int rr = sub + 4 * i;
+        const int row = row_base + rr;
+        if (row < p.M) {
+          const float4 cs = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc));
+          const float4 sn = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc));
+          const float4 a = stg_get(bufA, rr, cq);
+          const float4 b = stg_get(bufB, rr, cq);
+          const float ua[4] = {a.x * gA[0], a.y * gA[1], a.z * gA[2], a.w * gA[3]};
+          const float ub[4] = {b.x * gB[0], b.y * gB[1], b.z * gB[2], b.w * gB[3]};
+          const float c[4] = {cs.x, cs.y, cs.z, cs.w};
+          const float sv[4] = {sn.x, sn.y, sn.z, sn.w};
+          float r1[4], r2[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            o1[4 * j + e] = pack_bf16(r1[2 * e], r1[2 * e + 1]);
-            o2[4 * j + e] = pack_bf16(r2[2 * e], r2[2 * e + 1]);
+            r1[e] = ua[e] * c[e] - ub[e] * sv[e];
+            r2[e] = ub[e] * c[e] + ua[e] * sv[e];
           }
+          uint2 o1, o2;
+          o1.x = pack_bf16(r1[0], r1[1]); o1.y = pack_bf16(r1[2], r1[3]);
+          o2.x = pack_bf16(r2[0], r2[1]); o2.y = pack_bf16(r2[2], r2[3]);
+          __nv_bfloat16* dst = p.qkv + (size_t)row * p.ld_qkv + col0 + cc;
+          *reinterpret_cast<uint2*>(dst) = o1;
+          *reinterpret_cast<uint2*>(dst + HD2) = o2;
         }
-        uint4* d1 = reinterpret_cast<uint4*>(p.qkv + (size_t)row * p.ld_qkv + col0 + c0);
-        uint4* d2 = reinterpret_cast<uint4*>(p.qkv + (size_t)row * p.ld_qkv + col0 + HD2 + c0);
-        d1[0] = make_uint4(o1[0], o1[1], o1[2], o1[3]);
-        d1[1] = make_uint4(o1[4], o1[5], o1[6], o1[7]);
-        d2[0] = make_uint4(o2[0], o2[1], o2[2], o2[3]);
-        d2[1] = make_uint4(o2[4], o2[5], o2[6], o2[7]);
       }
+      __syncwarp();
     }
   }
 }
@@ -280,6 +360,7 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   uint64_t* tfull = bars + 2 * STAGES;
   uint64_t* tempty = tfull + 2;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+  float* stg_all = reinterpret_cast<float*>(smem + STAGES * Cfg::STAGE_BYTES + Cfg::BAR_BYTES);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -373,9 +454,11 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       tc_fence_after();
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
       if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row, valid, n_blk);
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row, valid, n_blk);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row, valid, n_blk);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row, valid, n_blk);
+      float* stg = stg_all + quad * (Cfg::STG_WARP_BYTES / 4);
+      const int row_base = m_blk * GEMM_BM + quad * 32;
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg);
       tc_fence_before();
       mbar_arrive(&tempty[acc]);
     }
@@ -384,6 +467,157 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------ CTA-pair (cta_group::2) kernel
+// Same pipeline, but a cluster of two CTAs (one SM pair) computes a 256 x BN tile: each CTA loads its
+// own 128 A rows and HALF of the B tile (BN/2 weight rows); the leader CTA issues
+// tcgen05.mma.cta_group::2 (M = 256), which reads both halves of B and writes rows 0-127 of D into
+// the leader's TMEM and rows 128-255 into the peer's.  Per SM this moves A 16 KB + B BN/2 x 128 B per
+// 64-deep k-block instead of A 16 KB + B BN x 128 B: 1.5x less L2->SM traffic at BN = 256.
+template <int BN>
+struct Gemm2Cfg {
+  static constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
+  static constexpr int B_BYTES = (BN / 2) * GEMM_BK * 2;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int STAGES = (BN == 256) ? 6 : 8;
+  static constexpr int BAR_BYTES = 256;
+  static constexpr int STG_WARP_BYTES = 2 * 32 * 32 * 4;
+  static constexpr int STG_BYTES = 4 * STG_WARP_BYTES;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STG_BYTES + 1024;
+  static constexpr int TMEM_COLS = 2 * BN;
+};
+
+template <int BN, int EPI, int DH>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
+te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const GemmParams p) {
+  using Cfg = Gemm2Cfg<BN>;
+  constexpr int STAGES = Cfg::STAGES;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* sA = smem;
+  uint8_t* sB = smem + STAGES * Cfg::A_BYTES;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * Cfg::STAGE_BYTES);
+  uint64_t* full = bars;                 // used in the leader CTA only
+  uint64_t* empty = bars + STAGES;       // one set per CTA (each producer waits on its own)
+  uint64_t* tfull = bars + 2 * STAGES;   // one set per CTA (each CTA's epilogue waits on its own)
+  uint64_t* tempty = tfull + 2;          // used in the leader CTA only (count 256: both CTAs' epilogues)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+  float* stg_all = reinterpret_cast<float*>(smem + STAGES * Cfg::STAGE_BYTES + Cfg::BAR_BYTES);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const bool leader = rank == 0;
+
+  if (warp == 0 && elect_one()) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB);
+  }
+  if (warp == 1) {
+    if (elect_one()) {
+      for (int i = 0; i < STAGES; ++i) {
+        mbar_init(&full[i], 1);
+        mbar_init(&empty[i], 1);
+      }
+      for (int i = 0; i < 2; ++i) {
+        mbar_init(&tfull[i], 1);
+        mbar_init(&tempty[i], 256);
+      }
+      fence_mbar_init();
+    }
+    __syncwarp();
+    tmem_alloc_cg2(tmem_slot, Cfg::TMEM_COLS);
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  const int num_kb = p.K / GEMM_BK;
+  const int num_mp = (p.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);
+  const int num_tiles = num_mp * p.num_n_blk;
+  const int pair = blockIdx.x >> 1;
+  const int num_pairs = gridDim.x >> 1;
+
+  if (warp == 0) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (elect_one()) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int tile = pair; tile < num_tiles; tile += num_pairs) {
+        const int mp = tile % num_mp;
+        const int n_blk = tile / num_mp;
+        const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
+        const int b_row = n_blk * BN + rank * (BN / 2);
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&empty[stage], phase ^ 1);
+          if (leader) mbar_arrive_expect_tx(&full[stage], 2 * Cfg::STAGE_BYTES);
+          const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
+          tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
+          tma_load_2d_cg2(sB + stage * Cfg::B_BYTES, &tmB, bar, kb * GEMM_BK, b_row);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (leader CTA only) =====================
+    if (leader && elect_one()) {
+      constexpr uint32_t idesc = umma_idesc_bf16(2 * GEMM_BM, BN);
+      int stage = 0;
+      uint32_t phase = 0;
+      int it = 0;
+      for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
+        const int acc = it & 1;
+        const uint32_t acc_phase = (it >> 1) & 1;
+        mbar_wait(&tempty[acc], acc_phase ^ 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * BN;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&full[stage], phase);
+          tc_fence_after();
+          const uint64_t a_desc = umma_smem_desc_sw128(smem_u32(sA + stage * Cfg::A_BYTES));
+          const uint64_t b_desc = umma_smem_desc_sw128(smem_u32(sB + stage * Cfg::B_BYTES));
+#pragma unroll
+          for (int k = 0; k < GEMM_BK / 16; ++k)
+            umma_bf16_cg2(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          umma_commit_cg2(&empty[stage], 0x3);  // frees this stage in BOTH CTAs
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        umma_commit_cg2(&tfull[acc], 0x3);      // accumulator ready in BOTH CTAs
+      }
+    }
+  } else {
+    // ===================== epilogue warps (both CTAs, own 128 rows) =====================
+    const int quad = warp & 3;
+    int it = 0;
+    for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
+      const int mp = tile % num_mp;
+      const int n_blk = tile / num_mp;
+      const int acc = it & 1;
+      const uint32_t acc_phase = (it >> 1) & 1;
+      mbar_wait(&tfull[acc], acc_phase);
+      tc_fence_after();
+      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
+      float* stg = stg_all + quad * (Cfg::STG_WARP_BYTES / 4);
+      const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
+      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg);
+      tc_fence_before();
+      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();  // the peer may still be signalling our barriers / reading our smem until here
+  if (warp == 1) {
+    __syncwarp();
+    tc_fence_after();
+    tmem_dealloc_cg2(tmem_base, Cfg::TMEM_COLS);
   }
 }
 

@@ -73,13 +73,16 @@ struct te_handle {
   int sm_count = 0;
   bool loaded = false;
   // tile choices
-  int bn_qkv = 256, bn_gu = 256, bn_res = 256;
+  int bn_qkv = 256, bn_gu = 256, bn_res = 128;
+  int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   // weights
   bf16* w = nullptr;
   size_t w_elems = 0;
   std::vector<LayerOff> off;
   size_t gf_off = 0;
-  std::vector<CUtensorMap> tm_qkv, tm_o, tm_gu, tm_d;
+  // weight tensor maps per layer, one per B box height {64, 128, 256} rows (index 0, 1, 2)
+  struct LayerMaps { CUtensorMap qkv[3], o[3], gu[3], d[3]; };
+  std::vector<LayerMaps> tm;
   // workspace
   int32_t *cu = nullptr, *pos = nullptr, *flag = nullptr;
   float *cos_t = nullptr, *sin_t = nullptr, *ssq = nullptr;
@@ -136,6 +139,8 @@ int validate_config(const te_config& c) {
   return TE_OK;
 }
 
+inline int box_index(int rows) { return rows == 64 ? 0 : (rows == 128 ? 1 : 2); }
+
 template <int BN, int EPI, int DH>
 cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, int sm_count,
                         cudaStream_t st) {
@@ -146,15 +151,36 @@ cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const te
   return cudaGetLastError();
 }
 
+template <int BN, int EPI, int DH>
+cudaError_t launch_gemm2(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, int sm_count,
+                         cudaStream_t st) {
+  using Cfg = te::Gemm2Cfg<BN>;
+  const int tiles = ((p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM)) * p.num_n_blk;
+  const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
+  te::te_gemm2_kernel<BN, EPI, DH><<<2 * pairs, te::GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, p);
+  return cudaGetLastError();
+}
+
+// pair = 0: one CTA per 128 x bn tile; pair = 1: one CTA pair per 256 x bn tile (cta_group::2)
 template <int EPI>
-cudaError_t launch_gemm_bn(int bn, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p, int sms,
-                           cudaStream_t st) {
+cudaError_t launch_gemm_bn(int bn, int pair, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p,
+                           int sms, cudaStream_t st) {
   if constexpr (EPI == te::EPI_QKV) {
+    if (pair) {
+      if (bn == 256 && dh == 128) return launch_gemm2<256, EPI, 128>(a, b, p, sms, st);
+      if (bn == 256 && dh == 64) return launch_gemm2<256, EPI, 64>(a, b, p, sms, st);
+      if (bn == 128 && dh == 128) return launch_gemm2<128, EPI, 128>(a, b, p, sms, st);
+      return launch_gemm2<128, EPI, 64>(a, b, p, sms, st);
+    }
     if (bn == 256 && dh == 128) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
     if (bn == 256 && dh == 64) return launch_gemm<256, EPI, 64>(a, b, p, sms, st);
     if (bn == 128 && dh == 128) return launch_gemm<128, EPI, 128>(a, b, p, sms, st);
     return launch_gemm<128, EPI, 64>(a, b, p, sms, st);
   } else {
+    if (pair) {
+      if (bn == 256) return launch_gemm2<256, EPI, 128>(a, b, p, sms, st);
+      return launch_gemm2<128, EPI, 128>(a, b, p, sms, st);
+    }
     if (bn == 256) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
     return launch_gemm<128, EPI, 128>(a, b, p, sms, st);
   }
@@ -170,8 +196,11 @@ cudaError_t launch_attn(const te::AttnParams& p, int q_blocks, int n_frames, cud
 
 template <int BN, int EPI, int DH>
 cudaError_t set_gemm_attr() {
-  return cudaFuncSetAttribute(te::te_gemm_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              te::GemmCfg<BN>::SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(te::te_gemm_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       te::GemmCfg<BN>::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(te::te_gemm2_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              te::Gemm2Cfg<BN>::SMEM_BYTES);
 }
 // Opt every kernel instantiation into its dynamic shared-memory size (once per process, outside
 // any stream capture).
@@ -205,6 +234,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int n_q = c.n_q_heads * dh;
   const int lb = h->dbg_lb, le = h->dbg_le;
   const int parts = d / h->bn_res;
+  // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
+  // one CTA per tile so that more SMs stream weights (HBM-bound regime).
+  const int pair = h->pair_mode == 2 ? (T >= 1024 ? 1 : 0) : h->pair_mode;
+  const int bx_qkv = box_index(pair ? h->bn_qkv / 2 : h->bn_qkv);
+  const int bx_gu = box_index(pair ? h->bn_gu / 2 : h->bn_gu);
+  const int bx_res = box_index(pair ? h->bn_res / 2 : h->bn_res);
   int nk = 0;
   // Optional per-kernel CUDA-event bracketing (TE_OPT_KERNEL_TIMING; never inside a capture).
   cudaEvent_t ev_a = nullptr;
@@ -262,7 +297,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
       p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(h->bn_qkv, dh, tmA_xg, h->tm_qkv[l], p, h->sm_count, st));
+      TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(h->bn_qkv, pair, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
       tock(TE_KCLASS_QKV);
       ++nk;
     }
@@ -281,7 +316,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.N = d; p.K = n_q; p.num_n_blk = d / h->bn_res;
       p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm_o[l], p, h->sm_count, st));
+      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_attn, h->tm[l].o[bx_res], p, h->sm_count, st));
       tock(TE_KCLASS_OPROJ);
       ++nk;
     }
@@ -291,7 +326,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / h->bn_gu;
       p.act = h->act; p.ld_act = F;
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, dh, tmA_xg, h->tm_gu[l], p, h->sm_count, st));
+      TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, pair, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
       tock(TE_KCLASS_GATEUP);
       ++nk;
     }
@@ -301,7 +336,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.x = out; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
       p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm_d[l], p, h->sm_count, st));
+      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_act, h->tm[l].d[bx_res], p, h->sm_count, st));
       tock(TE_KCLASS_DOWN);
       ++nk;
     }
@@ -358,7 +393,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim;
   h->bn_qkv = (n_qkv % 256 == 0) ? 256 : 128;
   h->bn_gu = ((2 * c.ffn) % 256 == 0) ? 256 : 128;
-  h->bn_res = (c.hidden % 256 == 0) ? 256 : 128;
+  h->bn_res = 128;  // O/down: N = hidden is small -> 128-wide tiles halve the wave-quantisation loss
   h->ssq_parts_cap = c.hidden / 128;
 
   auto fail = [&](int code) {
@@ -408,7 +443,7 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
   bf16* stage = nullptr;
   TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&stage), 2 * F * d * sizeof(bf16)));
   h->off.resize(c.n_layers);
-  h->tm_qkv.resize(c.n_layers); h->tm_o.resize(c.n_layers); h->tm_gu.resize(c.n_layers); h->tm_d.resize(c.n_layers);
+  h->tm.resize(c.n_layers);
   size_t o = 0;
   bool ok = true;
   for (int l = 0; l < c.n_layers; ++l) {
@@ -433,10 +468,13 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
       cudaFree(stage);
       return TE_ERR_CUDA;
     }
-    ok = ok && make_tmap(&h->tm_qkv[l], h->w + L.wqkv, n_qkv, d, h->bn_qkv);
-    ok = ok && make_tmap(&h->tm_o[l], h->w + L.wo, d, n_q, h->bn_res);
-    ok = ok && make_tmap(&h->tm_gu[l], h->w + L.wgu, 2 * F, d, h->bn_gu);
-    ok = ok && make_tmap(&h->tm_d[l], h->w + L.wd, d, F, h->bn_res);
+    for (int bi = 0; bi < 3; ++bi) {
+      const uint32_t box = 64u << bi;
+      ok = ok && make_tmap(&h->tm[l].qkv[bi], h->w + L.wqkv, n_qkv, d, box);
+      ok = ok && make_tmap(&h->tm[l].o[bi], h->w + L.wo, d, n_q, box);
+      ok = ok && make_tmap(&h->tm[l].gu[bi], h->w + L.wgu, 2 * F, d, box);
+      ok = ok && make_tmap(&h->tm[l].d[bi], h->w + L.wd, d, F, box);
+    }
   }
   h->gf_off = o;
   cudaError_t e = cudaDeviceSynchronize();
@@ -577,6 +615,18 @@ int te_set_option(te_handle* h, int option, int value) {
     h->timing = value ? 1 : 0;
     return TE_OK;
   }
+  if (option == TE_OPT_CTA_PAIR) {
+    if (value < 0 || value > 2) return TE_ERR_INVALID_ARG;
+    h->pair_mode = value;
+    free_graphs(h);
+    return TE_OK;
+  }
+  if (option == TE_OPT_RESID_BLOCK_N) {
+    if ((value != 128 && value != 256) || h->cfg.hidden % value != 0) return TE_ERR_INVALID_ARG;
+    h->bn_res = value;
+    free_graphs(h);
+    return TE_OK;
+  }
   return TE_ERR_INVALID_ARG;
 }
 
@@ -633,7 +683,7 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
 }
 
 int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
-                  int32_t block_n) {
+                  int32_t block_n, int32_t cta_pair) {
   if (!a || !b || !cmat || m < 1 || n < 1 || k < 1) return TE_ERR_INVALID_ARG;
   if ((block_n != 128 && block_n != 256) || n % block_n != 0 || k % 64 != 0) return TE_ERR_UNSUPPORTED;
   if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
@@ -642,11 +692,12 @@ int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t
   if (prop.major != 10) return TE_ERR_UNSUPPORTED;
   if (init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
   CUtensorMap ta, tb;
-  if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, block_n)) return TE_ERR_CUDA;
+  if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, cta_pair ? block_n / 2 : block_n))
+    return TE_ERR_CUDA;
   te::GemmParams p{};
   p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
   p.c = cmat; p.ld_c = n;
-  cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(block_n, 128, ta, tb, p, prop.multiProcessorCount, nullptr);
+  cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(block_n, cta_pair ? 1 : 0, 128, ta, tb, p, prop.multiProcessorCount, nullptr);
   if (e != cudaSuccess) return TE_ERR_CUDA;
   return cudaDeviceSynchronize() == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }

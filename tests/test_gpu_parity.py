@@ -31,9 +31,11 @@ def _assert_final(m, tag=""):
 
 
 # --------------------------------------------------------------------------- GEMM main loop
+@pytest.mark.parametrize("pair", [0, 1])
 @pytest.mark.parametrize("M,N,K,bn", [(128, 256, 64, 256), (1, 128, 64, 128), (300, 512, 256, 256),
-                                       (300, 512, 256, 128), (517, 768, 832, 256), (3072, 2048, 2048, 256)])
-def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn):
+                                       (300, 512, 256, 128), (517, 768, 832, 256), (3072, 2048, 2048, 256),
+                                       (3072, 2048, 6144, 128)])
+def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn, pair):
     """TMA + tcgen05 main loop alone: several tiles, ragged M tail, K spanning >1 pipeline ring."""
     import torch
     import paper_2606_05981_b200 as te
@@ -44,7 +46,7 @@ def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn):
     ad = torch.from_numpy(a.view(np.int16)).cuda()
     bd = torch.from_numpy(b.view(np.int16)).cuda()
     c = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
-    te.te_debug_gemm(0, ad, bd, c, M, N, K, bn)
+    te.te_debug_gemm(0, ad, bd, c, M, N, K, bn, pair)
     out = c.cpu().numpy()
     assert np.isfinite(out).all()
     # fp32 accumulation of exact bf16 products: error ~ sqrt(K) * 2^-24 relative to |a||b|
@@ -108,6 +110,30 @@ def test_cfg1_full_stack(H, O):
     assert np.array_equal(out, out_direct)                 # graph replay == direct launches, bitwise
     out_again = g.encode(emb, tl, 4, 4)
     assert np.array_equal(out, out_again)                  # deterministic
+    g.close()
+
+
+@pytest.mark.parametrize("cta_pair,resid_bn", [(1, 128), (1, 256), (0, 256), (0, 128)])
+def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn):
+    """Force each GEMM tiling (one CTA per tile / CTA pairs, 128- and 256-wide residual tiles)."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4)
+    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, 4, 4), ref, emb), f"pair={cta_pair} bn={resid_bn}")
+    g.close()
+
+
+def test_ragged_stack_cta_pairs(H, O):
+    """CTA-pair tiles on a ragged batch: 3 M tiles of 256 rows with a ragged tail (T = 593 - 10)."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    tl = [5, 0, 190, 33, 240, 65]
+    gh, gw = 2, 5
+    T = len(tl) * gh * gw + sum(tl)
+    emb = np.random.default_rng(4).standard_normal((T, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    g = H.GpuTE(m, len(tl), T, blob, cta_pair=1)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, gh, gw), ref, emb), "ragged pairs")
     g.close()
 
 
