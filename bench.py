@@ -202,6 +202,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-timing-steps", type=int, default=3)
+    ap.add_argument("--opt", default="", help="library options for experiments, e.g. pdl=0,cta_pair=1,resid_bn=256")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -239,6 +240,11 @@ def main():
 
     enc = te.TextEncoder(m, w.n_frames, T, device=local_rank)
     enc.load_weights(blob)
+    opt_ids = {"pdl": te.TE_OPT_PDL, "cta_pair": te.TE_OPT_CTA_PAIR, "resid_bn": te.TE_OPT_RESID_BLOCK_N,
+               "graph": te.TE_OPT_USE_GRAPH}
+    for kv in filter(None, args.opt.split(",")):
+        k, v = kv.split("=")
+        te.te_set_option(enc.h, opt_ids[k], int(v))
     e_dev = torch.from_numpy(emb).cuda()
     lens_dev = torch.from_numpy(tl).cuda()
     out_dev = torch.empty_like(e_dev)
@@ -356,7 +362,8 @@ def main():
                    "n_layers": m.n_layers, "hidden": m.hidden,
                    "l2": ("L2 flushed (256 MiB memset) before every timed step" if flush_l2 else
                           "no flush: per-step working set (2.8 GB weights + activations) exceeds the 126 MB L2"),
-                   "parallelism": f"replica x{world} (frames sharded, no collective)"},
+                   "parallelism": f"replica x{world} (frames sharded, no collective)",
+                   "opt": args.opt or "defaults"},
         "tokens_per_s": tokens_per_s,
         "ms_per_step_min": min(step_ms), "ms_per_step_median": statistics.median(step_ms),
         "wall_ms_per_step": 1000.0 * t_wall / args.steps,

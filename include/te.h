@@ -114,7 +114,8 @@ enum {
                               graph); read with te_kernel_times.  Measurement aid, default 0.     */
   TE_OPT_CTA_PAIR = 2,     /* GEMM tiling: 0 = one CTA per 128-row tile, 1 = CTA pairs (cta_group::2,
                               256-row tiles), 2 = auto by token count (default)                    */
-  TE_OPT_RESID_BLOCK_N = 3 /* tile width (128 default, or 256) of the O-proj / down GEMMs          */
+  TE_OPT_RESID_BLOCK_N = 3,/* tile width (128 default, or 256) of the O-proj / down GEMMs          */
+  TE_OPT_PDL = 4           /* 1 (default): kernels are chained with programmatic dependent launch   */
 };
 int te_set_option(te_handle* h, int option, int value);
 

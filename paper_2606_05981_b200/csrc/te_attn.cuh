@@ -77,6 +77,8 @@ __global__ void __launch_bounds__(ATT_THREADS, 3) te_attn_kernel(const AttnParam
   const int b = blockIdx.z;
   const int head = blockIdx.y;
   const int qb = blockIdx.x;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");  // qkv / cu_seqlens come from predecessor kernels
   const int seq0 = p.cu_seqlens[b];
   const int S = min(p.cu_seqlens[b + 1], p.total_tokens) - seq0;
   const int q0 = qb * ATT_BQ;

@@ -388,6 +388,7 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_launch_dependents();
 
   const int num_kb = p.K / GEMM_BK;
   const int num_tiles = p.num_m_blk * p.num_n_blk;
@@ -397,16 +398,33 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
+      // Weights do not depend on the predecessor kernel: start streaming the first ring of B tiles
+      // before the grid-dependency wait; the matching A tiles follow after it.
+      const int pre = (blockIdx.x < num_tiles) ? (num_kb < STAGES ? num_kb : STAGES) : 0;
+      {
+        const int n_blk0 = blockIdx.x / p.num_m_blk;
+        for (int kb = 0; kb < pre; ++kb) {
+          mbar_arrive_expect_tx(&full[kb], Cfg::STAGE_BYTES);
+          tma_load_2d(sB + kb * Cfg::B_BYTES, &tmB, &full[kb], kb * GEMM_BK, n_blk0 * BN);
+        }
+      }
+      pdl_wait();
+      bool first = true;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         const int m_blk = tile % p.num_m_blk;
         const int n_blk = tile / p.num_m_blk;
         for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1);
-          mbar_arrive_expect_tx(&full[stage], Cfg::STAGE_BYTES);
-          tma_load_2d(sA + stage * Cfg::A_BYTES, &tmA, &full[stage], kb * GEMM_BK, m_blk * GEMM_BM);
-          tma_load_2d(sB + stage * Cfg::B_BYTES, &tmB, &full[stage], kb * GEMM_BK, n_blk * BN);
+          if (first && kb < pre) {
+            tma_load_2d(sA + stage * Cfg::A_BYTES, &tmA, &full[stage], kb * GEMM_BK, m_blk * GEMM_BM);
+          } else {
+            mbar_wait(&empty[stage], phase ^ 1);
+            mbar_arrive_expect_tx(&full[stage], Cfg::STAGE_BYTES);
+            tma_load_2d(sA + stage * Cfg::A_BYTES, &tmA, &full[stage], kb * GEMM_BK, m_blk * GEMM_BM);
+            tma_load_2d(sB + stage * Cfg::B_BYTES, &tmB, &full[stage], kb * GEMM_BK, n_blk * BN);
+          }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
+        first = false;
       }
     }
   } else if (warp == 1) {
@@ -443,6 +461,7 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const int quad = warp & 3;
     const int row_in_tile = quad * 32 + lane;
     int it = 0;
+    pdl_wait();
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
       const int m_blk = tile % p.num_m_blk;
       const int n_blk = tile / p.num_m_blk;
@@ -535,6 +554,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   cluster_sync_all();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_launch_dependents();
 
   const int num_kb = p.K / GEMM_BK;
   const int num_mp = (p.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);
@@ -547,19 +567,35 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
+      // weights first (independent of the predecessor kernel), then the dependency wait, then A
+      const int pre = (pair < num_tiles) ? (num_kb < STAGES ? num_kb : STAGES) : 0;
+      {
+        const int b_row0 = (pair / num_mp) * BN + rank * (BN / 2);
+        for (int kb = 0; kb < pre; ++kb) {
+          if (leader) mbar_arrive_expect_tx(&full[kb], 2 * Cfg::STAGE_BYTES);
+          tma_load_2d_cg2(sB + kb * Cfg::B_BYTES, &tmB, mapa_u32(smem_u32(&full[kb]), 0), kb * GEMM_BK, b_row0);
+        }
+      }
+      pdl_wait();
+      bool first = true;
       for (int tile = pair; tile < num_tiles; tile += num_pairs) {
         const int mp = tile % num_mp;
         const int n_blk = tile / num_mp;
         const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
         const int b_row = n_blk * BN + rank * (BN / 2);
         for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1);
-          if (leader) mbar_arrive_expect_tx(&full[stage], 2 * Cfg::STAGE_BYTES);
           const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
-          tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
-          tma_load_2d_cg2(sB + stage * Cfg::B_BYTES, &tmB, bar, kb * GEMM_BK, b_row);
+          if (first && kb < pre) {
+            tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
+          } else {
+            mbar_wait(&empty[stage], phase ^ 1);
+            if (leader) mbar_arrive_expect_tx(&full[stage], 2 * Cfg::STAGE_BYTES);
+            tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
+            tma_load_2d_cg2(sB + stage * Cfg::B_BYTES, &tmB, bar, kb * GEMM_BK, b_row);
+          }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
+        first = false;
       }
     }
   } else if (warp == 1) {
@@ -593,6 +629,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     // ===================== epilogue warps (both CTAs, own 128 rows) =====================
     const int quad = warp & 3;
     int it = 0;
+    pdl_wait();
     for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
       const int mp = tile % num_mp;
       const int n_blk = tile / num_mp;

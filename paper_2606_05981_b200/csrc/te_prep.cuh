@@ -16,6 +16,8 @@ enum { FLAG_BAD_LEN = 1, FLAG_BAD_TOTAL = 2, FLAG_TOO_LONG = 4 };
 // that later kernels never touch rows beyond the caller's buffers even when validation fails.
 __global__ void te_scan_kernel(const int32_t* __restrict__ text_lens, int n_frames, int n_vis, int total_tokens,
                                int max_tokens_per_frame, int32_t* __restrict__ cu, int32_t* __restrict__ flag) {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous call's kernels still read cu / flag
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   long long acc = 0;
   int f = 0;
@@ -52,6 +54,8 @@ struct PrepParams {
 __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tok = blockIdx.x * 8 + warp;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   if (tok >= p.total_tokens) return;
   // frame of this token: largest b with cu[b] <= tok
   int lo = 0, hi = p.n_frames - 1;
@@ -108,6 +112,8 @@ __global__ void __launch_bounds__(256) te_final_norm_kernel(float* __restrict__ 
                                                             int total_tokens, int d, float eps) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tok = blockIdx.x * 8 + warp;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   if (tok >= total_tokens) return;
   float4* row = reinterpret_cast<float4*>(x + (size_t)tok * d);
   float ss = 0.f;

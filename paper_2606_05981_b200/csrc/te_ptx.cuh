@@ -23,6 +23,14 @@ __device__ __forceinline__ bool elect_one() {
   return pred != 0;
 }
 
+// ---------------------------------------------------------- programmatic dependent launch (PDL)
+// Every kernel of the stack is launched with programmatic stream serialisation: it may start while
+// its predecessor drains.  pdl_launch_dependents() lets the successor be scheduled as soon as SM
+// resources free up; pdl_wait() blocks until ALL predecessor grids have completed and their
+// memory is visible.  Nothing written by / read by a predecessor may be touched before pdl_wait().
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ------------------------------------------------------------------------------ mbarrier
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");

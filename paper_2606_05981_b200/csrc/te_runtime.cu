@@ -97,6 +97,7 @@ struct te_handle {
   std::vector<GraphEntry> cache;
   uint64_t stamp = 0;
   int use_graph = 1;
+  int pdl = 1;
   int timing = 0;
   struct TimedLaunch { int kclass; cudaEvent_t a, b; };
   std::vector<TimedLaunch> timed;
@@ -139,6 +140,24 @@ int validate_config(const te_config& c) {
   return TE_OK;
 }
 
+// Launch with (optional) programmatic stream serialisation: the kernel may begin while its
+// predecessor in the stream drains; the kernels order themselves with griddepcontrol.wait.
+bool g_pdl = true;
+template <typename... KArgs, typename... Args>
+cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = g_pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 inline int box_index(int rows) { return rows == 64 ? 0 : (rows == 128 ? 1 : 2); }
 
 template <int BN, int EPI, int DH>
@@ -147,8 +166,7 @@ cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const te
   using Cfg = te::GemmCfg<BN>;
   const int tiles = p.num_m_blk * p.num_n_blk;
   const int grid = tiles < sm_count ? tiles : sm_count;
-  te::te_gemm_kernel<BN, EPI, DH><<<grid, te::GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, p);
-  return cudaGetLastError();
+  return launch_k(te::te_gemm_kernel<BN, EPI, DH>, dim3(grid), dim3(te::GEMM_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB, p);
 }
 
 template <int BN, int EPI, int DH>
@@ -157,8 +175,8 @@ cudaError_t launch_gemm2(const CUtensorMap& tmA, const CUtensorMap& tmB, const t
   using Cfg = te::Gemm2Cfg<BN>;
   const int tiles = ((p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM)) * p.num_n_blk;
   const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
-  te::te_gemm2_kernel<BN, EPI, DH><<<2 * pairs, te::GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, p);
-  return cudaGetLastError();
+  return launch_k(te::te_gemm2_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB,
+                  p);
 }
 
 // pair = 0: one CTA per 128 x bn tile; pair = 1: one CTA pair per 256 x bn tile (cta_group::2)
@@ -190,8 +208,7 @@ template <int DH>
 cudaError_t launch_attn(const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
   using Cfg = te::AttnCfg<DH>;
   dim3 grid(q_blocks, p.n_q_heads, n_frames);
-  te::te_attn_kernel<DH><<<grid, te::ATT_THREADS, Cfg::SMEM_BYTES, st>>>(p);
-  return cudaGetLastError();
+  return launch_k(te::te_attn_kernel<DH>, grid, dim3(te::ATT_THREADS), Cfg::SMEM_BYTES, st, p);
 }
 
 template <int BN, int EPI, int DH>
@@ -257,8 +274,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   };
 
   tick();
-  te::te_scan_kernel<<<1, 32, 0, st>>>(lens, n_frames, grid_h * grid_w, T, c.max_tokens_per_frame, h->cu, h->flag);
-  TE_CUDA(h, cudaGetLastError());
+  g_pdl = h->pdl && !h->timing;
+  TE_CUDA(h, launch_k(te::te_scan_kernel, dim3(1), dim3(32), 0, st, lens, n_frames, grid_h * grid_w, T,
+                      c.max_tokens_per_frame, h->cu, h->flag));
   tock(TE_KCLASS_SCAN);
   ++nk;
   {
@@ -268,8 +286,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     pp.ssq_parts = parts; pp.ssq_stride = c.max_tokens; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
     pp.half_dim = dh / 2; pp.grid_h = grid_h; pp.grid_w = grid_w; pp.sec_t = c.rope_sec_t; pp.sec_h = c.rope_sec_h;
     tick();
-    te::te_prep_kernel<<<(T + 7) / 8, 256, 0, st>>>(pp);
-    TE_CUDA(h, cudaGetLastError());
+    TE_CUDA(h, launch_k(te::te_prep_kernel, dim3((T + 7) / 8), dim3(256), 0, st, pp));
     tock(TE_KCLASS_PREP);
     ++nk;
   }
@@ -343,8 +360,8 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   }
   if (c.final_norm && le == c.n_layers && !h->dbg_stop) {  // a6
     tick();
-    te::te_final_norm_kernel<<<(T + 7) / 8, 256, 0, st>>>(out, h->w + h->gf_off, T, d, c.rms_eps);
-    TE_CUDA(h, cudaGetLastError());
+    TE_CUDA(h, launch_k(te::te_final_norm_kernel, dim3((T + 7) / 8), dim3(256), 0, st, out,
+                        static_cast<const bf16*>(h->w + h->gf_off), T, d, c.rms_eps));
     tock(TE_KCLASS_FINAL_NORM);
     ++nk;
   }
@@ -615,6 +632,11 @@ int te_set_option(te_handle* h, int option, int value) {
     h->timing = value ? 1 : 0;
     return TE_OK;
   }
+  if (option == TE_OPT_PDL) {
+    h->pdl = value ? 1 : 0;
+    free_graphs(h);
+    return TE_OK;
+  }
   if (option == TE_OPT_CTA_PAIR) {
     if (value < 0 || value > 2) return TE_ERR_INVALID_ARG;
     h->pair_mode = value;
@@ -697,6 +719,7 @@ int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t
   te::GemmParams p{};
   p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
   p.c = cmat; p.ld_c = n;
+  g_pdl = false;
   cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(block_n, cta_pair ? 1 : 0, 128, ta, tb, p, prop.multiProcessorCount, nullptr);
   if (e != cudaSuccess) return TE_ERR_CUDA;
   return cudaDeviceSynchronize() == cudaSuccess ? TE_OK : TE_ERR_CUDA;
