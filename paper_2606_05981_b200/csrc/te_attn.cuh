@@ -15,7 +15,6 @@ namespace te {
 
 constexpr int ATT_BQ = 64;
 constexpr int ATT_BKV = 64;
-constexpr int ATT_THREADS = 128;
 
 struct AttnParams {
   const __nv_bfloat16* qkv;  // [T, ld] : q heads | k heads | v heads
@@ -27,10 +26,14 @@ struct AttnParams {
   float scale_log2;  // log2(e) / sqrt(dh)
 };
 
-template <int DH>
+// GH = q heads served by one CTA (they share one kv head: GH divides Hq/Hkv); 4 warps per head.
+template <int DH, int GH>
 struct AttnCfg {
   static constexpr int ROW = DH + 8;  // padded row (elements): 16 B pad -> conflict-free ldmatrix
-  static constexpr int SMEM_BYTES = (ATT_BQ + 2 * ATT_BKV) * ROW * 2;
+  static constexpr int THREADS = 128 * GH;
+  static constexpr int Q_ELEMS = GH * ATT_BQ * ROW;
+  static constexpr int KV_STAGE_ELEMS = 2 * ATT_BKV * ROW;  // K block + V block
+  static constexpr int SMEM_BYTES = (Q_ELEMS + 2 * KV_STAGE_ELEMS) * 2;
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, bool pred) {
@@ -38,8 +41,10 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, boo
   const int sz = pred ? 16 : 0;  // src-size 0 -> zero fill
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() {
-  asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 __device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], const void* p) {
   const uint32_t a = static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -64,58 +69,77 @@ __device__ __forceinline__ uint32_t pack2_bf16(float a, float b) {
   return *reinterpret_cast<uint32_t*>(&v);
 }
 
-// grid: (q blocks, Hq, B); block: 128 threads
-template <int DH>
-__global__ void __launch_bounds__(ATT_THREADS, 3) te_attn_kernel(const AttnParams p) {
-  using Cfg = AttnCfg<DH>;
+// grid: (q blocks, Hq / GH, B); block: 128 * GH threads.
+// K/V blocks of 64 keys are double-buffered (cp.async group per block) and shared by the GH q heads
+// of the CTA; query blocks are issued heaviest-first (causal: block qb needs qb + 1 key blocks).
+template <int DH, int GH>
+__global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p) {
+  using Cfg = AttnCfg<DH, GH>;
   constexpr int ROW = Cfg::ROW;
+  constexpr int THREADS = Cfg::THREADS;
   extern __shared__ __align__(16) uint8_t att_smem[];
   __nv_bfloat16* sQ = reinterpret_cast<__nv_bfloat16*>(att_smem);
-  __nv_bfloat16* sK = sQ + ATT_BQ * ROW;
-  __nv_bfloat16* sV = sK + ATT_BKV * ROW;
+  __nv_bfloat16* sKV = sQ + Cfg::Q_ELEMS;
 
   const int b = blockIdx.z;
-  const int head = blockIdx.y;
-  const int qb = blockIdx.x;
+  const int head0 = blockIdx.y * GH;
+  const int qb = gridDim.x - 1 - blockIdx.x;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");  // qkv / cu_seqlens come from predecessor kernels
   const int seq0 = p.cu_seqlens[b];
   const int S = min(p.cu_seqlens[b + 1], p.total_tokens) - seq0;
   const int q0 = qb * ATT_BQ;
   if (q0 >= S) return;
-  const int kvh = head / (p.n_q_heads / p.n_kv_heads);
+  const int kvh = head0 / (p.n_q_heads / p.n_kv_heads);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int hl = warp >> 2;       // local q head of this warp
+  const int wr = warp & 3;        // 16-row group inside the 64-row query block
   const int g = lane >> 2, t = lane & 3;
 
-  const __nv_bfloat16* gq = p.qkv + (size_t)seq0 * p.ld + head * DH;
+  const __nv_bfloat16* gq = p.qkv + (size_t)seq0 * p.ld + head0 * DH;
   const __nv_bfloat16* gk = p.qkv + (size_t)seq0 * p.ld + (p.n_q_heads + kvh) * DH;
   const __nv_bfloat16* gv = p.qkv + (size_t)seq0 * p.ld + (p.n_q_heads + p.n_kv_heads + kvh) * DH;
 
   constexpr int CH = DH / 8;  // 16-byte chunks per row
-  for (int i = tid; i < ATT_BQ * CH; i += ATT_THREADS) {
-    const int r = i / CH, c = i % CH;
-    cp_async16(sQ + r * ROW + c * 8, gq + (size_t)(q0 + r) * p.ld + c * 8, q0 + r < S);
+  auto load_kv = [&](int kb, int stage) {
+    __nv_bfloat16* sK = sKV + stage * Cfg::KV_STAGE_ELEMS;
+    __nv_bfloat16* sV = sK + ATT_BKV * ROW;
+    const int k0 = kb * ATT_BKV;
+    for (int i = tid; i < ATT_BKV * CH; i += THREADS) {
+      const int r = i / CH, c = i % CH;
+      const bool ok = k0 + r < S;
+      cp_async16(sK + r * ROW + c * 8, gk + (size_t)(k0 + r) * p.ld + c * 8, ok);
+      cp_async16(sV + r * ROW + c * 8, gv + (size_t)(k0 + r) * p.ld + c * 8, ok);
+    }
+  };
+  for (int i = tid; i < GH * ATT_BQ * CH; i += THREADS) {
+    const int h = i / (ATT_BQ * CH), r = (i / CH) % ATT_BQ, c = i % CH;
+    cp_async16(sQ + (h * ATT_BQ + r) * ROW + c * 8, gq + (size_t)(q0 + r) * p.ld + h * DH + c * 8, q0 + r < S);
   }
+  load_kv(0, 0);
+  cp_async_commit();
 
   float o[DH / 8][4];
 #pragma unroll
   for (int i = 0; i < DH / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
   float m_run[2] = {-INFINITY, -INFINITY};
   float l_run[2] = {0.f, 0.f};
-  const int qrow0 = q0 + warp * 16 + g;  // this thread's rows: qrow0 and qrow0 + 8 (index within the frame)
+  const int qrow0 = q0 + wr * 16 + g;  // this thread's rows: qrow0 and qrow0 + 8 (index within the frame)
+  const __nv_bfloat16* sQh = sQ + (hl * ATT_BQ + wr * 16) * ROW;
 
   const int n_kv_blocks = qb + 1;  // causal: keys [0, q0 + 64)
   for (int kb = 0; kb < n_kv_blocks; ++kb) {
-    const int k0 = kb * ATT_BKV;
-    __syncthreads();  // previous block's smem reads are done
-    for (int i = tid; i < ATT_BKV * CH; i += ATT_THREADS) {
-      const int r = i / CH, c = i % CH;
-      const bool ok = k0 + r < S;
-      cp_async16(sK + r * ROW + c * 8, gk + (size_t)(k0 + r) * p.ld + c * 8, ok);
-      cp_async16(sV + r * ROW + c * 8, gv + (size_t)(k0 + r) * p.ld + c * 8, ok);
+    if (kb + 1 < n_kv_blocks) {
+      load_kv(kb + 1, (kb + 1) & 1);  // stage (kb+1)&1 was released by the barrier ending iteration kb-1
+      cp_async_commit();
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
     }
-    cp_async_wait_all();
     __syncthreads();
+    const __nv_bfloat16* sK = sKV + (kb & 1) * Cfg::KV_STAGE_ELEMS;
+    const __nv_bfloat16* sV = sK + ATT_BKV * ROW;
+    const int k0 = kb * ATT_BKV;
 
     // ---- S = Q K^T  (16 x 64 per warp)
     float s[ATT_BKV / 8][4];
@@ -126,7 +150,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 3) te_attn_kernel(const AttnParam
       uint32_t a[4];
       {
         const int mi = lane >> 3, r = lane & 7;
-        ldsm_x4(a, sQ + (warp * 16 + (mi & 1) * 8 + r) * ROW + kk * 16 + (mi >> 1) * 8);
+        ldsm_x4(a, sQh + ((mi & 1) * 8 + r) * ROW + kk * 16 + (mi >> 1) * 8);
       }
 #pragma unroll
       for (int nt = 0; nt < ATT_BKV / 16; ++nt) {
@@ -201,6 +225,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 3) te_attn_kernel(const AttnParam
         mma_bf16_16816(o[2 * nt + 1], a, bfr[2], bfr[3]);
       }
     }
+    __syncthreads();  // all warps are done with this K/V stage before it is refilled
   }
   // ---- finalize: row sums across the 4 threads of a row, normalise, store
 #pragma unroll
@@ -209,7 +234,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 3) te_attn_kernel(const AttnParam
     l_run[i] += __shfl_xor_sync(0xffffffffu, l_run[i], 2);
   }
   const float inv0 = 1.0f / l_run[0], inv1 = 1.0f / l_run[1];
-  __nv_bfloat16* out0 = p.out + (size_t)(seq0 + qrow0) * (p.n_q_heads * DH) + head * DH + 2 * t;
+  __nv_bfloat16* out0 = p.out + (size_t)(seq0 + qrow0) * (p.n_q_heads * DH) + (head0 + hl) * DH + 2 * t;
   __nv_bfloat16* out1 = out0 + (size_t)8 * (p.n_q_heads * DH);
 #pragma unroll
   for (int nt = 0; nt < DH / 8; ++nt) {

@@ -81,10 +81,12 @@ __device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u 
 __device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
 
 // ----------------------------------------------------------------------------- epilogues
+// `part` / `nparts`: the epilogue warps that share one TMEM lane quadrant split the tile's columns.
 template <int BN>
-__device__ __forceinline__ void epi_plain(const GemmParams& p, uint32_t t_row, int row, bool valid, int n_blk) {
+__device__ __forceinline__ void epi_plain(const GemmParams& p, uint32_t t_row, int row, bool valid, int n_blk,
+                                          int part, int nparts) {
 #pragma unroll 1
-  for (int c0 = 0; c0 < BN; c0 += 32) {
+  for (int c0 = part * (BN / nparts); c0 < (part + 1) * (BN / nparts); c0 += 32) {
     uint32_t r[32];
     tmem_ld32(t_row + c0, r);
     tmem_ld_wait();
@@ -116,7 +118,7 @@ __device__ __forceinline__ float4 stg_get(const float* buf, int rr, int cq) {
 // Residual epilogue: x += acc (fp32, in place), xg = bf16(x * g_next), per-row partial sum of squares.
 template <int BN>
 __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
-                                          float* stg) {
+                                          float* stg, int part, int nparts) {
   const int sub = lane >> 3;  // row within a group of 4
   const int cq = lane & 7;    // 4-column group inside the 32-column chunk
   const bool has_g = p.g_next != nullptr;
@@ -124,7 +126,7 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
 #pragma unroll
   for (int i = 0; i < 8; ++i) ss[i] = 0.f;
 #pragma unroll 1
-  for (int c0 = 0; c0 < BN; c0 += 32) {
+  for (int c0 = part * (BN / nparts); c0 < (part + 1) * (BN / nparts); c0 += 32) {
     {
       uint32_t r[32];
       tmem_ld32(t_row + c0, r);
@@ -179,7 +181,7 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const int row = row_base + sub + 4 * i;
-      if (row < p.M) p.ssq_out[(size_t)n_blk * p.ssq_stride + row] = ss[i];
+      if (row < p.M) p.ssq_out[(size_t)(n_blk * nparts + part) * p.ssq_stride + row] = ss[i];
     }
   }
 }
@@ -213,12 +215,12 @@ __device__ __forceinline__ void stg_store_bf16(const float* buf, int lane, int r
 // The arithmetic runs in the thread-per-row domain; only the bf16 store is transposed.
 template <int BN>
 __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
-                                           float* stg) {
+                                           float* stg, int part, int nparts) {
   const int my_row = row_base + lane;
   const float rstd = row_rstd(p, my_row, my_row < p.M);
   constexpr int HALF = BN / 2;
 #pragma unroll 1
-  for (int c0 = 0; c0 < HALF; c0 += 32) {
+  for (int c0 = part * (HALF / nparts); c0 < (part + 1) * (HALF / nparts); c0 += 32) {
     float a[32];
     {
       uint32_t g[32], u[32];
@@ -229,7 +231,7 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
       for (int j = 0; j < 32; ++j) {
         const float gv = __uint_as_float(g[j]) * rstd;
         const float uv = __uint_as_float(u[j]) * rstd;
-        a[j] = gv / (1.0f + __expf(-gv)) * uv;
+        a[j] = __fdividef(gv, 1.0f + __expf(-gv)) * uv;  // silu(g) * u; fast divide (2 ulp) ahead of a bf16 store
       }
     }
     stg_put_row(stg, lane, a);
@@ -244,15 +246,19 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
 // domain, where the cos/sin rows are read as whole 128-byte segments.
 template <int BN, int DH>
 __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
-                                        float* stg) {
+                                        float* stg, int part, int nparts) {
   const int my_row = row_base + lane;
   const float rstd = row_rstd(p, my_row, my_row < p.M);
   constexpr int HD2 = DH / 2;
   const int sub = lane >> 3, cq = lane & 7;
   float* bufA = stg;
   float* bufB = stg + 32 * 32;
+  constexpr int HEADS = BN / DH;
+  // heads of the tile are split between the warps of a quadrant; a single head is not split
+  const int hh_begin = (HEADS % nparts == 0) ? part * (HEADS / nparts) : (part == 0 ? 0 : HEADS);
+  const int hh_end = (HEADS % nparts == 0) ? (part + 1) * (HEADS / nparts) : HEADS;
 #pragma unroll 1
-  for (int hh = 0; hh < BN / DH; ++hh) {
+  for (int hh = hh_begin; hh < hh_end; ++hh) {
     const int col0 = n_blk * BN + hh * DH;  // first column of this head in the fused qkv row
     const uint32_t t_head = t_row + hh * DH;
     if (col0 >= p.k_cols_end) {
@@ -472,12 +478,12 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       mbar_wait(&tfull[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
-      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row, valid, n_blk);
+      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row, valid, n_blk, 0, 1);
       float* stg = stg_all + quad * (Cfg::STG_WARP_BYTES / 4);
       const int row_base = m_blk * GEMM_BM + quad * 32;
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, 0, 1);
       tc_fence_before();
       mbar_arrive(&tempty[acc]);
     }
@@ -495,23 +501,30 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 // tcgen05.mma.cta_group::2 (M = 256), which reads both halves of B and writes rows 0-127 of D into
 // the leader's TMEM and rows 128-255 into the peer's.  Per SM this moves A 16 KB + B BN/2 x 128 B per
 // 64-deep k-block instead of A 16 KB + B BN x 128 B: 1.5x less L2->SM traffic at BN = 256.
-template <int BN>
+constexpr int GEMM2_EPI_WARPS = 8;  // two per TMEM lane quadrant: the epilogue is issue-latency-bound per warp
+constexpr int GEMM2_THREADS = 64 + 32 * GEMM2_EPI_WARPS;
+
+template <int BN, int EPI>
 struct Gemm2Cfg {
   static constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
   static constexpr int B_BYTES = (BN / 2) * GEMM_BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int STAGES = (BN == 256) ? 6 : 8;
   static constexpr int BAR_BYTES = 256;
-  static constexpr int STG_WARP_BYTES = 2 * 32 * 32 * 4;
-  static constexpr int STG_BYTES = 4 * STG_WARP_BYTES;
+  // staging per epilogue warp: one swizzled 32x32 fp32 chunk, two for the rotary pairs of EPI_QKV
+  static constexpr int STG_WARP_BYTES = (EPI == EPI_QKV ? 2 : 1) * 32 * 32 * 4;
+  static constexpr int STG_BYTES = GEMM2_EPI_WARPS * STG_WARP_BYTES;
+  static constexpr int SMEM_LIMIT = 232448;  // 227 KB
+  static constexpr int STAGES_FIT = (SMEM_LIMIT - 1024 - BAR_BYTES - STG_BYTES) / STAGE_BYTES;
+  static constexpr int STAGES = STAGES_FIT > 8 ? 8 : STAGES_FIT;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STG_BYTES + 1024;
   static constexpr int TMEM_COLS = 2 * BN;
+  static_assert(STAGES >= 3 && 2 * STAGES + 5 <= BAR_BYTES / 8, "pipeline configuration");
 };
 
 template <int BN, int EPI, int DH>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM2_THREADS, 1)
 te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const GemmParams p) {
-  using Cfg = Gemm2Cfg<BN>;
+  using Cfg = Gemm2Cfg<BN, EPI>;
   constexpr int STAGES = Cfg::STAGES;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -521,7 +534,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   uint64_t* full = bars;                 // used in the leader CTA only
   uint64_t* empty = bars + STAGES;       // one set per CTA (each producer waits on its own)
   uint64_t* tfull = bars + 2 * STAGES;   // one set per CTA (each CTA's epilogue waits on its own)
-  uint64_t* tempty = tfull + 2;          // used in the leader CTA only (count 256: both CTAs' epilogues)
+  uint64_t* tempty = tfull + 2;          // used in the leader CTA only (all epilogue threads of both CTAs)
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
   float* stg_all = reinterpret_cast<float*>(smem + STAGES * Cfg::STAGE_BYTES + Cfg::BAR_BYTES);
 
@@ -542,7 +555,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       }
       for (int i = 0; i < 2; ++i) {
         mbar_init(&tfull[i], 1);
-        mbar_init(&tempty[i], 256);
+        mbar_init(&tempty[i], 2 * 32 * GEMM2_EPI_WARPS);
       }
       fence_mbar_init();
     }
@@ -627,7 +640,9 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
   } else {
     // ===================== epilogue warps (both CTAs, own 128 rows) =====================
-    const int quad = warp & 3;
+    const int quad = warp & 3;         // TMEM lane quadrant this warp may read
+    const int part = (warp - 2) >> 2;  // which share of the tile's columns (two warps per quadrant)
+    constexpr int NPARTS = GEMM2_EPI_WARPS / 4;
     int it = 0;
     pdl_wait();
     for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
@@ -638,12 +653,12 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       mbar_wait(&tfull[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
-      float* stg = stg_all + quad * (Cfg::STG_WARP_BYTES / 4);
+      float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
       const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
-      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk);
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg);
+      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk, part, NPARTS);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS);
       tc_fence_before();
       mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
     }

@@ -172,10 +172,10 @@ cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const te
 template <int BN, int EPI, int DH>
 cudaError_t launch_gemm2(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, int sm_count,
                          cudaStream_t st) {
-  using Cfg = te::Gemm2Cfg<BN>;
+  using Cfg = te::Gemm2Cfg<BN, EPI>;
   const int tiles = ((p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM)) * p.num_n_blk;
   const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
-  return launch_k(te::te_gemm2_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB,
+  return launch_k(te::te_gemm2_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM2_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB,
                   p);
 }
 
@@ -204,11 +204,16 @@ cudaError_t launch_gemm_bn(int bn, int pair, int dh, const CUtensorMap& a, const
   }
 }
 
-template <int DH>
+template <int DH, int GH>
 cudaError_t launch_attn(const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
-  using Cfg = te::AttnCfg<DH>;
-  dim3 grid(q_blocks, p.n_q_heads, n_frames);
-  return launch_k(te::te_attn_kernel<DH>, grid, dim3(te::ATT_THREADS), Cfg::SMEM_BYTES, st, p);
+  using Cfg = te::AttnCfg<DH, GH>;
+  dim3 grid(q_blocks, p.n_q_heads / GH, n_frames);
+  return launch_k(te::te_attn_kernel<DH, GH>, grid, dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, p);
+}
+cudaError_t launch_attn_any(int dh, const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
+  const bool two = (p.n_q_heads / p.n_kv_heads) % 2 == 0;  // pairs of q heads share their kv head
+  if (dh == 128) return two ? launch_attn<128, 2>(p, q_blocks, n_frames, st) : launch_attn<128, 1>(p, q_blocks, n_frames, st);
+  return two ? launch_attn<64, 2>(p, q_blocks, n_frames, st) : launch_attn<64, 1>(p, q_blocks, n_frames, st);
 }
 
 template <int BN, int EPI, int DH>
@@ -217,7 +222,7 @@ cudaError_t set_gemm_attr() {
                                        te::GemmCfg<BN>::SMEM_BYTES);
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(te::te_gemm2_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              te::Gemm2Cfg<BN>::SMEM_BYTES);
+                              te::Gemm2Cfg<BN, EPI>::SMEM_BYTES);
 }
 // Opt every kernel instantiation into its dynamic shared-memory size (once per process, outside
 // any stream capture).
@@ -234,10 +239,14 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
   TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
-  TE_ATTR(cudaFuncSetAttribute(te::te_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               te::AttnCfg<128>::SMEM_BYTES));
-  TE_ATTR(cudaFuncSetAttribute(te::te_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               te::AttnCfg<64>::SMEM_BYTES));
+  TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::AttnCfg<128, 1>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::AttnCfg<128, 2>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::AttnCfg<64, 1>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::AttnCfg<64, 2>::SMEM_BYTES)));
 #undef TE_ATTR
   return cudaSuccess;
 }
@@ -250,13 +259,14 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
   const int n_q = c.n_q_heads * dh;
   const int lb = h->dbg_lb, le = h->dbg_le;
-  const int parts = d / h->bn_res;
   // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
   // one CTA per tile so that more SMs stream weights (HBM-bound regime).
   const int pair = h->pair_mode == 2 ? (T >= 1024 ? 1 : 0) : h->pair_mode;
   const int bx_qkv = box_index(pair ? h->bn_qkv / 2 : h->bn_qkv);
   const int bx_gu = box_index(pair ? h->bn_gu / 2 : h->bn_gu);
   const int bx_res = box_index(pair ? h->bn_res / 2 : h->bn_res);
+  // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
+  const int parts = (d / h->bn_res) * (pair ? te::GEMM2_EPI_WARPS / 4 : 1);
   int nk = 0;
   // Optional per-kernel CUDA-event bracketing (TE_OPT_KERNEL_TIMING; never inside a capture).
   cudaEvent_t ev_a = nullptr;
@@ -324,7 +334,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       ap.n_kv_heads = c.n_kv_heads; ap.total_tokens = T;
       ap.scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
       tick();
-      TE_CUDA(h, dh == 128 ? launch_attn<128>(ap, q_blocks, n_frames, st) : launch_attn<64>(ap, q_blocks, n_frames, st));
+      TE_CUDA(h, launch_attn_any(dh, ap, q_blocks, n_frames, st));
       tock(TE_KCLASS_ATTN);
       ++nk;
     }
@@ -411,7 +421,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   h->bn_qkv = (n_qkv % 256 == 0) ? 256 : 128;
   h->bn_gu = ((2 * c.ffn) % 256 == 0) ? 256 : 128;
   h->bn_res = 128;  // O/down: N = hidden is small -> 128-wide tiles halve the wave-quantisation loss
-  h->ssq_parts_cap = c.hidden / 128;
+  h->ssq_parts_cap = (c.hidden / 128) * (te::GEMM2_EPI_WARPS / 4);
 
   auto fail = [&](int code) {
     te_destroy(h);
