@@ -115,7 +115,9 @@ enum {
   TE_OPT_CTA_PAIR = 2,     /* GEMM tiling: 0 = one CTA per 128-row tile, 1 = CTA pairs (cta_group::2,
                               256-row tiles), 2 = auto by token count (default)                    */
   TE_OPT_RESID_BLOCK_N = 3,/* tile width (128 default, or 256) of the O-proj / down GEMMs          */
-  TE_OPT_PDL = 4           /* 1 (default): kernels are chained with programmatic dependent launch   */
+  TE_OPT_PDL = 4,          /* 1 (default): kernels are chained with programmatic dependent launch   */
+  TE_OPT_TRACE = 5         /* 1: CTA-pair GEMM kernels stamp %globaltimer at pipeline events (debug
+                              aid; read with te_debug_tap(TE_TAP_TRACE)); default 0                 */
 };
 int te_set_option(te_handle* h, int option, int value);
 
@@ -145,7 +147,9 @@ enum {
   TE_TAP_SIN = 3,        /* fp32  [T, dh/2]                                     */
   TE_TAP_QKV = 4,        /* bf16  [T, (Hq+2Hkv)*dh]  q (normed+rotated) | k | v  */
   TE_TAP_ATTN = 5,       /* bf16  [T, Hq*dh]                                    */
-  TE_TAP_ACT = 6         /* bf16  [T, F]       silu(gate)*up                    */
+  TE_TAP_ACT = 6,        /* bf16  [T, F]       silu(gate)*up                    */
+  TE_TAP_TRACE = 7       /* u64   [4 GEMM classes (qkv,oproj,gateup,down)][n_SMs][48] ns stamps
+                            of the last launch of each class (TE_OPT_TRACE)     */
 };
 int te_debug_set_range(te_handle* h, int32_t layer_begin, int32_t layer_end,
                        int32_t stop_after_attn);

@@ -24,8 +24,9 @@ TE_OPT_KERNEL_TIMING = 1
 TE_OPT_CTA_PAIR = 2
 TE_OPT_RESID_BLOCK_N = 3
 TE_OPT_PDL = 4
+TE_OPT_TRACE = 5
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
-TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT = range(7)
+TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 
 EXPORTS = [
     "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_host",

@@ -56,7 +56,17 @@ struct GemmParams {
   // EPI_PLAIN
   float* c;
   int ld_c;
+  // optional cycle trace (debug): trace[blockIdx.x * TRACE_SLOTS + slot] = globaltimer ns
+  unsigned long long* trace;
 };
+constexpr int TRACE_SLOTS = 48;
+__device__ __forceinline__ void trace_stamp(const GemmParams& p, int slot) {
+  if (p.trace != nullptr) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    p.trace[(size_t)blockIdx.x * TRACE_SLOTS + slot] = t;
+  }
+}
 
 template <int BN>
 struct GemmCfg {
@@ -116,17 +126,35 @@ __device__ __forceinline__ float4 stg_get(const float* buf, int rr, int cq) {
 }
 
 // Residual epilogue: x += acc (fp32, in place), xg = bf16(x * g_next), per-row partial sum of squares.
+// The x operand is software-pipelined: ResidPrefetch::issue() is called BEFORE the accumulator is
+// ready (the epilogue warps idle during the main loop), and each chunk's loads are issued one
+// chunk ahead, so the L2 round trips are off the critical path.
+struct ResidPrefetch {
+  float4 xv[8];
+};
+template <int BN>
+__device__ __forceinline__ void resid_issue(const GemmParams& p, ResidPrefetch& pf, int row_base, int lane, int n_blk,
+                                            int c0) {
+  const int sub = lane >> 3, cq = lane & 7;
+  const int col = n_blk * BN + c0 + cq * 4;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int row = row_base + sub + 4 * i;
+    if (row < p.M) pf.xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
+  }
+}
 template <int BN>
 __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
-                                          float* stg, int part, int nparts) {
+                                          float* stg, int part, int nparts, ResidPrefetch& pf) {
   const int sub = lane >> 3;  // row within a group of 4
   const int cq = lane & 7;    // 4-column group inside the 32-column chunk
   const bool has_g = p.g_next != nullptr;
   float ss[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) ss[i] = 0.f;
+  const int c_end = (part + 1) * (BN / nparts);
 #pragma unroll 1
-  for (int c0 = part * (BN / nparts); c0 < (part + 1) * (BN / nparts); c0 += 32) {
+  for (int c0 = part * (BN / nparts); c0 < c_end; c0 += 32) {
     {
       uint32_t r[32];
       tmem_ld32(t_row + c0, r);
@@ -145,10 +173,8 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
     }
     float4 xv[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int row = row_base + sub + 4 * i;
-      if (row < p.M) xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
-    }
+    for (int i = 0; i < 8; ++i) xv[i] = pf.xv[i];
+    if (c0 + 32 < c_end) resid_issue<BN>(p, pf, row_base, lane, n_blk, c0 + 32);  // next chunk's x in flight
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const int rr = sub + 4 * i;
@@ -170,7 +196,7 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
     }
     __syncwarp();
   }
-  // per-row sum of squares over this tile's columns: fixed-order reduction over the row's 8 lanes
+  // per-row sum of squares over this warp's columns: fixed-order reduction over the row's 8 lanes
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 1);
@@ -215,9 +241,7 @@ __device__ __forceinline__ void stg_store_bf16(const float* buf, int lane, int r
 // The arithmetic runs in the thread-per-row domain; only the bf16 store is transposed.
 template <int BN>
 __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
-                                           float* stg, int part, int nparts) {
-  const int my_row = row_base + lane;
-  const float rstd = row_rstd(p, my_row, my_row < p.M);
+                                           float* stg, int part, int nparts, float rstd) {
   constexpr int HALF = BN / 2;
 #pragma unroll 1
   for (int c0 = part * (HALF / nparts); c0 < (part + 1) * (HALF / nparts); c0 += 32) {
@@ -234,10 +258,20 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
         a[j] = __fdividef(gv, 1.0f + __expf(-gv)) * uv;  // silu(g) * u; fast divide (2 ulp) ahead of a bf16 store
       }
     }
+#ifdef TE_EXP_SWIGLU_DIRECT
+    if (row_base + lane < p.M) {
+      uint4* dst = reinterpret_cast<uint4*>(p.act + (size_t)(row_base + lane) * p.ld_act + n_blk * HALF + c0);
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        dst[j] = make_uint4(pack_bf16(a[8 * j], a[8 * j + 1]), pack_bf16(a[8 * j + 2], a[8 * j + 3]),
+                            pack_bf16(a[8 * j + 4], a[8 * j + 5]), pack_bf16(a[8 * j + 6], a[8 * j + 7]));
+    }
+#else
     stg_put_row(stg, lane, a);
     __syncwarp();
     stg_store_bf16(stg, lane, row_base, p.M, p.act, p.ld_act, n_blk * HALF + c0);
     __syncwarp();
+#endif
   }
 }
 
@@ -246,9 +280,7 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
 // domain, where the cos/sin rows are read as whole 128-byte segments.
 template <int BN, int DH>
 __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
-                                        float* stg, int part, int nparts) {
-  const int my_row = row_base + lane;
-  const float rstd = row_rstd(p, my_row, my_row < p.M);
+                                        float* stg, int part, int nparts, float rstd) {
   constexpr int HD2 = DH / 2;
   const int sub = lane >> 3, cq = lane & 7;
   float* bufA = stg;
@@ -295,9 +327,25 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
       }
     }
     const float sc = rstd / sqrtf(ss * (1.0f / DH) + p.eps);
-    // ---- Pass 2: normalised halves a = u[c0..c0+32), b = u[HD2+c0..) -> staging -> rotate -> store
+#ifdef TE_EXP_QKV_STAMPS
+    if (lane == 0 && part == 0 && (row_base & 127) == 0 && p.trace && p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 40] == 0) trace_stamp(p, 40);
+#endif
+    // ---- Pass 2: normalised halves a = u[c0..c0+32), b = u[HD2+c0..) -> staging -> rotate -> store.
+    // All cos/sin segments of the step are requested up front (16 independent 16-byte loads per
+    // lane) so that their L2 round trips overlap the TMEM reads and the staging instead of
+    // serialising behind each other.
 #pragma unroll 1
     for (int c0 = 0; c0 < HD2; c0 += 32) {
+      const int cc = c0 + cq * 4;  // this lane's 4 columns inside the half
+      float4 cs[8], sn[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int row = min(row_base + sub + 4 * i, p.M - 1);
+        cs[i] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc));
+        sn[i] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc));
+      }
+      const uint2 ga = __ldg(reinterpret_cast<const uint2*>(gain + cc));
+      const uint2 gb = __ldg(reinterpret_cast<const uint2*>(gain + HD2 + cc));
       {
         float v[32];
         uint32_t r[32];
@@ -313,9 +361,6 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
         stg_put_row(bufB, lane, v);
       }
       __syncwarp();
-      const int cc = c0 + cq * 4;  // this lane's 4 columns inside the half
-      const uint2 ga = __ldg(reinterpret_cast<const uint2*>(gain + cc));
-      const uint2 gb = __ldg(reinterpret_cast<const uint2*>(gain + HD2 + cc));
       const float gA[4] = {bf16_lo(ga.x), bf16_hi(ga.x), bf16_lo(ga.y), bf16_hi(ga.y)};
       const float gB[4] = {bf16_lo(gb.x), bf16_hi(gb.x), bf16_lo(gb.y), bf16_hi(gb.y)};
 #pragma unroll
@@ -323,14 +368,12 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
         const int rr = sub + 4 * i;
         const int row = row_base + rr;
         if (row < p.M) {
-          const float4 cs = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc));
-          const float4 sn = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc));
           const float4 a = stg_get(bufA, rr, cq);
           const float4 b = stg_get(bufB, rr, cq);
           const float ua[4] = {a.x * gA[0], a.y * gA[1], a.z * gA[2], a.w * gA[3]};
           const float ub[4] = {b.x * gB[0], b.y * gB[1], b.z * gB[2], b.w * gB[3]};
-          const float c[4] = {cs.x, cs.y, cs.z, cs.w};
-          const float sv[4] = {sn.x, sn.y, sn.z, sn.w};
+          const float c[4] = {cs[i].x, cs[i].y, cs[i].z, cs[i].w};
+          const float sv[4] = {sn[i].x, sn[i].y, sn[i].z, sn[i].w};
           float r1[4], r2[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
@@ -346,6 +389,10 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
         }
       }
       __syncwarp();
+#ifdef TE_EXP_QKV_STAMPS
+      if (lane == 0 && part == 0 && (row_base & 127) == 0 && p.trace && c0 == 0 && p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 42] == 0) trace_stamp(p, 42);
+      if (lane == 0 && part == 0 && (row_base & 127) == 0 && p.trace && c0 == 32 && p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 43] == 0) trace_stamp(p, 43);
+#endif
     }
   }
 }
@@ -475,19 +522,25 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const uint32_t acc_phase = (it >> 1) & 1;
       const int row = m_blk * GEMM_BM + row_in_tile;
       const bool valid = row < p.M;
+      // operands that do not depend on the accumulator are fetched while the main loop still runs
+      float rstd = 0.f;
+      ResidPrefetch pf;
+      if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row, valid);
+      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, pf, m_blk * GEMM_BM + quad * 32, lane, n_blk, 0);
       mbar_wait(&tfull[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
       if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row, valid, n_blk, 0, 1);
       float* stg = stg_all + quad * (Cfg::STG_WARP_BYTES / 4);
       const int row_base = m_blk * GEMM_BM + quad * 32;
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, 0, 1);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1, pf);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1, rstd);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, 0, 1, rstd);
       tc_fence_before();
       mbar_arrive(&tempty[acc]);
     }
   }
+  __syncwarp();  // the elected producer / MMA lanes rejoin their warps before the block barrier
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
@@ -542,6 +595,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const int lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const bool leader = rank == 0;
+  if (threadIdx.x == 0) trace_stamp(p, 0);
 
   if (warp == 0 && elect_one()) {
     tma_prefetch_desc(&tmA);
@@ -568,6 +622,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_stamp(p, 1);
 
   const int num_kb = p.K / GEMM_BK;
   const int num_mp = (p.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);
@@ -590,6 +645,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         }
       }
       pdl_wait();
+      trace_stamp(p, 2);
       bool first = true;
       for (int tile = pair; tile < num_tiles; tile += num_pairs) {
         const int mp = tile % num_mp;
@@ -626,6 +682,7 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         const uint32_t d_tmem = tmem_base + acc * BN;
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&full[stage], phase);
+          if (kb == 0 && it < 10) trace_stamp(p, 3 + it);
           tc_fence_after();
           const uint64_t a_desc = umma_smem_desc_sw128(smem_u32(sA + stage * Cfg::A_BYTES));
           const uint64_t b_desc = umma_smem_desc_sw128(smem_u32(sB + stage * Cfg::B_BYTES));
@@ -650,22 +707,32 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       const int n_blk = tile / num_mp;
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
+      const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
+      // operands that do not depend on the accumulator are fetched while the main loop still runs
+      float rstd = 0.f;
+      ResidPrefetch pf;
+      if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row_base + lane, row_base + lane < p.M);
+      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, pf, row_base, lane, n_blk, part * (BN / NPARTS));
       mbar_wait(&tfull[acc], acc_phase);
+      if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 14 + it);
       tc_fence_after();
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
       float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
-      const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
       if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk, part, NPARTS);
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
       tc_fence_before();
       mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
+      if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 25 + it);
     }
   }
   tc_fence_before();
+  __syncwarp();  // the elected producer / MMA lanes rejoin their warps before the block barrier
   __syncthreads();
+  if (threadIdx.x == 0) trace_stamp(p, 36);
   cluster_sync_all();  // the peer may still be signalling our barriers / reading our smem until here
+  if (threadIdx.x == 0) trace_stamp(p, 37);
   if (warp == 1) {
     __syncwarp();
     tc_fence_after();

@@ -89,6 +89,8 @@ struct te_handle {
   double* inv_freq = nullptr;
   bf16 *xg = nullptr, *qkv = nullptr, *attn = nullptr, *act = nullptr;
   int ssq_parts_cap = 0;
+  unsigned long long* trace = nullptr;  // [4 GEMM classes][sm_count][TRACE_SLOTS] (debug, TE_OPT_TRACE)
+  int trace_on = 0;
   // host-path staging
   float *stg_embeds = nullptr, *stg_out = nullptr;
   int32_t* stg_lens = nullptr;
@@ -310,6 +312,8 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   te::GemmParams base{};
   base.M = T; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = parts; base.ssq_stride = c.max_tokens;
   base.inv_d = 1.0f / static_cast<float>(d); base.eps = c.rms_eps;
+  const size_t trace_stride = (size_t)h->sm_count * te::TRACE_SLOTS;
+  auto trace_ptr = [&](int cls) { return h->trace_on ? h->trace + cls * trace_stride : nullptr; };
 
   // host-side upper bound of S_b for the attention grid (exact lengths stay on the device)
   int s_bound = T - (n_frames - 1) * (grid_h * grid_w);
@@ -323,6 +327,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / h->bn_qkv;
       p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
       p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
+      p.trace = trace_ptr(0);
       tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(h->bn_qkv, pair, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
       tock(TE_KCLASS_QKV);
@@ -342,6 +347,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       te::GemmParams p = base;
       p.N = d; p.K = n_q; p.num_n_blk = d / h->bn_res;
       p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
+      p.trace = trace_ptr(1);
       tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_attn, h->tm[l].o[bx_res], p, h->sm_count, st));
       tock(TE_KCLASS_OPROJ);
@@ -352,6 +358,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       te::GemmParams p = base;
       p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / h->bn_gu;
       p.act = h->act; p.ld_act = F;
+      p.trace = trace_ptr(2);
       tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, pair, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
       tock(TE_KCLASS_GATEUP);
@@ -362,6 +369,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.N = d; p.K = F; p.num_n_blk = d / h->bn_res;
       p.x = out; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
       p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
+      p.trace = trace_ptr(3);
       tick();
       TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_act, h->tm[l].d[bx_res], p, h->sm_count, st));
       tock(TE_KCLASS_DOWN);
@@ -642,6 +650,16 @@ int te_set_option(te_handle* h, int option, int value) {
     h->timing = value ? 1 : 0;
     return TE_OK;
   }
+  if (option == TE_OPT_TRACE) {
+    if (value && !h->trace) {
+      const size_t bytes = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+      TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->trace), bytes));
+      TE_CUDA(h, cudaMemset(h->trace, 0, bytes));
+    }
+    h->trace_on = value ? 1 : 0;
+    free_graphs(h);
+    return TE_OK;
+  }
   if (option == TE_OPT_PDL) {
     h->pdl = value ? 1 : 0;
     free_graphs(h);
@@ -705,6 +723,11 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
     case TE_TAP_QKV: src = h->qkv; need = T * (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim * sizeof(bf16); break;
     case TE_TAP_ATTN: src = h->attn; need = T * (size_t)c.n_q_heads * c.head_dim * sizeof(bf16); break;
     case TE_TAP_ACT: src = h->act; need = T * (size_t)c.ffn * sizeof(bf16); break;
+    case TE_TAP_TRACE:
+      src = h->trace;
+      need = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+      if (!src) return TE_ERR_INVALID_ARG;
+      break;
     default: return TE_ERR_INVALID_ARG;
   }
   if (T == 0 || n_bytes != need) return TE_ERR_INVALID_ARG;
@@ -742,7 +765,7 @@ void te_destroy(te_handle* h) {
   free_graphs(h);
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
-                  h->act, h->stg_embeds, h->stg_out, h->stg_lens};
+                  h->act, h->stg_embeds, h->stg_out, h->stg_lens, h->trace};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
