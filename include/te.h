@@ -116,8 +116,10 @@ enum {
                               256-row tiles), 2 = auto by token count (default)                    */
   TE_OPT_RESID_BLOCK_N = 3,/* tile width (128 default, or 256) of the O-proj / down GEMMs          */
   TE_OPT_PDL = 4,          /* 1 (default): kernels are chained with programmatic dependent launch   */
-  TE_OPT_TRACE = 5         /* 1: CTA-pair GEMM kernels stamp %globaltimer at pipeline events (debug
+  TE_OPT_TRACE = 5,        /* 1: CTA-pair GEMM kernels stamp %globaltimer at pipeline events (debug
                               aid; read with te_debug_tap(TE_TAP_TRACE)); default 0                 */
+  TE_OPT_ATTN_IMPL = 6     /* attention kernel: 1 (default) = tcgen05 kernel (S, P, O in tensor memory)
+                              when Hq/Hkv is a power of two <= 8, 0 = mma.sync flash kernel          */
 };
 int te_set_option(te_handle* h, int option, int value);
 

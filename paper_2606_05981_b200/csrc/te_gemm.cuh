@@ -59,12 +59,13 @@ struct GemmParams {
   // optional cycle trace (debug): trace[blockIdx.x * TRACE_SLOTS + slot] = globaltimer ns
   unsigned long long* trace;
 };
-constexpr int TRACE_SLOTS = 48;
+constexpr int TRACE_SLOTS = 96;  // [0,48): globaltimer ns, [48,96): SM clock of the same stamp
 __device__ __forceinline__ void trace_stamp(const GemmParams& p, int slot) {
   if (p.trace != nullptr) {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     p.trace[(size_t)blockIdx.x * TRACE_SLOTS + slot] = t;
+    p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 48 + slot] = static_cast<unsigned long long>(clock64());
   }
 }
 

@@ -12,6 +12,7 @@
 
 #include "../../include/te.h"
 #include "te_attn.cuh"
+#include "te_attn_tc.cuh"
 #include "te_gemm.cuh"
 #include "te_prep.cuh"
 
@@ -74,6 +75,7 @@ struct te_handle {
   bool loaded = false;
   // tile choices
   int bn_qkv = 256, bn_gu = 256, bn_res = 128;
+  int attn_impl = 1;  // 1: tcgen05 kernel (te_attn_tc.cuh) when Hq/Hkv is a power of two <= 8; 0: mma.sync kernel
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   // weights
   bf16* w = nullptr;
@@ -218,6 +220,14 @@ cudaError_t launch_attn_any(int dh, const te::AttnParams& p, int q_blocks, int n
   return two ? launch_attn<64, 2>(p, q_blocks, n_frames, st) : launch_attn<64, 1>(p, q_blocks, n_frames, st);
 }
 
+template <int DH>
+cudaError_t launch_attn_tc(const CUtensorMap& tmQ, const CUtensorMap& tmKV, const te::AttnTcParams& p, int n_split,
+                           int n_frames, cudaStream_t st) {
+  using Cfg = te::AttnTcCfg<DH>;
+  dim3 grid(n_split, p.n_kv_heads, n_frames);
+  return launch_k(te::te_attn_tc_kernel<DH>, grid, dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, tmQ, tmKV, p);
+}
+
 template <int BN, int EPI, int DH>
 cudaError_t set_gemm_attr() {
   cudaError_t e = cudaFuncSetAttribute(te::te_gemm_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -249,6 +259,10 @@ cudaError_t init_kernel_attrs() {
                                 te::AttnCfg<64, 1>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::AttnCfg<64, 2>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_attn_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::AttnTcCfg<128>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_attn_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::AttnTcCfg<64>::SMEM_BYTES)));
 #undef TE_ATTR
   return cudaSuccess;
 }
@@ -319,6 +333,25 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   int s_bound = T - (n_frames - 1) * (grid_h * grid_w);
   if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
   const int q_blocks = (s_bound + te::ATT_BQ - 1) / te::ATT_BQ;
+  // tcgen05 attention: one CTA per (frame, kv head), optionally split over query tiles when the batch
+  // alone cannot fill the SMs; needs G = Hq/Hkv to be a power of two with >= 16 positions per 128-row tile
+  const int G = c.n_q_heads / c.n_kv_heads;
+  int g_shift = 0;
+  while ((1 << g_shift) < G) ++g_shift;
+  const bool attn_tc = h->attn_impl == 1 && (1 << g_shift) == G && G <= 8;
+  CUtensorMap tmQ, tmKV;
+  int attn_split = 1;
+  if (attn_tc) {
+    const int pt = 128 >> g_shift;
+    if (!make_tmap(&tmQ, h->qkv, T, n_qkv, pt) || !make_tmap(&tmKV, h->qkv, T, n_qkv, 64)) {
+      h->err = "cuTensorMapEncodeTiled failed for a qkv map";
+      return TE_ERR_CUDA;
+    }
+    const int tiles_max = (s_bound + pt - 1) / pt;
+    attn_split = h->sm_count / (n_frames * c.n_kv_heads);
+    if (attn_split < 1) attn_split = 1;
+    if (attn_split > tiles_max) attn_split = tiles_max;
+  }
 
   for (int l = lb; l < le; ++l) {
     const LayerOff& o = h->off[l];
@@ -339,7 +372,15 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       ap.n_kv_heads = c.n_kv_heads; ap.total_tokens = T;
       ap.scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
       tick();
-      TE_CUDA(h, launch_attn_any(dh, ap, q_blocks, n_frames, st));
+      if (attn_tc) {
+        te::AttnTcParams tp{};
+        tp.out = h->attn; tp.cu_seqlens = h->cu; tp.n_q_heads = c.n_q_heads; tp.n_kv_heads = c.n_kv_heads;
+        tp.g_shift = g_shift; tp.total_tokens = T; tp.scale_log2 = ap.scale_log2;
+        TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(tmQ, tmKV, tp, attn_split, n_frames, st)
+                             : launch_attn_tc<64>(tmQ, tmKV, tp, attn_split, n_frames, st));
+      } else {
+        TE_CUDA(h, launch_attn_any(dh, ap, q_blocks, n_frames, st));
+      }
       tock(TE_KCLASS_ATTN);
       ++nk;
     }
@@ -668,6 +709,12 @@ int te_set_option(te_handle* h, int option, int value) {
   if (option == TE_OPT_CTA_PAIR) {
     if (value < 0 || value > 2) return TE_ERR_INVALID_ARG;
     h->pair_mode = value;
+    free_graphs(h);
+    return TE_OK;
+  }
+  if (option == TE_OPT_ATTN_IMPL) {
+    if (value < 0 || value > 1) return TE_ERR_INVALID_ARG;
+    h->attn_impl = value;
     free_graphs(h);
     return TE_OK;
   }
