@@ -241,7 +241,7 @@ def main():
     enc = te.TextEncoder(m, w.n_frames, T, device=local_rank)
     enc.load_weights(blob)
     opt_ids = {"pdl": te.TE_OPT_PDL, "cta_pair": te.TE_OPT_CTA_PAIR, "resid_bn": te.TE_OPT_RESID_BLOCK_N,
-               "graph": te.TE_OPT_USE_GRAPH}
+               "graph": te.TE_OPT_USE_GRAPH, "attn_impl": te.TE_OPT_ATTN_IMPL}
     for kv in filter(None, args.opt.split(",")):
         k, v = kv.split("=")
         te.te_set_option(enc.h, opt_ids[k], int(v))
@@ -325,6 +325,9 @@ def main():
         return
 
     peaks = load_peaks()
+    # dram__bytes_read.sum + dram__bytes_write.sum of one gate/up launch, from the committed ncu --set full
+    # capture (profiles/r01c_ncu_full_layer_cfg4.md); only that workload was captured
+    traffic = {"cfg4_28L_B16": 63.348992e6 + 15.863552e6}.get(w.name)
     flops, wbytes, abytes = stack_work(m, seq_lens)
     t_compute = flops / (peaks["tf_sustained"] * 1e12)
     t_hbm = (wbytes + abytes) / (peaks["hbm_gbs"] * 1e9)
@@ -340,13 +343,15 @@ def main():
         roofline = {"bound": "tensor", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
                     "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sustained"],
                     "peak_kind": f"bf16_tflops_sustained ({peaks['src']}); kernel timed inside a long step",
-                    "frac_of_burst": achieved / peaks["tf_burst"], "traffic": None}
+                    "frac_of_burst": achieved / peaks["tf_burst"], "traffic": traffic,
+                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01c)",
+                    "algorithmic_bytes": 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn}
     else:
         gu_bytes = 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
         achieved = gu_bytes / (gu_ms / gu_n / 1000.0) / 1e9
         roofline = {"bound": "hbm", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                    "peak_kind": f"hbm_gbs ({peaks['src']})", "traffic": None}
+                    "peak_kind": f"hbm_gbs ({peaks['src']})", "traffic": traffic}
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
