@@ -118,8 +118,12 @@ enum {
   TE_OPT_PDL = 4,          /* 1 (default): kernels are chained with programmatic dependent launch   */
   TE_OPT_TRACE = 5,        /* 1: CTA-pair GEMM kernels stamp %globaltimer at pipeline events (debug
                               aid; read with te_debug_tap(TE_TAP_TRACE)); default 0                 */
-  TE_OPT_ATTN_IMPL = 6     /* attention kernel: 1 (default) = tcgen05 kernel (S, P, O in tensor memory)
+  TE_OPT_ATTN_IMPL = 6,    /* attention kernel: 1 (default) = tcgen05 kernel (S, P, O in tensor memory)
                               when Hq/Hkv is a power of two <= 8, 0 = mma.sync flash kernel          */
+  TE_OPT_SPLIT_K = 7       /* 1 (default): small batches (fewer 128-row tiles than SMs in a GEMM, no
+                              CTA pairs) run the split-K kernel: several CTAs per output tile, each
+                              streaming its own K-slice of the weights; partial tiles are summed in a
+                              fixed order (deterministic).  0: one CTA per tile                      */
 };
 int te_set_option(te_handle* h, int option, int value);
 
@@ -163,6 +167,12 @@ int te_debug_tap(te_handle* h, int what, void* dst_host, size_t n_bytes);
  * kernel (256-row tiles).  Synchronous. */
 int te_debug_gemm(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
                   int32_t n, int32_t k, int32_t block_n, int32_t cta_pair);
+
+/* Test-only: the same product through the split-K kernel (te_gemm_splitk.cuh): `splits` CTAs
+ * (1..8, <= k/64) per 128 x block_n tile, fixed-order reduction of the fp32 partial tiles.
+ * Needs tiles * splits <= number of SMs (TE_ERR_UNSUPPORTED otherwise).  Synchronous. */
+int te_debug_gemm_splitk(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
+                         int32_t n, int32_t k, int32_t block_n, int32_t splits);
 
 void te_destroy(te_handle* h);
 const char* te_strerror(int code);

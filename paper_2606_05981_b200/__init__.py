@@ -26,13 +26,14 @@ TE_OPT_RESID_BLOCK_N = 3
 TE_OPT_PDL = 4
 TE_OPT_TRACE = 5
 TE_OPT_ATTN_IMPL = 6
+TE_OPT_SPLIT_K = 7
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 
 EXPORTS = [
     "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_host",
     "te_query_async_error", "te_set_option", "te_kernel_launches", "te_kernel_times", "te_debug_set_range",
-    "te_debug_tap", "te_debug_gemm", "te_destroy", "te_strerror", "te_last_error",
+    "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_destroy", "te_strerror", "te_last_error",
 ]
 
 
@@ -91,6 +92,8 @@ def lib() -> ctypes.CDLL:
     L.te_debug_tap.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
     L.te_debug_gemm.restype = c_int
     L.te_debug_gemm.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
+    L.te_debug_gemm_splitk.restype = c_int
+    L.te_debug_gemm_splitk.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
     L.te_destroy.restype = None
     L.te_destroy.argtypes = [c_void_p]
     L.te_strerror.restype = c_char_p
@@ -194,6 +197,10 @@ def te_debug_tap(h, what: int, dst_host):
 
 def te_debug_gemm(device, a_bf16, b_bf16, c, m, n, k, block_n=256, cta_pair=0):
     _check(lib().te_debug_gemm(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, cta_pair))
+
+
+def te_debug_gemm_splitk(device, a_bf16, b_bf16, c, m, n, k, block_n=128, splits=2):
+    _check(lib().te_debug_gemm_splitk(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, splits))
 
 
 def te_destroy(h):

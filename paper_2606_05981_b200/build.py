@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libte_b200.so")
 SOURCES = ["te_runtime.cu"]
-HEADERS = ["te_ptx.cuh", "te_gemm.cuh", "te_attn.cuh", "te_attn_tc.cuh", "te_prep.cuh"]
+HEADERS = ["te_ptx.cuh", "te_gemm.cuh", "te_gemm_splitk.cuh", "te_attn.cuh", "te_attn_tc.cuh", "te_prep.cuh"]
 
 
 def _stale() -> bool:
@@ -27,7 +27,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
            "-shared", "-Xcompiler", "-fPIC", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    cmd += ["-lcuda"] if False else []   # driver entry points are resolved through cudart
+    cmd += os.environ.get("TE_NVCC_EXTRA", "").split()   # e.g. -DTE_DBG_... for experiments
     if verbose:
         cmd += ["-Xptxas", "-v"]
     r = subprocess.run(cmd, capture_output=True, text=True)

@@ -29,7 +29,8 @@ enum { EPI_PLAIN = 0, EPI_QKV = 1, EPI_RESID = 2, EPI_SWIGLU = 3 };
 struct GemmParams {
   int M, N, K;
   int num_m_blk, num_n_blk;
-  // RMSNorm statistics of the A rows (consumer side): ssq_in[part * ssq_stride + row]
+  // RMSNorm statistics of the A rows (consumer side): ssq_in[row * ssq_stride + part], one 16-byte-aligned
+  // run of `ssq_parts` partial sums of squares per row (a row's parts share a cache line)
   const float* ssq_in;
   int ssq_parts;
   int ssq_stride;
@@ -49,7 +50,7 @@ struct GemmParams {
   int ld_x;
   const __nv_bfloat16* g_next;  // may be null (no next norm)
   __nv_bfloat16* xg;            // [T, ld_x] bf16(x * g_next)
-  float* ssq_out;               // [num_n_blk][ssq_stride]
+  float* ssq_out;               // [T][ssq_stride], entry n_blk * nparts + part
   // EPI_SWIGLU
   __nv_bfloat16* act;
   int ld_act;
@@ -58,6 +59,10 @@ struct GemmParams {
   int ld_c;
   // optional cycle trace (debug): trace[blockIdx.x * TRACE_SLOTS + slot] = globaltimer ns
   unsigned long long* trace;
+  // split-K kernel (te_gemm_splitk.cuh): CTAs per output tile, fp32 partial-tile scratch, per-tile semaphores
+  int splits;
+  float* sk_scratch;
+  int* sk_sem;
 };
 constexpr int TRACE_SLOTS = 96;  // [0,48): globaltimer ns, [48,96): SM clock of the same stamp
 __device__ __forceinline__ void trace_stamp(const GemmParams& p, int slot) {
@@ -208,15 +213,22 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const int row = row_base + sub + 4 * i;
-      if (row < p.M) p.ssq_out[(size_t)(n_blk * nparts + part) * p.ssq_stride + row] = ss[i];
+      if (row < p.M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * nparts + part)] = ss[i];
     }
   }
 }
 
 __device__ __forceinline__ float row_rstd(const GemmParams& p, int row, bool valid) {
   float s = 0.f;
-  if (valid)
-    for (int i = 0; i < p.ssq_parts; ++i) s += p.ssq_in[(size_t)i * p.ssq_stride + row];
+  if (valid) {
+    const float* q = p.ssq_in + (size_t)row * p.ssq_stride;
+    int i = 0;
+    for (; i + 4 <= p.ssq_parts; i += 4) {  // sequential sum, fixed order
+      const float4 v = *reinterpret_cast<const float4*>(q + i);
+      s += v.x; s += v.y; s += v.z; s += v.w;
+    }
+    for (; i < p.ssq_parts; ++i) s += q[i];
+  }
   return 1.0f / sqrtf(s * p.inv_d + p.eps);
 }
 

@@ -12,82 +12,106 @@ namespace te {
 
 enum { FLAG_BAD_LEN = 1, FLAG_BAD_TOTAL = 2, FLAG_TOO_LONG = 4 };
 
-// One block; thread 0 scans (B is at most a few thousand).  cu[b] is clamped to total_tokens so
-// that later kernels never touch rows beyond the caller's buffers even when validation fails.
-__global__ void te_scan_kernel(const int32_t* __restrict__ text_lens, int n_frames, int n_vis, int total_tokens,
-                               int max_tokens_per_frame, int32_t* __restrict__ cu, int32_t* __restrict__ flag) {
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous call's kernels still read cu / flag
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  long long acc = 0;
-  int f = 0;
-  cu[0] = 0;
-  for (int b = 0; b < n_frames; ++b) {
-    int tl = text_lens[b];
-    if (tl < 0) { f |= FLAG_BAD_LEN; tl = 0; }
-    const int s = n_vis + tl;
-    if (s > max_tokens_per_frame) f |= FLAG_TOO_LONG;
-    acc += s;
-    cu[b + 1] = static_cast<int32_t>(acc < total_tokens ? acc : total_tokens);
-  }
-  if (acc != total_tokens) f |= FLAG_BAD_TOTAL;
-  if (f) atomicOr(flag, f);
-}
-
 struct PrepParams {
-  const float* embeds;  // [T, d]
-  float* out;           // [T, d]  fp32 residual stream
-  const int32_t* cu;    // [B+1]
-  int32_t* pos;         // [3, T]
-  float* cos_t;         // [T, dh/2]
+  const float* embeds;       // [T, d]
+  const int32_t* text_lens;  // [B]
+  float* out;                // [T, d]  fp32 residual stream
+  int32_t* cu;               // [B+1]   packing offsets (written by block 0)
+  int32_t* flag;             // sticky validation flag
+  int32_t* pos;              // [3, T]
+  float* cos_t;              // [T, dh/2]
   float* sin_t;
   const double* inv_freq;       // [dh/2]  omega_i = theta^(-2i/dh)
   const __nv_bfloat16* g_first; // gain of the first RMSNorm that will consume the residual
   __nv_bfloat16* xg;            // [T, d]  bf16(x * g_first)
-  float* ssq;                   // [parts][ssq_stride]
+  float* ssq;                   // [T][ssq_stride], first ssq_parts entries of a row used
   int ssq_parts, ssq_stride;
-  int n_frames, total_tokens, d, half_dim;
+  int n_frames, total_tokens, d, half_dim, max_tokens_per_frame;
   int grid_h, grid_w, sec_t, sec_h;
 };
 
-// One warp per token.
+// One block per token.  Warp 0 of EVERY block scans text_lens itself (B is a few dozen frames; the
+// scan is cheaper than a second kernel and a grid-wide dependency): cu[b+1] = min(sum_{i<=b} S_i, T),
+// clamped so that no kernel touches rows beyond the caller's buffers even when validation fails; the
+// token's frame is the largest b with cu[b] <= tok.  Block 0 also publishes cu[] and the validation flag.
 __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
+  __shared__ int s_start;
+  __shared__ float s_ss[8];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tok = blockIdx.x * 8 + warp;
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  if (tok >= p.total_tokens) return;
-  // frame of this token: largest b with cu[b] <= tok
-  int lo = 0, hi = p.n_frames - 1;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (p.cu[mid] <= tok) lo = mid; else hi = mid - 1;
-  }
-  const int n = tok - p.cu[lo];
+  const int tok = blockIdx.x;
   const int n_vis = p.grid_h * p.grid_w;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous call's kernels still read cu / flag / out
+  if (warp == 0) {
+    long long carry = 0;
+    int best_b = 0, best_start = 0, f = 0;
+    for (int base = 0; base < p.n_frames; base += 32) {
+      const int b = base + lane;
+      int sb = 0;
+      if (b < p.n_frames) {
+        int tl = p.text_lens[b];
+        if (tl < 0) { f |= FLAG_BAD_LEN; tl = 0; }
+        sb = n_vis + tl;
+        if (sb > p.max_tokens_per_frame) f |= FLAG_TOO_LONG;
+      }
+      long long incl = sb;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const long long o = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += o;
+      }
+      incl += carry;
+      if (b < p.n_frames) {
+        const long long excl = incl - sb;
+        const int start = static_cast<int>(excl < p.total_tokens ? excl : p.total_tokens);
+        if (start <= tok) { best_b = b; best_start = start; }  // starts are non-decreasing in b
+        if (tok == 0) {
+          if (b == 0) p.cu[0] = 0;
+          p.cu[b + 1] = static_cast<int32_t>(incl < p.total_tokens ? incl : p.total_tokens);
+        }
+      }
+      carry = __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (carry != p.total_tokens) f |= FLAG_BAD_TOTAL;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const int ob = __shfl_xor_sync(0xffffffffu, best_b, off);
+      const int os = __shfl_xor_sync(0xffffffffu, best_start, off);
+      if (ob > best_b) { best_b = ob; best_start = os; }
+      f |= __shfl_xor_sync(0xffffffffu, f, off);
+    }
+    if (lane == 0) {
+      s_start = best_start;
+      if (tok == 0 && f) atomicOr(p.flag, f);
+    }
+  }
+  __syncthreads();
+  if (tok >= p.total_tokens) return;
+  const int n = tok - s_start;
   int pt, ph, pw;
   if (n < n_vis) {
     pt = 0; ph = n / p.grid_w; pw = n % p.grid_w;     // visual token: row-major grid, t = 0
   } else {
     pt = ph = pw = max(p.grid_h, p.grid_w) + (n - n_vis);  // text: continues from max grid id + 1
   }
-  if (lane == 0) {
+  if (threadIdx.x == 0) {
     p.pos[tok] = pt;
     p.pos[p.total_tokens + tok] = ph;
     p.pos[2 * p.total_tokens + tok] = pw;
   }
-  for (int i = lane; i < p.half_dim; i += 32) {
+  // the rotary table on the last warps, so that it overlaps the row copy of the first ones
+  for (int i = 255 - threadIdx.x; i < p.half_dim; i += 256) {
     const int pid = (i < p.sec_t) ? pt : ((i < p.sec_t + p.sec_h) ? ph : pw);
-    double s, c;
-    sincos(static_cast<double>(pid) * p.inv_freq[i], &s, &c);
-    p.cos_t[(size_t)tok * p.half_dim + i] = static_cast<float>(c);
-    p.sin_t[(size_t)tok * p.half_dim + i] = static_cast<float>(s);
+    double sn, cs;
+    sincos(static_cast<double>(pid) * p.inv_freq[i], &sn, &cs);
+    p.cos_t[(size_t)tok * p.half_dim + i] = static_cast<float>(cs);
+    p.sin_t[(size_t)tok * p.half_dim + i] = static_cast<float>(sn);
   }
   // residual copy + sum of squares + bf16(x * g)
   const float4* src = reinterpret_cast<const float4*>(p.embeds + (size_t)tok * p.d);
   float4* dst = reinterpret_cast<float4*>(p.out + (size_t)tok * p.d);
   float ss = 0.f;
-  for (int c4 = lane; c4 < p.d / 4; c4 += 32) {
+  for (int c4 = threadIdx.x; c4 < p.d / 4; c4 += 256) {
     const float4 v = __ldg(src + c4);
     dst[c4] = v;
     ss = fmaf(v.x, v.x, ss); ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
@@ -101,9 +125,14 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
-  if (lane == 0) {
-    p.ssq[tok] = ss;
-    for (int i = 1; i < p.ssq_parts; ++i) p.ssq[(size_t)i * p.ssq_stride + tok] = 0.f;
+  if (lane == 0) s_ss[warp] = ss;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float tot = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tot += s_ss[i];  // fixed order: deterministic
+    p.ssq[(size_t)tok * p.ssq_stride] = tot;
+    for (int i = 1; i < p.ssq_parts; ++i) p.ssq[(size_t)tok * p.ssq_stride + i] = 0.f;
   }
 }
 

@@ -14,6 +14,7 @@
 #include "te_attn.cuh"
 #include "te_attn_tc.cuh"
 #include "te_gemm.cuh"
+#include "te_gemm_splitk.cuh"
 #include "te_prep.cuh"
 
 namespace {
@@ -77,6 +78,9 @@ struct te_handle {
   int bn_qkv = 256, bn_gu = 256, bn_res = 128;
   int attn_impl = 1;  // 1: tcgen05 kernel (te_attn_tc.cuh) when Hq/Hkv is a power of two <= 8; 0: mma.sync kernel
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
+  int splitk = 1;     // 1: small batches (no CTA pairs) use the split-K kernel when a GEMM has <= one tile per SM
+  float* sk_scratch = nullptr;  // [sm_count][128 x 256] fp32 partial tiles
+  int* sk_sem = nullptr;        // [sm_count][2] per-tile arrival / departure counters (zero between launches)
   // weights
   bf16* w = nullptr;
   size_t w_elems = 0;
@@ -208,6 +212,33 @@ cudaError_t launch_gemm_bn(int bn, int pair, int dh, const CUtensorMap& a, const
   }
 }
 
+// split-K kernel: `p.splits` CTAs per 128 x bn tile (small batches; te_gemm_splitk.cuh)
+template <int BN, int EPI, int DH>
+cudaError_t launch_gemmk(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, cudaStream_t st) {
+  using Cfg = te::GemmKCfg<BN, EPI>;
+  const int tiles = p.num_m_blk * p.num_n_blk;
+  return launch_k(te::te_gemmk_kernel<BN, EPI, DH>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS), Cfg::SMEM_BYTES, st,
+                  tmA, tmB, p);
+}
+template <int EPI>
+cudaError_t launch_gemmk_bn(int bn, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p,
+                            cudaStream_t st) {
+  if constexpr (EPI == te::EPI_QKV) {
+    if (dh == 128) return launch_gemmk<128, EPI, 128>(a, b, p, st);
+    return launch_gemmk<128, EPI, 64>(a, b, p, st);
+  } else {
+    if (bn == 256) return launch_gemmk<256, EPI, 128>(a, b, p, st);
+    return launch_gemmk<128, EPI, 128>(a, b, p, st);
+  }
+}
+// CTAs per tile: fill the SMs, keep >= 2 k-blocks per CTA
+inline int choose_splits(int tiles, int num_kb, int sm_count) {
+  int s = sm_count / tiles;
+  if (s > te::GEMMK_MAX_SPLITS) s = te::GEMMK_MAX_SPLITS;
+  if (s > num_kb / 2) s = num_kb / 2;
+  return s < 1 ? 1 : s;
+}
+
 template <int DH, int GH>
 cudaError_t launch_attn(const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
   using Cfg = te::AttnCfg<DH, GH>;
@@ -233,6 +264,11 @@ cudaError_t set_gemm_attr() {
   cudaError_t e = cudaFuncSetAttribute(te::te_gemm_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        te::GemmCfg<BN>::SMEM_BYTES);
   if (e != cudaSuccess) return e;
+  if constexpr (EPI != te::EPI_QKV || BN == 128) {
+    e = cudaFuncSetAttribute(te::te_gemmk_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             te::GemmKCfg<BN, EPI>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+  }
   return cudaFuncSetAttribute(te::te_gemm2_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               te::Gemm2Cfg<BN, EPI>::SMEM_BYTES);
 }
@@ -278,11 +314,22 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
   // one CTA per tile so that more SMs stream weights (HBM-bound regime).
   const int pair = h->pair_mode == 2 ? (T >= 1024 ? 1 : 0) : h->pair_mode;
-  const int bx_qkv = box_index(pair ? h->bn_qkv / 2 : h->bn_qkv);
-  const int bx_gu = box_index(pair ? h->bn_gu / 2 : h->bn_gu);
+  // Small batches: when a GEMM has at most one 128-row tile per SM it runs on the split-K kernel, with
+  // as many CTAs per tile as the SM count allows (QKV then uses one-head-wide 128-column tiles).
+  const int num_m = (T + te::GEMM_BM - 1) / te::GEMM_BM;
+  const bool kmode = !pair && h->splitk;
+  const int bn_qkv = (kmode && num_m * (n_qkv / 128) <= h->sm_count) ? 128 : h->bn_qkv;
+  const bool k_qkv = kmode && num_m * (n_qkv / bn_qkv) <= h->sm_count;
+  const bool k_gu = kmode && num_m * (2 * F / h->bn_gu) <= h->sm_count;
+  const bool k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;
+  const int bx_qkv = box_index(pair ? bn_qkv / 2 : bn_qkv);
+  // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
+  // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
+  const bool pair_gu = pair || (kmode && !k_gu && T > te::GEMM_BM && h->pair_mode == 2);
+  const int bx_gu = box_index(pair_gu ? h->bn_gu / 2 : h->bn_gu);
   const int bx_res = box_index(pair ? h->bn_res / 2 : h->bn_res);
   // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
-  const int parts = (d / h->bn_res) * (pair ? te::GEMM2_EPI_WARPS / 4 : 1);
+  const int parts = (d / h->bn_res) * ((pair || k_res) ? 2 : 1);
   int nk = 0;
   // Optional per-kernel CUDA-event bracketing (TE_OPT_KERNEL_TIMING; never inside a capture).
   cudaEvent_t ev_a = nullptr;
@@ -299,20 +346,17 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     h->timed.push_back({kclass, ev_a, ev_b});
   };
 
-  tick();
   g_pdl = h->pdl && !h->timing;
-  TE_CUDA(h, launch_k(te::te_scan_kernel, dim3(1), dim3(32), 0, st, lens, n_frames, grid_h * grid_w, T,
-                      c.max_tokens_per_frame, h->cu, h->flag));
-  tock(TE_KCLASS_SCAN);
-  ++nk;
   {
     te::PrepParams pp{};
-    pp.embeds = embeds; pp.out = out; pp.cu = h->cu; pp.pos = h->pos; pp.cos_t = h->cos_t; pp.sin_t = h->sin_t;
+    pp.embeds = embeds; pp.text_lens = lens; pp.out = out; pp.cu = h->cu; pp.flag = h->flag; pp.pos = h->pos;
+    pp.cos_t = h->cos_t; pp.sin_t = h->sin_t;
     pp.inv_freq = h->inv_freq; pp.g_first = h->w + h->off[lb].g1; pp.xg = h->xg; pp.ssq = h->ssq;
-    pp.ssq_parts = parts; pp.ssq_stride = c.max_tokens; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
-    pp.half_dim = dh / 2; pp.grid_h = grid_h; pp.grid_w = grid_w; pp.sec_t = c.rope_sec_t; pp.sec_h = c.rope_sec_h;
+    pp.ssq_parts = parts; pp.ssq_stride = h->ssq_parts_cap; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
+    pp.half_dim = dh / 2; pp.max_tokens_per_frame = c.max_tokens_per_frame;
+    pp.grid_h = grid_h; pp.grid_w = grid_w; pp.sec_t = c.rope_sec_t; pp.sec_h = c.rope_sec_h;
     tick();
-    TE_CUDA(h, launch_k(te::te_prep_kernel, dim3((T + 7) / 8), dim3(256), 0, st, pp));
+    TE_CUDA(h, launch_k(te::te_prep_kernel, dim3(T), dim3(256), 0, st, pp));
     tock(TE_KCLASS_PREP);
     ++nk;
   }
@@ -322,9 +366,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     h->err = "cuTensorMapEncodeTiled failed for an activation map";
     return TE_ERR_CUDA;
   }
-  const int num_m = (T + te::GEMM_BM - 1) / te::GEMM_BM;
   te::GemmParams base{};
-  base.M = T; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = parts; base.ssq_stride = c.max_tokens;
+  base.splits = 1; base.sk_scratch = h->sk_scratch; base.sk_sem = h->sk_sem;
+  base.M = T; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = parts; base.ssq_stride = h->ssq_parts_cap;
   base.inv_d = 1.0f / static_cast<float>(d); base.eps = c.rms_eps;
   const size_t trace_stride = (size_t)h->sm_count * te::TRACE_SLOTS;
   auto trace_ptr = [&](int cls) { return h->trace_on ? h->trace + cls * trace_stride : nullptr; };
@@ -357,12 +401,17 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     const LayerOff& o = h->off[l];
     {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
       te::GemmParams p = base;
-      p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / h->bn_qkv;
+      p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / bn_qkv;
       p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
       p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
       p.trace = trace_ptr(0);
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(h->bn_qkv, pair, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
+      if (k_qkv) {
+        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_QKV>(bn_qkv, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, st));
+      } else {
+        TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(bn_qkv, pair, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
+      }
       tock(TE_KCLASS_QKV);
       ++nk;
     }
@@ -390,7 +439,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
       p.trace = trace_ptr(1);
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_attn, h->tm[l].o[bx_res], p, h->sm_count, st));
+      if (k_res) {
+        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm[l].o[bx_res], p, st));
+      } else {
+        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_attn, h->tm[l].o[bx_res], p, h->sm_count, st));
+      }
       tock(TE_KCLASS_OPROJ);
       ++nk;
     }
@@ -401,7 +455,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.act = h->act; p.ld_act = F;
       p.trace = trace_ptr(2);
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, pair, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
+      if (k_gu) {
+        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(h->bn_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, st));
+      } else {
+        TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, pair_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
+      }
       tock(TE_KCLASS_GATEUP);
       ++nk;
     }
@@ -412,7 +471,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
       p.trace = trace_ptr(3);
       tick();
-      TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_act, h->tm[l].d[bx_res], p, h->sm_count, st));
+      if (k_res) {
+        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm[l].d[bx_res], p, st));
+      } else {
+        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_act, h->tm[l].d[bx_res], p, h->sm_count, st));
+      }
       tock(TE_KCLASS_DOWN);
       ++nk;
     }
@@ -470,7 +534,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   h->bn_qkv = (n_qkv % 256 == 0) ? 256 : 128;
   h->bn_gu = ((2 * c.ffn) % 256 == 0) ? 256 : 128;
   h->bn_res = 128;  // O/down: N = hidden is small -> 128-wide tiles halve the wave-quantisation loss
-  h->ssq_parts_cap = (c.hidden / 128) * (te::GEMM2_EPI_WARPS / 4);
+  h->ssq_parts_cap = ((c.hidden / 128) * (te::GEMM2_EPI_WARPS / 4) + 3) & ~3;  // row stride of ssq (16-byte aligned rows)
 
   auto fail = [&](int code) {
     te_destroy(h);
@@ -490,7 +554,10 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   TE_ALLOC(h->qkv, T * n_qkv * sizeof(bf16));
   TE_ALLOC(h->attn, T * (size_t)c.n_q_heads * c.head_dim * sizeof(bf16));
   TE_ALLOC(h->act, T * c.ffn * sizeof(bf16));
+  TE_ALLOC(h->sk_scratch, (size_t)h->sm_count * te::GEMM_BM * 256 * sizeof(float));
+  TE_ALLOC(h->sk_sem, 2 * (size_t)h->sm_count * sizeof(int));
 #undef TE_ALLOC
+  if (cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess) return fail(TE_ERR_CUDA);
   if (cudaMemset(h->flag, 0, sizeof(int32_t)) != cudaSuccess) return fail(TE_ERR_CUDA);
   std::vector<double> invf(hd2);
   for (size_t i = 0; i < hd2; ++i) invf[i] = std::pow(c.rope_theta, -2.0 * (double)i / (double)c.head_dim);
@@ -718,6 +785,11 @@ int te_set_option(te_handle* h, int option, int value) {
     free_graphs(h);
     return TE_OK;
   }
+  if (option == TE_OPT_SPLIT_K) {
+    h->splitk = value ? 1 : 0;
+    free_graphs(h);
+    return TE_OK;
+  }
   if (option == TE_OPT_RESID_BLOCK_N) {
     if ((value != 128 && value != 256) || h->cfg.hidden % value != 0) return TE_ERR_INVALID_ARG;
     h->bn_res = value;
@@ -805,6 +877,40 @@ int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t
   return cudaDeviceSynchronize() == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
+int te_debug_gemm_splitk(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                         int32_t block_n, int32_t splits) {
+  if (!a || !b || !cmat || m < 1 || n < 1 || k < 1) return TE_ERR_INVALID_ARG;
+  if ((block_n != 128 && block_n != 256) || n % block_n != 0 || k % 64 != 0) return TE_ERR_UNSUPPORTED;
+  if (splits < 1 || splits > te::GEMMK_MAX_SPLITS || splits > k / 64) return TE_ERR_INVALID_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TE_ERR_CUDA;
+  if (prop.major != 10) return TE_ERR_UNSUPPORTED;
+  if (init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
+  CUtensorMap ta, tb;
+  if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, block_n)) return TE_ERR_CUDA;
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
+  p.c = cmat; p.ld_c = n; p.splits = splits;
+  const size_t tiles = (size_t)p.num_m_blk * p.num_n_blk;
+  // the group leader spins on its peers: the whole grid must be co-resident (one CTA per SM)
+  if (tiles * splits > (size_t)prop.multiProcessorCount) return TE_ERR_UNSUPPORTED;
+  if (cudaMalloc(reinterpret_cast<void**>(&p.sk_scratch), tiles * splits * te::GEMM_BM * block_n * sizeof(float)) !=
+      cudaSuccess)
+    return TE_ERR_CUDA;
+  if (cudaMalloc(reinterpret_cast<void**>(&p.sk_sem), 2 * tiles * sizeof(int)) != cudaSuccess) {
+    cudaFree(p.sk_scratch);
+    return TE_ERR_CUDA;
+  }
+  cudaMemset(p.sk_sem, 0, 2 * tiles * sizeof(int));
+  g_pdl = false;
+  cudaError_t e = launch_gemmk_bn<te::EPI_PLAIN>(block_n, 128, ta, tb, p, nullptr);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  cudaFree(p.sk_scratch);
+  cudaFree(p.sk_sem);
+  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+}
+
 void te_destroy(te_handle* h) {
   if (!h) return;
   cudaSetDevice(h->device);
@@ -812,7 +918,7 @@ void te_destroy(te_handle* h) {
   free_graphs(h);
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
-                  h->act, h->stg_embeds, h->stg_out, h->stg_lens, h->trace};
+                  h->act, h->stg_embeds, h->stg_out, h->stg_lens, h->trace, h->sk_scratch, h->sk_sem};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);

@@ -22,7 +22,8 @@ def cached_blob(model, seed, gains="randn"):
 class GpuTE:
     """Owns one handle; encode() returns numpy arrays."""
 
-    def __init__(self, model, max_frames, max_tokens, blob, final_norm=None, cta_pair=None, resid_bn=None):
+    def __init__(self, model, max_frames, max_tokens, blob, final_norm=None, cta_pair=None, resid_bn=None,
+                 split_k=None):
         import torch
         import paper_2606_05981_b200 as te
         self.te, self.torch, self.model = te, torch, model
@@ -32,6 +33,8 @@ class GpuTE:
             te.te_set_option(self.enc.h, te.TE_OPT_CTA_PAIR, cta_pair)
         if resid_bn is not None:
             te.te_set_option(self.enc.h, te.TE_OPT_RESID_BLOCK_N, resid_bn)
+        if split_k is not None:
+            te.te_set_option(self.enc.h, te.TE_OPT_SPLIT_K, split_k)
 
     def encode(self, embeds, text_lens, gh, gw, layer_range=None, stop_after_attn=0, stream=None,
                total_tokens=None, use_graph=1):

@@ -54,6 +54,33 @@ def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn, pair):
     assert np.max(np.abs(out - ref)) < 1e-4 * np.sqrt(K) * 4
 
 
+@pytest.mark.parametrize("M,N,K,bn,splits", [(128, 256, 128, 256, 2), (1, 128, 128, 128, 2), (80, 512, 256, 128, 2),
+                                              (300, 512, 832, 128, 4), (128, 768, 832, 256, 3),
+                                              (128, 2048, 2048, 128, 8), (128, 2048, 6144, 128, 8),
+                                              (512, 2048, 6144, 128, 2), (128, 4096, 2048, 128, 4),
+                                              (128, 12288, 2048, 256, 3), (512, 4096, 2048, 128, 1)])
+def test_gemm_splitk_vs_fp64_matmul(H, M, N, K, bn, splits):
+    """Split-K kernel: `splits` CTAs per tile (uneven K-slices included), partial tiles through the L2
+    scratch, fixed-order sum -> same result as one fp64 matmul, and bitwise repeatable."""
+    import torch
+    import paper_2606_05981_b200 as te
+    rng = np.random.default_rng(M * 11 + N + splits)
+    a = W.f32_to_bf16_bits(rng.standard_normal((M, K)).astype(np.float32))
+    b = W.f32_to_bf16_bits(rng.standard_normal((N, K)).astype(np.float32))
+    ref = H.bf16_bits_to_f64(a).reshape(M, K) @ H.bf16_bits_to_f64(b).reshape(N, K).T
+    ad = torch.from_numpy(a.view(np.int16)).cuda()
+    bd = torch.from_numpy(b.view(np.int16)).cuda()
+    outs = []
+    for _ in range(2):
+        c = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
+        te.te_debug_gemm_splitk(0, ad, bd, c, M, N, K, bn, splits)
+        outs.append(c.cpu().numpy())
+    assert np.isfinite(outs[0]).all()
+    assert PM.rel_l2(outs[0], ref) < 1e-5
+    assert np.max(np.abs(outs[0] - ref)) < 1e-4 * np.sqrt(K) * 4
+    assert np.array_equal(outs[0], outs[1])
+
+
 # ------------------------------------------------------------------- ids / packing / rotary table
 @pytest.mark.parametrize("gh,gw,tl", [(4, 4, [24, 24]), (8, 8, [64]), (4, 16, [3, 0, 17]), (16, 4, [0, 9]),
                                       (1, 5, [1, 2, 3, 4, 5, 6, 7])])
@@ -113,13 +140,16 @@ def test_cfg1_full_stack(H, O):
     g.close()
 
 
-@pytest.mark.parametrize("cta_pair,resid_bn", [(1, 128), (1, 256), (0, 256), (0, 128)])
-def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn):
-    """Force each GEMM tiling (one CTA per tile / CTA pairs, 128- and 256-wide residual tiles)."""
+@pytest.mark.parametrize("cta_pair,resid_bn,split_k", [(1, 128, 1), (1, 256, 1), (0, 256, 1), (0, 128, 1),
+                                                       (0, 256, 0), (0, 128, 0)])
+def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn, split_k):
+    """Force each GEMM tiling (one CTA per tile / CTA pairs / split-K groups, 128- and 256-wide residual
+    tiles)."""
     w, blob, tl, T, emb, ch = H.workload_inputs(1)
     ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4)
-    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn)
-    _assert_final(PM.stack_metrics(g.encode(emb, tl, 4, 4), ref, emb), f"pair={cta_pair} bn={resid_bn}")
+    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn, split_k=split_k)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, 4, 4), ref, emb),
+                  f"pair={cta_pair} bn={resid_bn} split_k={split_k}")
     g.close()
 
 
@@ -314,7 +344,7 @@ def test_encode_is_async_no_sync_and_counts_launches(H):
         done_at_return = st.query()
     st.synchronize()
     assert not done_at_return
-    assert te.te_kernel_launches(g.enc.h) - n0 == 2 + 5 * w.model.n_layers
+    assert te.te_kernel_launches(g.enc.h) - n0 == 1 + 5 * w.model.n_layers
     g.close()
 
 
