@@ -299,9 +299,14 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
   float* bufA = stg;
   float* bufB = stg + 32 * 32;
   constexpr int HEADS = BN / DH;
-  // heads of the tile are split between the warps of a quadrant; a single head is not split
-  const int hh_begin = (HEADS % nparts == 0) ? part * (HEADS / nparts) : (part == 0 ? 0 : HEADS);
-  const int hh_end = (HEADS % nparts == 0) ? (part + 1) * (HEADS / nparts) : HEADS;
+  // heads of the tile are split between the warps of a quadrant; when they do not divide evenly (one head
+  // per tile, two warps) every warp takes every head but only its share of the 32-column chunks: the
+  // head's sum of squares (pass 1, TMEM reads only) is then computed redundantly
+  const bool split_heads = HEADS % nparts == 0;
+  const int hh_begin = split_heads ? part * (HEADS / nparts) : 0;
+  const int hh_end = split_heads ? (part + 1) * (HEADS / nparts) : HEADS;
+  const int c_first = split_heads ? 0 : part * 32;
+  const int c_step = split_heads ? 32 : nparts * 32;
 #pragma unroll 1
   for (int hh = hh_begin; hh < hh_end; ++hh) {
     const int col0 = n_blk * BN + hh * DH;  // first column of this head in the fused qkv row
@@ -309,7 +314,7 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
     if (col0 >= p.k_cols_end) {
       // ---- v head: scale and store
 #pragma unroll 1
-      for (int c0 = 0; c0 < DH; c0 += 32) {
+      for (int c0 = c_first; c0 < DH; c0 += c_step) {
         float v[32];
         {
           uint32_t r[32];
@@ -348,7 +353,7 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
     // lane) so that their L2 round trips overlap the TMEM reads and the staging instead of
     // serialising behind each other.
 #pragma unroll 1
-    for (int c0 = 0; c0 < HD2; c0 += 32) {
+    for (int c0 = c_first; c0 < HD2; c0 += c_step) {
       const int cc = c0 + cq * 4;  // this lane's 4 columns inside the half
       float4 cs[8], sn[8];
 #pragma unroll

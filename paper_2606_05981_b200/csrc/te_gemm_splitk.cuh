@@ -67,12 +67,76 @@ __device__ __forceinline__ void red_release_gpu_add(int* p, int v) {
 // block v (NV = BN/128 blocks).  The S fp32 partials of the row are summed in the order 0..S-1; the
 // arithmetic that follows restates the epilogues of te_gemm.cuh in this domain (per-head reductions and
 // the rotary partner are warp shuffles).
-// One batch of RB rows (r0, r0 + dr, ...): every global load of the batch — the S partials of each row
-// and the epilogue operands (x, cos/sin, statistics) — is issued before the first use, so a batch costs
-// about one L2 round trip instead of several per row.  S * NV <= CAP float4 per row are in flight.
+// Epilogue operands of one batch of RB rows that do not depend on the accumulators (x, cos/sin, RMSNorm
+// statistics, gains).  The first batch's are fetched BEFORE the CTA waits for its main loop and its group.
+template <int NV, int RB>
+struct SliceAux {
+  float4 xv[RB][NV];
+  float4 cs[RB], sn[RB];
+  float rstd[RB];
+  uint2 gn[NV];  // next norm's gain (EPI_RESID) / this head's QK-norm gain (EPI_QKV)
+};
+template <int BN, int EPI, int DH, int RB>
+__device__ __forceinline__ void slice_aux_load(const GemmParams& p, SliceAux<BN / 128, RB>& ax, int r0, int dr, int lane,
+                                               int m_blk, int n_blk) {
+  constexpr int NV = BN / 128;
+  constexpr int HD2 = DH / 2;
+  [[maybe_unused]] const int ch = (4 * lane) % DH;                      // lane's first column inside its head
+  [[maybe_unused]] const int col0 = n_blk * BN + (4 * lane / DH) * DH;  // first column of the lane's head
+  if constexpr (EPI == EPI_RESID) {
+    if (p.g_next != nullptr) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v)
+        ax.gn[v] = __ldg(reinterpret_cast<const uint2*>(p.g_next + n_blk * BN + v * 128 + 4 * lane));
+    }
+  }
+  if constexpr (EPI == EPI_QKV) ax.gn[0] = __ldg(reinterpret_cast<const uint2*>(((col0 < p.q_cols_end) ? p.gq : p.gk) + ch));
+#pragma unroll
+  for (int b = 0; b < RB; ++b) {
+    const int r = r0 + b * dr;
+    const int row = m_blk * GEMM_BM + r;
+    const bool ok = r < GEMM_BM && row < p.M;
+    if constexpr (EPI == EPI_RESID) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v)
+        if (ok) ax.xv[b][v] = *(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + n_blk * BN + v * 128) + lane);
+    }
+    if constexpr (EPI == EPI_QKV) {
+      if (ok) {
+        ax.cs[b] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + (ch % HD2)));
+        ax.sn[b] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + (ch % HD2)));
+      }
+    }
+    if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) {
+      // a row's parts are contiguous: lane i takes part i (branch-free for the usual <= 64 parts so that
+      // the loads of all batch rows issue back to back)
+      float sq = 0.f;
+      if (ok) {
+        const float* q = p.ssq_in + (size_t)row * p.ssq_stride;
+        sq = (lane < p.ssq_parts) ? q[lane] : 0.f;
+        sq += (lane + 32 < p.ssq_parts) ? q[lane + 32] : 0.f;
+        for (int i = lane + 64; i < p.ssq_parts; i += 32) sq += q[i];
+      }
+      ax.rstd[b] = sq;
+    }
+  }
+  // RMSNorm scale: lanes hold the parts round-robin -> fixed xor tree (deterministic)
+  if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) {
+#pragma unroll
+    for (int b = 0; b < RB; ++b) {
+      float sq = ax.rstd[b];
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) sq += __shfl_xor_sync(0xffffffffu, sq, off);
+      ax.rstd[b] = 1.0f / sqrtf(sq * p.inv_d + p.eps);
+    }
+  }
+}
+
+// One batch of RB rows (r0, r0 + dr, ...): the S partials of every row of the batch are requested before
+// the first use, so a batch costs about one L2 round trip.  S * NV <= CAP float4 per row are in flight.
 template <int BN, int EPI, int DH, int RB, int CAP>
 __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* scratch, int S, int r0, int dr, int lane,
-                                            int m_blk, int n_blk) {
+                                            int m_blk, int n_blk, const SliceAux<BN / 128, RB>& ax) {
   constexpr int NV = BN / 128;
   constexpr int HD2 = DH / 2;
   constexpr int HL = DH / 4;  // lanes per head
@@ -92,55 +156,8 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
         pv[b][q] = __ldcg(reinterpret_cast<const float4*>(scratch + (size_t)(q / NV) * TILE_F + (size_t)r * BN +
                                                           (q % NV) * 128) + lane);
   }
-  // ---- epilogue operands
-  [[maybe_unused]] float4 xv[RB][NV];
-  [[maybe_unused]] float4 cs[RB], sn[RB];
-  [[maybe_unused]] float rstd[RB];  // first the lane's share of the row's sum-of-squares parts, then 1/rms
-  [[maybe_unused]] uint2 gn[NV];    // next norm's gain (EPI_RESID) / this head's QK-norm gain (EPI_QKV)
-  [[maybe_unused]] const int ch = (4 * lane) % DH;                      // lane's first column inside its head
-  [[maybe_unused]] const int col0 = n_blk * BN + (4 * lane / DH) * DH;  // first column of the lane's head
-  if constexpr (EPI == EPI_RESID) {
-    if (p.g_next != nullptr) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) gn[v] = __ldg(reinterpret_cast<const uint2*>(p.g_next + n_blk * BN + v * 128 + 4 * lane));
-    }
-  }
-  if constexpr (EPI == EPI_QKV) gn[0] = __ldg(reinterpret_cast<const uint2*>(((col0 < p.q_cols_end) ? p.gq : p.gk) + ch));
-#pragma unroll
-  for (int b = 0; b < RB; ++b) {
-    if (!ok[b]) continue;
-    if constexpr (EPI == EPI_RESID) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v)
-        xv[b][v] = *(reinterpret_cast<const float4*>(p.x + (size_t)row[b] * p.ld_x + n_blk * BN + v * 128) + lane);
-    }
-    if constexpr (EPI == EPI_QKV) {
-      cs[b] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row[b] * HD2 + (ch % HD2)));
-      sn[b] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row[b] * HD2 + (ch % HD2)));
-    }
-    if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) {
-      // a row's parts are contiguous: lane i takes part i (branch-free for the usual <= 64 parts so that
-      // the loads of all batch rows issue back to back)
-      const float* q = p.ssq_in + (size_t)row[b] * p.ssq_stride;
-      float sq = (lane < p.ssq_parts) ? q[lane] : 0.f;
-      sq += (lane + 32 < p.ssq_parts) ? q[lane + 32] : 0.f;
-      for (int i = lane + 64; i < p.ssq_parts; i += 32) sq += q[i];
-      rstd[b] = sq;
-    }
-  }
-  // RMSNorm scale: lanes hold the parts round-robin -> fixed xor tree (deterministic)
-  if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) {
-#pragma unroll
-    for (int b = 0; b < RB; ++b) {
-      float sq = ok[b] ? rstd[b] : 0.f;
-#pragma unroll
-      for (int off = 1; off < 32; off <<= 1) sq += __shfl_xor_sync(0xffffffffu, sq, off);
-      rstd[b] = 1.0f / sqrtf(sq * p.inv_d + p.eps);
-    }
-  }
-#ifdef TE_DBG_SLICE
-  if (threadIdx.x == 64 && r0 < dr) trace_stamp(p, 11);
-#endif
+  [[maybe_unused]] const int ch = (4 * lane) % DH;
+  [[maybe_unused]] const int col0 = n_blk * BN + (4 * lane / DH) * DH;
   // ---- reduce (fixed order 0..S-1) + fused epilogue, row by row
 #pragma unroll
   for (int b = 0; b < RB; ++b) {
@@ -154,9 +171,6 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
         float4& a = acc[q % NV];
         a.x += pv[b][q].x; a.y += pv[b][q].y; a.z += pv[b][q].z; a.w += pv[b][q].w;
       }
-#ifdef TE_DBG_SLICE
-    if (threadIdx.x == 64 && r0 < dr && b == 0 && acc[0].x != 123.456f) trace_stamp(p, 12);
-#endif
     if constexpr (EPI == EPI_PLAIN) {
 #pragma unroll
       for (int v = 0; v < NV; ++v)
@@ -167,12 +181,12 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
 #pragma unroll
       for (int v = 0; v < NV; ++v) {
         const int col = n_blk * BN + v * 128 + 4 * lane;
-        float4 x = xv[b][v];
+        float4 x = ax.xv[b][v];
         x.x += acc[v].x; x.y += acc[v].y; x.z += acc[v].z; x.w += acc[v].w;
         *reinterpret_cast<float4*>(p.x + (size_t)row[b] * p.ld_x + col) = x;
         ss = fmaf(x.x, x.x, ss); ss = fmaf(x.y, x.y, ss); ss = fmaf(x.z, x.z, ss); ss = fmaf(x.w, x.w, ss);
         if (p.g_next != nullptr) {
-          const uint2 g = gn[v];
+          const uint2 g = ax.gn[v];
           uint2 o;
           o.x = pack_bf16(x.x * bf16_lo(g.x), x.y * bf16_hi(g.x));
           o.y = pack_bf16(x.z * bf16_lo(g.y), x.w * bf16_hi(g.y));
@@ -197,8 +211,8 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
         u.x = __shfl_down_sync(0xffffffffu, acc[0].x, 16); u.y = __shfl_down_sync(0xffffffffu, acc[0].y, 16);
         u.z = __shfl_down_sync(0xffffffffu, acc[0].z, 16); u.w = __shfl_down_sync(0xffffffffu, acc[0].w, 16);
       }
-      const float gv[4] = {g.x * rstd[b], g.y * rstd[b], g.z * rstd[b], g.w * rstd[b]};
-      const float uv[4] = {u.x * rstd[b], u.y * rstd[b], u.z * rstd[b], u.w * rstd[b]};
+      const float gv[4] = {g.x * ax.rstd[b], g.y * ax.rstd[b], g.z * ax.rstd[b], g.w * ax.rstd[b]};
+      const float uv[4] = {u.x * ax.rstd[b], u.y * ax.rstd[b], u.z * ax.rstd[b], u.w * ax.rstd[b]};
       float a[4];
 #pragma unroll
       for (int e = 0; e < 4; ++e) a[e] = __fdividef(gv[e], 1.0f + __expf(-gv[e])) * uv[e];
@@ -214,24 +228,24 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
       float ss = 0.f;
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
-        const float y = a4[e] * rstd[b];
+        const float y = a4[e] * ax.rstd[b];
         ss = fmaf(y, y, ss);
       }
 #pragma unroll
       for (int off = 1; off < HL; off <<= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
-      const float sc = rstd[b] / sqrtf(ss * (1.0f / DH) + p.eps);
+      const float sc = ax.rstd[b] / sqrtf(ss * (1.0f / DH) + p.eps);
       const bool is_v = col0 >= p.k_cols_end;
-      const uint2 g = gn[0];
+      const uint2 g = ax.gn[0];
       const float gg[4] = {bf16_lo(g.x), bf16_hi(g.x), bf16_lo(g.y), bf16_hi(g.y)};
-      const float c4[4] = {cs[b].x, cs[b].y, cs[b].z, cs[b].w};
-      const float s4[4] = {sn[b].x, sn[b].y, sn[b].z, sn[b].w};
+      const float c4[4] = {ax.cs[b].x, ax.cs[b].y, ax.cs[b].z, ax.cs[b].w};
+      const float s4[4] = {ax.sn[b].x, ax.sn[b].y, ax.sn[b].z, ax.sn[b].w};
       float out[4];
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const float w = a4[e] * sc * gg[e];
         const float partner = __shfl_xor_sync(0xffffffffu, w, HL / 2);
         const float rot = (ch < HD2) ? (w * c4[e] - partner * s4[e]) : (w * c4[e] + partner * s4[e]);
-        out[e] = is_v ? a4[e] * rstd[b] : rot;
+        out[e] = is_v ? a4[e] * ax.rstd[b] : rot;
       }
       uint2 o;
       o.x = pack_bf16(out[0], out[1]);
@@ -241,27 +255,65 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
   }
 }
 
-// CTA s of a group finishes rows r = s (mod S); its warp ew takes every 8th of them (16/S rows).  The batch
-// size is chosen so that all partials of a batch (RB rows x S*NV float4) fit in ~16-18 float4 per lane: for
-// 128-wide tiles a warp's rows are then a single batch.
-template <int BN, int EPI, int DH>
-__device__ __forceinline__ void slice_rows(const GemmParams& p, const float* scratch, int S, int s, int ew, int lane,
-                                           int m_blk, int n_blk) {
+// Epilogue of a split-K group member, for one batch shape (RB rows per batch, CAP partial float4 per row).
+// CTA s of the group finishes rows r = s (mod S) of the tile; its warp ew takes every 8th of them (16/S rows).
+//   (0) prefetch the first batch's accumulator-independent operands
+//   (1) wait for the own main loop, store the fp32 partial tile row-major to the L2 scratch
+//   (2) meet the group at the tile's arrival counter
+//   (3) batches: sum the S partials of each row in the fixed order 0..S-1, fused epilogue
+template <int BN, int EPI, int DH, int RB, int CAP>
+__device__ __forceinline__ void group_finish(const GemmParams& p, uint64_t* tfull, uint32_t t_row, float* stg, float* scratch,
+                                             int S, int s, int tile, int warp, int lane, int m_blk, int n_blk) {
   constexpr int NV = BN / 128;
+  constexpr int NPARTS = GEMMK_EPI_WARPS / 4;
+  constexpr int COLS = BN / NPARTS;
+  constexpr size_t TILE_F = (size_t)GEMM_BM * BN;
+  const int ew = warp - 2, quad = warp & 3, part = ew >> 2;
   const int dr = GEMMK_EPI_WARPS * S;  // row stride between a warp's consecutive rows
   const int r_first = s + ew * S;
-  const int snv = S * NV;
-#define TE_SLICE_LOOP(RB, CAP)                                          \
-  _Pragma("unroll 1") for (int r0 = r_first; r0 < GEMM_BM; r0 += RB * dr) \
-      slice_batch<BN, EPI, DH, RB, CAP>(p, scratch, S, r0, dr, lane, m_blk, n_blk)
-  // (EPI_QKV also keeps a cos/sin row per batch row in registers: at most 4 rows per batch there)
-  if (EPI != EPI_QKV && snv <= 2) { TE_SLICE_LOOP(8, 2); }
-  else if (EPI != EPI_QKV && snv <= 3) { TE_SLICE_LOOP(6, 3); }
-  else if (snv <= 4) { TE_SLICE_LOOP(4, 4); }
-  else if (snv <= 6) { TE_SLICE_LOOP(3, 6); }
-  else if (snv <= 8) { TE_SLICE_LOOP(2, 8); }
-  else { TE_SLICE_LOOP(1, 16); }
-#undef TE_SLICE_LOOP
+  const bool tr = warp == 2 && lane == 0;
+  SliceAux<NV, RB> ax;
+  slice_aux_load<BN, EPI, DH, RB>(p, ax, r_first, dr, lane, m_blk, n_blk);
+  mbar_wait(tfull, 0);
+  tc_fence_after();
+  if (tr) trace_stamp(p, 5);
+  {
+    float* dst = scratch + (size_t)s * TILE_F + (size_t)(quad * 32) * BN;
+    const int sub = lane >> 3, cq = lane & 7;
+#pragma unroll 1
+    for (int c0 = part * COLS; c0 < (part + 1) * COLS; c0 += 32) {
+      uint32_t r[32];
+      tmem_ld32(t_row + c0, r);
+      tmem_ld_wait();
+      float v[32];
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+      stg_put_row(stg, lane, v);
+      __syncwarp();
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int rr = sub + 4 * i;
+        __stcg(reinterpret_cast<float4*>(dst + (size_t)rr * BN + c0 + cq * 4), stg_get(stg, rr, cq));
+      }
+      __syncwarp();
+    }
+  }
+  // bar.sync orders the warps' scratch stores before the elected thread's gpu-scope release
+  epi_bar_sync();
+  if (warp == 2 && lane == 0) {
+    red_release_gpu_add(p.sk_sem + 2 * tile, 1);
+    while (ld_acquire_gpu(p.sk_sem + 2 * tile) < S) {
+    }
+  }
+  epi_bar_sync();
+  if (tr) trace_stamp(p, 7);
+  slice_batch<BN, EPI, DH, RB, CAP>(p, scratch, S, r_first, dr, lane, m_blk, n_blk, ax);
+#pragma unroll 1
+  for (int r0 = r_first + RB * dr; r0 < GEMM_BM; r0 += RB * dr) {
+    slice_aux_load<BN, EPI, DH, RB>(p, ax, r0, dr, lane, m_blk, n_blk);
+    slice_batch<BN, EPI, DH, RB, CAP>(p, scratch, S, r0, dr, lane, m_blk, n_blk, ax);
+  }
+  if (tr) trace_stamp(p, 9);
 }
 
 // Scratch layout: [tile][split][128 rows][BN] fp32, row-major (written coalesced through the staging
@@ -388,47 +440,21 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
       if (tr) trace_stamp(p, 9);
     } else {
-      // ---- split-K group: (1) every CTA stores its fp32 partial tile row-major to the L2 scratch,
-      // (2) the group meets at the tile's arrival counter, (3) CTA s reduces and finishes the rows
-      // r = s (mod S) of the tile: sum over the S partials in the fixed order 0..S-1, then the fused
-      // epilogue in the lane-per-column domain (a warp holds one whole row of the tile).
-      mbar_wait(tfull, 0);
-      tc_fence_after();
-      if (tr) trace_stamp(p, 5);
-      constexpr size_t TILE_F = (size_t)GEMM_BM * BN;
-      float* scratch = p.sk_scratch + (size_t)tile * S * TILE_F;
-      {
-        float* dst = scratch + (size_t)s * TILE_F + (size_t)(quad * 32) * BN;
-        const int sub = lane >> 3, cq = lane & 7;
-#pragma unroll 1
-        for (int c0 = part * COLS; c0 < (part + 1) * COLS; c0 += 32) {
-          uint32_t r[32];
-          tmem_ld32(t_row + c0, r);
-          tmem_ld_wait();
-          float v[32];
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
-          stg_put_row(stg, lane, v);
-          __syncwarp();
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const int rr = sub + 4 * i;
-            __stcg(reinterpret_cast<float4*>(dst + (size_t)rr * BN + c0 + cq * 4), stg_get(stg, rr, cq));
-          }
-          __syncwarp();
-        }
-      }
-      // bar.sync orders the warps' scratch stores before the elected thread's gpu-scope release
-      epi_bar_sync();
-      if (warp == 2 && lane == 0) {
-        red_release_gpu_add(p.sk_sem + 2 * tile, 1);
-        while (ld_acquire_gpu(p.sk_sem + 2 * tile) < S) {
-        }
-      }
-      epi_bar_sync();
-      if (tr) trace_stamp(p, 7);
-      slice_rows<BN, EPI, DH>(p, scratch, S, s, warp - 2, lane, m_blk, n_blk);
-      if (tr) trace_stamp(p, 9);
+      // ---- split-K group (see group_finish).  The batch shape is chosen so that all partials of a batch
+      // (RB rows x S*NV float4) fit in ~16-18 float4 per lane: for 128-wide tiles a warp's 16/S rows are a
+      // single batch.  (EPI_QKV also keeps a cos/sin row per batch row: at most 4 rows per batch there.)
+      constexpr int NV = BN / 128;
+      float* scratch = p.sk_scratch + (size_t)tile * S * GEMM_BM * BN;
+      const int snv = S * NV;
+#define TE_GROUP_FINISH(RB, CAP) \
+  group_finish<BN, EPI, DH, RB, CAP>(p, tfull, t_row, stg, scratch, S, s, tile, warp, lane, m_blk, n_blk)
+      if (EPI != EPI_QKV && snv <= 2) { TE_GROUP_FINISH(8, 2); }
+      else if (EPI != EPI_QKV && snv <= 3) { TE_GROUP_FINISH(6, 3); }
+      else if (snv <= 4) { TE_GROUP_FINISH(4, 4); }
+      else if (snv <= 6) { TE_GROUP_FINISH(3, 6); }
+      else if (snv <= 8) { TE_GROUP_FINISH(2, 8); }
+      else { TE_GROUP_FINISH(1, 16); }
+#undef TE_GROUP_FINISH
       // the last CTA of the group to leave re-arms both counters for the next launch
       epi_bar_sync();
       if (warp == 2 && lane == 0) {

@@ -232,8 +232,10 @@ cudaError_t launch_gemmk_bn(int bn, int dh, const CUtensorMap& a, const CUtensor
   }
 }
 // CTAs per tile: fill the SMs, keep >= 2 k-blocks per CTA
+int g_split_target = 0;  // experiments: target CTA count of a split-K launch (0 = one per SM)
 inline int choose_splits(int tiles, int num_kb, int sm_count) {
-  int s = sm_count / tiles;
+  const int target = (g_split_target > 0 && g_split_target < sm_count) ? g_split_target : sm_count;
+  int s = target / tiles;
   if (s > te::GEMMK_MAX_SPLITS) s = te::GEMMK_MAX_SPLITS;
   if (s > num_kb / 2) s = num_kb / 2;
   return s < 1 ? 1 : s;
@@ -787,6 +789,7 @@ int te_set_option(te_handle* h, int option, int value) {
   }
   if (option == TE_OPT_SPLIT_K) {
     h->splitk = value ? 1 : 0;
+    g_split_target = value > 1 ? value : 0;
     free_graphs(h);
     return TE_OK;
   }
