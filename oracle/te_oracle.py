@@ -49,26 +49,34 @@ def unpack_layer(blob_bits: np.ndarray, layout: dict, layer: int) -> dict:
 
 
 # ------------------------------------------------------------- step 1-2: packing, position ids
-def cu_seqlens(text_lens, grid_h: int, grid_w: int) -> np.ndarray:
-    """§8c step 1: S_b = gh*gw + text_len[b]; cu[0]=0, cu[b+1]=cu[b]+S_b.  int32."""
+def cu_seqlens(text_lens, grid_h: int, grid_w: int, prefix_len: int = 0) -> np.ndarray:
+    """§8c step 1: S_b = prefix_len + gh*gw + text_len[b]; cu[0]=0, cu[b+1]=cu[b]+S_b.  int32.
+    (prefix_len > 0: SURVEY §8(f) NEXT-1, the shared text prefix of PAPER.md:389.)"""
     cu = [0]
     for tl in text_lens:
-        cu.append(cu[-1] + grid_h * grid_w + int(tl))
+        cu.append(cu[-1] + int(prefix_len) + grid_h * grid_w + int(tl))
     return np.asarray(cu, dtype=np.int32)
 
 
-def position_ids(text_lens, grid_h: int, grid_w: int) -> np.ndarray:
+def position_ids(text_lens, grid_h: int, grid_w: int, prefix_len: int = 0) -> np.ndarray:
     """§8c step 2 (BASELINE.json:configs[0]: "4x4 grid (t=0) followed by 24 text tokens
     (positions continue from max grid id + 1)"): int32 [3, T], rows (t, h, w).
       visual token k in [0, gh*gw): (0, k // gw, k % gw)            (row-major, Q5)
       text token j in [0, text_len): t = h = w = max(gh, gw) + j    (Q4)
     This is the computation whose host round-trip the paper locates in the TE's rotary
-    code (PAPER.md:23, 114)."""
+    code (PAPER.md:23, 114).
+    NEXT-1 (the real chat template puts an 80-token system prompt BEFORE the
+    image): with a text prefix of P tokens per frame the same rule applies with
+    every id continuing from the prefix (reading Q22, DESIGN.md §3): prefix token j: t=h=w=j;
+    visual token k: (P, P + k // gw, P + k % gw); text token j: P + max(gh, gw) + j."""
+    P = int(prefix_len)
     cols = []
     for tl in text_lens:
+        for j in range(P):
+            cols.append((j, j, j))
         for k in range(grid_h * grid_w):
-            cols.append((0, k // grid_w, k % grid_w))
-        start = max(grid_h, grid_w)
+            cols.append((P, P + k // grid_w, P + k % grid_w))
+        start = P + max(grid_h, grid_w)
         for j in range(int(tl)):
             cols.append((start + j, start + j, start + j))
     return np.asarray(cols, dtype=np.int32).reshape(-1, 3).T.copy()
@@ -81,18 +89,33 @@ def inv_freq(head_dim: int, theta: float) -> np.ndarray:
     return np.float64(theta) ** (-2.0 * i / np.float64(head_dim))
 
 
-def rope_axis(head_dim: int, sections) -> np.ndarray:
+def rope_axis(head_dim: int, sections, interleaved: bool = False) -> np.ndarray:
     """§8c step 3 / Q1 (contiguous sections, t first): axis(i) = 0 (t) if i < s_t,
-    1 (h) if s_t <= i < s_t + s_h, else 2 (w)."""
+    1 (h) if s_t <= i < s_t + s_h, else 2 (w).
+    NEXT-5 (SURVEY §8f, Q1 "keep axis(i) a table so the interleaved variant is a one-line
+    change"): interleaved=True deals the frequency pairs round-robin t,h,w,t,h,w,... to the
+    axes that still have pairs left in their section, so every axis keeps its section count
+    but spans the whole frequency range (reading Q23)."""
     s_t, s_h, s_w = sections
     assert s_t + s_h + s_w == head_dim // 2
-    return np.asarray([0] * s_t + [1] * s_h + [2] * s_w, dtype=np.int64)
+    if not interleaved:
+        return np.asarray([0] * s_t + [1] * s_h + [2] * s_w, dtype=np.int64)
+    left = [s_t, s_h, s_w]
+    ax = []
+    a = 0
+    while len(ax) < head_dim // 2:
+        if left[a] > 0:
+            ax.append(a)
+            left[a] -= 1
+        a = (a + 1) % 3
+    return np.asarray(ax, dtype=np.int64)
 
 
-def mrope_angles(pos: np.ndarray, head_dim: int, sections, theta: float) -> np.ndarray:
+def mrope_angles(pos: np.ndarray, head_dim: int, sections, theta: float,
+                 interleaved: bool = False) -> np.ndarray:
     """phi[n, i] = pos[axis(i), n] * omega_i   -> float64 [T, dh/2]."""
     om = inv_freq(head_dim, theta)
-    ax = rope_axis(head_dim, sections)
+    ax = rope_axis(head_dim, sections, interleaved)
     return pos[ax, :].T.astype(np.float64) * om[None, :]
 
 
@@ -172,17 +195,21 @@ def layer_forward(x: np.ndarray, W: dict, phi: np.ndarray, m, taps: dict | None 
 def encode(blob_bits: np.ndarray, layout: dict, m, embeds: np.ndarray, text_lens,
            grid_h: int, grid_w: int, *, frames=None, layer_begin: int = 0,
            layer_end: int | None = None, stop_after_attn: bool = False,
-           final_norm: int | None = None, taps: dict | None = None) -> np.ndarray:
+           final_norm: int | None = None, taps: dict | None = None,
+           prefix_len: int = 0) -> np.ndarray:
     """te_encode in fp64 (§8c steps 1-5).  embeds: fp32/fp64 [T, d] frame-major packed.
     Returns float64 [T, d].  `frames` restricts the computation to a subset of frames
     (frames never interact, BASELINE.json:configs[4]); rows of other frames are NaN.
     taps (optional dict) collects per-layer intermediates, each a list over layers of
-    [T, ...] arrays assembled in packed order (only when frames is None)."""
+    [T, ...] arrays assembled in packed order (only when frames is None).
+    prefix_len = P > 0 (NEXT-1): every frame's rows are [P prefix | gh*gw visual | text];
+    the prefix is simply part of each frame's causal sequence — no reuse, no shortcut."""
     text_lens = [int(t) for t in text_lens]
     B = len(text_lens)
-    cu = cu_seqlens(text_lens, grid_h, grid_w)
-    pos = position_ids(text_lens, grid_h, grid_w)
-    phi = mrope_angles(pos, m.head_dim, m.rope_sections, m.rope_theta)
+    cu = cu_seqlens(text_lens, grid_h, grid_w, prefix_len)
+    pos = position_ids(text_lens, grid_h, grid_w, prefix_len)
+    phi = mrope_angles(pos, m.head_dim, m.rope_sections, m.rope_theta,
+                       bool(getattr(m, "rope_interleaved", False)))
     T = int(cu[-1])
     assert embeds.shape == (T, m.hidden)
     L_end = m.n_layers if layer_end is None else layer_end

@@ -51,12 +51,12 @@ def test_clean_passes_own_gates(clean):
     assert _rejected(clean, out2, t2) == []
 
 
-def _swap_hw(head_dim, sections):
+def _swap_hw(head_dim, sections, interleaved=False):
     s_t, s_h, s_w = sections
     return np.asarray([0] * s_t + [2] * s_h + [1] * s_w, dtype=np.int64)
 
 
-def _ids_seq_index(text_lens, gh, gw):
+def _ids_seq_index(text_lens, gh, gw, prefix_len=0):
     cols = []
     for tl in text_lens:
         for k in range(gh * gw):

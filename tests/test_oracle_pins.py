@@ -82,6 +82,23 @@ def test_position_ids_nonsquare_enumeration(gh, gw):
 
 
 # ------------------------------------------------------------------------ angles / RoPE
+def test_position_ids_prefix_golden():
+    """NEXT-1: worked ids with a 3-token prefix before a 2x3 grid (tests/golden/position_ids_prefix.txt)."""
+    lines = [l.split() for l in open(os.path.join(GOLD, "position_ids_prefix.txt")) if l.strip() and l[0] != "#"]
+    cu = [int(x) for x in lines[0][1:]]
+    rows = np.asarray([[int(x) for x in l] for l in lines[1:]], dtype=np.int32)
+    assert O.cu_seqlens([2, 0], 2, 3, prefix_len=3).tolist() == cu
+    pos = O.position_ids([2, 0], 2, 3, prefix_len=3)
+    assert pos.shape == (3, 20)
+    assert np.array_equal(pos[:, :11].T, rows[:, 1:])
+    assert np.array_equal(pos[:, 11:20], pos[:, :9])          # second frame: same prefix + grid, no text
+    # P = 0 is the base rule
+    assert np.array_equal(O.position_ids([2, 0], 2, 3, prefix_len=0), O.position_ids([2, 0], 2, 3))
+    assert np.array_equal(O.cu_seqlens([2, 0], 2, 3, 0), O.cu_seqlens([2, 0], 2, 3))
+    # a "frame" that is only text (no grid) counts 0, 1, 2, ...: what the prefix-alone pass uses
+    assert O.position_ids([4], 0, 0).tolist() == [[0, 1, 2, 3]] * 3
+
+
 def test_inv_freq_closed_forms():
     om = O.inv_freq(128, 1e6)
     assert om[0] == 1.0
@@ -96,6 +113,29 @@ def test_rope_axis_sections():
     assert ax[:16].tolist() == [0] * 16 and ax[16:40].tolist() == [1] * 24 and ax[40:].tolist() == [2] * 24
     ax = O.rope_axis(64, (8, 12, 12))
     assert (ax[:8] == 0).all() and (ax[8:20] == 1).all() and (ax[20:] == 2).all()
+
+
+def test_rope_axis_interleaved():
+    """NEXT-5: round-robin t,h,w over the axes that still have pairs; section counts preserved."""
+    ax = O.rope_axis(64, (8, 12, 12), interleaved=True)
+    assert ax.tolist() == [0, 1, 2] * 8 + [1, 2] * 4                      # typed by hand
+    ax = O.rope_axis(128, (16, 24, 24), interleaved=True)
+    assert ax[:48].tolist() == [0, 1, 2] * 16 and ax[48:].tolist() == [1, 2] * 8
+    for dh, sec in [(128, (16, 24, 24)), (64, (8, 12, 12)), (128, (24, 20, 20)), (64, (32, 0, 0)), (64, (1, 30, 1))]:
+        ax = O.rope_axis(dh, sec, interleaved=True)
+        assert [int((ax == a).sum()) for a in range(3)] == list(sec)
+    # independent closed form for t-heavy sections (the published interleaved layout of this model family):
+    # pair i is h if i % 3 == 1 and i < 3*s_h, w if i % 3 == 2 and i < 3*s_w, else t
+    s_t, s_h, s_w = 24, 20, 20
+    want = [1 if (i % 3 == 1 and i < 3 * s_h) else (2 if (i % 3 == 2 and i < 3 * s_w) else 0) for i in range(64)]
+    assert O.rope_axis(128, (s_t, s_h, s_w), interleaved=True).tolist() == want
+    # angles follow the table
+    pos = np.asarray([[1], [10], [100]], dtype=np.int32)
+    phi = O.mrope_angles(pos, 64, (8, 12, 12), 1e6, interleaved=True)
+    om = [1e6 ** (-2.0 * i / 64) for i in range(32)]
+    assert abs(phi[0, 0] - 1 * om[0]) < 1e-12 and abs(phi[0, 1] - 10 * om[1]) < 1e-12
+    assert abs(phi[0, 2] - 100 * om[2]) < 1e-12 and abs(phi[0, 31] - 100 * om[31]) < 1e-12
+    assert abs(phi[0, 30] - 10 * om[30]) < 1e-12
 
 
 def test_mrope_angles_pick_the_right_axis():
@@ -288,6 +328,59 @@ def test_position_shift_invariance(monkeypatch):
     monkeypatch.setattr(O, "position_ids", lambda *a: orig(*a) + np.asarray([[5], [0], [0]], dtype=np.int32))
     out3 = O.encode(blob, lay, w.model, emb, tl, 4, 4)
     assert np.max(np.abs(out - out3)) < 1e-11
+
+
+def test_prefix_is_shared_and_reusable():
+    """NEXT-1 pins.  With a shared text prefix in front of every frame (a) the prefix rows of every frame
+    equal each other and equal the prefix encoded ALONE (causal prefix: it sees nothing after it), which is
+    what makes prefix K/V reuse exact; (b) P = 0 is the base path; (c) the ids of the tokens after the
+    prefix must continue from it: keeping them un-shifted changes the output."""
+    w, blob, lay, tl, emb = _tiny_inputs()
+    m = w.model
+    P = 5
+    rng = np.random.default_rng(7)
+    pre = rng.standard_normal((P, m.hidden)).astype(np.float32)
+    full = np.concatenate([pre, emb[:40], pre, emb[40:]])
+    out = O.encode(blob, lay, m, full, tl, 4, 4, prefix_len=P)
+    assert out.shape == (2 * (P + 40), m.hidden)
+    alone = O.encode(blob, lay, m, pre, [P], 0, 0)
+    assert np.array_equal(out[:P], out[P + 40:2 * P + 40])
+    assert np.max(np.abs(out[:P] - alone)) < 1e-12
+    base = O.encode(blob, lay, m, emb, tl, 4, 4)
+    assert np.array_equal(O.encode(blob, lay, m, emb, tl, 4, 4, prefix_len=0), base)
+    # the prefix changes what the frame tokens compute (they attend to it) ...
+    upd = np.linalg.norm(out[P:P + 40] - base[:40]) / np.linalg.norm(base[:40] - emb[:40])
+    assert upd > 0.05
+    # ... and the continuation of the ids matters (mutant: ids after the prefix restart at the base values)
+    orig = O.position_ids
+
+    def restart(text_lens, gh, gw, prefix_len=0):
+        pos = orig(text_lens, gh, gw, prefix_len).copy()
+        S = prefix_len + gh * gw
+        cu = O.cu_seqlens(text_lens, gh, gw, prefix_len)
+        for b in range(len(text_lens)):
+            pos[:, cu[b] + prefix_len:cu[b + 1]] -= prefix_len
+        return pos
+    O.position_ids = restart
+    try:
+        mut = O.encode(blob, lay, m, full, tl, 4, 4, prefix_len=P)
+    finally:
+        O.position_ids = orig
+    d = np.linalg.norm((mut - out)[P:P + 40]) / np.linalg.norm(out[P:P + 40] - full[P:P + 40])
+    assert d > 0.03, d
+
+
+def test_interleaved_rope_changes_output_and_keeps_shift_invariance(monkeypatch):
+    w, blob, lay, tl, emb = _tiny_inputs()
+    mi = w.model.replace(rope_interleaved=True)
+    base = O.encode(blob, lay, w.model, emb, tl, 4, 4)
+    out = O.encode(blob, lay, mi, emb, tl, 4, 4)
+    d = np.linalg.norm(out - base) / np.linalg.norm(base - emb)
+    assert d > 1e-3, d
+    orig = O.position_ids
+    monkeypatch.setattr(O, "position_ids", lambda *a: orig(*a) + np.asarray([[3], [0], [7]], dtype=np.int32))
+    out2 = O.encode(blob, lay, mi, emb, tl, 4, 4)
+    assert np.max(np.abs(out - out2)) < 1e-11
 
 
 def test_final_norm_flag():

@@ -21,6 +21,7 @@ class TEModelConfig:
     rms_eps: float = 1e-6
     rope_theta: float = 1e6
     final_norm: int = 0    # raw last-layer residual by default
+    rope_interleaved: bool = False   # round-robin t,h,w frequency pairs instead of contiguous
 
     def __post_init__(self):
         assert sum(self.rope_sections) == self.head_dim // 2
@@ -31,9 +32,12 @@ class TEModelConfig:
         return (self.n_q_heads + 2 * self.n_kv_heads) * self.head_dim
 
     def with_layers(self, n_layers: int) -> "TEModelConfig":
+        return self.replace(n_layers=n_layers)
+
+    def replace(self, **kw) -> "TEModelConfig":
         d = asdict(self)
-        d["n_layers"] = n_layers
         d["rope_sections"] = tuple(d["rope_sections"])
+        d.update(kw)
         return TEModelConfig(**d)
 
 
