@@ -48,13 +48,17 @@ typedef struct te_config {
   int32_t n_kv_heads; /* Hkv; Hq % Hkv == 0 (GQA: q head a uses kv head a / (Hq/Hkv)) */
   int32_t head_dim;   /* dh in {64, 128}                                           */
   int32_t ffn;        /* F; multiple of 128                                        */
-  int32_t rope_sec_t, rope_sec_h, rope_sec_w; /* contiguous M-RoPE sections, sum == dh/2 */
+  int32_t rope_sec_t, rope_sec_h, rope_sec_w; /* M-RoPE sections (pairs per axis), sum == dh/2 */
   float rms_eps;      /* RMSNorm epsilon (inside the root)                         */
   double rope_theta;  /* omega_i = theta^(-2i/dh)                                  */
   int32_t max_frames;           /* capacity: frames per call                       */
   int32_t max_tokens;           /* capacity: total packed tokens per call          */
   int32_t max_tokens_per_frame; /* capacity: S_b <= this (<= 256)                  */
   int32_t final_norm;           /* 0: out = raw last-layer residual (default); 1: RMSNorm(x; gf) */
+  int32_t rope_interleaved;     /* 0 (default): sections are contiguous [t | h | w] over the frequency
+                                   pairs; 1: pairs are dealt round-robin t,h,w,t,h,w,... to the axes that
+                                   still have pairs left                      */
+  int32_t max_prefix_tokens;    /* capacity of the shared text prefix (te_encode_prefix); 0 = none   */
 } te_config;
 
 /* Exact size in bytes of the canonical weight blob for cfg (see te_load_weights). */
@@ -95,6 +99,22 @@ int te_load_weights(te_handle* h, const void* bf16_blob, size_t n_bytes);
 int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w,
               const float* embeds, const int32_t* text_lens, int32_t total_tokens, float* out,
               void* cuda_stream);
+
+/* Shared text prefix with K/V reuse.  The real chat template puts the same
+ * system prompt (80 tokens: 13 % of the TE's time) in front of every frame's image.  Being
+ * a causal prefix it sees nothing after it, so its hidden states and its per-layer keys/values are the
+ * same for every frame and every call: te_encode_prefix runs the stack ONCE over the prefix tokens
+ * (ids t=h=w=0..P-1) and keeps every layer's K/V (after QK-norm and rotation) in library memory.
+ * Afterwards te_encode treats each frame as [prefix | grid | text] WITHOUT re-encoding the prefix:
+ * `embeds`/`out` still hold only the S_b = grid_h*grid_w + text_lens[b] own tokens of each frame, their
+ * ids continue from the prefix (visual token k: (P, P + k/grid_w, P + k%grid_w); text j:
+ * P + max(grid_h,grid_w) + j) and their queries attend to the P cached keys plus their own causal keys.
+ *   prefix_embeds  DEVICE fp32 [prefix_len, hidden]
+ *   prefix_len     P in [0, max_prefix_tokens]; 0 removes the prefix
+ *   prefix_out     DEVICE fp32 [prefix_len, hidden] or NULL: hidden states of the prefix tokens
+ * Synchronous with respect to `cuda_stream` ordering only (work is enqueued; no host sync). */
+int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_len, float* prefix_out,
+                     void* cuda_stream);
 
 /* Same call with HOST buffers (end-to-end path): copies embeds/text_lens host->device into
  * library staging buffers, runs te_encode, copies `out` device->host, and synchronises.

@@ -31,7 +31,7 @@ TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "fi
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 
 EXPORTS = [
-    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_host",
+    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host",
     "te_query_async_error", "te_set_option", "te_kernel_launches", "te_kernel_times", "te_debug_set_range",
     "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_destroy", "te_strerror", "te_last_error",
 ]
@@ -45,7 +45,7 @@ class TEConfig(Structure):
         ("rope_sec_t", c_int32), ("rope_sec_h", c_int32), ("rope_sec_w", c_int32),
         ("rms_eps", c_float), ("rope_theta", c_double),
         ("max_frames", c_int32), ("max_tokens", c_int32), ("max_tokens_per_frame", c_int32),
-        ("final_norm", c_int32),
+        ("final_norm", c_int32), ("rope_interleaved", c_int32), ("max_prefix_tokens", c_int32),
     ]
 
 
@@ -76,6 +76,8 @@ def lib() -> ctypes.CDLL:
     L.te_load_weights.argtypes = [c_void_p, c_void_p, c_size_t]
     L.te_encode.restype = c_int
     L.te_encode.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_int32, c_void_p, c_void_p]
+    L.te_encode_prefix.restype = c_int
+    L.te_encode_prefix.argtypes = [c_void_p, c_void_p, c_int32, c_void_p, c_void_p]
     L.te_encode_host.restype = c_int
     L.te_encode_host.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_void_p]
     L.te_query_async_error.restype = c_int
@@ -129,12 +131,13 @@ def _check(code: int, h=None):
 
 
 def make_config(model, max_frames: int, max_tokens: int, max_tokens_per_frame: int = 256,
-                final_norm: int | None = None) -> TEConfig:
+                final_norm: int | None = None, max_prefix_tokens: int = 0) -> TEConfig:
     """TEConfig from a workloads.TEModelConfig-like object (duck-typed)."""
     s_t, s_h, s_w = model.rope_sections
     return TEConfig(model.n_layers, model.hidden, model.n_q_heads, model.n_kv_heads, model.head_dim,
                     model.ffn, s_t, s_h, s_w, model.rms_eps, model.rope_theta, max_frames, max_tokens,
-                    max_tokens_per_frame, model.final_norm if final_norm is None else final_norm)
+                    max_tokens_per_frame, model.final_norm if final_norm is None else final_norm,
+                    1 if getattr(model, "rope_interleaved", False) else 0, max_prefix_tokens)
 
 
 # ---------------------------------------------------------------- C-ABI names, marshalling only
@@ -159,6 +162,11 @@ def te_encode(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out,
     """embeds/out: DEVICE fp32 [T, d]; text_lens: DEVICE int32 [B]; stream: cudaStream_t as int."""
     _check(lib().te_encode(h, n_frames, grid_h, grid_w, _ptr(embeds), _ptr(text_lens), total_tokens,
                            _ptr(out), _ptr(stream)), h)
+
+
+def te_encode_prefix(h, prefix_embeds, prefix_len, prefix_out=None, stream=None):
+    """prefix_embeds / prefix_out: DEVICE fp32 [P, d] (prefix_out may be None)."""
+    _check(lib().te_encode_prefix(h, _ptr(prefix_embeds), prefix_len, _ptr(prefix_out), _ptr(stream)), h)
 
 
 def te_encode_host(h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host):
@@ -219,9 +227,9 @@ class TextEncoder:
     """Convenience owner of a handle (create -> load -> encode -> destroy)."""
 
     def __init__(self, model, max_frames: int, max_tokens: int, device: int = 0,
-                 max_tokens_per_frame: int = 256, final_norm: int | None = None):
+                 max_tokens_per_frame: int = 256, final_norm: int | None = None, max_prefix_tokens: int = 0):
         self.model = model
-        self.cfg = make_config(model, max_frames, max_tokens, max_tokens_per_frame, final_norm)
+        self.cfg = make_config(model, max_frames, max_tokens, max_tokens_per_frame, final_norm, max_prefix_tokens)
         self.h = te_create(self.cfg, device)
 
     def load_weights(self, blob):
@@ -229,6 +237,9 @@ class TextEncoder:
 
     def encode(self, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream=None):
         te_encode(self.h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream)
+
+    def encode_prefix(self, prefix_embeds, prefix_len, prefix_out=None, stream=None):
+        te_encode_prefix(self.h, prefix_embeds, prefix_len, prefix_out, stream)
 
     def encode_host(self, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host):
         te_encode_host(self.h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host)

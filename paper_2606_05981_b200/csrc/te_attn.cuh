@@ -24,6 +24,11 @@ struct AttnParams {
   int n_q_heads, n_kv_heads;
   int total_tokens;
   float scale_log2;  // log2(e) / sqrt(dh)
+  // shared text prefix (te_encode_prefix): P cached keys/values per layer that every query of every frame
+  // sees in front of its own causal keys.  kv_prefix: [P, ld_prefix] = k heads | v heads; null when P = 0.
+  const __nv_bfloat16* kv_prefix;
+  int prefix_len;
+  int ld_prefix;
 };
 
 // GH = q heads served by one CTA (they share one kv head: GH divides Hq/Hkv); 4 warps per head.
@@ -100,6 +105,10 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
   const __nv_bfloat16* gk = p.qkv + (size_t)seq0 * p.ld + (p.n_q_heads + kvh) * DH;
   const __nv_bfloat16* gv = p.qkv + (size_t)seq0 * p.ld + (p.n_q_heads + p.n_kv_heads + kvh) * DH;
 
+  // key index space of a frame: [0, P) = cached prefix keys, [P, P + S) = the frame's own keys
+  const int P = p.prefix_len;
+  const __nv_bfloat16* pk = p.kv_prefix + kvh * DH;
+  const __nv_bfloat16* pv = p.kv_prefix + (p.n_kv_heads + kvh) * DH;
   constexpr int CH = DH / 8;  // 16-byte chunks per row
   auto load_kv = [&](int kb, int stage) {
     __nv_bfloat16* sK = sKV + stage * Cfg::KV_STAGE_ELEMS;
@@ -107,9 +116,13 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
     const int k0 = kb * ATT_BKV;
     for (int i = tid; i < ATT_BKV * CH; i += THREADS) {
       const int r = i / CH, c = i % CH;
-      const bool ok = k0 + r < S;
-      cp_async16(sK + r * ROW + c * 8, gk + (size_t)(k0 + r) * p.ld + c * 8, ok);
-      cp_async16(sV + r * ROW + c * 8, gv + (size_t)(k0 + r) * p.ld + c * 8, ok);
+      const int key = k0 + r;
+      const bool ok = key < P + S;
+      const bool in_prefix = key < P;
+      const __nv_bfloat16* ksrc = in_prefix ? pk + (size_t)key * p.ld_prefix : gk + (size_t)(key - P) * p.ld;
+      const __nv_bfloat16* vsrc = in_prefix ? pv + (size_t)key * p.ld_prefix : gv + (size_t)(key - P) * p.ld;
+      cp_async16(sK + r * ROW + c * 8, (ok ? ksrc : gk) + c * 8, ok);
+      cp_async16(sV + r * ROW + c * 8, (ok ? vsrc : gv) + c * 8, ok);
     }
   };
   for (int i = tid; i < GH * ATT_BQ * CH; i += THREADS) {
@@ -127,7 +140,8 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
   const int qrow0 = q0 + wr * 16 + g;  // this thread's rows: qrow0 and qrow0 + 8 (index within the frame)
   const __nv_bfloat16* sQh = sQ + (hl * ATT_BQ + wr * 16) * ROW;
 
-  const int n_kv_blocks = qb + 1;  // causal: keys [0, q0 + 64)
+  // causal: combined keys [0, P + q0 + 64), capped at the frame's end
+  const int n_kv_blocks = (min(P + q0 + ATT_BQ, P + S) + ATT_BKV - 1) / ATT_BKV;
   for (int kb = 0; kb < n_kv_blocks; ++kb) {
     if (kb + 1 < n_kv_blocks) {
       load_kv(kb + 1, (kb + 1) & 1);  // stage (kb+1)&1 was released by the barrier ending iteration kb-1
@@ -161,11 +175,12 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
         mma_bf16_16816(s[2 * nt + 1], a, bfr[2], bfr[3]);
       }
     }
-    // ---- causal mask (only the diagonal block needs it) + online softmax
-    if (kb == qb) {
+    // ---- causal mask (only blocks reaching past the first query row's diagonal need it) + online softmax:
+    // query row n sees combined keys 0 .. P + n
+    if (k0 + ATT_BKV - 1 > P + q0) {
 #pragma unroll
       for (int nt = 0; nt < ATT_BKV / 8; ++nt) {
-        const int key = k0 + nt * 8 + 2 * t;
+        const int key = k0 + nt * 8 + 2 * t - P;
         if (key > qrow0) s[nt][0] = -INFINITY;
         if (key + 1 > qrow0) s[nt][1] = -INFINITY;
         if (key > qrow0 + 8) s[nt][2] = -INFINITY;

@@ -27,7 +27,9 @@ struct PrepParams {
   float* ssq;                   // [T][ssq_stride], first ssq_parts entries of a row used
   int ssq_parts, ssq_stride;
   int n_frames, total_tokens, d, half_dim, max_tokens_per_frame;
-  int grid_h, grid_w, sec_t, sec_h;
+  int grid_h, grid_w;
+  int pos_offset;   // length P of the shared text prefix in front of every frame (ids continue from it)
+  int8_t axis[64];  // M-RoPE axis (0 = t, 1 = h, 2 = w) of frequency pair i (contiguous or interleaved sections)
 };
 
 // One block per token.  Warp 0 of EVERY block scans text_lens itself (B is a few dozen frames; the
@@ -89,10 +91,11 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   if (tok >= p.total_tokens) return;
   const int n = tok - s_start;
   int pt, ph, pw;
+  const int off = p.pos_offset;
   if (n < n_vis) {
-    pt = 0; ph = n / p.grid_w; pw = n % p.grid_w;     // visual token: row-major grid, t = 0
+    pt = off; ph = off + n / p.grid_w; pw = off + n % p.grid_w;  // visual token: row-major grid, t constant
   } else {
-    pt = ph = pw = max(p.grid_h, p.grid_w) + (n - n_vis);  // text: continues from max grid id + 1
+    pt = ph = pw = off + max(p.grid_h, p.grid_w) + (n - n_vis);  // text: continues from max grid id + 1
   }
   if (threadIdx.x == 0) {
     p.pos[tok] = pt;
@@ -101,7 +104,8 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   }
   // the rotary table on the last warps, so that it overlaps the row copy of the first ones
   for (int i = 255 - threadIdx.x; i < p.half_dim; i += 256) {
-    const int pid = (i < p.sec_t) ? pt : ((i < p.sec_t + p.sec_h) ? ph : pw);
+    const int ax = p.axis[i];
+    const int pid = (ax == 0) ? pt : ((ax == 1) ? ph : pw);
     double sn, cs;
     sincos(static_cast<double>(pid) * p.inv_freq[i], &sn, &cs);
     p.cos_t[(size_t)tok * p.half_dim + i] = static_cast<float>(cs);

@@ -55,7 +55,7 @@ struct LayerOff {
 };
 
 struct GraphKey {
-  int n_frames, grid_h, grid_w, total_tokens, lb, le, stop;
+  int n_frames, grid_h, grid_w, total_tokens, lb, le, stop, prefix_len;
   const void *embeds, *lens, *out;
   bool operator==(const GraphKey& o) const { return memcmp(this, &o, sizeof(GraphKey)) == 0; }
 };
@@ -97,6 +97,13 @@ struct te_handle {
   int ssq_parts_cap = 0;
   unsigned long long* trace = nullptr;  // [4 GEMM classes][sm_count][TRACE_SLOTS] (debug, TE_OPT_TRACE)
   int trace_on = 0;
+  // M-RoPE axis of every frequency pair (contiguous or interleaved sections)
+  int8_t axis[64] = {};
+  // shared text prefix (te_encode_prefix): per-layer keys | values of the P prefix tokens, [L][max_prefix][2*Hkv*dh]
+  bf16* kv_prefix = nullptr;
+  float* prefix_buf = nullptr;    // [max_prefix, d] residual of the prefix pass when the caller wants no output
+  int32_t* prefix_lens = nullptr; // device [1]
+  int prefix_len = 0;
   // host-path staging
   float *stg_embeds = nullptr, *stg_out = nullptr;
   int32_t* stg_lens = nullptr;
@@ -139,6 +146,10 @@ int validate_config(const te_config& c) {
   if (c.rope_sec_t < 0 || c.rope_sec_h < 0 || c.rope_sec_w < 0) return TE_ERR_INVALID_ARG;
   if (c.rope_sec_t + c.rope_sec_h + c.rope_sec_w != c.head_dim / 2) return TE_ERR_INVALID_ARG;
   if (c.max_frames < 1 || c.max_tokens < 1 || c.max_tokens_per_frame < 1) return TE_ERR_INVALID_ARG;
+  if (c.rope_interleaved < 0 || c.rope_interleaved > 1) return TE_ERR_INVALID_ARG;
+  if (c.max_prefix_tokens < 0 || c.max_prefix_tokens > c.max_tokens ||
+      c.max_prefix_tokens > c.max_tokens_per_frame)
+    return TE_ERR_INVALID_ARG;
   if (!(c.rms_eps > 0.f) || !(c.rope_theta > 0.0)) return TE_ERR_INVALID_ARG;
   if (c.head_dim != 64 && c.head_dim != 128) return TE_ERR_UNSUPPORTED;
   if (c.hidden % 128 != 0 || c.ffn % 128 != 0) return TE_ERR_UNSUPPORTED;
@@ -306,13 +317,17 @@ cudaError_t init_kernel_attrs() {
 }
 
 // Enqueue the whole stack on `st`.  Returns the number of kernels launched via *n_kernels.
+// prefix_pass: the one-frame pass of te_encode_prefix (text only, ids 0..T-1) that also saves every layer's K/V.
 int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const float* embeds, const int32_t* lens, int T,
-                  float* out, cudaStream_t st, int* n_kernels) {
+                  float* out, cudaStream_t st, int* n_kernels, bool prefix_pass = false) {
   const te_config& c = h->cfg;
   const int d = c.hidden, dh = c.head_dim, F = c.ffn;
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
   const int n_q = c.n_q_heads * dh;
-  const int lb = h->dbg_lb, le = h->dbg_le;
+  const int lb = prefix_pass ? 0 : h->dbg_lb, le = prefix_pass ? c.n_layers : h->dbg_le;
+  const bool dbg_stop = !prefix_pass && h->dbg_stop;
+  const int P = prefix_pass ? 0 : h->prefix_len;  // cached prefix keys in front of every frame
+  const int n_kv = 2 * c.n_kv_heads * dh;
   // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
   // one CTA per tile so that more SMs stream weights (HBM-bound regime).
   const int pair = h->pair_mode == 2 ? (T >= 1024 ? 1 : 0) : h->pair_mode;
@@ -356,7 +371,8 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     pp.inv_freq = h->inv_freq; pp.g_first = h->w + h->off[lb].g1; pp.xg = h->xg; pp.ssq = h->ssq;
     pp.ssq_parts = parts; pp.ssq_stride = h->ssq_parts_cap; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
     pp.half_dim = dh / 2; pp.max_tokens_per_frame = c.max_tokens_per_frame;
-    pp.grid_h = grid_h; pp.grid_w = grid_w; pp.sec_t = c.rope_sec_t; pp.sec_h = c.rope_sec_h;
+    pp.grid_h = grid_h; pp.grid_w = grid_w; pp.pos_offset = P;
+    memcpy(pp.axis, h->axis, sizeof(pp.axis));
     tick();
     TE_CUDA(h, launch_k(te::te_prep_kernel, dim3(T), dim3(256), 0, st, pp));
     tock(TE_KCLASS_PREP);
@@ -384,7 +400,8 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int G = c.n_q_heads / c.n_kv_heads;
   int g_shift = 0;
   while ((1 << g_shift) < G) ++g_shift;
-  const bool attn_tc = h->attn_impl == 1 && (1 << g_shift) == G && G <= 8;
+  // (with a cached prefix the keys of a frame are prefix + own, possibly > 256: the streaming flash kernel)
+  const bool attn_tc = h->attn_impl == 1 && (1 << g_shift) == G && G <= 8 && P == 0;
   CUtensorMap tmQ, tmKV;
   int attn_split = 1;
   if (attn_tc) {
@@ -417,11 +434,18 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       tock(TE_KCLASS_QKV);
       ++nk;
     }
+    if (prefix_pass) {  // keep this layer's keys | values of the prefix tokens
+      TE_CUDA(h, cudaMemcpy2DAsync(h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv, (size_t)n_kv * sizeof(bf16),
+                                   h->qkv + n_q, (size_t)n_qkv * sizeof(bf16), (size_t)n_kv * sizeof(bf16), T,
+                                   cudaMemcpyDeviceToDevice, st));
+    }
     {  // a2: causal GQA attention
       te::AttnParams ap{};
       ap.qkv = h->qkv; ap.out = h->attn; ap.cu_seqlens = h->cu; ap.ld = n_qkv; ap.n_q_heads = c.n_q_heads;
       ap.n_kv_heads = c.n_kv_heads; ap.total_tokens = T;
       ap.scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
+      ap.prefix_len = P; ap.ld_prefix = n_kv;
+      ap.kv_prefix = P > 0 ? h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv : nullptr;
       tick();
       if (attn_tc) {
         te::AttnTcParams tp{};
@@ -450,7 +474,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       tock(TE_KCLASS_OPROJ);
       ++nk;
     }
-    if (h->dbg_stop && l == le - 1) break;
+    if (dbg_stop && l == le - 1) break;
     {  // a4: RMSNorm -> gate/up GEMM -> SiLU(gate) * up
       te::GemmParams p = base;
       p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / h->bn_gu;
@@ -483,7 +507,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       ++nk;
     }
   }
-  if (c.final_norm && le == c.n_layers && !h->dbg_stop) {  // a6
+  if (c.final_norm && le == c.n_layers && !dbg_stop) {  // a6
     tick();
     TE_CUDA(h, launch_k(te::te_final_norm_kernel, dim3((T + 7) / 8), dim3(256), 0, st, out,
                         static_cast<const bf16*>(h->w + h->gf_off), T, d, c.rms_eps));
@@ -560,6 +584,29 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   TE_ALLOC(h->sk_sem, 2 * (size_t)h->sm_count * sizeof(int));
 #undef TE_ALLOC
   if (cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess) return fail(TE_ERR_CUDA);
+  if (c.max_prefix_tokens > 0) {
+    const size_t n_kv = 2 * (size_t)c.n_kv_heads * c.head_dim;
+    if (cudaMalloc(reinterpret_cast<void**>(&h->kv_prefix), (size_t)c.n_layers * c.max_prefix_tokens * n_kv * sizeof(bf16)) !=
+            cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->prefix_buf), (size_t)c.max_prefix_tokens * c.hidden * sizeof(float)) !=
+            cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->prefix_lens), sizeof(int32_t)) != cudaSuccess)
+      return fail(TE_ERR_CUDA);
+  }
+  {  // axis of frequency pair i: contiguous [t | h | w], or round-robin over the axes with pairs left
+    int left[3] = {c.rope_sec_t, c.rope_sec_h, c.rope_sec_w};
+    int a = 0;
+    for (size_t i = 0; i < hd2; ++i) {
+      if (c.rope_interleaved) {
+        while (left[a] == 0) a = (a + 1) % 3;
+        h->axis[i] = static_cast<int8_t>(a);
+        --left[a];
+        a = (a + 1) % 3;
+      } else {
+        h->axis[i] = static_cast<int8_t>((int)i < c.rope_sec_t ? 0 : ((int)i < c.rope_sec_t + c.rope_sec_h ? 1 : 2));
+      }
+    }
+  }
   if (cudaMemset(h->flag, 0, sizeof(int32_t)) != cudaSuccess) return fail(TE_ERR_CUDA);
   std::vector<double> invf(hd2);
   for (size_t i = 0; i < hd2; ++i) invf[i] = std::pow(c.rope_theta, -2.0 * (double)i / (double)c.head_dim);
@@ -662,7 +709,7 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
   GraphKey key;
   memset(&key, 0, sizeof(key));
   key.n_frames = n_frames; key.grid_h = grid_h; key.grid_w = grid_w; key.total_tokens = total_tokens;
-  key.lb = h->dbg_lb; key.le = h->dbg_le; key.stop = h->dbg_stop;
+  key.lb = h->dbg_lb; key.le = h->dbg_le; key.stop = h->dbg_stop; key.prefix_len = h->prefix_len;
   key.embeds = embeds; key.lens = text_lens; key.out = out;
   GraphEntry* hit = nullptr;
   for (auto& e : h->cache)
@@ -702,6 +749,31 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
   hit->stamp = ++h->stamp;
   TE_CUDA(h, cudaGraphLaunch(hit->exec, st));
   h->launches += hit->n_kernels;
+  return TE_OK;
+}
+
+int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_len, float* prefix_out, void* cuda_stream) {
+  if (!h) return TE_ERR_INVALID_ARG;
+  if (!h->loaded) return TE_ERR_NOT_LOADED;
+  const te_config& c = h->cfg;
+  if (prefix_len < 0 || prefix_len > c.max_prefix_tokens) return TE_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  free_graphs(h);  // captured graphs bake in the ids / attention variant of the previous prefix
+  h->prefix_len = 0;
+  if (prefix_len == 0) return TE_OK;
+  if (!prefix_embeds || prefix_embeds == prefix_out) return TE_ERR_INVALID_ARG;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (st != nullptr) TE_CUDA(h, cudaStreamIsCapturing(st, &cap));
+  if (cap != cudaStreamCaptureStatusNone || h->timing) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaSetDevice(h->device));
+  TE_CUDA(h, cudaMemcpyAsync(h->prefix_lens, &prefix_len, sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  int nk = 0;
+  // one text-only frame (no grid): ids t = h = w = 0..P-1; every layer's K/V is copied to the cache
+  int rc = enqueue_stack(h, 1, 0, 0, prefix_embeds, h->prefix_lens, prefix_len, prefix_out ? prefix_out : h->prefix_buf, st,
+                         &nk, /*prefix_pass=*/true);
+  if (rc != TE_OK) return rc;
+  h->launches += nk;
+  h->prefix_len = prefix_len;
   return TE_OK;
 }
 
@@ -921,7 +993,8 @@ void te_destroy(te_handle* h) {
   free_graphs(h);
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
-                  h->act, h->stg_embeds, h->stg_out, h->stg_lens, h->trace, h->sk_scratch, h->sk_sem};
+                  h->act, h->stg_embeds, h->stg_out, h->stg_lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix,
+                  h->prefix_buf, h->prefix_lens};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);

@@ -23,11 +23,12 @@ class GpuTE:
     """Owns one handle; encode() returns numpy arrays."""
 
     def __init__(self, model, max_frames, max_tokens, blob, final_norm=None, cta_pair=None, resid_bn=None,
-                 split_k=None):
+                 split_k=None, max_prefix_tokens=0):
         import torch
         import paper_2606_05981_b200 as te
         self.te, self.torch, self.model = te, torch, model
-        self.enc = te.TextEncoder(model, max_frames, max_tokens, final_norm=final_norm)
+        self.enc = te.TextEncoder(model, max_frames, max_tokens, final_norm=final_norm,
+                                  max_prefix_tokens=max_prefix_tokens)
         self.enc.load_weights(blob)
         if cta_pair is not None:
             te.te_set_option(self.enc.h, te.TE_OPT_CTA_PAIR, cta_pair)
@@ -50,6 +51,19 @@ class GpuTE:
         torch.cuda.synchronize()
         self._keep = (e, tl, out)
         return out.cpu().numpy()
+
+    def encode_prefix(self, prefix_embeds, want_out=True):
+        """te_encode_prefix: caches the prefix K/V in the handle; returns the prefix hidden states."""
+        torch = self.torch
+        P = int(prefix_embeds.shape[0])
+        if P == 0:
+            self.enc.encode_prefix(None, 0)
+            return None
+        e = torch.from_numpy(np.ascontiguousarray(prefix_embeds, dtype=np.float32)).cuda()
+        out = torch.empty_like(e) if want_out else None
+        self.enc.encode_prefix(e, P, out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy() if want_out else None
 
     def tap(self, what, shape, dtype):
         buf = np.empty(shape, dtype=dtype)

@@ -32,9 +32,10 @@ def test_library_exports_every_declared_symbol(te):
 
 
 def test_config_struct_layout_matches_header(te):
-    # te_config: 9 int32, float, (pad) double, 4 int32 -> natural C layout
-    assert ctypes.sizeof(te.TEConfig) == 64
+    # te_config: 9 int32, float, (pad) double, 6 int32 -> natural C layout
+    assert ctypes.sizeof(te.TEConfig) == 72
     assert te.TEConfig.rope_theta.offset == 40 and te.TEConfig.max_frames.offset == 48
+    assert te.TEConfig.rope_interleaved.offset == 64 and te.TEConfig.max_prefix_tokens.offset == 68
 
 
 def test_blob_bytes_and_strerror_without_gpu(te):

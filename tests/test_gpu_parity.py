@@ -358,3 +358,85 @@ def test_host_path_matches_device_path(H):
     g.enc.encode_host(2, 4, 4, eh, np.asarray(tl, dtype=np.int32), oh)
     assert np.array_equal(oh.numpy(), out)
     g.close()
+
+
+# ------------------------------------------------- interleaved M-RoPE sections
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_interleaved_mrope(H, O, cfg_id):
+    """Round-robin t,h,w frequency pairs: rotary table against the oracle's (abs err <= 1e-5), whole stack
+    within the gates, and different from the contiguous layout."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    m = w.model.replace(rope_interleaved=True)
+    taps = {}
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, w.grid_h, w.grid_w, taps=taps)
+    g = H.GpuTE(m, w.n_frames, T, blob)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    t = g.taps(T, w.n_frames)
+    assert np.max(np.abs(t["cos"] - taps["cos"])) <= PM.GATE_COSSIN_ABS
+    assert np.max(np.abs(t["sin"] - taps["sin"])) <= PM.GATE_COSSIN_ABS
+    _assert_final(PM.stack_metrics(out, ref, emb), f"interleaved cfg{cfg_id}")
+    base = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, w.grid_h, w.grid_w)
+    assert PM.rel_l2(out - emb, base - emb) > 10 * PM.rel_l2(out - emb, ref - emb)   # the layout is visible
+    g.close()
+
+
+# ------------------------------------------- SURVEY §8(f) NEXT-1: shared text prefix with K/V reuse
+def _with_prefix(pre, emb, cu):
+    return np.concatenate([np.concatenate([pre, emb[cu[b]:cu[b + 1]]]) for b in range(len(cu) - 1)])
+
+
+def _strip_prefix(full, P, cu):
+    return np.concatenate([full[cu[b] + (b + 1) * P: cu[b + 1] + (b + 1) * P] for b in range(len(cu) - 1)])
+
+
+@pytest.mark.parametrize("cfg_id,P", [(1, 7), (1, 64), (2, 80)])
+def test_prefix_kv_reuse_matches_full_recompute(H, O, cfg_id, P):
+    """te_encode_prefix once, then te_encode on the frames' own tokens only == the oracle run on the full
+    [prefix | grid | text] sequences of every frame (ids continue through the prefix); the prefix rows
+    equal the oracle's prefix rows; removing the prefix restores the base path bitwise."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    m = w.model
+    pre = np.random.default_rng(11 + P).standard_normal((P, m.hidden)).astype(np.float32)
+    cu = O.cu_seqlens(tl, w.grid_h, w.grid_w)
+    full = _with_prefix(pre, emb, cu)
+    ref_full = O.encode(blob, W.blob_layout(m), m, full, tl, w.grid_h, w.grid_w, prefix_len=P)
+    ref = _strip_prefix(ref_full, P, cu)
+    g = H.GpuTE(m, w.n_frames, T, blob, max_prefix_tokens=max(P, 1))
+    base = g.encode(emb, tl, w.grid_h, w.grid_w)
+    pre_out = g.encode_prefix(pre)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    pos = g.tap(g.te.TE_TAP_POS, (3, T), np.int32)
+    want_pos = _strip_prefix(O.position_ids(tl, w.grid_h, w.grid_w, prefix_len=P).T, P, cu).T
+    assert np.array_equal(pos, want_pos)
+    _assert_final(PM.stack_metrics(out, ref, emb), f"prefix cfg{cfg_id} P={P}")
+    _assert_final(PM.stack_metrics(pre_out, ref_full[:P], pre), "prefix rows")
+    assert PM.rel_l2(out - emb, base - emb) > 10 * PM.rel_l2(out - emb, ref - emb)   # the prefix is visible
+    assert np.array_equal(out, g.encode(emb, tl, w.grid_h, w.grid_w, use_graph=0))
+    g.encode_prefix(np.zeros((0, m.hidden), dtype=np.float32))
+    assert np.array_equal(g.encode(emb, tl, w.grid_h, w.grid_w), base)
+    g.close()
+
+
+def test_prefix_28_layers_ragged_sampled_frames(H, O):
+    """Full depth, ragged batch (cfg 5 lengths, first 12 frames) behind an 80-token prefix:
+    S_b + P reaches 240 keys; sampled frames against the oracle's full recompute."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(5)
+    m = w.model
+    B = 12
+    tl = tl[:B]
+    cu = O.cu_seqlens(tl, w.grid_h, w.grid_w)
+    T = int(cu[-1])
+    emb = emb[:T]
+    P = 80
+    pre = np.random.default_rng(5).standard_normal((P, m.hidden)).astype(np.float32)
+    g = H.GpuTE(m, B, T, blob, max_prefix_tokens=P)
+    g.encode_prefix(pre, want_out=False)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    assert np.isfinite(out).all()
+    for b in (0, 7, 11):
+        fe = np.concatenate([pre, emb[cu[b]:cu[b + 1]]])
+        ref = O.encode(blob, W.blob_layout(m), m, fe, [tl[b]], w.grid_h, w.grid_w, prefix_len=P)[P:]
+        met = PM.stack_metrics(out[cu[b]:cu[b + 1]], ref, emb[cu[b]:cu[b + 1]], ch)
+        print(f"prefix cfg5 frame {b}: {met}")
+        _assert_final(met, f"prefix 28L frame {b}")
+    g.close()
