@@ -399,7 +399,8 @@ def main():
     peaks = load_peaks()
     # dram__bytes_read.sum + dram__bytes_write.sum of one gate/up launch, from the committed ncu --set full
     # capture (profiles/r01c_ncu_full_layer_cfg4.md); only that workload was captured
-    traffic = {"cfg4_28L_B16": 63.348992e6 + 15.863552e6}.get(w.name)
+    # (cfg 2: profiles/r01d_ncu_full_small_batch.md, gate/up on the split-K kernel)
+    traffic = {"cfg4_28L_B16": 63.348992e6 + 15.863552e6, "cfg2_1L_B1": 50.973952e6 + 1.491456e6}.get(w.name)
     flops, wbytes, abytes = stack_work(m, seq_lens)
     flops += m.n_layers * sum(4.0 * m.head_dim * m.n_q_heads * s * args.prefix for s in seq_lens)  # prefix keys
     t_compute = flops / (peaks["tf_sustained"] * 1e12)
@@ -424,7 +425,8 @@ def main():
         achieved = gu_bytes / (gu_ms / gu_n / 1000.0) / 1e9
         roofline = {"bound": "hbm", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                    "peak_kind": f"hbm_gbs ({peaks['src']})", "traffic": traffic}
+                    "peak_kind": f"hbm_gbs ({peaks['src']})", "traffic": traffic,
+                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01d)", "algorithmic_bytes": gu_bytes}
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
