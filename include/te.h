@@ -140,6 +140,11 @@ enum {
                               aid; read with te_debug_tap(TE_TAP_TRACE)); default 0                 */
   TE_OPT_ATTN_IMPL = 6,    /* attention kernel: 1 (default) = tcgen05 kernel (S, P, O in tensor memory)
                               when Hq/Hkv is a power of two <= 8, 0 = mma.sync flash kernel          */
+  TE_OPT_STREAM_K = 8,     /* 1: the CTA-pair GEMM kernels give every SM pair an equal contiguous share of the
+                              (tile, k-block) work units (stream-K); a tile cut by a share boundary is completed
+                              by the pair that holds its first k-blocks, on top of the other pieces' fp32 partials
+                              summed in a fixed order (deterministic).  0 (default): whole tiles, round-robin —
+                              measured faster on every config                                    */
   TE_OPT_SPLIT_K = 7       /* 1 (default): small batches (fewer 128-row tiles than SMs in a GEMM, no
                               CTA pairs) run the split-K kernel: several CTAs per output tile, each
                               streaming its own K-slice of the weights; partial tiles are summed in a
@@ -183,8 +188,9 @@ int te_debug_tap(te_handle* h, int what, void* dst_host, size_t n_bytes);
 
 /* Test-only: C[M,N] (DEVICE fp32, row-major) = A[M,K] * B[N,K]^T with A, B DEVICE bf16
  * row-major, through the same TMA + tcgen05 main loop as the stack's GEMMs (plain epilogue).
- * K % 64 == 0, N % block_n == 0, block_n in {128, 256}; cta_pair selects the cta_group::2
- * kernel (256-row tiles).  Synchronous. */
+ * K % 64 == 0, N % block_n == 0, block_n in {128, 256}; cta_pair = 1 selects the cta_group::2
+ * kernel (256-row tiles) with whole tiles per pair, cta_pair = 2 the same kernel with stream-K
+ * scheduling.  Synchronous. */
 int te_debug_gemm(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
                   int32_t n, int32_t k, int32_t block_n, int32_t cta_pair);
 

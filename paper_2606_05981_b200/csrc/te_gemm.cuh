@@ -63,6 +63,9 @@ struct GemmParams {
   int splits;
   float* sk_scratch;
   int* sk_sem;
+  // stream-K scheduling of the CTA-pair kernel: 1 = every pair gets an equal contiguous share of the
+  // (tile, k-block) work units; tiles cut by a share boundary are completed through sk_scratch / sk_sem
+  int streamk;
 };
 constexpr int TRACE_SLOTS = 96;  // [0,48): globaltimer ns, [48,96): SM clock of the same stamp
 __device__ __forceinline__ void trace_stamp(const GemmParams& p, int slot) {
@@ -573,6 +576,55 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 // the leader's TMEM and rows 128-255 into the peer's.  Per SM this moves A 16 KB + B BN/2 x 128 B per
 // 64-deep k-block instead of A 16 KB + B BN x 128 B: 1.5x less L2->SM traffic at BN = 256.
 constexpr int GEMM2_EPI_WARPS = 8;  // two per TMEM lane quadrant: the epilogue is issue-latency-bound per warp
+
+// Work of one CTA pair as a sequence of segments (tile, k-blocks [kb0, kb1)).
+//   classic : whole tiles pair, pair + num_pairs, ...
+//   stream-K: the pair's equal share [U*pair/NP, U*(pair+1)/NP) of the U = tiles * num_kb work units, cut at
+//             tile boundaries.  A tile cut by a share boundary has one HEAD piece (kb0 == 0; it is the LAST
+//             segment of its pair, which owns the tile's epilogue) and one or more later pieces, each the FIRST
+//             segment of the following pairs: those store their fp32 partial tile to the pair's scratch slot and
+//             raise the pair's flag; the owner's epilogue warps sum them in pair order INTO the accumulator buffer
+//             before the head piece's MMAs start (they accumulate on top; fixed order -> deterministic), i.e.
+//             while the owner's previous segment is still in its main loop: the fix-up is off the critical
+//             path.  A pair never waits before its first segment is published, so the waits cannot cycle.
+struct SegIter {
+  long long u, u_end;
+  int num_kb, tile_next, tile_step, num_tiles, streamk;
+  __device__ __forceinline__ SegIter(int pair, int num_pairs, int num_tiles_, int num_kb_, int streamk_)
+      : num_kb(num_kb_), tile_next(pair), tile_step(num_pairs), num_tiles(num_tiles_), streamk(streamk_) {
+    const long long U = (long long)num_tiles_ * num_kb_;
+    u = U * pair / num_pairs;
+    u_end = U * (pair + 1) / num_pairs;
+  }
+  __device__ __forceinline__ bool next(int& tile, int& kb0, int& kb1) {
+    if (!streamk) {
+      if (tile_next >= num_tiles) return false;
+      tile = tile_next; kb0 = 0; kb1 = num_kb;
+      tile_next += tile_step;
+      return true;
+    }
+    if (u >= u_end) return false;
+    tile = static_cast<int>(u / num_kb);
+    kb0 = static_cast<int>(u - (long long)tile * num_kb);
+    const long long e = min(u_end, (long long)(tile + 1) * num_kb);
+    kb1 = kb0 + static_cast<int>(e - u);
+    u = e;
+    return true;
+  }
+};
+__device__ __forceinline__ void gemm2_epi_bar() {  // named barrier 1: the epilogue warps of one CTA
+  asm volatile("bar.sync 1, %0;" ::"n"(32 * GEMM2_EPI_WARPS) : "memory");
+}
+__device__ __forceinline__ void tmem_st32_(uint32_t taddr, const uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
+      "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
+      "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+      : "memory");
+}
 constexpr int GEMM2_THREADS = 64 + 32 * GEMM2_EPI_WARPS;
 
 template <int BN, int EPI>
@@ -653,26 +705,29 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
+      SegIter seg(pair, num_pairs, num_tiles, num_kb, p.streamk);
+      int tile, kb0, kb1;
+      bool have = seg.next(tile, kb0, kb1);
       // weights first (independent of the predecessor kernel), then the dependency wait, then A
-      const int pre = (pair < num_tiles) ? (num_kb < STAGES ? num_kb : STAGES) : 0;
-      {
-        const int b_row0 = (pair / num_mp) * BN + rank * (BN / 2);
-        for (int kb = 0; kb < pre; ++kb) {
-          if (leader) mbar_arrive_expect_tx(&full[kb], 2 * Cfg::STAGE_BYTES);
-          tma_load_2d_cg2(sB + kb * Cfg::B_BYTES, &tmB, mapa_u32(smem_u32(&full[kb]), 0), kb * GEMM_BK, b_row0);
+      const int pre = have ? ((kb1 - kb0) < STAGES ? (kb1 - kb0) : STAGES) : 0;
+      if (have) {
+        const int b_row0 = (tile / num_mp) * BN + rank * (BN / 2);
+        for (int i = 0; i < pre; ++i) {
+          if (leader) mbar_arrive_expect_tx(&full[i], 2 * Cfg::STAGE_BYTES);
+          tma_load_2d_cg2(sB + i * Cfg::B_BYTES, &tmB, mapa_u32(smem_u32(&full[i]), 0), (kb0 + i) * GEMM_BK, b_row0);
         }
       }
       pdl_wait();
       trace_stamp(p, 2);
       bool first = true;
-      for (int tile = pair; tile < num_tiles; tile += num_pairs) {
+      for (; have; have = seg.next(tile, kb0, kb1)) {
         const int mp = tile % num_mp;
         const int n_blk = tile / num_mp;
         const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
         const int b_row = n_blk * BN + rank * (BN / 2);
-        for (int kb = 0; kb < num_kb; ++kb) {
+        for (int kb = kb0; kb < kb1; ++kb) {
           const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
-          if (first && kb < pre) {
+          if (first && kb - kb0 < pre) {
             tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
           } else {
             mbar_wait(&empty[stage], phase ^ 1);
@@ -692,21 +747,26 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
+      SegIter seg(pair, num_pairs, num_tiles, num_kb, p.streamk);
+      int tile, kb0, kb1;
+      for (; seg.next(tile, kb0, kb1); ++it) {
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
-        mbar_wait(&tempty[acc], acc_phase ^ 1);
+        // the epilogue warps hand over each accumulator buffer explicitly (also before its first use): a
+        // stream-K head piece finds the other pieces' partial sums already in the buffer and accumulates on them
+        mbar_wait(&tempty[acc], acc_phase);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * BN;
-        for (int kb = 0; kb < num_kb; ++kb) {
+        const bool preloaded = kb0 == 0 && kb1 != num_kb;
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&full[stage], phase);
-          if (kb == 0 && it < 10) trace_stamp(p, 3 + it);
+          if (kb == kb0 && it < 10) trace_stamp(p, 3 + it);
           tc_fence_after();
           const uint64_t a_desc = umma_smem_desc_sw128(smem_u32(sA + stage * Cfg::A_BYTES));
           const uint64_t b_desc = umma_smem_desc_sw128(smem_u32(sB + stage * Cfg::B_BYTES));
 #pragma unroll
           for (int k = 0; k < GEMM_BK / 16; ++k)
-            umma_bf16_cg2(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+            umma_bf16_cg2(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (preloaded || kb > kb0 || k != 0) ? 1u : 0u);
           umma_commit_cg2(&empty[stage], 0x3);  // frees this stage in BOTH CTAs
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
@@ -718,14 +778,99 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int quad = warp & 3;         // TMEM lane quadrant this warp may read
     const int part = (warp - 2) >> 2;  // which share of the tile's columns (two warps per quadrant)
     constexpr int NPARTS = GEMM2_EPI_WARPS / 4;
+    constexpr int COLS = BN / NPARTS;
+    constexpr size_t SLOT_F4 = (size_t)(BN / 4) * GEMM_BM;  // one CTA's fp32 partial tile: float4 [BN/4][128 rows]
+    const int row_in_tile = quad * 32 + lane;
     int it = 0;
     pdl_wait();
-    for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
+    // Hand-over of an accumulator buffer to the MMA issuer for the segment (tile_n, [kb0_n, kb1_n)) that will use
+    // it next.  If that segment is a stream-K head piece, the later pieces of its tile (pairs q = pair+1, ... —
+    // each one the FIRST segment of its pair, so long done by the time this pair reaches its last one) are
+    // summed in pair order into the buffer first; the MMAs then accumulate on top (fixed order: deterministic).
+    auto hand_over = [&](bool have_n, int tile_n, int kb0_n, int kb1_n, int acc_n) {
+      if (have_n && kb0_n == 0 && kb1_n != num_kb) {
+        const uint32_t t_row_n = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc_n * BN;
+        const long long U = (long long)num_tiles * num_kb;
+        const long long tile_end = (long long)(tile_n + 1) * num_kb;
+        bool first_piece = true;
+        for (int q = pair + 1; q < num_pairs && U * q / num_pairs < tile_end; ++q) {
+          const int src_cta = 2 * q + static_cast<int>(rank);
+          if (warp == 2 && lane == 0) {
+            int v;
+            do {
+              asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p.sk_sem + src_cta) : "memory");
+            } while (v == 0);
+          }
+          gemm2_epi_bar();
+          const float4* src = reinterpret_cast<const float4*>(p.sk_scratch) + (size_t)src_cta * SLOT_F4;
+#pragma unroll 1
+          for (int c0 = part * COLS; c0 < (part + 1) * COLS; c0 += 32) {
+            float4 v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) v[j] = __ldcg(src + (size_t)(c0 / 4 + j) * GEMM_BM + row_in_tile);
+            uint32_t r[32];
+            if (first_piece) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) r[j] = 0u;
+            } else {
+              tmem_ld32(t_row_n + c0, r);
+              tmem_ld_wait();
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              r[4 * j] = __float_as_uint(__uint_as_float(r[4 * j]) + v[j].x);
+              r[4 * j + 1] = __float_as_uint(__uint_as_float(r[4 * j + 1]) + v[j].y);
+              r[4 * j + 2] = __float_as_uint(__uint_as_float(r[4 * j + 2]) + v[j].z);
+              r[4 * j + 3] = __float_as_uint(__uint_as_float(r[4 * j + 3]) + v[j].w);
+            }
+            tmem_st32_(t_row_n + c0, r);
+          }
+          tmem_st_wait();
+          gemm2_epi_bar();  // every warp has read the slot
+          if (warp == 2 && lane == 0) p.sk_sem[src_cta] = 0;  // re-armed for the next launch
+          first_piece = false;
+        }
+      }
+      tc_fence_before();
+      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc_n]), 0));
+    };
+    SegIter seg(pair, num_pairs, num_tiles, num_kb, p.streamk);
+    SegIter ahead(pair, num_pairs, num_tiles, num_kb, p.streamk);  // runs two segments ahead of `seg`
+    int tile, kb0, kb1;
+    int tile_n, kb0_n, kb1_n;
+    for (int i = 0; i < 2; ++i) {  // the first use of both buffers
+      const bool have_n = ahead.next(tile_n, kb0_n, kb1_n);
+      hand_over(have_n, tile_n, kb0_n, kb1_n, i);
+    }
+    for (; seg.next(tile, kb0, kb1); ++it) {
       const int mp = tile % num_mp;
       const int n_blk = tile / num_mp;
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
       const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
+      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
+      const bool have_n = ahead.next(tile_n, kb0_n, kb1_n);  // the segment that reuses this buffer
+      if (kb0 != 0) {
+        // ---- stream-K: a later piece of a tile owned by an earlier pair -> publish the fp32 partial
+        mbar_wait(&tfull[acc], acc_phase);
+        tc_fence_after();
+        float4* dst = reinterpret_cast<float4*>(p.sk_scratch) + (size_t)blockIdx.x * SLOT_F4;
+#pragma unroll 1
+        for (int c0 = part * COLS; c0 < (part + 1) * COLS; c0 += 32) {
+          uint32_t r[32];
+          tmem_ld32(t_row + c0, r);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            __stcg(dst + (size_t)(c0 / 4 + j) * GEMM_BM + row_in_tile,
+                   make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]), __uint_as_float(r[4 * j + 2]),
+                               __uint_as_float(r[4 * j + 3])));
+        }
+        gemm2_epi_bar();  // orders every warp's stores before the elected thread's gpu-scope release
+        if (warp == 2 && lane == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.sk_sem + blockIdx.x), "r"(1) : "memory");
+        hand_over(have_n, tile_n, kb0_n, kb1_n, acc);
+        continue;
+      }
       // operands that do not depend on the accumulator are fetched while the main loop still runs
       float rstd = 0.f;
       ResidPrefetch pf;
@@ -734,14 +879,12 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       mbar_wait(&tfull[acc], acc_phase);
       if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 14 + it);
       tc_fence_after();
-      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
       float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
       if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk, part, NPARTS);
       if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
       if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
       if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
-      tc_fence_before();
-      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
+      hand_over(have_n, tile_n, kb0_n, kb1_n, acc);
       if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 25 + it);
     }
   }

@@ -78,6 +78,7 @@ struct te_handle {
   int bn_qkv = 256, bn_gu = 256, bn_res = 128;
   int attn_impl = 1;  // 1: tcgen05 kernel (te_attn_tc.cuh) when Hq/Hkv is a power of two <= 8; 0: mma.sync kernel
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
+  int streamk = 0;    // 1: CTA-pair GEMMs balance (tile, k-block) units over all SM pairs (stream-K; measured slower)
   int splitk = 1;     // 1: small batches (no CTA pairs) use the split-K kernel when a GEMM has <= one tile per SM
   float* sk_scratch = nullptr;  // [sm_count][128 x 256] fp32 partial tiles
   int* sk_sem = nullptr;        // [sm_count][2] per-tile arrival / departure counters (zero between launches)
@@ -193,7 +194,11 @@ cudaError_t launch_gemm2(const CUtensorMap& tmA, const CUtensorMap& tmB, const t
                          cudaStream_t st) {
   using Cfg = te::Gemm2Cfg<BN, EPI>;
   const int tiles = ((p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM)) * p.num_n_blk;
-  const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
+  // stream-K: every SM pair takes an equal share of the (tile, k-block) units, so all pairs are used as soon as
+  // there are that many units; classic: one pair per tile at most
+  const long long units = (long long)tiles * (p.K / te::GEMM_BK);
+  const int cap = p.streamk ? (int)(units < sm_count / 2 ? units : sm_count / 2) : tiles;
+  const int pairs = cap < sm_count / 2 ? cap : sm_count / 2;
   return launch_k(te::te_gemm2_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM2_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB,
                   p);
 }
@@ -385,7 +390,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     return TE_ERR_CUDA;
   }
   te::GemmParams base{};
-  base.splits = 1; base.sk_scratch = h->sk_scratch; base.sk_sem = h->sk_sem;
+  base.splits = 1; base.sk_scratch = h->sk_scratch; base.sk_sem = h->sk_sem; base.streamk = h->streamk;
   base.M = T; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = parts; base.ssq_stride = h->ssq_parts_cap;
   base.inv_d = 1.0f / static_cast<float>(d); base.eps = c.rms_eps;
   const size_t trace_stride = (size_t)h->sm_count * te::TRACE_SLOTS;
@@ -859,6 +864,11 @@ int te_set_option(te_handle* h, int option, int value) {
     free_graphs(h);
     return TE_OK;
   }
+  if (option == TE_OPT_STREAM_K) {
+    h->streamk = value ? 1 : 0;
+    free_graphs(h);
+    return TE_OK;
+  }
   if (option == TE_OPT_SPLIT_K) {
     h->splitk = value ? 1 : 0;
     g_split_target = value > 1 ? value : 0;
@@ -946,10 +956,25 @@ int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t
   te::GemmParams p{};
   p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
   p.c = cmat; p.ld_c = n;
+  p.streamk = cta_pair == 2 ? 1 : 0;
+  if (p.streamk) {  // one fp32 partial-tile slot and one flag per CTA
+    const size_t n_cta = prop.multiProcessorCount;
+    if (cudaMalloc(reinterpret_cast<void**>(&p.sk_scratch), n_cta * te::GEMM_BM * block_n * sizeof(float)) != cudaSuccess)
+      return TE_ERR_CUDA;
+    if (cudaMalloc(reinterpret_cast<void**>(&p.sk_sem), n_cta * sizeof(int)) != cudaSuccess) {
+      cudaFree(p.sk_scratch);
+      return TE_ERR_CUDA;
+    }
+    cudaMemset(p.sk_sem, 0, n_cta * sizeof(int));
+  }
   g_pdl = false;
   cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(block_n, cta_pair ? 1 : 0, 128, ta, tb, p, prop.multiProcessorCount, nullptr);
-  if (e != cudaSuccess) return TE_ERR_CUDA;
-  return cudaDeviceSynchronize() == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (p.streamk) {
+    cudaFree(p.sk_scratch);
+    cudaFree(p.sk_sem);
+  }
+  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
 int te_debug_gemm_splitk(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,

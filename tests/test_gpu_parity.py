@@ -31,12 +31,15 @@ def _assert_final(m, tag=""):
 
 
 # --------------------------------------------------------------------------- GEMM main loop
-@pytest.mark.parametrize("pair", [0, 1])
+@pytest.mark.parametrize("pair", [0, 1, 2])
 @pytest.mark.parametrize("M,N,K,bn", [(128, 256, 64, 256), (1, 128, 64, 128), (300, 512, 256, 256),
                                        (300, 512, 256, 128), (517, 768, 832, 256), (3072, 2048, 2048, 256),
-                                       (3072, 2048, 6144, 128)])
+                                       (3072, 2048, 6144, 128), (3072, 2048, 6144, 256), (3072, 4096, 2048, 256),
+                                       (512, 12288, 2048, 256), (1024, 2048, 2048, 256)])
 def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn, pair):
-    """TMA + tcgen05 main loop alone: several tiles, ragged M tail, K spanning >1 pipeline ring."""
+    """TMA + tcgen05 main loop alone: several tiles, ragged M tail, K spanning >1 pipeline ring.
+    pair: 0 = one CTA per tile, 1 = CTA pairs, 2 = CTA pairs with stream-K scheduling (tiles cut by share
+    boundaries, incl. fewer tiles than SM pairs, are completed through the partial-tile scratch)."""
     import torch
     import paper_2606_05981_b200 as te
     rng = np.random.default_rng(M * 7 + N)
@@ -140,16 +143,20 @@ def test_cfg1_full_stack(H, O):
     g.close()
 
 
-@pytest.mark.parametrize("cta_pair,resid_bn,split_k", [(1, 128, 1), (1, 256, 1), (0, 256, 1), (0, 128, 1),
-                                                       (0, 256, 0), (0, 128, 0)])
-def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn, split_k):
-    """Force each GEMM tiling (one CTA per tile / CTA pairs / split-K groups, 128- and 256-wide residual
-    tiles)."""
+@pytest.mark.parametrize("cta_pair,resid_bn,split_k,stream_k", [(1, 128, 1, 1), (1, 256, 1, 1), (1, 128, 1, 0),
+                                                                (1, 256, 1, 0), (0, 256, 1, 1), (0, 128, 1, 1),
+                                                                (0, 256, 0, 1), (0, 128, 0, 1)])
+def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn, split_k, stream_k):
+    """Force each GEMM tiling (one CTA per tile / CTA pairs with and without stream-K / split-K groups,
+    128- and 256-wide residual tiles)."""
     w, blob, tl, T, emb, ch = H.workload_inputs(1)
     ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4)
-    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn, split_k=split_k)
-    _assert_final(PM.stack_metrics(g.encode(emb, tl, 4, 4), ref, emb),
-                  f"pair={cta_pair} bn={resid_bn} split_k={split_k}")
+    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn, split_k=split_k,
+                stream_k=stream_k)
+    out = g.encode(emb, tl, 4, 4)
+    _assert_final(PM.stack_metrics(out, ref, emb),
+                  f"pair={cta_pair} bn={resid_bn} split_k={split_k} stream_k={stream_k}")
+    assert np.array_equal(out, g.encode(emb, tl, 4, 4))    # deterministic (fixed-order partial sums)
     g.close()
 
 
@@ -162,9 +169,10 @@ def test_ragged_stack_cta_pairs(H, O):
     T = len(tl) * gh * gw + sum(tl)
     emb = np.random.default_rng(4).standard_normal((T, m.hidden)).astype(np.float32)
     ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
-    g = H.GpuTE(m, len(tl), T, blob, cta_pair=1)
-    _assert_final(PM.stack_metrics(g.encode(emb, tl, gh, gw), ref, emb), "ragged pairs")
-    g.close()
+    for stream_k in (0, 1):
+        g = H.GpuTE(m, len(tl), T, blob, cta_pair=1, stream_k=stream_k)
+        _assert_final(PM.stack_metrics(g.encode(emb, tl, gh, gw), ref, emb), f"ragged pairs stream_k={stream_k}")
+        g.close()
 
 
 def test_cfg1_final_norm(H, O):
