@@ -123,6 +123,17 @@ int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_le
 int te_encode_host(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w,
                    const float* embeds_host, const int32_t* text_lens_host, float* out_host);
 
+/* Pipelined host path: te_encode_host_submit enqueues [host->device copy | te_encode | device->host copy] of
+ * one batch on three library streams chained by events and returns at once with a slot id (0 or 1);
+ * te_encode_host_wait(slot) blocks until that batch's out_host is complete.  Two batches can be in flight:
+ * submitting batch n+1 before waiting for batch n overlaps the copies of one with the kernels of the other
+ * (te_encode_host = submit + wait).  The HOST buffers must stay valid until the wait (pinned memory for real
+ * overlap).  A third submit without a wait returns TE_ERR_INVALID_ARG. */
+int te_encode_host_submit(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w,
+                          const float* embeds_host, const int32_t* text_lens_host, float* out_host,
+                          int32_t* slot_out);
+int te_encode_host_wait(te_handle* h, int32_t slot);
+
 /* Synchronises the device and returns TE_ERR_DEVICE_CHECK if the device-side validation flag
  * was raised since the last query (and clears it), TE_ERR_CUDA on a CUDA error, else TE_OK. */
 int te_query_async_error(te_handle* h);

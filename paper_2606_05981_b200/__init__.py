@@ -32,7 +32,7 @@ TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "fi
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 
 EXPORTS = [
-    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host",
+    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host", "te_encode_host_submit", "te_encode_host_wait",
     "te_query_async_error", "te_set_option", "te_kernel_launches", "te_kernel_times", "te_debug_set_range",
     "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_destroy", "te_strerror", "te_last_error",
 ]
@@ -81,6 +81,10 @@ def lib() -> ctypes.CDLL:
     L.te_encode_prefix.argtypes = [c_void_p, c_void_p, c_int32, c_void_p, c_void_p]
     L.te_encode_host.restype = c_int
     L.te_encode_host.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_void_p]
+    L.te_encode_host_submit.restype = c_int
+    L.te_encode_host_submit.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_void_p, c_void_p]
+    L.te_encode_host_wait.restype = c_int
+    L.te_encode_host_wait.argtypes = [c_void_p, c_int32]
     L.te_query_async_error.restype = c_int
     L.te_query_async_error.argtypes = [c_void_p]
     L.te_set_option.restype = c_int
@@ -175,6 +179,17 @@ def te_encode_host(h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out
                                 _ptr(out_host)), h)
 
 
+def te_encode_host_submit(h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host) -> int:
+    slot = c_int32(-1)
+    _check(lib().te_encode_host_submit(h, n_frames, grid_h, grid_w, _ptr(embeds_host), _ptr(text_lens_host),
+                                       _ptr(out_host), byref(slot)), h)
+    return int(slot.value)
+
+
+def te_encode_host_wait(h, slot: int):
+    _check(lib().te_encode_host_wait(h, slot), h)
+
+
 def te_query_async_error(h) -> int:
     return int(lib().te_query_async_error(h))
 
@@ -244,6 +259,12 @@ class TextEncoder:
 
     def encode_host(self, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host):
         te_encode_host(self.h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host)
+
+    def encode_host_submit(self, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host) -> int:
+        return te_encode_host_submit(self.h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host)
+
+    def encode_host_wait(self, slot: int):
+        te_encode_host_wait(self.h, slot)
 
     def close(self):
         if self.h:

@@ -106,9 +106,14 @@ struct te_handle {
   int32_t* prefix_lens = nullptr; // device [1]
   int prefix_len = 0;
   // host-path staging
-  float *stg_embeds = nullptr, *stg_out = nullptr;
-  int32_t* stg_lens = nullptr;
-  cudaStream_t own_stream = nullptr;
+  struct HostSlot {  // one batch in flight on the host path: device staging + the events that chain its three stages
+    float *embeds = nullptr, *out = nullptr;
+    int32_t* lens = nullptr;
+    cudaEvent_t h2d_done = nullptr, compute_done = nullptr, d2h_done = nullptr;
+    bool busy = false;
+  } slot[2];
+  int next_slot = 0;
+  cudaStream_t own_stream = nullptr, h2d_stream = nullptr, d2h_stream = nullptr;
   // graphs
   std::vector<GraphEntry> cache;
   uint64_t stamp = 0;
@@ -782,9 +787,9 @@ int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_le
   return TE_OK;
 }
 
-int te_encode_host(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds_host,
-                   const int32_t* text_lens_host, float* out_host) {
-  if (!h || !embeds_host || !text_lens_host || !out_host) return TE_ERR_INVALID_ARG;
+int te_encode_host_submit(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds_host,
+                          const int32_t* text_lens_host, float* out_host, int32_t* slot_out) {
+  if (!h || !embeds_host || !text_lens_host || !out_host || !slot_out) return TE_ERR_INVALID_ARG;
   if (!h->loaded) return TE_ERR_NOT_LOADED;
   const te_config& c = h->cfg;
   if (n_frames < 1 || n_frames > c.max_frames || grid_h < 1 || grid_w < 1) return TE_ERR_INVALID_ARG;
@@ -795,20 +800,54 @@ int te_encode_host(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_
   }
   if (T < 1 || T > c.max_tokens) return TE_ERR_INVALID_ARG;
   TE_CUDA(h, cudaSetDevice(h->device));
-  if (!h->stg_embeds) {
-    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->stg_embeds), (size_t)c.max_tokens * c.hidden * sizeof(float)));
-    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->stg_out), (size_t)c.max_tokens * c.hidden * sizeof(float)));
-    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->stg_lens), (size_t)c.max_frames * sizeof(int32_t)));
+  const int si = h->next_slot;
+  te_handle::HostSlot& sl = h->slot[si];
+  if (sl.busy) return TE_ERR_INVALID_ARG;  // both slots in flight: te_encode_host_wait first
+  if (!h->h2d_stream) {
+    TE_CUDA(h, cudaStreamCreateWithFlags(&h->h2d_stream, cudaStreamNonBlocking));
+    TE_CUDA(h, cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking));
+  }
+  if (!sl.embeds) {
+    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&sl.embeds), (size_t)c.max_tokens * c.hidden * sizeof(float)));
+    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&sl.out), (size_t)c.max_tokens * c.hidden * sizeof(float)));
+    TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&sl.lens), (size_t)c.max_frames * sizeof(int32_t)));
+    TE_CUDA(h, cudaEventCreateWithFlags(&sl.h2d_done, cudaEventDisableTiming));
+    TE_CUDA(h, cudaEventCreateWithFlags(&sl.compute_done, cudaEventDisableTiming));
+    TE_CUDA(h, cudaEventCreateWithFlags(&sl.d2h_done, cudaEventDisableTiming));
   }
   const size_t bytes = (size_t)T * c.hidden * sizeof(float);
-  cudaStream_t st = h->own_stream;
-  TE_CUDA(h, cudaMemcpyAsync(h->stg_lens, text_lens_host, n_frames * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  TE_CUDA(h, cudaMemcpyAsync(h->stg_embeds, embeds_host, bytes, cudaMemcpyHostToDevice, st));
-  int rc = te_encode(h, n_frames, grid_h, grid_w, h->stg_embeds, h->stg_lens, (int32_t)T, h->stg_out, st);
+  // stage 1: host -> device on the copy-in stream (the slot's previous batch was waited for, so its buffers are free)
+  TE_CUDA(h, cudaMemcpyAsync(sl.lens, text_lens_host, n_frames * sizeof(int32_t), cudaMemcpyHostToDevice, h->h2d_stream));
+  TE_CUDA(h, cudaMemcpyAsync(sl.embeds, embeds_host, bytes, cudaMemcpyHostToDevice, h->h2d_stream));
+  TE_CUDA(h, cudaEventRecord(sl.h2d_done, h->h2d_stream));
+  // stage 2: the stack on the compute stream (batches are serialised there: they share the workspace)
+  TE_CUDA(h, cudaStreamWaitEvent(h->own_stream, sl.h2d_done, 0));
+  int rc = te_encode(h, n_frames, grid_h, grid_w, sl.embeds, sl.lens, (int32_t)T, sl.out, h->own_stream);
   if (rc != TE_OK) return rc;
-  TE_CUDA(h, cudaMemcpyAsync(out_host, h->stg_out, bytes, cudaMemcpyDeviceToHost, st));
-  TE_CUDA(h, cudaStreamSynchronize(st));
+  TE_CUDA(h, cudaEventRecord(sl.compute_done, h->own_stream));
+  // stage 3: device -> host on the copy-out stream
+  TE_CUDA(h, cudaStreamWaitEvent(h->d2h_stream, sl.compute_done, 0));
+  TE_CUDA(h, cudaMemcpyAsync(out_host, sl.out, bytes, cudaMemcpyDeviceToHost, h->d2h_stream));
+  TE_CUDA(h, cudaEventRecord(sl.d2h_done, h->d2h_stream));
+  sl.busy = true;
+  h->next_slot = si ^ 1;
+  *slot_out = si;
   return TE_OK;
+}
+
+int te_encode_host_wait(te_handle* h, int32_t slot) {
+  if (!h || slot < 0 || slot > 1 || !h->slot[slot].busy) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaEventSynchronize(h->slot[slot].d2h_done));
+  h->slot[slot].busy = false;
+  return TE_OK;
+}
+
+int te_encode_host(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds_host,
+                   const int32_t* text_lens_host, float* out_host) {
+  int32_t slot = 0;
+  int rc = te_encode_host_submit(h, n_frames, grid_h, grid_w, embeds_host, text_lens_host, out_host, &slot);
+  if (rc != TE_OK) return rc;
+  return te_encode_host_wait(h, slot);
 }
 
 int te_query_async_error(te_handle* h) {
@@ -1018,11 +1057,15 @@ void te_destroy(te_handle* h) {
   free_graphs(h);
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
-                  h->act, h->stg_embeds, h->stg_out, h->stg_lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix,
-                  h->prefix_buf, h->prefix_lens};
+                  h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
+                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens};
   for (void* p : ptrs)
     if (p) cudaFree(p);
-  if (h->own_stream) cudaStreamDestroy(h->own_stream);
+  for (auto& sl : h->slot)
+    for (cudaEvent_t e : {sl.h2d_done, sl.compute_done, sl.d2h_done})
+      if (e) cudaEventDestroy(e);
+  for (cudaStream_t st : {h->own_stream, h->h2d_stream, h->d2h_stream})
+    if (st) cudaStreamDestroy(st);
   delete h;
 }
 

@@ -448,3 +448,34 @@ def test_prefix_28_layers_ragged_sampled_frames(H, O):
         print(f"prefix cfg5 frame {b}: {met}")
         _assert_final(met, f"prefix 28L frame {b}")
     g.close()
+
+
+def test_pipelined_host_path_matches_blocking_call(H):
+    """te_encode_host_submit / _wait with two batches in flight == te_encode_host, bitwise; a third submit
+    without a wait is refused."""
+    import torch
+    import paper_2606_05981_b200 as te
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    g = H.GpuTE(w.model, w.n_frames, T, blob)
+    embs = [emb, (emb * 0.5 + 0.25).astype(np.float32), emb[::-1].copy()]
+    want = []
+    for e in embs:
+        o = np.empty_like(e)
+        g.enc.encode_host(w.n_frames, w.grid_h, w.grid_w, e, tl, o)
+        want.append(o)
+    ins = [torch.from_numpy(e).pin_memory() for e in embs]
+    outs = [torch.empty_like(i).pin_memory() for i in ins]
+    s0 = g.enc.encode_host_submit(w.n_frames, w.grid_h, w.grid_w, ins[0], tl, outs[0])
+    s1 = g.enc.encode_host_submit(w.n_frames, w.grid_h, w.grid_w, ins[1], tl, outs[1])
+    assert {s0, s1} == {0, 1}
+    with pytest.raises(te.TEError):
+        g.enc.encode_host_submit(w.n_frames, w.grid_h, w.grid_w, ins[2], tl, outs[2])
+    g.enc.encode_host_wait(s0)
+    s2 = g.enc.encode_host_submit(w.n_frames, w.grid_h, w.grid_w, ins[2], tl, outs[2])
+    g.enc.encode_host_wait(s1)
+    g.enc.encode_host_wait(s2)
+    for o, wnt in zip(outs, want):
+        assert np.array_equal(o.numpy(), wnt)
+    with pytest.raises(te.TEError):
+        g.enc.encode_host_wait(s2)                      # nothing in flight in that slot any more
+    g.close()
