@@ -66,6 +66,9 @@ struct GemmParams {
   // stream-K scheduling of the CTA-pair kernel: 1 = every pair gets an equal contiguous share of the
   // (tile, k-block) work units; tiles cut by a share boundary are completed through sk_scratch / sk_sem
   int streamk;
+  // EPI_SWIGLU with 128-wide tiles over weights interleaved per 256 rows (128 gate | 128 up): tile n' takes gate
+  // rows (n'>>1)*256 + (n'&1)*64 .. +64 and the matching up rows 128 further on, as two 64-row halves
+  int gu_half;
 };
 constexpr int TRACE_SLOTS = 96;  // [0,48): globaltimer ns, [48,96): SM clock of the same stamp
 __device__ __forceinline__ void trace_stamp(const GemmParams& p, int slot) {
@@ -711,7 +714,9 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // weights first (independent of the predecessor kernel), then the dependency wait, then A
       const int pre = have ? ((kb1 - kb0) < STAGES ? (kb1 - kb0) : STAGES) : 0;
       if (have) {
-        const int b_row0 = (tile / num_mp) * BN + rank * (BN / 2);
+        const int nb0 = tile / num_mp;
+        const int b_row0 = p.gu_half ? (nb0 >> 1) * 256 + static_cast<int>(rank) * 128 + (nb0 & 1) * 64
+                                     : nb0 * BN + static_cast<int>(rank) * (BN / 2);
         for (int i = 0; i < pre; ++i) {
           if (leader) mbar_arrive_expect_tx(&full[i], 2 * Cfg::STAGE_BYTES);
           tma_load_2d_cg2(sB + i * Cfg::B_BYTES, &tmB, mapa_u32(smem_u32(&full[i]), 0), (kb0 + i) * GEMM_BK, b_row0);
@@ -724,7 +729,8 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         const int mp = tile % num_mp;
         const int n_blk = tile / num_mp;
         const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
-        const int b_row = n_blk * BN + rank * (BN / 2);
+        const int b_row = p.gu_half ? (n_blk >> 1) * 256 + static_cast<int>(rank) * 128 + (n_blk & 1) * 64
+                                    : n_blk * BN + static_cast<int>(rank) * (BN / 2);
         for (int kb = kb0; kb < kb1; ++kb) {
           const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
           if (first && kb - kb0 < pre) {

@@ -374,10 +374,21 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (elect_one()) {
+      // B tile of one k-block: BN weight rows in one box, or (gu_half: 128-wide SwiGLU tile over weights
+      // interleaved per 256 rows; tmB then has 64-row boxes) the 64 gate rows and the 64 matching up rows
+      auto load_b = [&](uint8_t* dst, uint64_t* bar, int kb) {
+        if (p.gu_half) {
+          const int g_row = (n_blk >> 1) * 256 + (n_blk & 1) * 64;
+          tma_load_2d(dst, &tmB, bar, kb * GEMM_BK, g_row);
+          tma_load_2d(dst + 64 * GEMM_BK * 2, &tmB, bar, kb * GEMM_BK, g_row + 128);
+        } else {
+          tma_load_2d(dst, &tmB, bar, kb * GEMM_BK, n_blk * BN);
+        }
+      };
       const int pre = nkb < STAGES ? nkb : STAGES;
       for (int i = 0; i < pre; ++i) {  // weights first: independent of the predecessor kernel
         mbar_arrive_expect_tx(&full[i], Cfg::STAGE_BYTES);
-        tma_load_2d(sB + i * Cfg::B_BYTES, &tmB, &full[i], (kb0 + i) * GEMM_BK, n_blk * BN);
+        load_b(sB + i * Cfg::B_BYTES, &full[i], kb0 + i);
       }
       pdl_wait();
       trace_stamp(p, 2);
@@ -387,7 +398,7 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         if (i >= pre) {
           mbar_wait(&empty[stage], phase ^ 1);
           mbar_arrive_expect_tx(&full[stage], Cfg::STAGE_BYTES);
-          tma_load_2d(sB + stage * Cfg::B_BYTES, &tmB, &full[stage], (kb0 + i) * GEMM_BK, n_blk * BN);
+          load_b(sB + stage * Cfg::B_BYTES, &full[stage], kb0 + i);
         }
         tma_load_2d(sA + stage * Cfg::A_BYTES, &tmA, &full[stage], (kb0 + i) * GEMM_BK, m_blk * GEMM_BM);
         if (++stage == STAGES) { stage = 0; phase ^= 1; }

@@ -347,13 +347,19 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const bool kmode = !pair && h->splitk;
   const int bn_qkv = (kmode && num_m * (n_qkv / 128) <= h->sm_count) ? 128 : h->bn_qkv;
   const bool k_qkv = kmode && num_m * (n_qkv / bn_qkv) <= h->sm_count;
-  const bool k_gu = kmode && num_m * (2 * F / h->bn_gu) <= h->sm_count;
+  // gate/up tile width: the weights are interleaved per bn_gu = 256 rows; 128-wide tiles read them as two 64-row
+  // halves (gu_half).  With one row block (T <= 128) 96 one-CTA tiles stream the weights with no split-K exchange
+  // (cfg 2: 27 -> 19 us).  (128-wide CTA-pair tiles at T = 512, 3 waves instead of 2 imbalanced ones, measured
+  // the same as 256-wide ones: they are L2->SM-bound.)
+  const bool gu128_k = kmode && h->bn_gu == 256 && num_m * (2 * F / 128) <= h->sm_count;
+  const int bn_gu = gu128_k ? 128 : h->bn_gu;
+  const bool k_gu = kmode && num_m * (2 * F / bn_gu) <= h->sm_count;
   const bool k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;
   const int bx_qkv = box_index(pair ? bn_qkv / 2 : bn_qkv);
   // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
   // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
   const bool pair_gu = pair || (kmode && !k_gu && T > te::GEMM_BM && h->pair_mode == 2);
-  const int bx_gu = box_index(pair_gu ? h->bn_gu / 2 : h->bn_gu);
+  const int bx_gu = (bn_gu != h->bn_gu) ? 0 : box_index(pair_gu ? h->bn_gu / 2 : h->bn_gu);  // gu_half: 64-row boxes
   const int bx_res = box_index(pair ? h->bn_res / 2 : h->bn_res);
   // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
   const int parts = (d / h->bn_res) * ((pair || k_res) ? 2 : 1);
@@ -487,15 +493,15 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     if (dbg_stop && l == le - 1) break;
     {  // a4: RMSNorm -> gate/up GEMM -> SiLU(gate) * up
       te::GemmParams p = base;
-      p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / h->bn_gu;
+      p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / bn_gu; p.gu_half = (bn_gu != h->bn_gu) ? 1 : 0;
       p.act = h->act; p.ld_act = F;
       p.trace = trace_ptr(2);
       tick();
       if (k_gu) {
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
-        TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(h->bn_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, st));
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(bn_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, st));
       } else {
-        TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(h->bn_gu, pair_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
+        TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(bn_gu, pair_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
       }
       tock(TE_KCLASS_GATEUP);
       ++nk;
