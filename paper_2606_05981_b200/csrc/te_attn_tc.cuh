@@ -28,6 +28,15 @@ struct AttnTcParams {
   int g_shift;  // log2(Hq / Hkv)
   int total_tokens;
   float scale_log2;  // log2(e) / sqrt(dh)
+  // Shared text prefix (te_encode_prefix), handled as a SECOND launch of this kernel per layer:
+  //   launch 1 (prefix_mode 0, stats != null): frame-local causal attention as usual, plus the row statistics
+  //            (max raw score, sum of exp) of every (token, q head) -> stats[T, Hq]
+  //   launch 2 (prefix_mode 1): tmKV addresses the layer's prefix cache [P, 2*Hkv*dh] (k heads | v heads); every
+  //            query sees all P keys (no mask); the epilogue merges with launch 1's normalised output in place:
+  //            out = (l_f e^(m_f-m) out_f + e^(m_p-m) O_p) / (l_f e^(m_f-m) + l_p e^(m_p-m)),  m = max(m_f, m_p)
+  float2* stats;
+  int prefix_mode;
+  int prefix_len;
 };
 
 template <int DH>
@@ -117,8 +126,13 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int n_tiles = (S + PT - 1) / PT;
   const int n_my = (n_tiles > split) ? (n_tiles - split + n_split - 1) / n_split : 0;
   const int S16 = (S + 15) & ~15;
-  // keys tile j can see: positions < PT * (j + 1), rounded to the MMA granularity (16) and capped at the frame
-  auto nk_of = [&](int j) { return min(S16, (PT * (j + 1) + 15) & ~15); };
+  const int P16 = (p.prefix_len + 15) & ~15;
+  // keys tile j can see: positions < PT * (j + 1), rounded to the MMA granularity (16) and capped at the frame;
+  // prefix mode: all P prefix keys for every tile
+  auto nk_of = [&](int j) { return p.prefix_mode ? P16 : min(S16, (PT * (j + 1) + 15) & ~15); };
+  const int kv_row0 = p.prefix_mode ? 0 : seq0;                                   // first K/V row in tmKV
+  const int k_col0 = (p.prefix_mode ? kvh : p.n_q_heads + kvh) * DH;              // this kv head's K columns
+  const int v_col0 = (p.prefix_mode ? p.n_kv_heads + kvh : p.n_q_heads + p.n_kv_heads + kvh) * DH;
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -139,15 +153,13 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_arrive_expect_tx(&k_full[kb], Cfg::KV_BLOCK_BYTES);
         for (int s = 0; s < SLABS; ++s)
-          tma_load_2d(sK + s * Cfg::KV_SLAB_BYTES + kb * 8192, &tmKV, &k_full[kb], (p.n_q_heads + kvh) * DH + 64 * s,
-                      seq0 + 64 * kb);
+          tma_load_2d(sK + s * Cfg::KV_SLAB_BYTES + kb * 8192, &tmKV, &k_full[kb], k_col0 + 64 * s, kv_row0 + 64 * kb);
       }
       if (n_my > 1) load_q(1);
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_arrive_expect_tx(&v_full[kb], Cfg::KV_BLOCK_BYTES);
         for (int s = 0; s < SLABS; ++s)
-          tma_load_2d(sV + s * Cfg::KV_SLAB_BYTES + kb * 8192, &tmKV, &v_full[kb],
-                      (p.n_q_heads + p.n_kv_heads + kvh) * DH + 64 * s, seq0 + 64 * kb);
+          tma_load_2d(sV + s * Cfg::KV_SLAB_BYTES + kb * 8192, &tmKV, &v_full[kb], v_col0 + 64 * s, kv_row0 + 64 * kb);
       }
       for (int i = 2; i < n_my; ++i) load_q(i);
     }
@@ -208,7 +220,7 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       const int j = split + i * n_split;
       const int nk = nk_of(j);
       const int pos = j * PT + pr;      // position of this row's query inside the frame
-      const int lim = min(pos, S - 1);  // keys 0..lim are visible
+      const int lim = p.prefix_mode ? p.prefix_len - 1 : min(pos, S - 1);  // keys 0..lim are visible
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + 256 * t;
       mbar_wait(&s_full[t], u & 1);
       tc_fence_after();
@@ -248,8 +260,24 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // ---- epilogue: O / l -> bf16 -> global
       mbar_wait(&o_full[t], u & 1);
       tc_fence_after();
-      const float inv = 1.0f / l;
-      __nv_bfloat16* dst = p.out + (size_t)(seq0 + pos) * (p.n_q_heads * DH) + ((kvh << g_shift) + hl) * DH;
+      const int head = (kvh << g_shift) + hl;
+      __nv_bfloat16* dst = p.out + (size_t)(seq0 + pos) * (p.n_q_heads * DH) + head * DH;
+      // scale of this pass's unnormalised O, and (prefix mode) of the frame-local result already in `out`
+      float w_new = 1.0f / l, w_old = 0.f;
+      if (pos < S) {
+        float2* st = p.stats ? p.stats + (size_t)(seq0 + pos) * p.n_q_heads + head : nullptr;
+        if (p.prefix_mode) {
+          const float2 f = *st;  // (m_f, l_f) of the frame-local pass
+          const float m = fmaxf(f.x, mx);
+          const float a = f.y * ex2_approx((f.x - m) * sc);
+          const float b = ex2_approx((mx - m) * sc);
+          const float inv = 1.0f / (a + b * l);
+          w_old = a * inv;
+          w_new = b * inv;
+        } else if (st) {
+          *st = make_float2(mx, l);
+        }
+      }
 #pragma unroll 1
       for (int c0 = 0; c0 < DH; c0 += 32) {
         uint32_t r[32];
@@ -258,11 +286,15 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         if (pos < S) {
 #pragma unroll
           for (int q4 = 0; q4 < 4; ++q4) {
+            uint4 old4 = make_uint4(0u, 0u, 0u, 0u);
+            if (p.prefix_mode) old4 = *reinterpret_cast<const uint4*>(dst + c0 + 8 * q4);
+            const uint32_t ow[4] = {old4.x, old4.y, old4.z, old4.w};
             uint32_t o[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-              __nv_bfloat162 v = __floats2bfloat162_rn(__uint_as_float(r[8 * q4 + 2 * e]) * inv,
-                                                       __uint_as_float(r[8 * q4 + 2 * e + 1]) * inv);
+              const float lo = __uint_as_float(r[8 * q4 + 2 * e]) * w_new + __uint_as_float(ow[e] << 16) * w_old;
+              const float hi = __uint_as_float(r[8 * q4 + 2 * e + 1]) * w_new + __uint_as_float(ow[e] & 0xFFFF0000u) * w_old;
+              __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
               o[e] = *reinterpret_cast<uint32_t*>(&v);
             }
             *reinterpret_cast<uint4*>(dst + c0 + 8 * q4) = make_uint4(o[0], o[1], o[2], o[3]);

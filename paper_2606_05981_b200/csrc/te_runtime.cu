@@ -102,6 +102,8 @@ struct te_handle {
   int8_t axis[64] = {};
   // shared text prefix (te_encode_prefix): per-layer keys | values of the P prefix tokens, [L][max_prefix][2*Hkv*dh]
   bf16* kv_prefix = nullptr;
+  std::vector<CUtensorMap> tm_prefix;  // per layer: the prefix cache [P, 2*Hkv*dh] in 64-row boxes (tcgen05 attention)
+  float2* attn_stats = nullptr;        // [max_tokens, Hq] (row max, row sum) of the frame-local attention pass
   float* prefix_buf = nullptr;    // [max_prefix, d] residual of the prefix pass when the caller wants no output
   int32_t* prefix_lens = nullptr; // device [1]
   int prefix_len = 0;
@@ -416,8 +418,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int G = c.n_q_heads / c.n_kv_heads;
   int g_shift = 0;
   while ((1 << g_shift) < G) ++g_shift;
-  // (with a cached prefix the keys of a frame are prefix + own, possibly > 256: the streaming flash kernel)
-  const bool attn_tc = h->attn_impl == 1 && (1 << g_shift) == G && G <= 8 && P == 0;
+  // (with a cached prefix the tcgen05 kernel runs twice per layer: frame-local keys, then the prefix keys merged
+  //  into the result through the saved row statistics)
+  const bool attn_tc = h->attn_impl == 1 && (1 << g_shift) == G && G <= 8;
   CUtensorMap tmQ, tmKV;
   int attn_split = 1;
   if (attn_tc) {
@@ -467,8 +470,15 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
         te::AttnTcParams tp{};
         tp.out = h->attn; tp.cu_seqlens = h->cu; tp.n_q_heads = c.n_q_heads; tp.n_kv_heads = c.n_kv_heads;
         tp.g_shift = g_shift; tp.total_tokens = T; tp.scale_log2 = ap.scale_log2;
+        tp.stats = P > 0 ? h->attn_stats : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
         TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(tmQ, tmKV, tp, attn_split, n_frames, st)
                              : launch_attn_tc<64>(tmQ, tmKV, tp, attn_split, n_frames, st));
+        if (P > 0) {  // second pass: the P cached prefix keys of this layer, merged in place
+          tp.prefix_mode = 1; tp.prefix_len = P;
+          TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(tmQ, h->tm_prefix[l], tp, attn_split, n_frames, st)
+                               : launch_attn_tc<64>(tmQ, h->tm_prefix[l], tp, attn_split, n_frames, st));
+          ++nk;
+        }
       } else {
         TE_CUDA(h, launch_attn_any(dh, ap, q_blocks, n_frames, st));
       }
@@ -606,7 +616,9 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
             cudaSuccess ||
         cudaMalloc(reinterpret_cast<void**>(&h->prefix_buf), (size_t)c.max_prefix_tokens * c.hidden * sizeof(float)) !=
             cudaSuccess ||
-        cudaMalloc(reinterpret_cast<void**>(&h->prefix_lens), sizeof(int32_t)) != cudaSuccess)
+        cudaMalloc(reinterpret_cast<void**>(&h->prefix_lens), sizeof(int32_t)) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->attn_stats), (size_t)c.max_tokens * c.n_q_heads * sizeof(float2)) !=
+            cudaSuccess)
       return fail(TE_ERR_CUDA);
   }
   {  // axis of frequency pair i: contiguous [t | h | w], or round-robin over the axes with pairs left
@@ -789,6 +801,14 @@ int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_le
                          &nk, /*prefix_pass=*/true);
   if (rc != TE_OK) return rc;
   h->launches += nk;
+  // tensor maps over each layer's cached K|V rows: exactly prefix_len rows, so that rows past the prefix read as zero
+  h->tm_prefix.resize(c.n_layers);
+  const size_t n_kv = 2 * (size_t)c.n_kv_heads * c.head_dim;
+  for (int l = 0; l < c.n_layers; ++l)
+    if (!make_tmap(&h->tm_prefix[l], h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv, prefix_len, n_kv, 64)) {
+      h->err = "cuTensorMapEncodeTiled failed for a prefix K/V map";
+      return TE_ERR_CUDA;
+    }
   h->prefix_len = prefix_len;
   return TE_OK;
 }

@@ -397,8 +397,9 @@ def _strip_prefix(full, P, cu):
     return np.concatenate([full[cu[b] + (b + 1) * P: cu[b + 1] + (b + 1) * P] for b in range(len(cu) - 1)])
 
 
+@pytest.mark.parametrize("attn_impl", [1, 0])
 @pytest.mark.parametrize("cfg_id,P", [(1, 7), (1, 64), (2, 80)])
-def test_prefix_kv_reuse_matches_full_recompute(H, O, cfg_id, P):
+def test_prefix_kv_reuse_matches_full_recompute(H, O, cfg_id, P, attn_impl):
     """te_encode_prefix once, then te_encode on the frames' own tokens only == the oracle run on the full
     [prefix | grid | text] sequences of every frame (ids continue through the prefix); the prefix rows
     equal the oracle's prefix rows; removing the prefix restores the base path bitwise."""
@@ -409,7 +410,9 @@ def test_prefix_kv_reuse_matches_full_recompute(H, O, cfg_id, P):
     full = _with_prefix(pre, emb, cu)
     ref_full = O.encode(blob, W.blob_layout(m), m, full, tl, w.grid_h, w.grid_w, prefix_len=P)
     ref = _strip_prefix(ref_full, P, cu)
-    g = H.GpuTE(m, w.n_frames, T, blob, max_prefix_tokens=max(P, 1))
+    # attn_impl 1: tcgen05 kernel twice per layer (frame keys, then prefix keys merged through the row
+    # statistics); 0: streaming mma.sync kernel over [cached prefix keys | own keys]
+    g = H.GpuTE(m, w.n_frames, T, blob, max_prefix_tokens=max(P, 1), attn_impl=attn_impl)
     base = g.encode(emb, tl, w.grid_h, w.grid_w)
     pre_out = g.encode_prefix(pre)
     out = g.encode(emb, tl, w.grid_h, w.grid_w)
