@@ -247,6 +247,7 @@ template <int EPI>
 cudaError_t launch_gemmk_bn(int bn, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p,
                             cudaStream_t st) {
   if constexpr (EPI == te::EPI_QKV) {
+    if (bn != 128) return cudaErrorInvalidValue;  // the split-K QKV kernel has one-head-wide (128-column) tiles only
     if (dh == 128) return launch_gemmk<128, EPI, 128>(a, b, p, st);
     return launch_gemmk<128, EPI, 64>(a, b, p, st);
   } else {
@@ -348,7 +349,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int num_m = (T + te::GEMM_BM - 1) / te::GEMM_BM;
   const bool kmode = !pair && h->splitk;
   const int bn_qkv = (kmode && num_m * (n_qkv / 128) <= h->sm_count) ? 128 : h->bn_qkv;
-  const bool k_qkv = kmode && num_m * (n_qkv / bn_qkv) <= h->sm_count;
+  const bool k_qkv = kmode && bn_qkv == 128;
+  // more one-head tiles than SMs (512 < T < 1024 at full width): 256-row CTA-pair tiles, as for gate/up below
+  const bool pair_qkv = pair || (kmode && !k_qkv && T > te::GEMM_BM && h->pair_mode == 2);
   // gate/up tile width: the weights are interleaved per bn_gu = 256 rows; 128-wide tiles read them as two 64-row
   // halves (gu_half).  With one row block (T <= 128) 96 one-CTA tiles stream the weights with no split-K exchange
   // (cfg 2: 27 -> 19 us).  (128-wide CTA-pair tiles at T = 512, 3 waves instead of 2 imbalanced ones, measured
@@ -357,7 +360,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const int bn_gu = gu128_k ? 128 : h->bn_gu;
   const bool k_gu = kmode && num_m * (2 * F / bn_gu) <= h->sm_count;
   const bool k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;
-  const int bx_qkv = box_index(pair ? bn_qkv / 2 : bn_qkv);
+  const int bx_qkv = box_index(pair_qkv ? bn_qkv / 2 : bn_qkv);
   // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
   // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
   const bool pair_gu = pair || (kmode && !k_gu && T > te::GEMM_BM && h->pair_mode == 2);
@@ -448,7 +451,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_QKV>(bn_qkv, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, st));
       } else {
-        TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(bn_qkv, pair, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
+        TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(bn_qkv, pair_qkv, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
       }
       tock(TE_KCLASS_QKV);
       ++nk;

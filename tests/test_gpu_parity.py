@@ -482,3 +482,59 @@ def test_pipelined_host_path_matches_blocking_call(H):
     with pytest.raises(te.TEError):
         g.enc.encode_host_wait(s2)                      # nothing in flight in that slot any more
     g.close()
+
+
+@pytest.mark.parametrize("T_target", [1, 127, 129, 255, 257, 513, 767, 1023, 1024, 1025, 1500])
+def test_token_count_sweep_across_kernel_regimes(H, O, T_target):
+    """Tiny stack at token counts on both sides of every dispatch threshold (one row block / split-K groups /
+    CTA pairs at 1024, ragged last row block, 128-wide gate/up tiles): each regime against the oracle."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    gh, gw = 1, 1
+    tl, left = [], T_target
+    rng = np.random.default_rng(T_target)
+    while left > 0:                                   # frames of 1 visual + up to 254 text tokens
+        s = int(min(left, rng.integers(1, 256)))
+        tl.append(s - 1)
+        left -= s
+    T = len(tl) + sum(tl)
+    assert T == T_target
+    emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    g = H.GpuTE(m, len(tl), T, blob)
+    out = g.encode(emb, tl, gh, gw)
+    _assert_final(PM.stack_metrics(out, ref, emb), f"T={T}")
+    assert np.array_equal(g.tap(g.te.TE_TAP_CU_SEQLENS, (len(tl) + 1,), np.int32), O.cu_seqlens(tl, gh, gw))
+    g.close()
+
+
+@pytest.mark.parametrize("T_target", [256, 384, 640, 1024, 1280])
+def test_full_width_layer_token_sweep(H, O, T_target):
+    """One full-width layer (cfg 2 shape) at mid token counts: the per-GEMM choice between split-K groups, one CTA per
+    tile and CTA pairs depends on tiles vs SMs (e.g. T = 256: QKV 64 tiles x 2 K-slices, O-proj/down 32 x 4,
+    gate/up 96 tiles; T = 640: gate/up on CTA pairs)."""
+    w, blob, _, _, _, _ = H.workload_inputs(2)
+    m = w.model
+    rng = np.random.default_rng(T_target)
+    tl, left = [], T_target
+    while left > 0:
+        s = int(min(left, 64 + rng.integers(1, 192)))
+        if s <= 64:
+            tl[-1] += s                              # fold a short remainder into the previous frame's text
+            left = 0
+            break
+        tl.append(s - 64)
+        left -= s
+    tl = [int(t) for t in tl]
+    assert all(64 + t <= 256 for t in tl[:-1])
+    if 64 + tl[-1] > 256:                            # keep every frame within max_tokens_per_frame
+        extra = 64 + tl[-1] - 256
+        tl[-1] -= extra
+        tl.append(max(0, extra - 64))
+    T = 64 * len(tl) + sum(tl)
+    emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, 8, 8)
+    g = H.GpuTE(m, len(tl), T, blob)
+    out = g.encode(emb, tl, 8, 8)
+    _assert_final(PM.stack_metrics(out, ref, emb), f"full-width T={T}")
+    g.close()
