@@ -538,3 +538,43 @@ def test_full_width_layer_token_sweep(H, O, T_target):
     out = g.encode(emb, tl, 8, 8)
     _assert_final(PM.stack_metrics(out, ref, emb), f"full-width T={T}")
     g.close()
+
+
+@pytest.mark.parametrize("hq,hkv,dh", [(4, 4, 64), (8, 2, 64), (8, 1, 64), (6, 2, 64), (2, 2, 128), (6, 1, 128)])
+def test_gqa_group_sizes(H, O, hq, hkv, dh):
+    """Query-group sizes G = Hq/Hkv in {1, 2, 3, 4, 6, 8}: the tcgen05 attention kernel stacks G heads into a query
+    tile when G is a power of two <= 8; other G (3, 6) run on the streaming kernel.  Small 2-layer stacks vs oracle."""
+    hidden = 256
+    sec = (8, 12, 12) if dh == 64 else (16, 24, 24)
+    m = W.TEModelConfig(n_layers=2, hidden=hidden, n_q_heads=hq, n_kv_heads=hkv, head_dim=dh, ffn=512,
+                        rope_sections=sec)
+    if ((hq + 2 * hkv) * dh) % 128 != 0:
+        pytest.skip("fused QKV width must be a multiple of 128")
+    blob = W.make_weight_blob(m, 7)
+    tl = [30, 0, 201, 77]
+    gh, gw = 3, 4
+    T = len(tl) * gh * gw + sum(tl)
+    emb = np.random.default_rng(hq * 10 + hkv).standard_normal((T, hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    g = H.GpuTE(m, len(tl), T, blob)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, gh, gw), ref, emb), f"Hq={hq} Hkv={hkv} dh={dh}")
+    g.close()
+
+
+def test_many_small_frames(H, O):
+    """300 frames of 1-6 tokens: the device-side scan runs over several 32-frame chunks, every attention CTA sees a
+    nearly empty frame, frames straddle row-block boundaries."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    rng = np.random.default_rng(12)
+    tl = [int(t) for t in rng.integers(0, 6, size=300)]
+    gh, gw = 1, 1
+    T = len(tl) + sum(tl)
+    emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    g = H.GpuTE(m, len(tl), T, blob)
+    out = g.encode(emb, tl, gh, gw)
+    assert np.array_equal(g.tap(g.te.TE_TAP_POS, (3, T), np.int32), O.position_ids(tl, gh, gw))
+    assert np.array_equal(g.tap(g.te.TE_TAP_CU_SEQLENS, (len(tl) + 1,), np.int32), O.cu_seqlens(tl, gh, gw))
+    _assert_final(PM.stack_metrics(out, ref, emb), "300 frames")
+    g.close()
