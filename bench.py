@@ -252,6 +252,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-timing-steps", type=int, default=3)
+    ap.add_argument("--frames", type=int, default=0,
+                    help="override the number of frames B of the chosen config (batch-scaling table, the analogue of "
+                         "the paper's Table V: TE wall at B = 1/2/4/8, PAPER.md:249-258)")
     ap.add_argument("--prefix", type=int, default=0,
                     help="SURVEY 8f NEXT-1: shared text prefix of this many tokens in front of every frame, encoded "
                          "once (te_encode_prefix) and reused through its cached K/V (PAPER.md:389: 80)")
@@ -267,6 +270,9 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
     w = W.get_workload(args.config)
+    if args.frames > 0:
+        import dataclasses as _dc
+        w = _dc.replace(w, n_frames=args.frames, name=f"{w.name}_framesB{args.frames}")
     m = w.model
     tl = W.make_text_lens(w)
     T = W.total_tokens(w, tl)
