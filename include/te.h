@@ -159,6 +159,10 @@ enum {
                               by the pair that holds its first k-blocks, on top of the other pieces' fp32 partials
                               summed in a fixed order (deterministic).  0 (default): whole tiles, round-robin —
                               measured faster on every config                                    */
+  TE_OPT_RESID_WIDE = 9,   /* O-proj / down on CTA pairs: 1 (default) = when their 128-wide tiles would need two or
+                              more waves, ONE wave of wide tiles (width = hidden / n rounded up to 32, <= 512
+                              columns, two MMAs per k-step; te_gemm_wide.cuh); 0 = never; n in 2..16 = always,
+                              with n tiles across the hidden dimension (tests)                                  */
   TE_OPT_SPLIT_K = 7       /* 1 (default): small batches (fewer 128-row tiles than SMs in a GEMM, no
                               CTA pairs) run the split-K kernel: several CTAs per output tile, each
                               streaming its own K-slice of the weights; partial tiles are summed in a

@@ -28,6 +28,7 @@ TE_OPT_TRACE = 5
 TE_OPT_ATTN_IMPL = 6
 TE_OPT_SPLIT_K = 7
 TE_OPT_STREAM_K = 8
+TE_OPT_RESID_WIDE = 9
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 

@@ -149,6 +149,7 @@ __device__ __forceinline__ void resid_issue(const GemmParams& p, ResidPrefetch& 
                                             int c0) {
   const int sub = lane >> 3, cq = lane & 7;
   const int col = n_blk * BN + c0 + cq * 4;
+  if (col >= p.N) return;  // chunk past the last column (N is not a multiple of a 192-wide tile)
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const int row = row_base + sub + 4 * i;
@@ -167,6 +168,7 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
   const int c_end = (part + 1) * (BN / nparts);
 #pragma unroll 1
   for (int c0 = part * (BN / nparts); c0 < c_end; c0 += 32) {
+    if (n_blk * BN + c0 >= p.N) break;  // columns past N (zero-filled weight rows): nothing to store
     {
       uint32_t r[32];
       tmem_ld32(t_row + c0, r);
@@ -643,7 +645,7 @@ struct Gemm2Cfg {
   static constexpr int STAGES_FIT = (SMEM_LIMIT - 1024 - BAR_BYTES - STG_BYTES) / STAGE_BYTES;
   static constexpr int STAGES = STAGES_FIT > 8 ? 8 : STAGES_FIT;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STG_BYTES + 1024;
-  static constexpr int TMEM_COLS = 2 * BN;
+  static constexpr int TMEM_COLS = (2 * BN <= 256) ? 256 : 512;  // power of two >= two BN-column accumulators
   static_assert(STAGES >= 3 && 2 * STAGES + 5 <= BAR_BYTES / 8, "pipeline configuration");
 };
 

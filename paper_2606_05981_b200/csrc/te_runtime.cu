@@ -15,6 +15,7 @@
 #include "te_attn_tc.cuh"
 #include "te_gemm.cuh"
 #include "te_gemm_splitk.cuh"
+#include "te_gemm_wide.cuh"
 #include "te_prep.cuh"
 
 namespace {
@@ -76,8 +77,11 @@ struct te_handle {
   bool loaded = false;
   // tile choices
   int bn_qkv = 256, bn_gu = 256, bn_res = 128;
+  bool bn_res_auto = true;  // CTA-pair residual tile width chosen per token count until TE_OPT_RESID_BLOCK_N is set
   int attn_impl = 1;  // 1: tcgen05 kernel (te_attn_tc.cuh) when Hq/Hkv is a power of two <= 8; 0: mma.sync kernel
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
+  int resid_wide = 1; // residual GEMMs on CTA pairs: 1 = auto (one wave of wide tiles when 128-wide tiles need >= 2
+                      // waves), 0 = never, n >= 2 = always with n tiles across N (tests)
   int streamk = 0;    // 1: CTA-pair GEMMs balance (tile, k-block) units over all SM pairs (stream-K; measured slower)
   int splitk = 1;     // 1: small batches (no CTA pairs) use the split-K kernel when a GEMM has <= one tile per SM
   float* sk_scratch = nullptr;  // [sm_count][128 x 256] fp32 partial tiles
@@ -228,6 +232,9 @@ cudaError_t launch_gemm_bn(int bn, int pair, int dh, const CUtensorMap& a, const
   } else {
     if (pair) {
       if (bn == 256) return launch_gemm2<256, EPI, 128>(a, b, p, sms, st);
+      if constexpr (EPI == te::EPI_RESID) {
+        if (bn == 192) return launch_gemm2<192, EPI, 128>(a, b, p, sms, st);
+      }
       return launch_gemm2<128, EPI, 128>(a, b, p, sms, st);
     }
     if (bn == 256) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
@@ -313,6 +320,10 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
   TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm2_kernel<192, te::EPI_RESID, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::Gemm2Cfg<192, te::EPI_RESID>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::AttnCfg<128, 1>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -327,6 +338,17 @@ cudaError_t init_kernel_attrs() {
                                 te::AttnTcCfg<64>::SMEM_BYTES)));
 #undef TE_ATTR
   return cudaSuccess;
+}
+
+// One wave of wide CTA-pair tiles for a residual GEMM (te_gemm_wide.cuh).  W: [n_rows, k_cols] weights.
+cudaError_t launch_wide(te_handle* h, const bf16* W, int n_rows, int k_cols, const CUtensorMap& tmA, const te::GemmParams& p,
+                        int n_tiles, int bn, cudaStream_t st) {
+  CUtensorMap tmB;
+  if (!make_tmap(&tmB, W, n_rows, k_cols, bn / 4)) return cudaErrorInvalidValue;  // box = one MMA's rows of one CTA
+  const int num_mp = (p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
+  (void)h;
+  return launch_k(te::te_gemm_wide_kernel, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
+                  te::GemmWideCfg::smem_bytes(bn), st, tmA, tmB, p, bn);
 }
 
 // Enqueue the whole stack on `st`.  Returns the number of kernels launched via *n_kernels.
@@ -359,15 +381,47 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const bool gu128_k = kmode && h->bn_gu == 256 && num_m * (2 * F / 128) <= h->sm_count;
   const int bn_gu = gu128_k ? 128 : h->bn_gu;
   const bool k_gu = kmode && num_m * (2 * F / bn_gu) <= h->sm_count;
-  const bool k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;
+  const bool k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;  // (kmode: bn_res == h->bn_res)
   const int bx_qkv = box_index(pair_qkv ? bn_qkv / 2 : bn_qkv);
   // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
   // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
   const bool pair_gu = pair || (kmode && !k_gu && T > te::GEMM_BM && h->pair_mode == 2);
   const int bx_gu = (bn_gu != h->bn_gu) ? 0 : box_index(pair_gu ? h->bn_gu / 2 : h->bn_gu);  // gu_half: 64-row boxes
-  const int bx_res = box_index(pair ? h->bn_res / 2 : h->bn_res);
+
+  // Residual GEMMs on CTA pairs: when their 128-wide tiles would take >= 2 waves, one wave of wide tiles instead
+  // (te_gemm_wide.cuh): n_tiles = pairs / row-pair blocks, width = N / n_tiles rounded up to 32 (<= 512).
+  int wide_tiles = 0, wide_bn = 0;
+  if (pair && h->resid_wide) {
+    const int np = h->sm_count / 2;
+    const int mp_cnt = (T + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
+    int nt = h->resid_wide >= 2 ? h->resid_wide : np / mp_cnt;
+    const int cap = h->ssq_parts_cap / 2 < d / 32 ? h->ssq_parts_cap / 2 : d / 32;
+    if (nt > cap) nt = cap;
+    if (nt >= 1) {
+      const int bn = (((d + nt - 1) / nt) + 31) / 32 * 32;
+      const int waves128 = (mp_cnt * (d / 128) + np - 1) / np;
+      const bool wins = waves128 >= 2 && bn * 4 < waves128 * 128 * 5;
+      if (bn <= 512 && mp_cnt * nt <= np && (h->resid_wide >= 2 || wins)) { wide_tiles = nt; wide_bn = bn; }
+    }
+  }
+  // Residual tile width on CTA pairs (auto when TE_OPT_RESID_BLOCK_N was not set): cost ~ waves x width, with 128-wide
+  // tiles 1.3x dearer per column (they are L2->SM-bound); 192-wide tiles give cfg 4 132 tiles = 2 waves.
+  int bn_res = h->bn_res;
+  if (pair && !wide_tiles && h->bn_res_auto) {
+    const int np = h->sm_count / 2;
+    const int mp_cnt = (T + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
+    double best = 1e30;
+    for (int bn : {128, 192, 256}) {
+      const int tiles = mp_cnt * ((d + bn - 1) / bn);
+      const double cost = (double)((tiles + np - 1) / np) * bn * (bn == 128 ? 1.3 : 1.0);
+      if (cost < best - 1e-9 && 2 * ((d + bn - 1) / bn) <= h->ssq_parts_cap) { best = cost; bn_res = bn; }
+    }
+  }
+  CUtensorMap tm_res192_o, tm_res192_d;  // 96-row boxes for the 192-wide pair tiles (encoded per layer below)
   // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
-  const int parts = (d / h->bn_res) * ((pair || k_res) ? 2 : 1);
+  const int bx_res = box_index(pair ? (bn_res == 192 ? 128 : bn_res) / 2 : bn_res);
+  const int n_blk_res = (d + bn_res - 1) / bn_res;
+  const int parts = wide_tiles ? wide_tiles * 2 : n_blk_res * ((pair || k_res) ? 2 : 1);
   int nk = 0;
   // Optional per-kernel CUDA-event bracketing (TE_OPT_KERNEL_TIMING; never inside a capture).
   cudaEvent_t ev_a = nullptr;
@@ -490,15 +544,22 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     }
     {  // a3: O projection + residual add (+ next norm's gain / statistics)
       te::GemmParams p = base;
-      p.N = d; p.K = n_q; p.num_n_blk = d / h->bn_res;
+      p.N = d; p.K = n_q; p.num_n_blk = n_blk_res;
       p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
       p.trace = trace_ptr(1);
       tick();
-      if (k_res) {
+      if (wide_tiles) {
+        TE_CUDA(h, launch_wide(h, h->w + o.wo, d, n_q, tmA_attn, p, wide_tiles, wide_bn, st));
+      } else if (k_res) {
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm[l].o[bx_res], p, st));
       } else {
-        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_attn, h->tm[l].o[bx_res], p, h->sm_count, st));
+        const CUtensorMap* tmb = &h->tm[l].o[bx_res];
+        if (bn_res == 192) {
+          if (!make_tmap(&tm_res192_o, h->w + o.wo, d, n_q, 96)) { h->err = "tensor map (192-wide O-proj)"; return TE_ERR_CUDA; }
+          tmb = &tm_res192_o;
+        }
+        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(bn_res, pair, dh, tmA_attn, *tmb, p, h->sm_count, st));
       }
       tock(TE_KCLASS_OPROJ);
       ++nk;
@@ -521,16 +582,23 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     }
     {  // a5: down projection + residual add
       te::GemmParams p = base;
-      p.N = d; p.K = F; p.num_n_blk = d / h->bn_res;
+      p.N = d; p.K = F; p.num_n_blk = n_blk_res;
       p.x = out; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
       p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
       p.trace = trace_ptr(3);
       tick();
-      if (k_res) {
+      if (wide_tiles) {
+        TE_CUDA(h, launch_wide(h, h->w + o.wd, d, F, tmA_act, p, wide_tiles, wide_bn, st));
+      } else if (k_res) {
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm[l].d[bx_res], p, st));
       } else {
-        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(h->bn_res, pair, dh, tmA_act, h->tm[l].d[bx_res], p, h->sm_count, st));
+        const CUtensorMap* tmb = &h->tm[l].d[bx_res];
+        if (bn_res == 192) {
+          if (!make_tmap(&tm_res192_d, h->w + o.wd, d, F, 96)) { h->err = "tensor map (192-wide down)"; return TE_ERR_CUDA; }
+          tmb = &tm_res192_d;
+        }
+        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(bn_res, pair, dh, tmA_act, *tmb, p, h->sm_count, st));
       }
       tock(TE_KCLASS_DOWN);
       ++nk;
@@ -932,6 +1000,12 @@ int te_set_option(te_handle* h, int option, int value) {
     free_graphs(h);
     return TE_OK;
   }
+  if (option == TE_OPT_RESID_WIDE) {
+    if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
+    h->resid_wide = value;
+    free_graphs(h);
+    return TE_OK;
+  }
   if (option == TE_OPT_STREAM_K) {
     h->streamk = value ? 1 : 0;
     free_graphs(h);
@@ -946,6 +1020,7 @@ int te_set_option(te_handle* h, int option, int value) {
   if (option == TE_OPT_RESID_BLOCK_N) {
     if ((value != 128 && value != 256) || h->cfg.hidden % value != 0) return TE_ERR_INVALID_ARG;
     h->bn_res = value;
+    h->bn_res_auto = false;
     free_graphs(h);
     return TE_OK;
   }

@@ -578,3 +578,21 @@ def test_many_small_frames(H, O):
     assert np.array_equal(g.tap(g.te.TE_TAP_CU_SEQLENS, (len(tl) + 1,), np.int32), O.cu_seqlens(tl, gh, gw))
     _assert_final(PM.stack_metrics(out, ref, emb), "300 frames")
     g.close()
+
+
+@pytest.mark.parametrize("n_tiles", [2, 3, 5, 8])
+def test_wide_residual_tiles(H, O, n_tiles):
+    """O-proj / down as one wave of wide CTA-pair tiles (two MMAs per k-step): forced tile counts whose widths do and do
+    not divide the hidden size (a partly and a completely out-of-range last tile), ragged last row-pair block."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    tl = [5, 0, 190, 33, 240, 65]
+    gh, gw = 2, 5
+    T = len(tl) * gh * gw + sum(tl)
+    emb = np.random.default_rng(4).standard_normal((T, m.hidden)).astype(np.float32)
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    g = H.GpuTE(m, len(tl), T, blob, cta_pair=1, resid_wide=n_tiles)
+    out = g.encode(emb, tl, gh, gw)
+    _assert_final(PM.stack_metrics(out, ref, emb), f"wide residual tiles n={n_tiles}")
+    assert np.array_equal(out, g.encode(emb, tl, gh, gw))
+    g.close()
