@@ -418,9 +418,9 @@ def main():
 
     peaks = load_peaks()
     # dram__bytes_read.sum + dram__bytes_write.sum of one gate/up launch, from the committed ncu --set full
-    # capture (profiles/r01c_ncu_full_layer_cfg4.md); only that workload was captured
+    # capture (profiles/r01f_cfg4.md)
     # (cfg 2: profiles/r01d_ncu_full_small_batch.md, gate/up on the split-K kernel)
-    traffic = {"cfg4_28L_B16": 63.348992e6 + 15.863552e6, "cfg2_1L_B1": 50.973952e6 + 1.491456e6}.get(w.name)
+    traffic = {"cfg4_28L_B16": 63.364864e6 + 15.521024e6, "cfg2_1L_B1": 50.973952e6 + 1.491456e6}.get(w.name)
     flops, wbytes, abytes = stack_work(m, seq_lens)
     flops += m.n_layers * sum(4.0 * m.head_dim * m.n_q_heads * s * args.prefix for s in seq_lens)  # prefix keys
     t_compute = flops / (peaks["tf_sustained"] * 1e12)
@@ -438,7 +438,7 @@ def main():
                     "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sustained"],
                     "peak_kind": f"bf16_tflops_sustained ({peaks['src']}); kernel timed inside a long step",
                     "frac_of_burst": achieved / peaks["tf_burst"], "traffic": traffic,
-                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01c)",
+                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01f)",
                     "algorithmic_bytes": 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn}
     else:
         gu_bytes = 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
