@@ -9,6 +9,11 @@
 // and bn/2 weight rows: 54 B/clk per SM at bn = 352, i.e. the tile is tensor-bound again, and no wave is
 // partially filled.  Columns past N (the last tile) are zero-filled by TMA and never stored.
 // Same warp roles, PDL prologue and residual epilogue arithmetic as te_gemm2_kernel (te_gemm.cuh).
+//
+// EPI_SWIGLU variant (mid batches, e.g. T = 512: 96 pair tiles of 256 x 256 = 1.3 waves): the two MMAs of a tile
+// take the gate rows and the matching up rows of the NON-interleaved [Wgate; Wup] matrix, so that a tile of w
+// output columns (bn = 2w accumulator columns: [0,w) gate, [w,2w) up) can have any width that is a multiple of 32:
+// 32 x 192 output columns x 2 row-pair blocks = 64 tiles, one wave.
 #pragma once
 #include "te_gemm.cuh"
 
@@ -33,8 +38,10 @@ struct GemmWideCfg {
   }
 };
 
-// bn: tile width, a multiple of 32, <= 512; nh = bn/2 columns per MMA (multiple of 16, <= 256).
-// tmB: weight matrix [N, K] in boxes of nh/2 rows x 64 columns.
+// bn: accumulator width, a multiple of 32 (64 for EPI_SWIGLU), <= 512; nh = bn/2 columns per MMA (multiple of 16, <= 256).
+// tmB: weight matrix in boxes of nh/2 rows x 64 columns: [N, K] for EPI_RESID; [2F, K] = [Wgate; Wup] for EPI_SWIGLU
+// (p.N = 2F; the tile's output columns are n_blk*nh .. +nh of F).
+template <int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM2_THREADS, 1)
 te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const GemmParams p,
                     const int bn) {
@@ -87,15 +94,18 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
   const int tile = blockIdx.x >> 1;  // one tile per CTA pair
   const int mp = tile % num_mp;
   const int n_blk = tile / num_mp;
-  const int col_base = n_blk * bn;
+  // first output column of the tile; first weight row of MMA 0 / MMA 1
+  const int col_base = (EPI == EPI_SWIGLU) ? n_blk * nh : n_blk * bn;
+  const int w_row0 = col_base;
+  const int w_row1 = (EPI == EPI_SWIGLU) ? p.N / 2 + col_base : col_base + nh;
 
   if (warp == 0) {
     // ===================== TMA producer (both CTAs) =====================
     if (elect_one()) {
       const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
       // this CTA's weight rows for MMA j: [col_base + j*nh + rank*nh/2, + nh/2)
-      const int b_row0 = col_base + rank * (nh / 2);
-      const int b_row1 = col_base + nh + rank * (nh / 2);
+      const int b_row0 = w_row0 + rank * (nh / 2);
+      const int b_row1 = w_row1 + rank * (nh / 2);
       auto load_b = [&](int stage, int kb) {
         const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
         tma_load_2d_cg2(sB + stage * b_bytes, &tmB, bar, kb * GEMM_BK, b_row0);
@@ -147,18 +157,45 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
     // ===================== epilogue warps (both CTAs, own 128 rows): x += acc, xg, sum of squares ============
     const int quad = warp & 3;
     const int part = (warp - 2) >> 2;
-    const int sub = lane >> 3, cq = lane & 7;
+    [[maybe_unused]] const int sub = lane >> 3, cq = lane & 7;
     const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
     const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16);
     float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
-    // the tile's valid 32-column chunks are split between the two warps of a quadrant
-    int n_valid = p.N - col_base;
-    n_valid = n_valid < 0 ? 0 : (n_valid > bn ? bn : n_valid);
+    // the tile's valid 32-column chunks (of output columns) are split between the two warps of a quadrant
+    const int out_w = (EPI == EPI_SWIGLU) ? nh : bn;
+    int n_valid = ((EPI == EPI_SWIGLU) ? p.N / 2 : p.N) - col_base;
+    n_valid = n_valid < 0 ? 0 : (n_valid > out_w ? out_w : n_valid);
     const int chunks = n_valid / 32;
     const int c_begin = part == 0 ? 0 : ((chunks + 1) / 2) * 32;
     const int c_end = part == 0 ? ((chunks + 1) / 2) * 32 : chunks * 32;
-    const bool has_g = p.g_next != nullptr;
     pdl_wait();
+    if constexpr (EPI == EPI_SWIGLU) {
+      // ---- y = rstd * acc; act = silu(gate) * up, bf16 (arithmetic of epi_swiglu, te_gemm.cuh)
+      const float rstd = row_rstd(p, row_base + lane, row_base + lane < p.M);
+      mbar_wait(tfull, 0);
+      tc_fence_after();
+#pragma unroll 1
+      for (int c0 = c_begin; c0 < c_end; c0 += 32) {
+        float a[32];
+        {
+          uint32_t g[32], u[32];
+          tmem_ld32(t_row + c0, g);
+          tmem_ld32(t_row + nh + c0, u);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const float gv = __uint_as_float(g[j]) * rstd;
+            const float uv = __uint_as_float(u[j]) * rstd;
+            a[j] = __fdividef(gv, 1.0f + __expf(-gv)) * uv;
+          }
+        }
+        stg_put_row(stg, lane, a);
+        __syncwarp();
+        stg_store_bf16(stg, lane, row_base, p.M, p.act, p.ld_act, col_base + c0);
+        __syncwarp();
+      }
+    } else {
+    const bool has_g = p.g_next != nullptr;
     auto issue_x = [&](float4 (&xv)[8], int c0) {
       const int col = col_base + c0 + cq * 4;
 #pragma unroll
@@ -232,6 +269,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         if (row < p.M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * 2 + part)] = ss[i];
       }
     }
+    }  // EPI_RESID
   }
   tc_fence_before();
   __syncwarp();  // the elected producer / MMA lanes rejoin their warps before the block barrier

@@ -89,6 +89,7 @@ struct te_handle {
   // weights
   bf16* w = nullptr;
   size_t w_elems = 0;
+  bf16* w_gu_plain = nullptr;  // [L][2F, d] = [Wgate; Wup] as in the blob (not interleaved): wide SwiGLU tiles
   std::vector<LayerOff> off;
   size_t gf_off = 0;
   // weight tensor maps per layer, one per B box height {64, 128, 256} rows (index 0, 1, 2)
@@ -322,7 +323,9 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm2_kernel<192, te::EPI_RESID, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::Gemm2Cfg<192, te::EPI_RESID>::SMEM_BYTES)));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmWideCfg::SMEM_LIMIT)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::AttnCfg<128, 1>::SMEM_BYTES)));
@@ -341,13 +344,13 @@ cudaError_t init_kernel_attrs() {
 }
 
 // One wave of wide CTA-pair tiles for a residual GEMM (te_gemm_wide.cuh).  W: [n_rows, k_cols] weights.
-cudaError_t launch_wide(te_handle* h, const bf16* W, int n_rows, int k_cols, const CUtensorMap& tmA, const te::GemmParams& p,
+template <int EPI>
+cudaError_t launch_wide(const bf16* W, int n_rows, int k_cols, const CUtensorMap& tmA, const te::GemmParams& p,
                         int n_tiles, int bn, cudaStream_t st) {
   CUtensorMap tmB;
   if (!make_tmap(&tmB, W, n_rows, k_cols, bn / 4)) return cudaErrorInvalidValue;  // box = one MMA's rows of one CTA
   const int num_mp = (p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
-  (void)h;
-  return launch_k(te::te_gemm_wide_kernel, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
+  return launch_k(te::te_gemm_wide_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
                   te::GemmWideCfg::smem_bytes(bn), st, tmA, tmB, p, bn);
 }
 
@@ -386,6 +389,20 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
   // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
   const bool pair_gu = pair || (kmode && !k_gu && T > te::GEMM_BM && h->pair_mode == 2);
+  // ... and when those pair tiles need two or more waves (T = 512: 96 tiles on 74 pairs), ONE wave of wide SwiGLU tiles
+  // over the non-interleaved [Wgate; Wup] instead: w output columns per tile = F / (pairs / row-pair blocks),
+  // rounded up to 32 (te_gemm_wide.cuh)
+  int gu_wide_tiles = 0, gu_wide_w = 0;
+  if (kmode && pair_gu && h->resid_wide == 1) {
+    const int np = h->sm_count / 2;
+    const int mp_cnt = (T + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
+    const int nt = np / mp_cnt;
+    if (nt >= 1) {
+      const int w = (((F + nt - 1) / nt) + 31) / 32 * 32;
+      const int waves256 = (mp_cnt * (2 * F / h->bn_gu) + np - 1) / np;
+      if (2 * w <= 512 && waves256 >= 2 && 2 * w < waves256 * h->bn_gu) { gu_wide_w = w; gu_wide_tiles = (F + w - 1) / w; }
+    }
+  }
   const int bx_gu = (bn_gu != h->bn_gu) ? 0 : box_index(pair_gu ? h->bn_gu / 2 : h->bn_gu);  // gu_half: 64-row boxes
 
   // Residual GEMMs on CTA pairs: when their 128-wide tiles would take >= 2 waves, one wave of wide tiles instead
@@ -549,7 +566,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.trace = trace_ptr(1);
       tick();
       if (wide_tiles) {
-        TE_CUDA(h, launch_wide(h, h->w + o.wo, d, n_q, tmA_attn, p, wide_tiles, wide_bn, st));
+        TE_CUDA(h, launch_wide<te::EPI_RESID>(h->w + o.wo, d, n_q, tmA_attn, p, wide_tiles, wide_bn, st));
       } else if (k_res) {
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm[l].o[bx_res], p, st));
@@ -571,7 +588,11 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.act = h->act; p.ld_act = F;
       p.trace = trace_ptr(2);
       tick();
-      if (k_gu) {
+      if (gu_wide_tiles) {
+        p.gu_half = 0;
+        TE_CUDA(h, launch_wide<te::EPI_SWIGLU>(h->w_gu_plain + (size_t)l * 2 * F * d, 2 * F, d, tmA_xg, p, gu_wide_tiles,
+                                               2 * gu_wide_w, st));
+      } else if (k_gu) {
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(bn_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, st));
       } else {
@@ -588,7 +609,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
       p.trace = trace_ptr(3);
       tick();
       if (wide_tiles) {
-        TE_CUDA(h, launch_wide(h, h->w + o.wd, d, F, tmA_act, p, wide_tiles, wide_bn, st));
+        TE_CUDA(h, launch_wide<te::EPI_RESID>(h->w + o.wd, d, F, tmA_act, p, wide_tiles, wide_bn, st));
       } else if (k_res) {
         p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm[l].d[bx_res], p, st));
@@ -731,8 +752,10 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
   TE_CUDA(h, cudaMemcpy(h->w, blob, n_bytes, cudaMemcpyDefault));
   const size_t d = c.hidden, dh = c.head_dim, F = c.ffn;
   const size_t n_qkv = (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * dh, n_q = (size_t)c.n_q_heads * dh;
+  // [Wgate; Wup] of every layer is also kept as it is in the blob (wide SwiGLU tiles take gate and up rows from
+  // separate MMAs); that copy doubles as the source of the interleave below
+  if (!h->w_gu_plain) TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->w_gu_plain), (size_t)c.n_layers * 2 * F * d * sizeof(bf16)));
   bf16* stage = nullptr;
-  TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&stage), 2 * F * d * sizeof(bf16)));
   h->off.resize(c.n_layers);
   h->tm.resize(c.n_layers);
   size_t o = 0;
@@ -747,6 +770,7 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
     L.g2 = o; o += d;
     L.wgu = o; o += 2 * F * d;
     L.wd = o; o += d * F;
+    stage = h->w_gu_plain + (size_t)l * 2 * F * d;
     cudaError_t e = cudaMemcpy(stage, h->w + L.wgu, 2 * F * d * sizeof(bf16), cudaMemcpyDeviceToDevice);
     if (e == cudaSuccess) {
       te::te_interleave_gate_up_kernel<<<(unsigned)(2 * F), 128>>>(
@@ -756,7 +780,6 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
     }
     if (e != cudaSuccess) {
       h->err = std::string("gate/up interleave: ") + cudaGetErrorString(e);
-      cudaFree(stage);
       return TE_ERR_CUDA;
     }
     for (int bi = 0; bi < 3; ++bi) {
@@ -769,7 +792,6 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
   }
   h->gf_off = o;
   cudaError_t e = cudaDeviceSynchronize();
-  cudaFree(stage);
   if (e != cudaSuccess) {
     h->err = std::string("te_load_weights: ") + cudaGetErrorString(e);
     return TE_ERR_CUDA;
@@ -1160,7 +1182,7 @@ void te_destroy(te_handle* h) {
   cudaDeviceSynchronize();
   free_graphs(h);
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
-  void* ptrs[] = {h->w, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
+  void* ptrs[] = {h->w, h->w_gu_plain, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
                   h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
                   h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens};
   for (void* p : ptrs)
