@@ -163,6 +163,10 @@ enum {
                               more waves, ONE wave of wide tiles (width = hidden / n rounded up to 32, <= 512
                               columns, two MMAs per k-step; te_gemm_wide.cuh); 0 = never; n in 2..16 = always,
                               with n tiles across the hidden dimension (tests)                                  */
+  TE_OPT_L2_RESIDUAL = 10, /* 1 (default): the fp32 residual stream (`out`) is an L2-persisting access-policy window
+                              of every kernel, so that the residual GEMMs' read-add-write passes stay out of DRAM.
+                              The first te_encode raises the DEVICE-WIDE limit cudaLimitPersistingL2CacheSize to
+                              min(max_tokens * hidden * 4, 64 MiB, device maximum).  0: no window                 */
   TE_OPT_SPLIT_K = 7       /* 1 (default): small batches (fewer 128-row tiles than SMs in a GEMM, no
                               CTA pairs) run the split-K kernel: several CTAs per output tile, each
                               streaming its own K-slice of the weights; partial tiles are summed in a

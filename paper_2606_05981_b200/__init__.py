@@ -29,6 +29,7 @@ TE_OPT_ATTN_IMPL = 6
 TE_OPT_SPLIT_K = 7
 TE_OPT_STREAM_K = 8
 TE_OPT_RESID_WIDE = 9
+TE_OPT_L2_RESIDUAL = 10
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 

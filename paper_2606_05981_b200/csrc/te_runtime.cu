@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -82,6 +83,9 @@ struct te_handle {
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   int resid_wide = 1; // residual GEMMs on CTA pairs: 1 = auto (one wave of wide tiles when 128-wide tiles need >= 2
                       // waves), 0 = never, n >= 2 = always with n tiles across N (tests)
+  int l2_resid = 1;          // 1: the residual stream is an L2-persisting access window of every kernel
+  size_t l2_limit_bytes = 0; // persisting-L2 carve-out requested for it (0 until the first te_encode sets the limit)
+  size_t l2_max_persist = 0; // device property persistingL2CacheMaxSize
   int streamk = 0;    // 1: CTA-pair GEMMs balance (tile, k-block) units over all SM pairs (stream-K; measured slower)
   int splitk = 1;     // 1: small batches (no CTA pairs) use the split-K kernel when a GEMM has <= one tile per SM
   float* sk_scratch = nullptr;  // [sm_count][128 x 256] fp32 partial tiles
@@ -175,6 +179,7 @@ int validate_config(const te_config& c) {
 // Launch with (optional) programmatic stream serialisation: the kernel may begin while its
 // predecessor in the stream drains; the kernels order themselves with griddepcontrol.wait.
 bool g_pdl = true;
+cudaAccessPolicyWindow g_l2_window{};
 template <typename... KArgs, typename... Args>
 cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
   cudaLaunchConfig_t cfg{};
@@ -182,11 +187,20 @@ cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
   cfg.blockDim = block;
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchAttribute at[2];
+  int n = 0;
+  if (g_pdl) {
+    at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[n].val.programmaticStreamSerializationAllowed = 1;
+    ++n;
+  }
+  if (g_l2_window.num_bytes) {  // experiment (TE_EXP_L2_RESID): keep the fp32 residual resident in L2
+    at[n].id = cudaLaunchAttributeAccessPolicyWindow;
+    at[n].val.accessPolicyWindow = g_l2_window;
+    ++n;
+  }
   cfg.attrs = at;
-  cfg.numAttrs = g_pdl ? 1 : 0;
+  cfg.numAttrs = n;
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
@@ -456,6 +470,17 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   };
 
   g_pdl = h->pdl && !h->timing;
+  // The fp32 residual stream (read and rewritten by both residual GEMMs of every layer) is marked persisting in L2
+  // for every kernel of the stack, so that its 2 x 2 passes per layer stay out of DRAM (TE_OPT_L2_RESIDUAL).
+  g_l2_window = cudaAccessPolicyWindow{};
+  if (h->l2_resid && h->l2_limit_bytes > 0) {
+    const size_t bytes = (size_t)T * d * sizeof(float);
+    g_l2_window.base_ptr = out;
+    g_l2_window.num_bytes = bytes;
+    g_l2_window.hitRatio = bytes <= h->l2_limit_bytes ? 1.0f : (float)h->l2_limit_bytes / (float)bytes;
+    g_l2_window.hitProp = cudaAccessPropertyPersisting;
+    g_l2_window.missProp = cudaAccessPropertyStreaming;
+  }
   {
     te::PrepParams pp{};
     pp.embeds = embeds; pp.text_lens = lens; pp.out = out; pp.cu = h->cu; pp.flag = h->flag; pp.pos = h->pos;
@@ -671,6 +696,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   h->cfg = *cfg;
   h->device = device;
   h->sm_count = prop.multiProcessorCount;
+  h->l2_max_persist = (size_t)prop.persistingL2CacheMaxSize;
   h->dbg_lb = 0;
   h->dbg_le = cfg->n_layers;
   const te_config& c = h->cfg;
@@ -822,6 +848,15 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
   if (st != nullptr) TE_CUDA(h, cudaStreamIsCapturing(st, &cap));
   int nk = 0;
   if (h->timing && cap != cudaStreamCaptureStatusNone) return TE_ERR_INVALID_ARG;
+  if (h->l2_resid && h->l2_limit_bytes == 0 && cap == cudaStreamCaptureStatusNone) {
+    // once per handle, outside any capture: reserve persisting L2 for the residual stream (a device-wide limit)
+    size_t want = (size_t)c.max_tokens * c.hidden * sizeof(float);
+    if (want > (64u << 20)) want = 64u << 20;
+    if (want > h->l2_max_persist) want = h->l2_max_persist;
+    if (want > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) h->l2_limit_bytes = want;
+    else h->l2_resid = 0;
+    cudaGetLastError();
+  }
   if (!h->use_graph || h->timing || cap != cudaStreamCaptureStatusNone) {
     int rc = enqueue_stack(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, st, &nk);
     if (rc == TE_OK) h->launches += nk;
@@ -1019,6 +1054,11 @@ int te_set_option(te_handle* h, int option, int value) {
   if (option == TE_OPT_ATTN_IMPL) {
     if (value < 0 || value > 1) return TE_ERR_INVALID_ARG;
     h->attn_impl = value;
+    free_graphs(h);
+    return TE_OK;
+  }
+  if (option == TE_OPT_L2_RESIDUAL) {
+    h->l2_resid = value ? 1 : 0;
     free_graphs(h);
     return TE_OK;
   }
