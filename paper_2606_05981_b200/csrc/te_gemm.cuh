@@ -279,20 +279,10 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
         a[j] = __fdividef(gv, 1.0f + __expf(-gv)) * uv;  // silu(g) * u; fast divide (2 ulp) ahead of a bf16 store
       }
     }
-#ifdef TE_EXP_SWIGLU_DIRECT
-    if (row_base + lane < p.M) {
-      uint4* dst = reinterpret_cast<uint4*>(p.act + (size_t)(row_base + lane) * p.ld_act + n_blk * HALF + c0);
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-        dst[j] = make_uint4(pack_bf16(a[8 * j], a[8 * j + 1]), pack_bf16(a[8 * j + 2], a[8 * j + 3]),
-                            pack_bf16(a[8 * j + 4], a[8 * j + 5]), pack_bf16(a[8 * j + 6], a[8 * j + 7]));
-    }
-#else
     stg_put_row(stg, lane, a);
     __syncwarp();
     stg_store_bf16(stg, lane, row_base, p.M, p.act, p.ld_act, n_blk * HALF + c0);
     __syncwarp();
-#endif
   }
 }
 
@@ -353,9 +343,6 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
       }
     }
     const float sc = rstd / sqrtf(ss * (1.0f / DH) + p.eps);
-#ifdef TE_EXP_QKV_STAMPS
-    if (lane == 0 && part == 0 && (row_base & 127) == 0 && p.trace && p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 40] == 0) trace_stamp(p, 40);
-#endif
     // ---- Pass 2: normalised halves a = u[c0..c0+32), b = u[HD2+c0..) -> staging -> rotate -> store.
     // All cos/sin segments of the step are requested up front (16 independent 16-byte loads per
     // lane) so that their L2 round trips overlap the TMEM reads and the staging instead of
@@ -415,10 +402,6 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
         }
       }
       __syncwarp();
-#ifdef TE_EXP_QKV_STAMPS
-      if (lane == 0 && part == 0 && (row_base & 127) == 0 && p.trace && c0 == 0 && p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 42] == 0) trace_stamp(p, 42);
-      if (lane == 0 && part == 0 && (row_base & 127) == 0 && p.trace && c0 == 32 && p.trace[(size_t)blockIdx.x * TRACE_SLOTS + 43] == 0) trace_stamp(p, 43);
-#endif
     }
   }
 }

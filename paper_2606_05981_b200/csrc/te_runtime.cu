@@ -194,7 +194,7 @@ cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
     at[n].val.programmaticStreamSerializationAllowed = 1;
     ++n;
   }
-  if (g_l2_window.num_bytes) {  // experiment (TE_EXP_L2_RESID): keep the fp32 residual resident in L2
+  if (g_l2_window.num_bytes) {  // TE_OPT_L2_RESIDUAL: the fp32 residual stays resident in L2
     at[n].id = cudaLaunchAttributeAccessPolicyWindow;
     at[n].val.accessPolicyWindow = g_l2_window;
     ++n;
