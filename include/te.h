@@ -14,10 +14,10 @@
  *
  * Conventions.  Plain C, no torch types.  Every pointer argument says HOST or DEVICE.  All
  * functions return 0 (TE_OK) or a negative te_status; none throws, aborts or prints.
- * The library is single-GPU and not thread-safe per handle.  The small-batch (split-K) kernels of one
- * call synchronise their CTAs through device memory and assume that they can all become resident:
- * do not run te_encode of TWO handles concurrently on one GPU (other kernels that finish on their
- * own — copies, a denoiser on another stream — are fine, see bench.py --overlap).  There is NO CPU fallback:
+ * The library is single-GPU and not thread-safe per handle.  The small-batch (split-K) kernels
+ * synchronise the CTAs of a group through device memory; they are launched as cooperative grids
+ * (all CTAs resident at once, at most one CTA per SM), so other work on the GPU — another handle
+ * on another stream, a denoiser (bench.py --overlap) — can delay them but not deadlock them.  There is NO CPU fallback:
  * te_create fails with TE_ERR_UNSUPPORTED on a device that is not sm_100.
  */
 #ifndef TE_B200_H_

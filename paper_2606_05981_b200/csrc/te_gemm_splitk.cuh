@@ -10,7 +10,8 @@
 //                   single SM has to ingest all partials)
 //
 // The group spins on each other, so the whole grid must be co-resident: the host launches this kernel
-// only with tiles * S <= number of SMs (one CTA per SM).  The sum order is fixed -> bitwise deterministic.
+// only with tiles * S <= number of SMs (one CTA per SM) and, for S > 1, as a COOPERATIVE grid (the launch
+// waits until every CTA can be resident).  The sum order is fixed -> bitwise deterministic.
 // S == 1 degenerates to one CTA per tile with the TMEM epilogues of te_gemm.cuh.
 // Weights of the CTA's first ring are requested before griddepcontrol.wait (they do not depend on the
 // predecessor kernel), so under programmatic dependent launch the weight stream of kernel n+1 overlaps

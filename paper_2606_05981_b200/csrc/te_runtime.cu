@@ -179,6 +179,7 @@ int validate_config(const te_config& c) {
 // Launch with (optional) programmatic stream serialisation: the kernel may begin while its
 // predecessor in the stream drains; the kernels order themselves with griddepcontrol.wait.
 bool g_pdl = true;
+bool g_coop = false;
 cudaAccessPolicyWindow g_l2_window{};
 template <typename... KArgs, typename... Args>
 cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
@@ -187,8 +188,13 @@ cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
   cfg.blockDim = block;
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
-  cudaLaunchAttribute at[2];
+  cudaLaunchAttribute at[3];
   int n = 0;
+  if (g_coop) {  // all CTAs of the grid resident at once, or the launch waits: the split-K groups spin on each other
+    at[n].id = cudaLaunchAttributeCooperative;
+    at[n].val.cooperative = 1;
+    ++n;
+  }
   if (g_pdl) {
     at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[n].val.programmaticStreamSerializationAllowed = 1;
@@ -262,8 +268,11 @@ template <int BN, int EPI, int DH>
 cudaError_t launch_gemmk(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, cudaStream_t st) {
   using Cfg = te::GemmKCfg<BN, EPI>;
   const int tiles = p.num_m_blk * p.num_n_blk;
-  return launch_k(te::te_gemmk_kernel<BN, EPI, DH>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS), Cfg::SMEM_BYTES, st,
-                  tmA, tmB, p);
+  g_coop = p.splits > 1;
+  cudaError_t e = launch_k(te::te_gemmk_kernel<BN, EPI, DH>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS),
+                           Cfg::SMEM_BYTES, st, tmA, tmB, p);
+  g_coop = false;
+  return e;
 }
 template <int EPI>
 cudaError_t launch_gemmk_bn(int bn, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p,
