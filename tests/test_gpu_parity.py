@@ -596,3 +596,25 @@ def test_wide_residual_tiles(H, O, n_tiles):
     _assert_final(PM.stack_metrics(out, ref, emb), f"wide residual tiles n={n_tiles}")
     assert np.array_equal(out, g.encode(emb, tl, gh, gw))
     g.close()
+
+
+def test_two_handles_share_the_gpu(H):
+    """Two encoders running their split-K (spinning) kernels on two streams at the same time: cooperative launches
+    keep each group co-resident, so the runs interleave instead of deadlocking, and the results are unchanged."""
+    import torch
+    w, blob, tl, T, emb, ch = H.workload_inputs(2)
+    ga = H.GpuTE(w.model, w.n_frames, T, blob)
+    gb = H.GpuTE(w.model, w.n_frames, T, blob)
+    want = ga.encode(emb, tl, w.grid_h, w.grid_w)
+    e = torch.from_numpy(emb).cuda()
+    lens = torch.from_numpy(tl).cuda()
+    oa, ob = torch.empty_like(e), torch.empty_like(e)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(50):
+        ga.enc.encode(w.n_frames, w.grid_h, w.grid_w, e, lens, T, oa, sa.cuda_stream)
+        gb.enc.encode(w.n_frames, w.grid_h, w.grid_w, e, lens, T, ob, sb.cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(oa.cpu().numpy(), want) and np.array_equal(ob.cpu().numpy(), want)
+    ga.close()
+    gb.close()
