@@ -618,3 +618,26 @@ def test_two_handles_share_the_gpu(H):
     assert np.array_equal(oa.cpu().numpy(), want) and np.array_equal(ob.cpu().numpy(), want)
     ga.close()
     gb.close()
+
+
+def test_encode_inside_a_callers_graph_capture(H):
+    """The call performs no sync, copy or allocation, so a caller can capture it into a CUDA graph of its own
+    (e.g. together with the denoiser step): the library then enqueues its kernels directly into that capture."""
+    import torch
+    w, blob, tl, T, emb, ch = H.workload_inputs(1)
+    g = H.GpuTE(w.model, w.n_frames, T, blob)
+    want = g.encode(emb, tl, w.grid_h, w.grid_w)
+    e = torch.from_numpy(emb).cuda()
+    lens = torch.from_numpy(tl).cuda()
+    out = torch.zeros_like(e)
+    st = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(graph, stream=st):
+        g.enc.encode(w.n_frames, w.grid_h, w.grid_w, e, lens, T, out, torch.cuda.current_stream().cuda_stream)
+    for _ in range(3):
+        out.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), want)
+    g.close()
