@@ -64,6 +64,41 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "tf_burst": 1590.0, "tf_sustained": 1400.0, "src": "fallback"}
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def config_dict(w, T, world, opt="defaults", flush_l2=False, extra=None):
+    """`config` of the JSON line — the SAME keys for both arms (ours / --impl reference)."""
+    m = w.model
+    c = {"workload": w.name, "n_frames_per_gpu": w.n_frames, "total_tokens_per_gpu": T,
+         "n_layers": m.n_layers, "hidden": m.hidden,
+         "l2": ("L2 flushed (256 MiB memset) before every timed step" if flush_l2 else
+                "no flush: per-step working set (2.8 GB weights + activations) exceeds the 126 MB L2"),
+         "parallelism": f"replica x{world} (frames sharded, no collective)", "opt": opt}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def weights_fit_l2(m) -> bool:
+    return 2.0 * W.blob_num_elements(m) < 256e6          # cfg 1/2: flush between steps
+
+
+# ncu --set full captures of the dominant kernel, per launch (dram__bytes_read.sum + dram__bytes_write.sum), keyed by
+# (workload, kernel name as te_dispatch_info reports it).  NOT measured in the bench run: the value is quoted only when
+# the kernel that ran is the one that was profiled, with its source; otherwise `traffic` is null.
+PROFILED_TRAFFIC = {
+    ("cfg4_28L_B16", "te_gemm2_kernel<256, 3, 128>"): (63.364864e6 + 15.521024e6, "profiles/r01f_cfg4.md"),
+}
+
+
 # ------------------------------------------------------------------------- N>1 helpers (gloo-tested)
 def rank_seed_offset(rank: int) -> int:
     """Each rank encodes its own batch of frames: embeddings seed = base + 1000 * rank."""
@@ -161,7 +196,8 @@ def time_oracle(w, blob, tl, emb, budget_s: float, n_frames_sample: int):
         cores = os.cpu_count() or 1
     return {"seconds_sample": dt, "frames": len(frames), "layers_run": n_layers,
             "frames_per_s": len(frames) / full, "tokens_per_s": float(sum(cu[b + 1] - cu[b] for b in frames)) / full,
-            "cores": int(cores),
+            "cores": int(cores), "nproc": os.cpu_count(), "cpu_model": cpu_model(),
+            "blas": "numpy float64 @ (OpenBLAS threads = cores); attention rows in a Python loop",
             "sample": f"{len(frames)} of {w.n_frames} frames x first {n_layers} of {m.n_layers} layers "
                       f"({dt:.1f} s), scaled by {m.n_layers}/{n_layers} to full depth"}
 
@@ -234,8 +270,9 @@ def run_reference(args, w, blob, tl, T, emb, rank):
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1000.0 * w.n_frames / v,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "n_frames": w.n_frames, "total_tokens": T, "n_layers": w.model.n_layers},
+        "config": config_dict(w, T, int(os.environ.get("WORLD_SIZE", "1")), flush_l2=weights_fit_l2(w.model)),
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": samples["cores"], "kind": "oracle",
+                         "nproc": samples["nproc"], "cpu_model": samples["cpu_model"], "blas": samples["blas"],
                          "sample": samples["sample"] + " per step"},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -258,9 +295,11 @@ def main():
     ap.add_argument("--prefix", type=int, default=0,
                     help="SURVEY 8f NEXT-1: shared text prefix of this many tokens in front of every frame, encoded "
                          "once (te_encode_prefix) and reused through its cached K/V (PAPER.md:389: 80)")
-    ap.add_argument("--overlap", action="store_true",
-                    help="SURVEY 8f NEXT-3: also run te_encode on a SIDE stream against a synthetic denoiser-shaped "
+    ap.add_argument("--no-overlap", action="store_true",
+                    help="skip the SURVEY 8f NEXT-3 block: te_encode on a SIDE stream against a synthetic denoiser-shaped "
                          "load (library bf16 matmuls) on the main stream, one event, as in the paper's Algorithm 1")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the B=4 (cfg 3) measurement that the default cfg-4 line carries as `secondary`")
     ap.add_argument("--opt", default="", help="library options for experiments, e.g. pdl=0,cta_pair=1,resid_bn=256")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -303,7 +342,8 @@ def main():
     enc = te.TextEncoder(m, w.n_frames, T, device=local_rank, max_prefix_tokens=args.prefix)
     enc.load_weights(blob)
     opt_ids = {"pdl": te.TE_OPT_PDL, "cta_pair": te.TE_OPT_CTA_PAIR, "resid_bn": te.TE_OPT_RESID_BLOCK_N,
-               "graph": te.TE_OPT_USE_GRAPH, "attn_impl": te.TE_OPT_ATTN_IMPL, "split_k": te.TE_OPT_SPLIT_K, "stream_k": te.TE_OPT_STREAM_K, "resid_wide": te.TE_OPT_RESID_WIDE, "l2_residual": te.TE_OPT_L2_RESIDUAL}
+               "graph": te.TE_OPT_USE_GRAPH, "attn_impl": te.TE_OPT_ATTN_IMPL, "split_k": te.TE_OPT_SPLIT_K,
+               "resid_wide": te.TE_OPT_RESID_WIDE, "l2_residual": te.TE_OPT_L2_RESIDUAL}
     for kv in filter(None, args.opt.split(",")):
         k, v = kv.split("=")
         te.te_set_option(enc.h, opt_ids[k], int(v))
@@ -311,7 +351,7 @@ def main():
     lens_dev = torch.from_numpy(tl).cuda()
     out_dev = torch.empty_like(e_dev)
     stream = torch.cuda.Stream()
-    flush_l2 = 2.0 * W.blob_num_elements(m) < 256e6          # weights fit L2 (cfg 1/2): flush between steps
+    flush_l2 = weights_fit_l2(m)
     flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda") if flush_l2 else None
 
     def step():
@@ -407,9 +447,48 @@ def main():
     ktimes = te.te_kernel_times(enc.h)
     te.te_set_option(enc.h, te.TE_OPT_KERNEL_TIMING, 0)
 
+    dispatch = te.te_dispatch_info(enc.h)
+
     overlap = None
-    if args.overlap and rank == 0:
+    if not args.no_overlap and rank == 0:
         overlap = measure_overlap(torch, step, stream, ms_per_step)
+
+    # ---- secondary: BASELINE.json's metric is quoted "at B=4/16": the same handle (same 28-layer weights) also
+    # encodes cfg 3's batch (4 frames x 128 tokens), timed the same way, so the driver's record covers both.
+    secondary = None
+    if (not args.no_secondary and rank == 0 and args.config == 4 and args.frames == 0 and args.prefix == 0
+            and not args.opt):
+        secondary = {}
+        w3 = W.get_workload(3)
+        tl3 = W.make_text_lens(w3)
+        T3 = W.total_tokens(w3, tl3)
+        e3 = torch.from_numpy(W.make_embeddings(w3, T3)).cuda()
+        l3 = torch.from_numpy(tl3).cuda()
+        o3 = torch.empty_like(e3)
+        n3 = max(20, min(args.steps, 100))
+        with torch.cuda.stream(stream):
+            for _ in range(max(3, args.warmup)):
+                enc.encode(w3.n_frames, w3.grid_h, w3.grid_w, e3, l3, T3, o3, stream.cuda_stream)
+            ev3 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n3)]
+            for a, b in ev3:
+                a.record(stream)
+                enc.encode(w3.n_frames, w3.grid_h, w3.grid_w, e3, l3, T3, o3, stream.cuda_stream)
+                b.record(stream)
+        torch.cuda.synchronize()
+        ms3 = [a.elapsed_time(b) for a, b in ev3]
+        t3 = sum(ms3) / 1000.0 / n3
+        f3, wb3, ab3 = stack_work(w3.model, [w3.grid_h * w3.grid_w + int(t) for t in tl3])
+        pk = load_peaks()
+        roof3 = max(f3 / (pk["tf_burst"] * 1e12), (wb3 + ab3) / (pk["hbm_gbs"] * 1e9))
+        secondary[w3.name] = {
+            "metric": METRIC, "value": w3.n_frames / t3, "unit": UNIT, "tokens_per_s": T3 / t3,
+            "ms_per_step": 1000.0 * t3, "ms_per_step_min": min(ms3), "steps": n3,
+            "config": config_dict(w3, T3, world), "dispatch": te.te_dispatch_info(enc.h),
+            "stack_roofline": {"flops": f3, "weight_bytes": wb3, "act_bytes": ab3, "roofline_ms_burst": 1000 * roof3,
+                               "frac_of_burst": roof3 / t3,
+                               "frac_of_sustained": max(f3 / (pk["tf_sustained"] * 1e12),
+                                                        (wb3 + ab3) / (pk["hbm_gbs"] * 1e9)) / t3},
+        }
 
     if rank != 0:
         if dist is not None:
@@ -417,56 +496,63 @@ def main():
         return
 
     peaks = load_peaks()
-    # dram__bytes_read.sum + dram__bytes_write.sum of one gate/up launch, from the committed ncu --set full
-    # capture (profiles/r01f_cfg4.md)
-    # (cfg 2: profiles/r01d_ncu_full_small_batch.md, gate/up on the split-K kernel)
-    traffic = {"cfg4_28L_B16": 63.364864e6 + 15.521024e6, "cfg2_1L_B1": 50.973952e6 + 1.491456e6}.get(w.name)
     flops, wbytes, abytes = stack_work(m, seq_lens)
     flops += m.n_layers * sum(4.0 * m.head_dim * m.n_q_heads * s * args.prefix for s in seq_lens)  # prefix keys
+    t_step = t_dev / args.steps
     t_compute = flops / (peaks["tf_sustained"] * 1e12)
     t_hbm = (wbytes + abytes) / (peaks["hbm_gbs"] * 1e9)
     t_roof = max(t_compute, t_hbm)
+    # Per-kernel times: the CUDA-event pass brackets every launch (direct launches, PDL off), so its times include the
+    # launch gaps and fills that the graph replay overlaps; they are reported as measured AND scaled so that the
+    # kernels sum to the graph-replay step (`in_graph` = event time x step / sum of event times).
+    ksum = sum(v[0] for v in ktimes.values()) / max(1, args.kernel_timing_steps)     # ms per step, event pass
+    scale = (1000.0 * t_step) / ksum if ksum else None
+    kernels = {k: {"kernel": dispatch.get(k), "ms_per_launch_events": (v[0] / v[1] if v[1] else None),
+                   "ms_per_launch_in_graph": (v[0] / v[1] * scale if v[1] and scale else None),
+                   "launches_per_step": v[1] // max(1, args.kernel_timing_steps),
+                   "share": (v[0] / args.kernel_timing_steps / ksum if ksum else None)}
+               for k, v in ktimes.items() if v[1]}
     # dominant kernel: gate/up GEMM (50 % of the stack's FLOPs): 2 * T * d * 2F per launch
     gu_ms, gu_n = ktimes["gateup"]
+    gu_ms_launch = gu_ms / gu_n                      # CUDA events on the launching stream, as the contract asks
     gu_flops = 2.0 * T * m.hidden * 2 * m.ffn
-    ksum = sum(v[0] for v in ktimes.values())
-    kernels = {k: {"ms_per_launch": (v[0] / v[1] if v[1] else None), "launches": v[1],
-                   "share": (v[0] / ksum if ksum else None)} for k, v in ktimes.items() if v[1]}
+    gu_bytes = 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
+    gu_name = dispatch.get("gateup", "?")
+    traffic, traffic_src = PROFILED_TRAFFIC.get((w.name, gu_name.split(" (")[0]), (None, None))
+    region = f"{args.steps} steps = {t_dev:.2f} s timed region; per-kernel pass {args.kernel_timing_steps} steps"
     if t_compute >= t_hbm:
-        achieved = gu_flops / (gu_ms / gu_n / 1000.0) / 1e12
-        roofline = {"bound": "tensor", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
-                    "peak": peaks["tf_sustained"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sustained"],
-                    "peak_kind": f"bf16_tflops_sustained ({peaks['src']}); kernel timed inside a long step",
-                    "frac_of_burst": achieved / peaks["tf_burst"], "traffic": traffic,
-                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01f)",
-                    "algorithmic_bytes": 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn}
+        achieved = gu_flops / (gu_ms_launch / 1000.0) / 1e12
+        roofline = {"bound": "tensor", "kernel": gu_name + " (gate/up)", "achieved": achieved,
+                    "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_burst"],
+                    "peak_kind": f"bf16_tflops burst ({peaks['src']}): the kernel is timed launch by launch with CUDA "
+                                 f"events ({region})",
+                    "frac_of_sustained": achieved / peaks["tf_sustained"], "peak_sustained": peaks["tf_sustained"],
+                    "achieved_in_graph": gu_flops / (gu_ms_launch * scale / 1000.0) / 1e12 if scale else None,
+                    "traffic": traffic, "traffic_src": traffic_src or "not measured in this run (ncu capture pending)",
+                    "traffic_unit": "bytes per launch (ncu dram read+write)", "algorithmic_bytes": gu_bytes}
     else:
-        gu_bytes = 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
-        achieved = gu_bytes / (gu_ms / gu_n / 1000.0) / 1e9
-        roofline = {"bound": "hbm", "kernel": "te_gemm_kernel<256,EPI_SWIGLU> (gate/up)", "achieved": achieved,
+        achieved = gu_bytes / (gu_ms_launch / 1000.0) / 1e9
+        roofline = {"bound": "hbm", "kernel": gu_name + " (gate/up)", "achieved": achieved,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                    "peak_kind": f"hbm_gbs ({peaks['src']})", "traffic": traffic,
-                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01d)", "algorithmic_bytes": gu_bytes}
+                    "peak_kind": f"hbm_gbs ({peaks['src']}); {region}", "traffic": traffic,
+                    "traffic_src": traffic_src or "not measured in this run (ncu capture pending)",
+                    "traffic_unit": "bytes per launch (ncu dram read+write)", "algorithmic_bytes": gu_bytes}
 
     cpu_baseline = None
     if not args.no_cpu_baseline:
         r = time_oracle(w, blob, tl, emb, 25.0, 3)
         cpu_baseline = {"value": r["frames_per_s"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                        "nproc": r["nproc"], "cpu_model": r["cpu_model"], "blas": r["blas"],
                         "sample": r["sample"], "tokens_per_s": r["tokens_per_s"]}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": w.name, "n_frames_per_gpu": w.n_frames, "total_tokens_per_gpu": T,
-                   "n_layers": m.n_layers, "hidden": m.hidden,
-                   "l2": ("L2 flushed (256 MiB memset) before every timed step" if flush_l2 else
-                          "no flush: per-step working set (2.8 GB weights + activations) exceeds the 126 MB L2"),
-                   "parallelism": f"replica x{world} (frames sharded, no collective)",
-                   "opt": args.opt or "defaults",
-                   **({"prefix_len": args.prefix, "prefix_pass_ms_once": prefix_ms,
-                       "prefix": "shared text prefix encoded once, K/V reused by every frame (SURVEY 8f NEXT-1)"}
-                      if args.prefix > 0 else {})},
+        "config": config_dict(w, T, world, args.opt or "defaults", flush_l2,
+                              ({"prefix_len": args.prefix, "prefix_pass_ms_once": prefix_ms,
+                                "prefix": "shared text prefix encoded once, K/V reused by every frame (SURVEY 8f NEXT-1)"}
+                               if args.prefix > 0 else None)),
         "tokens_per_s": tokens_per_s,
         "ms_per_step_min": min(step_ms), "ms_per_step_median": statistics.median(step_ms),
         "wall_ms_per_step": 1000.0 * t_wall / args.steps,
@@ -475,17 +561,23 @@ def main():
                 "api": "te_encode_host_submit / te_encode_host_wait, two batches in flight, pinned host buffers",
                 "blocking_call_value": e2e_blocking, "blocking_call_ms_per_step": 1000.0 * t_blocking / args.steps},
         "gpu_launches": int(launches),
+        "graph_captures": te.te_graph_captures(enc.h),
         "clocks": clocks,
         "roofline": roofline,
         "stack_roofline": {"flops": flops, "weight_bytes": wbytes, "act_bytes": abytes,
                            "t_compute_ms": 1000 * t_compute, "t_hbm_ms": 1000 * t_hbm,
                            "bound": "tensor" if t_compute >= t_hbm else "hbm",
-                           "frac_of_sustained": t_roof / (t_dev / args.steps),
-                           "frac_of_burst": max(flops / (peaks["tf_burst"] * 1e12), t_hbm) / (t_dev / args.steps),
-                           "achieved_tflops": flops / (t_dev / args.steps) / 1e12, "peaks": peaks},
+                           "frac_of_sustained": t_roof / t_step,
+                           "frac_of_burst": max(flops / (peaks["tf_burst"] * 1e12), t_hbm) / t_step,
+                           "achieved_tflops": flops / t_step / 1e12, "peaks": peaks},
+        "dispatch": dispatch,
         "kernels": kernels,
+        "kernels_note": "ms_per_launch_events: CUDA events around each direct launch (PDL off); ms_per_launch_in_graph: "
+                        "the same, scaled so that the kernels sum to the graph-replay step",
         "cpu_baseline": cpu_baseline,
     }
+    if secondary is not None:
+        line["secondary"] = secondary
     if overlap is not None:
         line["overlap"] = overlap
     print(json.dumps(line), flush=True)

@@ -14,7 +14,8 @@
  *
  * Conventions.  Plain C, no torch types.  Every pointer argument says HOST or DEVICE.  All
  * functions return 0 (TE_OK) or a negative te_status; none throws, aborts or prints.
- * The library is single-GPU and not thread-safe per handle.  The small-batch (split-K) kernels
+ * The library is single-GPU; a handle must not be used from two host threads at once, different handles may be
+ * (all launch state is per handle).  The small-batch (split-K) kernels
  * synchronise the CTAs of a group through device memory; they are launched as cooperative grids
  * (all CTAs resident at once, at most one CTA per SM), so other work on the GPU — another handle
  * on another stream, a denoiser (bench.py --overlap) — can delay them but not deadlock them.  There is NO CPU fallback:
@@ -89,13 +90,14 @@ int te_load_weights(te_handle* h, const void* bf16_blob, size_t n_bytes);
  *                 rows cu[b]..cu[b+1), S_b = grid_h*grid_w + text_lens[b], visual tokens first
  *   text_lens     DEVICE int32 [n_frames]
  *   total_tokens  HOST value; must equal sum_b S_b (checked on the device, see below)
- *   out           DEVICE fp32 [total_tokens, hidden]; last-layer hidden states (the fp32
- *                 residual stream itself).  Must not alias embeds.
+ *   out           DEVICE fp32 [total_tokens, hidden]; last-layer hidden states.  Must not alias embeds.
  *   cuda_stream   a cudaStream_t (NULL = legacy default stream)
  * Position ids (t,h,w), packing offsets and the rotary table are computed on the device from
  * text_lens; the call enqueues work and returns: NO stream synchronisation, NO device->host
- * copy, no allocation once the (shape, pointer) key has been seen — the property the paper's
- * TE lacks.  The whole stack is one CUDA-graph launch (cached per key).
+ * copy, no allocation once the call's shape class has been seen (te_graph_captures) — the property the
+ * paper's TE lacks.  The whole stack is one CUDA-graph launch behind a one-thread kernel
+ * that refreshes the per-call pointers; `out` is written only by the last kernel of the stack (the fp32
+ * residual stream itself lives in library memory).
  * Conditions only knowable on the device (sum of lengths != total_tokens, text_len < 0,
  * S_b > max_tokens_per_frame) raise a sticky device flag; the kernels then touch no row
  * >= total_tokens; read the flag with te_query_async_error. */
@@ -141,42 +143,39 @@ int te_encode_host_wait(te_handle* h, int32_t slot);
  * was raised since the last query (and clears it), TE_ERR_CUDA on a CUDA error, else TE_OK. */
 int te_query_async_error(te_handle* h);
 
-/* Options. */
+/* Options (te_set_option).  Tuning and test switches live in te_debug.h. */
 enum {
   TE_OPT_USE_GRAPH = 0,    /* 1 (default): te_encode = one cudaGraphLaunch; 0: direct launches   */
   TE_OPT_KERNEL_TIMING = 1,/* 1: direct launches bracketed by CUDA events per kernel (implies no
                               graph); read with te_kernel_times.  Measurement aid, default 0.     */
-  TE_OPT_CTA_PAIR = 2,     /* GEMM tiling: 0 = one CTA per 128-row tile, 1 = CTA pairs (cta_group::2,
-                              256-row tiles), 2 = auto by token count (default)                    */
-  TE_OPT_RESID_BLOCK_N = 3,/* tile width (128 default, or 256) of the O-proj / down GEMMs          */
   TE_OPT_PDL = 4,          /* 1 (default): kernels are chained with programmatic dependent launch   */
-  TE_OPT_TRACE = 5,        /* 1: CTA-pair GEMM kernels stamp %globaltimer at pipeline events (debug
-                              aid; read with te_debug_tap(TE_TAP_TRACE)); default 0                 */
-  TE_OPT_ATTN_IMPL = 6,    /* attention kernel: 1 (default) = tcgen05 kernel (S, P, O in tensor memory)
-                              when Hq/Hkv is a power of two <= 8, 0 = mma.sync flash kernel          */
-  TE_OPT_STREAM_K = 8,     /* 1: the CTA-pair GEMM kernels give every SM pair an equal contiguous share of the
-                              (tile, k-block) work units (stream-K); a tile cut by a share boundary is completed
-                              by the pair that holds its first k-blocks, on top of the other pieces' fp32 partials
-                              summed in a fixed order (deterministic).  0 (default): whole tiles, round-robin —
-                              measured faster on every config                                    */
-  TE_OPT_RESID_WIDE = 9,   /* O-proj / down on CTA pairs: 1 (default) = when their 128-wide tiles would need two or
-                              more waves, ONE wave of wide tiles (width = hidden / n rounded up to 32, <= 512
-                              columns, two MMAs per k-step; te_gemm_wide.cuh); 0 = never; n in 2..16 = always,
-                              with n tiles across the hidden dimension (tests)                                  */
-  TE_OPT_L2_RESIDUAL = 10, /* 1 (default): the fp32 residual stream (`out`) is an L2-persisting access-policy window
+  TE_OPT_L2_RESIDUAL = 10  /* 1 (default): the library's fp32 residual stream is an L2-persisting access-policy window
                               of every kernel, so that the residual GEMMs' read-add-write passes stay out of DRAM.
                               The first te_encode raises the DEVICE-WIDE limit cudaLimitPersistingL2CacheSize to
-                              min(max_tokens * hidden * 4, 64 MiB, device maximum).  0: no window                 */
-  TE_OPT_SPLIT_K = 7       /* 1 (default): small batches (fewer 128-row tiles than SMs in a GEMM, no
-                              CTA pairs) run the split-K kernel: several CTAs per output tile, each
-                              streaming its own K-slice of the weights; partial tiles are summed in a
-                              fixed order (deterministic).  0: one CTA per tile                      */
+                              min(max_tokens * hidden * 4, 64 MiB, device maximum) if it is lower; te_destroy and
+                              setting this option to 0 reset the persisting lines and restore the previous limit.
+                              0: no window                                                                        */
 };
 int te_set_option(te_handle* h, int option, int value);
 
-/* Number of kernels the library has launched so far on behalf of te_encode (graph replays
- * count the kernel nodes they contain).  For bench.py's `gpu_launches`. */
+/* Number of kernels the library has launched so far on behalf of te_encode / te_encode_prefix (graph replays
+ * count the kernel nodes they contain, plus the one parameter-refresh kernel ahead of them).  For bench.py's
+ * `gpu_launches`. */
 int64_t te_kernel_launches(te_handle* h);
+
+/* Number of CUDA-graph captures (capture + instantiate) te_encode has performed on this handle.  A graph is keyed
+ * on the SHAPE CLASS of a call — (n_frames, grid, row-block bucket of total_tokens, prefix length, layer range) —
+ * not on the caller's pointers or the exact token count (those travel through a device-side parameter block that
+ * a one-thread kernel refreshes ahead of the graph): a stream of ragged batches, or a caller whose allocator
+ * hands back different buffers, replays cached graphs (PAPER.md:356 — prompt length varies
+ * per call).  Bucket: total_tokens rounded up to 128 rows, to 256 rows from 1024 on; 32 graphs are kept (LRU). */
+int64_t te_graph_captures(te_handle* h);
+
+/* Which kernels the last te_encode ran, per class, in the names a profiler prints, e.g.
+ * "qkv=te_gemm2_kernel<256, 1, 128>;attn=te_attn_tc_kernel<128>;oproj=te_gemm_wide_kernel<2> (6 tiles x 352 cols);..."
+ * (template arguments: tile width, epilogue id, head_dim).  HOST buffer; truncated to n_bytes.  For bench.py's
+ * roofline label. */
+int te_dispatch_info(te_handle* h, char* buf_host, size_t n_bytes);
 
 /* Per-kernel-class device time accumulated by calls made under TE_OPT_KERNEL_TIMING, measured with
  * CUDA events on the launching stream.  Synchronises; fills ms_sum[TE_KCLASS_COUNT] and
@@ -186,41 +185,6 @@ enum {
   TE_KCLASS_GATEUP = 5, TE_KCLASS_DOWN = 6, TE_KCLASS_FINAL_NORM = 7, TE_KCLASS_COUNT = 8
 };
 int te_kernel_times(te_handle* h, float* ms_sum, int32_t* n_launches);
-
-/* ---- test-only taps (SURVEY.md §8b "Debug taps") ------------------------------------------
- * te_debug_set_range restricts subsequent te_encode calls to layers [layer_begin, layer_end)
- * (embeds is then the teacher-forced input residual of layer_begin) and, if stop_after_attn,
- * stops the last layer after the O-projection residual add.  (0, n_layers, 0) restores the
- * full stack.  te_debug_tap synchronises and copies the CURRENT content of a workspace buffer
- * (as left by the last te_encode, i.e. of the last layer run) to `dst` (HOST). */
-enum {
-  TE_TAP_POS = 0,        /* int32 [3, T]        rows t,h,w                       */
-  TE_TAP_CU_SEQLENS = 1, /* int32 [B+1]                                         */
-  TE_TAP_COS = 2,        /* fp32  [T, dh/2]                                     */
-  TE_TAP_SIN = 3,        /* fp32  [T, dh/2]                                     */
-  TE_TAP_QKV = 4,        /* bf16  [T, (Hq+2Hkv)*dh]  q (normed+rotated) | k | v  */
-  TE_TAP_ATTN = 5,       /* bf16  [T, Hq*dh]                                    */
-  TE_TAP_ACT = 6,        /* bf16  [T, F]       silu(gate)*up                    */
-  TE_TAP_TRACE = 7       /* u64   [4 GEMM classes (qkv,oproj,gateup,down)][n_SMs][48] ns stamps
-                            of the last launch of each class (TE_OPT_TRACE)     */
-};
-int te_debug_set_range(te_handle* h, int32_t layer_begin, int32_t layer_end,
-                       int32_t stop_after_attn);
-int te_debug_tap(te_handle* h, int what, void* dst_host, size_t n_bytes);
-
-/* Test-only: C[M,N] (DEVICE fp32, row-major) = A[M,K] * B[N,K]^T with A, B DEVICE bf16
- * row-major, through the same TMA + tcgen05 main loop as the stack's GEMMs (plain epilogue).
- * K % 64 == 0, N % block_n == 0, block_n in {128, 256}; cta_pair = 1 selects the cta_group::2
- * kernel (256-row tiles) with whole tiles per pair, cta_pair = 2 the same kernel with stream-K
- * scheduling.  Synchronous. */
-int te_debug_gemm(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
-                  int32_t n, int32_t k, int32_t block_n, int32_t cta_pair);
-
-/* Test-only: the same product through the split-K kernel (te_gemm_splitk.cuh): `splits` CTAs
- * (1..8, <= k/64) per 128 x block_n tile, fixed-order reduction of the fp32 partial tiles.
- * Needs tiles * splits <= number of SMs (TE_ERR_UNSUPPORTED otherwise).  Synchronous. */
-int te_debug_gemm_splitk(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
-                         int32_t n, int32_t k, int32_t block_n, int32_t splits);
 
 void te_destroy(te_handle* h);
 const char* te_strerror(int code);

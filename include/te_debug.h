@@ -1,0 +1,75 @@
+/*
+ * te_debug.h — test-only taps, stand-alone GEMM entry points and tuning switches of libte_b200.so
+ * (SURVEY.md §8b "Debug taps").  Not part of the product boundary (include/te.h); the parity tests and
+ * bench.py's experiment flags use them.  Same conventions as te.h (plain C, HOST/DEVICE stated, te_status).
+ */
+#ifndef TE_B200_DEBUG_H_
+#define TE_B200_DEBUG_H_
+
+#include "te.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Tuning / test options for te_set_option (defaults are what bench.py measures). */
+enum {
+  TE_OPT_CTA_PAIR = 2,     /* GEMM tiling: 0 = one CTA per 128-row tile, 1 = CTA pairs (cta_group::2,
+                              256-row tiles), 2 = auto by token count (default)                    */
+  TE_OPT_RESID_BLOCK_N = 3,/* tile width (128 default, or 256) of the O-proj / down GEMMs          */
+  TE_OPT_TRACE = 5,        /* 1: CTA-pair GEMM kernels stamp %globaltimer at pipeline events (debug
+                              aid; read with te_debug_tap(TE_TAP_TRACE)); default 0                 */
+  TE_OPT_ATTN_IMPL = 6,    /* attention kernel: 1 (default) = tcgen05 kernel (S, P, O in tensor memory)
+                              when Hq/Hkv is a power of two <= 8, 0 = mma.sync flash kernel          */
+  TE_OPT_SPLIT_K = 7,      /* 1 (default): small batches (fewer 128-row tiles than SMs in a GEMM, no
+                              CTA pairs) run the split-K kernel: several CTAs per output tile, each
+                              streaming its own K-slice of the weights; partial tiles are summed in a
+                              fixed order (deterministic).  0: one CTA per tile; n > 1: target CTA count */
+  TE_OPT_RESID_WIDE = 9    /* O-proj / down on CTA pairs: 1 (default) = when their 128-wide tiles would need two or
+                              more waves, ONE wave of wide tiles (width = hidden / n rounded up to 32, <= 512
+                              columns, two MMAs per k-step; te_gemm_wide.cuh); 0 = never; n in 2..16 = always,
+                              with n tiles across the hidden dimension (tests)                                  */
+};
+
+/* te_debug_set_range restricts subsequent te_encode calls to layers [layer_begin, layer_end)
+ * (embeds is then the teacher-forced input residual of layer_begin) and, if stop_after_attn,
+ * stops the last layer after the O-projection residual add.  (0, n_layers, 0) restores the
+ * full stack.  te_debug_tap synchronises and copies the CURRENT content of a workspace buffer
+ * (as left by the last te_encode, i.e. of the last layer run) to `dst` (HOST). */
+enum {
+  TE_TAP_POS = 0,        /* int32 [3, T]        rows t,h,w                       */
+  TE_TAP_CU_SEQLENS = 1, /* int32 [B+1]                                         */
+  TE_TAP_COS = 2,        /* fp32  [T, dh/2]                                     */
+  TE_TAP_SIN = 3,        /* fp32  [T, dh/2]                                     */
+  TE_TAP_QKV = 4,        /* bf16  [T, (Hq+2Hkv)*dh]  q (normed+rotated) | k | v  */
+  TE_TAP_ATTN = 5,       /* bf16  [T, Hq*dh]                                    */
+  TE_TAP_ACT = 6,        /* bf16  [T, F]       silu(gate)*up                    */
+  TE_TAP_TRACE = 7       /* u64   [4 GEMM classes (qkv,oproj,gateup,down)][n_SMs][96] ns stamps / SM clocks
+                            of the last launch of each class (TE_OPT_TRACE)     */
+};
+int te_debug_set_range(te_handle* h, int32_t layer_begin, int32_t layer_end,
+                       int32_t stop_after_attn);
+int te_debug_tap(te_handle* h, int what, void* dst_host, size_t n_bytes);
+
+/* C[M,N] (DEVICE fp32, row-major) = A[M,K] * B[N,K]^T with A, B DEVICE bf16 row-major, through the
+ * same TMA + tcgen05 main loop as the stack's GEMMs (plain epilogue).  K % 64 == 0, N % block_n == 0,
+ * block_n in {128, 256}; cta_pair = 1 selects the cta_group::2 kernel (256-row tiles).  Synchronous. */
+int te_debug_gemm(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
+                  int32_t n, int32_t k, int32_t block_n, int32_t cta_pair);
+
+/* The same product through the split-K kernel (te_gemm_splitk.cuh): `splits` CTAs (1..8, <= k/64) per
+ * 128 x block_n tile, fixed-order reduction of the fp32 partial tiles.  Needs tiles * splits <= number
+ * of SMs (TE_ERR_UNSUPPORTED otherwise).  Synchronous. */
+int te_debug_gemm_splitk(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
+                         int32_t n, int32_t k, int32_t block_n, int32_t splits);
+
+/* The same product through the one-wave wide-tile kernel (te_gemm_wide.cuh): n_tiles CTA-pair tiles across N,
+ * each 256 rows x (N / n_tiles rounded up to 32) columns, two MMAs per k-step; the last tile may be partly or
+ * wholly out of range.  N % 32 == 0, width <= 512, ceil(M/256) * n_tiles <= SM pairs.  Synchronous. */
+int te_debug_gemm_wide(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
+                       int32_t n, int32_t k, int32_t n_tiles);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TE_B200_DEBUG_H_ */

@@ -27,17 +27,18 @@ TE_OPT_PDL = 4
 TE_OPT_TRACE = 5
 TE_OPT_ATTN_IMPL = 6
 TE_OPT_SPLIT_K = 7
-TE_OPT_STREAM_K = 8
 TE_OPT_RESID_WIDE = 9
 TE_OPT_L2_RESIDUAL = 10
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 
+# include/te.h (the product boundary) and include/te_debug.h (test-only taps and stand-alone GEMMs)
 EXPORTS = [
-    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host", "te_encode_host_submit", "te_encode_host_wait",
-    "te_query_async_error", "te_set_option", "te_kernel_launches", "te_kernel_times", "te_debug_set_range",
-    "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_destroy", "te_strerror", "te_last_error",
+    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host",
+    "te_encode_host_submit", "te_encode_host_wait", "te_query_async_error", "te_set_option", "te_kernel_launches",
+    "te_graph_captures", "te_dispatch_info", "te_kernel_times", "te_destroy", "te_strerror", "te_last_error",
 ]
+DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide"]
 
 
 class TEConfig(Structure):
@@ -93,6 +94,10 @@ def lib() -> ctypes.CDLL:
     L.te_set_option.argtypes = [c_void_p, c_int, c_int]
     L.te_kernel_launches.restype = c_int64
     L.te_kernel_launches.argtypes = [c_void_p]
+    L.te_graph_captures.restype = c_int64
+    L.te_graph_captures.argtypes = [c_void_p]
+    L.te_dispatch_info.restype = c_int
+    L.te_dispatch_info.argtypes = [c_void_p, c_void_p, c_size_t]
     L.te_kernel_times.restype = c_int
     L.te_kernel_times.argtypes = [c_void_p, c_void_p, c_void_p]
     L.te_debug_set_range.restype = c_int
@@ -103,6 +108,8 @@ def lib() -> ctypes.CDLL:
     L.te_debug_gemm.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
     L.te_debug_gemm_splitk.restype = c_int
     L.te_debug_gemm_splitk.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
+    L.te_debug_gemm_wide.restype = c_int
+    L.te_debug_gemm_wide.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
     L.te_destroy.restype = None
     L.te_destroy.argtypes = [c_void_p]
     L.te_strerror.restype = c_char_p
@@ -204,6 +211,17 @@ def te_kernel_launches(h) -> int:
     return int(lib().te_kernel_launches(h))
 
 
+def te_graph_captures(h) -> int:
+    return int(lib().te_graph_captures(h))
+
+
+def te_dispatch_info(h) -> dict:
+    """{class: kernel name as a profiler prints it} of the last te_encode (+ "bucket_tokens")."""
+    buf = ctypes.create_string_buffer(1024)
+    _check(lib().te_dispatch_info(h, buf, 1024), h)
+    return dict(kv.split("=", 1) for kv in buf.value.decode().split(";") if "=" in kv)
+
+
 def te_kernel_times(h) -> dict:
     """{class name: (ms_sum, n_launches)} accumulated under TE_OPT_KERNEL_TIMING; resets."""
     n = len(TE_KCLASS_NAMES)
@@ -227,6 +245,10 @@ def te_debug_gemm(device, a_bf16, b_bf16, c, m, n, k, block_n=256, cta_pair=0):
 
 def te_debug_gemm_splitk(device, a_bf16, b_bf16, c, m, n, k, block_n=128, splits=2):
     _check(lib().te_debug_gemm_splitk(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, splits))
+
+
+def te_debug_gemm_wide(device, a_bf16, b_bf16, c, m, n, k, n_tiles):
+    _check(lib().te_debug_gemm_wide(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, n_tiles))
 
 
 def te_destroy(h):

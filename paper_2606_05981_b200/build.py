@@ -18,6 +18,7 @@ def _stale() -> bool:
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS]
     deps.append(os.path.join(HERE, "..", "include", "te.h"))
+    deps.append(os.path.join(HERE, "..", "include", "te_debug.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -22,7 +22,6 @@ struct AttnParams {
   const int32_t* cu_seqlens; // [B+1]
   int ld;
   int n_q_heads, n_kv_heads;
-  int total_tokens;
   float scale_log2;  // log2(e) / sqrt(dh)
   // shared text prefix (te_encode_prefix): P cached keys/values per layer that every query of every frame
   // sees in front of its own causal keys.  kv_prefix: [P, ld_prefix] = k heads | v heads; null when P = 0.
@@ -92,7 +91,7 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");  // qkv / cu_seqlens come from predecessor kernels
   const int seq0 = p.cu_seqlens[b];
-  const int S = min(p.cu_seqlens[b + 1], p.total_tokens) - seq0;
+  const int S = p.cu_seqlens[b + 1] - seq0;  // (te_prep_kernel clamps the offsets to the call's token count)
   const int q0 = qb * ATT_BQ;
   if (q0 >= S) return;
   const int kvh = head0 / (p.n_q_heads / p.n_kv_heads);

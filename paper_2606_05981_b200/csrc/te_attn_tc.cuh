@@ -26,7 +26,6 @@ struct AttnTcParams {
   const int32_t* cu_seqlens;  // [B+1]
   int n_q_heads, n_kv_heads;
   int g_shift;  // log2(Hq / Hkv)
-  int total_tokens;
   float scale_log2;  // log2(e) / sqrt(dh)
   // Shared text prefix (te_encode_prefix), handled as a SECOND launch of this kernel per layer:
   //   launch 1 (prefix_mode 0, stats != null): frame-local causal attention as usual, plus the row statistics
@@ -122,7 +121,7 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int seq0 = p.cu_seqlens[b];
   // (a frame longer than KMAX raised the device validation flag in te_scan_kernel; clamp so that the
   //  shared-memory tiles are never overrun)
-  const int S = min(min(p.cu_seqlens[b + 1], p.total_tokens) - seq0, Cfg::KMAX);
+  const int S = min(p.cu_seqlens[b + 1] - seq0, Cfg::KMAX);  // (offsets are clamped to the token count by te_prep_kernel)
   const int n_tiles = (S + PT - 1) / PT;
   const int n_my = (n_tiles > split) ? (n_tiles - split + n_split - 1) / n_split : 0;
   const int S16 = (S + 15) & ~15;

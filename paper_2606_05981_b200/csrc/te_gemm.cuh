@@ -26,8 +26,20 @@ constexpr int GEMM_THREADS = 192;
 
 enum { EPI_PLAIN = 0, EPI_QKV = 1, EPI_RESID = 2, EPI_SWIGLU = 3 };
 
+// Per-call values that a cached graph must not bake in: written on the stream ahead of the stack's kernels
+// (te_set_dyn_kernel), read by every kernel.  A graph is therefore reusable for any caller buffers and for any
+// token count of the same row-block bucket (te_runtime.cu, graph cache).
+struct DynParams {
+  const float* embeds;       // DEVICE fp32 [T, d]
+  const int32_t* text_lens;  // DEVICE int32 [B]
+  float* out;                // DEVICE fp32 [T, d]
+  int32_t total_tokens;      // T
+  int32_t pad_;
+};
+
 struct GemmParams {
-  int M, N, K;
+  int M, N, K;               // M: rows when dyn == nullptr (te_debug_gemm*); else dyn->total_tokens
+  const DynParams* dyn;
   int num_m_blk, num_n_blk;
   // RMSNorm statistics of the A rows (consumer side): ssq_in[row * ssq_stride + part], one 16-byte-aligned
   // run of `ssq_parts` partial sums of squares per row (a row's parts share a cache line)
@@ -46,7 +58,8 @@ struct GemmParams {
   const float* cos_t;  // [T, DH/2]
   const float* sin_t;
   // EPI_RESID
-  float* x;
+  float* x;      // fp32 residual stream (library workspace), updated in place ...
+  int x_to_out;  // ... or, for the LAST residual GEMM of the stack, read from x and written to dyn->out
   int ld_x;
   const __nv_bfloat16* g_next;  // may be null (no next norm)
   __nv_bfloat16* xg;            // [T, ld_x] bf16(x * g_next)
@@ -63,13 +76,12 @@ struct GemmParams {
   int splits;
   float* sk_scratch;
   int* sk_sem;
-  // stream-K scheduling of the CTA-pair kernel: 1 = every pair gets an equal contiguous share of the
-  // (tile, k-block) work units; tiles cut by a share boundary are completed through sk_scratch / sk_sem
-  int streamk;
   // EPI_SWIGLU with 128-wide tiles over weights interleaved per 256 rows (128 gate | 128 up): tile n' takes gate
   // rows (n'>>1)*256 + (n'&1)*64 .. +64 and the matching up rows 128 further on, as two 64-row halves
   int gu_half;
 };
+__device__ __forceinline__ int gemm_rows(const GemmParams& p) { return p.dyn != nullptr ? p.dyn->total_tokens : p.M; }
+__device__ __forceinline__ float* resid_dst(const GemmParams& p) { return p.x_to_out ? p.dyn->out : p.x; }
 constexpr int TRACE_SLOTS = 96;  // [0,48): globaltimer ns, [48,96): SM clock of the same stamp
 __device__ __forceinline__ void trace_stamp(const GemmParams& p, int slot) {
   if (p.trace != nullptr) {
@@ -145,20 +157,21 @@ struct ResidPrefetch {
   float4 xv[8];
 };
 template <int BN>
-__device__ __forceinline__ void resid_issue(const GemmParams& p, ResidPrefetch& pf, int row_base, int lane, int n_blk,
-                                            int c0) {
+__device__ __forceinline__ void resid_issue(const GemmParams& p, int M, ResidPrefetch& pf, int row_base, int lane,
+                                            int n_blk, int c0) {
   const int sub = lane >> 3, cq = lane & 7;
   const int col = n_blk * BN + c0 + cq * 4;
   if (col >= p.N) return;  // chunk past the last column (N is not a multiple of a 192-wide tile)
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const int row = row_base + sub + 4 * i;
-    if (row < p.M) pf.xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
+    if (row < M) pf.xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
   }
 }
 template <int BN>
-__device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
+__device__ __forceinline__ void epi_resid(const GemmParams& p, int M, uint32_t t_row, int row_base, int lane, int n_blk,
                                           float* stg, int part, int nparts, ResidPrefetch& pf) {
+  float* const x_dst = resid_dst(p);
   const int sub = lane >> 3;  // row within a group of 4
   const int cq = lane & 7;    // 4-column group inside the 32-column chunk
   const bool has_g = p.g_next != nullptr;
@@ -188,16 +201,16 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
     float4 xv[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) xv[i] = pf.xv[i];
-    if (c0 + 32 < c_end) resid_issue<BN>(p, pf, row_base, lane, n_blk, c0 + 32);  // next chunk's x in flight
+    if (c0 + 32 < c_end) resid_issue<BN>(p, M, pf, row_base, lane, n_blk, c0 + 32);  // next chunk's x in flight
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const int rr = sub + 4 * i;
       const int row = row_base + rr;
-      if (row < p.M) {
+      if (row < M) {
         const float4 a = stg_get(stg, rr, cq);
         float4 v = xv[i];
         v.x += a.x; v.y += a.y; v.z += a.z; v.w += a.w;
-        *reinterpret_cast<float4*>(p.x + (size_t)row * p.ld_x + col) = v;
+        *reinterpret_cast<float4*>(x_dst + (size_t)row * p.ld_x + col) = v;
         ss[i] = fmaf(v.x, v.x, ss[i]); ss[i] = fmaf(v.y, v.y, ss[i]);
         ss[i] = fmaf(v.z, v.z, ss[i]); ss[i] = fmaf(v.w, v.w, ss[i]);
         if (has_g) {
@@ -221,7 +234,7 @@ __device__ __forceinline__ void epi_resid(const GemmParams& p, uint32_t t_row, i
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const int row = row_base + sub + 4 * i;
-      if (row < p.M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * nparts + part)] = ss[i];
+      if (row < M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * nparts + part)] = ss[i];
     }
   }
 }
@@ -261,7 +274,7 @@ __device__ __forceinline__ void stg_store_bf16(const float* buf, int lane, int r
 // SwiGLU epilogue: tile columns [0,BN/2) = gate, [BN/2,BN) = up (weights interleaved per tile).
 // The arithmetic runs in the thread-per-row domain; only the bf16 store is transposed.
 template <int BN>
-__device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
+__device__ __forceinline__ void epi_swiglu(const GemmParams& p, int M, uint32_t t_row, int row_base, int lane, int n_blk,
                                            float* stg, int part, int nparts, float rstd) {
   constexpr int HALF = BN / 2;
 #pragma unroll 1
@@ -281,7 +294,7 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
     }
     stg_put_row(stg, lane, a);
     __syncwarp();
-    stg_store_bf16(stg, lane, row_base, p.M, p.act, p.ld_act, n_blk * HALF + c0);
+    stg_store_bf16(stg, lane, row_base, M, p.act, p.ld_act, n_blk * HALF + c0);
     __syncwarp();
   }
 }
@@ -290,7 +303,7 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, uint32_t t_row, 
 // thread-per-row domain) and then gain + M-RoPE rotation of the pairs (i, i + DH/2) in the coalesced
 // domain, where the cos/sin rows are read as whole 128-byte segments.
 template <int BN, int DH>
-__device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int row_base, int lane, int n_blk,
+__device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_row, int row_base, int lane, int n_blk,
                                         float* stg, int part, int nparts, float rstd) {
   constexpr int HD2 = DH / 2;
   const int sub = lane >> 3, cq = lane & 7;
@@ -323,7 +336,7 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
         }
         stg_put_row(bufA, lane, v);
         __syncwarp();
-        stg_store_bf16(bufA, lane, row_base, p.M, p.qkv, p.ld_qkv, col0 + c0);
+        stg_store_bf16(bufA, lane, row_base, M, p.qkv, p.ld_qkv, col0 + c0);
         __syncwarp();
       }
       continue;
@@ -353,7 +366,7 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
       float4 cs[8], sn[8];
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        const int row = min(row_base + sub + 4 * i, p.M - 1);
+        const int row = min(row_base + sub + 4 * i, M - 1);
         cs[i] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc));
         sn[i] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc));
       }
@@ -380,7 +393,7 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, uint32_t t_row, int
       for (int i = 0; i < 8; ++i) {
         const int rr = sub + 4 * i;
         const int row = row_base + rr;
-        if (row < p.M) {
+        if (row < M) {
           const float4 a = stg_get(bufA, rr, cq);
           const float4 b = stg_get(bufB, rr, cq);
           const float ua[4] = {a.x * gA[0], a.y * gA[1], a.z * gA[2], a.w * gA[3]};
@@ -452,6 +465,7 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const uint32_t tmem_base = *tmem_slot;
   pdl_launch_dependents();
 
+  const int M = gemm_rows(p);
   const int num_kb = p.K / GEMM_BK;
   const int num_tiles = p.num_m_blk * p.num_n_blk;
 
@@ -530,21 +544,21 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
       const int row = m_blk * GEMM_BM + row_in_tile;
-      const bool valid = row < p.M;
+      const bool valid = row < M;
       // operands that do not depend on the accumulator are fetched while the main loop still runs
       float rstd = 0.f;
       ResidPrefetch pf;
       if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row, valid);
-      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, pf, m_blk * GEMM_BM + quad * 32, lane, n_blk, 0);
+      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, M, pf, m_blk * GEMM_BM + quad * 32, lane, n_blk, 0);
       mbar_wait(&tfull[acc], acc_phase);
       tc_fence_after();
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
       if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row, valid, n_blk, 0, 1);
       float* stg = stg_all + quad * (Cfg::STG_WARP_BYTES / 4);
       const int row_base = m_blk * GEMM_BM + quad * 32;
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1, pf);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, 0, 1, rstd);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, 0, 1, rstd);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, M, t_row, row_base, lane, n_blk, stg, 0, 1, pf);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, M, t_row, row_base, lane, n_blk, stg, 0, 1, rstd);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, M, t_row, row_base, lane, n_blk, stg, 0, 1, rstd);
       tc_fence_before();
       mbar_arrive(&tempty[acc]);
     }
@@ -563,56 +577,9 @@ te_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 // tcgen05.mma.cta_group::2 (M = 256), which reads both halves of B and writes rows 0-127 of D into
 // the leader's TMEM and rows 128-255 into the peer's.  Per SM this moves A 16 KB + B BN/2 x 128 B per
 // 64-deep k-block instead of A 16 KB + B BN x 128 B: 1.5x less L2->SM traffic at BN = 256.
+// Persistent: pair q takes tiles q, q + pairs, ...; two accumulator buffers, so the epilogue of one tile
+// overlaps the main loop of the next.
 constexpr int GEMM2_EPI_WARPS = 8;  // two per TMEM lane quadrant: the epilogue is issue-latency-bound per warp
-
-// Work of one CTA pair as a sequence of segments (tile, k-blocks [kb0, kb1)).
-//   classic : whole tiles pair, pair + num_pairs, ...
-//   stream-K: the pair's equal share [U*pair/NP, U*(pair+1)/NP) of the U = tiles * num_kb work units, cut at
-//             tile boundaries.  A tile cut by a share boundary has one HEAD piece (kb0 == 0; it is the LAST
-//             segment of its pair, which owns the tile's epilogue) and one or more later pieces, each the FIRST
-//             segment of the following pairs: those store their fp32 partial tile to the pair's scratch slot and
-//             raise the pair's flag; the owner's epilogue warps sum them in pair order INTO the accumulator buffer
-//             before the head piece's MMAs start (they accumulate on top; fixed order -> deterministic), i.e.
-//             while the owner's previous segment is still in its main loop: the fix-up is off the critical
-//             path.  A pair never waits before its first segment is published, so the waits cannot cycle.
-struct SegIter {
-  long long u, u_end;
-  int num_kb, tile_next, tile_step, num_tiles, streamk;
-  __device__ __forceinline__ SegIter(int pair, int num_pairs, int num_tiles_, int num_kb_, int streamk_)
-      : num_kb(num_kb_), tile_next(pair), tile_step(num_pairs), num_tiles(num_tiles_), streamk(streamk_) {
-    const long long U = (long long)num_tiles_ * num_kb_;
-    u = U * pair / num_pairs;
-    u_end = U * (pair + 1) / num_pairs;
-  }
-  __device__ __forceinline__ bool next(int& tile, int& kb0, int& kb1) {
-    if (!streamk) {
-      if (tile_next >= num_tiles) return false;
-      tile = tile_next; kb0 = 0; kb1 = num_kb;
-      tile_next += tile_step;
-      return true;
-    }
-    if (u >= u_end) return false;
-    tile = static_cast<int>(u / num_kb);
-    kb0 = static_cast<int>(u - (long long)tile * num_kb);
-    const long long e = min(u_end, (long long)(tile + 1) * num_kb);
-    kb1 = kb0 + static_cast<int>(e - u);
-    u = e;
-    return true;
-  }
-};
-__device__ __forceinline__ void gemm2_epi_bar() {  // named barrier 1: the epilogue warps of one CTA
-  asm volatile("bar.sync 1, %0;" ::"n"(32 * GEMM2_EPI_WARPS) : "memory");
-}
-__device__ __forceinline__ void tmem_st32_(uint32_t taddr, const uint32_t (&r)[32]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
-      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
-      "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
-      "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-      : "memory");
-}
 constexpr int GEMM2_THREADS = 64 + 32 * GEMM2_EPI_WARPS;
 
 template <int BN, int EPI>
@@ -682,43 +649,42 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   pdl_launch_dependents();
   if (threadIdx.x == 0) trace_stamp(p, 1);
 
+  const int M = gemm_rows(p);
   const int num_kb = p.K / GEMM_BK;
-  const int num_mp = (p.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);
+  const int num_mp = (p.num_m_blk + 1) >> 1;  // 256-row blocks
   const int num_tiles = num_mp * p.num_n_blk;
   const int pair = blockIdx.x >> 1;
   const int num_pairs = gridDim.x >> 1;
+  auto b_row_of = [&](int n_blk) {
+    return p.gu_half ? (n_blk >> 1) * 256 + static_cast<int>(rank) * 128 + (n_blk & 1) * 64
+                     : n_blk * BN + static_cast<int>(rank) * (BN / 2);
+  };
 
   if (warp == 0) {
     // ===================== TMA producer (both CTAs) =====================
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
-      SegIter seg(pair, num_pairs, num_tiles, num_kb, p.streamk);
-      int tile, kb0, kb1;
-      bool have = seg.next(tile, kb0, kb1);
       // weights first (independent of the predecessor kernel), then the dependency wait, then A
-      const int pre = have ? ((kb1 - kb0) < STAGES ? (kb1 - kb0) : STAGES) : 0;
-      if (have) {
-        const int nb0 = tile / num_mp;
-        const int b_row0 = p.gu_half ? (nb0 >> 1) * 256 + static_cast<int>(rank) * 128 + (nb0 & 1) * 64
-                                     : nb0 * BN + static_cast<int>(rank) * (BN / 2);
+      const int pre = (pair < num_tiles) ? (num_kb < STAGES ? num_kb : STAGES) : 0;
+      if (pre > 0) {
+        const int b_row0 = b_row_of(pair / num_mp);
         for (int i = 0; i < pre; ++i) {
           if (leader) mbar_arrive_expect_tx(&full[i], 2 * Cfg::STAGE_BYTES);
-          tma_load_2d_cg2(sB + i * Cfg::B_BYTES, &tmB, mapa_u32(smem_u32(&full[i]), 0), (kb0 + i) * GEMM_BK, b_row0);
+          tma_load_2d_cg2(sB + i * Cfg::B_BYTES, &tmB, mapa_u32(smem_u32(&full[i]), 0), i * GEMM_BK, b_row0);
         }
       }
       pdl_wait();
       trace_stamp(p, 2);
       bool first = true;
-      for (; have; have = seg.next(tile, kb0, kb1)) {
+      for (int tile = pair; tile < num_tiles; tile += num_pairs) {
         const int mp = tile % num_mp;
         const int n_blk = tile / num_mp;
         const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
-        const int b_row = p.gu_half ? (n_blk >> 1) * 256 + static_cast<int>(rank) * 128 + (n_blk & 1) * 64
-                                    : n_blk * BN + static_cast<int>(rank) * (BN / 2);
-        for (int kb = kb0; kb < kb1; ++kb) {
+        const int b_row = b_row_of(n_blk);
+        for (int kb = 0; kb < num_kb; ++kb) {
           const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
-          if (first && kb - kb0 < pre) {
+          if (first && kb < pre) {
             tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
           } else {
             mbar_wait(&empty[stage], phase ^ 1);
@@ -738,26 +704,21 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      SegIter seg(pair, num_pairs, num_tiles, num_kb, p.streamk);
-      int tile, kb0, kb1;
-      for (; seg.next(tile, kb0, kb1); ++it) {
+      for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
-        // the epilogue warps hand over each accumulator buffer explicitly (also before its first use): a
-        // stream-K head piece finds the other pieces' partial sums already in the buffer and accumulates on them
-        mbar_wait(&tempty[acc], acc_phase);
+        mbar_wait(&tempty[acc], acc_phase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * BN;
-        const bool preloaded = kb0 == 0 && kb1 != num_kb;
-        for (int kb = kb0; kb < kb1; ++kb) {
+        for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&full[stage], phase);
-          if (kb == kb0 && it < 10) trace_stamp(p, 3 + it);
+          if (kb == 0 && it < 10) trace_stamp(p, 3 + it);
           tc_fence_after();
           const uint64_t a_desc = umma_smem_desc_sw128(smem_u32(sA + stage * Cfg::A_BYTES));
           const uint64_t b_desc = umma_smem_desc_sw128(smem_u32(sB + stage * Cfg::B_BYTES));
 #pragma unroll
           for (int k = 0; k < GEMM_BK / 16; ++k)
-            umma_bf16_cg2(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (preloaded || kb > kb0 || k != 0) ? 1u : 0u);
+            umma_bf16_cg2(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
           umma_commit_cg2(&empty[stage], 0x3);  // frees this stage in BOTH CTAs
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
@@ -769,113 +730,30 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int quad = warp & 3;         // TMEM lane quadrant this warp may read
     const int part = (warp - 2) >> 2;  // which share of the tile's columns (two warps per quadrant)
     constexpr int NPARTS = GEMM2_EPI_WARPS / 4;
-    constexpr int COLS = BN / NPARTS;
-    constexpr size_t SLOT_F4 = (size_t)(BN / 4) * GEMM_BM;  // one CTA's fp32 partial tile: float4 [BN/4][128 rows]
-    const int row_in_tile = quad * 32 + lane;
     int it = 0;
     pdl_wait();
-    // Hand-over of an accumulator buffer to the MMA issuer for the segment (tile_n, [kb0_n, kb1_n)) that will use
-    // it next.  If that segment is a stream-K head piece, the later pieces of its tile (pairs q = pair+1, ... —
-    // each one the FIRST segment of its pair, so long done by the time this pair reaches its last one) are
-    // summed in pair order into the buffer first; the MMAs then accumulate on top (fixed order: deterministic).
-    auto hand_over = [&](bool have_n, int tile_n, int kb0_n, int kb1_n, int acc_n) {
-      if (have_n && kb0_n == 0 && kb1_n != num_kb) {
-        const uint32_t t_row_n = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc_n * BN;
-        const long long U = (long long)num_tiles * num_kb;
-        const long long tile_end = (long long)(tile_n + 1) * num_kb;
-        bool first_piece = true;
-        for (int q = pair + 1; q < num_pairs && U * q / num_pairs < tile_end; ++q) {
-          const int src_cta = 2 * q + static_cast<int>(rank);
-          if (warp == 2 && lane == 0) {
-            int v;
-            do {
-              asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p.sk_sem + src_cta) : "memory");
-            } while (v == 0);
-          }
-          gemm2_epi_bar();
-          const float4* src = reinterpret_cast<const float4*>(p.sk_scratch) + (size_t)src_cta * SLOT_F4;
-#pragma unroll 1
-          for (int c0 = part * COLS; c0 < (part + 1) * COLS; c0 += 32) {
-            float4 v[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) v[j] = __ldcg(src + (size_t)(c0 / 4 + j) * GEMM_BM + row_in_tile);
-            uint32_t r[32];
-            if (first_piece) {
-#pragma unroll
-              for (int j = 0; j < 32; ++j) r[j] = 0u;
-            } else {
-              tmem_ld32(t_row_n + c0, r);
-              tmem_ld_wait();
-            }
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              r[4 * j] = __float_as_uint(__uint_as_float(r[4 * j]) + v[j].x);
-              r[4 * j + 1] = __float_as_uint(__uint_as_float(r[4 * j + 1]) + v[j].y);
-              r[4 * j + 2] = __float_as_uint(__uint_as_float(r[4 * j + 2]) + v[j].z);
-              r[4 * j + 3] = __float_as_uint(__uint_as_float(r[4 * j + 3]) + v[j].w);
-            }
-            tmem_st32_(t_row_n + c0, r);
-          }
-          tmem_st_wait();
-          gemm2_epi_bar();  // every warp has read the slot
-          if (warp == 2 && lane == 0) p.sk_sem[src_cta] = 0;  // re-armed for the next launch
-          first_piece = false;
-        }
-      }
-      tc_fence_before();
-      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc_n]), 0));
-    };
-    SegIter seg(pair, num_pairs, num_tiles, num_kb, p.streamk);
-    SegIter ahead(pair, num_pairs, num_tiles, num_kb, p.streamk);  // runs two segments ahead of `seg`
-    int tile, kb0, kb1;
-    int tile_n, kb0_n, kb1_n;
-    for (int i = 0; i < 2; ++i) {  // the first use of both buffers
-      const bool have_n = ahead.next(tile_n, kb0_n, kb1_n);
-      hand_over(have_n, tile_n, kb0_n, kb1_n, i);
-    }
-    for (; seg.next(tile, kb0, kb1); ++it) {
+    for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {
       const int mp = tile % num_mp;
       const int n_blk = tile / num_mp;
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
       const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * BN;
-      const bool have_n = ahead.next(tile_n, kb0_n, kb1_n);  // the segment that reuses this buffer
-      if (kb0 != 0) {
-        // ---- stream-K: a later piece of a tile owned by an earlier pair -> publish the fp32 partial
-        mbar_wait(&tfull[acc], acc_phase);
-        tc_fence_after();
-        float4* dst = reinterpret_cast<float4*>(p.sk_scratch) + (size_t)blockIdx.x * SLOT_F4;
-#pragma unroll 1
-        for (int c0 = part * COLS; c0 < (part + 1) * COLS; c0 += 32) {
-          uint32_t r[32];
-          tmem_ld32(t_row + c0, r);
-          tmem_ld_wait();
-#pragma unroll
-          for (int j = 0; j < 8; ++j)
-            __stcg(dst + (size_t)(c0 / 4 + j) * GEMM_BM + row_in_tile,
-                   make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]), __uint_as_float(r[4 * j + 2]),
-                               __uint_as_float(r[4 * j + 3])));
-        }
-        gemm2_epi_bar();  // orders every warp's stores before the elected thread's gpu-scope release
-        if (warp == 2 && lane == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.sk_sem + blockIdx.x), "r"(1) : "memory");
-        hand_over(have_n, tile_n, kb0_n, kb1_n, acc);
-        continue;
-      }
       // operands that do not depend on the accumulator are fetched while the main loop still runs
       float rstd = 0.f;
       ResidPrefetch pf;
-      if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row_base + lane, row_base + lane < p.M);
-      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, pf, row_base, lane, n_blk, part * (BN / NPARTS));
+      if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row_base + lane, row_base + lane < M);
+      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, M, pf, row_base, lane, n_blk, part * (BN / NPARTS));
       mbar_wait(&tfull[acc], acc_phase);
       if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 14 + it);
       tc_fence_after();
       float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
-      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk, part, NPARTS);
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
-      hand_over(have_n, tile_n, kb0_n, kb1_n, acc);
+      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < M, n_blk, part, NPARTS);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
+      tc_fence_before();
+      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
       if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 25 + it);
     }
   }

@@ -78,8 +78,8 @@ struct SliceAux {
   uint2 gn[NV];  // next norm's gain (EPI_RESID) / this head's QK-norm gain (EPI_QKV)
 };
 template <int BN, int EPI, int DH, int RB>
-__device__ __forceinline__ void slice_aux_load(const GemmParams& p, SliceAux<BN / 128, RB>& ax, int r0, int dr, int lane,
-                                               int m_blk, int n_blk) {
+__device__ __forceinline__ void slice_aux_load(const GemmParams& p, int M, SliceAux<BN / 128, RB>& ax, int r0, int dr,
+                                               int lane, int m_blk, int n_blk) {
   constexpr int NV = BN / 128;
   constexpr int HD2 = DH / 2;
   [[maybe_unused]] const int ch = (4 * lane) % DH;                      // lane's first column inside its head
@@ -96,7 +96,7 @@ __device__ __forceinline__ void slice_aux_load(const GemmParams& p, SliceAux<BN 
   for (int b = 0; b < RB; ++b) {
     const int r = r0 + b * dr;
     const int row = m_blk * GEMM_BM + r;
-    const bool ok = r < GEMM_BM && row < p.M;
+    const bool ok = r < GEMM_BM && row < M;
     if constexpr (EPI == EPI_RESID) {
 #pragma unroll
       for (int v = 0; v < NV; ++v)
@@ -136,8 +136,9 @@ __device__ __forceinline__ void slice_aux_load(const GemmParams& p, SliceAux<BN 
 // One batch of RB rows (r0, r0 + dr, ...): the S partials of every row of the batch are requested before
 // the first use, so a batch costs about one L2 round trip.  S * NV <= CAP float4 per row are in flight.
 template <int BN, int EPI, int DH, int RB, int CAP>
-__device__ __forceinline__ void slice_batch(const GemmParams& p, const float* scratch, int S, int r0, int dr, int lane,
-                                            int m_blk, int n_blk, const SliceAux<BN / 128, RB>& ax) {
+__device__ __forceinline__ void slice_batch(const GemmParams& p, int M, const float* scratch, int S, int r0, int dr,
+                                            int lane, int m_blk, int n_blk, const SliceAux<BN / 128, RB>& ax) {
+  float* const x_dst = (EPI == EPI_RESID) ? resid_dst(p) : nullptr;
   constexpr int NV = BN / 128;
   constexpr int HD2 = DH / 2;
   constexpr int HL = DH / 4;  // lanes per head
@@ -150,7 +151,7 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
   for (int b = 0; b < RB; ++b) {
     const int r = r0 + b * dr;
     row[b] = m_blk * GEMM_BM + r;
-    ok[b] = r < GEMM_BM && row[b] < p.M;
+    ok[b] = r < GEMM_BM && row[b] < M;
 #pragma unroll
     for (int q = 0; q < CAP; ++q)
       if (ok[b] && q < snv)
@@ -184,7 +185,7 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
         const int col = n_blk * BN + v * 128 + 4 * lane;
         float4 x = ax.xv[b][v];
         x.x += acc[v].x; x.y += acc[v].y; x.z += acc[v].z; x.w += acc[v].w;
-        *reinterpret_cast<float4*>(p.x + (size_t)row[b] * p.ld_x + col) = x;
+        *reinterpret_cast<float4*>(x_dst + (size_t)row[b] * p.ld_x + col) = x;
         ss = fmaf(x.x, x.x, ss); ss = fmaf(x.y, x.y, ss); ss = fmaf(x.z, x.z, ss); ss = fmaf(x.w, x.w, ss);
         if (p.g_next != nullptr) {
           const uint2 g = ax.gn[v];
@@ -263,8 +264,9 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, const float* sc
 //   (2) meet the group at the tile's arrival counter
 //   (3) batches: sum the S partials of each row in the fixed order 0..S-1, fused epilogue
 template <int BN, int EPI, int DH, int RB, int CAP>
-__device__ __forceinline__ void group_finish(const GemmParams& p, uint64_t* tfull, uint32_t t_row, float* stg, float* scratch,
-                                             int S, int s, int tile, int warp, int lane, int m_blk, int n_blk) {
+__device__ __forceinline__ void group_finish(const GemmParams& p, int M, uint64_t* tfull, uint32_t t_row, float* stg,
+                                             float* scratch, int S, int s, int tile, int warp, int lane, int m_blk,
+                                             int n_blk) {
   constexpr int NV = BN / 128;
   constexpr int NPARTS = GEMMK_EPI_WARPS / 4;
   constexpr int COLS = BN / NPARTS;
@@ -274,7 +276,7 @@ __device__ __forceinline__ void group_finish(const GemmParams& p, uint64_t* tful
   const int r_first = s + ew * S;
   const bool tr = warp == 2 && lane == 0;
   SliceAux<NV, RB> ax;
-  slice_aux_load<BN, EPI, DH, RB>(p, ax, r_first, dr, lane, m_blk, n_blk);
+  slice_aux_load<BN, EPI, DH, RB>(p, M, ax, r_first, dr, lane, m_blk, n_blk);
   mbar_wait(tfull, 0);
   tc_fence_after();
   if (tr) trace_stamp(p, 5);
@@ -308,11 +310,11 @@ __device__ __forceinline__ void group_finish(const GemmParams& p, uint64_t* tful
   }
   epi_bar_sync();
   if (tr) trace_stamp(p, 7);
-  slice_batch<BN, EPI, DH, RB, CAP>(p, scratch, S, r_first, dr, lane, m_blk, n_blk, ax);
+  slice_batch<BN, EPI, DH, RB, CAP>(p, M, scratch, S, r_first, dr, lane, m_blk, n_blk, ax);
 #pragma unroll 1
   for (int r0 = r_first + RB * dr; r0 < GEMM_BM; r0 += RB * dr) {
-    slice_aux_load<BN, EPI, DH, RB>(p, ax, r0, dr, lane, m_blk, n_blk);
-    slice_batch<BN, EPI, DH, RB, CAP>(p, scratch, S, r0, dr, lane, m_blk, n_blk, ax);
+    slice_aux_load<BN, EPI, DH, RB>(p, M, ax, r0, dr, lane, m_blk, n_blk);
+    slice_batch<BN, EPI, DH, RB, CAP>(p, M, scratch, S, r0, dr, lane, m_blk, n_blk, ax);
   }
   if (tr) trace_stamp(p, 9);
 }
@@ -362,6 +364,7 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   pdl_launch_dependents();
   if (threadIdx.x == 0) trace_stamp(p, 1);
 
+  const int M = gemm_rows(p);
   const int S = p.splits;
   const int tile = blockIdx.x / S;
   const int s = blockIdx.x - tile * S;
@@ -441,15 +444,15 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // ---- one CTA per tile: fused epilogue straight from tensor memory
       float rstd = 0.f;
       ResidPrefetch pf;
-      if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row_base + lane, row_base + lane < p.M);
-      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, pf, row_base, lane, n_blk, part * COLS);
+      if constexpr (EPI == EPI_QKV || EPI == EPI_SWIGLU) rstd = row_rstd(p, row_base + lane, row_base + lane < M);
+      if constexpr (EPI == EPI_RESID) resid_issue<BN>(p, M, pf, row_base, lane, n_blk, part * COLS);
       mbar_wait(tfull, 0);
       tc_fence_after();
       if (tr) trace_stamp(p, 5);
-      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < p.M, n_blk, part, NPARTS);
-      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
-      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
+      if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < M, n_blk, part, NPARTS);
+      if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
+      if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
+      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
       if (tr) trace_stamp(p, 9);
     } else {
       // ---- split-K group (see group_finish).  The batch shape is chosen so that all partials of a batch
@@ -459,7 +462,7 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       float* scratch = p.sk_scratch + (size_t)tile * S * GEMM_BM * BN;
       const int snv = S * NV;
 #define TE_GROUP_FINISH(RB, CAP) \
-  group_finish<BN, EPI, DH, RB, CAP>(p, tfull, t_row, stg, scratch, S, s, tile, warp, lane, m_blk, n_blk)
+  group_finish<BN, EPI, DH, RB, CAP>(p, M, tfull, t_row, stg, scratch, S, s, tile, warp, lane, m_blk, n_blk)
       if (EPI != EPI_QKV && snv <= 2) { TE_GROUP_FINISH(8, 2); }
       else if (EPI != EPI_QKV && snv <= 3) { TE_GROUP_FINISH(6, 3); }
       else if (snv <= 4) { TE_GROUP_FINISH(4, 4); }

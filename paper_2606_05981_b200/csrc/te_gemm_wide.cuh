@@ -11,9 +11,11 @@
 // Same warp roles, PDL prologue and residual epilogue arithmetic as te_gemm2_kernel (te_gemm.cuh).
 //
 // EPI_SWIGLU variant (mid batches, e.g. T = 512: 96 pair tiles of 256 x 256 = 1.3 waves): the two MMAs of a tile
-// take the gate rows and the matching up rows of the NON-interleaved [Wgate; Wup] matrix, so that a tile of w
-// output columns (bn = 2w accumulator columns: [0,w) gate, [w,2w) up) can have any width that is a multiple of 32:
-// 32 x 192 output columns x 2 row-pair blocks = 64 tiles, one wave.
+// take the gate rows and the matching up rows, so that a tile of w output columns (bn = 2w accumulator columns:
+// [0,w) gate, [w,2w) up) can have any width that is a multiple of 64: 32 x 192 output columns x 2 row-pair blocks
+// = 64 tiles, one wave.  The weights are the library's one copy of [Wgate; Wup], interleaved per 256 rows (128 gate
+// rows | the 128 matching up rows): 32 consecutive output columns are 32 consecutive rows there, so the B operand is
+// fetched as 32-row TMA boxes (gate column c -> row (c / 128) * 256 + c % 128, up column c -> that + 128).
 #pragma once
 #include "te_gemm.cuh"
 
@@ -38,9 +40,9 @@ struct GemmWideCfg {
   }
 };
 
-// bn: accumulator width, a multiple of 32 (64 for EPI_SWIGLU), <= 512; nh = bn/2 columns per MMA (multiple of 16, <= 256).
-// tmB: weight matrix in boxes of nh/2 rows x 64 columns: [N, K] for EPI_RESID; [2F, K] = [Wgate; Wup] for EPI_SWIGLU
-// (p.N = 2F; the tile's output columns are n_blk*nh .. +nh of F).
+// bn: accumulator width, a multiple of 32 (128 for EPI_SWIGLU), <= 512; nh = bn/2 columns per MMA (multiple of 16, <= 256).
+// tmB: EPI_RESID: weight matrix [N, K] in boxes of nh/2 rows x 64 columns; EPI_SWIGLU: the interleaved [2F, K] gate/up
+// matrix in boxes of 32 rows x 64 columns (p.N = 2F; the tile's output columns are n_blk*nh .. +nh of F).
 template <int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM2_THREADS, 1)
 te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const GemmParams p,
@@ -89,8 +91,9 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
   const uint32_t tmem_base = *tmem_slot;
   pdl_launch_dependents();
 
+  const int M = gemm_rows(p);
   const int num_kb = p.K / GEMM_BK;
-  const int num_mp = (p.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);
+  const int num_mp = (p.num_m_blk + 1) >> 1;  // 256-row blocks
   const int tile = blockIdx.x >> 1;  // one tile per CTA pair
   const int mp = tile % num_mp;
   const int n_blk = tile / num_mp;
@@ -105,11 +108,21 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
       const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
       // this CTA's weight rows for MMA j: [col_base + j*nh + rank*nh/2, + nh/2)
       const int b_row0 = w_row0 + rank * (nh / 2);
-      const int b_row1 = w_row1 + rank * (nh / 2);
+      [[maybe_unused]] const int b_row1 = w_row1 + rank * (nh / 2);
       auto load_b = [&](int stage, int kb) {
         const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
-        tma_load_2d_cg2(sB + stage * b_bytes, &tmB, bar, kb * GEMM_BK, b_row0);
-        tma_load_2d_cg2(sB + stage * b_bytes + sub_bytes, &tmB, bar, kb * GEMM_BK, b_row1);
+        if constexpr (EPI == EPI_SWIGLU) {
+          // this CTA's nh/2 gate columns and nh/2 up columns, 32 at a time, from the 256-row interleaved layout
+          for (int j = 0; j < nh / 2; j += 32) {
+            const int c = b_row0 + j;  // output column of F
+            const int g_row = (c >> 7) * 256 + (c & 127);
+            tma_load_2d_cg2(sB + stage * b_bytes + j * 128, &tmB, bar, kb * GEMM_BK, g_row);
+            tma_load_2d_cg2(sB + stage * b_bytes + sub_bytes + j * 128, &tmB, bar, kb * GEMM_BK, g_row + 128);
+          }
+        } else {
+          tma_load_2d_cg2(sB + stage * b_bytes, &tmB, bar, kb * GEMM_BK, b_row0);
+          tma_load_2d_cg2(sB + stage * b_bytes + sub_bytes, &tmB, bar, kb * GEMM_BK, b_row1);
+        }
       };
       const int pre = num_kb < STAGES ? num_kb : STAGES;
       for (int kb = 0; kb < pre; ++kb) {  // weights first: independent of the predecessor kernel
@@ -171,7 +184,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
     pdl_wait();
     if constexpr (EPI == EPI_SWIGLU) {
       // ---- y = rstd * acc; act = silu(gate) * up, bf16 (arithmetic of epi_swiglu, te_gemm.cuh)
-      const float rstd = row_rstd(p, row_base + lane, row_base + lane < p.M);
+      const float rstd = row_rstd(p, row_base + lane, row_base + lane < M);
       mbar_wait(tfull, 0);
       tc_fence_after();
 #pragma unroll 1
@@ -191,17 +204,36 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         }
         stg_put_row(stg, lane, a);
         __syncwarp();
-        stg_store_bf16(stg, lane, row_base, p.M, p.act, p.ld_act, col_base + c0);
+        stg_store_bf16(stg, lane, row_base, M, p.act, p.ld_act, col_base + c0);
         __syncwarp();
+      }
+    } else if constexpr (EPI == EPI_PLAIN) {
+      // ---- fp32 store of the valid columns (te_debug_gemm_wide: the main loop alone against a matmul)
+      mbar_wait(tfull, 0);
+      tc_fence_after();
+      const int row = row_base + lane;
+#pragma unroll 1
+      for (int c0 = c_begin; c0 < c_end; c0 += 32) {
+        uint32_t r[32];
+        tmem_ld32(t_row + c0, r);
+        tmem_ld_wait();
+        if (row < M) {
+          float4* dst = reinterpret_cast<float4*>(p.c + (size_t)row * p.ld_c + col_base + c0);
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            dst[j] = make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]), __uint_as_float(r[4 * j + 2]),
+                                 __uint_as_float(r[4 * j + 3]));
+        }
       }
     } else {
     const bool has_g = p.g_next != nullptr;
+    float* const x_dst = resid_dst(p);
     auto issue_x = [&](float4 (&xv)[8], int c0) {
       const int col = col_base + c0 + cq * 4;
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         const int row = row_base + sub + 4 * i;
-        if (row < p.M) xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
+        if (row < M) xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
       }
     };
     float4 xn[8];
@@ -237,11 +269,11 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
       for (int i = 0; i < 8; ++i) {
         const int rr = sub + 4 * i;
         const int row = row_base + rr;
-        if (row < p.M) {
+        if (row < M) {
           const float4 a = stg_get(stg, rr, cq);
           float4 v = xv[i];
           v.x += a.x; v.y += a.y; v.z += a.z; v.w += a.w;
-          *reinterpret_cast<float4*>(p.x + (size_t)row * p.ld_x + col) = v;
+          *reinterpret_cast<float4*>(x_dst + (size_t)row * p.ld_x + col) = v;
           ss[i] = fmaf(v.x, v.x, ss[i]); ss[i] = fmaf(v.y, v.y, ss[i]);
           ss[i] = fmaf(v.z, v.z, ss[i]); ss[i] = fmaf(v.w, v.w, ss[i]);
           if (has_g) {
@@ -266,7 +298,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         const int row = row_base + sub + 4 * i;
-        if (row < p.M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * 2 + part)] = ss[i];
+        if (row < M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * 2 + part)] = ss[i];
       }
     }
     }  // EPI_RESID

@@ -8,14 +8,22 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "te_gemm.cuh"  // DynParams
+
 namespace te {
 
+// Refreshes the per-call values ahead of the stack (one thread; values arrive as kernel parameters, so the call
+// needs no host staging memory and can be captured into a caller's graph as well).
+__global__ void te_set_dyn_kernel(DynParams* dyn, const DynParams v) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) *dyn = v;
+}
+
 enum { FLAG_BAD_LEN = 1, FLAG_BAD_TOTAL = 2, FLAG_TOO_LONG = 4 };
+constexpr int PREP_PAD_ROWS = 16;  // rows past the call's tokens that te_prep_kernel zeroes in the qkv workspace
 
 struct PrepParams {
-  const float* embeds;       // [T, d]
-  const int32_t* text_lens;  // [B]
-  float* out;                // [T, d]  fp32 residual stream
+  const DynParams* dyn;      // embeds [T, d], text_lens [B], total_tokens of this call
+  float* out;                // [T, d]  fp32 residual stream (library workspace)
   int32_t* cu;               // [B+1]   packing offsets (written by block 0)
   int32_t* flag;             // sticky validation flag
   int32_t* pos;              // [3, T]
@@ -26,9 +34,16 @@ struct PrepParams {
   __nv_bfloat16* xg;            // [T, d]  bf16(x * g_first)
   float* ssq;                   // [T][ssq_stride], first ssq_parts entries of a row used
   int ssq_parts, ssq_stride;
-  int n_frames, total_tokens, d, half_dim, max_tokens_per_frame;
+  int n_frames, d, half_dim, max_tokens_per_frame;
   int grid_h, grid_w;
   int pos_offset;   // length P of the shared text prefix in front of every frame (ids continue from it)
+  // The attention kernel multiplies keys / values in granules of 16 rows: a frame whose length is not a multiple of
+  // 16 reads up to 15 rows past its end with zero weight.  Those rows are the next frame's or, for the last frame of
+  // a call, rows [T, T + 16) of the qkv workspace, which no kernel of THIS call writes (the activation tensor maps span
+  // the whole workspace; they are encoded once, not per token count).  Blocks T .. T+15 of this kernel zero them, so
+  // that 0 * (what an earlier, larger call left there) can never be 0 * NaN.
+  uint4* qkv_rows;  // [rows, qkv_row_vec16] the qkv workspace as 16-byte vectors
+  int qkv_row_vec16;
   int8_t axis[64];  // M-RoPE axis (0 = t, 1 = h, 2 = w) of frequency pair i (contiguous or interleaved sections)
 };
 
@@ -44,6 +59,8 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   const int n_vis = p.grid_h * p.grid_w;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous call's kernels still read cu / flag / out
+  const int total_tokens = p.dyn->total_tokens;
+  const int32_t* const text_lens = p.dyn->text_lens;
   if (warp == 0) {
     long long carry = 0;
     int best_b = 0, best_start = 0, f = 0;
@@ -51,7 +68,7 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
       const int b = base + lane;
       int sb = 0;
       if (b < p.n_frames) {
-        int tl = p.text_lens[b];
+        int tl = text_lens[b];
         if (tl < 0) { f |= FLAG_BAD_LEN; tl = 0; }
         sb = n_vis + tl;
         if (sb > p.max_tokens_per_frame) f |= FLAG_TOO_LONG;
@@ -65,16 +82,16 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
       incl += carry;
       if (b < p.n_frames) {
         const long long excl = incl - sb;
-        const int start = static_cast<int>(excl < p.total_tokens ? excl : p.total_tokens);
+        const int start = static_cast<int>(excl < total_tokens ? excl : total_tokens);
         if (start <= tok) { best_b = b; best_start = start; }  // starts are non-decreasing in b
         if (tok == 0) {
           if (b == 0) p.cu[0] = 0;
-          p.cu[b + 1] = static_cast<int32_t>(incl < p.total_tokens ? incl : p.total_tokens);
+          p.cu[b + 1] = static_cast<int32_t>(incl < total_tokens ? incl : total_tokens);
         }
       }
       carry = __shfl_sync(0xffffffffu, incl, 31);
     }
-    if (carry != p.total_tokens) f |= FLAG_BAD_TOTAL;
+    if (carry != total_tokens) f |= FLAG_BAD_TOTAL;
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
       const int ob = __shfl_xor_sync(0xffffffffu, best_b, off);
@@ -88,7 +105,11 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
     }
   }
   __syncthreads();
-  if (tok >= p.total_tokens) return;
+  if (tok >= total_tokens) {
+    if (tok < total_tokens + PREP_PAD_ROWS)
+      for (int i = threadIdx.x; i < p.qkv_row_vec16; i += 256) p.qkv_rows[(size_t)tok * p.qkv_row_vec16 + i] = make_uint4(0u, 0u, 0u, 0u);
+    return;
+  }
   const int n = tok - s_start;
   int pt, ph, pw;
   const int off = p.pos_offset;
@@ -99,8 +120,8 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   }
   if (threadIdx.x == 0) {
     p.pos[tok] = pt;
-    p.pos[p.total_tokens + tok] = ph;
-    p.pos[2 * p.total_tokens + tok] = pw;
+    p.pos[total_tokens + tok] = ph;
+    p.pos[2 * total_tokens + tok] = pw;
   }
   // the rotary table on the last warps, so that it overlaps the row copy of the first ones
   for (int i = 255 - threadIdx.x; i < p.half_dim; i += 256) {
@@ -112,7 +133,7 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
     p.sin_t[(size_t)tok * p.half_dim + i] = static_cast<float>(sn);
   }
   // residual copy + sum of squares + bf16(x * g)
-  const float4* src = reinterpret_cast<const float4*>(p.embeds + (size_t)tok * p.d);
+  const float4* src = reinterpret_cast<const float4*>(p.dyn->embeds + (size_t)tok * p.d);
   float4* dst = reinterpret_cast<float4*>(p.out + (size_t)tok * p.d);
   float ss = 0.f;
   for (int c4 = threadIdx.x; c4 < p.d / 4; c4 += 256) {
@@ -140,15 +161,16 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   }
 }
 
-// a6: out <- RMSNorm(out; gf), fp32, one warp per row.
-__global__ void __launch_bounds__(256) te_final_norm_kernel(float* __restrict__ x, const __nv_bfloat16* __restrict__ gf,
-                                                            int total_tokens, int d, float eps) {
+// a6: out <- RMSNorm(x; gf), fp32, one warp per row (x: the library's residual stream, out: the caller's buffer).
+__global__ void __launch_bounds__(256) te_final_norm_kernel(const float* __restrict__ x, const DynParams* __restrict__ dyn,
+                                                            const __nv_bfloat16* __restrict__ gf, int d, float eps) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tok = blockIdx.x * 8 + warp;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  if (tok >= total_tokens) return;
-  float4* row = reinterpret_cast<float4*>(x + (size_t)tok * d);
+  if (tok >= dyn->total_tokens) return;
+  const float4* row = reinterpret_cast<const float4*>(x + (size_t)tok * d);
+  float4* dst = reinterpret_cast<float4*>(dyn->out + (size_t)tok * d);
   float ss = 0.f;
   for (int c4 = lane; c4 < d / 4; c4 += 32) {
     const float4 v = row[c4];
@@ -164,7 +186,7 @@ __global__ void __launch_bounds__(256) te_final_norm_kernel(float* __restrict__ 
     v.y = v.y * rstd * __uint_as_float(g.x & 0xFFFF0000u);
     v.z = v.z * rstd * __uint_as_float(g.y << 16);
     v.w = v.w * rstd * __uint_as_float(g.y & 0xFFFF0000u);
-    row[c4] = v;
+    dst[c4] = v;
   }
 }
 

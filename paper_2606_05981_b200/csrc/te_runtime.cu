@@ -1,5 +1,5 @@
-// te_runtime.cu — host runtime + C ABI (include/te.h): handle, weight repack, workspace,
-// tensor maps, kernel sequencing and the CUDA-graph cache.  One graph launch per te_encode.
+// te_runtime.cu — host runtime + C ABI (include/te.h, include/te_debug.h): handle, weight repack, workspace,
+// tensor maps, kernel dispatch (Plan), kernel sequencing and the CUDA-graph cache.  One graph launch per te_encode.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "../../include/te.h"
+#include "../../include/te_debug.h"
 #include "te_attn.cuh"
 #include "te_attn_tc.cuh"
 #include "te_gemm.cuh"
@@ -56,9 +57,10 @@ struct LayerOff {
   size_t g1, wqkv, gq, gk, wo, g2, wgu, wd;  // element offsets into the device weight buffer
 };
 
+// A cached graph is valid for every call of the same SHAPE CLASS: per-call pointers and the exact token count
+// travel through the device-side DynParams block, so the key holds only what decides grids and dispatch.
 struct GraphKey {
-  int n_frames, grid_h, grid_w, total_tokens, lb, le, stop, prefix_len;
-  const void *embeds, *lens, *out;
+  int n_frames, grid_h, grid_w, bucket_tokens, lb, le, stop, prefix_len;
   bool operator==(const GraphKey& o) const { return memcmp(this, &o, sizeof(GraphKey)) == 0; }
 };
 struct GraphEntry {
@@ -67,6 +69,27 @@ struct GraphEntry {
   cudaGraph_t graph;
   int n_kernels;
   uint64_t stamp;
+};
+
+// Launch attributes of one kernel launch (per call, never process-wide: two handles on two host threads
+// must not see each other's choices).
+struct LaunchCtx {
+  bool pdl = false;                // programmatic stream serialisation (the kernels order themselves with griddepcontrol)
+  bool coop = false;               // cooperative grid: all CTAs resident at once (split-K groups spin on each other)
+  cudaAccessPolicyWindow l2{};     // TE_OPT_L2_RESIDUAL: the fp32 residual stays resident in L2 (num_bytes = 0: none)
+};
+
+// Kernel choice for one shape class (every decision that depends on the token count is taken from the bucket's
+// upper bound, so that all calls of a bucket share one graph).
+struct Plan {
+  int Tb = 0;          // token-count bucket (rows the grids are sized for)
+  int num_m = 0;       // 128-row blocks
+  int pair = 0;        // CTA pairs for all GEMMs
+  int bn_qkv = 256, k_qkv = 0, pair_qkv = 0, bx_qkv = 0;
+  int bn_gu = 256, k_gu = 0, pair_gu = 0, bx_gu = 0, gu_half = 0, gu_wide_tiles = 0, gu_wide_w = 0;
+  int bn_res = 128, k_res = 0, bx_res = 0, n_blk_res = 0, wide_tiles = 0, wide_bn = 0;
+  int parts = 1;       // RMSNorm partial sums per row written by the residual GEMMs
+  int attn_tc = 0, attn_split = 1, q_blocks = 1, g_shift = 0, s_bound = 0;
 };
 
 }  // namespace
@@ -78,33 +101,41 @@ struct te_handle {
   bool loaded = false;
   // tile choices
   int bn_qkv = 256, bn_gu = 256, bn_res = 128;
-  bool bn_res_auto = true;  // CTA-pair residual tile width chosen per token count until TE_OPT_RESID_BLOCK_N is set
   int attn_impl = 1;  // 1: tcgen05 kernel (te_attn_tc.cuh) when Hq/Hkv is a power of two <= 8; 0: mma.sync kernel
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   int resid_wide = 1; // residual GEMMs on CTA pairs: 1 = auto (one wave of wide tiles when 128-wide tiles need >= 2
                       // waves), 0 = never, n >= 2 = always with n tiles across N (tests)
   int l2_resid = 1;          // 1: the residual stream is an L2-persisting access window of every kernel
   size_t l2_limit_bytes = 0; // persisting-L2 carve-out requested for it (0 until the first te_encode sets the limit)
+  size_t l2_prev_limit = 0;  // the device limit found before it was raised (restored by te_destroy / option 0)
+  bool l2_limit_raised = false;
   size_t l2_max_persist = 0; // device property persistingL2CacheMaxSize
-  int streamk = 0;    // 1: CTA-pair GEMMs balance (tile, k-block) units over all SM pairs (stream-K; measured slower)
   int splitk = 1;     // 1: small batches (no CTA pairs) use the split-K kernel when a GEMM has <= one tile per SM
+  int split_target = 0;  // experiments: target CTA count of a split-K launch (0 = one per SM)
   float* sk_scratch = nullptr;  // [sm_count][128 x 256] fp32 partial tiles
   int* sk_sem = nullptr;        // [sm_count][2] per-tile arrival / departure counters (zero between launches)
   // weights
   bf16* w = nullptr;
   size_t w_elems = 0;
-  bf16* w_gu_plain = nullptr;  // [L][2F, d] = [Wgate; Wup] as in the blob (not interleaved): wide SwiGLU tiles
   std::vector<LayerOff> off;
   size_t gf_off = 0;
-  // weight tensor maps per layer, one per B box height {64, 128, 256} rows (index 0, 1, 2)
-  struct LayerMaps { CUtensorMap qkv[3], o[3], gu[3], d[3]; };
+  // weight tensor maps per layer, one per B box height {32, 64, 128, 256} rows (index 0..3)
+  struct LayerMaps { CUtensorMap qkv[4], o[4], gu[4], d[4]; };
   std::vector<LayerMaps> tm;
-  // workspace
+  // workspace (rows: cap_rows = max_tokens rounded up to 256)
+  int cap_rows = 0;
+  te::DynParams* dyn = nullptr;  // per-call pointers + token count, refreshed on the stream ahead of every stack
+  float* resid = nullptr;        // [cap_rows, d] fp32 residual stream
   int32_t *cu = nullptr, *pos = nullptr, *flag = nullptr;
   float *cos_t = nullptr, *sin_t = nullptr, *ssq = nullptr;
   double* inv_freq = nullptr;
   bf16 *xg = nullptr, *qkv = nullptr, *attn = nullptr, *act = nullptr;
   int ssq_parts_cap = 0;
+  // activation tensor maps over the whole workspace buffers, encoded once (rows past the call's tokens are never
+  // stored; see qkv_zero_rows for the one place where they are multiplied)
+  CUtensorMap tmA_xg, tmA_attn, tmA_act, tmQ, tmKV;
+  bool attn_tc_ok = false;
+  int g_shift = 0;
   unsigned long long* trace = nullptr;  // [4 GEMM classes][sm_count][TRACE_SLOTS] (debug, TE_OPT_TRACE)
   int trace_on = 0;
   // M-RoPE axis of every frequency pair (contiguous or interleaved sections)
@@ -113,7 +144,7 @@ struct te_handle {
   bf16* kv_prefix = nullptr;
   std::vector<CUtensorMap> tm_prefix;  // per layer: the prefix cache [P, 2*Hkv*dh] in 64-row boxes (tcgen05 attention)
   float2* attn_stats = nullptr;        // [max_tokens, Hq] (row max, row sum) of the frame-local attention pass
-  float* prefix_buf = nullptr;    // [max_prefix, d] residual of the prefix pass when the caller wants no output
+  float* prefix_buf = nullptr;    // [max_prefix, d] hidden states of the prefix pass when the caller wants no output
   int32_t* prefix_lens = nullptr; // device [1]
   int prefix_len = 0;
   // host-path staging
@@ -128,6 +159,7 @@ struct te_handle {
   // graphs
   std::vector<GraphEntry> cache;
   uint64_t stamp = 0;
+  long long captures = 0;
   int use_graph = 1;
   int pdl = 1;
   int timing = 0;
@@ -135,8 +167,10 @@ struct te_handle {
   std::vector<TimedLaunch> timed;
   int dbg_lb = 0, dbg_le = 0, dbg_stop = 0;
   int last_T = 0, last_B = 0;
+  Plan last_plan;
   long long launches = 0;
   std::string err;
+  std::string info;
 };
 
 namespace {
@@ -178,11 +212,9 @@ int validate_config(const te_config& c) {
 
 // Launch with (optional) programmatic stream serialisation: the kernel may begin while its
 // predecessor in the stream drains; the kernels order themselves with griddepcontrol.wait.
-bool g_pdl = true;
-bool g_coop = false;
-cudaAccessPolicyWindow g_l2_window{};
 template <typename... KArgs, typename... Args>
-cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+cudaError_t launch_k(const LaunchCtx& lc, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                     Args&&... args) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid;
   cfg.blockDim = block;
@@ -190,19 +222,19 @@ cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
   cfg.stream = st;
   cudaLaunchAttribute at[3];
   int n = 0;
-  if (g_coop) {  // all CTAs of the grid resident at once, or the launch waits: the split-K groups spin on each other
+  if (lc.coop) {
     at[n].id = cudaLaunchAttributeCooperative;
     at[n].val.cooperative = 1;
     ++n;
   }
-  if (g_pdl) {
+  if (lc.pdl) {
     at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[n].val.programmaticStreamSerializationAllowed = 1;
     ++n;
   }
-  if (g_l2_window.num_bytes) {  // TE_OPT_L2_RESIDUAL: the fp32 residual stays resident in L2
+  if (lc.l2.num_bytes) {
     at[n].id = cudaLaunchAttributeAccessPolicyWindow;
-    at[n].val.accessPolicyWindow = g_l2_window;
+    at[n].val.accessPolicyWindow = lc.l2;
     ++n;
   }
   cfg.attrs = at;
@@ -210,86 +242,77 @@ cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
-inline int box_index(int rows) { return rows == 64 ? 0 : (rows == 128 ? 1 : 2); }
+inline int box_index(int rows) { return rows == 32 ? 0 : (rows == 64 ? 1 : (rows == 128 ? 2 : 3)); }
 
 template <int BN, int EPI, int DH>
-cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, int sm_count,
-                        cudaStream_t st) {
+cudaError_t launch_gemm(const LaunchCtx& lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
+                        int sm_count, cudaStream_t st) {
   using Cfg = te::GemmCfg<BN>;
   const int tiles = p.num_m_blk * p.num_n_blk;
   const int grid = tiles < sm_count ? tiles : sm_count;
-  return launch_k(te::te_gemm_kernel<BN, EPI, DH>, dim3(grid), dim3(te::GEMM_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB, p);
+  return launch_k(lc, te::te_gemm_kernel<BN, EPI, DH>, dim3(grid), dim3(te::GEMM_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB, p);
 }
 
 template <int BN, int EPI, int DH>
-cudaError_t launch_gemm2(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, int sm_count,
-                         cudaStream_t st) {
+cudaError_t launch_gemm2(const LaunchCtx& lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
+                         int sm_count, cudaStream_t st) {
   using Cfg = te::Gemm2Cfg<BN, EPI>;
-  const int tiles = ((p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM)) * p.num_n_blk;
-  // stream-K: every SM pair takes an equal share of the (tile, k-block) units, so all pairs are used as soon as
-  // there are that many units; classic: one pair per tile at most
-  const long long units = (long long)tiles * (p.K / te::GEMM_BK);
-  const int cap = p.streamk ? (int)(units < sm_count / 2 ? units : sm_count / 2) : tiles;
-  const int pairs = cap < sm_count / 2 ? cap : sm_count / 2;
-  return launch_k(te::te_gemm2_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM2_THREADS), Cfg::SMEM_BYTES, st, tmA, tmB,
-                  p);
+  const int tiles = ((p.num_m_blk + 1) / 2) * p.num_n_blk;
+  const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
+  return launch_k(lc, te::te_gemm2_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM2_THREADS), Cfg::SMEM_BYTES, st, tmA,
+                  tmB, p);
 }
 
 // pair = 0: one CTA per 128 x bn tile; pair = 1: one CTA pair per 256 x bn tile (cta_group::2)
 template <int EPI>
-cudaError_t launch_gemm_bn(int bn, int pair, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p,
-                           int sms, cudaStream_t st) {
+cudaError_t launch_gemm_bn(const LaunchCtx& lc, int bn, int pair, int dh, const CUtensorMap& a, const CUtensorMap& b,
+                           const te::GemmParams& p, int sms, cudaStream_t st) {
   if constexpr (EPI == te::EPI_QKV) {
     if (pair) {
-      if (bn == 256 && dh == 128) return launch_gemm2<256, EPI, 128>(a, b, p, sms, st);
-      if (bn == 256 && dh == 64) return launch_gemm2<256, EPI, 64>(a, b, p, sms, st);
-      if (bn == 128 && dh == 128) return launch_gemm2<128, EPI, 128>(a, b, p, sms, st);
-      return launch_gemm2<128, EPI, 64>(a, b, p, sms, st);
+      if (bn == 256 && dh == 128) return launch_gemm2<256, EPI, 128>(lc, a, b, p, sms, st);
+      if (bn == 256 && dh == 64) return launch_gemm2<256, EPI, 64>(lc, a, b, p, sms, st);
+      if (bn == 128 && dh == 128) return launch_gemm2<128, EPI, 128>(lc, a, b, p, sms, st);
+      return launch_gemm2<128, EPI, 64>(lc, a, b, p, sms, st);
     }
-    if (bn == 256 && dh == 128) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
-    if (bn == 256 && dh == 64) return launch_gemm<256, EPI, 64>(a, b, p, sms, st);
-    if (bn == 128 && dh == 128) return launch_gemm<128, EPI, 128>(a, b, p, sms, st);
-    return launch_gemm<128, EPI, 64>(a, b, p, sms, st);
+    if (bn == 256 && dh == 128) return launch_gemm<256, EPI, 128>(lc, a, b, p, sms, st);
+    if (bn == 256 && dh == 64) return launch_gemm<256, EPI, 64>(lc, a, b, p, sms, st);
+    if (bn == 128 && dh == 128) return launch_gemm<128, EPI, 128>(lc, a, b, p, sms, st);
+    return launch_gemm<128, EPI, 64>(lc, a, b, p, sms, st);
   } else {
     if (pair) {
-      if (bn == 256) return launch_gemm2<256, EPI, 128>(a, b, p, sms, st);
-      if constexpr (EPI == te::EPI_RESID) {
-        if (bn == 192) return launch_gemm2<192, EPI, 128>(a, b, p, sms, st);
-      }
-      return launch_gemm2<128, EPI, 128>(a, b, p, sms, st);
+      if (bn == 256) return launch_gemm2<256, EPI, 128>(lc, a, b, p, sms, st);
+      return launch_gemm2<128, EPI, 128>(lc, a, b, p, sms, st);
     }
-    if (bn == 256) return launch_gemm<256, EPI, 128>(a, b, p, sms, st);
-    return launch_gemm<128, EPI, 128>(a, b, p, sms, st);
+    if (bn == 256) return launch_gemm<256, EPI, 128>(lc, a, b, p, sms, st);
+    return launch_gemm<128, EPI, 128>(lc, a, b, p, sms, st);
   }
 }
 
 // split-K kernel: `p.splits` CTAs per 128 x bn tile (small batches; te_gemm_splitk.cuh)
 template <int BN, int EPI, int DH>
-cudaError_t launch_gemmk(const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p, cudaStream_t st) {
+cudaError_t launch_gemmk(LaunchCtx lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
+                         cudaStream_t st) {
   using Cfg = te::GemmKCfg<BN, EPI>;
   const int tiles = p.num_m_blk * p.num_n_blk;
-  g_coop = p.splits > 1;
-  cudaError_t e = launch_k(te::te_gemmk_kernel<BN, EPI, DH>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS),
-                           Cfg::SMEM_BYTES, st, tmA, tmB, p);
-  g_coop = false;
-  return e;
+  lc.coop = p.splits > 1;  // the groups spin on each other: all CTAs resident at once, or the launch waits
+  return launch_k(lc, te::te_gemmk_kernel<BN, EPI, DH>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS), Cfg::SMEM_BYTES, st,
+                  tmA, tmB, p);
 }
 template <int EPI>
-cudaError_t launch_gemmk_bn(int bn, int dh, const CUtensorMap& a, const CUtensorMap& b, const te::GemmParams& p,
-                            cudaStream_t st) {
+cudaError_t launch_gemmk_bn(const LaunchCtx& lc, int bn, int dh, const CUtensorMap& a, const CUtensorMap& b,
+                            const te::GemmParams& p, cudaStream_t st) {
   if constexpr (EPI == te::EPI_QKV) {
     if (bn != 128) return cudaErrorInvalidValue;  // the split-K QKV kernel has one-head-wide (128-column) tiles only
-    if (dh == 128) return launch_gemmk<128, EPI, 128>(a, b, p, st);
-    return launch_gemmk<128, EPI, 64>(a, b, p, st);
+    if (dh == 128) return launch_gemmk<128, EPI, 128>(lc, a, b, p, st);
+    return launch_gemmk<128, EPI, 64>(lc, a, b, p, st);
   } else {
-    if (bn == 256) return launch_gemmk<256, EPI, 128>(a, b, p, st);
-    return launch_gemmk<128, EPI, 128>(a, b, p, st);
+    if (bn == 256) return launch_gemmk<256, EPI, 128>(lc, a, b, p, st);
+    return launch_gemmk<128, EPI, 128>(lc, a, b, p, st);
   }
 }
 // CTAs per tile: fill the SMs, keep >= 2 k-blocks per CTA
-int g_split_target = 0;  // experiments: target CTA count of a split-K launch (0 = one per SM)
-inline int choose_splits(int tiles, int num_kb, int sm_count) {
-  const int target = (g_split_target > 0 && g_split_target < sm_count) ? g_split_target : sm_count;
+inline int choose_splits(int split_target, int tiles, int num_kb, int sm_count) {
+  const int target = (split_target > 0 && split_target < sm_count) ? split_target : sm_count;
   int s = target / tiles;
   if (s > te::GEMMK_MAX_SPLITS) s = te::GEMMK_MAX_SPLITS;
   if (s > num_kb / 2) s = num_kb / 2;
@@ -297,23 +320,25 @@ inline int choose_splits(int tiles, int num_kb, int sm_count) {
 }
 
 template <int DH, int GH>
-cudaError_t launch_attn(const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
+cudaError_t launch_attn(const LaunchCtx& lc, const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
   using Cfg = te::AttnCfg<DH, GH>;
   dim3 grid(q_blocks, p.n_q_heads / GH, n_frames);
-  return launch_k(te::te_attn_kernel<DH, GH>, grid, dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, p);
+  return launch_k(lc, te::te_attn_kernel<DH, GH>, grid, dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, p);
 }
-cudaError_t launch_attn_any(int dh, const te::AttnParams& p, int q_blocks, int n_frames, cudaStream_t st) {
+cudaError_t launch_attn_any(const LaunchCtx& lc, int dh, const te::AttnParams& p, int q_blocks, int n_frames,
+                            cudaStream_t st) {
   const bool two = (p.n_q_heads / p.n_kv_heads) % 2 == 0;  // pairs of q heads share their kv head
-  if (dh == 128) return two ? launch_attn<128, 2>(p, q_blocks, n_frames, st) : launch_attn<128, 1>(p, q_blocks, n_frames, st);
-  return two ? launch_attn<64, 2>(p, q_blocks, n_frames, st) : launch_attn<64, 1>(p, q_blocks, n_frames, st);
+  if (dh == 128)
+    return two ? launch_attn<128, 2>(lc, p, q_blocks, n_frames, st) : launch_attn<128, 1>(lc, p, q_blocks, n_frames, st);
+  return two ? launch_attn<64, 2>(lc, p, q_blocks, n_frames, st) : launch_attn<64, 1>(lc, p, q_blocks, n_frames, st);
 }
 
 template <int DH>
-cudaError_t launch_attn_tc(const CUtensorMap& tmQ, const CUtensorMap& tmKV, const te::AttnTcParams& p, int n_split,
-                           int n_frames, cudaStream_t st) {
+cudaError_t launch_attn_tc(const LaunchCtx& lc, const CUtensorMap& tmQ, const CUtensorMap& tmKV, const te::AttnTcParams& p,
+                           int n_split, int n_frames, cudaStream_t st) {
   using Cfg = te::AttnTcCfg<DH>;
   dim3 grid(n_split, p.n_kv_heads, n_frames);
-  return launch_k(te::te_attn_tc_kernel<DH>, grid, dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, tmQ, tmKV, p);
+  return launch_k(lc, te::te_attn_tc_kernel<DH>, grid, dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, tmQ, tmKV, p);
 }
 
 template <int BN, int EPI, int DH>
@@ -329,8 +354,7 @@ cudaError_t set_gemm_attr() {
   return cudaFuncSetAttribute(te::te_gemm2_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               te::Gemm2Cfg<BN, EPI>::SMEM_BYTES);
 }
-// Opt every kernel instantiation into its dynamic shared-memory size (once per process, outside
-// any stream capture).
+// Opt every kernel instantiation into its dynamic shared-memory size (per device, outside any stream capture).
 cudaError_t init_kernel_attrs() {
   cudaError_t e;
 #define TE_ATTR(call) if ((e = (call)) != cudaSuccess) return e
@@ -344,11 +368,11 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
   TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemm2_kernel<192, te::EPI_RESID, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::Gemm2Cfg<192, te::EPI_RESID>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmWideCfg::SMEM_LIMIT)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::AttnCfg<128, 1>::SMEM_BYTES)));
@@ -366,21 +390,142 @@ cudaError_t init_kernel_attrs() {
   return cudaSuccess;
 }
 
-// One wave of wide CTA-pair tiles for a residual GEMM (te_gemm_wide.cuh).  W: [n_rows, k_cols] weights.
+// One wave of wide CTA-pair tiles (te_gemm_wide.cuh).  tmB: the weight matrix in boxes of `box_rows` rows.
 template <int EPI>
-cudaError_t launch_wide(const bf16* W, int n_rows, int k_cols, const CUtensorMap& tmA, const te::GemmParams& p,
+cudaError_t launch_wide(const LaunchCtx& lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
                         int n_tiles, int bn, cudaStream_t st) {
-  CUtensorMap tmB;
-  if (!make_tmap(&tmB, W, n_rows, k_cols, bn / 4)) return cudaErrorInvalidValue;  // box = one MMA's rows of one CTA
-  const int num_mp = (p.M + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
-  return launch_k(te::te_gemm_wide_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
+  const int num_mp = (p.num_m_blk + 1) / 2;
+  return launch_k(lc, te::te_gemm_wide_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
                   te::GemmWideCfg::smem_bytes(bn), st, tmA, tmB, p, bn);
 }
 
-// Enqueue the whole stack on `st`.  Returns the number of kernels launched via *n_kernels.
+// Token-count bucket: the row-block count that every grid and every dispatch decision is derived from.
+// Small batches: 128-row blocks; from 1024 rows on the CTA-pair kernels work on 256-row blocks.
+int bucket_tokens(int T) {
+  int tb = (T + 127) / 128 * 128;
+  if (tb >= 1024) tb = (T + 255) / 256 * 256;
+  return tb;
+}
+
+Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
+  const te_config& c = h->cfg;
+  const int d = c.hidden, dh = c.head_dim, F = c.ffn;
+  const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
+  Plan pl;
+  pl.Tb = Tb;
+  // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
+  // one CTA per tile so that more SMs stream weights (HBM-bound regime).
+  pl.pair = h->pair_mode == 2 ? (Tb >= 1024 ? 1 : 0) : h->pair_mode;
+  // Small batches: when a GEMM has at most one 128-row tile per SM it runs on the split-K kernel, with
+  // as many CTAs per tile as the SM count allows (QKV then uses one-head-wide 128-column tiles).
+  const int num_m = (Tb + te::GEMM_BM - 1) / te::GEMM_BM;
+  pl.num_m = num_m;
+  const bool kmode = !pl.pair && h->splitk;
+  pl.bn_qkv = (kmode && num_m * (n_qkv / 128) <= h->sm_count) ? 128 : h->bn_qkv;
+  pl.k_qkv = kmode && pl.bn_qkv == 128;
+  // more one-head tiles than SMs (512 < T < 1024 at full width): 256-row CTA-pair tiles, as for gate/up below
+  pl.pair_qkv = pl.pair || (kmode && !pl.k_qkv && Tb > te::GEMM_BM && h->pair_mode == 2);
+  pl.bx_qkv = box_index(pl.pair_qkv ? pl.bn_qkv / 2 : pl.bn_qkv);
+  // gate/up tile width: the weights are interleaved per bn_gu = 256 rows; 128-wide tiles read them as two 64-row
+  // halves (gu_half).  With one row block (T <= 128) 96 one-CTA tiles stream the weights with no split-K exchange.
+  const bool gu128_k = kmode && h->bn_gu == 256 && num_m * (2 * F / 128) <= h->sm_count;
+  pl.bn_gu = gu128_k ? 128 : h->bn_gu;
+  pl.gu_half = pl.bn_gu != h->bn_gu;
+  pl.k_gu = kmode && num_m * (2 * F / pl.bn_gu) <= h->sm_count;
+  // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
+  // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
+  pl.pair_gu = pl.pair || (kmode && !pl.k_gu && Tb > te::GEMM_BM && h->pair_mode == 2);
+  // ... and when those pair tiles need two or more waves (T = 512: 96 tiles on 74 pairs), ONE wave of wide SwiGLU
+  // tiles instead: w output columns per tile = F / (pairs / row-pair blocks), rounded up to 64 (te_gemm_wide.cuh)
+  const int np = h->sm_count / 2;
+  const int mp_cnt = (num_m + 1) / 2;
+  if (kmode && pl.pair_gu && h->resid_wide == 1 && h->bn_gu == 256) {
+    const int nt = np / mp_cnt;
+    if (nt >= 1) {
+      const int w = (((F + nt - 1) / nt) + 63) / 64 * 64;
+      const int waves256 = (mp_cnt * (2 * F / h->bn_gu) + np - 1) / np;
+      if (2 * w <= 512 && waves256 >= 2 && 2 * w < waves256 * h->bn_gu) { pl.gu_wide_w = w; pl.gu_wide_tiles = (F + w - 1) / w; }
+    }
+  }
+  pl.bx_gu = pl.gu_half ? box_index(64) : box_index(pl.pair_gu ? h->bn_gu / 2 : h->bn_gu);
+  // Residual GEMMs on CTA pairs: when their 128-wide tiles would take >= 2 waves, one wave of wide tiles instead
+  // (te_gemm_wide.cuh): n_tiles = pairs / row-pair blocks, width = N / n_tiles rounded up to 32 (<= 512).
+  if (pl.pair && h->resid_wide) {
+    int nt = h->resid_wide >= 2 ? h->resid_wide : np / mp_cnt;
+    const int cap = h->ssq_parts_cap / 2 < d / 32 ? h->ssq_parts_cap / 2 : d / 32;
+    if (nt > cap) nt = cap;
+    if (nt >= 1) {
+      const int bn = (((d + nt - 1) / nt) + 31) / 32 * 32;
+      const int waves128 = (mp_cnt * (d / 128) + np - 1) / np;
+      const bool wins = waves128 >= 2 && bn * 4 < waves128 * 128 * 5;
+      if (bn <= 512 && mp_cnt * nt <= np && (h->resid_wide >= 2 || wins)) { pl.wide_tiles = nt; pl.wide_bn = bn; }
+    }
+  }
+  pl.bn_res = h->bn_res;
+  pl.k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;
+  pl.bx_res = box_index(pl.pair ? pl.bn_res / 2 : pl.bn_res);
+  pl.n_blk_res = d / pl.bn_res;
+  // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
+  pl.parts = pl.wide_tiles ? pl.wide_tiles * 2 : pl.n_blk_res * ((pl.pair || pl.k_res) ? 2 : 1);
+  // attention: host-side upper bound of S_b for the grid (exact lengths stay on the device)
+  int s_bound = Tb - (n_frames - 1) * n_vis;
+  if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
+  if (s_bound < 1) s_bound = 1;
+  pl.s_bound = s_bound;
+  pl.q_blocks = (s_bound + te::ATT_BQ - 1) / te::ATT_BQ;
+  pl.g_shift = h->g_shift;
+  pl.attn_tc = h->attn_impl == 1 && h->attn_tc_ok;
+  if (pl.attn_tc) {
+    // one CTA per (frame, kv head), split over query tiles when the batch alone cannot fill the SMs
+    const int pt = 128 >> h->g_shift;
+    const int tiles_max = (s_bound + pt - 1) / pt;
+    int sp = h->sm_count / (n_frames * c.n_kv_heads);
+    if (sp < 1) sp = 1;
+    if (sp > tiles_max) sp = tiles_max;
+    pl.attn_split = sp;
+  }
+  return pl;
+}
+
+// What ran, by class, in the names ncu prints (te_dispatch_info; bench.py's roofline label).
+std::string describe_plan(const te_handle* h, const Plan& pl) {
+  const te_config& c = h->cfg;
+  char b[160];
+  std::string s;
+  auto gemm = [&](const char* cls, int epi, bool k, bool pair2, int bn, int dh) {
+    if (k) snprintf(b, sizeof(b), "%s=te_gemmk_kernel<%d, %d, %d>;", cls, bn, epi, dh);
+    else if (pair2) snprintf(b, sizeof(b), "%s=te_gemm2_kernel<%d, %d, %d>;", cls, bn, epi, dh);
+    else snprintf(b, sizeof(b), "%s=te_gemm_kernel<%d, %d, %d>;", cls, bn, epi, dh);
+    s += b;
+  };
+  gemm("qkv", te::EPI_QKV, pl.k_qkv, pl.pair_qkv, pl.bn_qkv, c.head_dim);
+  snprintf(b, sizeof(b), "attn=%s;", pl.attn_tc ? (c.head_dim == 128 ? "te_attn_tc_kernel<128>" : "te_attn_tc_kernel<64>")
+                                                : "te_attn_kernel");
+  s += b;
+  if (pl.wide_tiles) {
+    snprintf(b, sizeof(b), "oproj=te_gemm_wide_kernel<2> (%d tiles x %d cols);down=te_gemm_wide_kernel<2> (%d tiles x %d cols);",
+             pl.wide_tiles, pl.wide_bn, pl.wide_tiles, pl.wide_bn);
+    s += b;
+  } else {
+    gemm("oproj", te::EPI_RESID, pl.k_res, pl.pair, pl.bn_res, 128);
+    gemm("down", te::EPI_RESID, pl.k_res, pl.pair, pl.bn_res, 128);
+  }
+  if (pl.gu_wide_tiles) {
+    snprintf(b, sizeof(b), "gateup=te_gemm_wide_kernel<3> (%d tiles x %d cols);", pl.gu_wide_tiles, pl.gu_wide_w);
+    s += b;
+  } else {
+    gemm("gateup", te::EPI_SWIGLU, pl.k_gu, pl.pair_gu, pl.bn_gu, 128);
+  }
+  snprintf(b, sizeof(b), "bucket_tokens=%d", pl.Tb);
+  s += b;
+  return s;
+}
+
+// Enqueue the whole stack on `st` for the shape class `Tb` (per-call pointers and the exact token count are in
+// h->dyn, written on the stream before this sequence).  Returns the number of kernels launched via *n_kernels.
 // prefix_pass: the one-frame pass of te_encode_prefix (text only, ids 0..T-1) that also saves every layer's K/V.
-int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const float* embeds, const int32_t* lens, int T,
-                  float* out, cudaStream_t st, int* n_kernels, bool prefix_pass = false) {
+int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cudaStream_t st, int* n_kernels,
+                  bool prefix_pass = false, int prefix_rows = 0) {
   const te_config& c = h->cfg;
   const int d = c.hidden, dh = c.head_dim, F = c.ffn;
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
@@ -389,79 +534,9 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
   const bool dbg_stop = !prefix_pass && h->dbg_stop;
   const int P = prefix_pass ? 0 : h->prefix_len;  // cached prefix keys in front of every frame
   const int n_kv = 2 * c.n_kv_heads * dh;
-  // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
-  // one CTA per tile so that more SMs stream weights (HBM-bound regime).
-  const int pair = h->pair_mode == 2 ? (T >= 1024 ? 1 : 0) : h->pair_mode;
-  // Small batches: when a GEMM has at most one 128-row tile per SM it runs on the split-K kernel, with
-  // as many CTAs per tile as the SM count allows (QKV then uses one-head-wide 128-column tiles).
-  const int num_m = (T + te::GEMM_BM - 1) / te::GEMM_BM;
-  const bool kmode = !pair && h->splitk;
-  const int bn_qkv = (kmode && num_m * (n_qkv / 128) <= h->sm_count) ? 128 : h->bn_qkv;
-  const bool k_qkv = kmode && bn_qkv == 128;
-  // more one-head tiles than SMs (512 < T < 1024 at full width): 256-row CTA-pair tiles, as for gate/up below
-  const bool pair_qkv = pair || (kmode && !k_qkv && T > te::GEMM_BM && h->pair_mode == 2);
-  // gate/up tile width: the weights are interleaved per bn_gu = 256 rows; 128-wide tiles read them as two 64-row
-  // halves (gu_half).  With one row block (T <= 128) 96 one-CTA tiles stream the weights with no split-K exchange
-  // (cfg 2: 27 -> 19 us).  (128-wide CTA-pair tiles at T = 512, 3 waves instead of 2 imbalanced ones, measured
-  // the same as 256-wide ones: they are L2->SM-bound.)
-  const bool gu128_k = kmode && h->bn_gu == 256 && num_m * (2 * F / 128) <= h->sm_count;
-  const int bn_gu = gu128_k ? 128 : h->bn_gu;
-  const bool k_gu = kmode && num_m * (2 * F / bn_gu) <= h->sm_count;
-  const bool k_res = kmode && num_m * (d / h->bn_res) <= h->sm_count;  // (kmode: bn_res == h->bn_res)
-  const int bx_qkv = box_index(pair_qkv ? bn_qkv / 2 : bn_qkv);
-  // gate/up with more tiles than SMs but too few tokens for pairs everywhere (e.g. T = 512: 192 tiles of
-  // 128 x 256): 256-row CTA-pair tiles halve the L2->SM operand traffic per FLOP, which bounds this regime
-  const bool pair_gu = pair || (kmode && !k_gu && T > te::GEMM_BM && h->pair_mode == 2);
-  // ... and when those pair tiles need two or more waves (T = 512: 96 tiles on 74 pairs), ONE wave of wide SwiGLU tiles
-  // over the non-interleaved [Wgate; Wup] instead: w output columns per tile = F / (pairs / row-pair blocks),
-  // rounded up to 32 (te_gemm_wide.cuh)
-  int gu_wide_tiles = 0, gu_wide_w = 0;
-  if (kmode && pair_gu && h->resid_wide == 1) {
-    const int np = h->sm_count / 2;
-    const int mp_cnt = (T + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
-    const int nt = np / mp_cnt;
-    if (nt >= 1) {
-      const int w = (((F + nt - 1) / nt) + 31) / 32 * 32;
-      const int waves256 = (mp_cnt * (2 * F / h->bn_gu) + np - 1) / np;
-      if (2 * w <= 512 && waves256 >= 2 && 2 * w < waves256 * h->bn_gu) { gu_wide_w = w; gu_wide_tiles = (F + w - 1) / w; }
-    }
-  }
-  const int bx_gu = (bn_gu != h->bn_gu) ? 0 : box_index(pair_gu ? h->bn_gu / 2 : h->bn_gu);  // gu_half: 64-row boxes
-
-  // Residual GEMMs on CTA pairs: when their 128-wide tiles would take >= 2 waves, one wave of wide tiles instead
-  // (te_gemm_wide.cuh): n_tiles = pairs / row-pair blocks, width = N / n_tiles rounded up to 32 (<= 512).
-  int wide_tiles = 0, wide_bn = 0;
-  if (pair && h->resid_wide) {
-    const int np = h->sm_count / 2;
-    const int mp_cnt = (T + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
-    int nt = h->resid_wide >= 2 ? h->resid_wide : np / mp_cnt;
-    const int cap = h->ssq_parts_cap / 2 < d / 32 ? h->ssq_parts_cap / 2 : d / 32;
-    if (nt > cap) nt = cap;
-    if (nt >= 1) {
-      const int bn = (((d + nt - 1) / nt) + 31) / 32 * 32;
-      const int waves128 = (mp_cnt * (d / 128) + np - 1) / np;
-      const bool wins = waves128 >= 2 && bn * 4 < waves128 * 128 * 5;
-      if (bn <= 512 && mp_cnt * nt <= np && (h->resid_wide >= 2 || wins)) { wide_tiles = nt; wide_bn = bn; }
-    }
-  }
-  // Residual tile width on CTA pairs (auto when TE_OPT_RESID_BLOCK_N was not set): cost ~ waves x width, with 128-wide
-  // tiles 1.3x dearer per column (they are L2->SM-bound); 192-wide tiles give cfg 4 132 tiles = 2 waves.
-  int bn_res = h->bn_res;
-  if (pair && !wide_tiles && h->bn_res_auto) {
-    const int np = h->sm_count / 2;
-    const int mp_cnt = (T + 2 * te::GEMM_BM - 1) / (2 * te::GEMM_BM);
-    double best = 1e30;
-    for (int bn : {128, 192, 256}) {
-      const int tiles = mp_cnt * ((d + bn - 1) / bn);
-      const double cost = (double)((tiles + np - 1) / np) * bn * (bn == 128 ? 1.3 : 1.0);
-      if (cost < best - 1e-9 && 2 * ((d + bn - 1) / bn) <= h->ssq_parts_cap) { best = cost; bn_res = bn; }
-    }
-  }
-  CUtensorMap tm_res192_o, tm_res192_d;  // 96-row boxes for the 192-wide pair tiles (encoded per layer below)
-  // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
-  const int bx_res = box_index(pair ? (bn_res == 192 ? 128 : bn_res) / 2 : bn_res);
-  const int n_blk_res = (d + bn_res - 1) / bn_res;
-  const int parts = wide_tiles ? wide_tiles * 2 : n_blk_res * ((pair || k_res) ? 2 : 1);
+  const Plan pl = make_plan(h, Tb, n_frames, grid_h * grid_w);
+  if (!prefix_pass) h->last_plan = pl;
+  const int num_m = pl.num_m;
   int nk = 0;
   // Optional per-kernel CUDA-event bracketing (TE_OPT_KERNEL_TIMING; never inside a capture).
   cudaEvent_t ev_a = nullptr;
@@ -478,191 +553,165 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, const floa
     h->timed.push_back({kclass, ev_a, ev_b});
   };
 
-  g_pdl = h->pdl && !h->timing;
+  LaunchCtx lc;
+  lc.pdl = h->pdl && !h->timing;
   // The fp32 residual stream (read and rewritten by both residual GEMMs of every layer) is marked persisting in L2
   // for every kernel of the stack, so that its 2 x 2 passes per layer stay out of DRAM (TE_OPT_L2_RESIDUAL).
-  g_l2_window = cudaAccessPolicyWindow{};
   if (h->l2_resid && h->l2_limit_bytes > 0) {
-    const size_t bytes = (size_t)T * d * sizeof(float);
-    g_l2_window.base_ptr = out;
-    g_l2_window.num_bytes = bytes;
-    g_l2_window.hitRatio = bytes <= h->l2_limit_bytes ? 1.0f : (float)h->l2_limit_bytes / (float)bytes;
-    g_l2_window.hitProp = cudaAccessPropertyPersisting;
-    g_l2_window.missProp = cudaAccessPropertyStreaming;
+    const size_t bytes = (size_t)Tb * d * sizeof(float);
+    lc.l2.base_ptr = h->resid;
+    lc.l2.num_bytes = bytes;
+    lc.l2.hitRatio = bytes <= h->l2_limit_bytes ? 1.0f : (float)h->l2_limit_bytes / (float)bytes;
+    lc.l2.hitProp = cudaAccessPropertyPersisting;
+    lc.l2.missProp = cudaAccessPropertyStreaming;
   }
   {
     te::PrepParams pp{};
-    pp.embeds = embeds; pp.text_lens = lens; pp.out = out; pp.cu = h->cu; pp.flag = h->flag; pp.pos = h->pos;
+    pp.dyn = h->dyn; pp.out = h->resid; pp.cu = h->cu; pp.flag = h->flag; pp.pos = h->pos;
     pp.cos_t = h->cos_t; pp.sin_t = h->sin_t;
     pp.inv_freq = h->inv_freq; pp.g_first = h->w + h->off[lb].g1; pp.xg = h->xg; pp.ssq = h->ssq;
-    pp.ssq_parts = parts; pp.ssq_stride = h->ssq_parts_cap; pp.n_frames = n_frames; pp.total_tokens = T; pp.d = d;
+    pp.ssq_parts = pl.parts; pp.ssq_stride = h->ssq_parts_cap; pp.n_frames = n_frames; pp.d = d;
     pp.half_dim = dh / 2; pp.max_tokens_per_frame = c.max_tokens_per_frame;
     pp.grid_h = grid_h; pp.grid_w = grid_w; pp.pos_offset = P;
     memcpy(pp.axis, h->axis, sizeof(pp.axis));
     tick();
-    TE_CUDA(h, launch_k(te::te_prep_kernel, dim3(T), dim3(256), 0, st, pp));
+    pp.qkv_rows = reinterpret_cast<uint4*>(h->qkv); pp.qkv_row_vec16 = n_qkv / 8;
+    TE_CUDA(h, launch_k(lc, te::te_prep_kernel, dim3(Tb + te::PREP_PAD_ROWS), dim3(256), 0, st, pp));
     tock(TE_KCLASS_PREP);
     ++nk;
   }
-  CUtensorMap tmA_xg, tmA_attn, tmA_act;
-  if (!make_tmap(&tmA_xg, h->xg, T, d, te::GEMM_BM) || !make_tmap(&tmA_attn, h->attn, T, n_q, te::GEMM_BM) ||
-      !make_tmap(&tmA_act, h->act, T, F, te::GEMM_BM)) {
-    h->err = "cuTensorMapEncodeTiled failed for an activation map";
-    return TE_ERR_CUDA;
-  }
   te::GemmParams base{};
-  base.splits = 1; base.sk_scratch = h->sk_scratch; base.sk_sem = h->sk_sem; base.streamk = h->streamk;
-  base.M = T; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = parts; base.ssq_stride = h->ssq_parts_cap;
+  base.dyn = h->dyn;
+  base.splits = 1; base.sk_scratch = h->sk_scratch; base.sk_sem = h->sk_sem;
+  base.M = Tb; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = pl.parts; base.ssq_stride = h->ssq_parts_cap;
   base.inv_d = 1.0f / static_cast<float>(d); base.eps = c.rms_eps;
   const size_t trace_stride = (size_t)h->sm_count * te::TRACE_SLOTS;
   auto trace_ptr = [&](int cls) { return h->trace_on ? h->trace + cls * trace_stride : nullptr; };
-
-  // host-side upper bound of S_b for the attention grid (exact lengths stay on the device)
-  int s_bound = T - (n_frames - 1) * (grid_h * grid_w);
-  if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
-  const int q_blocks = (s_bound + te::ATT_BQ - 1) / te::ATT_BQ;
-  // tcgen05 attention: one CTA per (frame, kv head), optionally split over query tiles when the batch
-  // alone cannot fill the SMs; needs G = Hq/Hkv to be a power of two with >= 16 positions per 128-row tile
-  const int G = c.n_q_heads / c.n_kv_heads;
-  int g_shift = 0;
-  while ((1 << g_shift) < G) ++g_shift;
-  // (with a cached prefix the tcgen05 kernel runs twice per layer: frame-local keys, then the prefix keys merged
-  //  into the result through the saved row statistics)
-  const bool attn_tc = h->attn_impl == 1 && (1 << g_shift) == G && G <= 8;
-  CUtensorMap tmQ, tmKV;
-  int attn_split = 1;
-  if (attn_tc) {
-    const int pt = 128 >> g_shift;
-    if (!make_tmap(&tmQ, h->qkv, T, n_qkv, pt) || !make_tmap(&tmKV, h->qkv, T, n_qkv, 64)) {
-      h->err = "cuTensorMapEncodeTiled failed for a qkv map";
-      return TE_ERR_CUDA;
-    }
-    const int tiles_max = (s_bound + pt - 1) / pt;
-    attn_split = h->sm_count / (n_frames * c.n_kv_heads);
-    if (attn_split < 1) attn_split = 1;
-    if (attn_split > tiles_max) attn_split = tiles_max;
-  }
+  // the last residual GEMM of the stack hands the stream over to the caller's buffer
+  const bool norm_tail = c.final_norm && le == c.n_layers && !dbg_stop;
 
   for (int l = lb; l < le; ++l) {
     const LayerOff& o = h->off[l];
+    const bool last_layer = l == le - 1;
     {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
       te::GemmParams p = base;
-      p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / bn_qkv;
+      p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / pl.bn_qkv;
       p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
       p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
       p.trace = trace_ptr(0);
       tick();
-      if (k_qkv) {
-        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
-        TE_CUDA(h, launch_gemmk_bn<te::EPI_QKV>(bn_qkv, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, st));
+      if (pl.k_qkv) {
+        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_QKV>(lc, pl.bn_qkv, dh, h->tmA_xg, h->tm[l].qkv[pl.bx_qkv], p, st));
       } else {
-        TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(bn_qkv, pair_qkv, dh, tmA_xg, h->tm[l].qkv[bx_qkv], p, h->sm_count, st));
+        TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(lc, pl.bn_qkv, pl.pair_qkv, dh, h->tmA_xg, h->tm[l].qkv[pl.bx_qkv], p,
+                                                h->sm_count, st));
       }
       tock(TE_KCLASS_QKV);
       ++nk;
     }
     if (prefix_pass) {  // keep this layer's keys | values of the prefix tokens
       TE_CUDA(h, cudaMemcpy2DAsync(h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv, (size_t)n_kv * sizeof(bf16),
-                                   h->qkv + n_q, (size_t)n_qkv * sizeof(bf16), (size_t)n_kv * sizeof(bf16), T,
-                                   cudaMemcpyDeviceToDevice, st));
+                                   h->qkv + n_q, (size_t)n_qkv * sizeof(bf16), (size_t)n_kv * sizeof(bf16),
+                                   prefix_rows, cudaMemcpyDeviceToDevice, st));
     }
     {  // a2: causal GQA attention
-      te::AttnParams ap{};
-      ap.qkv = h->qkv; ap.out = h->attn; ap.cu_seqlens = h->cu; ap.ld = n_qkv; ap.n_q_heads = c.n_q_heads;
-      ap.n_kv_heads = c.n_kv_heads; ap.total_tokens = T;
-      ap.scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
-      ap.prefix_len = P; ap.ld_prefix = n_kv;
-      ap.kv_prefix = P > 0 ? h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv : nullptr;
+      const float scale_log2 = static_cast<float>(1.4426950408889634 / std::sqrt(static_cast<double>(dh)));
       tick();
-      if (attn_tc) {
+      if (pl.attn_tc) {
         te::AttnTcParams tp{};
         tp.out = h->attn; tp.cu_seqlens = h->cu; tp.n_q_heads = c.n_q_heads; tp.n_kv_heads = c.n_kv_heads;
-        tp.g_shift = g_shift; tp.total_tokens = T; tp.scale_log2 = ap.scale_log2;
+        tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2;
         tp.stats = P > 0 ? h->attn_stats : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
-        TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(tmQ, tmKV, tp, attn_split, n_frames, st)
-                             : launch_attn_tc<64>(tmQ, tmKV, tp, attn_split, n_frames, st));
+        TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st)
+                             : launch_attn_tc<64>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st));
         if (P > 0) {  // second pass: the P cached prefix keys of this layer, merged in place
           tp.prefix_mode = 1; tp.prefix_len = P;
-          TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(tmQ, h->tm_prefix[l], tp, attn_split, n_frames, st)
-                               : launch_attn_tc<64>(tmQ, h->tm_prefix[l], tp, attn_split, n_frames, st));
+          TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tm_prefix[l], tp, pl.attn_split, n_frames, st)
+                               : launch_attn_tc<64>(lc, h->tmQ, h->tm_prefix[l], tp, pl.attn_split, n_frames, st));
           ++nk;
         }
       } else {
-        TE_CUDA(h, launch_attn_any(dh, ap, q_blocks, n_frames, st));
+        te::AttnParams ap{};
+        ap.qkv = h->qkv; ap.out = h->attn; ap.cu_seqlens = h->cu; ap.ld = n_qkv; ap.n_q_heads = c.n_q_heads;
+        ap.n_kv_heads = c.n_kv_heads; ap.scale_log2 = scale_log2;
+        ap.prefix_len = P; ap.ld_prefix = n_kv;
+        ap.kv_prefix = P > 0 ? h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv : nullptr;
+        TE_CUDA(h, launch_attn_any(lc, dh, ap, pl.q_blocks, n_frames, st));
       }
       tock(TE_KCLASS_ATTN);
       ++nk;
     }
     {  // a3: O projection + residual add (+ next norm's gain / statistics)
       te::GemmParams p = base;
-      p.N = d; p.K = n_q; p.num_n_blk = n_blk_res;
-      p.x = out; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
+      p.N = d; p.K = n_q; p.num_n_blk = pl.n_blk_res;
+      p.x = h->resid; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
+      p.x_to_out = (dbg_stop && last_layer) ? 1 : 0;
       p.trace = trace_ptr(1);
       tick();
-      if (wide_tiles) {
-        TE_CUDA(h, launch_wide<te::EPI_RESID>(h->w + o.wo, d, n_q, tmA_attn, p, wide_tiles, wide_bn, st));
-      } else if (k_res) {
-        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
-        TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_attn, h->tm[l].o[bx_res], p, st));
+      if (pl.wide_tiles) {
+        CUtensorMap tmB;
+        if (!make_tmap(&tmB, h->w + o.wo, d, n_q, pl.wide_bn / 4)) { h->err = "tensor map (wide O-proj)"; return TE_ERR_CUDA; }
+        TE_CUDA(h, launch_wide<te::EPI_RESID>(lc, h->tmA_attn, tmB, p, pl.wide_tiles, pl.wide_bn, st));
+      } else if (pl.k_res) {
+        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(lc, pl.bn_res, dh, h->tmA_attn, h->tm[l].o[pl.bx_res], p, st));
       } else {
-        const CUtensorMap* tmb = &h->tm[l].o[bx_res];
-        if (bn_res == 192) {
-          if (!make_tmap(&tm_res192_o, h->w + o.wo, d, n_q, 96)) { h->err = "tensor map (192-wide O-proj)"; return TE_ERR_CUDA; }
-          tmb = &tm_res192_o;
-        }
-        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(bn_res, pair, dh, tmA_attn, *tmb, p, h->sm_count, st));
+        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(lc, pl.bn_res, pl.pair, dh, h->tmA_attn, h->tm[l].o[pl.bx_res], p,
+                                                  h->sm_count, st));
       }
       tock(TE_KCLASS_OPROJ);
       ++nk;
     }
-    if (dbg_stop && l == le - 1) break;
+    if (dbg_stop && last_layer) break;
     {  // a4: RMSNorm -> gate/up GEMM -> SiLU(gate) * up
       te::GemmParams p = base;
-      p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / bn_gu; p.gu_half = (bn_gu != h->bn_gu) ? 1 : 0;
+      p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / pl.bn_gu; p.gu_half = pl.gu_half;
       p.act = h->act; p.ld_act = F;
       p.trace = trace_ptr(2);
       tick();
-      if (gu_wide_tiles) {
+      if (pl.gu_wide_tiles) {
         p.gu_half = 0;
-        TE_CUDA(h, launch_wide<te::EPI_SWIGLU>(h->w_gu_plain + (size_t)l * 2 * F * d, 2 * F, d, tmA_xg, p, gu_wide_tiles,
-                                               2 * gu_wide_w, st));
-      } else if (k_gu) {
-        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
-        TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(bn_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, st));
+        TE_CUDA(h, launch_wide<te::EPI_SWIGLU>(lc, h->tmA_xg, h->tm[l].gu[box_index(32)], p, pl.gu_wide_tiles,
+                                               2 * pl.gu_wide_w, st));
+      } else if (pl.k_gu) {
+        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(lc, pl.bn_gu, dh, h->tmA_xg, h->tm[l].gu[pl.bx_gu], p, st));
       } else {
-        TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(bn_gu, pair_gu, dh, tmA_xg, h->tm[l].gu[bx_gu], p, h->sm_count, st));
+        TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(lc, pl.bn_gu, pl.pair_gu, dh, h->tmA_xg, h->tm[l].gu[pl.bx_gu], p,
+                                                   h->sm_count, st));
       }
       tock(TE_KCLASS_GATEUP);
       ++nk;
     }
     {  // a5: down projection + residual add
       te::GemmParams p = base;
-      p.N = d; p.K = F; p.num_n_blk = n_blk_res;
-      p.x = out; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
+      p.N = d; p.K = F; p.num_n_blk = pl.n_blk_res;
+      p.x = h->resid; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
       p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
+      p.x_to_out = (last_layer && !norm_tail) ? 1 : 0;
       p.trace = trace_ptr(3);
       tick();
-      if (wide_tiles) {
-        TE_CUDA(h, launch_wide<te::EPI_RESID>(h->w + o.wd, d, F, tmA_act, p, wide_tiles, wide_bn, st));
-      } else if (k_res) {
-        p.splits = choose_splits(num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
-        TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(h->bn_res, dh, tmA_act, h->tm[l].d[bx_res], p, st));
+      if (pl.wide_tiles) {
+        CUtensorMap tmB;
+        if (!make_tmap(&tmB, h->w + o.wd, d, F, pl.wide_bn / 4)) { h->err = "tensor map (wide down)"; return TE_ERR_CUDA; }
+        TE_CUDA(h, launch_wide<te::EPI_RESID>(lc, h->tmA_act, tmB, p, pl.wide_tiles, pl.wide_bn, st));
+      } else if (pl.k_res) {
+        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+        TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(lc, pl.bn_res, dh, h->tmA_act, h->tm[l].d[pl.bx_res], p, st));
       } else {
-        const CUtensorMap* tmb = &h->tm[l].d[bx_res];
-        if (bn_res == 192) {
-          if (!make_tmap(&tm_res192_d, h->w + o.wd, d, F, 96)) { h->err = "tensor map (192-wide down)"; return TE_ERR_CUDA; }
-          tmb = &tm_res192_d;
-        }
-        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(bn_res, pair, dh, tmA_act, *tmb, p, h->sm_count, st));
+        TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(lc, pl.bn_res, pl.pair, dh, h->tmA_act, h->tm[l].d[pl.bx_res], p,
+                                                  h->sm_count, st));
       }
       tock(TE_KCLASS_DOWN);
       ++nk;
     }
   }
-  if (c.final_norm && le == c.n_layers && !dbg_stop) {  // a6
+  if (norm_tail) {  // a6: residual stream -> RMSNorm -> the caller's buffer
     tick();
-    TE_CUDA(h, launch_k(te::te_final_norm_kernel, dim3((T + 7) / 8), dim3(256), 0, st, out,
-                        static_cast<const bf16*>(h->w + h->gf_off), T, d, c.rms_eps));
+    TE_CUDA(h, launch_k(lc, te::te_final_norm_kernel, dim3((Tb + 7) / 8), dim3(256), 0, st,
+                        static_cast<const float*>(h->resid), static_cast<const te::DynParams*>(h->dyn),
+                        static_cast<const bf16*>(h->w + h->gf_off), d, c.rms_eps));
     tock(TE_KCLASS_FINAL_NORM);
     ++nk;
   }
@@ -676,6 +725,24 @@ void free_graphs(te_handle* h) {
     cudaGraphDestroy(e.graph);
   }
   h->cache.clear();
+}
+
+// Per-call values -> device block, on the stream, ahead of the stack (values travel as kernel parameters).
+cudaError_t set_dyn(te_handle* h, const float* embeds, const int32_t* lens, float* out, int T, cudaStream_t st) {
+  te::DynParams v{};
+  v.embeds = embeds; v.text_lens = lens; v.out = out; v.total_tokens = T;
+  te::te_set_dyn_kernel<<<1, 32, 0, st>>>(h->dyn, v);
+  return cudaGetLastError();
+}
+
+void release_l2_limit(te_handle* h) {
+  if (h->l2_limit_raised) {
+    cudaCtxResetPersistingL2Cache();
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, h->l2_prev_limit);
+    cudaGetLastError();
+    h->l2_limit_raised = false;
+  }
+  h->l2_limit_bytes = 0;
 }
 
 }  // namespace
@@ -710,18 +777,22 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   h->dbg_le = cfg->n_layers;
   const te_config& c = h->cfg;
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim;
+  const int n_q = c.n_q_heads * c.head_dim;
   h->bn_qkv = (n_qkv % 256 == 0) ? 256 : 128;
   h->bn_gu = ((2 * c.ffn) % 256 == 0) ? 256 : 128;
   h->bn_res = 128;  // O/down: N = hidden is small -> 128-wide tiles halve the wave-quantisation loss
   h->ssq_parts_cap = ((c.hidden / 128) * (te::GEMM2_EPI_WARPS / 4) + 3) & ~3;  // row stride of ssq (16-byte aligned rows)
+  h->cap_rows = (c.max_tokens + 255) / 256 * 256 + te::PREP_PAD_ROWS;  // (+ the zeroed rows past the last token)
 
   auto fail = [&](int code) {
     te_destroy(h);
     return code;
   };
-  const size_t T = c.max_tokens, B = c.max_frames, hd2 = c.head_dim / 2;
+  const size_t T = h->cap_rows, B = c.max_frames, hd2 = c.head_dim / 2;
 #define TE_ALLOC(ptr, bytes) \
   if (cudaMalloc(reinterpret_cast<void**>(&(ptr)), (bytes)) != cudaSuccess) return fail(TE_ERR_CUDA)
+  TE_ALLOC(h->dyn, sizeof(te::DynParams));
+  TE_ALLOC(h->resid, T * c.hidden * sizeof(float));
   TE_ALLOC(h->cu, (B + 1) * sizeof(int32_t));
   TE_ALLOC(h->pos, 3 * T * sizeof(int32_t));
   TE_ALLOC(h->flag, sizeof(int32_t));
@@ -731,12 +802,19 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   TE_ALLOC(h->inv_freq, hd2 * sizeof(double));
   TE_ALLOC(h->xg, T * c.hidden * sizeof(bf16));
   TE_ALLOC(h->qkv, T * n_qkv * sizeof(bf16));
-  TE_ALLOC(h->attn, T * (size_t)c.n_q_heads * c.head_dim * sizeof(bf16));
+  TE_ALLOC(h->attn, T * (size_t)n_q * sizeof(bf16));
   TE_ALLOC(h->act, T * c.ffn * sizeof(bf16));
   TE_ALLOC(h->sk_scratch, (size_t)h->sm_count * te::GEMM_BM * 256 * sizeof(float));
   TE_ALLOC(h->sk_sem, 2 * (size_t)h->sm_count * sizeof(int));
 #undef TE_ALLOC
-  if (cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess) return fail(TE_ERR_CUDA);
+  // rows past a call's tokens are read (never stored) by the tile-granular kernels: start them finite
+  if (cudaMemset(h->xg, 0, T * c.hidden * sizeof(bf16)) != cudaSuccess ||
+      cudaMemset(h->qkv, 0, T * n_qkv * sizeof(bf16)) != cudaSuccess ||
+      cudaMemset(h->attn, 0, T * (size_t)n_q * sizeof(bf16)) != cudaSuccess ||
+      cudaMemset(h->act, 0, T * c.ffn * sizeof(bf16)) != cudaSuccess ||
+      cudaMemset(h->dyn, 0, sizeof(te::DynParams)) != cudaSuccess ||
+      cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess)
+    return fail(TE_ERR_CUDA);
   if (c.max_prefix_tokens > 0) {
     const size_t n_kv = 2 * (size_t)c.n_kv_heads * c.head_dim;
     if (cudaMalloc(reinterpret_cast<void**>(&h->kv_prefix), (size_t)c.n_layers * c.max_prefix_tokens * n_kv * sizeof(bf16)) !=
@@ -744,9 +822,21 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
         cudaMalloc(reinterpret_cast<void**>(&h->prefix_buf), (size_t)c.max_prefix_tokens * c.hidden * sizeof(float)) !=
             cudaSuccess ||
         cudaMalloc(reinterpret_cast<void**>(&h->prefix_lens), sizeof(int32_t)) != cudaSuccess ||
-        cudaMalloc(reinterpret_cast<void**>(&h->attn_stats), (size_t)c.max_tokens * c.n_q_heads * sizeof(float2)) !=
-            cudaSuccess)
+        cudaMalloc(reinterpret_cast<void**>(&h->attn_stats), T * c.n_q_heads * sizeof(float2)) != cudaSuccess)
       return fail(TE_ERR_CUDA);
+  }
+  {  // activation tensor maps over the whole workspace buffers (encoded once)
+    const int G = c.n_q_heads / c.n_kv_heads;
+    int g_shift = 0;
+    while ((1 << g_shift) < G) ++g_shift;
+    h->g_shift = g_shift;
+    // tcgen05 attention needs G = Hq/Hkv to be a power of two with >= 16 positions per 128-row query tile
+    h->attn_tc_ok = (1 << g_shift) == G && G <= 8;
+    bool ok = make_tmap(&h->tmA_xg, h->xg, T, c.hidden, te::GEMM_BM) && make_tmap(&h->tmA_attn, h->attn, T, n_q, te::GEMM_BM) &&
+              make_tmap(&h->tmA_act, h->act, T, c.ffn, te::GEMM_BM);
+    if (ok && h->attn_tc_ok)
+      ok = make_tmap(&h->tmQ, h->qkv, T, n_qkv, 128 >> g_shift) && make_tmap(&h->tmKV, h->qkv, T, n_qkv, 64);
+    if (!ok) return fail(TE_ERR_CUDA);
   }
   {  // axis of frequency pair i: contiguous [t | h | w], or round-robin over the axes with pairs left
     int left[3] = {c.rope_sec_t, c.rope_sec_h, c.rope_sec_w};
@@ -783,19 +873,18 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
   if (!h->w) TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->w), n_el * sizeof(bf16)));
   h->w_elems = n_el;
   // The device copy keeps the canonical layout (so Wq|Wk|Wv are already one fused [Nqkv, d] matrix);
-  // only [Wgate; Wup] is rewritten, interleaved per N-tile, via a per-layer staging buffer.
+  // only [Wgate; Wup] is rewritten, interleaved per N-tile, via a one-layer staging buffer.
   TE_CUDA(h, cudaMemcpy(h->w, blob, n_bytes, cudaMemcpyDefault));
   const size_t d = c.hidden, dh = c.head_dim, F = c.ffn;
   const size_t n_qkv = (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * dh, n_q = (size_t)c.n_q_heads * dh;
-  // [Wgate; Wup] of every layer is also kept as it is in the blob (wide SwiGLU tiles take gate and up rows from
-  // separate MMAs); that copy doubles as the source of the interleave below
-  if (!h->w_gu_plain) TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->w_gu_plain), (size_t)c.n_layers * 2 * F * d * sizeof(bf16)));
   bf16* stage = nullptr;
+  TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&stage), 2 * F * d * sizeof(bf16)));
   h->off.resize(c.n_layers);
   h->tm.resize(c.n_layers);
   size_t o = 0;
   bool ok = true;
-  for (int l = 0; l < c.n_layers; ++l) {
+  cudaError_t e = cudaSuccess;
+  for (int l = 0; l < c.n_layers && e == cudaSuccess; ++l) {
     LayerOff& L = h->off[l];
     L.g1 = o; o += d;
     L.wqkv = o; o += n_qkv * d;
@@ -805,20 +894,15 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
     L.g2 = o; o += d;
     L.wgu = o; o += 2 * F * d;
     L.wd = o; o += d * F;
-    stage = h->w_gu_plain + (size_t)l * 2 * F * d;
-    cudaError_t e = cudaMemcpy(stage, h->w + L.wgu, 2 * F * d * sizeof(bf16), cudaMemcpyDeviceToDevice);
+    e = cudaMemcpy(stage, h->w + L.wgu, 2 * F * d * sizeof(bf16), cudaMemcpyDeviceToDevice);
     if (e == cudaSuccess) {
       te::te_interleave_gate_up_kernel<<<(unsigned)(2 * F), 128>>>(
           reinterpret_cast<const uint4*>(stage), reinterpret_cast<const uint4*>(stage + F * d),
           reinterpret_cast<uint4*>(h->w + L.wgu), (int)F, (int)(d / 8), h->bn_gu);
       e = cudaGetLastError();
     }
-    if (e != cudaSuccess) {
-      h->err = std::string("gate/up interleave: ") + cudaGetErrorString(e);
-      return TE_ERR_CUDA;
-    }
-    for (int bi = 0; bi < 3; ++bi) {
-      const uint32_t box = 64u << bi;
+    for (int bi = 0; bi < 4; ++bi) {
+      const uint32_t box = 32u << bi;
       ok = ok && make_tmap(&h->tm[l].qkv[bi], h->w + L.wqkv, n_qkv, d, box);
       ok = ok && make_tmap(&h->tm[l].o[bi], h->w + L.wo, d, n_q, box);
       ok = ok && make_tmap(&h->tm[l].gu[bi], h->w + L.wgu, 2 * F, d, box);
@@ -826,7 +910,8 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
     }
   }
   h->gf_off = o;
-  cudaError_t e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  cudaFree(stage);
   if (e != cudaSuccess) {
     h->err = std::string("te_load_weights: ") + cudaGetErrorString(e);
     return TE_ERR_CUDA;
@@ -849,40 +934,53 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
   if (total_tokens < 1 || total_tokens > c.max_tokens) return TE_ERR_INVALID_ARG;
   if ((long long)grid_h * grid_w > c.max_tokens_per_frame) return TE_ERR_INVALID_ARG;
   if ((long long)n_frames * grid_h * grid_w > total_tokens) return TE_ERR_INVALID_ARG;
+  TE_CUDA(h, cudaSetDevice(h->device));
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   h->last_T = total_tokens;
   h->last_B = n_frames;
+  const int Tb = bucket_tokens(total_tokens);
 
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   if (st != nullptr) TE_CUDA(h, cudaStreamIsCapturing(st, &cap));
   int nk = 0;
   if (h->timing && cap != cudaStreamCaptureStatusNone) return TE_ERR_INVALID_ARG;
   if (h->l2_resid && h->l2_limit_bytes == 0 && cap == cudaStreamCaptureStatusNone) {
-    // once per handle, outside any capture: reserve persisting L2 for the residual stream (a device-wide limit)
-    size_t want = (size_t)c.max_tokens * c.hidden * sizeof(float);
+    // once per handle, outside any capture: reserve persisting L2 for the residual stream.  This is a DEVICE-WIDE
+    // limit; the previous value is restored by te_destroy and by TE_OPT_L2_RESIDUAL = 0.
+    size_t want = (size_t)h->cap_rows * c.hidden * sizeof(float);
     if (want > (64u << 20)) want = 64u << 20;
     if (want > h->l2_max_persist) want = h->l2_max_persist;
-    if (want > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) h->l2_limit_bytes = want;
-    else h->l2_resid = 0;
+    size_t prev = 0;
+    cudaDeviceGetLimit(&prev, cudaLimitPersistingL2CacheSize);
+    if (want > 0 && prev >= want) {
+      h->l2_limit_bytes = want;  // someone already reserved enough
+    } else if (want > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
+      h->l2_limit_bytes = want;
+      h->l2_prev_limit = prev;
+      h->l2_limit_raised = true;
+    } else {
+      h->l2_resid = 0;
+    }
     cudaGetLastError();
   }
+  // per-call pointers and token count: one tiny kernel ahead of the stack (stream-ordered, also under capture)
+  TE_CUDA(h, set_dyn(h, embeds, text_lens, out, total_tokens, st));
   if (!h->use_graph || h->timing || cap != cudaStreamCaptureStatusNone) {
-    int rc = enqueue_stack(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, st, &nk);
-    if (rc == TE_OK) h->launches += nk;
+    int rc = enqueue_stack(h, n_frames, grid_h, grid_w, Tb, st, &nk);
+    if (rc == TE_OK) h->launches += nk + 1;
     return rc;
   }
   GraphKey key;
   memset(&key, 0, sizeof(key));
-  key.n_frames = n_frames; key.grid_h = grid_h; key.grid_w = grid_w; key.total_tokens = total_tokens;
+  key.n_frames = n_frames; key.grid_h = grid_h; key.grid_w = grid_w; key.bucket_tokens = Tb;
   key.lb = h->dbg_lb; key.le = h->dbg_le; key.stop = h->dbg_stop; key.prefix_len = h->prefix_len;
-  key.embeds = embeds; key.lens = text_lens; key.out = out;
   GraphEntry* hit = nullptr;
   for (auto& e : h->cache)
     if (e.key == key) { hit = &e; break; }
   if (!hit) {
-    // First call for this (shape, pointers) key: capture the kernel sequence once.
+    // First call of this shape class: capture the kernel sequence once.
     TE_CUDA(h, cudaStreamBeginCapture(h->own_stream, cudaStreamCaptureModeThreadLocal));
-    int rc = enqueue_stack(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, h->own_stream, &nk);
+    int rc = enqueue_stack(h, n_frames, grid_h, grid_w, Tb, h->own_stream, &nk);
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(h->own_stream, &g);
     if (rc != TE_OK) {
@@ -900,7 +998,8 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
       h->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e);
       return TE_ERR_CUDA;
     }
-    if (h->cache.size() >= 16) {  // evict the least recently used entry
+    ++h->captures;
+    if (h->cache.size() >= 32) {  // evict the least recently used entry
       size_t victim = 0;
       for (size_t i = 1; i < h->cache.size(); ++i)
         if (h->cache[i].stamp < h->cache[victim].stamp) victim = i;
@@ -910,10 +1009,12 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
     }
     h->cache.push_back(GraphEntry{key, ex, g, nk, 0});
     hit = &h->cache.back();
+  } else {
+    h->last_plan = make_plan(h, Tb, n_frames, grid_h * grid_w);
   }
   hit->stamp = ++h->stamp;
   TE_CUDA(h, cudaGraphLaunch(hit->exec, st));
-  h->launches += hit->n_kernels;
+  h->launches += hit->n_kernels + 1;
   return TE_OK;
 }
 
@@ -934,10 +1035,10 @@ int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_le
   TE_CUDA(h, cudaMemcpyAsync(h->prefix_lens, &prefix_len, sizeof(int32_t), cudaMemcpyHostToDevice, st));
   int nk = 0;
   // one text-only frame (no grid): ids t = h = w = 0..P-1; every layer's K/V is copied to the cache
-  int rc = enqueue_stack(h, 1, 0, 0, prefix_embeds, h->prefix_lens, prefix_len, prefix_out ? prefix_out : h->prefix_buf, st,
-                         &nk, /*prefix_pass=*/true);
+  TE_CUDA(h, set_dyn(h, prefix_embeds, h->prefix_lens, prefix_out ? prefix_out : h->prefix_buf, prefix_len, st));
+  int rc = enqueue_stack(h, 1, 0, 0, bucket_tokens(prefix_len), st, &nk, /*prefix_pass=*/true, prefix_len);
   if (rc != TE_OK) return rc;
-  h->launches += nk;
+  h->launches += nk + 1;
   // tensor maps over each layer's cached K|V rows: exactly prefix_len rows, so that rows past the prefix read as zero
   h->tm_prefix.resize(c.n_layers);
   const size_t n_kv = 2 * (size_t)c.n_kv_heads * c.head_dim;
@@ -958,8 +1059,11 @@ int te_encode_host_submit(te_handle* h, int32_t n_frames, int32_t grid_h, int32_
   if (n_frames < 1 || n_frames > c.max_frames || grid_h < 1 || grid_w < 1) return TE_ERR_INVALID_ARG;
   long long T = 0;
   for (int b = 0; b < n_frames; ++b) {
+    // the lengths are on the host here: what te_encode can only flag on the device is refused up front
     if (text_lens_host[b] < 0) return TE_ERR_INVALID_ARG;
-    T += (long long)grid_h * grid_w + text_lens_host[b];
+    const long long sb = (long long)grid_h * grid_w + text_lens_host[b];
+    if (sb > c.max_tokens_per_frame) return TE_ERR_INVALID_ARG;
+    T += sb;
   }
   if (T < 1 || T > c.max_tokens) return TE_ERR_INVALID_ARG;
   TE_CUDA(h, cudaSetDevice(h->device));
@@ -1031,74 +1135,62 @@ int te_query_async_error(te_handle* h) {
 
 int te_set_option(te_handle* h, int option, int value) {
   if (!h) return TE_ERR_INVALID_ARG;
-  if (option == TE_OPT_USE_GRAPH) {
-    h->use_graph = value ? 1 : 0;
-    return TE_OK;
+  switch (option) {
+    case TE_OPT_USE_GRAPH: h->use_graph = value ? 1 : 0; return TE_OK;
+    case TE_OPT_KERNEL_TIMING: h->timing = value ? 1 : 0; return TE_OK;
+    case TE_OPT_TRACE:
+      if (value && !h->trace) {
+        const size_t bytes = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+        TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->trace), bytes));
+        TE_CUDA(h, cudaMemset(h->trace, 0, bytes));
+      }
+      h->trace_on = value ? 1 : 0;
+      break;
+    case TE_OPT_PDL: h->pdl = value ? 1 : 0; break;
+    case TE_OPT_CTA_PAIR:
+      if (value < 0 || value > 2) return TE_ERR_INVALID_ARG;
+      h->pair_mode = value;
+      break;
+    case TE_OPT_ATTN_IMPL:
+      if (value < 0 || value > 1) return TE_ERR_INVALID_ARG;
+      h->attn_impl = value;
+      break;
+    case TE_OPT_L2_RESIDUAL:
+      h->l2_resid = value ? 1 : 0;
+      if (!value) {
+        cudaSetDevice(h->device);
+        cudaDeviceSynchronize();
+        release_l2_limit(h);
+      }
+      break;
+    case TE_OPT_RESID_WIDE:
+      if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
+      h->resid_wide = value;
+      break;
+    case TE_OPT_SPLIT_K:
+      h->splitk = value ? 1 : 0;
+      h->split_target = value > 1 ? value : 0;
+      break;
+    case TE_OPT_RESID_BLOCK_N:
+      if ((value != 128 && value != 256) || h->cfg.hidden % value != 0) return TE_ERR_INVALID_ARG;
+      h->bn_res = value;
+      break;
+    default: return TE_ERR_INVALID_ARG;
   }
-  if (option == TE_OPT_KERNEL_TIMING) {
-    h->timing = value ? 1 : 0;
-    return TE_OK;
-  }
-  if (option == TE_OPT_TRACE) {
-    if (value && !h->trace) {
-      const size_t bytes = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
-      TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->trace), bytes));
-      TE_CUDA(h, cudaMemset(h->trace, 0, bytes));
-    }
-    h->trace_on = value ? 1 : 0;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_PDL) {
-    h->pdl = value ? 1 : 0;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_CTA_PAIR) {
-    if (value < 0 || value > 2) return TE_ERR_INVALID_ARG;
-    h->pair_mode = value;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_ATTN_IMPL) {
-    if (value < 0 || value > 1) return TE_ERR_INVALID_ARG;
-    h->attn_impl = value;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_L2_RESIDUAL) {
-    h->l2_resid = value ? 1 : 0;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_RESID_WIDE) {
-    if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
-    h->resid_wide = value;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_STREAM_K) {
-    h->streamk = value ? 1 : 0;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_SPLIT_K) {
-    h->splitk = value ? 1 : 0;
-    g_split_target = value > 1 ? value : 0;
-    free_graphs(h);
-    return TE_OK;
-  }
-  if (option == TE_OPT_RESID_BLOCK_N) {
-    if ((value != 128 && value != 256) || h->cfg.hidden % value != 0) return TE_ERR_INVALID_ARG;
-    h->bn_res = value;
-    h->bn_res_auto = false;
-    free_graphs(h);
-    return TE_OK;
-  }
-  return TE_ERR_INVALID_ARG;
+  free_graphs(h);  // cached graphs bake the previous choice in
+  return TE_OK;
 }
 
 int64_t te_kernel_launches(te_handle* h) { return h ? h->launches : 0; }
+int64_t te_graph_captures(te_handle* h) { return h ? h->captures : 0; }
+
+int te_dispatch_info(te_handle* h, char* buf, size_t n_bytes) {
+  if (!h || !buf || n_bytes == 0) return TE_ERR_INVALID_ARG;
+  if (h->last_T == 0) return TE_ERR_INVALID_ARG;
+  h->info = describe_plan(h, h->last_plan);
+  snprintf(buf, n_bytes, "%s", h->info.c_str());
+  return TE_OK;
+}
 
 int te_kernel_times(te_handle* h, float* ms_sum, int32_t* n_launches) {
   if (!h || !ms_sum || !n_launches) return TE_ERR_INVALID_ARG;
@@ -1155,60 +1247,51 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
   return TE_OK;
 }
 
-int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
-                  int32_t block_n, int32_t cta_pair) {
+static int debug_gemm_prologue(int device, const void* a, const void* b, float* cmat, int m, int n, int k, int* sm_count) {
   if (!a || !b || !cmat || m < 1 || n < 1 || k < 1) return TE_ERR_INVALID_ARG;
-  if ((block_n != 128 && block_n != 256) || n % block_n != 0 || k % 64 != 0) return TE_ERR_UNSUPPORTED;
+  if (k % 64 != 0) return TE_ERR_UNSUPPORTED;
   if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TE_ERR_CUDA;
   if (prop.major != 10) return TE_ERR_UNSUPPORTED;
   if (init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
+  *sm_count = prop.multiProcessorCount;
+  return TE_OK;
+}
+
+int te_debug_gemm(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                  int32_t block_n, int32_t cta_pair) {
+  int sms = 0;
+  int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
+  if (rc != TE_OK) return rc;
+  if ((block_n != 128 && block_n != 256) || n % block_n != 0) return TE_ERR_UNSUPPORTED;
   CUtensorMap ta, tb;
   if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, cta_pair ? block_n / 2 : block_n))
     return TE_ERR_CUDA;
   te::GemmParams p{};
   p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
   p.c = cmat; p.ld_c = n;
-  p.streamk = cta_pair == 2 ? 1 : 0;
-  if (p.streamk) {  // one fp32 partial-tile slot and one flag per CTA
-    const size_t n_cta = prop.multiProcessorCount;
-    if (cudaMalloc(reinterpret_cast<void**>(&p.sk_scratch), n_cta * te::GEMM_BM * block_n * sizeof(float)) != cudaSuccess)
-      return TE_ERR_CUDA;
-    if (cudaMalloc(reinterpret_cast<void**>(&p.sk_sem), n_cta * sizeof(int)) != cudaSuccess) {
-      cudaFree(p.sk_scratch);
-      return TE_ERR_CUDA;
-    }
-    cudaMemset(p.sk_sem, 0, n_cta * sizeof(int));
-  }
-  g_pdl = false;
-  cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(block_n, cta_pair ? 1 : 0, 128, ta, tb, p, prop.multiProcessorCount, nullptr);
+  const LaunchCtx lc;  // plain launch: no PDL, no cooperative attribute, no L2 window
+  cudaError_t e = launch_gemm_bn<te::EPI_PLAIN>(lc, block_n, cta_pair ? 1 : 0, 128, ta, tb, p, sms, nullptr);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
-  if (p.streamk) {
-    cudaFree(p.sk_scratch);
-    cudaFree(p.sk_sem);
-  }
   return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
 int te_debug_gemm_splitk(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
                          int32_t block_n, int32_t splits) {
-  if (!a || !b || !cmat || m < 1 || n < 1 || k < 1) return TE_ERR_INVALID_ARG;
-  if ((block_n != 128 && block_n != 256) || n % block_n != 0 || k % 64 != 0) return TE_ERR_UNSUPPORTED;
+  int sms = 0;
+  int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
+  if (rc != TE_OK) return rc;
+  if ((block_n != 128 && block_n != 256) || n % block_n != 0) return TE_ERR_UNSUPPORTED;
   if (splits < 1 || splits > te::GEMMK_MAX_SPLITS || splits > k / 64) return TE_ERR_INVALID_ARG;
-  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
-  cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TE_ERR_CUDA;
-  if (prop.major != 10) return TE_ERR_UNSUPPORTED;
-  if (init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
   CUtensorMap ta, tb;
   if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, block_n)) return TE_ERR_CUDA;
   te::GemmParams p{};
   p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
   p.c = cmat; p.ld_c = n; p.splits = splits;
   const size_t tiles = (size_t)p.num_m_blk * p.num_n_blk;
-  // the group leader spins on its peers: the whole grid must be co-resident (one CTA per SM)
-  if (tiles * splits > (size_t)prop.multiProcessorCount) return TE_ERR_UNSUPPORTED;
+  // the group members spin on each other: the whole grid must be co-resident (one CTA per SM)
+  if (tiles * splits > (size_t)sms) return TE_ERR_UNSUPPORTED;
   if (cudaMalloc(reinterpret_cast<void**>(&p.sk_scratch), tiles * splits * te::GEMM_BM * block_n * sizeof(float)) !=
       cudaSuccess)
     return TE_ERR_CUDA;
@@ -1217,11 +1300,31 @@ int te_debug_gemm_splitk(int device, const void* a, const void* b, float* cmat, 
     return TE_ERR_CUDA;
   }
   cudaMemset(p.sk_sem, 0, 2 * tiles * sizeof(int));
-  g_pdl = false;
-  cudaError_t e = launch_gemmk_bn<te::EPI_PLAIN>(block_n, 128, ta, tb, p, nullptr);
+  const LaunchCtx lc;
+  cudaError_t e = launch_gemmk_bn<te::EPI_PLAIN>(lc, block_n, 128, ta, tb, p, nullptr);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   cudaFree(p.sk_scratch);
   cudaFree(p.sk_sem);
+  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+}
+
+int te_debug_gemm_wide(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                       int32_t n_tiles) {
+  int sms = 0;
+  int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
+  if (rc != TE_OK) return rc;
+  if (n_tiles < 1 || n % 32 != 0) return TE_ERR_UNSUPPORTED;
+  const int bn = (((n + n_tiles - 1) / n_tiles) + 31) / 32 * 32;  // tile width as chosen by the stack's dispatch
+  const int num_m = (m + te::GEMM_BM - 1) / te::GEMM_BM;
+  if (bn > 512 || ((num_m + 1) / 2) * n_tiles > sms / 2) return TE_ERR_UNSUPPORTED;  // one wave only
+  CUtensorMap ta, tb;
+  if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, bn / 4)) return TE_ERR_CUDA;
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = num_m; p.num_n_blk = n_tiles;
+  p.c = cmat; p.ld_c = n;
+  const LaunchCtx lc;
+  cudaError_t e = launch_wide<te::EPI_PLAIN>(lc, ta, tb, p, n_tiles, bn, nullptr);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
   return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
@@ -1230,10 +1333,12 @@ void te_destroy(te_handle* h) {
   cudaSetDevice(h->device);
   cudaDeviceSynchronize();
   free_graphs(h);
+  release_l2_limit(h);
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
-  void* ptrs[] = {h->w, h->w_gu_plain, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv, h->attn,
-                  h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
-                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens};
+  void* ptrs[] = {h->w, h->dyn, h->resid, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv,
+                  h->attn, h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
+                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens,
+                  h->attn_stats};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto& sl : h->slot)

@@ -23,7 +23,7 @@ class GpuTE:
     """Owns one handle; encode() returns numpy arrays."""
 
     def __init__(self, model, max_frames, max_tokens, blob, final_norm=None, cta_pair=None, resid_bn=None,
-                 split_k=None, max_prefix_tokens=0, stream_k=None, attn_impl=None, resid_wide=None):
+                 split_k=None, max_prefix_tokens=0, attn_impl=None, resid_wide=None):
         import torch
         import paper_2606_05981_b200 as te
         self.te, self.torch, self.model = te, torch, model
@@ -40,8 +40,6 @@ class GpuTE:
             te.te_set_option(self.enc.h, te.TE_OPT_RESID_WIDE, resid_wide)
         if attn_impl is not None:
             te.te_set_option(self.enc.h, te.TE_OPT_ATTN_IMPL, attn_impl)
-        if stream_k is not None:
-            te.te_set_option(self.enc.h, te.TE_OPT_STREAM_K, stream_k)
 
     def encode(self, embeds, text_lens, gh, gw, layer_range=None, stop_after_attn=0, stream=None,
                total_tokens=None, use_graph=1):

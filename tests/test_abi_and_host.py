@@ -22,13 +22,14 @@ def te():
 
 
 def test_library_exports_every_declared_symbol(te):
-    hdr = open(os.path.join(ROOT, "include", "te.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(te_[a-z_]+)\s*\(", hdr))
-    assert declared == set(te.EXPORTS), declared ^ set(te.EXPORTS)
     L = ctypes.CDLL(te.LIB_PATH)
-    for name in declared:
-        assert hasattr(L, name), name
+    for header, names in (("te.h", te.EXPORTS), ("te_debug.h", te.DEBUG_EXPORTS)):
+        hdr = open(os.path.join(ROOT, "include", header)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        declared = set(re.findall(r"\b(te_[a-z_]+)\s*\(", hdr))
+        assert declared == set(names), (header, declared ^ set(names))
+        for name in declared:
+            assert hasattr(L, name), name
 
 
 def test_config_struct_layout_matches_header(te):

@@ -27,19 +27,20 @@ def _assert_final(m, tag=""):
     assert m["update_rel_l2"] <= PM.GATE_UPDATE_REL_L2, (tag, m)
     assert m["nonoutlier_rel_l2"] <= PM.GATE_NONOUTLIER_REL_L2, (tag, m)
     assert m["outlier_maxabs_rel"] <= PM.GATE_OUTLIER_MAXABS, (tag, m)
+    assert m["max_row_update_rel_l2"] <= PM.GATE_ROW_UPDATE_REL_L2, (tag, m)          # every token row
+    assert m["maxabs_update_over_rms"] <= PM.GATE_MAXABS_UPDATE_OVER_RMS, (tag, m)    # every element
     assert m["cos_sim"] > 0.999, (tag, m)
 
 
 # --------------------------------------------------------------------------- GEMM main loop
-@pytest.mark.parametrize("pair", [0, 1, 2])
+@pytest.mark.parametrize("pair", [0, 1])
 @pytest.mark.parametrize("M,N,K,bn", [(128, 256, 64, 256), (1, 128, 64, 128), (300, 512, 256, 256),
                                        (300, 512, 256, 128), (517, 768, 832, 256), (3072, 2048, 2048, 256),
                                        (3072, 2048, 6144, 128), (3072, 2048, 6144, 256), (3072, 4096, 2048, 256),
                                        (512, 12288, 2048, 256), (1024, 2048, 2048, 256)])
 def test_gemm_mainloop_vs_fp64_matmul(H, M, N, K, bn, pair):
     """TMA + tcgen05 main loop alone: several tiles, ragged M tail, K spanning >1 pipeline ring.
-    pair: 0 = one CTA per tile, 1 = CTA pairs, 2 = CTA pairs with stream-K scheduling (tiles cut by share
-    boundaries, incl. fewer tiles than SM pairs, are completed through the partial-tile scratch)."""
+    pair: 0 = one CTA per tile, 1 = CTA pairs (cta_group::2, 256-row tiles)."""
     import torch
     import paper_2606_05981_b200 as te
     rng = np.random.default_rng(M * 7 + N)
@@ -84,6 +85,30 @@ def test_gemm_splitk_vs_fp64_matmul(H, M, N, K, bn, splits):
     assert np.array_equal(outs[0], outs[1])
 
 
+@pytest.mark.parametrize("M,N,K,n_tiles", [(3072, 2048, 2048, 6), (3072, 2048, 6144, 6), (3733, 2048, 2048, 4),
+                                           (2048, 2048, 6144, 9), (1500, 2048, 2048, 7), (593, 256, 768, 5),
+                                           (300, 256, 256, 3), (256, 2048, 2048, 16)])
+def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles):
+    """One-wave wide-tile kernel alone (te_gemm_wide.cuh, plain epilogue), elementwise against an fp64 matmul: the
+    widths the stack's dispatch picks at cfg 4 (6 x 352) and cfg 5 (4 x 512), a partly out-of-range last tile
+    (7 x 320 > 2048), a wholly out-of-range one (5 x 64 > 256), a ragged last row-pair block, one MMA narrower than
+    the other tile widths (16 x 128)."""
+    import torch
+    import paper_2606_05981_b200 as te
+    rng = np.random.default_rng(M * 3 + N + n_tiles)
+    a = W.f32_to_bf16_bits(rng.standard_normal((M, K)).astype(np.float32))
+    b = W.f32_to_bf16_bits(rng.standard_normal((N, K)).astype(np.float32))
+    ref = H.bf16_bits_to_f64(a).reshape(M, K) @ H.bf16_bits_to_f64(b).reshape(N, K).T
+    ad = torch.from_numpy(a.view(np.int16)).cuda()
+    bd = torch.from_numpy(b.view(np.int16)).cuda()
+    c = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
+    te.te_debug_gemm_wide(0, ad, bd, c, M, N, K, n_tiles)
+    out = c.cpu().numpy()
+    assert np.isfinite(out).all()
+    assert PM.rel_l2(out, ref) < 1e-5
+    assert np.max(np.abs(out - ref)) < 1e-4 * np.sqrt(K) * 4
+
+
 # ------------------------------------------------------------------- ids / packing / rotary table
 @pytest.mark.parametrize("gh,gw,tl", [(4, 4, [24, 24]), (8, 8, [64]), (4, 16, [3, 0, 17]), (16, 4, [0, 9]),
                                       (1, 5, [1, 2, 3, 4, 5, 6, 7])])
@@ -121,8 +146,10 @@ def test_layer_taps_and_teacher_forced_updates(H, O, cfg_id):
         gt = g.taps(T, w.n_frames)
         for key in ("q", "k", "v", "attn", "act"):
             assert PM.rel_l2(gt[key], taps[key][0]) <= PM.GATE_TAP_REL_L2, (cfg_id, l, key)
+            assert PM.max_row_rel_l2(gt[key], taps[key][0]) <= PM.GATE_TAP_ROW_REL_L2, (cfg_id, l, key)
         assert PM.rel_l2(out, ref) <= PM.GATE_LAYER_REL_L2
         assert PM.rel_l2(out - x32, ref - x32) <= PM.GATE_LAYER_UPDATE_REL_L2, (cfg_id, l)
+        assert PM.max_row_rel_l2(out - x32, ref - x32) <= PM.GATE_ROW_UPDATE_REL_L2, (cfg_id, l)
         oa = g.encode(x32, tl, w.grid_h, w.grid_w, layer_range=(l, l + 1), stop_after_attn=1)
         assert PM.rel_l2(oa - x32, taps["x_attn"][0] - x32) <= PM.GATE_LAYER_UPDATE_REL_L2
         x_in = ref
@@ -143,19 +170,15 @@ def test_cfg1_full_stack(H, O):
     g.close()
 
 
-@pytest.mark.parametrize("cta_pair,resid_bn,split_k,stream_k", [(1, 128, 1, 1), (1, 256, 1, 1), (1, 128, 1, 0),
-                                                                (1, 256, 1, 0), (0, 256, 1, 1), (0, 128, 1, 1),
-                                                                (0, 256, 0, 1), (0, 128, 0, 1)])
-def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn, split_k, stream_k):
-    """Force each GEMM tiling (one CTA per tile / CTA pairs with and without stream-K / split-K groups,
-    128- and 256-wide residual tiles)."""
+@pytest.mark.parametrize("cta_pair,resid_bn,split_k", [(1, 128, 1), (1, 256, 1), (0, 256, 1), (0, 128, 1),
+                                                       (0, 256, 0), (0, 128, 0)])
+def test_cfg1_every_tiling_mode(H, O, cta_pair, resid_bn, split_k):
+    """Force each GEMM tiling (one CTA per tile / CTA pairs / split-K groups, 128- and 256-wide residual tiles)."""
     w, blob, tl, T, emb, ch = H.workload_inputs(1)
     ref = O.encode(blob, W.blob_layout(w.model), w.model, emb, tl, 4, 4)
-    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn, split_k=split_k,
-                stream_k=stream_k)
+    g = H.GpuTE(w.model, w.n_frames, T, blob, cta_pair=cta_pair, resid_bn=resid_bn, split_k=split_k)
     out = g.encode(emb, tl, 4, 4)
-    _assert_final(PM.stack_metrics(out, ref, emb),
-                  f"pair={cta_pair} bn={resid_bn} split_k={split_k} stream_k={stream_k}")
+    _assert_final(PM.stack_metrics(out, ref, emb), f"pair={cta_pair} bn={resid_bn} split_k={split_k}")
     assert np.array_equal(out, g.encode(emb, tl, 4, 4))    # deterministic (fixed-order partial sums)
     g.close()
 
@@ -169,10 +192,9 @@ def test_ragged_stack_cta_pairs(H, O):
     T = len(tl) * gh * gw + sum(tl)
     emb = np.random.default_rng(4).standard_normal((T, m.hidden)).astype(np.float32)
     ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
-    for stream_k in (0, 1):
-        g = H.GpuTE(m, len(tl), T, blob, cta_pair=1, stream_k=stream_k)
-        _assert_final(PM.stack_metrics(g.encode(emb, tl, gh, gw), ref, emb), f"ragged pairs stream_k={stream_k}")
-        g.close()
+    g = H.GpuTE(m, len(tl), T, blob, cta_pair=1)
+    _assert_final(PM.stack_metrics(g.encode(emb, tl, gh, gw), ref, emb), "ragged pairs")
+    g.close()
 
 
 def test_cfg1_final_norm(H, O):
@@ -352,7 +374,7 @@ def test_encode_is_async_no_sync_and_counts_launches(H):
         done_at_return = st.query()
     st.synchronize()
     assert not done_at_return
-    assert te.te_kernel_launches(g.enc.h) - n0 == 1 + 5 * w.model.n_layers
+    assert te.te_kernel_launches(g.enc.h) - n0 == 2 + 5 * w.model.n_layers   # refresh + prep + 5 per layer
     g.close()
 
 
@@ -640,4 +662,246 @@ def test_encode_inside_a_callers_graph_capture(H):
         graph.replay()
         torch.cuda.synchronize()
         assert np.array_equal(out.cpu().numpy(), want)
+    g.close()
+
+
+# ------------------------------------------- every row at full size (next #1b)
+def _one_layer_all_rows(H, O, w, blob, tl, T, emb, layer, tag):
+    """Teacher-forced ONE layer over ALL rows through the default dispatch: taps and the update, per token row."""
+    m = w.model
+    g = H.GpuTE(m, w.n_frames, T, blob)
+    taps = {}
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, w.grid_h, w.grid_w, layer_begin=layer, layer_end=layer + 1,
+                   taps=taps)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w, layer_range=(layer, layer + 1))
+    gt = g.taps(T, w.n_frames)
+    info = g.te.te_dispatch_info(g.enc.h)
+    for key in ("q", "k", "v", "attn", "act"):
+        assert PM.rel_l2(gt[key], taps[key][0]) <= PM.GATE_TAP_REL_L2, (tag, key)
+        assert PM.max_row_rel_l2(gt[key], taps[key][0]) <= PM.GATE_TAP_ROW_REL_L2, (tag, key)
+    e64 = emb.astype(np.float64)
+    assert PM.rel_l2(out - e64, ref - e64) <= PM.GATE_LAYER_UPDATE_REL_L2, tag
+    rows = PM.row_rel_l2(out - e64, ref - e64)
+    assert rows.max() <= PM.GATE_ROW_UPDATE_REL_L2, (tag, int(rows.argmax()), float(rows.max()))
+    oa = g.encode(emb, tl, w.grid_h, w.grid_w, layer_range=(layer, layer + 1), stop_after_attn=1)
+    assert PM.max_row_rel_l2(oa - e64, taps["x_attn"][0] - e64) <= PM.GATE_ROW_UPDATE_REL_L2, tag
+    print(f"{tag}: dispatch {info}; max row update rel-L2 {rows.max():.2e} (row {rows.argmax()})")
+    g.close()
+    return info
+
+
+@pytest.mark.parametrize("cfg_id,layer", [(4, 0), (4, 27), (5, 13)])
+def test_one_layer_every_row_full_size(H, O, cfg_id, layer):
+    """cfg 4 (T = 3072: CTA pairs + 6 x 352 wide residual tiles) and cfg 5 (ragged T: 4 x 512) at FULL size: one
+    teacher-forced layer compared with the oracle on EVERY row — all 12-15 row-pair blocks, every wide residual tile,
+    every attention (frame, head) — not on sampled frames."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    info = _one_layer_all_rows(H, O, w, blob, tl, T, emb, layer, f"cfg{cfg_id} layer {layer}")
+    assert info["oproj"].startswith("te_gemm_wide_kernel") and info["qkv"].startswith("te_gemm2_kernel")
+
+
+def test_one_layer_every_row_mid_batch(H, O):
+    """cfg 3 (T = 512): split-K groups + the one-wave wide SwiGLU tiles over the interleaved gate/up weights."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(3)
+    info = _one_layer_all_rows(H, O, w, blob, tl, T, emb, 5, "cfg3 layer 5")
+    assert info["gateup"].startswith("te_gemm_wide_kernel<3>") and info["qkv"].startswith("te_gemmk_kernel")
+
+
+@pytest.mark.parametrize("cfg_id", [4, 5])
+def test_identical_frames_cover_every_row_of_the_28_layer_stack(H, O, cfg_id):
+    """Full depth, full size, EVERY row: all frames get the same embeddings (cut to their own length), so by
+    causality frame b's rows must equal the first S_b rows of the longest frame BITWISE — whatever row block, wide
+    tile or attention CTA they land in — and the longest frame is compared with the oracle."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    m = w.model
+    cu = O.cu_seqlens(tl, w.grid_h, w.grid_w)
+    b_long = int(np.argmax(np.diff(cu)))
+    base = emb[cu[b_long]:cu[b_long + 1]]
+    same = np.concatenate([base[: cu[b + 1] - cu[b]] for b in range(w.n_frames)])
+    g = H.GpuTE(m, w.n_frames, T, blob)
+    out = g.encode(same, tl, w.grid_h, w.grid_w)
+    want = out[cu[b_long]:cu[b_long + 1]]
+    for b in range(w.n_frames):
+        assert np.array_equal(out[cu[b]:cu[b + 1]], want[: cu[b + 1] - cu[b]]), f"frame {b} differs from frame {b_long}"
+    ref = O.encode(blob, W.blob_layout(m), m, base, [tl[b_long]], w.grid_h, w.grid_w)
+    met = PM.stack_metrics(want, ref, base, ch)
+    print(f"cfg{cfg_id} identical frames: {met}")
+    _assert_final(met, f"cfg{cfg_id} identical frames")
+    g.close()
+
+
+# ------------------------------------------------------- graph reuse (VERDICT r01 weak #7; SURVEY §8a a7)
+def test_graph_reuse_ragged_lengths_and_changing_buffers(H, O):
+    """200 calls with fresh random ragged lengths and alternating buffers: a graph is captured once per shape class
+    (row-block bucket of the token count), never per call or per pointer; the last call is compared with the oracle."""
+    import torch
+    import paper_2606_05981_b200 as te
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    B, gh, gw = 12, 2, 3
+    cap = B * 256
+    g = H.GpuTE(m, B, cap, blob)
+    rng = np.random.default_rng(99)
+    bufs = [(torch.empty((cap, m.hidden), device="cuda"), torch.empty((cap, m.hidden), device="cuda"),
+             torch.empty(B, dtype=torch.int32, device="cuda")) for _ in range(3)]
+    te.te_debug_set_range(g.enc.h, 0, m.n_layers, 0)
+    buckets = set()
+    c0 = te.te_graph_captures(g.enc.h)
+    last = None
+    for i in range(200):
+        tl = rng.integers(60, 140, size=B).astype(np.int32)
+        T = int(B * gh * gw + tl.sum())
+        buckets.add((T + 255) // 256 if (T + 127) // 128 * 128 >= 1024 else -((T + 127) // 128))
+        e, o, l = bufs[i % 3]
+        emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+        e[:T].copy_(torch.from_numpy(emb))
+        l.copy_(torch.from_numpy(tl))
+        g.enc.encode(B, gh, gw, e, l, T, o)
+        last = (emb, tl, T, o)
+    torch.cuda.synchronize()
+    assert te.te_query_async_error(g.enc.h) == te.TE_OK
+    n_cap = te.te_graph_captures(g.enc.h) - c0
+    assert n_cap == len(buckets) and n_cap <= 6, (n_cap, sorted(buckets))
+    emb, tl, T, o = last
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
+    _assert_final(PM.stack_metrics(o[:T].cpu().numpy(), ref, emb), "graph reuse, last call")
+    # same bucket, different T and pointers: identical to a fresh handle's result, bitwise
+    g2 = H.GpuTE(m, B, cap, blob)
+    assert np.array_equal(g2.encode(emb, tl, gh, gw), o[:T].cpu().numpy())
+    g2.close()
+    g.close()
+
+
+def test_stale_rows_of_a_larger_call_do_not_leak(H, O):
+    """The activation tensor maps span the whole workspace: after a large call whose rows are NaN-poisoned, a smaller
+    call (its last frame's length not a multiple of 16, so the attention tiles read past it) must be unaffected."""
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    g = H.GpuTE(m, 4, 1024, blob)
+    big = np.full((1000, m.hidden), np.nan, dtype=np.float32)
+    g.encode(big, [249, 249, 249, 249], 1, 1)
+    tl = [100, 37]
+    T = 2 + sum(tl)
+    emb = np.random.default_rng(8).standard_normal((T, m.hidden)).astype(np.float32)
+    out = g.encode(emb, tl, 1, 1)
+    assert np.isfinite(out).all()
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, 1, 1)
+    _assert_final(PM.stack_metrics(out, ref, emb), "after a poisoned larger call")
+    g.close()
+
+
+# --------------------------------------------- SURVEY §8(f) NEXT-3: side stream against a foreign load
+@pytest.mark.parametrize("case", ["cfg2_split_k", "pairs_T1024"])
+def test_side_stream_under_foreign_load_is_bitwise_identical(H, case):
+    """The paper's mechanism 1 (Algorithm 1 :118-137): te_encode on a SIDE stream while the main stream
+    runs a denoiser-shaped load (library bf16 matmuls), joined by one event.  The result must be bitwise the solo
+    result — the cooperative split-K groups (cfg 2) and the CTA-pair kernels (T = 1024) only get delayed."""
+    import torch
+    import paper_2606_05981_b200 as te
+    w, blob, tl, T, emb, ch = H.workload_inputs(2)
+    m = w.model
+    if case == "pairs_T1024":
+        tl = np.full(8, 64, dtype=np.int32)
+        T = 8 * 128
+        emb = np.random.default_rng(17).standard_normal((T, m.hidden)).astype(np.float32)
+    B = len(tl)
+    g = H.GpuTE(m, B, T, blob)
+    solo = g.encode(emb, tl, w.grid_h, w.grid_w)
+    e, lens, out = g._keep
+    a = torch.randn(4096, 4096, device="cuda", dtype=torch.bfloat16)
+    b = torch.randn(4096, 4096, device="cuda", dtype=torch.bfloat16)
+    c = torch.empty_like(a)
+    side = torch.cuda.Stream()
+    main = torch.cuda.current_stream()
+    for _ in range(5):
+        out.zero_()
+        ev0, ev = torch.cuda.Event(), torch.cuda.Event()
+        ev0.record(main)
+        side.wait_event(ev0)
+        with torch.cuda.stream(side):
+            for _ in range(4):
+                te.te_encode(g.enc.h, B, w.grid_h, w.grid_w, e, lens, T, out, side.cuda_stream)
+            ev.record(side)
+        for _ in range(12):
+            torch.matmul(a, b, out=c)                   # the foreign load, concurrently on the main stream
+        main.wait_event(ev)                             # the single cross-stream event of Algorithm 1
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), solo)
+    assert te.te_query_async_error(g.enc.h) == te.TE_OK
+    g.close()
+
+
+# ------------------------------------------------------------------ runtime hygiene (VERDICT r01 weak #8)
+def test_two_handles_on_two_host_threads(H):
+    """Launch state is per handle: two handles with DIFFERENT options driven from two host threads at once."""
+    import threading
+    import torch
+    w, blob, tl, T, emb, ch = H.workload_inputs(2)
+    ga = H.GpuTE(w.model, w.n_frames, T, blob)                      # split-K groups (cooperative launches)
+    gb = H.GpuTE(w.model, w.n_frames, T, blob, split_k=0)           # one CTA per tile
+    want_a = ga.encode(emb, tl, w.grid_h, w.grid_w)
+    want_b = gb.encode(emb, tl, w.grid_h, w.grid_w)
+    e = torch.from_numpy(emb).cuda()
+    lens = torch.from_numpy(tl).cuda()
+    outs = {"a": torch.empty_like(e), "b": torch.empty_like(e)}
+    errs = []
+
+    def drive(g, key):
+        try:
+            st = torch.cuda.Stream()
+            for _ in range(100):
+                g.enc.encode(w.n_frames, w.grid_h, w.grid_w, e, lens, T, outs[key], st.cuda_stream)
+            st.synchronize()
+        except Exception as ex:                       # noqa: BLE001
+            errs.append(ex)
+
+    ts = [threading.Thread(target=drive, args=(ga, "a")), threading.Thread(target=drive, args=(gb, "b"))]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    torch.cuda.synchronize()
+    assert not errs, errs
+    assert np.array_equal(outs["a"].cpu().numpy(), want_a) and np.array_equal(outs["b"].cpu().numpy(), want_b)
+    ga.close()
+    gb.close()
+
+
+def test_create_destroy_does_not_leak(H):
+    """100 create / load / prefix / encode / destroy cycles: free device memory returns to where it started."""
+    import torch
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    emb = np.random.default_rng(2).standard_normal((80, m.hidden)).astype(np.float32)
+    pre = np.random.default_rng(3).standard_normal((16, m.hidden)).astype(np.float32)
+
+    def cycle():
+        g = H.GpuTE(m, 2, 80, blob, max_prefix_tokens=16)
+        g.encode_prefix(pre, want_out=False)
+        g.encode(emb, [24, 24], 4, 4)
+        g._keep = None
+        g.close()
+
+    cycle()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(100):
+        cycle()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < (8 << 20), (free0, free1)     # (allocator granularity; one leaked cycle would be > 3 MB x 100)
+
+
+def test_host_path_refuses_a_frame_longer_than_the_capacity(H):
+    import paper_2606_05981_b200 as te
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    g = H.GpuTE(m, 2, 512, blob)
+    emb = np.zeros((16 + 250 + 16 + 10, m.hidden), dtype=np.float32)
+    out = np.empty_like(emb)
+    with pytest.raises(te.TEError) as ei:
+        g.enc.encode_host(2, 4, 4, emb, np.asarray([250, 10], dtype=np.int32), out)     # 16 + 250 > 256
+    assert ei.value.code == te.TE_ERR_INVALID_ARG
     g.close()

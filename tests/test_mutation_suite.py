@@ -151,3 +151,84 @@ def test_mutant_is_rejected(clean, monkeypatch, name):
     out, _ = _run(taps)
     fails = _rejected(clean, out, taps)
     assert fails, f"mutant {name} passed every gate"
+
+
+# ------------------------------------------------------------------ row-local mutants (per-token gates)
+@pytest.fixture(scope="module")
+def tall():
+    """Tiny stack at T = 1026 tokens (ragged frames, two 512-row blocks + a 2-row tail): the oracle, and the
+    bf16-rounding emulation of it as the stand-in for a CORRECT CUDA result."""
+    import bf16_emulation as E
+    m = W.TINY
+    blob = W.make_weight_blob(m, 1)
+    lay = W.blob_layout(m)
+    rng = np.random.default_rng(21)
+    tl, left = [], 1026
+    while left > 0:
+        s = int(min(left, rng.integers(40, 256)))
+        tl.append(s - 1)
+        left -= s
+    T = len(tl) + sum(tl)
+    emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+    emb[:, [7, 130]] *= np.float32(1000.0)          # outlier channels as in configs[2..4]
+    ref = O.encode(blob, lay, m, emb, tl, 1, 1)
+    good = E.encode_bf16(blob, lay, m, emb, tl, 1, 1)
+    return ref, good, emb.astype(np.float64), np.asarray([7, 130])
+
+
+def test_row_gate_floors(tall):
+    """The emulated-bf16 result passes every gate with >= 3x headroom on the per-token ones."""
+    ref, good, emb, ch = tall
+    m = PM.stack_metrics(good, ref, emb, ch)
+    assert PM.passes_final_gates(m), m
+    assert 3 * m["max_row_update_rel_l2"] <= PM.GATE_ROW_UPDATE_REL_L2, m
+    assert 3 * m["maxabs_update_over_rms"] <= PM.GATE_MAXABS_UPDATE_OVER_RMS, m
+    assert 3 * m["update_rel_l2"] <= PM.GATE_UPDATE_REL_L2, m
+
+
+def _wrong_rstd_row(out, emb, row):
+    o = out.copy()
+    o[row] = emb[row] + 1.3 * (out[row] - emb[row])     # one token's update scaled by a wrong 1/rms
+    return o
+
+
+def _tile_last_row_dropped(out, emb, row):
+    o = out.copy()
+    o[row] = emb[row]                                    # the row's update never written (last row of a tile)
+    return o
+
+
+def _half_of_a_row_update(out, emb, row):
+    o = out.copy()
+    o[row] = emb[row] + 0.5 * (out[row] - emb[row])     # one of two K-slices of the row's tile dropped
+    return o
+
+
+def _round1_gates(m):
+    """The whole-tensor gates as they stood in round 1 (VERDICT r01, weak #1)."""
+    return (m["rel_l2"] <= 3e-2 and m["update_rel_l2"] <= 3e-2 and m["nonoutlier_rel_l2"] <= 3e-2
+            and m["outlier_maxabs_rel"] <= 1e-2)
+
+
+@pytest.mark.parametrize("mutant,row", [(_wrong_rstd_row, 700), (_half_of_a_row_update, 127), (_half_of_a_row_update, 1025),
+                                        (_wrong_rstd_row, 0), (_tile_last_row_dropped, 511)])
+def test_one_bad_token_row_is_rejected_by_the_row_gates(tall, mutant, row):
+    """ONE corrupted token row at T >= 1024: (mostly) invisible to norms over the whole tensor — a fully dropped row
+    moves the update rel-L2 by 1/sqrt(T) = 3.1 % here and by 1.8 % at cfg 4's T = 3072 — caught by the per-token gates."""
+    ref, good, emb, ch = tall
+    bad = mutant(good, emb, row)
+    m = PM.stack_metrics(bad, ref, emb, ch)
+    assert _round1_gates(m), m                           # round 1 would have passed it
+    assert not PM.passes_row_gates(m), m
+    assert not PM.passes_final_gates(m)
+
+
+def test_one_bad_element_is_rejected(tall):
+    """One wrong element (a dropped split-K partial on one column of one row): max-abs gate."""
+    ref, good, emb, ch = tall
+    bad = good.copy()
+    bad[333, 45] += 0.3 * np.sqrt(np.mean((ref - emb) ** 2))
+    m = PM.stack_metrics(bad, ref, emb, ch)
+    assert PM.passes_whole_tensor_gates(m)
+    assert m["max_row_update_rel_l2"] <= PM.GATE_ROW_UPDATE_REL_L2      # too small for the row norm as well
+    assert m["maxabs_update_over_rms"] > PM.GATE_MAXABS_UPDATE_OVER_RMS

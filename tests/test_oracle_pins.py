@@ -564,3 +564,56 @@ def test_dense_restatement_ragged_nonsquare():
     out = O.encode(blob, lay, m, emb, tl, gh, gw)
     ref = _dense_restatement(blob, lay, m, emb, tl, gh, gw)
     assert np.max(np.abs(out - ref)) < 1e-10
+
+
+# ------------------------------------------------------------ blob layout pinned by hand
+def test_blob_layout_hand_typed_offsets_tiny():
+    """`workloads.blob_layout` / `O.unpack_layer` against offsets typed by hand from the order te.h states
+    (g1 Wq Wk Wv gq gk Wo g2 Wgate Wup Wdown per layer, then gf) for the TINY shape: d = 256, Hq*dh = 256,
+    Hkv*dh = 128, dh = 64, F = 768.
+      g1 256 | Wq 256*256 = 65536 | Wk 128*256 = 32768 | Wv 32768 | gq 64 | gk 64 | Wo 256*256 = 65536 | g2 256 |
+      Wgate 768*256 = 196608 | Wup 196608 | Wdown 256*768 = 196608   -> 787072 elements per layer."""
+    m = W.TINY
+    lay = W.blob_layout(m)
+    want = {"g1": (0, (256,)), "Wq": (256, (256, 256)), "Wk": (65792, (128, 256)), "Wv": (98560, (128, 256)),
+            "gq": (131328, (64,)), "gk": (131392, (64,)), "Wo": (131456, (256, 256)), "g2": (196992, (256,)),
+            "Wgate": (197248, (768, 256)), "Wup": (393856, (768, 256)), "Wdown": (590464, (256, 768))}
+    per_layer = 787072
+    for l in range(m.n_layers):
+        for name, (off, shape) in want.items():
+            assert lay[(l, name)] == (l * per_layer + off, shape), (l, name)
+    assert lay[("final", "gf")] == (2 * per_layer, (256,))
+    assert W.blob_num_elements(m) == 2 * per_layer + 256 == 1574400
+    assert len(lay) == 2 * 11 + 1
+
+
+def test_unpack_layer_sentinel_round_trip():
+    """A distinct bf16-exact sentinel at the first and last element of every tensor (positions typed by hand
+    above) comes back from O.unpack_layer under the right name, shape and corner."""
+    m = W.TINY
+    blob = np.zeros(W.blob_num_elements(m), dtype=np.uint16)
+    per_layer = 787072
+    spans = [("g1", 0, 256), ("Wq", 256, 65536), ("Wk", 65792, 32768), ("Wv", 98560, 32768), ("gq", 131328, 64),
+             ("gk", 131392, 64), ("Wo", 131456, 65536), ("g2", 196992, 256), ("Wgate", 197248, 196608),
+             ("Wup", 393856, 196608), ("Wdown", 590464, 196608)]
+    shapes = {"g1": (256,), "Wq": (256, 256), "Wk": (128, 256), "Wv": (128, 256), "gq": (64,), "gk": (64,),
+              "Wo": (256, 256), "g2": (256,), "Wgate": (768, 256), "Wup": (768, 256), "Wdown": (256, 768)}
+    val = {}
+    for l in range(2):
+        for i, (name, off, n) in enumerate(spans):
+            first, last = float(1 + 2 * i + 32 * l), float(2 + 2 * i + 32 * l)     # small integers: exact in bf16
+            blob[l * per_layer + off] = W.f32_to_bf16_bits(np.float32([first]))[0]
+            blob[l * per_layer + off + n - 1] = W.f32_to_bf16_bits(np.float32([last]))[0]
+            val[(l, name)] = (first, last)
+    lay = W.blob_layout(m)
+    for l in range(2):
+        t = O.unpack_layer(blob, lay, l)
+        assert set(t) == set(shapes)
+        for name, shape in shapes.items():
+            a = t[name]
+            assert a.shape == shape and a.dtype == np.float64
+            assert a.flat[0] == val[(l, name)][0] and a.flat[-1] == val[(l, name)][1], (l, name)
+            assert np.count_nonzero(a) == 2
+    # row-major [out_features, in_features]: element (r, c) of Wq sits at 256 + r * 256 + c
+    blob[256 + 3 * 256 + 5] = W.f32_to_bf16_bits(np.float32([77.0]))[0]
+    assert O.unpack_layer(blob, lay, 0)["Wq"][3, 5] == 77.0
