@@ -63,6 +63,12 @@ typedef struct te_config {
                                    pairs; 1: pairs are dealt round-robin t,h,w,t,h,w,... to the axes that
                                    still have pairs left                      */
   int32_t max_prefix_tokens;    /* capacity of the shared text prefix (te_encode_prefix); 0 = none   */
+  int32_t weight_dtype;         /* 0 (default): bf16 weights and GEMM operands.  1: block-scaled FP8 (OCP MXFP8; SURVEY.md
+                                   §8(f) NEXT-2, DESIGN.md §3 Q24-Q27): te_load_weights still TAKES the bf16 blob and
+                                   quantises the four matrices of every layer to E4M3 with one E8M0 scale per 32
+                                   in_features; the GEMMs' A operands (x*g, attention output, SwiGLU output) are
+                                   quantised the same way in the producing epilogues; attention, accumulation and the
+                                   residual stream are unchanged.  Needs Hq/Hkv a power of two <= 8 and no prefix      */
 } te_config;
 
 /* Exact size in bytes of the canonical weight blob for cfg (see te_load_weights). */

@@ -44,8 +44,13 @@ enum {
   TE_TAP_QKV = 4,        /* bf16  [T, (Hq+2Hkv)*dh]  q (normed+rotated) | k | v  */
   TE_TAP_ATTN = 5,       /* bf16  [T, Hq*dh]                                    */
   TE_TAP_ACT = 6,        /* bf16  [T, F]       silu(gate)*up                    */
-  TE_TAP_TRACE = 7       /* u64   [4 GEMM classes (qkv,oproj,gateup,down)][n_SMs][96] ns stamps / SM clocks
+  TE_TAP_TRACE = 7,      /* u64   [4 GEMM classes (qkv,oproj,gateup,down)][n_SMs][96] ns stamps / SM clocks
                             of the last launch of each class (TE_OPT_TRACE)     */
+  /* weight_dtype = 1 (MXFP8): the quantised A operands; scales in the tiled order of te_debug_mx_quantise */
+  TE_TAP_ATTN8 = 8,      /* u8 E4M3 [T, Hq*dh]                                  */
+  TE_TAP_ACT8 = 9,       /* u8 E4M3 [T, F]                                      */
+  TE_TAP_SF_ATTN = 10,   /* u8 E8M0 [ceil(T/128), Hq*dh/128, 512]               */
+  TE_TAP_SF_ACT = 11     /* u8 E8M0 [ceil(T/128), F/128, 512]                   */
 };
 int te_debug_set_range(te_handle* h, int32_t layer_begin, int32_t layer_end,
                        int32_t stop_after_attn);
@@ -68,6 +73,17 @@ int te_debug_gemm_splitk(int device, const void* a_bf16, const void* b_bf16, flo
  * wholly out of range.  N % 32 == 0, width <= 512, ceil(M/256) * n_tiles <= SM pairs.  Synchronous. */
 int te_debug_gemm_wide(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
                        int32_t n, int32_t k, int32_t n_tiles);
+
+/* MXFP8 quantiser alone (te_config.weight_dtype = 1; DESIGN.md §3 Q24-Q25): src DEVICE bf16 [rows, k] ->
+ * codes DEVICE uint8 [rows, k] (E4M3) and scales_tiled DEVICE uint8 [rows/128 (rounded up), k/128, 512] (E8M0): the
+ * scale of (row r, 32-element block b) is byte  ((r/128) * (k/128) + b/4) * 512 + (r%32)*16 + ((r/32)%4)*4 + b%4
+ * (the order the tensor core's scale copy takes).  k % 128 == 0.  Synchronous. */
+int te_debug_mx_quantise(int device, const void* src_bf16, int32_t rows, int32_t k, void* codes, void* scales_tiled);
+
+/* C = Q(A) * Q(B)^T through the block-scaled tcgen05 kernel (te_gemm8.cuh, plain epilogue): A, B DEVICE bf16 are
+ * quantised to MXFP8 on the device first.  k % 128 == 0, n % block_n == 0, block_n in {128, 256}.  Synchronous. */
+int te_debug_gemm_mxfp8(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m, int32_t n,
+                        int32_t k, int32_t block_n);
 
 #ifdef __cplusplus
 }

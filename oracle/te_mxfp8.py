@@ -61,6 +61,17 @@ def e4m3_encode_rne(v: np.ndarray) -> np.ndarray:
     return np.where(np.signbit(v), code | 0x80, code).astype(np.uint8)
 
 
+def e4m3_round(v: np.ndarray) -> np.ndarray:
+    """float -> the nearest E4M3 VALUE (ties to even), |v| <= 448: the definition of rounding to a 3-bit mantissa —
+    the grid step of the binade of |v| is 2^(floor(log2|v|) - 3), at least the subnormal step 2^-9, and np.rint
+    rounds half to even.  Same function as e4m3_decode(e4m3_encode_rne(v)) (pinned), without the table search."""
+    v = np.asarray(v, dtype=np.float64)
+    a = np.minimum(np.abs(v), E4M3_MAX)
+    _, e = np.frexp(a)                                     # a = f * 2^e, f in [0.5, 1)  ->  floor(log2 a) = e - 1
+    step = np.ldexp(1.0, np.maximum(e - 1, -6) - 3)
+    return np.copysign(np.rint(a / step) * step, v)
+
+
 def scale_code(amax32: np.ndarray) -> np.ndarray:
     """Q25: E8M0 code of the block scale from the block's float32 amax."""
     bits = np.asarray(amax32, dtype=np.float32).view(np.uint32).astype(np.int64)
@@ -91,8 +102,12 @@ def dequantise(codes: np.ndarray, scales: np.ndarray) -> np.ndarray:
 
 
 def fake_quant(x: np.ndarray) -> np.ndarray:
-    """dequantise(quantise(x)) -> float64 (what the quantised network computes with)."""
-    return dequantise(*quantise(x))
+    """dequantise(quantise(x)) -> float64 (what the quantised network computes with), evaluated on values
+    (e4m3_round) instead of through the byte codes; identical by construction, pinned in tests/test_mxfp8_pins.py."""
+    x32 = np.asarray(x, dtype=np.float32)
+    blk = x32.reshape(x32.shape[:-1] + (x32.shape[-1] // BLOCK, BLOCK))
+    X = np.float64(2.0) ** (scale_code(np.max(np.abs(blk), axis=-1)).astype(np.float64) - 127.0)
+    return (e4m3_round(blk.astype(np.float64) / X[..., None]) * X[..., None]).reshape(x32.shape)
 
 
 # ------------------------------------------------------------------ the quantised network (Q26)
@@ -136,8 +151,10 @@ def layer_forward_mxfp8(x: np.ndarray, Wq: dict, phi: np.ndarray, m, taps: dict 
 
 
 def encode_mxfp8(blob_bits, layout, m, embeds, text_lens, grid_h, grid_w, *, frames=None, layer_begin=0,
-                 layer_end=None, taps=None) -> np.ndarray:
-    """te_encode of the MXFP8 network in float64 (positions, packing and angles are te_oracle's)."""
+                 layer_end=None, taps=None, weights_cache: dict | None = None) -> np.ndarray:
+    """te_encode of the MXFP8 network in float64 (positions, packing and angles are te_oracle's).
+    weights_cache (optional, plumbing only): {layer: quantised weights} kept between calls on the same blob as float32
+    (dequantised MXFP8 values are exact in float32), so that several workloads share one pass of the quantiser."""
     from . import te_oracle as O
     text_lens = [int(t) for t in text_lens]
     cu = O.cu_seqlens(text_lens, grid_h, grid_w)
@@ -147,7 +164,13 @@ def encode_mxfp8(blob_bits, layout, m, embeds, text_lens, grid_h, grid_w, *, fra
     x = {b: np.asarray(embeds[cu[b]:cu[b + 1]], dtype=np.float64).copy() for b in sel}
     ftaps = {b: ({} if taps is not None else None) for b in sel}
     for l in range(layer_begin, m.n_layers if layer_end is None else layer_end):
-        Wl = quantise_layer_weights(O.unpack_layer(blob_bits, layout, l))
+        if weights_cache is not None and l in weights_cache:
+            Wl = {k: v.astype(np.float64) for k, v in weights_cache[l].items()}
+        else:
+            Wl = quantise_layer_weights(O.unpack_layer(blob_bits, layout, l))
+            if weights_cache is not None:
+                weights_cache[l] = {k: v.astype(np.float32) for k, v in Wl.items()}
+                assert all(np.array_equal(weights_cache[l][k].astype(np.float64), Wl[k]) for k in ("Wq", "g1"))
         for b in sel:
             x[b] = layer_forward_mxfp8(x[b], Wl, phi[cu[b]:cu[b + 1]], m, ftaps[b])
     if m.final_norm:

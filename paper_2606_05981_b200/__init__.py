@@ -31,6 +31,7 @@ TE_OPT_RESID_WIDE = 9
 TE_OPT_L2_RESIDUAL = 10
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
+TE_TAP_ATTN8, TE_TAP_ACT8, TE_TAP_SF_ATTN, TE_TAP_SF_ACT = 8, 9, 10, 11
 
 # include/te.h (the product boundary) and include/te_debug.h (test-only taps and stand-alone GEMMs)
 EXPORTS = [
@@ -38,7 +39,9 @@ EXPORTS = [
     "te_encode_host_submit", "te_encode_host_wait", "te_query_async_error", "te_set_option", "te_kernel_launches",
     "te_graph_captures", "te_dispatch_info", "te_kernel_times", "te_destroy", "te_strerror", "te_last_error",
 ]
-DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide"]
+DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide",
+                 "te_debug_mx_quantise", "te_debug_gemm_mxfp8"]
+TE_DTYPE_BF16, TE_DTYPE_MXFP8 = 0, 1
 
 
 class TEConfig(Structure):
@@ -50,6 +53,7 @@ class TEConfig(Structure):
         ("rms_eps", c_float), ("rope_theta", c_double),
         ("max_frames", c_int32), ("max_tokens", c_int32), ("max_tokens_per_frame", c_int32),
         ("final_norm", c_int32), ("rope_interleaved", c_int32), ("max_prefix_tokens", c_int32),
+        ("weight_dtype", c_int32),
     ]
 
 
@@ -110,6 +114,10 @@ def lib() -> ctypes.CDLL:
     L.te_debug_gemm_splitk.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
     L.te_debug_gemm_wide.restype = c_int
     L.te_debug_gemm_wide.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
+    L.te_debug_mx_quantise.restype = c_int
+    L.te_debug_mx_quantise.argtypes = [c_int, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
+    L.te_debug_gemm_mxfp8.restype = c_int
+    L.te_debug_gemm_mxfp8.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
     L.te_destroy.restype = None
     L.te_destroy.argtypes = [c_void_p]
     L.te_strerror.restype = c_char_p
@@ -145,13 +153,13 @@ def _check(code: int, h=None):
 
 
 def make_config(model, max_frames: int, max_tokens: int, max_tokens_per_frame: int = 256,
-                final_norm: int | None = None, max_prefix_tokens: int = 0) -> TEConfig:
+                final_norm: int | None = None, max_prefix_tokens: int = 0, weight_dtype: int = 0) -> TEConfig:
     """TEConfig from a workloads.TEModelConfig-like object (duck-typed)."""
     s_t, s_h, s_w = model.rope_sections
     return TEConfig(model.n_layers, model.hidden, model.n_q_heads, model.n_kv_heads, model.head_dim,
                     model.ffn, s_t, s_h, s_w, model.rms_eps, model.rope_theta, max_frames, max_tokens,
                     max_tokens_per_frame, model.final_norm if final_norm is None else final_norm,
-                    1 if getattr(model, "rope_interleaved", False) else 0, max_prefix_tokens)
+                    1 if getattr(model, "rope_interleaved", False) else 0, max_prefix_tokens, weight_dtype)
 
 
 # ---------------------------------------------------------------- C-ABI names, marshalling only
@@ -247,6 +255,14 @@ def te_debug_gemm_splitk(device, a_bf16, b_bf16, c, m, n, k, block_n=128, splits
     _check(lib().te_debug_gemm_splitk(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, splits))
 
 
+def te_debug_mx_quantise(device, src_bf16, rows, k, codes, scales_tiled):
+    _check(lib().te_debug_mx_quantise(device, _ptr(src_bf16), rows, k, _ptr(codes), _ptr(scales_tiled)))
+
+
+def te_debug_gemm_mxfp8(device, a_bf16, b_bf16, c, m, n, k, block_n=256):
+    _check(lib().te_debug_gemm_mxfp8(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n))
+
+
 def te_debug_gemm_wide(device, a_bf16, b_bf16, c, m, n, k, n_tiles):
     _check(lib().te_debug_gemm_wide(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, n_tiles))
 
@@ -267,9 +283,11 @@ class TextEncoder:
     """Convenience owner of a handle (create -> load -> encode -> destroy)."""
 
     def __init__(self, model, max_frames: int, max_tokens: int, device: int = 0,
-                 max_tokens_per_frame: int = 256, final_norm: int | None = None, max_prefix_tokens: int = 0):
+                 max_tokens_per_frame: int = 256, final_norm: int | None = None, max_prefix_tokens: int = 0,
+                 weight_dtype: int = 0):
         self.model = model
-        self.cfg = make_config(model, max_frames, max_tokens, max_tokens_per_frame, final_norm, max_prefix_tokens)
+        self.cfg = make_config(model, max_frames, max_tokens, max_tokens_per_frame, final_norm, max_prefix_tokens,
+                               weight_dtype)
         self.h = te_create(self.cfg, device)
 
     def load_weights(self, blob):

@@ -17,6 +17,7 @@
 // [0, nk), P packed over [0, nk/2), O in [128, 128 + dh)), so the tensor core, the softmax of one
 // tile and the epilogue of the previous one overlap.
 #pragma once
+#include "te_gemm8.cuh"  // MXFP8 quantiser of the output (te_config.weight_dtype = 1)
 #include "te_ptx.cuh"
 
 namespace te {
@@ -36,6 +37,9 @@ struct AttnTcParams {
   float2* stats;
   int prefix_mode;
   int prefix_len;
+  // MXFP8 variant: the output (= A operand of the O projection) is written as E4M3 + block scales instead of bf16
+  uint8_t* out8;    // [T, Hq*DH] or null
+  uint8_t* sf_out;  // tiled scales (te_gemm8.cuh)
 };
 
 template <int DH>
@@ -282,6 +286,16 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         uint32_t r[32];
         tmem_ld32(taddr + Cfg::O_COL + c0, r);
         tmem_ld_wait();
+        if (p.out8 != nullptr) {  // one 32-column chunk of a row = one MX block
+          if (pos < S) {
+            float v[32];
+#pragma unroll
+            for (int x = 0; x < 32; ++x) v[x] = __uint_as_float(r[x]) * w_new;
+            const int row = seq0 + pos, col = head * DH + c0, ld = p.n_q_heads * DH;
+            mx_store_block(v, p.out8 + (size_t)row * ld + col, p.sf_out + mx_sf_offset(row, col >> 5, ld / 128));
+          }
+          continue;
+        }
         if (pos < S) {
 #pragma unroll
           for (int q4 = 0; q4 < 4; ++q4) {

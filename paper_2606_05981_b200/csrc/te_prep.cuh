@@ -8,7 +8,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "te_gemm.cuh"  // DynParams
+#include "te_gemm8.cuh"  // DynParams, MXFP8 quantiser
 
 namespace te {
 
@@ -44,6 +44,9 @@ struct PrepParams {
   // that 0 * (what an earlier, larger call left there) can never be 0 * NaN.
   uint4* qkv_rows;  // [rows, qkv_row_vec16] the qkv workspace as 16-byte vectors
   int qkv_row_vec16;
+  // MXFP8 variant (te_config.weight_dtype = 1): x * g_first is written as E4M3 + block scales instead of bf16
+  uint8_t* xg8;     // [T, d] or null
+  uint8_t* sf_xg;   // tiled scales (te_gemm8.cuh)
   int8_t axis[64];  // M-RoPE axis (0 = t, 1 = h, 2 = w) of frequency pair i (contiguous or interleaved sections)
 };
 
@@ -146,7 +149,21 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
     uint2 o;
     o.x = *reinterpret_cast<uint32_t*>(&o0);
     o.y = *reinterpret_cast<uint32_t*>(&o1);
-    reinterpret_cast<uint2*>(p.xg + (size_t)tok * p.d)[c4] = o;
+    if (p.xg8 == nullptr) {
+      reinterpret_cast<uint2*>(p.xg + (size_t)tok * p.d)[c4] = o;
+    } else {
+      // 8 consecutive lanes hold one 32-column MX block (d % 128 == 0: whole blocks, whole warps)
+      const float q0 = v.x * __uint_as_float(g.x << 16), q1 = v.y * __uint_as_float(g.x & 0xFFFF0000u);
+      const float q2 = v.z * __uint_as_float(g.y << 16), q3 = v.w * __uint_as_float(g.y & 0xFFFF0000u);
+      float amax = fmaxf(fmaxf(fabsf(q0), fabsf(q1)), fmaxf(fabsf(q2), fabsf(q3)));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 1));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 2));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 4));
+      const uint32_t code = mx_scale_code(amax);
+      const float inv = mx_inv_scale(code);
+      reinterpret_cast<uint32_t*>(p.xg8 + (size_t)tok * p.d)[c4] = pack_e4m3x4(q0 * inv, q1 * inv, q2 * inv, q3 * inv);
+      if ((c4 & 7) == 0) p.sf_xg[mx_sf_offset(tok, c4 >> 3, p.d / 128)] = static_cast<uint8_t>(code);
+    }
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);

@@ -16,6 +16,7 @@
 #include "te_attn.cuh"
 #include "te_attn_tc.cuh"
 #include "te_gemm.cuh"
+#include "te_gemm8.cuh"
 #include "te_gemm_splitk.cuh"
 #include "te_gemm_wide.cuh"
 #include "te_prep.cuh"
@@ -53,8 +54,36 @@ bool make_tmap(CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, u
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// 2-D E4M3 row-major [rows, cols] tensor (MXFP8 operands), box = [box_rows, 128 cols = 128 B], 128-byte swizzle.
+bool make_tmap_u8(CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols};
+  cuuint32_t box[2] = {128, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Tiled MXFP8 block scales as a [tiles, 128] uint32 tensor: one 512-byte scale tile per row, box = one tile.
+bool make_tmap_sf(CUtensorMap* m, const void* base, uint64_t n_tiles) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {128, n_tiles};
+  cuuint64_t strides[1] = {512};
+  cuuint32_t box[2] = {128, 1};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 struct LayerOff {
   size_t g1, wqkv, gq, gk, wo, g2, wgu, wd;  // element offsets into the device weight buffer
+  // MXFP8 copy (te_config.weight_dtype = 1): byte offsets into w8 (elements) and sfw (tiled block scales)
+  size_t q8, o8, gu8, d8, sq8, so8, sgu8, sd8;
 };
 
 // A cached graph is valid for every call of the same SHAPE CLASS: per-call pointers and the exact token count
@@ -90,6 +119,7 @@ struct Plan {
   int bn_res = 128, k_res = 0, bx_res = 0, n_blk_res = 0, wide_tiles = 0, wide_bn = 0;
   int parts = 1;       // RMSNorm partial sums per row written by the residual GEMMs
   int attn_tc = 0, attn_split = 1, q_blocks = 1, g_shift = 0, s_bound = 0;
+  int mx = 0;          // MXFP8 variant: every GEMM on te_gemm8_kernel (CTA pairs, block-scaled tcgen05)
 };
 
 }  // namespace
@@ -119,6 +149,15 @@ struct te_handle {
   size_t w_elems = 0;
   std::vector<LayerOff> off;
   size_t gf_off = 0;
+  // MXFP8 variant: E4M3 copies of the four matrices of every layer + their tiled E8M0 block scales; E4M3
+  // activations (A operands) with their scales; per-layer tensor maps in 64- and 128-row boxes
+  uint8_t *w8 = nullptr, *sfw = nullptr;
+  uint8_t *xg8 = nullptr, *attn8 = nullptr, *act8 = nullptr, *sf_xg = nullptr, *sf_attn = nullptr, *sf_act = nullptr;
+  struct LayerMaps8 { CUtensorMap qkv[2], o[2], gu[2], d[2], sf_qkv, sf_o, sf_gu, sf_d; };
+  std::vector<LayerMaps8> tm8;
+  CUtensorMap tmA_xg8, tmA_attn8, tmA_act8, tmSF_xg, tmSF_attn, tmSF_act;
+  int bn8_qkv = 128;  // MXFP8 QKV tile width (128: two accumulator stages; 256: one)
+  int bn8_gu = 192;   // MXFP8 gate/up tile width (192: two accumulator stages, weights re-interleaved per 192 rows; 256: one)
   // weight tensor maps per layer, one per B box height {32, 64, 128, 256} rows (index 0..3)
   struct LayerMaps { CUtensorMap qkv[4], o[4], gu[4], d[4]; };
   std::vector<LayerMaps> tm;
@@ -207,6 +246,14 @@ int validate_config(const te_config& c) {
   if (((c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim) % 128 != 0) return TE_ERR_UNSUPPORTED;
   if ((c.n_q_heads * c.head_dim) % 64 != 0) return TE_ERR_UNSUPPORTED;
   if (c.max_tokens_per_frame > 256) return TE_ERR_UNSUPPORTED;
+  if (c.weight_dtype < 0 || c.weight_dtype > 1) return TE_ERR_INVALID_ARG;
+  if (c.weight_dtype == 1) {
+    // MXFP8: 128-element K chunks everywhere; the quantising attention epilogue exists in the tcgen05 kernel only
+    // (G = Hq/Hkv a power of two <= 8); no cached prefix (its merge pass re-reads a bf16 output)
+    const int G = c.n_q_heads / c.n_kv_heads;
+    if ((c.n_q_heads * c.head_dim) % 128 != 0 || (G & (G - 1)) != 0 || G > 8 || c.max_prefix_tokens > 0)
+      return TE_ERR_UNSUPPORTED;
+  }
   return TE_OK;
 }
 
@@ -286,6 +333,23 @@ cudaError_t launch_gemm_bn(const LaunchCtx& lc, int bn, int pair, int dh, const 
     if (bn == 256) return launch_gemm<256, EPI, 128>(lc, a, b, p, sms, st);
     return launch_gemm<128, EPI, 128>(lc, a, b, p, sms, st);
   }
+}
+
+// MXFP8 kernel: one CTA pair per 256 x BN tile, persistent (te_gemm8.cuh)
+template <int BN, int EPI, int DH>
+cudaError_t launch_gemm8(const LaunchCtx& lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmSFA,
+                         const CUtensorMap& tmSFB, const te::GemmParams& p, const te::Gemm8Extra& x8, int sm_count,
+                         cudaStream_t st) {
+  using Cfg = te::Gemm8Cfg<BN, EPI>;
+  const int tiles = ((p.num_m_blk + 1) / 2) * p.num_n_blk;
+  const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
+  return launch_k(lc, te::te_gemm8_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM2_THREADS), Cfg::SMEM_BYTES, st, tmA,
+                  tmB, tmSFA, tmSFB, p, x8);
+}
+template <int BN, int EPI, int DH>
+cudaError_t set_gemm8_attr() {
+  return cudaFuncSetAttribute(te::te_gemm8_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              te::Gemm8Cfg<BN, EPI>::SMEM_BYTES);
 }
 
 // split-K kernel: `p.splits` CTAs per 128 x bn tile (small batches; te_gemm_splitk.cuh)
@@ -374,6 +438,14 @@ cudaError_t init_kernel_attrs() {
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
+  TE_ATTR((set_gemm8_attr<128, te::EPI_QKV, 128>()));
+  TE_ATTR((set_gemm8_attr<128, te::EPI_QKV, 64>()));
+  TE_ATTR((set_gemm8_attr<256, te::EPI_QKV, 128>()));
+  TE_ATTR((set_gemm8_attr<128, te::EPI_RESID, 128>()));
+  TE_ATTR((set_gemm8_attr<256, te::EPI_SWIGLU, 128>()));
+  TE_ATTR((set_gemm8_attr<192, te::EPI_SWIGLU, 128>()));
+  TE_ATTR((set_gemm8_attr<128, te::EPI_PLAIN, 128>()));
+  TE_ATTR((set_gemm8_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::AttnCfg<128, 1>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_attn_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -413,6 +485,7 @@ Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
   Plan pl;
   pl.Tb = Tb;
+  pl.mx = c.weight_dtype == 1;
   // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
   // one CTA per tile so that more SMs stream weights (HBM-bound regime).
   pl.pair = h->pair_mode == 2 ? (Tb >= 1024 ? 1 : 0) : h->pair_mode;
@@ -467,6 +540,15 @@ Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
   pl.n_blk_res = d / pl.bn_res;
   // RMSNorm statistics: one partial sum of squares per residual N-tile and epilogue column share
   pl.parts = pl.wide_tiles ? pl.wide_tiles * 2 : pl.n_blk_res * ((pl.pair || pl.k_res) ? 2 : 1);
+  if (pl.mx) {  // MXFP8: CTA pairs for everything; QKV 128- or 256-wide, gate/up 256-wide, residual GEMMs 128-wide tiles
+    pl.pair = pl.pair_qkv = pl.pair_gu = 1;
+    pl.k_qkv = pl.k_gu = pl.k_res = pl.wide_tiles = pl.gu_wide_tiles = pl.gu_half = 0;
+    pl.bn_qkv = (n_qkv % h->bn8_qkv == 0) ? h->bn8_qkv : 128;
+    pl.bn_gu = h->bn8_gu;
+    pl.bn_res = 128;
+    pl.n_blk_res = d / 128;
+    pl.parts = pl.n_blk_res * 2;
+  }
   // attention: host-side upper bound of S_b for the grid (exact lengths stay on the device)
   int s_bound = Tb - (n_frames - 1) * n_vis;
   if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
@@ -490,7 +572,7 @@ Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
 // What ran, by class, in the names ncu prints (te_dispatch_info; bench.py's roofline label).
 std::string describe_plan(const te_handle* h, const Plan& pl) {
   const te_config& c = h->cfg;
-  char b[160];
+  char b[320];
   std::string s;
   auto gemm = [&](const char* cls, int epi, bool k, bool pair2, int bn, int dh) {
     if (k) snprintf(b, sizeof(b), "%s=te_gemmk_kernel<%d, %d, %d>;", cls, bn, epi, dh);
@@ -498,6 +580,12 @@ std::string describe_plan(const te_handle* h, const Plan& pl) {
     else snprintf(b, sizeof(b), "%s=te_gemm_kernel<%d, %d, %d>;", cls, bn, epi, dh);
     s += b;
   };
+  if (pl.mx) {
+    snprintf(b, sizeof(b), "qkv=te_gemm8_kernel<%d, 1, %d>;attn=te_attn_tc_kernel<%d>;oproj=te_gemm8_kernel<128, 2, 128>;"
+             "down=te_gemm8_kernel<128, 2, 128>;gateup=te_gemm8_kernel<%d, 3, 128>;bucket_tokens=%d", pl.bn_qkv,
+             c.head_dim, c.head_dim, pl.bn_gu, pl.Tb);
+    return std::string(b);
+  }
   gemm("qkv", te::EPI_QKV, pl.k_qkv, pl.pair_qkv, pl.bn_qkv, c.head_dim);
   snprintf(b, sizeof(b), "attn=%s;", pl.attn_tc ? (c.head_dim == 128 ? "te_attn_tc_kernel<128>" : "te_attn_tc_kernel<64>")
                                                 : "te_attn_kernel");
@@ -576,6 +664,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
     memcpy(pp.axis, h->axis, sizeof(pp.axis));
     tick();
     pp.qkv_rows = reinterpret_cast<uint4*>(h->qkv); pp.qkv_row_vec16 = n_qkv / 8;
+    pp.xg8 = pl.mx ? h->xg8 : nullptr; pp.sf_xg = h->sf_xg;
     TE_CUDA(h, launch_k(lc, te::te_prep_kernel, dim3(Tb + te::PREP_PAD_ROWS), dim3(256), 0, st, pp));
     tock(TE_KCLASS_PREP);
     ++nk;
@@ -600,7 +689,15 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
       p.trace = trace_ptr(0);
       tick();
-      if (pl.k_qkv) {
+      if (pl.mx) {
+        te::Gemm8Extra x8{};
+        const CUtensorMap& tb = h->tm8[l].qkv[pl.bn_qkv == 256 ? 1 : 0];
+        const CUtensorMap &sa = h->tmSF_xg, &sb = h->tm8[l].sf_qkv;
+        cudaError_t e = pl.bn_qkv == 256 ? launch_gemm8<256, te::EPI_QKV, 128>(lc, h->tmA_xg8, tb, sa, sb, p, x8, h->sm_count, st)
+                        : dh == 128     ? launch_gemm8<128, te::EPI_QKV, 128>(lc, h->tmA_xg8, tb, sa, sb, p, x8, h->sm_count, st)
+                                        : launch_gemm8<128, te::EPI_QKV, 64>(lc, h->tmA_xg8, tb, sa, sb, p, x8, h->sm_count, st);
+        TE_CUDA(h, e);
+      } else if (pl.k_qkv) {
         p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_QKV>(lc, pl.bn_qkv, dh, h->tmA_xg, h->tm[l].qkv[pl.bx_qkv], p, st));
       } else {
@@ -623,6 +720,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         tp.out = h->attn; tp.cu_seqlens = h->cu; tp.n_q_heads = c.n_q_heads; tp.n_kv_heads = c.n_kv_heads;
         tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2;
         tp.stats = P > 0 ? h->attn_stats : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
+        tp.out8 = pl.mx ? h->attn8 : nullptr; tp.sf_out = h->sf_attn;
         TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st)
                              : launch_attn_tc<64>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st));
         if (P > 0) {  // second pass: the P cached prefix keys of this layer, merged in place
@@ -649,7 +747,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       p.x_to_out = (dbg_stop && last_layer) ? 1 : 0;
       p.trace = trace_ptr(1);
       tick();
-      if (pl.wide_tiles) {
+      if (pl.mx) {
+        te::Gemm8Extra x8{};
+        x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
+        TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_attn8, h->tm8[l].o[0], h->tmSF_attn, h->tm8[l].sf_o, p, x8,
+                                                        h->sm_count, st)));
+      } else if (pl.wide_tiles) {
         CUtensorMap tmB;
         if (!make_tmap(&tmB, h->w + o.wo, d, n_q, pl.wide_bn / 4)) { h->err = "tensor map (wide O-proj)"; return TE_ERR_CUDA; }
         TE_CUDA(h, launch_wide<te::EPI_RESID>(lc, h->tmA_attn, tmB, p, pl.wide_tiles, pl.wide_bn, st));
@@ -670,7 +773,15 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       p.act = h->act; p.ld_act = F;
       p.trace = trace_ptr(2);
       tick();
-      if (pl.gu_wide_tiles) {
+      if (pl.mx) {
+        te::Gemm8Extra x8{};
+        x8.q_out = h->act8; x8.q_sf = h->sf_act; x8.q_kchunks = F / 128; x8.q_ld = F;
+        p.num_n_blk = 2 * F / pl.bn_gu;
+        TE_CUDA(h, pl.bn_gu == 192 ? (launch_gemm8<192, te::EPI_SWIGLU, 128>(lc, h->tmA_xg8, h->tm8[l].gu[0], h->tmSF_xg,
+                                                                            h->tm8[l].sf_gu, p, x8, h->sm_count, st))
+                                   : (launch_gemm8<256, te::EPI_SWIGLU, 128>(lc, h->tmA_xg8, h->tm8[l].gu[1], h->tmSF_xg,
+                                                                            h->tm8[l].sf_gu, p, x8, h->sm_count, st)));
+      } else if (pl.gu_wide_tiles) {
         p.gu_half = 0;
         TE_CUDA(h, launch_wide<te::EPI_SWIGLU>(lc, h->tmA_xg, h->tm[l].gu[box_index(32)], p, pl.gu_wide_tiles,
                                                2 * pl.gu_wide_w, st));
@@ -692,7 +803,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       p.x_to_out = (last_layer && !norm_tail) ? 1 : 0;
       p.trace = trace_ptr(3);
       tick();
-      if (pl.wide_tiles) {
+      if (pl.mx) {
+        te::Gemm8Extra x8{};
+        x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
+        TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_act8, h->tm8[l].d[0], h->tmSF_act, h->tm8[l].sf_d, p, x8,
+                                                        h->sm_count, st)));
+      } else if (pl.wide_tiles) {
         CUtensorMap tmB;
         if (!make_tmap(&tmB, h->w + o.wd, d, F, pl.wide_bn / 4)) { h->err = "tensor map (wide down)"; return TE_ERR_CUDA; }
         TE_CUDA(h, launch_wide<te::EPI_RESID>(lc, h->tmA_act, tmB, p, pl.wide_tiles, pl.wide_bn, st));
@@ -815,6 +931,27 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
       cudaMemset(h->dyn, 0, sizeof(te::DynParams)) != cudaSuccess ||
       cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess)
     return fail(TE_ERR_CUDA);
+  if (c.weight_dtype == 1) {  // MXFP8 activations (A operands) + tiled block scales (one byte per 32 elements)
+    const size_t rb = (T + 127) / 128;  // 128-row scale tiles
+    if (cudaMalloc(reinterpret_cast<void**>(&h->xg8), T * c.hidden) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->attn8), T * (size_t)n_q) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->act8), T * (size_t)c.ffn) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->sf_xg), rb * (c.hidden / 128) * 512) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->sf_attn), rb * (n_q / 128) * 512) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->sf_act), rb * (c.ffn / 128) * 512) != cudaSuccess)
+      return fail(TE_ERR_CUDA);
+    // rows past a call's tokens are multiplied (never stored): start them as zeros with unit scales
+    cudaMemset(h->xg8, 0, T * c.hidden);
+    cudaMemset(h->attn8, 0, T * (size_t)n_q);
+    cudaMemset(h->act8, 0, T * (size_t)c.ffn);
+    cudaMemset(h->sf_xg, 127, rb * (c.hidden / 128) * 512);
+    cudaMemset(h->sf_attn, 127, rb * (n_q / 128) * 512);
+    cudaMemset(h->sf_act, 127, rb * (c.ffn / 128) * 512);
+    if (!make_tmap_u8(&h->tmA_xg8, h->xg8, T, c.hidden, te::GEMM_BM) || !make_tmap_u8(&h->tmA_attn8, h->attn8, T, n_q, te::GEMM_BM) ||
+        !make_tmap_u8(&h->tmA_act8, h->act8, T, c.ffn, te::GEMM_BM) || !make_tmap_sf(&h->tmSF_xg, h->sf_xg, rb * (c.hidden / 128)) ||
+        !make_tmap_sf(&h->tmSF_attn, h->sf_attn, rb * (n_q / 128)) || !make_tmap_sf(&h->tmSF_act, h->sf_act, rb * (c.ffn / 128)))
+      return fail(TE_ERR_CUDA);
+  }
   if (c.max_prefix_tokens > 0) {
     const size_t n_kv = 2 * (size_t)c.n_kv_heads * c.head_dim;
     if (cudaMalloc(reinterpret_cast<void**>(&h->kv_prefix), (size_t)c.n_layers * c.max_prefix_tokens * n_kv * sizeof(bf16)) !=
@@ -910,6 +1047,47 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
     }
   }
   h->gf_off = o;
+  if (e == cudaSuccess && c.weight_dtype == 1) {
+    // MXFP8 copies of the four matrices of every layer (gate/up from the interleaved copy) + tiled block scales
+    // gate/up tile width of the MXFP8 GEMM: 192 (two accumulator stages) when it divides 2F, else 256
+    if ((2 * F) % 192 != 0 || h->bn_gu != 256) h->bn8_gu = 256;
+    const size_t gu_tile = (size_t)h->bn8_gu;
+    const size_t per_layer = n_qkv * d + d * n_q + 2 * F * d + d * F;
+    // scale tiles (512 B each): 128-row blocks x K/128 chunks; gate/up's are grouped per N tile (2 per 192 or 256 rows)
+    auto sf_tiles = [](size_t rows, size_t K, size_t tile_rows) { return rows / tile_rows * ((tile_rows + 127) / 128) * (K / 128); };
+    const size_t sf_layer = (sf_tiles(n_qkv, d, 128) + sf_tiles(d, n_q, 128) + sf_tiles(2 * F, d, gu_tile) + sf_tiles(d, F, 128)) * 512;
+    if (!h->w8) e = cudaMalloc(reinterpret_cast<void**>(&h->w8), per_layer * c.n_layers);
+    if (e == cudaSuccess && !h->sfw) e = cudaMalloc(reinterpret_cast<void**>(&h->sfw), sf_layer * c.n_layers);
+    if (e == cudaSuccess) e = cudaMemset(h->sfw, 127, sf_layer * c.n_layers);  // (half-used tiles of 192-row groups)
+    h->tm8.resize(c.n_layers);
+    size_t o8 = 0, os = 0;
+    auto quant = [&](size_t src_off, size_t rows, size_t K, size_t tile_rows, int gu_src, size_t* w_off, size_t* s_off,
+                     CUtensorMap* sf_map) {
+      *w_off = o8;
+      *s_off = os;
+      const long long blocks = (long long)rows * (K / 32);
+      te::te_mx_quantise_bf16_kernel<<<(unsigned)((blocks + 255) / 256), 256>>>(h->w + src_off, h->w8 + o8, h->sfw + os, (int)rows,
+                                                                              (int)K, (int)tile_rows, gu_src);
+      ok = ok && make_tmap_sf(sf_map, h->sfw + os, sf_tiles(rows, K, tile_rows));
+      o8 += rows * K;
+      os += sf_tiles(rows, K, tile_rows) * 512;
+    };
+    for (int l = 0; l < c.n_layers && e == cudaSuccess; ++l) {
+      LayerOff& L = h->off[l];
+      quant(L.wqkv, n_qkv, d, 128, 0, &L.q8, &L.sq8, &h->tm8[l].sf_qkv);
+      quant(L.wo, d, n_q, 128, 0, &L.o8, &L.so8, &h->tm8[l].sf_o);
+      quant(L.wgu, 2 * F, d, gu_tile, gu_tile == 256 ? 0 : h->bn_gu, &L.gu8, &L.sgu8, &h->tm8[l].sf_gu);
+      quant(L.wd, d, F, 128, 0, &L.d8, &L.sd8, &h->tm8[l].sf_d);
+      e = cudaGetLastError();
+      for (int bi = 0; bi < 2; ++bi) {
+        const uint32_t box = 64u << bi;
+        ok = ok && make_tmap_u8(&h->tm8[l].qkv[bi], h->w8 + L.q8, n_qkv, d, box);
+        ok = ok && make_tmap_u8(&h->tm8[l].o[bi], h->w8 + L.o8, d, n_q, box);
+        ok = ok && make_tmap_u8(&h->tm8[l].gu[bi], h->w8 + L.gu8, 2 * F, d, bi == 0 && gu_tile == 192 ? 96u : box);
+        ok = ok && make_tmap_u8(&h->tm8[l].d[bi], h->w8 + L.d8, d, F, box);
+      }
+    }
+  }
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   cudaFree(stage);
   if (e != cudaSuccess) {
@@ -1233,6 +1411,10 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
     case TE_TAP_QKV: src = h->qkv; need = T * (size_t)(c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim * sizeof(bf16); break;
     case TE_TAP_ATTN: src = h->attn; need = T * (size_t)c.n_q_heads * c.head_dim * sizeof(bf16); break;
     case TE_TAP_ACT: src = h->act; need = T * (size_t)c.ffn * sizeof(bf16); break;
+    case TE_TAP_ATTN8: src = h->attn8; need = T * (size_t)c.n_q_heads * c.head_dim; break;
+    case TE_TAP_ACT8: src = h->act8; need = T * (size_t)c.ffn; break;
+    case TE_TAP_SF_ATTN: src = h->sf_attn; need = (T + 127) / 128 * ((size_t)c.n_q_heads * c.head_dim / 128) * 512; break;
+    case TE_TAP_SF_ACT: src = h->sf_act; need = (T + 127) / 128 * ((size_t)c.ffn / 128) * 512; break;
     case TE_TAP_TRACE:
       src = h->trace;
       need = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
@@ -1240,7 +1422,7 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
       break;
     default: return TE_ERR_INVALID_ARG;
   }
-  if (T == 0 || n_bytes != need) return TE_ERR_INVALID_ARG;
+  if (T == 0 || n_bytes != need || !src) return TE_ERR_INVALID_ARG;
   TE_CUDA(h, cudaSetDevice(h->device));
   TE_CUDA(h, cudaDeviceSynchronize());
   TE_CUDA(h, cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost));
@@ -1328,6 +1510,54 @@ int te_debug_gemm_wide(int device, const void* a, const void* b, float* cmat, in
   return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
+int te_debug_mx_quantise(int device, const void* src_bf16, int32_t rows, int32_t k, void* codes, void* scales_tiled) {
+  if (!src_bf16 || !codes || !scales_tiled || rows < 1 || k < 128 || k % 128 != 0) return TE_ERR_INVALID_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
+  const long long blocks = (long long)rows * (k / 32);
+  te::te_mx_quantise_bf16_kernel<<<(unsigned)((blocks + 255) / 256), 256>>>(
+      static_cast<const bf16*>(src_bf16), static_cast<uint8_t*>(codes), static_cast<uint8_t*>(scales_tiled), rows, k, 128, 0);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+}
+
+int te_debug_gemm_mxfp8(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                        int32_t block_n) {
+  int sms = 0;
+  int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
+  if (rc != TE_OK) return rc;
+  if ((block_n != 128 && block_n != 256) || n % block_n != 0 || k % 128 != 0) return TE_ERR_UNSUPPORTED;
+  const size_t m_pad = ((size_t)m + 255) / 256 * 256;
+  uint8_t *a8 = nullptr, *b8 = nullptr, *sa = nullptr, *sb = nullptr;
+  auto done = [&](int code) {
+    for (void* q : {(void*)a8, (void*)b8, (void*)sa, (void*)sb})
+      if (q) cudaFree(q);
+    return code;
+  };
+  if (cudaMalloc(reinterpret_cast<void**>(&a8), m_pad * k) != cudaSuccess || cudaMalloc(reinterpret_cast<void**>(&b8), (size_t)n * k) != cudaSuccess ||
+      cudaMalloc(reinterpret_cast<void**>(&sa), m_pad * k / 32) != cudaSuccess ||
+      cudaMalloc(reinterpret_cast<void**>(&sb), (size_t)n * k / 32) != cudaSuccess)
+    return done(TE_ERR_CUDA);
+  cudaMemset(a8, 0, m_pad * k);
+  cudaMemset(sa, 127, m_pad * k / 32);
+  const long long ba = (long long)m * (k / 32), bb = (long long)n * (k / 32);
+  te::te_mx_quantise_bf16_kernel<<<(unsigned)((ba + 255) / 256), 256>>>(static_cast<const bf16*>(a), a8, sa, m, k, 128, 0);
+  te::te_mx_quantise_bf16_kernel<<<(unsigned)((bb + 255) / 256), 256>>>(static_cast<const bf16*>(b), b8, sb, n, k, 128, 0);
+  CUtensorMap ta, tb, tsa, tsb;
+  if (!make_tmap_u8(&ta, a8, m_pad, k, te::GEMM_BM) || !make_tmap_u8(&tb, b8, n, k, block_n / 2) ||
+      !make_tmap_sf(&tsa, sa, m_pad * k / 32 / 512) || !make_tmap_sf(&tsb, sb, ((size_t)n + 127) / 128 * (k / 128)))
+    return done(TE_ERR_CUDA);
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
+  p.c = cmat; p.ld_c = n;
+  te::Gemm8Extra x8{};
+  const LaunchCtx lc;
+  cudaError_t e = block_n == 256 ? launch_gemm8<256, te::EPI_PLAIN, 128>(lc, ta, tb, tsa, tsb, p, x8, sms, nullptr)
+                                 : launch_gemm8<128, te::EPI_PLAIN, 128>(lc, ta, tb, tsa, tsb, p, x8, sms, nullptr);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  return done(e == cudaSuccess ? TE_OK : TE_ERR_CUDA);
+}
+
 void te_destroy(te_handle* h) {
   if (!h) return;
   cudaSetDevice(h->device);
@@ -1338,7 +1568,7 @@ void te_destroy(te_handle* h) {
   void* ptrs[] = {h->w, h->dyn, h->resid, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv,
                   h->attn, h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
                   h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens,
-                  h->attn_stats};
+                  h->attn_stats, h->w8, h->sfw, h->xg8, h->attn8, h->act8, h->sf_xg, h->sf_attn, h->sf_act};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto& sl : h->slot)

@@ -23,12 +23,13 @@ class GpuTE:
     """Owns one handle; encode() returns numpy arrays."""
 
     def __init__(self, model, max_frames, max_tokens, blob, final_norm=None, cta_pair=None, resid_bn=None,
-                 split_k=None, max_prefix_tokens=0, attn_impl=None, resid_wide=None):
+                 split_k=None, max_prefix_tokens=0, attn_impl=None, resid_wide=None, weight_dtype=0):
         import torch
         import paper_2606_05981_b200 as te
         self.te, self.torch, self.model = te, torch, model
+        self.weight_dtype = weight_dtype
         self.enc = te.TextEncoder(model, max_frames, max_tokens, final_norm=final_norm,
-                                  max_prefix_tokens=max_prefix_tokens)
+                                  max_prefix_tokens=max_prefix_tokens, weight_dtype=weight_dtype)
         self.enc.load_weights(blob)
         if cta_pair is not None:
             te.te_set_option(self.enc.h, te.TE_OPT_CTA_PAIR, cta_pair)
@@ -90,8 +91,42 @@ class GpuTE:
             "act": bf16_bits_to_f64(self.tap(te.TE_TAP_ACT, (T, m.ffn), np.uint16)),
         }
 
+    def taps_mx(self, T):
+        """MXFP8 variant: q/k/v (bf16) and the dequantised attention / SwiGLU outputs (E4M3 codes x E8M0 scales)."""
+        m, te = self.model, self.te
+        nqkv = (m.n_q_heads + 2 * m.n_kv_heads) * m.head_dim
+        nq = m.n_q_heads * m.head_dim
+        nk = m.n_kv_heads * m.head_dim
+        qkv = bf16_bits_to_f64(self.tap(te.TE_TAP_QKV, (T, nqkv), np.uint16))
+        rb = (T + 127) // 128
+        out = {"q": qkv[:, :nq], "k": qkv[:, nq:nq + nk], "v": qkv[:, nq + nk:]}
+        for key, tap_c, tap_s, K in (("attn", te.TE_TAP_ATTN8, te.TE_TAP_SF_ATTN, nq), ("act", te.TE_TAP_ACT8, te.TE_TAP_SF_ACT, m.ffn)):
+            codes = self.tap(tap_c, (T, K), np.uint8)
+            sf = untile_scales(self.tap(tap_s, (rb, K // 128, 512), np.uint8), T, K)
+            out[key] = mx_dequant(codes, sf)
+        return out
+
     def close(self):
         self.enc.close()
+
+
+def untile_scales(tiled, rows, K):
+    """[ceil(rows/128), K/128, 512] in the tensor core's scale-copy order (include/te_debug.h) -> [rows, K/32]."""
+    r = np.arange(rows)[:, None]
+    b = np.arange(K // 32)[None, :]
+    off = (r % 32) * 16 + ((r // 32) % 4) * 4 + b % 4
+    return np.asarray(tiled)[r // 128, b // 4, off]
+
+
+def mx_dequant(codes, scales):
+    """E4M3 codes [rows, K] x 2^(scale-127) per 32-element block -> float64, decoded from the format definition
+    (written out here: the GPU tests do not route the device's bytes through the oracle's decoder)."""
+    c = np.asarray(codes, dtype=np.uint8).astype(np.int64)
+    e, mnt = (c >> 3) & 0xF, (c & 7).astype(np.float64)
+    mag = np.where(e == 0, mnt / 8.0 * 2.0 ** -6, (1.0 + mnt / 8.0) * 2.0 ** (e - 7.0))
+    val = np.where(c & 0x80, -mag, mag)
+    X = 2.0 ** (np.asarray(scales, dtype=np.uint8).astype(np.float64) - 127.0)
+    return val * np.repeat(X, 32, axis=1)
 
 
 def workload_inputs(cfg_id, outliers=None):

@@ -33,6 +33,33 @@ GATE_COSSIN_ABS = 1e-5
 GATE_TAP_REL_L2 = 1e-2
 
 
+# MXFP8 variant (te_config.weight_dtype = 1) against the MXFP8 oracle (oracle/te_mxfp8.py).  Both sides quantise their
+# A operands to 8 bits, but from values that differ in the last bf16/fp32 bits, so E4M3 codes near a rounding boundary
+# flip (a 6-12 % step on that element).  Floors from the emulation (tests/bf16_emulation.py::encode_bf16_mx, cfg 1 and a
+# 2-layer full-width stack with the x1000 channels): update rel-L2 1.1e-2 .. 1.9e-2, max row update rel-L2 2.9e-2 ..
+# 3.2e-2, max |err| / rms 0.11 .. 0.13; the quantisation noise itself (MXFP8 network vs unquantised network) is 6-7 %.
+# A flipped code perturbs the next layer's input, which flips further codes: the floor GROWS with depth (same emulation,
+# cfg-3 shape, after 1 / 2 / 4 / 8 / 14 / 28 layers: update 0.9 / 1.1 / 1.4 / 1.7 / 2.1 / 2.5 e-2, max row 2.4 / 3.2 /
+# 6.2 / 6.2 / 8.3 / 9.7 e-2 over 256 rows, max |err| / rms 0.10 / 0.11 / 0.21 / 0.25 / 0.33 / 0.37).  Shallow gates
+# (one or two layers, teacher-forced layers at any depth) keep >= 3x over the 1-2 layer floor; the full-depth gates
+# keep >= 2x over the 28-layer floor.  What certifies the deep stack layer by layer is the teacher-forced test.
+GATE_MX_UPDATE_REL_L2 = 5e-2
+GATE_MX_ROW_UPDATE_REL_L2 = 9e-2
+GATE_MX_MAXABS_UPDATE_OVER_RMS = 4e-1
+GATE_MX_DEEP_UPDATE_REL_L2 = 6e-2
+GATE_MX_DEEP_ROW_UPDATE_REL_L2 = 3e-1
+GATE_MX_DEEP_MAXABS_UPDATE_OVER_RMS = 1.2
+GATE_MX_TAP_REL_L2 = 4e-2          # dequantised attn / act taps (code flips); q/k/v of layer 0 use GATE_TAP_REL_L2
+
+
+def passes_mx_gates(m, deep=False):
+    upd, row, mab = ((GATE_MX_DEEP_UPDATE_REL_L2, GATE_MX_DEEP_ROW_UPDATE_REL_L2, GATE_MX_DEEP_MAXABS_UPDATE_OVER_RMS)
+                     if deep else (GATE_MX_UPDATE_REL_L2, GATE_MX_ROW_UPDATE_REL_L2, GATE_MX_MAXABS_UPDATE_OVER_RMS))
+    return (m["rel_l2"] <= GATE_FINAL_REL_L2 and m["outlier_maxabs_rel"] <= GATE_OUTLIER_MAXABS
+            and m["update_rel_l2"] <= upd and m["nonoutlier_rel_l2"] <= upd
+            and m["max_row_update_rel_l2"] <= row and m["maxabs_update_over_rms"] <= mab)
+
+
 def rel_l2(a, ref):
     a = np.asarray(a, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)

@@ -26,7 +26,7 @@ def test_library_exports_every_declared_symbol(te):
     for header, names in (("te.h", te.EXPORTS), ("te_debug.h", te.DEBUG_EXPORTS)):
         hdr = open(os.path.join(ROOT, "include", header)).read()
         hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-        declared = set(re.findall(r"\b(te_[a-z_]+)\s*\(", hdr))
+        declared = set(re.findall(r"\b(te_[a-z_0-9]+)\s*\(", hdr))
         assert declared == set(names), (header, declared ^ set(names))
         for name in declared:
             assert hasattr(L, name), name
@@ -34,9 +34,9 @@ def test_library_exports_every_declared_symbol(te):
 
 def test_config_struct_layout_matches_header(te):
     # te_config: 9 int32, float, (pad) double, 6 int32 -> natural C layout
-    assert ctypes.sizeof(te.TEConfig) == 72
+    assert ctypes.sizeof(te.TEConfig) == 80
     assert te.TEConfig.rope_theta.offset == 40 and te.TEConfig.max_frames.offset == 48
-    assert te.TEConfig.rope_interleaved.offset == 64 and te.TEConfig.max_prefix_tokens.offset == 68
+    assert te.TEConfig.rope_interleaved.offset == 64 and te.TEConfig.max_prefix_tokens.offset == 68 and te.TEConfig.weight_dtype.offset == 72
 
 
 def test_blob_bytes_and_strerror_without_gpu(te):

@@ -35,6 +35,21 @@ def test_e4m3_encode_round_to_nearest_even_hand_worked():
     assert np.array_equal(Q.e4m3_encode_rne(-Q.e4m3_decode(codes[1:])), codes[1:] | 0x80)
 
 
+def test_value_rounding_equals_code_rounding():
+    """e4m3_round (rint on the binade's step) == decode(encode) (nearest-value table search, ties to the even code)
+    on every midpoint, every grid value and a dense random sample; fake_quant == dequantise(quantise)."""
+    grid = Q.e4m3_decode(np.arange(0x7F, dtype=np.uint8))
+    mids = (grid[1:] + grid[:-1]) / 2
+    rng = np.random.default_rng(3)
+    v = np.concatenate([grid, mids, np.nextafter(mids, 0), np.nextafter(mids, 1e9), rng.uniform(0, 448, 200000),
+                        np.exp(rng.uniform(np.log(2.0 ** -12), np.log(448.0), 200000))])
+    v = np.concatenate([v, -v])
+    assert np.array_equal(Q.e4m3_round(v), Q.e4m3_decode(Q.e4m3_encode_rne(v)))
+    x = (rng.standard_normal((50, 512)) * np.exp(rng.uniform(-30, 30, size=(50, 1)))).astype(np.float32)
+    x[:, 7] *= 1000
+    assert np.array_equal(Q.fake_quant(x), Q.dequantise(*Q.quantise(x)))
+
+
 def test_scale_code_hand_worked_amax():
     """Q25: the smallest power of two X with amax / X <= 448.  448 = 1.75 * 2^8."""
     cases = [(448.0, 127), (448.0001, 128), (449.0, 128), (896.0, 128), (897.0, 129), (1.0, 127 - 8),
