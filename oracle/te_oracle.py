@@ -160,8 +160,10 @@ def attention_causal_gqa(q: np.ndarray, k: np.ndarray, v: np.ndarray) -> np.ndar
 
 # ---------------------------------------------------------------------------- step 4: a layer
 def layer_forward(x: np.ndarray, W: dict, phi: np.ndarray, m, taps: dict | None = None,
-                  stop_after_attn: bool = False) -> np.ndarray:
-    """§8c step 4a-g for ONE frame.  x: [S, d] residual (fp64).  Returns the new residual."""
+                  stop_after_attn: bool = False, attention=None) -> np.ndarray:
+    """§8c step 4a-g for ONE frame.  x: [S, d] residual (fp64).  Returns the new residual.
+    `attention` (plumbing for oracle/te_vision.py, NEXT-4): the attention function of step 4e; None = the
+    decoder's causal attention_causal_gqa."""
     S = x.shape[0]
     Hq, Hkv, dh = m.n_q_heads, m.n_kv_heads, m.head_dim
     h = rmsnorm(x, W["g1"], m.rms_eps)                                   # 4a
@@ -172,7 +174,7 @@ def layer_forward(x: np.ndarray, W: dict, phi: np.ndarray, m, taps: dict | None 
     k = rmsnorm(k, W["gk"], m.rms_eps)
     q = rope_apply(q, phi)                                               # 4d
     k = rope_apply(k, phi)
-    o = attention_causal_gqa(q, k, v)                                    # 4e
+    o = (attention or attention_causal_gqa)(q, k, v)                     # 4e
     x = x + o.reshape(S, Hq * dh) @ W["Wo"].T                            # 4f
     if taps is not None:
         taps.setdefault("q", []).append(q.reshape(S, -1))
@@ -196,7 +198,7 @@ def encode(blob_bits: np.ndarray, layout: dict, m, embeds: np.ndarray, text_lens
            grid_h: int, grid_w: int, *, frames=None, layer_begin: int = 0,
            layer_end: int | None = None, stop_after_attn: bool = False,
            final_norm: int | None = None, taps: dict | None = None,
-           prefix_len: int = 0) -> np.ndarray:
+           prefix_len: int = 0, attention=None) -> np.ndarray:
     """te_encode in fp64 (§8c steps 1-5).  embeds: fp32/fp64 [T, d] frame-major packed.
     Returns float64 [T, d].  `frames` restricts the computation to a subset of frames
     (frames never interact, BASELINE.json:configs[4]); rows of other frames are NaN.
@@ -220,7 +222,7 @@ def encode(blob_bits: np.ndarray, layout: dict, m, embeds: np.ndarray, text_lens
         W = unpack_layer(blob_bits, layout, l)
         for b in sel:
             x[b] = layer_forward(x[b], W, phi[cu[b]:cu[b + 1]], m, frame_taps[b],
-                                 stop_after_attn=stop_after_attn)
+                                 stop_after_attn=stop_after_attn, attention=attention)
     fn = m.final_norm if final_norm is None else final_norm
     if fn:                                                               # step 5 (Q8)
         off, shape = layout[("final", "gf")]

@@ -341,8 +341,21 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_r
       }
       continue;
     }
-    // ---- q or k head.  Pass 1: sum of squares of the head (thread = row, TMEM reads only)
+    // ---- q or k head.  The cos/sin segments of the first rotation step are requested up front (16 independent
+    // 16-byte loads per lane): their L2 round trip overlaps pass 1's TMEM reads instead of following them.
     const __nv_bfloat16* gain = (col0 < p.q_cols_end) ? p.gq : p.gk;
+    float4 cs[8], sn[8];
+    auto load_cs = [&](int c0) {
+      const int cc = c0 + cq * 4;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int row = min(row_base + sub + 4 * i, M - 1);
+        cs[i] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc));
+        sn[i] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc));
+      }
+    };
+    load_cs(c_first);
+    // Pass 1: sum of squares of the head (thread = row, TMEM reads only)
     float ss = 0.f;
 #pragma unroll 1
     for (int c0 = 0; c0 < DH; c0 += 32) {
@@ -357,19 +370,10 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_r
     }
     const float sc = rstd / sqrtf(ss * (1.0f / DH) + p.eps);
     // ---- Pass 2: normalised halves a = u[c0..c0+32), b = u[HD2+c0..) -> staging -> rotate -> store.
-    // All cos/sin segments of the step are requested up front (16 independent 16-byte loads per
-    // lane) so that their L2 round trips overlap the TMEM reads and the staging instead of
-    // serialising behind each other.
 #pragma unroll 1
     for (int c0 = c_first; c0 < HD2; c0 += c_step) {
       const int cc = c0 + cq * 4;  // this lane's 4 columns inside the half
-      float4 cs[8], sn[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int row = min(row_base + sub + 4 * i, M - 1);
-        cs[i] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc));
-        sn[i] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc));
-      }
+      if (c0 != c_first) load_cs(c0);  // (later steps: requested here, overlapping this step's TMEM reads and staging)
       const uint2 ga = __ldg(reinterpret_cast<const uint2*>(gain + cc));
       const uint2 gb = __ldg(reinterpret_cast<const uint2*>(gain + HD2 + cc));
       {

@@ -153,7 +153,11 @@ struct Gemm8Cfg {
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES + SFA_BYTES + SFB_BYTES;
   static constexpr int BAR_BYTES = 256;
   static constexpr int STG_WARP_BYTES = (EPI == EPI_QKV ? 2 : 1) * 32 * 32 * 4;
-  static constexpr int STG_BYTES = (EPI == EPI_SWIGLU || EPI == EPI_PLAIN) ? 0 : GEMM2_EPI_WARPS * STG_WARP_BYTES;
+  // epilogue warps: with the MMA twice as fast as in bf16 the kernels are epilogue-bound (ncu r02a: tensor pipe 25-69 %
+  // active), so the 192-wide SwiGLU tile (3 MX blocks per row and half) gets three warps per TMEM lane quadrant
+  static constexpr int EPI_WARPS = (EPI == EPI_SWIGLU && BN == 192) ? 12 : GEMM2_EPI_WARPS;
+  static constexpr int THREADS = 64 + 32 * EPI_WARPS;
+  static constexpr int STG_BYTES = (EPI == EPI_SWIGLU || EPI == EPI_PLAIN) ? 0 : EPI_WARPS * STG_WARP_BYTES;
   static constexpr int SMEM_LIMIT = 232448;
   static constexpr int STAGES_FIT = (SMEM_LIMIT - 1024 - BAR_BYTES - STG_BYTES) / STAGE_BYTES;
   static constexpr int STAGES = STAGES_FIT > 8 ? 8 : STAGES_FIT;
@@ -171,12 +175,10 @@ template <int BN>
 __device__ __forceinline__ void epi_swiglu8(const GemmParams& p, const Gemm8Extra& x8, int M, uint32_t t_row, int row,
                                             int n_blk, int part, int nparts, float rstd) {
   constexpr int HALF = BN / 2;
-  constexpr int CHUNKS = HALF / 32;  // 32-column MX blocks of the tile, dealt to the `nparts` (= 2) warps of a quadrant
   static_assert(HALF % 32 == 0, "whole MX blocks per tile");
-  const int c_begin = part == 0 ? 0 : ((CHUNKS + 1) / 2) * 32;
-  const int c_end = part == 0 ? ((CHUNKS + 1) / 2) * 32 : CHUNKS * 32;
+  // the tile's 32-column MX blocks are dealt round-robin to the `nparts` warps of a TMEM lane quadrant
 #pragma unroll 1
-  for (int c0 = c_begin; c0 < c_end; c0 += 32) {
+  for (int c0 = part * 32; c0 < HALF; c0 += nparts * 32) {
     float a[32];
     {
       uint32_t g[32], u[32];
@@ -277,7 +279,7 @@ __device__ __forceinline__ void epi_resid8(const GemmParams& p, const Gemm8Extra
 
 // --------------------------------------------------------------------------------- kernel
 template <int BN, int EPI, int DH>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM2_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__((Gemm8Cfg<BN, EPI>::THREADS), 1)
 te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                 const __grid_constant__ CUtensorMap tmSFA, const __grid_constant__ CUtensorMap tmSFB, const GemmParams p,
                 const Gemm8Extra x8) {
@@ -317,7 +319,7 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       }
       for (int i = 0; i < ACC; ++i) {
         mbar_init(&tfull[i], 1);
-        mbar_init(&tempty[i], 2 * 32 * GEMM2_EPI_WARPS);
+        mbar_init(&tempty[i], 2 * 32 * Cfg::EPI_WARPS);
       }
       fence_mbar_init();
     }
@@ -415,7 +417,7 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     // ===================== epilogue warps (both CTAs, own 128 rows) =====================
     const int quad = warp & 3;
     const int part = (warp - 2) >> 2;
-    constexpr int NPARTS = GEMM2_EPI_WARPS / 4;
+    constexpr int NPARTS = Cfg::EPI_WARPS / 4;
     int it = 0;
     pdl_wait();
     for (int tile = pair; tile < num_tiles; tile += num_pairs, ++it) {

@@ -343,7 +343,7 @@ cudaError_t launch_gemm8(const LaunchCtx& lc, const CUtensorMap& tmA, const CUte
   using Cfg = te::Gemm8Cfg<BN, EPI>;
   const int tiles = ((p.num_m_blk + 1) / 2) * p.num_n_blk;
   const int pairs = tiles < sm_count / 2 ? tiles : sm_count / 2;
-  return launch_k(lc, te::te_gemm8_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(te::GEMM2_THREADS), Cfg::SMEM_BYTES, st, tmA,
+  return launch_k(lc, te::te_gemm8_kernel<BN, EPI, DH>, dim3(2 * pairs), dim3(Cfg::THREADS), Cfg::SMEM_BYTES, st, tmA,
                   tmB, tmSFA, tmSFB, p, x8);
 }
 template <int BN, int EPI, int DH>
