@@ -77,3 +77,43 @@ CONFIGS = {
 
 def get_workload(cfg_id: int) -> Workload:
     return CONFIGS[int(cfg_id)]
+
+
+# ---------------------------------------------------------------- vision-tower front end
+@dataclass(frozen=True)
+class VisionConfig:
+    """Patch embedding + tower + 2x2 merger in front of the decoder (readings Q28-Q31).
+    `tower` is a decoder-shaped stack (non-causal attention, final norm on) of width d_v = tower.hidden."""
+    tower: TEModelConfig
+    patch: int            # P: pixels per patch side
+    image_h: int          # pixels; image_h / patch and image_w / patch are the (even) patch-grid sizes
+    image_w: int
+    out_hidden: int       # the decoder's hidden size (merger output)
+
+    @property
+    def grid_h(self) -> int:
+        return self.image_h // self.patch
+
+    @property
+    def grid_w(self) -> int:
+        return self.image_w // self.patch
+
+    @property
+    def patch_dim(self) -> int:
+        return self.patch * self.patch * 3
+
+    @property
+    def tokens_per_frame(self) -> int:
+        return (self.grid_h // 2) * (self.grid_w // 2)
+
+
+# CPU-sized: 32x32 image, 8x8 patches -> 4x4 patch grid -> 2x2 = 4 visual tokens of width 256 (TINY decoder)
+VISION_TINY = VisionConfig(
+    tower=TEModelConfig(n_layers=2, hidden=128, n_q_heads=2, n_kv_heads=2, head_dim=64, ffn=256,
+                        rope_sections=(8, 12, 12), final_norm=1),
+    patch=8, image_h=32, image_w=32, out_hidden=256)
+# the paper's shape: 256x256 source patch -> 16x16 grid of 16x16-pixel patches -> 8x8 = 64 visual tokens of width 2048
+VISION_FULL = VisionConfig(
+    tower=TEModelConfig(n_layers=4, hidden=1024, n_q_heads=16, n_kv_heads=16, head_dim=64, ffn=4096,
+                        rope_sections=(8, 12, 12), final_norm=1),
+    patch=16, image_h=256, image_w=256, out_hidden=2048)

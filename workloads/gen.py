@@ -140,3 +140,41 @@ def make_embeddings(w: Workload, n_tokens: int, outliers: str | None = None) -> 
     else:
         assert mode == "none"
     return x
+
+
+# ---------------------------------------------------------------- vision-tower front end
+def vision_blob_layout(v):
+    """Element offsets of the vision blob: W_pe [d_v, P*P*3] | tower blob (decoder layout, incl. gf) | W_m [hidden, 4*d_v]."""
+    d_v = v.tower.hidden
+    n_pe = d_v * v.patch_dim
+    n_tower = blob_num_elements(v.tower)
+    return {"W_pe": (0, (d_v, v.patch_dim)), "tower": (n_pe, n_tower),
+            "W_m": (n_pe + n_tower, (v.out_hidden, 4 * d_v)), "total": n_pe + n_tower + v.out_hidden * 4 * d_v}
+
+
+def make_vision_blob(v, seed: int = 11) -> np.ndarray:
+    """uint16 bf16 bits.  W_pe and W_m ~ N(0, 0.02) from Philox(key=[seed, 0xFFFE]); the tower exactly as
+    make_weight_blob(v.tower, seed)."""
+    lay = vision_blob_layout(v)
+    blob = np.empty(lay["total"], dtype=np.uint16)
+    rng = np.random.Generator(np.random.Philox(key=[seed, 0xFFFE]))
+    off, shape = lay["W_pe"]
+    blob[off:off + int(np.prod(shape))] = f32_to_bf16_bits(rng.standard_normal(int(np.prod(shape)), dtype=np.float32) * np.float32(0.02))
+    t_off, t_n = lay["tower"]
+    blob[t_off:t_off + t_n] = make_weight_blob(v.tower, seed)
+    off, shape = lay["W_m"]
+    blob[off:off + int(np.prod(shape))] = f32_to_bf16_bits(rng.standard_normal(int(np.prod(shape)), dtype=np.float32) * np.float32(0.02))
+    return blob
+
+
+def make_pixels(v, n_frames: int, seed: int = 12) -> np.ndarray:
+    """fp32 [B, H, W, 3] in [0, 1): a smooth seeded pattern plus noise (stands in for the DAVIS source patches)."""
+    rng = np.random.Generator(np.random.Philox(key=[seed, 0]))
+    yy, xx = np.meshgrid(np.arange(v.image_h, dtype=np.float32), np.arange(v.image_w, dtype=np.float32), indexing="ij")
+    out = np.empty((n_frames, v.image_h, v.image_w, 3), dtype=np.float32)
+    for b in range(n_frames):
+        f = rng.uniform(0.01, 0.2, size=(3, 2)).astype(np.float32)
+        for c in range(3):
+            out[b, :, :, c] = 0.5 + 0.35 * np.sin(f[c, 0] * yy + b) * np.cos(f[c, 1] * xx)
+    out += rng.uniform(-0.1, 0.1, size=out.shape).astype(np.float32)
+    return np.clip(out, 0.0, 0.999).astype(np.float32)
