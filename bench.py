@@ -252,6 +252,47 @@ def measure_overlap(torch, te_step, side, te_ms, reps: int = 20):
             "wall_over_max": t_both / max(t_main, t_side), "reps": reps}
 
 
+# ------------------------------------------------------------- vision-tower front end
+def measure_vision(torch, te, stream, n_frames: int, reps: int = 50):
+    """te_encode_image on the paper-shaped front end (W.VISION_FULL: 256x256 source patch -> 16x16 patches -> tower of
+    4 non-causal blocks, d_v = 1024 -> 2x2 merger -> 64 visual tokens of width 2048) for one batch of
+    frames, device-resident pixels, CUDA events on the launching stream."""
+    v = W.VISION_FULL
+    enc = te.VisionEncoder(v, n_frames)
+    enc.load_weights(W.make_vision_blob(v))
+    px = torch.from_numpy(W.make_pixels(v, n_frames)).cuda()
+    emb = torch.empty((n_frames * v.tokens_per_frame, v.out_hidden), dtype=torch.float32, device="cuda")
+    with torch.cuda.stream(stream):
+        for _ in range(5):
+            enc.encode_image(n_frames, px, None, emb, stream.cuda_stream)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        n0 = te.te_vision_kernel_launches(enc.v)
+        for a, b in evs:
+            a.record(stream)
+            enc.encode_image(n_frames, px, None, emb, stream.cuda_stream)
+            b.record(stream)
+    torch.cuda.synchronize()
+    launches = te.te_vision_kernel_launches(enc.v) - n0
+    ms = [a.elapsed_time(b) for a, b in evs]
+    enc.close()
+    t = sum(ms) / len(ms) / 1000.0
+    mv = v.tower
+    S = v.grid_h * v.grid_w
+    n_patch = n_frames * S
+    flops = (2.0 * n_patch * v.patch_dim * mv.hidden                                         # patch embedding
+             + mv.n_layers * (gemm_flops_per_token_layer(mv) * n_patch
+                              + n_frames * 4.0 * mv.head_dim * mv.n_q_heads * S * S)         # non-causal: all S^2 scores
+             + 2.0 * n_frames * v.tokens_per_frame * 4 * mv.hidden * v.out_hidden)           # merger
+    pk = load_peaks()
+    return {"metric": "vision_front_end_frames_per_s", "value": n_frames / t, "unit": UNIT, "ms_per_call": 1000.0 * t,
+            "ms_per_call_min": min(ms), "reps": reps, "gpu_launches_per_call": launches // reps,
+            "config": {"workload": f"vision_full_B{n_frames}", "image": f"{v.image_h}x{v.image_w}x3 fp32", "patch": v.patch,
+                       "patches_per_frame": S, "tower": f"{mv.n_layers} non-causal blocks, d_v {mv.hidden}, "
+                       f"{mv.n_q_heads} heads x {mv.head_dim}, ffn {mv.ffn}", "visual_tokens_per_frame": v.tokens_per_frame,
+                       "out_hidden": v.out_hidden},
+            "flops": flops, "achieved_tflops": flops / t / 1e12, "frac_of_burst": flops / (pk["tf_burst"] * 1e12) / t}
+
+
 # ------------------------------------------------------------------------------------------ main
 def run_reference(args, w, blob, tl, T, emb, rank):
     if rank != 0:
@@ -498,6 +539,8 @@ def main():
                                "frac_of_sustained": max(f3 / (pk["tf_sustained"] * 1e12),
                                                         (wb3 + ab3) / (pk["hbm_gbs"] * 1e9)) / t3},
         }
+        # the same frames' visual tokens from pixels: te_encode_image, B = this config's frames
+        secondary[f"vision_front_end_B{w.n_frames}"] = measure_vision(torch, te, stream, w.n_frames)
 
     if rank != 0:
         if dist is not None:

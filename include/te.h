@@ -69,6 +69,9 @@ typedef struct te_config {
                                    in_features; the GEMMs' A operands (x*g, attention output, SwiGLU output) are
                                    quantised the same way in the producing epilogues; attention, accumulation and the
                                    residual stream are unchanged.  Needs Hq/Hkv a power of two <= 8 and no prefix      */
+  int32_t non_causal;           /* 0 (default): causal attention by sequence index within the frame.  1: every query sees
+                                   every key of its own frame (the vision tower's blocks, te_vision_create; DESIGN.md §3
+                                   Q29); needs max_prefix_tokens == 0                                                  */
 } te_config;
 
 /* Exact size in bytes of the canonical weight blob for cfg (see te_load_weights). */
@@ -191,6 +194,47 @@ enum {
   TE_KCLASS_GATEUP = 5, TE_KCLASS_DOWN = 6, TE_KCLASS_FINAL_NORM = 7, TE_KCLASS_COUNT = 8
 };
 int te_kernel_times(te_handle* h, float* ms_sum, int32_t* n_launches);
+
+/* ---- Vision-tower front end.  The paper's TE takes the frame itself: the template's
+ * image-pad token is "processed by Qwen3-VL's vision tower" and a 256x256 source patch becomes ~64
+ * visual tokens.  The paper fixes no shape or equation of the tower; the front end built here is
+ * DESIGN.md §3 readings Q28-Q31 (oracle: oracle/te_vision.py):
+ *   patch embedding   pixels cut into P x P patches (row-major patch grid, (dy, dx, channel) inside a patch),
+ *                     x0 = patches * W_pe^T, W_pe [d_v, P*P*3], no bias
+ *   tower             `tower.n_layers` blocks of the decoder's pre-norm block (te_config `tower`: hidden = d_v) with
+ *                     NON-causal attention and rotary ids (0, py, px) on the patch grid, then the final RMSNorm
+ *   merger            each 2 x 2 block of neighbouring patches concatenated ((dy, dx) row-major, 4*d_v values) and
+ *                     multiplied by W_m [out_hidden, 4*d_v]; merged tokens row-major on the (gh/2) x (gw/2) grid
+ * Every step runs on the device in the stack's kernels (tcgen05 GEMMs, the tower = te_encode with non_causal = 1). */
+typedef struct te_vision te_vision; /* opaque; owned by the library */
+typedef struct te_vision_config {
+  te_config tower;      /* the tower's blocks: hidden = d_v, heads, ffn, rope sections, n_layers, rms_eps, rope_theta;
+                           final_norm / non_causal / capacities are set by the library                            */
+  int32_t patch;        /* P: pixels per patch side; P*P*3 must be a multiple of 64                               */
+  int32_t image_h, image_w; /* pixels; multiples of 2*P; (image_h/P) * (image_w/P) <= 256 patches per frame        */
+  int32_t out_hidden;   /* the decoder's hidden size (merger output width); multiple of 128                        */
+  int32_t max_frames;   /* capacity: frames per call                                                               */
+} te_vision_config;
+
+/* Exact size in bytes of the vision blob: W_pe [d_v, P*P*3] | the tower's blob (te_load_weights layout of
+ * `tower`, including gf) | W_m [out_hidden, 4*d_v], all bf16 row-major [out_features, in_features].  0 on a bad config. */
+size_t te_vision_blob_bytes(const te_vision_config* cfg);
+int te_vision_create(const te_vision_config* cfg, int device, te_vision** out);
+/* bf16_blob: HOST or DEVICE; n_bytes must equal te_vision_blob_bytes(cfg).  Synchronous; the blob may be freed. */
+int te_vision_load_weights(te_vision* v, const void* bf16_blob, size_t n_bytes);
+/* Encode the frames' images into the decoder's visual-token embeddings, IN PLACE in the decoder's input:
+ *   pixels     DEVICE fp32 [n_frames, image_h, image_w, 3]
+ *   text_lens  DEVICE int32 [n_frames] (the decoder call's text_lens) or NULL (= all zero)
+ *   embeds     DEVICE fp32 [T, out_hidden], the packed input of te_encode: the n_vis = (image_h/2P)*(image_w/2P)
+ *              merged tokens of frame b are written to rows cu[b] .. cu[b] + n_vis, cu[b] = b*n_vis + sum of
+ *              text_lens[0..b) — computed on the device; the text rows are not touched
+ * Enqueues on cuda_stream and returns (no synchronisation, no device->host copy). */
+int te_encode_image(te_vision* v, int32_t n_frames, const float* pixels, const int32_t* text_lens, float* embeds,
+                    void* cuda_stream);
+/* Kernels launched so far on behalf of te_encode_image (the tower's graph nodes included). */
+int64_t te_vision_kernel_launches(te_vision* v);
+const char* te_vision_last_error(te_vision* v);
+void te_vision_destroy(te_vision* v);
 
 void te_destroy(te_handle* h);
 const char* te_strerror(int code);

@@ -85,6 +85,16 @@ int te_debug_mx_quantise(int device, const void* src_bf16, int32_t rows, int32_t
 int te_debug_gemm_mxfp8(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m, int32_t n,
                         int32_t k, int32_t block_n);
 
+/* Vision front end taps (te_encode_image): synchronises and copies to `dst` (HOST). */
+enum {
+  TE_VTAP_PATCH_EMBEDS = 0, /* fp32 [n_frames*gh*gw, d_v]   x0 = patches * W_pe^T                  */
+  TE_VTAP_TOWER_OUT = 1,    /* fp32 [n_frames*gh*gw, d_v]   tower output after the final RMSNorm   */
+  TE_VTAP_MERGED = 2        /* fp32 [n_frames*n_vis, out_hidden]  merger output before the scatter */
+};
+int te_vision_debug_tap(te_vision* v, int what, void* dst_host, size_t n_bytes);
+/* The tower's te_handle (owned by `v`), for te_set_option / te_debug_tap on the tower itself. */
+te_handle* te_vision_debug_tower(te_vision* v);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,9 +38,12 @@ EXPORTS = [
     "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host",
     "te_encode_host_submit", "te_encode_host_wait", "te_query_async_error", "te_set_option", "te_kernel_launches",
     "te_graph_captures", "te_dispatch_info", "te_kernel_times", "te_destroy", "te_strerror", "te_last_error",
+    "te_vision_blob_bytes", "te_vision_create", "te_vision_load_weights", "te_encode_image", "te_vision_kernel_launches",
+    "te_vision_last_error", "te_vision_destroy",
 ]
 DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide",
-                 "te_debug_mx_quantise", "te_debug_gemm_mxfp8"]
+                 "te_debug_mx_quantise", "te_debug_gemm_mxfp8", "te_vision_debug_tap", "te_vision_debug_tower"]
+TE_VTAP_PATCH_EMBEDS, TE_VTAP_TOWER_OUT, TE_VTAP_MERGED = 0, 1, 2
 TE_DTYPE_BF16, TE_DTYPE_MXFP8 = 0, 1
 
 
@@ -53,7 +56,15 @@ class TEConfig(Structure):
         ("rms_eps", c_float), ("rope_theta", c_double),
         ("max_frames", c_int32), ("max_tokens", c_int32), ("max_tokens_per_frame", c_int32),
         ("final_norm", c_int32), ("rope_interleaved", c_int32), ("max_prefix_tokens", c_int32),
-        ("weight_dtype", c_int32),
+        ("weight_dtype", c_int32), ("non_causal", c_int32),
+    ]
+
+
+class TEVisionConfig(Structure):
+    """Mirror of `te_vision_config` (include/te.h)."""
+    _fields_ = [
+        ("tower", TEConfig), ("patch", c_int32), ("image_h", c_int32), ("image_w", c_int32),
+        ("out_hidden", c_int32), ("max_frames", c_int32),
     ]
 
 
@@ -118,6 +129,24 @@ def lib() -> ctypes.CDLL:
     L.te_debug_mx_quantise.argtypes = [c_int, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
     L.te_debug_gemm_mxfp8.restype = c_int
     L.te_debug_gemm_mxfp8.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
+    L.te_vision_blob_bytes.restype = c_size_t
+    L.te_vision_blob_bytes.argtypes = [POINTER(TEVisionConfig)]
+    L.te_vision_create.restype = c_int
+    L.te_vision_create.argtypes = [POINTER(TEVisionConfig), c_int, POINTER(c_void_p)]
+    L.te_vision_load_weights.restype = c_int
+    L.te_vision_load_weights.argtypes = [c_void_p, c_void_p, c_size_t]
+    L.te_encode_image.restype = c_int
+    L.te_encode_image.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p]
+    L.te_vision_kernel_launches.restype = c_int64
+    L.te_vision_kernel_launches.argtypes = [c_void_p]
+    L.te_vision_last_error.restype = c_char_p
+    L.te_vision_last_error.argtypes = [c_void_p]
+    L.te_vision_destroy.restype = None
+    L.te_vision_destroy.argtypes = [c_void_p]
+    L.te_vision_debug_tap.restype = c_int
+    L.te_vision_debug_tap.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
+    L.te_vision_debug_tower.restype = c_void_p
+    L.te_vision_debug_tower.argtypes = [c_void_p]
     L.te_destroy.restype = None
     L.te_destroy.argtypes = [c_void_p]
     L.te_strerror.restype = c_char_p
@@ -153,13 +182,21 @@ def _check(code: int, h=None):
 
 
 def make_config(model, max_frames: int, max_tokens: int, max_tokens_per_frame: int = 256,
-                final_norm: int | None = None, max_prefix_tokens: int = 0, weight_dtype: int = 0) -> TEConfig:
+                final_norm: int | None = None, max_prefix_tokens: int = 0, weight_dtype: int = 0,
+                non_causal: int = 0) -> TEConfig:
     """TEConfig from a workloads.TEModelConfig-like object (duck-typed)."""
     s_t, s_h, s_w = model.rope_sections
     return TEConfig(model.n_layers, model.hidden, model.n_q_heads, model.n_kv_heads, model.head_dim,
                     model.ffn, s_t, s_h, s_w, model.rms_eps, model.rope_theta, max_frames, max_tokens,
                     max_tokens_per_frame, model.final_norm if final_norm is None else final_norm,
-                    1 if getattr(model, "rope_interleaved", False) else 0, max_prefix_tokens, weight_dtype)
+                    1 if getattr(model, "rope_interleaved", False) else 0, max_prefix_tokens, weight_dtype, non_causal)
+
+
+def make_vision_config(vision, max_frames: int) -> TEVisionConfig:
+    """TEVisionConfig from a workloads.VisionConfig-like object (duck-typed); the library sets the tower's capacities."""
+    tower = make_config(vision.tower, max_frames, max_frames * vision.grid_h * vision.grid_w,
+                        vision.grid_h * vision.grid_w, final_norm=1, non_causal=1)
+    return TEVisionConfig(tower, vision.patch, vision.image_h, vision.image_w, vision.out_hidden, max_frames)
 
 
 # ---------------------------------------------------------------- C-ABI names, marshalling only
@@ -271,6 +308,58 @@ def te_destroy(h):
     lib().te_destroy(h)
 
 
+def _vcheck(code: int, v=None):
+    if code != TE_OK:
+        L = lib()
+        msg = L.te_strerror(code).decode()
+        if v:
+            extra = L.te_vision_last_error(v).decode()
+            if extra:
+                msg += f" ({extra})"
+        raise TEError(code, msg)
+
+
+def te_vision_blob_bytes(cfg: TEVisionConfig) -> int:
+    return int(lib().te_vision_blob_bytes(byref(cfg)))
+
+
+def te_vision_create(cfg: TEVisionConfig, device: int = 0) -> c_void_p:
+    v = c_void_p()
+    _vcheck(lib().te_vision_create(byref(cfg), device, byref(v)))
+    return v
+
+
+def te_vision_load_weights(v, blob, n_bytes: int | None = None):
+    if n_bytes is None:
+        n_bytes = int(blob.nbytes) if hasattr(blob, "nbytes") else int(blob.numel() * blob.element_size())
+    _vcheck(lib().te_vision_load_weights(v, _ptr(blob), n_bytes), v)
+
+
+def te_encode_image(v, n_frames, pixels, text_lens, embeds, stream=None):
+    """pixels: DEVICE fp32 [B, H, W, 3]; text_lens: DEVICE int32 [B] or None; embeds: DEVICE fp32 [T, out_hidden]."""
+    _vcheck(lib().te_encode_image(v, n_frames, _ptr(pixels), _ptr(text_lens), _ptr(embeds), _ptr(stream)), v)
+
+
+def te_vision_kernel_launches(v) -> int:
+    return int(lib().te_vision_kernel_launches(v))
+
+
+def te_vision_last_error(v) -> str:
+    return lib().te_vision_last_error(v).decode()
+
+
+def te_vision_debug_tap(v, what: int, dst_host):
+    _vcheck(lib().te_vision_debug_tap(v, what, _ptr(dst_host), int(dst_host.nbytes)), v)
+
+
+def te_vision_debug_tower(v) -> c_void_p:
+    return c_void_p(lib().te_vision_debug_tower(v))
+
+
+def te_vision_destroy(v):
+    lib().te_vision_destroy(v)
+
+
 def te_strerror(code: int) -> str:
     return lib().te_strerror(code).decode()
 
@@ -284,10 +373,10 @@ class TextEncoder:
 
     def __init__(self, model, max_frames: int, max_tokens: int, device: int = 0,
                  max_tokens_per_frame: int = 256, final_norm: int | None = None, max_prefix_tokens: int = 0,
-                 weight_dtype: int = 0):
+                 weight_dtype: int = 0, non_causal: int = 0):
         self.model = model
         self.cfg = make_config(model, max_frames, max_tokens, max_tokens_per_frame, final_norm, max_prefix_tokens,
-                               weight_dtype)
+                               weight_dtype, non_causal)
         self.h = te_create(self.cfg, device)
 
     def load_weights(self, blob):
@@ -312,6 +401,32 @@ class TextEncoder:
         if self.h:
             te_destroy(self.h)
             self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class VisionEncoder:
+    """Convenience owner of a vision front end (create -> load -> encode_image -> destroy)."""
+
+    def __init__(self, vision, max_frames: int, device: int = 0):
+        self.vision = vision
+        self.cfg = make_vision_config(vision, max_frames)
+        self.v = te_vision_create(self.cfg, device)
+
+    def load_weights(self, blob):
+        te_vision_load_weights(self.v, blob)
+
+    def encode_image(self, n_frames, pixels, text_lens, embeds, stream=None):
+        te_encode_image(self.v, n_frames, pixels, text_lens, embeds, stream)
+
+    def close(self):
+        if self.v:
+            te_vision_destroy(self.v)
+            self.v = None
 
     def __del__(self):
         try:

@@ -28,6 +28,7 @@ struct AttnParams {
   const __nv_bfloat16* kv_prefix;
   int prefix_len;
   int ld_prefix;
+  int non_causal;  // 1: every query sees all keys of its frame (te_config.non_causal); 0: causal by index
 };
 
 // GH = q heads served by one CTA (they share one kv head: GH divides Hq/Hkv); 4 warps per head.
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
   const __nv_bfloat16* sQh = sQ + (hl * ATT_BQ + wr * 16) * ROW;
 
   // causal: combined keys [0, P + q0 + 64), capped at the frame's end
-  const int n_kv_blocks = (min(P + q0 + ATT_BQ, P + S) + ATT_BKV - 1) / ATT_BKV;
+  const int n_kv_blocks = ((p.non_causal ? P + S : min(P + q0 + ATT_BQ, P + S)) + ATT_BKV - 1) / ATT_BKV;
   for (int kb = 0; kb < n_kv_blocks; ++kb) {
     if (kb + 1 < n_kv_blocks) {
       load_kv(kb + 1, (kb + 1) & 1);  // stage (kb+1)&1 was released by the barrier ending iteration kb-1
@@ -176,14 +177,16 @@ __global__ void __launch_bounds__(128 * GH, 2) te_attn_kernel(const AttnParams p
     }
     // ---- causal mask (only blocks reaching past the first query row's diagonal need it) + online softmax:
     // query row n sees combined keys 0 .. P + n
-    if (k0 + ATT_BKV - 1 > P + q0) {
+    // (non-causal: every row sees keys 0 .. P + S - 1; only the frame's last block has keys to mask)
+    if (p.non_causal ? (k0 + ATT_BKV > P + S) : (k0 + ATT_BKV - 1 > P + q0)) {
+      const int lim0 = p.non_causal ? S - 1 : qrow0, lim1 = p.non_causal ? S - 1 : qrow0 + 8;
 #pragma unroll
       for (int nt = 0; nt < ATT_BKV / 8; ++nt) {
         const int key = k0 + nt * 8 + 2 * t - P;
-        if (key > qrow0) s[nt][0] = -INFINITY;
-        if (key + 1 > qrow0) s[nt][1] = -INFINITY;
-        if (key > qrow0 + 8) s[nt][2] = -INFINITY;
-        if (key + 1 > qrow0 + 8) s[nt][3] = -INFINITY;
+        if (key > lim0) s[nt][0] = -INFINITY;
+        if (key + 1 > lim0) s[nt][1] = -INFINITY;
+        if (key > lim1) s[nt][2] = -INFINITY;
+        if (key + 1 > lim1) s[nt][3] = -INFINITY;
       }
     }
     float mx[2] = {-INFINITY, -INFINITY};

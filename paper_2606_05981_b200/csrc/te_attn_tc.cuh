@@ -28,6 +28,7 @@ struct AttnTcParams {
   int n_q_heads, n_kv_heads;
   int g_shift;  // log2(Hq / Hkv)
   float scale_log2;  // log2(e) / sqrt(dh)
+  int non_causal;    // 1: every query sees all keys of its frame (vision tower, te_config.non_causal); 0: causal
   // Shared text prefix (te_encode_prefix), handled as a SECOND launch of this kernel per layer:
   //   launch 1 (prefix_mode 0, stats != null): frame-local causal attention as usual, plus the row statistics
   //            (max raw score, sum of exp) of every (token, q head) -> stats[T, Hq]
@@ -132,7 +133,7 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int P16 = (p.prefix_len + 15) & ~15;
   // keys tile j can see: positions < PT * (j + 1), rounded to the MMA granularity (16) and capped at the frame;
   // prefix mode: all P prefix keys for every tile
-  auto nk_of = [&](int j) { return p.prefix_mode ? P16 : min(S16, (PT * (j + 1) + 15) & ~15); };
+  auto nk_of = [&](int j) { return p.prefix_mode ? P16 : (p.non_causal ? S16 : min(S16, (PT * (j + 1) + 15) & ~15)); };
   const int kv_row0 = p.prefix_mode ? 0 : seq0;                                   // first K/V row in tmKV
   const int k_col0 = (p.prefix_mode ? kvh : p.n_q_heads + kvh) * DH;              // this kv head's K columns
   const int v_col0 = (p.prefix_mode ? p.n_kv_heads + kvh : p.n_q_heads + p.n_kv_heads + kvh) * DH;
@@ -223,7 +224,7 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       const int j = split + i * n_split;
       const int nk = nk_of(j);
       const int pos = j * PT + pr;      // position of this row's query inside the frame
-      const int lim = p.prefix_mode ? p.prefix_len - 1 : min(pos, S - 1);  // keys 0..lim are visible
+      const int lim = p.prefix_mode ? p.prefix_len - 1 : (p.non_causal ? S - 1 : min(pos, S - 1));  // keys 0..lim are visible
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + 256 * t;
       mbar_wait(&s_full[t], u & 1);
       tc_fence_after();

@@ -20,6 +20,7 @@
 #include "te_gemm_splitk.cuh"
 #include "te_gemm_wide.cuh"
 #include "te_prep.cuh"
+#include "te_vision.cuh"
 
 namespace {
 
@@ -212,6 +213,26 @@ struct te_handle {
   std::string info;
 };
 
+// Vision-tower front end (te_vision_create .. te_encode_image, DESIGN.md §3 Q28-Q31).
+struct te_vision {
+  te_vision_config cfg{};
+  int device = 0;
+  int sm_count = 0;
+  bool loaded = false;
+  te_handle* tower = nullptr;       // the tower's blocks: the decoder stack with non_causal = 1, final_norm = 1
+  int gh = 0, gw = 0, n_vis = 0, patch_dim = 0, d_v = 0;
+  int rows_pe = 0, rows_m = 0;      // capacity rows of the two GEMM A operands (multiples of 256)
+  __nv_bfloat16 *w_pe = nullptr, *w_m = nullptr;  // [d_v, P*P*3], [out_hidden, 4*d_v]
+  __nv_bfloat16 *a_pe = nullptr, *a_m = nullptr;  // [rows_pe, P*P*3] patches, [rows_m, 4*d_v] merged tower rows
+  float *x0 = nullptr, *tower_out = nullptr, *vis = nullptr;
+  int32_t* zero_lens = nullptr;     // [max_frames] the tower's frames carry no text
+  CUtensorMap tmA_pe, tmA_m, tmB_pe, tmB_m;
+  int bn_pe = 128, pair_pe = 0, bn_m = 128, pair_m = 0;
+  int last_B = 0;
+  long long launches = 0;
+  std::string err;
+};
+
 namespace {
 
 #define TE_CUDA(h, expr)                                                                      \
@@ -247,6 +268,7 @@ int validate_config(const te_config& c) {
   if ((c.n_q_heads * c.head_dim) % 64 != 0) return TE_ERR_UNSUPPORTED;
   if (c.max_tokens_per_frame > 256) return TE_ERR_UNSUPPORTED;
   if (c.weight_dtype < 0 || c.weight_dtype > 1) return TE_ERR_INVALID_ARG;
+  if (c.non_causal < 0 || c.non_causal > 1 || (c.non_causal && c.max_prefix_tokens > 0)) return TE_ERR_INVALID_ARG;
   if (c.weight_dtype == 1) {
     // MXFP8: 128-element K chunks everywhere; the quantising attention epilogue exists in the tcgen05 kernel only
     // (G = Hq/Hkv a power of two <= 8); no cached prefix (its merge pass re-reads a bf16 output)
@@ -718,7 +740,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       if (pl.attn_tc) {
         te::AttnTcParams tp{};
         tp.out = h->attn; tp.cu_seqlens = h->cu; tp.n_q_heads = c.n_q_heads; tp.n_kv_heads = c.n_kv_heads;
-        tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2;
+        tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2; tp.non_causal = c.non_causal;
         tp.stats = P > 0 ? h->attn_stats : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
         tp.out8 = pl.mx ? h->attn8 : nullptr; tp.sf_out = h->sf_attn;
         TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st)
@@ -733,7 +755,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         te::AttnParams ap{};
         ap.qkv = h->qkv; ap.out = h->attn; ap.cu_seqlens = h->cu; ap.ld = n_qkv; ap.n_q_heads = c.n_q_heads;
         ap.n_kv_heads = c.n_kv_heads; ap.scale_log2 = scale_log2;
-        ap.prefix_len = P; ap.ld_prefix = n_kv;
+        ap.prefix_len = P; ap.ld_prefix = n_kv; ap.non_causal = c.non_causal;
         ap.kv_prefix = P > 0 ? h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv : nullptr;
         TE_CUDA(h, launch_attn_any(lc, dh, ap, pl.q_blocks, n_frames, st));
       }
@@ -1556,6 +1578,185 @@ int te_debug_gemm_mxfp8(int device, const void* a, const void* b, float* cmat, i
                                  : launch_gemm8<128, te::EPI_PLAIN, 128>(lc, ta, tb, tsa, tsb, p, x8, sms, nullptr);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   return done(e == cudaSuccess ? TE_OK : TE_ERR_CUDA);
+}
+
+// ---------------------------------------------------------------- vision-tower front end (NEXT-4)
+static int vision_validate(const te_vision_config& v, te_config* tower_cfg) {
+  if (v.patch < 1 || v.image_h < 1 || v.image_w < 1 || v.out_hidden < 1 || v.max_frames < 1) return TE_ERR_INVALID_ARG;
+  if (v.image_h % (2 * v.patch) != 0 || v.image_w % (2 * v.patch) != 0) return TE_ERR_INVALID_ARG;
+  const int gh = v.image_h / v.patch, gw = v.image_w / v.patch;
+  if (gh * gw > 256) return TE_ERR_UNSUPPORTED;                       // one frame's patches = one attention frame
+  if ((v.patch * v.patch * 3) % 64 != 0) return TE_ERR_UNSUPPORTED;   // K of the patch-embedding GEMM
+  if (v.out_hidden % 128 != 0) return TE_ERR_UNSUPPORTED;
+  te_config t = v.tower;
+  t.max_frames = v.max_frames;
+  t.max_tokens = v.max_frames * gh * gw;
+  t.max_tokens_per_frame = gh * gw;
+  t.final_norm = 1;
+  t.non_causal = 1;
+  t.max_prefix_tokens = 0;
+  t.weight_dtype = 0;
+  const int rc = validate_config(t);
+  if (rc != TE_OK) return rc;
+  if (t.hidden % 128 != 0) return TE_ERR_UNSUPPORTED;
+  *tower_cfg = t;
+  return TE_OK;
+}
+
+// C[M, N] fp32 = A[M, K] * B[N, K]^T on the stack's tcgen05 GEMM (plain epilogue); M is fixed per launch (no DynParams)
+static cudaError_t vision_gemm(const CUtensorMap& ta, const CUtensorMap& tb, float* cmat, int m, int n, int k, int bn, int pair,
+                               int sms, cudaStream_t st) {
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / bn;
+  p.c = cmat; p.ld_c = n;
+  const LaunchCtx lc;  // plain launches: these kernels do not take part in the stack's PDL chain
+  return launch_gemm_bn<te::EPI_PLAIN>(lc, bn, pair, 128, ta, tb, p, sms, st);
+}
+
+size_t te_vision_blob_bytes(const te_vision_config* cfg) {
+  te_config t;
+  if (!cfg || vision_validate(*cfg, &t) != TE_OK) return 0;
+  const size_t d_v = t.hidden, pd = (size_t)cfg->patch * cfg->patch * 3;
+  return (d_v * pd + blob_elems(t) + (size_t)cfg->out_hidden * 4 * d_v) * sizeof(bf16);
+}
+
+int te_vision_create(const te_vision_config* cfg, int device, te_vision** out) {
+  if (!cfg || !out) return TE_ERR_INVALID_ARG;
+  *out = nullptr;
+  te_config t;
+  int rc = vision_validate(*cfg, &t);
+  if (rc != TE_OK) return rc;
+  te_handle* tower = nullptr;
+  rc = te_create(&t, device, &tower);
+  if (rc != TE_OK) return rc;
+  te_vision* v = new te_vision();
+  v->cfg = *cfg;
+  v->cfg.tower = t;
+  v->device = device;
+  v->sm_count = tower->sm_count;
+  v->tower = tower;
+  v->gh = cfg->image_h / cfg->patch;
+  v->gw = cfg->image_w / cfg->patch;
+  v->n_vis = (v->gh / 2) * (v->gw / 2);
+  v->patch_dim = cfg->patch * cfg->patch * 3;
+  v->d_v = t.hidden;
+  v->rows_pe = (cfg->max_frames * v->gh * v->gw + 255) / 256 * 256;
+  v->rows_m = (cfg->max_frames * v->n_vis + 255) / 256 * 256;
+  auto fail = [&](int code) {
+    te_vision_destroy(v);
+    return code;
+  };
+  const size_t d_v = v->d_v, pd = v->patch_dim, oh = cfg->out_hidden;
+#define TE_VALLOC(ptr, bytes) \
+  if (cudaMalloc(reinterpret_cast<void**>(&(ptr)), (bytes)) != cudaSuccess) return fail(TE_ERR_CUDA)
+  TE_VALLOC(v->w_pe, d_v * pd * sizeof(bf16));
+  TE_VALLOC(v->w_m, oh * 4 * d_v * sizeof(bf16));
+  TE_VALLOC(v->a_pe, (size_t)v->rows_pe * pd * sizeof(bf16));
+  TE_VALLOC(v->a_m, (size_t)v->rows_m * 4 * d_v * sizeof(bf16));
+  TE_VALLOC(v->x0, (size_t)v->rows_pe * d_v * sizeof(float));
+  TE_VALLOC(v->tower_out, (size_t)v->rows_pe * d_v * sizeof(float));
+  TE_VALLOC(v->vis, (size_t)v->rows_m * oh * sizeof(float));
+  TE_VALLOC(v->zero_lens, (size_t)cfg->max_frames * sizeof(int32_t));
+#undef TE_VALLOC
+  // rows past a call's patches are multiplied (never stored) by the tile-granular GEMMs: start them finite
+  if (cudaMemset(v->a_pe, 0, (size_t)v->rows_pe * pd * sizeof(bf16)) != cudaSuccess ||
+      cudaMemset(v->a_m, 0, (size_t)v->rows_m * 4 * d_v * sizeof(bf16)) != cudaSuccess ||
+      cudaMemset(v->zero_lens, 0, (size_t)cfg->max_frames * sizeof(int32_t)) != cudaSuccess)
+    return fail(TE_ERR_CUDA);
+  // tile shapes of the two GEMMs: CTA pairs (256-row tiles) once there are >= 1024 rows, 256-wide tiles when N allows
+  v->bn_pe = (d_v % 256 == 0) ? 256 : 128;
+  v->bn_m = (oh % 256 == 0) ? 256 : 128;
+  v->pair_pe = v->rows_pe >= 1024;
+  v->pair_m = v->rows_m >= 1024;
+  if (!make_tmap(&v->tmA_pe, v->a_pe, v->rows_pe, pd, te::GEMM_BM) || !make_tmap(&v->tmA_m, v->a_m, v->rows_m, 4 * d_v, te::GEMM_BM) ||
+      !make_tmap(&v->tmB_pe, v->w_pe, d_v, pd, v->pair_pe ? v->bn_pe / 2 : v->bn_pe) ||
+      !make_tmap(&v->tmB_m, v->w_m, oh, 4 * d_v, v->pair_m ? v->bn_m / 2 : v->bn_m))
+    return fail(TE_ERR_CUDA);
+  *out = v;
+  return TE_OK;
+}
+
+int te_vision_load_weights(te_vision* v, const void* blob, size_t n_bytes) {
+  if (!v || !blob) return TE_ERR_INVALID_ARG;
+  if (n_bytes != te_vision_blob_bytes(&v->cfg)) return TE_ERR_BLOB_SIZE;
+  TE_CUDA(v, cudaSetDevice(v->device));
+  v->loaded = false;
+  const size_t n_pe = (size_t)v->d_v * v->patch_dim, n_tower = blob_elems(v->cfg.tower);
+  const size_t n_m = (size_t)v->cfg.out_hidden * 4 * v->d_v;
+  const bf16* src = static_cast<const bf16*>(blob);
+  TE_CUDA(v, cudaMemcpy(v->w_pe, src, n_pe * sizeof(bf16), cudaMemcpyDefault));
+  const int rc = te_load_weights(v->tower, src + n_pe, n_tower * sizeof(bf16));
+  if (rc != TE_OK) {
+    v->err = std::string("tower: ") + v->tower->err;
+    return rc;
+  }
+  TE_CUDA(v, cudaMemcpy(v->w_m, src + n_pe + n_tower, n_m * sizeof(bf16), cudaMemcpyDefault));
+  v->loaded = true;
+  return TE_OK;
+}
+
+int te_encode_image(te_vision* v, int32_t n_frames, const float* pixels, const int32_t* text_lens, float* embeds,
+                    void* cuda_stream) {
+  if (!v || !pixels || !embeds) return TE_ERR_INVALID_ARG;
+  if (!v->loaded) return TE_ERR_NOT_LOADED;
+  if (n_frames < 1 || n_frames > v->cfg.max_frames) return TE_ERR_INVALID_ARG;
+  TE_CUDA(v, cudaSetDevice(v->device));
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int gh = v->gh, gw = v->gw, d_v = v->d_v;
+  const int n_patch = n_frames * gh * gw, n_merged = n_frames * v->n_vis;
+  v->last_B = n_frames;
+  // Q28: patches -> bf16 rows, x0 = patches * W_pe^T
+  te::te_patchify_kernel<<<n_patch, 256, 0, st>>>(pixels, v->a_pe, v->cfg.image_h, v->cfg.image_w, v->cfg.patch, gh, gw);
+  TE_CUDA(v, cudaGetLastError());
+  TE_CUDA(v, vision_gemm(v->tmA_pe, v->tmB_pe, v->x0, n_patch, d_v, v->patch_dim, v->bn_pe, v->pair_pe, v->sm_count, st));
+  // Q29: the tower = the stack over frames of gh*gw patches with no text, non-causal, ids (0, py, px), final norm
+  const long long before = v->tower->launches;
+  const int rc = te_encode(v->tower, n_frames, gh, gw, v->x0, v->zero_lens, n_patch, v->tower_out, st);
+  if (rc != TE_OK) {
+    v->err = std::string("tower: ") + v->tower->err;
+    return rc;
+  }
+  // Q30: 2 x 2 neighbours side by side -> W_m -> the visual rows of the decoder's packed input
+  te::te_merge2x2_kernel<<<n_merged, 256, 0, st>>>(v->tower_out, v->a_m, gh, gw, d_v);
+  TE_CUDA(v, cudaGetLastError());
+  TE_CUDA(v, vision_gemm(v->tmA_m, v->tmB_m, v->vis, n_merged, v->cfg.out_hidden, 4 * d_v, v->bn_m, v->pair_m, v->sm_count, st));
+  te::te_scatter_visual_kernel<<<n_merged, 256, 0, st>>>(v->vis, embeds, text_lens, v->n_vis, v->cfg.out_hidden);
+  TE_CUDA(v, cudaGetLastError());
+  v->launches += 5 + (v->tower->launches - before);
+  return TE_OK;
+}
+
+int64_t te_vision_kernel_launches(te_vision* v) { return v ? v->launches : 0; }
+const char* te_vision_last_error(te_vision* v) { return v ? v->err.c_str() : ""; }
+te_handle* te_vision_debug_tower(te_vision* v) { return v ? v->tower : nullptr; }
+
+int te_vision_debug_tap(te_vision* v, int what, void* dst, size_t n_bytes) {
+  if (!v || !dst || v->last_B == 0) return TE_ERR_INVALID_ARG;
+  const size_t n_patch = (size_t)v->last_B * v->gh * v->gw, n_merged = (size_t)v->last_B * v->n_vis;
+  const void* src = nullptr;
+  size_t need = 0;
+  switch (what) {
+    case TE_VTAP_PATCH_EMBEDS: src = v->x0; need = n_patch * v->d_v * sizeof(float); break;
+    case TE_VTAP_TOWER_OUT: src = v->tower_out; need = n_patch * v->d_v * sizeof(float); break;
+    case TE_VTAP_MERGED: src = v->vis; need = n_merged * v->cfg.out_hidden * sizeof(float); break;
+    default: return TE_ERR_INVALID_ARG;
+  }
+  if (n_bytes != need) return TE_ERR_INVALID_ARG;
+  TE_CUDA(v, cudaSetDevice(v->device));
+  TE_CUDA(v, cudaDeviceSynchronize());
+  TE_CUDA(v, cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost));
+  return TE_OK;
+}
+
+void te_vision_destroy(te_vision* v) {
+  if (!v) return;
+  cudaSetDevice(v->device);
+  cudaDeviceSynchronize();
+  if (v->tower) te_destroy(v->tower);
+  void* ptrs[] = {v->w_pe, v->w_m, v->a_pe, v->a_m, v->x0, v->tower_out, v->vis, v->zero_lens};
+  for (void* q : ptrs)
+    if (q) cudaFree(q);
+  delete v;
 }
 
 void te_destroy(te_handle* h) {

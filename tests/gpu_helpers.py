@@ -23,13 +23,13 @@ class GpuTE:
     """Owns one handle; encode() returns numpy arrays."""
 
     def __init__(self, model, max_frames, max_tokens, blob, final_norm=None, cta_pair=None, resid_bn=None,
-                 split_k=None, max_prefix_tokens=0, attn_impl=None, resid_wide=None, weight_dtype=0):
+                 split_k=None, max_prefix_tokens=0, attn_impl=None, resid_wide=None, weight_dtype=0, non_causal=0):
         import torch
         import paper_2606_05981_b200 as te
         self.te, self.torch, self.model = te, torch, model
         self.weight_dtype = weight_dtype
         self.enc = te.TextEncoder(model, max_frames, max_tokens, final_norm=final_norm,
-                                  max_prefix_tokens=max_prefix_tokens, weight_dtype=weight_dtype)
+                                  max_prefix_tokens=max_prefix_tokens, weight_dtype=weight_dtype, non_causal=non_causal)
         self.enc.load_weights(blob)
         if cta_pair is not None:
             te.te_set_option(self.enc.h, te.TE_OPT_CTA_PAIR, cta_pair)

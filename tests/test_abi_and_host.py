@@ -37,6 +37,19 @@ def test_config_struct_layout_matches_header(te):
     assert ctypes.sizeof(te.TEConfig) == 80
     assert te.TEConfig.rope_theta.offset == 40 and te.TEConfig.max_frames.offset == 48
     assert te.TEConfig.rope_interleaved.offset == 64 and te.TEConfig.max_prefix_tokens.offset == 68 and te.TEConfig.weight_dtype.offset == 72
+    assert te.TEConfig.non_causal.offset == 76
+    # te_vision_config: te_config (80 bytes, 8-aligned) + 5 int32 -> 104
+    assert te.TEVisionConfig.patch.offset == 80 and te.TEVisionConfig.max_frames.offset == 96
+    assert ctypes.sizeof(te.TEVisionConfig) == 104
+
+
+def test_vision_blob_bytes_without_gpu(te):
+    import workloads as W
+    for v in (W.VISION_TINY, W.VISION_FULL):
+        assert te.te_vision_blob_bytes(te.make_vision_config(v, 4)) == 2 * W.vision_blob_layout(v)["total"]
+    bad = te.make_vision_config(W.VISION_TINY, 4)
+    bad.patch = 5                                          # image not a multiple of 2 * patch
+    assert te.te_vision_blob_bytes(bad) == 0
 
 
 def test_blob_bytes_and_strerror_without_gpu(te):
