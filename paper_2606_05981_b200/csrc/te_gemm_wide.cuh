@@ -67,6 +67,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
   const int lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const bool leader = rank == 0;
+  if (threadIdx.x == 0) trace_stamp(p, 0);
 
   if (warp == 0 && elect_one()) {
     tma_prefetch_desc(&tmA);
@@ -90,6 +91,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_stamp(p, 1);
 
   const int M = gemm_rows(p);
   const int num_kb = p.K / GEMM_BK;
@@ -130,6 +132,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         load_b(kb, kb);
       }
       pdl_wait();
+      trace_stamp(p, 2);
       int stage = 0;
       uint32_t phase = 0;
       for (int kb = 0; kb < num_kb; ++kb) {
@@ -151,6 +154,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
       uint32_t phase = 0;
       for (int kb = 0; kb < num_kb; ++kb) {
         mbar_wait(&full[stage], phase);
+        if (kb == 0) trace_stamp(p, 3);
         tc_fence_after();
         const uint64_t a_desc = umma_smem_desc_sw128(smem_u32(sA + stage * Cfg::A_BYTES));
         const uint64_t b_desc0 = umma_smem_desc_sw128(smem_u32(sB + stage * b_bytes));
@@ -239,6 +243,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
     float4 xn[8];
     if (c_begin < c_end) issue_x(xn, c_begin);  // first chunk's x while the main loop runs
     mbar_wait(tfull, 0);
+    if (warp == 2 && lane == 0) trace_stamp(p, 14);
     tc_fence_after();
     float ss[8];
 #pragma unroll
@@ -301,12 +306,15 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         if (row < M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * 2 + part)] = ss[i];
       }
     }
+    if (warp == 2 && lane == 0) trace_stamp(p, 25);
     }  // EPI_RESID
   }
   tc_fence_before();
   __syncwarp();  // the elected producer / MMA lanes rejoin their warps before the block barrier
   __syncthreads();
+  if (threadIdx.x == 0) trace_stamp(p, 36);
   cluster_sync_all();  // the peer may still be signalling our barriers / reading our smem until here
+  if (threadIdx.x == 0) trace_stamp(p, 37);
   if (warp == 1) {
     __syncwarp();
     tc_fence_after();
