@@ -304,7 +304,7 @@ __device__ __forceinline__ void epi_swiglu(const GemmParams& p, int M, uint32_t 
 // domain, where the cos/sin rows are read as whole 128-byte segments.
 template <int BN, int DH>
 __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_row, int row_base, int lane, int n_blk,
-                                        float* stg, int part, int nparts, float rstd) {
+                                        float* stg, int part, int nparts, float rstd, bool tr = false) {
   constexpr int HD2 = DH / 2;
   const int sub = lane >> 3, cq = lane & 7;
   float* bufA = stg;
@@ -355,6 +355,7 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_r
       }
     };
     load_cs(c_first);
+    if (tr && hh == hh_begin) trace_stamp(p, 38);
     // Pass 1: sum of squares of the head (thread = row, TMEM reads only)
     float ss = 0.f;
 #pragma unroll 1
@@ -369,28 +370,32 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_r
       }
     }
     const float sc = rstd / sqrtf(ss * (1.0f / DH) + p.eps);
+    if (tr && hh == hh_begin) trace_stamp(p, 39);
     // ---- Pass 2: normalised halves a = u[c0..c0+32), b = u[HD2+c0..) -> staging -> rotate -> store.
 #pragma unroll 1
     for (int c0 = c_first; c0 < HD2; c0 += c_step) {
       const int cc = c0 + cq * 4;  // this lane's 4 columns inside the half
-      if (c0 != c_first) load_cs(c0);  // (later steps: requested here, overlapping this step's TMEM reads and staging)
+      // (later steps: their cos/sin rows were requested row by row inside the previous step's rotation loop, as soon as
+      //  that step had consumed its own — the L2 round trip overlaps the rest of that loop, this step's TMEM reads and staging)
+      const bool more = c0 + c_step < HD2;
+      const int cc_next = c0 + c_step + cq * 4;
       const uint2 ga = __ldg(reinterpret_cast<const uint2*>(gain + cc));
       const uint2 gb = __ldg(reinterpret_cast<const uint2*>(gain + HD2 + cc));
       {
         float v[32];
-        uint32_t r[32];
-        tmem_ld32(t_head + c0, r);
+        uint32_t r[32], r2[32];
+        tmem_ld32(t_head + c0, r);  // both halves in flight: one TMEM round trip per step
+        tmem_ld32(t_head + HD2 + c0, r2);
         tmem_ld_wait();
 #pragma unroll
         for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) * sc;
         stg_put_row(bufA, lane, v);
-        tmem_ld32(t_head + HD2 + c0, r);
-        tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) * sc;
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r2[j]) * sc;
         stg_put_row(bufB, lane, v);
       }
       __syncwarp();
+      if (tr && hh == hh_begin && c0 == c_first) trace_stamp(p, 40);
       const float gA[4] = {bf16_lo(ga.x), bf16_hi(ga.x), bf16_lo(ga.y), bf16_hi(ga.y)};
       const float gB[4] = {bf16_lo(gb.x), bf16_hi(gb.x), bf16_lo(gb.y), bf16_hi(gb.y)};
 #pragma unroll
@@ -404,6 +409,10 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_r
           const float ub[4] = {b.x * gB[0], b.y * gB[1], b.z * gB[2], b.w * gB[3]};
           const float c[4] = {cs[i].x, cs[i].y, cs[i].z, cs[i].w};
           const float sv[4] = {sn[i].x, sn[i].y, sn[i].z, sn[i].w};
+          if (more) {
+            cs[i] = __ldg(reinterpret_cast<const float4*>(p.cos_t + (size_t)row * HD2 + cc_next));
+            sn[i] = __ldg(reinterpret_cast<const float4*>(p.sin_t + (size_t)row * HD2 + cc_next));
+          }
           float r1[4], r2[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
@@ -419,7 +428,9 @@ __device__ __forceinline__ void epi_qkv(const GemmParams& p, int M, uint32_t t_r
         }
       }
       __syncwarp();
+      if (tr && hh == hh_begin && c0 == c_first) trace_stamp(p, 41);
     }
+    if (tr && hh == hh_begin) trace_stamp(p, 42);
   }
 }
 
@@ -755,9 +766,10 @@ te_gemm2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       if constexpr (EPI == EPI_PLAIN) epi_plain<BN>(p, t_row, row_base + lane, row_base + lane < M, n_blk, part, NPARTS);
       if constexpr (EPI == EPI_RESID) epi_resid<BN>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, pf);
       if constexpr (EPI == EPI_SWIGLU) epi_swiglu<BN>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
-      if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
+      if constexpr (EPI == EPI_QKV)
+        epi_qkv<BN, DH>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd, warp == 2 && lane == 0 && it == 0);
       tc_fence_before();
-      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
+      mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty[acc]), 0));
       if (warp == 2 && lane == 0 && it < 10) trace_stamp(p, 25 + it);
     }
   }

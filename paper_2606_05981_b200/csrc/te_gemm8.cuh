@@ -439,7 +439,7 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       if constexpr (EPI == EPI_SWIGLU) epi_swiglu8<BN>(p, x8, M, t_row, row_base + lane, n_blk, part, NPARTS, rstd);
       if constexpr (EPI == EPI_QKV) epi_qkv<BN, DH>(p, M, t_row, row_base, lane, n_blk, stg, part, NPARTS, rstd);
       tc_fence_before();
-      mbar_arrive_cluster(mapa_u32(smem_u32(&tempty[acc]), 0));
+      mbar_arrive_cluster_relaxed(mapa_u32(smem_u32(&tempty[acc]), 0));
     }
   }
   tc_fence_before();

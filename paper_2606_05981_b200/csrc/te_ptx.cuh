@@ -180,6 +180,13 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t smem_addr, uint32_t rank) 
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// The same arrive without release semantics: for barriers that hand over TENSOR MEMORY only (the epilogue's "accumulator
+// buffer is free again": its tcgen05.ld have completed — tcgen05.wait::ld — and tcgen05.fence::before_thread_sync orders
+// them ahead of the arrive).  A cluster-scope RELEASE would also make the thread wait until its global stores of the
+// tile are visible across SMs (~2500 clk per tile in the pipeline trace), which nothing behind this barrier reads.
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 // TMA load issued by either CTA of a pair; completes its bytes on the barrier at `bar_cluster_addr`
 // (the leader CTA's full barrier).
 __device__ __forceinline__ void tma_load_2d_cg2(void* smem_dst, const CUtensorMap* m, uint32_t bar_cluster_addr,

@@ -136,6 +136,7 @@ struct te_handle {
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   int resid_wide = 1; // residual GEMMs on CTA pairs: 1 = auto (one wave of wide tiles when 128-wide tiles need >= 2
                       // waves), 0 = never, n >= 2 = always with n tiles across N (tests)
+  int resid_halves = 0; // wide residual tiles as two column halves (te_gemm_wide2_kernel): 1 = O-proj and down, 2 = O-proj, 0 = one pass
   int l2_resid = 1;          // 1: the residual stream is an L2-persisting access window of every kernel
   size_t l2_limit_bytes = 0; // persisting-L2 carve-out requested for it (0 until the first te_encode sets the limit)
   size_t l2_prev_limit = 0;  // the device limit found before it was raised (restored by te_destroy / option 0)
@@ -460,6 +461,10 @@ cudaError_t init_kernel_attrs() {
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide2_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmWideCfg::SMEM_LIMIT)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide2_kernel<te::EPI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((set_gemm8_attr<128, te::EPI_QKV, 128>()));
   TE_ATTR((set_gemm8_attr<128, te::EPI_QKV, 64>()));
   TE_ATTR((set_gemm8_attr<256, te::EPI_QKV, 128>()));
@@ -491,6 +496,20 @@ cudaError_t launch_wide(const LaunchCtx& lc, const CUtensorMap& tmA, const CUten
   const int num_mp = (p.num_m_blk + 1) / 2;
   return launch_k(lc, te::te_gemm_wide_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
                   te::GemmWideCfg::smem_bytes(bn), st, tmA, tmB, p, bn);
+}
+
+// The same tiles as two column halves accumulated one after the other (te_gemm_wide2_kernel): the first half's
+// epilogue overlaps the second half's main loop.  `w`: the weight matrix [N, K].
+template <int EPI>
+cudaError_t launch_wide2(const LaunchCtx& lc, const CUtensorMap& tmA, const void* w, int n_rows, int k, const te::GemmParams& p,
+                         int n_tiles, int bn, cudaStream_t st) {
+  const int w0 = te::GemmWideCfg::sub_w0(bn), w1 = bn - w0;
+  CUtensorMap tb0, tb1;
+  if (!make_tmap(&tb0, w, n_rows, k, w0 / 2) || !make_tmap(&tb1, w, n_rows, k, w1 > 0 ? w1 / 2 : w0 / 2))
+    return cudaErrorInvalidValue;
+  const int num_mp = (p.num_m_blk + 1) / 2;
+  return launch_k(lc, te::te_gemm_wide2_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
+                  te::GemmWideCfg::smem_bytes(bn, 1), st, tmA, tb0, tb1, p, bn);
 }
 
 // Token-count bucket: the row-block count that every grid and every dispatch decision is derived from.
@@ -613,8 +632,9 @@ std::string describe_plan(const te_handle* h, const Plan& pl) {
                                                 : "te_attn_kernel");
   s += b;
   if (pl.wide_tiles) {
-    snprintf(b, sizeof(b), "oproj=te_gemm_wide_kernel<2> (%d tiles x %d cols);down=te_gemm_wide_kernel<2> (%d tiles x %d cols);",
-             pl.wide_tiles, pl.wide_bn, pl.wide_tiles, pl.wide_bn);
+    const bool h_o = h->resid_halves != 0, h_d = (h->resid_halves & 1) && !(h->resid_halves & 2);
+    snprintf(b, sizeof(b), "oproj=te_gemm_wide%s_kernel<2> (%d tiles x %d cols);down=te_gemm_wide%s_kernel<2> (%d tiles x %d cols);",
+             h_o ? "2" : "", pl.wide_tiles, pl.wide_bn, h_d ? "2" : "", pl.wide_tiles, pl.wide_bn);
     s += b;
   } else {
     gemm("oproj", te::EPI_RESID, pl.k_res, pl.pair, pl.bn_res, 128);
@@ -774,6 +794,8 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
         TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_attn8, h->tm8[l].o[0], h->tmSF_attn, h->tm8[l].sf_o, p, x8,
                                                         h->sm_count, st)));
+      } else if (pl.wide_tiles && h->resid_halves) {
+        TE_CUDA(h, launch_wide2<te::EPI_RESID>(lc, h->tmA_attn, h->w + o.wo, d, n_q, p, pl.wide_tiles, pl.wide_bn, st));
       } else if (pl.wide_tiles) {
         CUtensorMap tmB;
         if (!make_tmap(&tmB, h->w + o.wo, d, n_q, pl.wide_bn / 4)) { h->err = "tensor map (wide O-proj)"; return TE_ERR_CUDA; }
@@ -830,6 +852,8 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
         TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_act8, h->tm8[l].d[0], h->tmSF_act, h->tm8[l].sf_d, p, x8,
                                                         h->sm_count, st)));
+      } else if (pl.wide_tiles && (h->resid_halves & 1) && !(h->resid_halves & 2)) {
+        TE_CUDA(h, launch_wide2<te::EPI_RESID>(lc, h->tmA_act, h->w + o.wd, d, F, p, pl.wide_tiles, pl.wide_bn, st));
       } else if (pl.wide_tiles) {
         CUtensorMap tmB;
         if (!make_tmap(&tmB, h->w + o.wd, d, F, pl.wide_bn / 4)) { h->err = "tensor map (wide down)"; return TE_ERR_CUDA; }
@@ -1367,6 +1391,10 @@ int te_set_option(te_handle* h, int option, int value) {
       if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
       h->resid_wide = value;
       break;
+    case TE_OPT_RESID_HALVES:
+      if (value < 0 || value > 3) return TE_ERR_INVALID_ARG;
+      h->resid_halves = value;
+      break;
     case TE_OPT_SPLIT_K:
       h->splitk = value ? 1 : 0;
       h->split_target = value > 1 ? value : 0;
@@ -1528,6 +1556,26 @@ int te_debug_gemm_wide(int device, const void* a, const void* b, float* cmat, in
   p.c = cmat; p.ld_c = n;
   const LaunchCtx lc;
   cudaError_t e = launch_wide<te::EPI_PLAIN>(lc, ta, tb, p, n_tiles, bn, nullptr);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+}
+
+int te_debug_gemm_wide2(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                        int32_t n_tiles) {
+  int sms = 0;
+  int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
+  if (rc != TE_OK) return rc;
+  if (n_tiles < 1 || n % 32 != 0) return TE_ERR_UNSUPPORTED;
+  const int bn = (((n + n_tiles - 1) / n_tiles) + 31) / 32 * 32;
+  const int num_m = (m + te::GEMM_BM - 1) / te::GEMM_BM;
+  if (bn > 512 || ((num_m + 1) / 2) * n_tiles > sms / 2) return TE_ERR_UNSUPPORTED;  // one wave only
+  CUtensorMap ta;
+  if (!make_tmap(&ta, a, m, k, te::GEMM_BM)) return TE_ERR_CUDA;
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = num_m; p.num_n_blk = n_tiles;
+  p.c = cmat; p.ld_c = n;
+  const LaunchCtx lc;
+  cudaError_t e = launch_wide2<te::EPI_PLAIN>(lc, ta, b, n, k, p, n_tiles, bn, nullptr);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }

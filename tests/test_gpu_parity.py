@@ -88,11 +88,13 @@ def test_gemm_splitk_vs_fp64_matmul(H, M, N, K, bn, splits):
 @pytest.mark.parametrize("M,N,K,n_tiles", [(3072, 2048, 2048, 6), (3072, 2048, 6144, 6), (3733, 2048, 2048, 4),
                                            (2048, 2048, 6144, 9), (1500, 2048, 2048, 7), (593, 256, 768, 5),
                                            (300, 256, 256, 3), (256, 2048, 2048, 16)])
-def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles):
+@pytest.mark.parametrize("halves", [0, 1])
+def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles, halves):
     """One-wave wide-tile kernel alone (te_gemm_wide.cuh, plain epilogue), elementwise against an fp64 matmul: the
     widths the stack's dispatch picks at cfg 4 (6 x 352) and cfg 5 (4 x 512), a partly out-of-range last tile
     (7 x 320 > 2048), a wholly out-of-range one (5 x 64 > 256), a ragged last row-pair block, one MMA narrower than
-    the other tile widths (16 x 128)."""
+    the other tile widths (16 x 128).  halves = 1: te_gemm_wide2_kernel — the tile's columns as two sub-tiles accumulated
+    one after the other (352 -> 192 + 160, 64 -> 32 + 32, 512 -> 256 + 256, 128 -> 64 + 64, 32 -> 32 + 0 ...)."""
     import torch
     import paper_2606_05981_b200 as te
     rng = np.random.default_rng(M * 3 + N + n_tiles)
@@ -102,7 +104,7 @@ def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles):
     ad = torch.from_numpy(a.view(np.int16)).cuda()
     bd = torch.from_numpy(b.view(np.int16)).cuda()
     c = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
-    te.te_debug_gemm_wide(0, ad, bd, c, M, N, K, n_tiles)
+    te.te_debug_gemm_wide(0, ad, bd, c, M, N, K, n_tiles, halves)
     out = c.cpu().numpy()
     assert np.isfinite(out).all()
     assert PM.rel_l2(out, ref) < 1e-5
@@ -602,10 +604,12 @@ def test_many_small_frames(H, O):
     g.close()
 
 
+@pytest.mark.parametrize("halves", [1, 0, 2])
 @pytest.mark.parametrize("n_tiles", [2, 3, 5, 8])
-def test_wide_residual_tiles(H, O, n_tiles):
-    """O-proj / down as one wave of wide CTA-pair tiles (two MMAs per k-step): forced tile counts whose widths do and do
-    not divide the hidden size (a partly and a completely out-of-range last tile), ragged last row-pair block."""
+def test_wide_residual_tiles(H, O, n_tiles, halves):
+    """O-proj / down as one wave of wide CTA-pair tiles: forced tile counts whose widths do and do not divide the hidden
+    size (a partly and a completely out-of-range last tile), ragged last row-pair block.  halves: 1 = both GEMMs as two
+    column halves (te_gemm_wide2_kernel), 0 = one pass with two MMAs per k-step (the default), 2 = O-proj only."""
     m = W.TINY
     blob = H.cached_blob(m, 1)
     tl = [5, 0, 190, 33, 240, 65]
@@ -614,8 +618,9 @@ def test_wide_residual_tiles(H, O, n_tiles):
     emb = np.random.default_rng(4).standard_normal((T, m.hidden)).astype(np.float32)
     ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
     g = H.GpuTE(m, len(tl), T, blob, cta_pair=1, resid_wide=n_tiles)
+    g.te.te_set_option(g.enc.h, g.te.TE_OPT_RESID_HALVES, halves)
     out = g.encode(emb, tl, gh, gw)
-    _assert_final(PM.stack_metrics(out, ref, emb), f"wide residual tiles n={n_tiles}")
+    _assert_final(PM.stack_metrics(out, ref, emb), f"wide residual tiles n={n_tiles} halves={halves}")
     assert np.array_equal(out, g.encode(emb, tl, gh, gw))
     g.close()
 
