@@ -114,6 +114,20 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w,
               const float* embeds, const int32_t* text_lens, int32_t total_tokens, float* out,
               void* cuda_stream);
 
+/* te_encode with one grid PER FRAME and / or bf16 embeddings ("bf16-embedding input, per-frame
+ * grids"; readings Q14, Q19 of SURVEY §8c generalised).
+ *   grids         DEVICE int32 [n_frames][2] = (grid_h, grid_w) of every frame, or NULL (then grid_h, grid_w as in
+ *                 te_encode).  Frame b holds grid_h[b]*grid_w[b] visual tokens (row-major on ITS grid, t = 0) followed by
+ *                 text_lens[b] text tokens whose ids start at max(grid_h[b], grid_w[b]); a negative entry or
+ *                 S_b > max_tokens_per_frame raises the device validation flag (te_query_async_error).  Not
+ *                 available together with a cached prefix (TE_ERR_UNSUPPORTED).
+ *   embeds_dtype  0: DEVICE fp32 [T, hidden] (as te_encode); 1: DEVICE bf16 [T, hidden] — widened exactly to the fp32
+ *                 residual stream by the first kernel, so the result equals te_encode on the same values
+ * Everything else as te_encode (asynchronous, one graph per shape class). */
+int te_encode_ex(te_handle* h, int32_t n_frames, const int32_t* grids, int32_t grid_h, int32_t grid_w,
+                 const void* embeds, int32_t embeds_dtype, const int32_t* text_lens, int32_t total_tokens,
+                 float* out, void* cuda_stream);
+
 /* Shared text prefix with K/V reuse.  The real chat template puts the same
  * system prompt (80 tokens: 13 % of the TE's time) in front of every frame's image.  Being
  * a causal prefix it sees nothing after it, so its hidden states and its per-layer keys/values are the

@@ -48,7 +48,7 @@ enum {
   TE_TAP_QKV = 4,        /* bf16  [T, (Hq+2Hkv)*dh]  q (normed+rotated) | k | v  */
   TE_TAP_ATTN = 5,       /* bf16  [T, Hq*dh]                                    */
   TE_TAP_ACT = 6,        /* bf16  [T, F]       silu(gate)*up                    */
-  TE_TAP_TRACE = 7,      /* u64   [4 GEMM classes (qkv,oproj,gateup,down)][n_SMs][96] ns stamps / SM clocks
+  TE_TAP_TRACE = 7,      /* u64   [5 classes (qkv,oproj,gateup,down,attn)][n_SMs][96] ns stamps / SM clocks
                             of the last launch of each class (TE_OPT_TRACE)     */
   /* weight_dtype = 1 (MXFP8): the quantised A operands; scales in the tiled order of te_debug_mx_quantise */
   TE_TAP_ATTN8 = 8,      /* u8 E4M3 [T, Hq*dh]                                  */

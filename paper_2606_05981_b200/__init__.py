@@ -36,7 +36,7 @@ TE_TAP_ATTN8, TE_TAP_ACT8, TE_TAP_SF_ATTN, TE_TAP_SF_ACT = 8, 9, 10, 11
 
 # include/te.h (the product boundary) and include/te_debug.h (test-only taps and stand-alone GEMMs)
 EXPORTS = [
-    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_prefix", "te_encode_host",
+    "te_blob_bytes", "te_create", "te_load_weights", "te_encode", "te_encode_ex", "te_encode_prefix", "te_encode_host",
     "te_encode_host_submit", "te_encode_host_wait", "te_query_async_error", "te_set_option", "te_kernel_launches",
     "te_graph_captures", "te_dispatch_info", "te_kernel_times", "te_destroy", "te_strerror", "te_last_error",
     "te_vision_blob_bytes", "te_vision_create", "te_vision_load_weights", "te_encode_image", "te_vision_kernel_launches",
@@ -96,6 +96,9 @@ def lib() -> ctypes.CDLL:
     L.te_load_weights.argtypes = [c_void_p, c_void_p, c_size_t]
     L.te_encode.restype = c_int
     L.te_encode.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_void_p, c_void_p, c_int32, c_void_p, c_void_p]
+    L.te_encode_ex.restype = c_int
+    L.te_encode_ex.argtypes = [c_void_p, c_int32, c_void_p, c_int32, c_int32, c_void_p, c_int32, c_void_p, c_int32, c_void_p,
+                               c_void_p]
     L.te_encode_prefix.restype = c_int
     L.te_encode_prefix.argtypes = [c_void_p, c_void_p, c_int32, c_void_p, c_void_p]
     L.te_encode_host.restype = c_int
@@ -224,6 +227,12 @@ def te_encode(h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out,
     """embeds/out: DEVICE fp32 [T, d]; text_lens: DEVICE int32 [B]; stream: cudaStream_t as int."""
     _check(lib().te_encode(h, n_frames, grid_h, grid_w, _ptr(embeds), _ptr(text_lens), total_tokens,
                            _ptr(out), _ptr(stream)), h)
+
+
+def te_encode_ex(h, n_frames, grids, grid_h, grid_w, embeds, embeds_dtype, text_lens, total_tokens, out, stream=None):
+    """grids: DEVICE int32 [B, 2] or None; embeds: DEVICE fp32 (embeds_dtype 0) or bf16 (1) [T, d]."""
+    _check(lib().te_encode_ex(h, n_frames, _ptr(grids), grid_h, grid_w, _ptr(embeds), embeds_dtype, _ptr(text_lens),
+                              total_tokens, _ptr(out), _ptr(stream)), h)
 
 
 def te_encode_prefix(h, prefix_embeds, prefix_len, prefix_out=None, stream=None):
@@ -388,6 +397,9 @@ class TextEncoder:
 
     def encode(self, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream=None):
         te_encode(self.h, n_frames, grid_h, grid_w, embeds, text_lens, total_tokens, out, stream)
+
+    def encode_ex(self, n_frames, grids, grid_h, grid_w, embeds, embeds_dtype, text_lens, total_tokens, out, stream=None):
+        te_encode_ex(self.h, n_frames, grids, grid_h, grid_w, embeds, embeds_dtype, text_lens, total_tokens, out, stream)
 
     def encode_prefix(self, prefix_embeds, prefix_len, prefix_out=None, stream=None):
         te_encode_prefix(self.h, prefix_embeds, prefix_len, prefix_out, stream)

@@ -41,6 +41,8 @@ struct AttnTcParams {
   // MXFP8 variant: the output (= A operand of the O projection) is written as E4M3 + block scales instead of bf16
   uint8_t* out8;    // [T, Hq*DH] or null
   uint8_t* sf_out;  // tiled scales (te_gemm8.cuh)
+  unsigned long long* trace;  // TE_OPT_TRACE: [trace_ctas][TRACE_SLOTS] stamps (null: off)
+  int trace_ctas;
 };
 
 template <int DH>
@@ -93,6 +95,17 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int split = blockIdx.x, n_split = gridDim.x, kvh = blockIdx.y, b = blockIdx.z;
   const int g_shift = p.g_shift;
+  const int cta_lin = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+  auto stamp = [&](int slot) {  // TE_OPT_TRACE (debug): slot 0 start, 1 set up, 2 past the dependency wait, per tile i < 4:
+    // 3+5i scores ready, 4+5i pass 1 done, 5+5i P written, 6+5i O ready, 7+5i stored; 37 end
+    if (p.trace != nullptr && cta_lin < p.trace_ctas) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)::"memory");
+      p.trace[(size_t)cta_lin * TRACE_SLOTS + slot] = t;
+      p.trace[(size_t)cta_lin * TRACE_SLOTS + 48 + slot] = static_cast<unsigned long long>(clock64());
+    }
+  };
+  if (threadIdx.x == 0) stamp(0);
   const int G = 1 << g_shift;
   const int PT = 128 >> g_shift;  // positions per query tile
 
@@ -121,7 +134,9 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   pdl_launch_dependents();
+  if (threadIdx.x == 0) stamp(1);
   pdl_wait();  // qkv and cu_seqlens are written by predecessor kernels
+  if (threadIdx.x == 0) stamp(2);
 
   const int seq0 = p.cu_seqlens[b];
   // (a frame longer than KMAX raised the device validation flag in te_scan_kernel; clamp so that the
@@ -228,6 +243,8 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + 256 * t;
       mbar_wait(&s_full[t], u & 1);
       tc_fence_after();
+      const bool tr = quad == 0 && lane == 0 && i < 4;
+      if (tr) stamp(3 + 5 * i);
       // ---- pass 1: row maximum over the visible keys
       float mx = -INFINITY;
 #pragma unroll 1
@@ -240,6 +257,7 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           if (c0 + x <= lim) mx = fmaxf(mx, __uint_as_float(r[x]));
       }
       const float msc = mx * sc;
+      if (tr) stamp(4 + 5 * i);
       // ---- pass 2: p = exp2(s * c - max * c), row sum in fp32, P (bf16) back into TMEM
       float l = 0.f;
 #pragma unroll 1
@@ -261,9 +279,11 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(&p_full[t]);
+      if (tr) stamp(5 + 5 * i);
       // ---- epilogue: O / l -> bf16 -> global
       mbar_wait(&o_full[t], u & 1);
       tc_fence_after();
+      if (tr) stamp(6 + 5 * i);
       const int head = (kvh << g_shift) + hl;
       __nv_bfloat16* dst = p.out + (size_t)(seq0 + pos) * (p.n_q_heads * DH) + head * DH;
       // scale of this pass's unnormalised O, and (prefix mode) of the frame-local result already in `out`
@@ -317,11 +337,13 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       }
       tc_fence_before();
       mbar_arrive(&buf_free[t]);
+      if (tr) stamp(7 + 5 * i);
     }
   }
   tc_fence_before();
   __syncwarp();
   __syncthreads();
+  if (threadIdx.x == 0) stamp(37);
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, Cfg::TMEM_COLS);

@@ -30,11 +30,12 @@ enum { EPI_PLAIN = 0, EPI_QKV = 1, EPI_RESID = 2, EPI_SWIGLU = 3 };
 // (te_set_dyn_kernel), read by every kernel.  A graph is therefore reusable for any caller buffers and for any
 // token count of the same row-block bucket (te_runtime.cu, graph cache).
 struct DynParams {
-  const float* embeds;       // DEVICE fp32 [T, d]
+  const void* embeds;        // DEVICE [T, d]: fp32, or bf16 when embeds_bf16 (te_encode_ex)
   const int32_t* text_lens;  // DEVICE int32 [B]
   float* out;                // DEVICE fp32 [T, d]
+  const int32_t* grids;      // DEVICE int32 [B][2] = (grid_h, grid_w) of every frame, or null: one grid per call
   int32_t total_tokens;      // T
-  int32_t pad_;
+  int32_t embeds_bf16;
 };
 
 struct GemmParams {

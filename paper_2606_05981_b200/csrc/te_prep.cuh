@@ -55,7 +55,7 @@ struct PrepParams {
 // clamped so that no kernel touches rows beyond the caller's buffers even when validation fails; the
 // token's frame is the largest b with cu[b] <= tok.  Block 0 also publishes cu[] and the validation flag.
 __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
-  __shared__ int s_start;
+  __shared__ int s_start, s_gh, s_gw;
   __shared__ float s_ss[8];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tok = blockIdx.x;
@@ -64,6 +64,7 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
   asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous call's kernels still read cu / flag / out
   const int total_tokens = p.dyn->total_tokens;
   const int32_t* const text_lens = p.dyn->text_lens;
+  const int32_t* const grids = p.dyn->grids;  // per-frame (grid_h, grid_w) (te_encode_ex) or null
   if (warp == 0) {
     long long carry = 0;
     int best_b = 0, best_start = 0, f = 0;
@@ -73,7 +74,13 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
       if (b < p.n_frames) {
         int tl = text_lens[b];
         if (tl < 0) { f |= FLAG_BAD_LEN; tl = 0; }
-        sb = n_vis + tl;
+        int nv = n_vis;
+        if (grids != nullptr) {
+          int gh = grids[2 * b], gw = grids[2 * b + 1];
+          if (gh < 0 || gw < 0) { f |= FLAG_BAD_LEN; gh = gw = 0; }
+          nv = (gh > p.max_tokens_per_frame || gw > p.max_tokens_per_frame) ? p.max_tokens_per_frame + 1 : gh * gw;
+        }
+        sb = nv + tl;
         if (sb > p.max_tokens_per_frame) f |= FLAG_TOO_LONG;
       }
       long long incl = sb;
@@ -104,6 +111,8 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
     }
     if (lane == 0) {
       s_start = best_start;
+      s_gh = grids != nullptr ? max(grids[2 * best_b], 0) : p.grid_h;
+      s_gw = grids != nullptr ? max(grids[2 * best_b + 1], 0) : p.grid_w;
       if (tok == 0 && f) atomicOr(p.flag, f);
     }
   }
@@ -114,12 +123,13 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
     return;
   }
   const int n = tok - s_start;
+  const int gh = s_gh, gw = s_gw;  // this token's frame's grid
   int pt, ph, pw;
   const int off = p.pos_offset;
-  if (n < n_vis) {
-    pt = off; ph = off + n / p.grid_w; pw = off + n % p.grid_w;  // visual token: row-major grid, t constant
+  if (n < gh * gw) {
+    pt = off; ph = off + n / gw; pw = off + n % gw;  // visual token: row-major grid, t constant
   } else {
-    pt = ph = pw = off + max(p.grid_h, p.grid_w) + (n - n_vis);  // text: continues from max grid id + 1
+    pt = ph = pw = off + max(gh, gw) + (n - gh * gw);  // text: continues from max grid id + 1
   }
   if (threadIdx.x == 0) {
     p.pos[tok] = pt;
@@ -136,11 +146,20 @@ __global__ void __launch_bounds__(256) te_prep_kernel(const PrepParams p) {
     p.sin_t[(size_t)tok * p.half_dim + i] = static_cast<float>(sn);
   }
   // residual copy + sum of squares + bf16(x * g)
-  const float4* src = reinterpret_cast<const float4*>(p.dyn->embeds + (size_t)tok * p.d);
+  const bool e16 = p.dyn->embeds_bf16 != 0;  // bf16 embeddings (te_encode_ex): widened exactly to the fp32 residual
+  const float4* src = reinterpret_cast<const float4*>(static_cast<const float*>(p.dyn->embeds) + (size_t)tok * p.d);
+  const uint2* src16 = reinterpret_cast<const uint2*>(static_cast<const __nv_bfloat16*>(p.dyn->embeds) + (size_t)tok * p.d);
   float4* dst = reinterpret_cast<float4*>(p.out + (size_t)tok * p.d);
   float ss = 0.f;
   for (int c4 = threadIdx.x; c4 < p.d / 4; c4 += 256) {
-    const float4 v = __ldg(src + c4);
+    float4 v;
+    if (e16) {
+      const uint2 u = __ldg(src16 + c4);
+      v = make_float4(__uint_as_float(u.x << 16), __uint_as_float(u.x & 0xFFFF0000u), __uint_as_float(u.y << 16),
+                      __uint_as_float(u.y & 0xFFFF0000u));
+    } else {
+      v = __ldg(src + c4);
+    }
     dst[c4] = v;
     ss = fmaf(v.x, v.x, ss); ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
     const uint2 g = __ldg(reinterpret_cast<const uint2*>(p.g_first) + c4);

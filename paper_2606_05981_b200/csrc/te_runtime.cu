@@ -664,7 +664,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
   const bool dbg_stop = !prefix_pass && h->dbg_stop;
   const int P = prefix_pass ? 0 : h->prefix_len;  // cached prefix keys in front of every frame
   const int n_kv = 2 * c.n_kv_heads * dh;
-  const Plan pl = make_plan(h, Tb, n_frames, grid_h * grid_w);
+  const Plan pl = make_plan(h, Tb, n_frames, grid_h < 0 ? 0 : grid_h * grid_w);
   if (!prefix_pass) h->last_plan = pl;
   const int num_m = pl.num_m;
   int nk = 0;
@@ -763,6 +763,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2; tp.non_causal = c.non_causal;
         tp.stats = P > 0 ? h->attn_stats : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
         tp.out8 = pl.mx ? h->attn8 : nullptr; tp.sf_out = h->sf_attn;
+        tp.trace = trace_ptr(4); tp.trace_ctas = h->sm_count;
         TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st)
                              : launch_attn_tc<64>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st));
         if (P > 0) {  // second pass: the P cached prefix keys of this layer, merged in place
@@ -890,9 +891,10 @@ void free_graphs(te_handle* h) {
 }
 
 // Per-call values -> device block, on the stream, ahead of the stack (values travel as kernel parameters).
-cudaError_t set_dyn(te_handle* h, const float* embeds, const int32_t* lens, float* out, int T, cudaStream_t st) {
+cudaError_t set_dyn(te_handle* h, const void* embeds, const int32_t* lens, float* out, int T, cudaStream_t st,
+                    const int32_t* grids = nullptr, int embeds_bf16 = 0) {
   te::DynParams v{};
-  v.embeds = embeds; v.text_lens = lens; v.out = out; v.total_tokens = T;
+  v.embeds = embeds; v.text_lens = lens; v.out = out; v.total_tokens = T; v.grids = grids; v.embeds_bf16 = embeds_bf16;
   te::te_set_dyn_kernel<<<1, 32, 0, st>>>(h->dyn, v);
   return cudaGetLastError();
 }
@@ -1148,16 +1150,25 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
   return TE_OK;
 }
 
-int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds,
-              const int32_t* text_lens, int32_t total_tokens, float* out, void* cuda_stream) {
+// te_encode / te_encode_ex.  grids != null: one (grid_h, grid_w) per frame on the device; the scalar grid is then unused
+// (-1 in the graph key; attention grids are sized for the longest frame the capacities allow).
+static int encode_impl(te_handle* h, int32_t n_frames, const int32_t* grids, int32_t grid_h, int32_t grid_w, const void* embeds,
+                       int embeds_bf16, const int32_t* text_lens, int32_t total_tokens, float* out, void* cuda_stream) {
   if (!h) return TE_ERR_INVALID_ARG;
   if (!h->loaded) return TE_ERR_NOT_LOADED;
   const te_config& c = h->cfg;
   if (!embeds || !text_lens || !out || embeds == out) return TE_ERR_INVALID_ARG;
-  if (n_frames < 1 || n_frames > c.max_frames || grid_h < 1 || grid_w < 1) return TE_ERR_INVALID_ARG;
+  if (n_frames < 1 || n_frames > c.max_frames) return TE_ERR_INVALID_ARG;
   if (total_tokens < 1 || total_tokens > c.max_tokens) return TE_ERR_INVALID_ARG;
-  if ((long long)grid_h * grid_w > c.max_tokens_per_frame) return TE_ERR_INVALID_ARG;
-  if ((long long)n_frames * grid_h * grid_w > total_tokens) return TE_ERR_INVALID_ARG;
+  if (grids == nullptr) {
+    if (grid_h < 1 || grid_w < 1) return TE_ERR_INVALID_ARG;
+    if ((long long)grid_h * grid_w > c.max_tokens_per_frame) return TE_ERR_INVALID_ARG;
+    if ((long long)n_frames * grid_h * grid_w > total_tokens) return TE_ERR_INVALID_ARG;
+  } else {
+    if (h->prefix_len > 0) return TE_ERR_UNSUPPORTED;  // (the cached-prefix passes take one grid per call)
+    grid_h = grid_w = -1;
+  }
+  const int n_vis_min = grids == nullptr ? grid_h * grid_w : 0;
   TE_CUDA(h, cudaSetDevice(h->device));
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   h->last_T = total_tokens;
@@ -1188,7 +1199,7 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
     cudaGetLastError();
   }
   // per-call pointers and token count: one tiny kernel ahead of the stack (stream-ordered, also under capture)
-  TE_CUDA(h, set_dyn(h, embeds, text_lens, out, total_tokens, st));
+  TE_CUDA(h, set_dyn(h, embeds, text_lens, out, total_tokens, st, grids, embeds_bf16));
   if (!h->use_graph || h->timing || cap != cudaStreamCaptureStatusNone) {
     int rc = enqueue_stack(h, n_frames, grid_h, grid_w, Tb, st, &nk);
     if (rc == TE_OK) h->launches += nk + 1;
@@ -1234,12 +1245,23 @@ int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, co
     h->cache.push_back(GraphEntry{key, ex, g, nk, 0});
     hit = &h->cache.back();
   } else {
-    h->last_plan = make_plan(h, Tb, n_frames, grid_h * grid_w);
+    h->last_plan = make_plan(h, Tb, n_frames, n_vis_min);
   }
   hit->stamp = ++h->stamp;
   TE_CUDA(h, cudaGraphLaunch(hit->exec, st));
   h->launches += hit->n_kernels + 1;
   return TE_OK;
+}
+
+int te_encode(te_handle* h, int32_t n_frames, int32_t grid_h, int32_t grid_w, const float* embeds,
+              const int32_t* text_lens, int32_t total_tokens, float* out, void* cuda_stream) {
+  return encode_impl(h, n_frames, nullptr, grid_h, grid_w, embeds, 0, text_lens, total_tokens, out, cuda_stream);
+}
+
+int te_encode_ex(te_handle* h, int32_t n_frames, const int32_t* grids, int32_t grid_h, int32_t grid_w, const void* embeds,
+                 int32_t embeds_dtype, const int32_t* text_lens, int32_t total_tokens, float* out, void* cuda_stream) {
+  if (embeds_dtype < 0 || embeds_dtype > 1) return TE_ERR_INVALID_ARG;
+  return encode_impl(h, n_frames, grids, grid_h, grid_w, embeds, embeds_dtype, text_lens, total_tokens, out, cuda_stream);
 }
 
 int te_encode_prefix(te_handle* h, const float* prefix_embeds, int32_t prefix_len, float* prefix_out, void* cuda_stream) {
@@ -1364,7 +1386,7 @@ int te_set_option(te_handle* h, int option, int value) {
     case TE_OPT_KERNEL_TIMING: h->timing = value ? 1 : 0; return TE_OK;
     case TE_OPT_TRACE:
       if (value && !h->trace) {
-        const size_t bytes = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+        const size_t bytes = 5 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
         TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->trace), bytes));
         TE_CUDA(h, cudaMemset(h->trace, 0, bytes));
       }
@@ -1467,7 +1489,7 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
     case TE_TAP_SF_ACT: src = h->sf_act; need = (T + 127) / 128 * ((size_t)c.ffn / 128) * 512; break;
     case TE_TAP_TRACE:
       src = h->trace;
-      need = 4 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+      need = 5 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
       if (!src) return TE_ERR_INVALID_ARG;
       break;
     default: return TE_ERR_INVALID_ARG;

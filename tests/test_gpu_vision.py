@@ -253,3 +253,88 @@ def test_vision_boundary_errors():
     # non_causal and a cached prefix exclude each other
     c = te.make_config(W.get_workload(1).model, 2, 80, max_prefix_tokens=8, non_causal=1)
     assert L.te_create(ctypes.byref(c), 0, ctypes.byref(h)) == te.TE_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------ te_encode_ex: per-frame grids, bf16 embeddings
+def test_per_frame_grids(O, H):
+    """One (grid_h, grid_w) per frame on the device: frames are independent, so the
+    oracle is te_oracle.encode frame by frame with that frame's grid.  ids bit-exact, stack within the gates; the
+    frames' text ids start at max(gh, gw) of THEIR grid; a frame with an empty grid (text only) is allowed."""
+    import torch
+    import paper_2606_05981_b200 as te
+    w = W.get_workload(1)
+    m = w.model
+    blob = H.cached_blob(m, w.seed_weights)
+    grids = np.asarray([[4, 4], [2, 7], [8, 1], [0, 0], [3, 5]], dtype=np.int32)
+    tl = np.asarray([24, 3, 0, 40, 17], dtype=np.int32)
+    S = grids[:, 0] * grids[:, 1] + tl
+    T = int(S.sum())
+    emb = W.make_embeddings(w, T)
+    enc = te.TextEncoder(m, len(tl), T)
+    enc.load_weights(blob)
+    e = torch.from_numpy(emb).cuda()
+    out = torch.empty_like(e)
+    enc.encode_ex(len(tl), torch.from_numpy(grids).cuda(), 0, 0, e, 0, torch.from_numpy(tl).cuda(), T, out)
+    torch.cuda.synchronize()
+    assert te.te_query_async_error(enc.h) == te.TE_OK
+    pos = np.empty((3, T), dtype=np.int32)
+    te.te_debug_tap(enc.h, te.TE_TAP_POS, pos)
+    cu = np.empty(len(tl) + 1, dtype=np.int32)
+    te.te_debug_tap(enc.h, te.TE_TAP_CU_SEQLENS, cu)
+    got = out.cpu().numpy()
+    lay = W.blob_layout(m)
+    ref = np.empty((T, m.hidden))
+    want_pos = np.empty((3, T), dtype=np.int64)
+    r = 0
+    for b in range(len(tl)):
+        gh, gw = int(grids[b, 0]), int(grids[b, 1])
+        rows = slice(r, r + int(S[b]))
+        if gh * gw == 0:        # text-only frame: ids 0, 1, 2, ... (max(gh, gw) = 0); the oracle takes a 1x0 grid
+            want_pos[:, rows] = np.arange(int(S[b]))[None, :]
+            ref[rows] = _text_only(O, blob, lay, m, emb[rows])
+        else:
+            want_pos[:, rows] = O.position_ids([int(tl[b])], gh, gw)
+            ref[rows] = O.encode(blob, lay, m, emb[rows], [int(tl[b])], gh, gw)
+        r += int(S[b])
+    assert np.array_equal(cu, np.concatenate([[0], np.cumsum(S)]))
+    assert np.array_equal(pos, want_pos)
+    mm = PM.stack_metrics(got, ref, emb)
+    assert PM.passes_final_gates(mm), mm
+    # an entry that makes a frame too long raises the device flag
+    bad = grids.copy()
+    bad[1] = [20, 20]
+    L = te.lib()
+    assert L.te_encode_ex(enc.h, len(tl), torch.from_numpy(bad).cuda().data_ptr(), 0, 0, e.data_ptr(), 0,
+                          torch.from_numpy(tl).cuda().data_ptr(), T, out.data_ptr(), 0) == te.TE_OK
+    assert te.te_query_async_error(enc.h) == te.TE_ERR_DEVICE_CHECK
+    enc.close()
+
+
+def _text_only(O, blob, lay, m, emb_rows):
+    """A frame without visual tokens = a text sequence with ids t = h = w = 0, 1, 2, ... — what te_oracle.encode computes
+    for a 0-token grid whose text starts at max(gh, gw) = 0; te_oracle takes it as grid 0 x 0."""
+    return O.encode(blob, lay, m, emb_rows, [emb_rows.shape[0]], 0, 0)
+
+
+def test_bf16_embeddings_equal_fp32_call(H):
+    """embeds_dtype = 1: the bf16 embeddings are widened exactly, so the stack's output is BITWISE that of te_encode on
+    the same (bf16-representable) fp32 values — one full-width layer, with the x1000 outlier channels of cfg 3's recipe."""
+    import torch
+    import paper_2606_05981_b200 as te
+    w, blob, tl, T, emb, ch = H.workload_inputs(2, outliers="x1000")
+    m = w.model
+    bits = W.f32_to_bf16_bits(emb)
+    emb_r = (bits.astype(np.uint32) << np.uint32(16)).view(np.float32).reshape(emb.shape)
+    enc = te.TextEncoder(m, w.n_frames, T)
+    enc.load_weights(blob)
+    lens = torch.from_numpy(tl).cuda()
+    e32 = torch.from_numpy(emb_r).cuda()
+    e16 = torch.from_numpy(bits.view(np.int16).reshape(emb.shape)).cuda()
+    o32, o16 = torch.empty_like(e32), torch.empty_like(e32)
+    enc.encode(w.n_frames, w.grid_h, w.grid_w, e32, lens, T, o32)
+    enc.encode_ex(w.n_frames, None, w.grid_h, w.grid_w, e16, 1, lens, T, o16)
+    torch.cuda.synchronize()
+    assert te.te_query_async_error(enc.h) == te.TE_OK
+    assert torch.equal(o32, o16)
+    assert te.te_graph_captures(enc.h) == 1          # same shape class: the second call replays the first graph
+    enc.close()
