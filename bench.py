@@ -95,7 +95,8 @@ def weights_fit_l2(m) -> bool:
 # (workload, kernel name as te_dispatch_info reports it).  NOT measured in the bench run: the value is quoted only when
 # the kernel that ran is the one that was profiled, with its source; otherwise `traffic` is null.
 PROFILED_TRAFFIC = {
-    ("cfg4_28L_B16", "te_gemm2_kernel<256, 3, 128>"): (63.364864e6 + 15.521024e6, "profiles/r01f_cfg4.md"),
+    ("cfg4_28L_B16", "te_gemm2_kernel<256, 3, 128>"): (63.342336e6 + 15.066368e6, "profiles/r02a_cfg4.md"),
+    ("cfg4_28L_B16", "te_gemm8_kernel<192, 3, 128>"): (33.131520e6 + 0.233728e6, "profiles/r02a_cfg4.md"),
 }
 
 
