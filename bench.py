@@ -310,7 +310,10 @@ def run_reference(args, w, blob, tl, T, emb, rank):
     v = statistics.median(vals)
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1000.0 * w.n_frames / v,
+        "steps": args.steps, "warmup": args.warmup,
+        # what was timed: one bounded sample per step (so ms_per_step x steps is this run's timed region); the value is
+        # that sample's rate, and the full batch at that rate would take ms_per_full_batch_extrapolated
+        "ms_per_step": 1000.0 * t_all / max(1, args.steps), "ms_per_full_batch_extrapolated": 1000.0 * w.n_frames / v,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": config_dict(w, T, int(os.environ.get("WORLD_SIZE", "1")), flush_l2=weights_fit_l2(w.model)),
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": samples["cores"], "kind": "oracle",

@@ -196,6 +196,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
       // ---- y = rstd * acc; act = silu(gate) * up, bf16 (arithmetic of epi_swiglu, te_gemm.cuh)
       const float rstd = row_rstd(p, row_base + lane, row_base + lane < M);
       mbar_wait(tfull, 0);
+      if (warp == 2 && lane == 0) trace_stamp(p, 14);
       tc_fence_after();
 #pragma unroll 1
       for (int c0 = c_begin; c0 < c_end; c0 += 32) {
@@ -217,6 +218,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
         stg_store_bf16(stg, lane, row_base, M, p.act, p.ld_act, col_base + c0);
         __syncwarp();
       }
+      if (warp == 2 && lane == 0) trace_stamp(p, 25);
     } else if constexpr (EPI == EPI_PLAIN) {
       // ---- fp32 store of the valid columns (te_debug_gemm_wide: the main loop alone against a matmul)
       mbar_wait(tfull, 0);
