@@ -294,6 +294,45 @@ def measure_vision(torch, te, stream, n_frames: int, reps: int = 50):
             "flops": flops, "achieved_tflops": flops / t / 1e12, "frac_of_burst": flops / (pk["tf_burst"] * 1e12) / t}
 
 
+# ------------------------------------------------------------- in-graph pipeline trace (TE_OPT_TRACE)
+def measure_pipeline_trace(torch, te, enc, step, stream, sm_count: int = 148):
+    """%globaltimer stamps that the kernels write at pipeline events DURING a graph replay (TE_OPT_TRACE; the stamps of a
+    class are those of its last launch = the last layer).  Returns, per kernel class, the median over CTAs of each
+    stamped event in microseconds relative to the QKV kernel's median CTA start, plus the layer span.  Slots: 0 CTA
+    start, 1 set up, 2 producer past the dependency wait, 3.. first MMA of tile i (attention: 3+5i scores ready, 4+5i
+    pass 1, 5+5i P written, 6+5i O ready, 7+5i stored), 14+i / 25+i epilogue of tile i begins / ends (split-K kernels:
+    4 main loop done, 5 partial published, 7 group met, 9 epilogue done), 37 CTA (pair) done."""
+    te.te_set_option(enc.h, te.TE_OPT_TRACE, 1)
+    with torch.cuda.stream(stream):
+        for _ in range(5):
+            step()
+    torch.cuda.synchronize()
+    buf = np.zeros((5, sm_count, 96), dtype=np.uint64)
+    te.te_debug_tap(enc.h, te.TE_TAP_TRACE, buf)
+    te.te_set_option(enc.h, te.TE_OPT_TRACE, 0)
+    ns = buf[:, :, :48].astype(np.int64)
+    names = ["qkv", "oproj", "gateup", "down", "attn"]
+    live0 = ns[0, :, 0] > 0
+    if not live0.any():
+        return None
+    ref = float(np.median(ns[0, live0, 0]))
+    out = {"unit": "us since the QKV kernel's median CTA start (last layer of the stack, inside the graph replay)"}
+    for c, nm in enumerate(names):
+        live = ns[c, :, 0] > 0
+        if not live.any():
+            continue
+        ev = {}
+        for slot in range(48):
+            if slot in (10, 36):      # stamps that the compiler may hoist above the preceding barrier: not reliable
+                continue
+            v = ns[c, live, slot]
+            v = v[v > 0]
+            if len(v):
+                ev[str(slot)] = round((float(np.median(v)) - ref) / 1000.0, 2)
+        out[nm] = {"ctas": int(live.sum()), "events_us": ev}
+    return out
+
+
 # ------------------------------------------------------------------------------------------ main
 def run_reference(args, w, blob, tl, T, emb, rank):
     if rank != 0:
@@ -349,6 +388,9 @@ def main():
                     help="mxfp8: the block-scaled FP8 variant (te_config.weight_dtype = 1; SURVEY 8f NEXT-2): E4M3 weights "
                          "and GEMM A operands with one E8M0 scale per 32 K-elements; roofline against 2x the measured "
                          "bf16 tensor peak (the profiling guide's nominal fp8:bf16 ratio)")
+    ap.add_argument("--pipeline-trace", action="store_true",
+                    help="add a `pipeline_trace` block: %%globaltimer stamps written by the kernels at pipeline events "
+                         "inside the graph replay (TE_OPT_TRACE), medians over CTAs, for the last layer")
     ap.add_argument("--opt", default="", help="library options for experiments, e.g. pdl=0,cta_pair=1,resid_bn=256")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -500,6 +542,11 @@ def main():
 
     dispatch = te.te_dispatch_info(enc.h)
 
+    pipeline_trace = None
+    if args.pipeline_trace and rank == 0:
+        pipeline_trace = measure_pipeline_trace(torch, te, enc, step, stream,
+                                                torch.cuda.get_device_properties(local_rank).multi_processor_count)
+
     overlap = None
     if not args.no_overlap and rank == 0:
         overlap = measure_overlap(torch, step, stream, ms_per_step)
@@ -643,6 +690,8 @@ def main():
         line["secondary"] = secondary
     if overlap is not None:
         line["overlap"] = overlap
+    if pipeline_trace is not None:
+        line["pipeline_trace"] = pipeline_trace
     print(json.dumps(line), flush=True)
     enc.close()
     if dist is not None:
