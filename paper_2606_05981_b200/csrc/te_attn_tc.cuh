@@ -33,9 +33,11 @@ struct AttnTcParams {
   //   launch 1 (prefix_mode 0, stats != null): frame-local causal attention as usual, plus the row statistics
   //            (max raw score, sum of exp) of every (token, q head) -> stats[T, Hq]
   //   launch 2 (prefix_mode 1): tmKV addresses the layer's prefix cache [P, 2*Hkv*dh] (k heads | v heads); every
-  //            query sees all P keys (no mask); the epilogue merges with launch 1's normalised output in place:
+  //            query sees all P keys (no mask); the epilogue merges with launch 1's normalised fp32 output (o32):
   //            out = (l_f e^(m_f-m) out_f + e^(m_p-m) O_p) / (l_f e^(m_f-m) + l_p e^(m_p-m)),  m = max(m_f, m_p)
   float2* stats;
+  float* o32;  // [T, Hq*DH] fp32: launch 1 leaves its normalised output HERE (not in `out`) when a prefix pass follows, and
+               // launch 2 blends in fp32 and rounds to bf16 ONCE (round 1 blended two bf16-rounded values)
   int prefix_mode;
   int prefix_len;
   // MXFP8 variant: the output (= A operand of the O projection) is written as E4M3 + block scales instead of bf16
@@ -318,20 +320,33 @@ te_attn_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           continue;
         }
         if (pos < S) {
+          float* o32row = p.o32 != nullptr ? p.o32 + (size_t)(seq0 + pos) * (p.n_q_heads * DH) + head * DH + c0 : nullptr;
+          if (!p.prefix_mode && o32row != nullptr) {
+            // frame-local pass ahead of a prefix pass: normalised fp32 to the scratch
 #pragma unroll
-          for (int q4 = 0; q4 < 4; ++q4) {
-            uint4 old4 = make_uint4(0u, 0u, 0u, 0u);
-            if (p.prefix_mode) old4 = *reinterpret_cast<const uint4*>(dst + c0 + 8 * q4);
-            const uint32_t ow[4] = {old4.x, old4.y, old4.z, old4.w};
-            uint32_t o[4];
+            for (int q = 0; q < 8; ++q)
+              reinterpret_cast<float4*>(o32row)[q] =
+                  make_float4(__uint_as_float(r[4 * q]) * w_new, __uint_as_float(r[4 * q + 1]) * w_new,
+                              __uint_as_float(r[4 * q + 2]) * w_new, __uint_as_float(r[4 * q + 3]) * w_new);
+          } else {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const float lo = __uint_as_float(r[8 * q4 + 2 * e]) * w_new + __uint_as_float(ow[e] << 16) * w_old;
-              const float hi = __uint_as_float(r[8 * q4 + 2 * e + 1]) * w_new + __uint_as_float(ow[e] & 0xFFFF0000u) * w_old;
-              __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
-              o[e] = *reinterpret_cast<uint32_t*>(&v);
+            for (int q4 = 0; q4 < 4; ++q4) {
+              float4 oa = make_float4(0.f, 0.f, 0.f, 0.f), ob = oa;
+              if (p.prefix_mode) {
+                oa = reinterpret_cast<const float4*>(o32row)[2 * q4];
+                ob = reinterpret_cast<const float4*>(o32row)[2 * q4 + 1];
+              }
+              const float ow[8] = {oa.x, oa.y, oa.z, oa.w, ob.x, ob.y, ob.z, ob.w};
+              uint32_t o[4];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const float lo = __uint_as_float(r[8 * q4 + 2 * e]) * w_new + ow[2 * e] * w_old;
+                const float hi = __uint_as_float(r[8 * q4 + 2 * e + 1]) * w_new + ow[2 * e + 1] * w_old;
+                __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+                o[e] = *reinterpret_cast<uint32_t*>(&v);
+              }
+              *reinterpret_cast<uint4*>(dst + c0 + 8 * q4) = make_uint4(o[0], o[1], o[2], o[3]);
             }
-            *reinterpret_cast<uint4*>(dst + c0 + 8 * q4) = make_uint4(o[0], o[1], o[2], o[3]);
           }
         }
       }

@@ -185,6 +185,7 @@ struct te_handle {
   bf16* kv_prefix = nullptr;
   std::vector<CUtensorMap> tm_prefix;  // per layer: the prefix cache [P, 2*Hkv*dh] in 64-row boxes (tcgen05 attention)
   float2* attn_stats = nullptr;        // [max_tokens, Hq] (row max, row sum) of the frame-local attention pass
+  float* attn_o32 = nullptr;           // [max_tokens, Hq*dh] its normalised fp32 output (blended with the prefix pass in fp32)
   float* prefix_buf = nullptr;    // [max_prefix, d] hidden states of the prefix pass when the caller wants no output
   int32_t* prefix_lens = nullptr; // device [1]
   int prefix_len = 0;
@@ -764,7 +765,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         te::AttnTcParams tp{};
         tp.out = h->attn; tp.cu_seqlens = h->cu; tp.n_q_heads = c.n_q_heads; tp.n_kv_heads = c.n_kv_heads;
         tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2; tp.non_causal = c.non_causal;
-        tp.stats = P > 0 ? h->attn_stats : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
+        tp.stats = P > 0 ? h->attn_stats : nullptr; tp.o32 = P > 0 ? h->attn_o32 : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
         tp.out8 = pl.mx ? h->attn8 : nullptr; tp.sf_out = h->sf_attn;
         tp.trace = trace_ptr(4); tp.trace_ctas = h->sm_count;
         TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st)
@@ -1010,7 +1011,8 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
         cudaMalloc(reinterpret_cast<void**>(&h->prefix_buf), (size_t)c.max_prefix_tokens * c.hidden * sizeof(float)) !=
             cudaSuccess ||
         cudaMalloc(reinterpret_cast<void**>(&h->prefix_lens), sizeof(int32_t)) != cudaSuccess ||
-        cudaMalloc(reinterpret_cast<void**>(&h->attn_stats), T * c.n_q_heads * sizeof(float2)) != cudaSuccess)
+        cudaMalloc(reinterpret_cast<void**>(&h->attn_stats), T * c.n_q_heads * sizeof(float2)) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&h->attn_o32), T * (size_t)n_q * sizeof(float)) != cudaSuccess)
       return fail(TE_ERR_CUDA);
   }
   {  // activation tensor maps over the whole workspace buffers (encoded once)
@@ -1842,7 +1844,7 @@ void te_destroy(te_handle* h) {
   void* ptrs[] = {h->w, h->dyn, h->resid, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv,
                   h->attn, h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
                   h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens,
-                  h->attn_stats, h->w8, h->sfw, h->xg8, h->attn8, h->act8, h->sf_xg, h->sf_attn, h->sf_act};
+                  h->attn_stats, h->attn_o32, h->w8, h->sfw, h->xg8, h->attn8, h->act8, h->sf_xg, h->sf_attn, h->sf_act};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto& sl : h->slot)
