@@ -338,3 +338,29 @@ def test_bf16_embeddings_equal_fp32_call(H):
     assert torch.equal(o32, o16)
     assert te.te_graph_captures(enc.h) == 1          # same shape class: the second call replays the first graph
     enc.close()
+
+
+def test_vision_handle_reuse_across_batch_sizes():
+    """One front-end handle, calls with shrinking and growing frame counts (operand rows left by a larger call stay in
+    the library's buffers; the tower replays one graph per shape class): every call equals a fresh handle's, bitwise."""
+    import torch
+    import paper_2606_05981_b200 as te
+    v = W.VISION_TINY
+    blob = W.make_vision_blob(v)
+    px = W.make_pixels(v, 5)
+    n_vis = v.tokens_per_frame
+    enc = te.VisionEncoder(v, 5)
+    enc.load_weights(blob)
+    got = {}
+    for B in (5, 2, 5, 1):
+        pd = torch.from_numpy(px[:B]).cuda()
+        emb = torch.zeros((B * n_vis, v.out_hidden), dtype=torch.float32, device="cuda")
+        enc.encode_image(B, pd, None, emb)
+        torch.cuda.synchronize()
+        got.setdefault(B, []).append(emb.cpu().numpy())
+    assert te.te_graph_captures(te.te_vision_debug_tower(enc.v)) <= 3
+    enc.close()
+    assert np.array_equal(got[5][0], got[5][1])
+    for B in (2, 1):
+        fresh, _, _ = _run_gpu(v, blob, px[:B])
+        assert np.array_equal(got[B][0], fresh), B
