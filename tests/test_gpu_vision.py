@@ -364,3 +364,45 @@ def test_vision_handle_reuse_across_batch_sizes():
     for B in (2, 1):
         fresh, _, _ = _run_gpu(v, blob, px[:B])
         assert np.array_equal(got[B][0], fresh), B
+
+
+def test_per_frame_grids_full_width_ragged(O, H):
+    """te_encode_ex at full width in the large-batch dispatch (CTA pairs, wide residual tiles, tcgen05 attention sized for
+    the longest frame the capacities allow): 32 frames with five different grids (square, wide, tall, odd, none) and
+    ragged text, one layer, every row against the per-frame oracle; ids and offsets bit-exact."""
+    import torch
+    import paper_2606_05981_b200 as te
+    m = W.FULL1
+    blob = H.cached_blob(m, 1)
+    rng = np.random.default_rng(77)
+    shapes = np.asarray([[8, 8], [4, 16], [12, 5], [7, 9], [0, 0]], dtype=np.int32)
+    grids = shapes[rng.integers(0, len(shapes), size=32)]
+    tl = rng.integers(16, 97, size=32).astype(np.int32)
+    S = grids[:, 0] * grids[:, 1] + tl
+    T = int(S.sum())
+    emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+    emb[:, [5, 1500]] *= np.float32(1000.0)
+    enc = te.TextEncoder(m, 32, T)
+    enc.load_weights(blob)
+    e = torch.from_numpy(emb).cuda()
+    out = torch.empty_like(e)
+    enc.encode_ex(32, torch.from_numpy(np.ascontiguousarray(grids)).cuda(), 0, 0, e, 0, torch.from_numpy(tl).cuda(), T, out)
+    torch.cuda.synchronize()
+    assert te.te_query_async_error(enc.h) == te.TE_OK
+    pos = np.empty((3, T), dtype=np.int32)
+    te.te_debug_tap(enc.h, te.TE_TAP_POS, pos)
+    got = out.cpu().numpy()
+    enc.close()
+    lay = W.blob_layout(m)
+    ref = np.empty((T, m.hidden))
+    want_pos = np.empty((3, T), dtype=np.int64)
+    r = 0
+    for b in range(32):
+        rows = slice(r, r + int(S[b]))
+        gh, gw = int(grids[b, 0]), int(grids[b, 1])
+        want_pos[:, rows] = O.position_ids([int(tl[b])], gh, gw)
+        ref[rows] = O.encode(blob, lay, m, emb[rows], [int(tl[b])], gh, gw)
+        r += int(S[b])
+    assert np.array_equal(pos, want_pos)
+    mm = PM.stack_metrics(got, ref, emb, outlier_ch=[5, 1500])
+    assert PM.passes_final_gates(mm), mm
