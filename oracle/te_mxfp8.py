@@ -151,8 +151,9 @@ def layer_forward_mxfp8(x: np.ndarray, Wq: dict, phi: np.ndarray, m, taps: dict 
 
 
 def encode_mxfp8(blob_bits, layout, m, embeds, text_lens, grid_h, grid_w, *, frames=None, layer_begin=0,
-                 layer_end=None, taps=None, weights_cache: dict | None = None) -> np.ndarray:
+                 layer_end=None, taps=None, weights_cache: dict | None = None, fp4_weights: bool = False) -> np.ndarray:
     """te_encode of the MXFP8 network in float64 (positions, packing and angles are te_oracle's).
+    fp4_weights: the weight matrices are MXFP4 instead (reading Q32; activations stay MXFP8).
     weights_cache (optional, plumbing only): {layer: quantised weights} kept between calls on the same blob as float32
     (dequantised MXFP8 values are exact in float32), so that several workloads share one pass of the quantiser."""
     from . import te_oracle as O
@@ -167,7 +168,7 @@ def encode_mxfp8(blob_bits, layout, m, embeds, text_lens, grid_h, grid_w, *, fra
         if weights_cache is not None and l in weights_cache:
             Wl = {k: v.astype(np.float64) for k, v in weights_cache[l].items()}
         else:
-            Wl = quantise_layer_weights(O.unpack_layer(blob_bits, layout, l))
+            Wl = (quantise_layer_weights_fp4 if fp4_weights else quantise_layer_weights)(O.unpack_layer(blob_bits, layout, l))
             if weights_cache is not None:
                 weights_cache[l] = {k: v.astype(np.float32) for k, v in Wl.items()}
                 assert all(np.array_equal(weights_cache[l][k].astype(np.float64), Wl[k]) for k in ("Wq", "g1"))
@@ -185,4 +186,85 @@ def encode_mxfp8(blob_bits, layout, m, embeds, text_lens, grid_h, grid_w, *, fra
         for key in ftaps[sel[0]]:
             taps[key] = [np.concatenate([ftaps[b][key][i] for b in sel], axis=0)
                          for i in range(len(ftaps[sel[0]][key]))]
+    return out
+
+
+# ====================================================================== MXFP4 weights (reading Q32)
+# te_config.weight_dtype = 2: the four weight matrices of a layer are OCP MXFP4 — blocks of 32 consecutive in_features
+# share one E8M0 scale, elements are FP4 E2M1 (1 sign, 2 exponent bits with bias 1, 1 mantissa bit: magnitudes
+# 0, 0.5, 1, 1.5, 2, 3, 4, 6) — while the GEMMs' A operands stay MXFP8 exactly as above ("W4A8": the tensor core's
+# kind::mxf8f6f4 multiplies E4M3 by E2M1 directly).  Scale rule as Q25 with the element maximum 6 = 1.5 * 2^2: X is the
+# smallest power of two with amax / X <= 6:  code = clamp(E - 2 + [1.m > 1.5], 0, 254).  The paper names MXFP4 on
+# Blackwell as future work and fixes nothing about it.
+E2M1_MAX = 6.0
+_GRID4 = np.asarray([0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0])   # magnitudes in code order (codes 0 .. 7)
+
+
+def e2m1_decode(code: np.ndarray) -> np.ndarray:
+    """FP4 E2M1 code (0 .. 15) -> float64 from the definition: s = bit 3, e = bits 2:1 (bias 1), m = bit 0:
+    e == 0 -> (-1)^s * m * 0.5;  else (-1)^s * (1 + m / 2) * 2^(e - 1)."""
+    c = np.asarray(code, dtype=np.uint8).astype(np.int64)
+    s = np.where(c & 0x8, -1.0, 1.0)
+    e = (c >> 1) & 0x3
+    m = (c & 0x1).astype(np.float64)
+    return s * np.where(e == 0, 0.5 * m, (1.0 + 0.5 * m) * 2.0 ** (e.astype(np.float64) - 1.0))
+
+
+def e2m1_encode_rne(v: np.ndarray) -> np.ndarray:
+    """float -> nearest E2M1 code (0 .. 15), ties to the even code (even mantissa bit), |v| <= 6 assumed (larger
+    magnitudes clamp to 6).  Nearest-value search over the eight magnitudes."""
+    v = np.asarray(v, dtype=np.float64)
+    a = np.minimum(np.abs(v), E2M1_MAX)
+    hi = np.clip(np.searchsorted(_GRID4, a, side="left"), 0, 7)
+    lo = np.clip(hi - 1, 0, 7)
+    d_lo, d_hi = a - _GRID4[lo], _GRID4[hi] - a
+    pick_hi = (d_hi < d_lo) | ((d_hi == d_lo) & (hi % 2 == 0))
+    code = np.where(pick_hi, hi, lo).astype(np.uint8)
+    return np.where(np.signbit(v), code | 0x8, code).astype(np.uint8)
+
+
+def scale_code_fp4(amax32: np.ndarray) -> np.ndarray:
+    """E8M0 code of an MXFP4 block from its float32 amax: smallest power of two X with amax / X <= 6."""
+    bits = np.asarray(amax32, dtype=np.float32).view(np.uint32).astype(np.int64)
+    E = (bits >> 23) & 0xFF
+    mant = bits & 0x7FFFFF
+    code = E - 2 + (mant > 0x400000)                      # 1.m > 1.5  <=>  mantissa field > 0.5 * 2^23
+    return np.clip(code, 0, 254).astype(np.uint8)
+
+
+def quantise_fp4(x: np.ndarray):
+    """x: [..., K] (K % 32 == 0).  Returns (codes uint8 [..., K] with values 0 .. 15, scales uint8 [..., K/32])."""
+    x32 = np.asarray(x, dtype=np.float32)
+    assert x32.shape[-1] % BLOCK == 0
+    blk = x32.reshape(x32.shape[:-1] + (x32.shape[-1] // BLOCK, BLOCK))
+    sc = scale_code_fp4(np.max(np.abs(blk), axis=-1))
+    X = np.float64(2.0) ** (sc.astype(np.float64) - 127.0)
+    codes = e2m1_encode_rne(blk.astype(np.float64) / X[..., None])
+    return codes.reshape(x32.shape), sc
+
+
+def pack_fp4(codes: np.ndarray) -> np.ndarray:
+    """[..., K] codes 0 .. 15 -> [..., K/2] bytes: element 2i in the low nibble, element 2i+1 in the high nibble."""
+    c = np.asarray(codes, dtype=np.uint8)
+    return (c[..., 0::2] | (c[..., 1::2] << 4)).astype(np.uint8)
+
+
+def dequantise_fp4(codes: np.ndarray, scales: np.ndarray) -> np.ndarray:
+    c = np.asarray(codes, dtype=np.uint8)
+    blk = e2m1_decode(c).reshape(c.shape[:-1] + (c.shape[-1] // BLOCK, BLOCK))
+    X = np.float64(2.0) ** (np.asarray(scales, dtype=np.uint8).astype(np.float64) - 127.0)
+    return (blk * X[..., None]).reshape(c.shape)
+
+
+def fake_quant_fp4(x: np.ndarray) -> np.ndarray:
+    """dequantise_fp4(quantise_fp4(x)) -> float64."""
+    c, s = quantise_fp4(x)
+    return dequantise_fp4(c, s)
+
+
+def quantise_layer_weights_fp4(W: dict) -> dict:
+    """The four GEMMs' matrices -> their dequantised MXFP4 values; gains unchanged."""
+    out = dict(W)
+    for name in ("Wq", "Wk", "Wv", "Wo", "Wgate", "Wup", "Wdown"):
+        out[name] = fake_quant_fp4(W[name])
     return out

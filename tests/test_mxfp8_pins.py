@@ -134,3 +134,71 @@ def test_quantised_network_special_cases():
     snapped = Q.fake_quant(Wl["Wq"])
     assert np.array_equal(Q.fake_quant(snapped), snapped)
     assert np.max(np.abs(snapped - Wl["Wq"]) / np.abs(Wl["Wq"]).max()) < 2.0 ** -4
+
+
+# ---------------------------------------------------------------- MXFP4 weights (reading Q32)
+def test_e2m1_codes_hand_typed():
+    """All sixteen E2M1 codes from the format definition (sign, 2-bit exponent with bias 1, 1 mantissa bit)."""
+    want = [0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0]
+    assert Q.e2m1_decode(np.arange(8)).tolist() == want
+    assert Q.e2m1_decode(np.arange(8, 16)).tolist() == [-x for x in want]
+
+
+def test_e2m1_rounding_hand_worked():
+    """Nearest value, ties to the even code: every midpoint of the grid typed by hand, plus off-midpoint and clamped cases."""
+    v = np.asarray([0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0])           # the seven midpoints
+    assert Q.e2m1_encode_rne(v).tolist() == [0, 2, 2, 4, 4, 6, 6]      # -> 0, 1, 1, 2, 2, 4, 4
+    assert Q.e2m1_encode_rne(-v).tolist() == [8, 10, 10, 12, 12, 14, 14]
+    v2 = np.asarray([0.2, 0.3, 0.74, 0.76, 2.49, 2.51, 4.99, 5.01, 6.0, 7.5, 100.0])
+    assert Q.e2m1_encode_rne(v2).tolist() == [0, 1, 1, 2, 4, 5, 6, 7, 7, 7, 7]
+    # decode(encode) is the identity on the grid and idempotent everywhere
+    g = Q.e2m1_decode(np.arange(16))
+    assert np.array_equal(Q.e2m1_decode(Q.e2m1_encode_rne(g))[1:], g[1:])
+    x = np.random.default_rng(0).uniform(-6, 6, 1000)
+    once = Q.e2m1_decode(Q.e2m1_encode_rne(x))
+    assert np.array_equal(Q.e2m1_decode(Q.e2m1_encode_rne(once)), once)
+    assert np.max(np.abs(once - x)) <= 1.0                              # half of the widest grid step (4 -> 6)
+
+
+def test_fp4_scale_codes_worked():
+    """Smallest power of two X with amax / X <= 6 (= 1.5 * 2^2): worked from the float32 fields."""
+    amax = np.asarray([6.0, 6.0001, 1.0, 1.5, 1.51, 0.0, 12.0, 0.02, 3.0e-3], dtype=np.float32)
+    code = Q.scale_code_fp4(amax)
+    assert code.tolist()[:7] == [127, 128, 125, 125, 126, 0, 128]
+    X = 2.0 ** (code.astype(np.float64) - 127)
+    nz = amax > 0
+    assert np.all(amax[nz] / X[nz] <= 6.0) and np.all(amax[nz] / (X[nz] / 2) > 6.0)       # smallest such power of two
+
+
+def test_fp4_block_worked_and_packing():
+    """One block typed by hand: amax 3.0 -> X = 0.5 (3 / 0.5 = 6), elements v / 0.5 rounded to the grid."""
+    blk = np.zeros(32, dtype=np.float32)
+    blk[:8] = [3.0, -1.5, 0.26, 0.74, 1.1, -0.6, 2.2, 0.1]
+    codes, sc = Q.quantise_fp4(blk[None, :])
+    assert sc.tolist() == [[126]]
+    # v / 0.5 = 6, -3, 0.52, 1.48, 2.2, -1.2, 4.4, 0.2  ->  6, -3, 0.5, 1.5, 2, -1, 4, 0
+    assert codes[0, :8].tolist() == [7, 13, 1, 3, 4, 10, 6, 0]
+    assert Q.dequantise_fp4(codes, sc)[0, :8].tolist() == [3.0, -1.5, 0.25, 0.75, 1.0, -0.5, 2.0, 0.0]
+    packed = Q.pack_fp4(codes)
+    assert packed.shape == (1, 16) and packed[0, :4].tolist() == [7 | (13 << 4), 1 | (3 << 4), 4 | (10 << 4), 6 | (0 << 4)]
+    assert np.array_equal(Q.fake_quant_fp4(blk[None, :]), Q.dequantise_fp4(codes, sc))
+
+
+def test_fp4_network_special_cases():
+    """The W4A8 network: weights exactly representable in MXFP4 make it the MXFP8 network; quantisation noise of the
+    weights is the expected ~10 % class on a GEMM (24 dB SQNR ballpark of a 1-mantissa-bit format)."""
+    import workloads as W
+    from oracle import te_oracle as O
+    m = W.TINY
+    blob = W.make_weight_blob(m, 1)
+    lay = W.blob_layout(m)
+    Wl = O.unpack_layer(blob, lay, 0)
+    W4 = Q.quantise_layer_weights_fp4(Wl)
+    again = Q.quantise_layer_weights_fp4(W4)                           # idempotent
+    assert all(np.array_equal(W4[k], again[k]) for k in ("Wq", "Wo", "Wgate", "Wdown"))
+    assert np.array_equal(W4["g1"], Wl["g1"])                           # gains untouched
+    rel = np.linalg.norm(W4["Wq"] - Wl["Wq"]) / np.linalg.norm(Wl["Wq"])
+    assert 0.05 < rel < 0.2, rel
+    # MXFP4-representable weights: MXFP8 quantisation leaves them unchanged too -> the two networks coincide
+    w8 = Q.quantise_layer_weights(W4)
+    assert all(np.array_equal(w8[k], W4[k]) for k in ("Wq", "Wk", "Wv", "Wo", "Wgate", "Wup", "Wdown"))
