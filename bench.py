@@ -384,10 +384,12 @@ def main():
                          "load (library bf16 matmuls) on the main stream, one event, as in the paper's Algorithm 1")
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the B=4 (cfg 3) measurement that the default cfg-4 line carries as `secondary`")
-    ap.add_argument("--dtype", default="bf16", choices=["bf16", "mxfp8"],
+    ap.add_argument("--dtype", default="bf16", choices=["bf16", "mxfp8", "mxfp4"],
                     help="mxfp8: the block-scaled FP8 variant (te_config.weight_dtype = 1; SURVEY 8f NEXT-2): E4M3 weights "
                          "and GEMM A operands with one E8M0 scale per 32 K-elements; roofline against 2x the measured "
-                         "bf16 tensor peak (the profiling guide's nominal fp8:bf16 ratio)")
+                         "bf16 tensor peak (the profiling guide's nominal fp8:bf16 ratio).  mxfp4: weights as OCP MXFP4 "
+                         "(E2M1, te_config.weight_dtype = 2), activations MXFP8 — same tensor-pipe rate (kind::mxf8f6f4), "
+                         "a quarter of the bf16 weight bytes")
     ap.add_argument("--pipeline-trace", action="store_true",
                     help="add a `pipeline_trace` block: %%globaltimer stamps written by the kernels at pipeline events "
                          "inside the graph replay (TE_OPT_TRACE), medians over CTAs, for the last layer")
@@ -430,8 +432,10 @@ def main():
     w_rank = dataclasses.replace(w, seed_embeds=w.seed_embeds + rank_seed_offset(rank))
     emb = W.make_embeddings(w_rank, T)
 
-    mx = args.dtype == "mxfp8"
-    enc = te.TextEncoder(m, w.n_frames, T, device=local_rank, max_prefix_tokens=args.prefix, weight_dtype=1 if mx else 0)
+    mx = args.dtype in ("mxfp8", "mxfp4")
+    fp4 = args.dtype == "mxfp4"
+    enc = te.TextEncoder(m, w.n_frames, T, device=local_rank, max_prefix_tokens=args.prefix,
+                         weight_dtype=(2 if fp4 else 1) if mx else 0)
     enc.load_weights(blob)
     opt_ids = {"pdl": te.TE_OPT_PDL, "cta_pair": te.TE_OPT_CTA_PAIR, "resid_bn": te.TE_OPT_RESID_BLOCK_N,
                "graph": te.TE_OPT_USE_GRAPH, "attn_impl": te.TE_OPT_ATTN_IMPL, "split_k": te.TE_OPT_SPLIT_K,
@@ -555,7 +559,7 @@ def main():
     # encodes cfg 3's batch (4 frames x 128 tokens), timed the same way, so the driver's record covers both.
     secondary = None
     tc_ratio = 2.0 if mx else 1.0          # nominal dense fp8 : bf16 tensor throughput (B200_PROFILING.md)
-    wscale = 0.5 if mx else 1.0            # weight bytes per element relative to bf16 (+ 1/32 for the block scales)
+    wscale = (0.25 if fp4 else 0.5) if mx else 1.0   # weight bytes per element relative to bf16 (+ the block scales below)
     if (not args.no_secondary and rank == 0 and args.config == 4 and args.frames == 0 and args.prefix == 0
             and not args.opt):
         secondary = {}
@@ -578,7 +582,7 @@ def main():
         ms3 = [a.elapsed_time(b) for a, b in ev3]
         t3 = sum(ms3) / 1000.0 / n3
         f3, wb3, ab3 = stack_work(w3.model, [w3.grid_h * w3.grid_w + int(t) for t in tl3])
-        wb3 *= wscale * (1 + 1 / 32 if mx else 1)
+        wb3 *= wscale * ((1 + 1 / 16 if fp4 else 1 + 1 / 32) if mx else 1)
         pk = load_peaks()
         pk = dict(pk, tf_burst=pk["tf_burst"] * tc_ratio, tf_sustained=pk["tf_sustained"] * tc_ratio)
         roof3 = max(f3 / (pk["tf_burst"] * 1e12), (wb3 + ab3) / (pk["hbm_gbs"] * 1e9))
@@ -604,7 +608,7 @@ def main():
         peaks = dict(peaks, tf_burst=peaks["tf_burst"] * tc_ratio, tf_sustained=peaks["tf_sustained"] * tc_ratio,
                      src=peaks["src"] + " bf16 x 2 (nominal fp8:bf16 ratio)")
     flops, wbytes, abytes = stack_work(m, seq_lens)
-    wbytes *= wscale * (1 + 1 / 32 if mx else 1)
+    wbytes *= wscale * ((1 + 1 / 16 if fp4 else 1 + 1 / 32) if mx else 1)
     flops += m.n_layers * sum(4.0 * m.head_dim * m.n_q_heads * s * args.prefix for s in seq_lens)  # prefix keys
     t_step = t_dev / args.steps
     t_compute = flops / (peaks["tf_sustained"] * 1e12)
@@ -624,7 +628,7 @@ def main():
     gu_ms, gu_n = ktimes["gateup"]
     gu_ms_launch = gu_ms / gu_n                      # CUDA events on the launching stream, as the contract asks
     gu_flops = 2.0 * T * m.hidden * 2 * m.ffn
-    gu_bytes = ((1.0 + 1 / 32) * (2 * m.ffn * m.hidden) + (1.0 + 1 / 32) * T * m.hidden + (1.0 + 1 / 32) * T * m.ffn) if mx \
+    gu_bytes = ((0.5 + 1 / 32 if fp4 else 1.0 + 1 / 32) * (2 * m.ffn * m.hidden) + (1.0 + 1 / 32) * T * m.hidden + (1.0 + 1 / 32) * T * m.ffn) if mx \
         else 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
     gu_name = dispatch.get("gateup", "?")
     traffic, traffic_src = PROFILED_TRAFFIC.get((w.name, gu_name.split(" (")[0]), (None, None))
@@ -657,7 +661,8 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "mxfp8 (e4m3 x e8m0 per 32; fp32 accumulate, bf16 attention)" if mx else "bf16",
+        "vs_baseline": None, "dtype": ("mxfp4 weights (e2m1) x mxfp8 activations (e4m3), e8m0 scale per 32; fp32 accumulate, bf16 attention" if fp4
+                  else "mxfp8 (e4m3 x e8m0 per 32; fp32 accumulate, bf16 attention)") if mx else "bf16",
         "data": "synthetic",
         "config": config_dict(w, T, world, args.opt or "defaults", flush_l2,
                               ({"prefix_len": args.prefix, "prefix_pass_ms_once": prefix_ms,

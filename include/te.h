@@ -68,7 +68,10 @@ typedef struct te_config {
                                    quantises the four matrices of every layer to E4M3 with one E8M0 scale per 32
                                    in_features; the GEMMs' A operands (x*g, attention output, SwiGLU output) are
                                    quantised the same way in the producing epilogues; attention, accumulation and the
-                                   residual stream are unchanged.  Needs Hq/Hkv a power of two <= 8 and no prefix      */
+                                   residual stream are unchanged.  Needs Hq/Hkv a power of two <= 8 and no prefix.
+                                   2: as 1, but the four weight matrices are OCP MXFP4 (FP4 E2M1 elements, one E8M0 scale per
+                                   32 in_features; DESIGN.md §3 Q32): half the weight bytes again, the A operands stay MXFP8
+                                   (the tensor core multiplies E4M3 by E2M1 directly)                                      */
   int32_t non_causal;           /* 0 (default): causal attention by sequence index within the frame.  1: every query sees
                                    every key of its own frame (the vision tower's blocks, te_vision_create; DESIGN.md §3
                                    Q29); needs max_prefix_tokens == 0                                                  */

@@ -93,6 +93,14 @@ int te_debug_mx_quantise(int device, const void* src_bf16, int32_t rows, int32_t
 int te_debug_gemm_mxfp8(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m, int32_t n,
                         int32_t k, int32_t block_n);
 
+/* MXFP4 weights (te_config.weight_dtype = 2; DESIGN.md §3 Q32).  te_debug_mx_quantise_fp4: src DEVICE bf16 [rows, k] ->
+ * codes_packed DEVICE uint8 [rows, k/2] (E2M1, element 2i in the low nibble of byte i) and scales_tiled as in
+ * te_debug_mx_quantise.  te_debug_gemm_mxfp4: C = Q8(A) * Q4(B)^T — A quantised to MXFP8, B to MXFP4 on the device,
+ * multiplied by the block-scaled tcgen05 kernel (kind::mxf8f6f4, E4M3 x E2M1).  Same constraints as te_debug_gemm_mxfp8. */
+int te_debug_mx_quantise_fp4(int device, const void* src_bf16, int32_t rows, int32_t k, void* codes_packed, void* scales_tiled);
+int te_debug_gemm_mxfp4(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m, int32_t n,
+                        int32_t k, int32_t block_n);
+
 /* Vision front end taps (te_encode_image): synchronises and copies to `dst` (HOST). */
 enum {
   TE_VTAP_PATCH_EMBEDS = 0, /* fp32 [n_frames*gh*gw, d_v]   x0 = patches * W_pe^T                  */

@@ -43,9 +43,9 @@ EXPORTS = [
     "te_vision_last_error", "te_vision_destroy",
 ]
 DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide", "te_debug_gemm_wide2",
-                 "te_debug_mx_quantise", "te_debug_gemm_mxfp8", "te_vision_debug_tap", "te_vision_debug_tower"]
+                 "te_debug_mx_quantise", "te_debug_gemm_mxfp8", "te_debug_mx_quantise_fp4", "te_debug_gemm_mxfp4", "te_vision_debug_tap", "te_vision_debug_tower"]
 TE_VTAP_PATCH_EMBEDS, TE_VTAP_TOWER_OUT, TE_VTAP_MERGED = 0, 1, 2
-TE_DTYPE_BF16, TE_DTYPE_MXFP8 = 0, 1
+TE_DTYPE_BF16, TE_DTYPE_MXFP8, TE_DTYPE_MXFP4 = 0, 1, 2
 
 
 class TEConfig(Structure):
@@ -135,6 +135,10 @@ def lib() -> ctypes.CDLL:
     L.te_debug_mx_quantise.argtypes = [c_int, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
     L.te_debug_gemm_mxfp8.restype = c_int
     L.te_debug_gemm_mxfp8.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
+    L.te_debug_mx_quantise_fp4.restype = c_int
+    L.te_debug_mx_quantise_fp4.argtypes = [c_int, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
+    L.te_debug_gemm_mxfp4.restype = c_int
+    L.te_debug_gemm_mxfp4.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
     L.te_vision_blob_bytes.restype = c_size_t
     L.te_vision_blob_bytes.argtypes = [POINTER(TEVisionConfig)]
     L.te_vision_create.restype = c_int
@@ -310,6 +314,14 @@ def te_debug_mx_quantise(device, src_bf16, rows, k, codes, scales_tiled):
 
 def te_debug_gemm_mxfp8(device, a_bf16, b_bf16, c, m, n, k, block_n=256):
     _check(lib().te_debug_gemm_mxfp8(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n))
+
+
+def te_debug_mx_quantise_fp4(device, src_bf16, rows, k, codes_packed, scales_tiled):
+    _check(lib().te_debug_mx_quantise_fp4(device, _ptr(src_bf16), rows, k, _ptr(codes_packed), _ptr(scales_tiled)))
+
+
+def te_debug_gemm_mxfp4(device, a_bf16, b_bf16, c, m, n, k, block_n=256):
+    _check(lib().te_debug_gemm_mxfp4(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n))
 
 
 def te_debug_gemm_wide(device, a_bf16, b_bf16, c, m, n, k, n_tiles, halves=0):

@@ -99,6 +99,59 @@ __global__ void te_mx_quantise_bf16_kernel(const __nv_bfloat16* __restrict__ src
   mx_store_block(v, dst + static_cast<size_t>(r) * K + kb * 32, sf + mx_sf_offset_tiled(r, kb, K / 128, tile_rows));
 }
 
+// MXFP4 (reading Q32): bf16 [rows, K] -> packed E2M1 [rows, K/2] (element 2i in the low nibble of byte i) + tiled E8M0
+// scales in the same layout as the MXFP8 weights.  Scale = smallest power of two X with amax / X <= 6; elements
+// round to nearest, ties to the even code, written as explicit comparisons against the seven midpoints of the grid
+// 0, 0.5, 1, 1.5, 2, 3, 4, 6 (v / X is exact).  One thread per 32-element block.  gu_src_tile as in the MXFP8 quantiser.
+__device__ __forceinline__ uint32_t e2m1_code(float v) {
+  const float a = fabsf(v);
+  const uint32_t c = (a > 0.25f) + (a >= 0.75f) + (a > 1.25f) + (a >= 1.75f) + (a > 2.5f) + (a >= 3.5f) + (a > 5.0f);
+  return c | (v < 0.f ? 8u : 0u);
+}
+__global__ void te_mx_quantise_fp4_kernel(const __nv_bfloat16* __restrict__ src, uint8_t* __restrict__ dst,
+                                          uint8_t* __restrict__ sf, int rows, int K, int tile_rows, int gu_src_tile) {
+  const int kb_per_row = K / 32;
+  const long long idx = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (idx >= static_cast<long long>(rows) * kb_per_row) return;
+  const int r = static_cast<int>(idx / kb_per_row), kb = static_cast<int>(idx % kb_per_row);
+  int r_src = r;
+  if (gu_src_tile > 0) {
+    const int half = tile_rows / 2, n = r / tile_rows, rl = r - n * tile_rows;
+    const int col = n * half + (rl < half ? rl : rl - half);
+    const int sh = gu_src_tile / 2;
+    r_src = (col / sh) * gu_src_tile + col % sh + (rl < half ? 0 : sh);
+  }
+  const uint4* s4 = reinterpret_cast<const uint4*>(src + static_cast<size_t>(r_src) * K + kb * 32);
+  float v[32];
+  float amax = 0.f;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const uint4 u = __ldg(s4 + q);
+    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      v[8 * q + 2 * e] = bf16_lo(w[e]);
+      v[8 * q + 2 * e + 1] = bf16_hi(w[e]);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 32; ++j) amax = fmaxf(amax, fabsf(v[j]));
+  const uint32_t b = __float_as_uint(amax);
+  int code = static_cast<int>((b >> 23) & 0xFFu) - 2 + ((b & 0x7FFFFFu) > 0x400000u ? 1 : 0);
+  code = min(max(code, 0), 254);
+  const float inv = mx_inv_scale(static_cast<uint32_t>(code));
+  uint32_t w4[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint32_t acc = 0;
+#pragma unroll
+    for (int e = 0; e < 8; ++e) acc |= e2m1_code(v[8 * q + e] * inv) << (4 * e);
+    w4[q] = acc;
+  }
+  *reinterpret_cast<uint4*>(dst + static_cast<size_t>(r) * (K / 2) + kb * 16) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+  sf[mx_sf_offset_tiled(r, kb, K / 128, tile_rows)] = static_cast<uint8_t>(code);
+}
+
 // ------------------------------------------------------------------ PTX wrappers
 // D[tmem of both CTAs] (+)= (A * SFA) * (B * SFB)^T, MXFP8, M = 256 over the pair.  ONE thread of the leader.
 __device__ __forceinline__ void umma_mxf8_cg2(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
@@ -140,7 +193,12 @@ struct Gemm8Extra {
   uint8_t* q_sf;
   int q_kchunks;
   int q_ld;
+  // MXFP4 weights (te_config.weight_dtype = 2): the B operand's elements are FP4 E2M1.  In shared memory they sit in the
+  // same 128-byte swizzled rows of 128 elements as E4M3 (the tensor map type 16U4_ALIGN16B unpacks 16 nibbles into every
+  // 16-byte chunk: 8 bytes of data, 8 bytes of gap), so only the instruction descriptor's B format changes.
+  int b_fp4;
 };
+constexpr uint32_t UMMA_F8F6F4_E2M1 = 5u;  // element format code of kind::mxf8f6f4 / f8f6f4 operands (E4M3 = 0)
 
 template <int BN, int EPI>
 struct Gemm8Cfg {
@@ -345,6 +403,9 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
+      // bytes that complete on a stage's barrier, both CTAs together.  A packed-FP4 weight box (16U4_ALIGN16B) counts its
+      // GLOBAL bytes (64 per 128-element row), not the 128 bytes it occupies in shared memory.
+      const uint32_t stage_tx = 2 * (Cfg::STAGE_BYTES - (x8.b_fp4 ? Cfg::B_BYTES / 2 : 0));
       auto load_b = [&](int st, int kb, int n_blk, uint32_t bar) {  // weights and their scales: no dependency
         tma_load_2d_cg2(sB + st * Cfg::B_BYTES, &tmB, bar, kb * GEMM8_BK, n_blk * BN + static_cast<int>(rank) * (BN / 2));
 #pragma unroll
@@ -355,7 +416,7 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       };
       const int pre = (pair < num_tiles) ? (num_kb < STAGES ? num_kb : STAGES) : 0;
       for (int i = 0; i < pre; ++i) {
-        if (leader) mbar_arrive_expect_tx(&full[i], 2 * Cfg::STAGE_BYTES);
+        if (leader) mbar_arrive_expect_tx(&full[i], stage_tx);
         load_b(i, i, pair / num_mp, mapa_u32(smem_u32(&full[i]), 0));
       }
       pdl_wait();
@@ -368,7 +429,7 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
           if (!(first && kb < pre)) {
             mbar_wait(&empty[stage], phase ^ 1);
-            if (leader) mbar_arrive_expect_tx(&full[stage], 2 * Cfg::STAGE_BYTES);
+            if (leader) mbar_arrive_expect_tx(&full[stage], stage_tx);
             load_b(stage, kb, n_blk, bar);
           }
           tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM8_BK, a_blk * GEMM_BM);
@@ -381,7 +442,7 @@ te_gemm8_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA only) =====================
     if (leader && elect_one()) {
-      constexpr uint32_t idesc = umma_idesc_mxf8(2 * GEMM_BM, BN);
+      const uint32_t idesc = umma_idesc_mxf8(2 * GEMM_BM, BN) | (x8.b_fp4 ? (UMMA_F8F6F4_E2M1 << 10) : 0u);  // B format [10,13)
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;

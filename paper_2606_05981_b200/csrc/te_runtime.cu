@@ -68,6 +68,21 @@ bool make_tmap_u8(CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// 2-D FP4 (E2M1, two per byte) row-major [rows, cols] weight tensor (MXFP4, te_config.weight_dtype = 2): box = [box_rows,
+// 128 elements]; the 16U4_ALIGN16B type unpacks every 16 nibbles into a 16-byte chunk of shared memory (8 bytes of data +
+// 8 bytes of gap), so a box row is 128 B there, the same geometry as an E4M3 row, with the 128-byte swizzle.
+bool make_tmap_u4(CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols / 2};
+  cuuint32_t box[2] = {128, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_16U4_ALIGN16B, 2, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // Tiled MXFP8 block scales as a [tiles, 128] uint32 tensor: one 512-byte scale tile per row, box = one tile.
 bool make_tmap_sf(CUtensorMap* m, const void* base, uint64_t n_tiles) {
   PFN_encodeTiled fn = get_encode_fn();
@@ -269,10 +284,10 @@ int validate_config(const te_config& c) {
   if (((c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim) % 128 != 0) return TE_ERR_UNSUPPORTED;
   if ((c.n_q_heads * c.head_dim) % 64 != 0) return TE_ERR_UNSUPPORTED;
   if (c.max_tokens_per_frame > 256) return TE_ERR_UNSUPPORTED;
-  if (c.weight_dtype < 0 || c.weight_dtype > 1) return TE_ERR_INVALID_ARG;
+  if (c.weight_dtype < 0 || c.weight_dtype > 2) return TE_ERR_INVALID_ARG;
   if (c.non_causal < 0 || c.non_causal > 1 || (c.non_causal && c.max_prefix_tokens > 0)) return TE_ERR_INVALID_ARG;
-  if (c.weight_dtype == 1) {
-    // MXFP8: 128-element K chunks everywhere; the quantising attention epilogue exists in the tcgen05 kernel only
+  if (c.weight_dtype >= 1) {
+    // MXFP8 / MXFP4 weights: 128-element K chunks everywhere; the quantising attention epilogue exists in the tcgen05 kernel only
     // (G = Hq/Hkv a power of two <= 8); no cached prefix (its merge pass re-reads a bf16 output)
     const int G = c.n_q_heads / c.n_kv_heads;
     if ((c.n_q_heads * c.head_dim) % 128 != 0 || (G & (G - 1)) != 0 || G > 8 || c.max_prefix_tokens > 0)
@@ -527,7 +542,7 @@ Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
   const int n_qkv = (c.n_q_heads + 2 * c.n_kv_heads) * dh;
   Plan pl;
   pl.Tb = Tb;
-  pl.mx = c.weight_dtype == 1;
+  pl.mx = c.weight_dtype >= 1;
   // CTA pairs pay off once there are enough 256-row tiles to fill the SM pairs; small batches keep
   // one CTA per tile so that more SMs stream weights (HBM-bound regime).
   pl.pair = h->pair_mode == 2 ? (Tb >= 1024 ? 1 : 0) : h->pair_mode;
@@ -734,6 +749,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
+        x8.b_fp4 = c.weight_dtype == 2;
         const CUtensorMap& tb = h->tm8[l].qkv[pl.bn_qkv == 256 ? 1 : 0];
         const CUtensorMap &sa = h->tmSF_xg, &sb = h->tm8[l].sf_qkv;
         cudaError_t e = pl.bn_qkv == 256 ? launch_gemm8<256, te::EPI_QKV, 128>(lc, h->tmA_xg8, tb, sa, sb, p, x8, h->sm_count, st)
@@ -796,6 +812,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
+        x8.b_fp4 = c.weight_dtype == 2;
         x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
         TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_attn8, h->tm8[l].o[0], h->tmSF_attn, h->tm8[l].sf_o, p, x8,
                                                         h->sm_count, st)));
@@ -824,6 +841,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
+        x8.b_fp4 = c.weight_dtype == 2;
         x8.q_out = h->act8; x8.q_sf = h->sf_act; x8.q_kchunks = F / 128; x8.q_ld = F;
         p.num_n_blk = 2 * F / pl.bn_gu;
         TE_CUDA(h, pl.bn_gu == 192 ? (launch_gemm8<192, te::EPI_SWIGLU, 128>(lc, h->tmA_xg8, h->tm8[l].gu[0], h->tmSF_xg,
@@ -854,6 +872,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
+        x8.b_fp4 = c.weight_dtype == 2;
         x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
         TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_act8, h->tm8[l].d[0], h->tmSF_act, h->tm8[l].sf_d, p, x8,
                                                         h->sm_count, st)));
@@ -983,7 +1002,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
       cudaMemset(h->dyn, 0, sizeof(te::DynParams)) != cudaSuccess ||
       cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess)
     return fail(TE_ERR_CUDA);
-  if (c.weight_dtype == 1) {  // MXFP8 activations (A operands) + tiled block scales (one byte per 32 elements)
+  if (c.weight_dtype >= 1) {  // MXFP8 activations (A operands) + tiled block scales (one byte per 32 elements)
     const size_t rb = (T + 127) / 128;  // 128-row scale tiles
     if (cudaMalloc(reinterpret_cast<void**>(&h->xg8), T * c.hidden) != cudaSuccess ||
         cudaMalloc(reinterpret_cast<void**>(&h->attn8), T * (size_t)n_q) != cudaSuccess ||
@@ -1100,12 +1119,13 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
     }
   }
   h->gf_off = o;
-  if (e == cudaSuccess && c.weight_dtype == 1) {
+  if (e == cudaSuccess && c.weight_dtype >= 1) {
+    const bool fp4 = c.weight_dtype == 2;  // MXFP4 weights: two elements per byte, same scale layout
     // MXFP8 copies of the four matrices of every layer (gate/up from the interleaved copy) + tiled block scales
     // gate/up tile width of the MXFP8 GEMM: 192 (two accumulator stages) when it divides 2F, else 256
     if ((2 * F) % 192 != 0 || h->bn_gu != 256) h->bn8_gu = 256;
     const size_t gu_tile = (size_t)h->bn8_gu;
-    const size_t per_layer = n_qkv * d + d * n_q + 2 * F * d + d * F;
+    const size_t per_layer = (n_qkv * d + d * n_q + 2 * F * d + d * F) / (fp4 ? 2 : 1);
     // scale tiles (512 B each): 128-row blocks x K/128 chunks; gate/up's are grouped per N tile (2 per 192 or 256 rows)
     auto sf_tiles = [](size_t rows, size_t K, size_t tile_rows) { return rows / tile_rows * ((tile_rows + 127) / 128) * (K / 128); };
     const size_t sf_layer = (sf_tiles(n_qkv, d, 128) + sf_tiles(d, n_q, 128) + sf_tiles(2 * F, d, gu_tile) + sf_tiles(d, F, 128)) * 512;
@@ -1119,10 +1139,14 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
       *w_off = o8;
       *s_off = os;
       const long long blocks = (long long)rows * (K / 32);
-      te::te_mx_quantise_bf16_kernel<<<(unsigned)((blocks + 255) / 256), 256>>>(h->w + src_off, h->w8 + o8, h->sfw + os, (int)rows,
-                                                                              (int)K, (int)tile_rows, gu_src);
+      if (fp4)
+        te::te_mx_quantise_fp4_kernel<<<(unsigned)((blocks + 255) / 256), 256>>>(h->w + src_off, h->w8 + o8, h->sfw + os, (int)rows,
+                                                                               (int)K, (int)tile_rows, gu_src);
+      else
+        te::te_mx_quantise_bf16_kernel<<<(unsigned)((blocks + 255) / 256), 256>>>(h->w + src_off, h->w8 + o8, h->sfw + os, (int)rows,
+                                                                                (int)K, (int)tile_rows, gu_src);
       ok = ok && make_tmap_sf(sf_map, h->sfw + os, sf_tiles(rows, K, tile_rows));
-      o8 += rows * K;
+      o8 += rows * K / (fp4 ? 2 : 1);
       os += sf_tiles(rows, K, tile_rows) * 512;
     };
     for (int l = 0; l < c.n_layers && e == cudaSuccess; ++l) {
@@ -1134,10 +1158,11 @@ int te_load_weights(te_handle* h, const void* blob, size_t n_bytes) {
       e = cudaGetLastError();
       for (int bi = 0; bi < 2; ++bi) {
         const uint32_t box = 64u << bi;
-        ok = ok && make_tmap_u8(&h->tm8[l].qkv[bi], h->w8 + L.q8, n_qkv, d, box);
-        ok = ok && make_tmap_u8(&h->tm8[l].o[bi], h->w8 + L.o8, d, n_q, box);
-        ok = ok && make_tmap_u8(&h->tm8[l].gu[bi], h->w8 + L.gu8, 2 * F, d, bi == 0 && gu_tile == 192 ? 96u : box);
-        ok = ok && make_tmap_u8(&h->tm8[l].d[bi], h->w8 + L.d8, d, F, box);
+        auto wmap = fp4 ? make_tmap_u4 : make_tmap_u8;
+        ok = ok && wmap(&h->tm8[l].qkv[bi], h->w8 + L.q8, n_qkv, d, box);
+        ok = ok && wmap(&h->tm8[l].o[bi], h->w8 + L.o8, d, n_q, box);
+        ok = ok && wmap(&h->tm8[l].gu[bi], h->w8 + L.gu8, 2 * F, d, bi == 0 && gu_tile == 192 ? 96u : box);
+        ok = ok && wmap(&h->tm8[l].d[bi], h->w8 + L.d8, d, F, box);
       }
     }
   }
@@ -1618,8 +1643,8 @@ int te_debug_mx_quantise(int device, const void* src_bf16, int32_t rows, int32_t
   return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
-int te_debug_gemm_mxfp8(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
-                        int32_t block_n) {
+static int debug_gemm_mx(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                        int32_t block_n, bool fp4) {
   int sms = 0;
   int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
   if (rc != TE_OK) return rc;
@@ -1631,7 +1656,8 @@ int te_debug_gemm_mxfp8(int device, const void* a, const void* b, float* cmat, i
       if (q) cudaFree(q);
     return code;
   };
-  if (cudaMalloc(reinterpret_cast<void**>(&a8), m_pad * k) != cudaSuccess || cudaMalloc(reinterpret_cast<void**>(&b8), (size_t)n * k) != cudaSuccess ||
+  if (cudaMalloc(reinterpret_cast<void**>(&a8), m_pad * k) != cudaSuccess ||
+      cudaMalloc(reinterpret_cast<void**>(&b8), (size_t)n * k / (fp4 ? 2 : 1)) != cudaSuccess ||
       cudaMalloc(reinterpret_cast<void**>(&sa), m_pad * k / 32) != cudaSuccess ||
       cudaMalloc(reinterpret_cast<void**>(&sb), (size_t)n * k / 32) != cudaSuccess)
     return done(TE_ERR_CUDA);
@@ -1639,20 +1665,46 @@ int te_debug_gemm_mxfp8(int device, const void* a, const void* b, float* cmat, i
   cudaMemset(sa, 127, m_pad * k / 32);
   const long long ba = (long long)m * (k / 32), bb = (long long)n * (k / 32);
   te::te_mx_quantise_bf16_kernel<<<(unsigned)((ba + 255) / 256), 256>>>(static_cast<const bf16*>(a), a8, sa, m, k, 128, 0);
-  te::te_mx_quantise_bf16_kernel<<<(unsigned)((bb + 255) / 256), 256>>>(static_cast<const bf16*>(b), b8, sb, n, k, 128, 0);
+  if (fp4)
+    te::te_mx_quantise_fp4_kernel<<<(unsigned)((bb + 255) / 256), 256>>>(static_cast<const bf16*>(b), b8, sb, n, k, 128, 0);
+  else
+    te::te_mx_quantise_bf16_kernel<<<(unsigned)((bb + 255) / 256), 256>>>(static_cast<const bf16*>(b), b8, sb, n, k, 128, 0);
   CUtensorMap ta, tb, tsa, tsb;
-  if (!make_tmap_u8(&ta, a8, m_pad, k, te::GEMM_BM) || !make_tmap_u8(&tb, b8, n, k, block_n / 2) ||
+  if (!make_tmap_u8(&ta, a8, m_pad, k, te::GEMM_BM) ||
+      !(fp4 ? make_tmap_u4(&tb, b8, n, k, block_n / 2) : make_tmap_u8(&tb, b8, n, k, block_n / 2)) ||
       !make_tmap_sf(&tsa, sa, m_pad * k / 32 / 512) || !make_tmap_sf(&tsb, sb, ((size_t)n + 127) / 128 * (k / 128)))
     return done(TE_ERR_CUDA);
   te::GemmParams p{};
   p.M = m; p.N = n; p.K = k; p.num_m_blk = (m + te::GEMM_BM - 1) / te::GEMM_BM; p.num_n_blk = n / block_n;
   p.c = cmat; p.ld_c = n;
   te::Gemm8Extra x8{};
+  x8.b_fp4 = fp4 ? 1 : 0;
   const LaunchCtx lc;
   cudaError_t e = block_n == 256 ? launch_gemm8<256, te::EPI_PLAIN, 128>(lc, ta, tb, tsa, tsb, p, x8, sms, nullptr)
                                  : launch_gemm8<128, te::EPI_PLAIN, 128>(lc, ta, tb, tsa, tsb, p, x8, sms, nullptr);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   return done(e == cudaSuccess ? TE_OK : TE_ERR_CUDA);
+}
+
+int te_debug_gemm_mxfp8(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                        int32_t block_n) {
+  return debug_gemm_mx(device, a, b, cmat, m, n, k, block_n, false);
+}
+
+int te_debug_gemm_mxfp4(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                        int32_t block_n) {
+  return debug_gemm_mx(device, a, b, cmat, m, n, k, block_n, true);
+}
+
+int te_debug_mx_quantise_fp4(int device, const void* src_bf16, int32_t rows, int32_t k, void* codes_packed, void* scales_tiled) {
+  if (!src_bf16 || !codes_packed || !scales_tiled || rows < 1 || k < 128 || k % 128 != 0) return TE_ERR_INVALID_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
+  const long long blocks = (long long)rows * (k / 32);
+  te::te_mx_quantise_fp4_kernel<<<(unsigned)((blocks + 255) / 256), 256>>>(
+      static_cast<const bf16*>(src_bf16), static_cast<uint8_t*>(codes_packed), static_cast<uint8_t*>(scales_tiled), rows, k, 128, 0);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
 
 // ---------------------------------------------------------------- vision-tower front end (NEXT-4)
