@@ -440,7 +440,7 @@ def main():
     opt_ids = {"pdl": te.TE_OPT_PDL, "cta_pair": te.TE_OPT_CTA_PAIR, "resid_bn": te.TE_OPT_RESID_BLOCK_N,
                "graph": te.TE_OPT_USE_GRAPH, "attn_impl": te.TE_OPT_ATTN_IMPL, "split_k": te.TE_OPT_SPLIT_K,
                "resid_wide": te.TE_OPT_RESID_WIDE, "l2_residual": te.TE_OPT_L2_RESIDUAL,
-               "resid_halves": te.TE_OPT_RESID_HALVES}
+               "resid_halves": te.TE_OPT_RESID_HALVES, "chain": te.TE_OPT_CHAIN}
     for kv in filter(None, args.opt.split(",")):
         k, v = kv.split("=")
         te.te_set_option(enc.h, opt_ids[k], int(v))

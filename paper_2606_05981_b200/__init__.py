@@ -30,6 +30,7 @@ TE_OPT_SPLIT_K = 7
 TE_OPT_RESID_WIDE = 9
 TE_OPT_L2_RESIDUAL = 10
 TE_OPT_RESID_HALVES = 11
+TE_OPT_CHAIN = 13
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 TE_TAP_ATTN8, TE_TAP_ACT8, TE_TAP_SF_ATTN, TE_TAP_SF_ACT = 8, 9, 10, 11

@@ -166,7 +166,7 @@ __device__ __forceinline__ void resid_issue(const GemmParams& p, int M, ResidPre
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const int row = row_base + sub + 4 * i;
-    if (row < M) pf.xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
+    if (row < M) pf.xv[i] = __ldcg(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col));  // (L2: see te_gemm_chain.cuh)
   }
 }
 template <int BN>
@@ -246,10 +246,10 @@ __device__ __forceinline__ float row_rstd(const GemmParams& p, int row, bool val
     const float* q = p.ssq_in + (size_t)row * p.ssq_stride;
     int i = 0;
     for (; i + 4 <= p.ssq_parts; i += 4) {  // sequential sum, fixed order
-      const float4 v = *reinterpret_cast<const float4*>(q + i);
+      const float4 v = __ldcg(reinterpret_cast<const float4*>(q + i));  // (L2: rewritten between phases of a chain launch)
       s += v.x; s += v.y; s += v.z; s += v.w;
     }
-    for (; i < p.ssq_parts; ++i) s += q[i];
+    for (; i < p.ssq_parts; ++i) s += __ldcg(q + i);
   }
   return 1.0f / sqrtf(s * p.inv_d + p.eps);
 }

@@ -100,7 +100,7 @@ __device__ __forceinline__ void slice_aux_load(const GemmParams& p, int M, Slice
     if constexpr (EPI == EPI_RESID) {
 #pragma unroll
       for (int v = 0; v < NV; ++v)
-        if (ok) ax.xv[b][v] = *(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + n_blk * BN + v * 128) + lane);
+        if (ok) ax.xv[b][v] = __ldcg(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + n_blk * BN + v * 128) + lane);
     }
     if constexpr (EPI == EPI_QKV) {
       if (ok) {
@@ -114,9 +114,9 @@ __device__ __forceinline__ void slice_aux_load(const GemmParams& p, int M, Slice
       float sq = 0.f;
       if (ok) {
         const float* q = p.ssq_in + (size_t)row * p.ssq_stride;
-        sq = (lane < p.ssq_parts) ? q[lane] : 0.f;
-        sq += (lane + 32 < p.ssq_parts) ? q[lane + 32] : 0.f;
-        for (int i = lane + 64; i < p.ssq_parts; i += 32) sq += q[i];
+        sq = (lane < p.ssq_parts) ? __ldcg(q + lane) : 0.f;
+        sq += (lane + 32 < p.ssq_parts) ? __ldcg(q + lane + 32) : 0.f;
+        for (int i = lane + 64; i < p.ssq_parts; i += 32) sq += __ldcg(q + i);
       }
       ax.rstd[b] = sq;
     }
@@ -266,7 +266,7 @@ __device__ __forceinline__ void slice_batch(const GemmParams& p, int M, const fl
 template <int BN, int EPI, int DH, int RB, int CAP>
 __device__ __forceinline__ void group_finish(const GemmParams& p, int M, uint64_t* tfull, uint32_t t_row, float* stg,
                                              float* scratch, int S, int s, int tile, int warp, int lane, int m_blk,
-                                             int n_blk) {
+                                             int n_blk, uint32_t tfull_parity = 0) {
   constexpr int NV = BN / 128;
   constexpr int NPARTS = GEMMK_EPI_WARPS / 4;
   constexpr int COLS = BN / NPARTS;
@@ -277,7 +277,7 @@ __device__ __forceinline__ void group_finish(const GemmParams& p, int M, uint64_
   const bool tr = warp == 2 && lane == 0;
   SliceAux<NV, RB> ax;
   slice_aux_load<BN, EPI, DH, RB>(p, M, ax, r_first, dr, lane, m_blk, n_blk);
-  mbar_wait(tfull, 0);
+  mbar_wait(tfull, tfull_parity);
   tc_fence_after();
   if (tr) trace_stamp(p, 5);
   {

@@ -18,6 +18,7 @@
 #include "te_gemm.cuh"
 #include "te_gemm8.cuh"
 #include "te_gemm_splitk.cuh"
+#include "te_gemm_chain.cuh"
 #include "te_gemm_wide.cuh"
 #include "te_prep.cuh"
 #include "te_vision.cuh"
@@ -135,6 +136,7 @@ struct Plan {
   int bn_res = 128, k_res = 0, bx_res = 0, n_blk_res = 0, wide_tiles = 0, wide_bn = 0;
   int parts = 1;       // RMSNorm partial sums per row written by the residual GEMMs
   int attn_tc = 0, attn_split = 1, q_blocks = 1, g_shift = 0, s_bound = 0;
+  int chain = 0;       // small batches: 4 = O-proj -> gate/up -> down -> next QKV in one launch, 2 = down -> next QKV, 0 = none
   int mx = 0;          // MXFP8 variant: every GEMM on te_gemm8_kernel (CTA pairs, block-scaled tcgen05)
 };
 
@@ -151,6 +153,8 @@ struct te_handle {
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   int resid_wide = 1; // residual GEMMs on CTA pairs: 1 = auto (one wave of wide tiles when 128-wide tiles need >= 2
                       // waves), 0 = never, n >= 2 = always with n tiles across N (tests)
+  int chain = 0;        // small batches: consecutive split-K GEMMs as phases of one launch (te_gemm_chain.cuh; measured slower)
+  int* chain_bar = nullptr;  // [2] its grid-barrier arrival / departure counters
   int resid_halves = 0; // wide residual tiles as two column halves (te_gemm_wide2_kernel): 1 = O-proj and down, 2 = O-proj, 0 = one pass
   int l2_resid = 1;          // 1: the residual stream is an L2-persisting access window of every kernel
   size_t l2_limit_bytes = 0; // persisting-L2 carve-out requested for it (0 until the first te_encode sets the limit)
@@ -471,6 +475,14 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
   TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -606,6 +618,9 @@ Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
     pl.n_blk_res = d / 128;
     pl.parts = pl.n_blk_res * 2;
   }
+  // chained launches (te_gemm_chain.cuh): consecutive GEMMs that are all one wave of 128 x 128 split-K tiles
+  if (h->chain && !h->timing && !pl.mx && pl.k_qkv && pl.bn_qkv == 128 && pl.k_res && pl.bn_res == 128)
+    pl.chain = (pl.k_gu && pl.bn_gu == 128) ? 4 : 2;
   // attention: host-side upper bound of S_b for the grid (exact lengths stay on the device)
   int s_bound = Tb - (n_frames - 1) * n_vis;
   if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
@@ -662,6 +677,8 @@ std::string describe_plan(const te_handle* h, const Plan& pl) {
   } else {
     gemm("gateup", te::EPI_SWIGLU, pl.k_gu, pl.pair_gu, pl.bn_gu, 128);
   }
+  if (pl.chain == 4) s += "chain=te_gemmk_chain_kernel (oproj, gateup, down and the next layer's qkv as phases of one launch);";
+  if (pl.chain == 2) s += "chain=te_gemmk_chain_kernel (down and the next layer's qkv as phases of one launch);";
   snprintf(b, sizeof(b), "bucket_tokens=%d", pl.Tb);
   s += b;
   return s;
@@ -737,15 +754,84 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
   // the last residual GEMM of the stack hands the stream over to the caller's buffer
   const bool norm_tail = c.final_norm && le == c.n_layers && !dbg_stop;
 
+  // ---- per-GEMM parameters of layer l (shared by the stand-alone launches and by the chained phases)
+  auto qkv_params = [&](int l) {
+    const LayerOff& o = h->off[l];
+    te::GemmParams p = base;
+    p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / pl.bn_qkv;
+    p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
+    p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
+    p.trace = trace_ptr(0);
+    if (pl.k_qkv) {
+      p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+      // two K slices per one-head tile (T = 256: 64 tiles) lose more in the exchange and the 64-row slice epilogues
+      // than they gain in the main loop: 17.6 us against 13.0 us unsplit (B = 2, measured)
+      if (p.splits == 2 && h->split_target == 0) p.splits = 1;
+    }
+    return p;
+  };
+  auto oproj_params = [&](int l, bool last_layer) {
+    const LayerOff& o = h->off[l];
+    te::GemmParams p = base;
+    p.N = d; p.K = n_q; p.num_n_blk = pl.n_blk_res;
+    p.x = h->resid; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
+    p.x_to_out = (dbg_stop && last_layer) ? 1 : 0;
+    p.trace = trace_ptr(1);
+    if (pl.k_res) p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+    return p;
+  };
+  auto gu_params = [&](int l) {
+    te::GemmParams p = base;
+    p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / pl.bn_gu; p.gu_half = pl.gu_half;
+    p.act = h->act; p.ld_act = F;
+    p.trace = trace_ptr(2);
+    if (pl.k_gu) p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+    return p;
+  };
+  auto down_params = [&](int l, bool last_layer) {
+    te::GemmParams p = base;
+    p.N = d; p.K = F; p.num_n_blk = pl.n_blk_res;
+    p.x = h->resid; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
+    p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
+    p.x_to_out = (last_layer && !norm_tail) ? 1 : 0;
+    p.trace = trace_ptr(3);
+    if (pl.k_res) p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
+    return p;
+  };
+  // Chained launches (te_gemm_chain.cuh): consecutive GEMMs that are all one wave of 128 x 128 split-K tiles run as
+  // phases of ONE cooperative grid.  chain4: O-proj -> gate/up -> down -> next layer's QKV (T <= 128);
+  // chain2: down -> next layer's QKV (e.g. T = 512, where gate/up runs on the wide CTA-pair kernel).
+  const bool chain_ok = pl.chain != 0 && !prefix_pass;
+  const bool chain4 = chain_ok && pl.chain == 4;
+  auto launch_chain = [&](int n_ph, const te::GemmParams* ps, const int* epis, const CUtensorMap* const* ma,
+                          const CUtensorMap* const* mb) -> cudaError_t {
+    te::ChainParams cp{};
+    int grid = 1;
+    for (int i = 0; i < n_ph; ++i) {
+      cp.p[i] = ps[i];
+      cp.epi[i] = epis[i];
+      const int ctas = ps[i].num_m_blk * ps[i].num_n_blk * ps[i].splits;
+      if (ctas > grid) grid = ctas;
+    }
+    cp.n_phases = n_ph;
+    cp.gbar = h->chain_bar;
+    LaunchCtx lcc = lc;
+    lcc.coop = true;  // the phases meet at a grid-wide counter: every CTA resident at once
+    const CUtensorMap* fa[te::CHAIN_MAX_PHASES];
+    const CUtensorMap* fb[te::CHAIN_MAX_PHASES];
+    for (int i = 0; i < te::CHAIN_MAX_PHASES; ++i) { fa[i] = ma[i < n_ph ? i : 0]; fb[i] = mb[i < n_ph ? i : 0]; }
+    auto kern = n_ph >= 3 ? (dh == 128 ? te::te_gemmk_chain_kernel<128, true> : te::te_gemmk_chain_kernel<64, true>)
+                          : (dh == 128 ? te::te_gemmk_chain_kernel<128, false> : te::te_gemmk_chain_kernel<64, false>);
+    return launch_k(lcc, kern, dim3(grid), dim3(te::GEMMK_THREADS), te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES, st, *fa[0],
+                    *fb[0], *fa[1], *fb[1], *fa[2], *fb[2], *fa[3], *fb[3], cp);
+  };
+
+  bool qkv_done = false;  // this layer's QKV was the last phase of the previous layer's chain
   for (int l = lb; l < le; ++l) {
     const LayerOff& o = h->off[l];
     const bool last_layer = l == le - 1;
-    {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
-      te::GemmParams p = base;
-      p.N = n_qkv; p.K = d; p.num_n_blk = n_qkv / pl.bn_qkv;
-      p.qkv = h->qkv; p.ld_qkv = n_qkv; p.q_cols_end = n_q; p.k_cols_end = n_q + c.n_kv_heads * dh;
-      p.gq = h->w + o.gq; p.gk = h->w + o.gk; p.cos_t = h->cos_t; p.sin_t = h->sin_t;
-      p.trace = trace_ptr(0);
+    if (!qkv_done) {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
+      te::GemmParams p = qkv_params(l);
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
@@ -757,10 +843,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
                                         : launch_gemm8<128, te::EPI_QKV, 64>(lc, h->tmA_xg8, tb, sa, sb, p, x8, h->sm_count, st);
         TE_CUDA(h, e);
       } else if (pl.k_qkv) {
-        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
-        // two K slices per one-head tile (T = 256: 64 tiles) lose more in the exchange and the 64-row slice epilogues
-        // than they gain in the main loop: 17.6 us against 13.0 us unsplit (B = 2, measured)
-        if (p.splits == 2 && h->split_target == 0) p.splits = 1;
         TE_CUDA(h, launch_gemmk_bn<te::EPI_QKV>(lc, pl.bn_qkv, dh, h->tmA_xg, h->tm[l].qkv[pl.bx_qkv], p, st));
       } else {
         TE_CUDA(h, launch_gemm_bn<te::EPI_QKV>(lc, pl.bn_qkv, pl.pair_qkv, dh, h->tmA_xg, h->tm[l].qkv[pl.bx_qkv], p,
@@ -769,6 +851,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tock(TE_KCLASS_QKV);
       ++nk;
     }
+    qkv_done = false;
     if (prefix_pass) {  // keep this layer's keys | values of the prefix tokens
       TE_CUDA(h, cudaMemcpy2DAsync(h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv, (size_t)n_kv * sizeof(bf16),
                                    h->qkv + n_q, (size_t)n_qkv * sizeof(bf16), (size_t)n_kv * sizeof(bf16),
@@ -803,12 +886,26 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tock(TE_KCLASS_ATTN);
       ++nk;
     }
+    const bool next_qkv = l + 1 < le;  // a following layer whose QKV can ride along
+    if (chain4 && !(dbg_stop && last_layer)) {
+      // a3 + a4 + a5 (+ the next layer's a1) as phases of one launch
+      te::GemmParams ps[4] = {oproj_params(l, last_layer), gu_params(l), down_params(l, last_layer), te::GemmParams{}};
+      int epis[4] = {te::EPI_RESID, te::EPI_SWIGLU, te::EPI_RESID, te::EPI_QKV};
+      const CUtensorMap* ma[4] = {&h->tmA_attn, &h->tmA_xg, &h->tmA_act, &h->tmA_xg};
+      const CUtensorMap* mb[4] = {&h->tm[l].o[pl.bx_res], &h->tm[l].gu[pl.bx_gu], &h->tm[l].d[pl.bx_res], nullptr};
+      int n_ph = 3;
+      if (next_qkv) {
+        ps[3] = qkv_params(l + 1);
+        mb[3] = &h->tm[l + 1].qkv[pl.bx_qkv];
+        n_ph = 4;
+      }
+      TE_CUDA(h, launch_chain(n_ph, ps, epis, ma, mb));
+      ++nk;
+      qkv_done = next_qkv;
+      continue;
+    }
     {  // a3: O projection + residual add (+ next norm's gain / statistics)
-      te::GemmParams p = base;
-      p.N = d; p.K = n_q; p.num_n_blk = pl.n_blk_res;
-      p.x = h->resid; p.ld_x = d; p.g_next = h->w + o.g2; p.xg = h->xg; p.ssq_out = h->ssq;
-      p.x_to_out = (dbg_stop && last_layer) ? 1 : 0;
-      p.trace = trace_ptr(1);
+      te::GemmParams p = oproj_params(l, last_layer);
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
@@ -823,7 +920,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         if (!make_tmap(&tmB, h->w + o.wo, d, n_q, pl.wide_bn / 4)) { h->err = "tensor map (wide O-proj)"; return TE_ERR_CUDA; }
         TE_CUDA(h, launch_wide<te::EPI_RESID>(lc, h->tmA_attn, tmB, p, pl.wide_tiles, pl.wide_bn, st));
       } else if (pl.k_res) {
-        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(lc, pl.bn_res, dh, h->tmA_attn, h->tm[l].o[pl.bx_res], p, st));
       } else {
         TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(lc, pl.bn_res, pl.pair, dh, h->tmA_attn, h->tm[l].o[pl.bx_res], p,
@@ -834,10 +930,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
     }
     if (dbg_stop && last_layer) break;
     {  // a4: RMSNorm -> gate/up GEMM -> SiLU(gate) * up
-      te::GemmParams p = base;
-      p.N = 2 * F; p.K = d; p.num_n_blk = 2 * F / pl.bn_gu; p.gu_half = pl.gu_half;
-      p.act = h->act; p.ld_act = F;
-      p.trace = trace_ptr(2);
+      te::GemmParams p = gu_params(l);
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
@@ -853,7 +946,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         TE_CUDA(h, launch_wide<te::EPI_SWIGLU>(lc, h->tmA_xg, h->tm[l].gu[box_index(32)], p, pl.gu_wide_tiles,
                                                2 * pl.gu_wide_w, st));
       } else if (pl.k_gu) {
-        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_SWIGLU>(lc, pl.bn_gu, dh, h->tmA_xg, h->tm[l].gu[pl.bx_gu], p, st));
       } else {
         TE_CUDA(h, launch_gemm_bn<te::EPI_SWIGLU>(lc, pl.bn_gu, pl.pair_gu, dh, h->tmA_xg, h->tm[l].gu[pl.bx_gu], p,
@@ -862,13 +954,18 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tock(TE_KCLASS_GATEUP);
       ++nk;
     }
+    if (chain_ok && next_qkv) {  // a5 + the next layer's a1 in one launch
+      te::GemmParams ps[2] = {down_params(l, last_layer), qkv_params(l + 1)};
+      int epis[2] = {te::EPI_RESID, te::EPI_QKV};
+      const CUtensorMap* ma[2] = {&h->tmA_act, &h->tmA_xg};
+      const CUtensorMap* mb[2] = {&h->tm[l].d[pl.bx_res], &h->tm[l + 1].qkv[pl.bx_qkv]};
+      TE_CUDA(h, launch_chain(2, ps, epis, ma, mb));
+      ++nk;
+      qkv_done = true;
+      continue;
+    }
     {  // a5: down projection + residual add
-      te::GemmParams p = base;
-      p.N = d; p.K = F; p.num_n_blk = pl.n_blk_res;
-      p.x = h->resid; p.ld_x = d; p.xg = h->xg; p.ssq_out = h->ssq;
-      p.g_next = (l + 1 < c.n_layers) ? h->w + h->off[l + 1].g1 : nullptr;
-      p.x_to_out = (last_layer && !norm_tail) ? 1 : 0;
-      p.trace = trace_ptr(3);
+      te::GemmParams p = down_params(l, last_layer);
       tick();
       if (pl.mx) {
         te::Gemm8Extra x8{};
@@ -883,7 +980,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         if (!make_tmap(&tmB, h->w + o.wd, d, F, pl.wide_bn / 4)) { h->err = "tensor map (wide down)"; return TE_ERR_CUDA; }
         TE_CUDA(h, launch_wide<te::EPI_RESID>(lc, h->tmA_act, tmB, p, pl.wide_tiles, pl.wide_bn, st));
       } else if (pl.k_res) {
-        p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
         TE_CUDA(h, launch_gemmk_bn<te::EPI_RESID>(lc, pl.bn_res, dh, h->tmA_act, h->tm[l].d[pl.bx_res], p, st));
       } else {
         TE_CUDA(h, launch_gemm_bn<te::EPI_RESID>(lc, pl.bn_res, pl.pair, dh, h->tmA_act, h->tm[l].d[pl.bx_res], p,
@@ -993,6 +1089,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   TE_ALLOC(h->act, T * c.ffn * sizeof(bf16));
   TE_ALLOC(h->sk_scratch, (size_t)h->sm_count * te::GEMM_BM * 256 * sizeof(float));
   TE_ALLOC(h->sk_sem, 2 * (size_t)h->sm_count * sizeof(int));
+  TE_ALLOC(h->chain_bar, 2 * sizeof(int));
 #undef TE_ALLOC
   // rows past a call's tokens are read (never stored) by the tile-granular kernels: start them finite
   if (cudaMemset(h->xg, 0, T * c.hidden * sizeof(bf16)) != cudaSuccess ||
@@ -1000,7 +1097,8 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
       cudaMemset(h->attn, 0, T * (size_t)n_q * sizeof(bf16)) != cudaSuccess ||
       cudaMemset(h->act, 0, T * c.ffn * sizeof(bf16)) != cudaSuccess ||
       cudaMemset(h->dyn, 0, sizeof(te::DynParams)) != cudaSuccess ||
-      cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess)
+      cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess ||
+      cudaMemset(h->chain_bar, 0, 2 * sizeof(int)) != cudaSuccess)
     return fail(TE_ERR_CUDA);
   if (c.weight_dtype >= 1) {  // MXFP8 activations (A operands) + tiled block scales (one byte per 32 elements)
     const size_t rb = (T + 127) / 128;  // 128-row scale tiles
@@ -1443,6 +1541,7 @@ int te_set_option(te_handle* h, int option, int value) {
       if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
       h->resid_wide = value;
       break;
+    case TE_OPT_CHAIN: h->chain = value ? 1 : 0; break;
     case TE_OPT_RESID_HALVES:
       if (value < 0 || value > 3) return TE_ERR_INVALID_ARG;
       h->resid_halves = value;
@@ -1895,7 +1994,7 @@ void te_destroy(te_handle* h) {
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->dyn, h->resid, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv,
                   h->attn, h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
-                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens,
+                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->chain_bar, h->kv_prefix, h->prefix_buf, h->prefix_lens,
                   h->attn_stats, h->attn_o32, h->w8, h->sfw, h->xg8, h->attn8, h->act8, h->sf_xg, h->sf_attn, h->sf_act};
   for (void* p : ptrs)
     if (p) cudaFree(p);

@@ -377,6 +377,12 @@ def test_encode_is_async_no_sync_and_counts_launches(H):
     st.synchronize()
     assert not done_at_return
     assert te.te_kernel_launches(g.enc.h) - n0 == 2 + 5 * w.model.n_layers   # refresh + prep + 5 per layer
+    te.te_set_option(g.enc.h, te.TE_OPT_CHAIN, 1)
+    g.encode(emb, tl, 4, 4)
+    n1 = te.te_kernel_launches(g.enc.h)
+    g.encode(emb, tl, 4, 4)
+    # chained: refresh + prep + first QKV + per layer [attention, one launch of O-proj / gate-up / down / next QKV]
+    assert te.te_kernel_launches(g.enc.h) - n1 == 3 + 2 * w.model.n_layers
     g.close()
 
 
@@ -909,4 +915,24 @@ def test_host_path_refuses_a_frame_longer_than_the_capacity(H):
     with pytest.raises(te.TEError) as ei:
         g.enc.encode_host(2, 4, 4, emb, np.asarray([250, 10], dtype=np.int32), out)     # 16 + 250 > 256
     assert ei.value.code == te.TE_ERR_INVALID_ARG
+    g.close()
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_chained_launches_equal_separate_launches_bitwise(H, cfg_id):
+    """te_gemm_chain.cuh: the same tiles, K slices, reduction order and epilogue arithmetic as one launch per GEMM, so
+    the chained stack (O-proj -> gate/up -> down -> next QKV at T <= 128 and on the tiny stack, down -> next QKV at
+    T = 512) must reproduce the unchained one BITWISE — at cfg 3 over all 28 layers — and stay so over repeated replays
+    (the grid-barrier counters are re-armed by every launch)."""
+    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
+    g = H.GpuTE(w.model, w.n_frames, T, blob)
+    g.te.te_set_option(g.enc.h, g.te.TE_OPT_CHAIN, 1)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    assert "chain" in g.te.te_dispatch_info(g.enc.h), g.te.te_dispatch_info(g.enc.h)
+    for _ in range(5):
+        assert np.array_equal(out, g.encode(emb, tl, w.grid_h, w.grid_w))
+    g.te.te_set_option(g.enc.h, g.te.TE_OPT_CHAIN, 0)
+    plain = g.encode(emb, tl, w.grid_h, w.grid_w)
+    assert "chain" not in g.te.te_dispatch_info(g.enc.h)
+    assert np.array_equal(out, plain)
     g.close()
