@@ -321,7 +321,14 @@ __device__ __forceinline__ void group_finish(const GemmParams& p, int M, uint64_
 
 // Scratch layout: [tile][split][128 rows][BN] fp32, row-major (written coalesced through the staging
 // transpose, read one whole row per warp).  Semaphores: sk_sem[2*tile] arrivals, [2*tile+1] departures.
-template <int BN, int EPI, int DH>
+// VAR: which epilogue the instantiation contains — 0: one CTA per tile (S == 1, fused epilogue from tensor memory);
+// 1..6: the split-K group epilogue for one batch shape (gemmk_variant(epi, S * BN / 128) below, for S > 1).  One variant per kernel keeps the code
+// of a launch compact: with all six in one kernel (150-280 KB of SASS) the epilogue, which every warp executes once
+// and cold, was measurably slower.
+__host__ __device__ constexpr int gemmk_variant(int epi, int snv) {
+  return snv <= 1 ? 0 : ((epi != EPI_QKV && snv <= 2) ? 1 : ((epi != EPI_QKV && snv <= 3) ? 2 : (snv <= 4 ? 3 : (snv <= 6 ? 4 : (snv <= 8 ? 5 : 6)))));
+}
+template <int BN, int EPI, int DH, int VAR>
 __global__ void __launch_bounds__(GEMMK_THREADS, 1)
 te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const GemmParams p) {
   using Cfg = GemmKCfg<BN, EPI>;
@@ -440,7 +447,7 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
     const bool tr = warp == 2 && lane == 0;
     pdl_wait();
-    if (S == 1) {
+    if constexpr (VAR == 0) {
       // ---- one CTA per tile: fused epilogue straight from tensor memory
       float rstd = 0.f;
       ResidPrefetch pf;
@@ -458,16 +465,14 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // ---- split-K group (see group_finish).  The batch shape is chosen so that all partials of a batch
       // (RB rows x S*NV float4) fit in ~16-18 float4 per lane: for 128-wide tiles a warp's 16/S rows are a
       // single batch.  (EPI_QKV also keeps a cos/sin row per batch row: at most 4 rows per batch there.)
-      constexpr int NV = BN / 128;
       float* scratch = p.sk_scratch + (size_t)tile * S * GEMM_BM * BN;
-      const int snv = S * NV;
 #define TE_GROUP_FINISH(RB, CAP) \
   group_finish<BN, EPI, DH, RB, CAP>(p, M, tfull, t_row, stg, scratch, S, s, tile, warp, lane, m_blk, n_blk)
-      if (EPI != EPI_QKV && snv <= 2) { TE_GROUP_FINISH(8, 2); }
-      else if (EPI != EPI_QKV && snv <= 3) { TE_GROUP_FINISH(6, 3); }
-      else if (snv <= 4) { TE_GROUP_FINISH(4, 4); }
-      else if (snv <= 6) { TE_GROUP_FINISH(3, 6); }
-      else if (snv <= 8) { TE_GROUP_FINISH(2, 8); }
+      if constexpr (VAR == 1) { TE_GROUP_FINISH(8, 2); }
+      else if constexpr (VAR == 2) { TE_GROUP_FINISH(6, 3); }
+      else if constexpr (VAR == 3) { TE_GROUP_FINISH(4, 4); }
+      else if constexpr (VAR == 4) { TE_GROUP_FINISH(3, 6); }
+      else if constexpr (VAR == 5) { TE_GROUP_FINISH(2, 8); }
       else { TE_GROUP_FINISH(1, 16); }
 #undef TE_GROUP_FINISH
       // the last CTA of the group to leave re-arms both counters for the next launch

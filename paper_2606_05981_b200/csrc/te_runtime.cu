@@ -396,14 +396,29 @@ cudaError_t set_gemm8_attr() {
 }
 
 // split-K kernel: `p.splits` CTAs per 128 x bn tile (small batches; te_gemm_splitk.cuh)
-template <int BN, int EPI, int DH>
-cudaError_t launch_gemmk(LaunchCtx lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
-                         cudaStream_t st) {
+template <int BN, int EPI, int DH, int VAR>
+cudaError_t launch_gemmk_var(LaunchCtx lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
+                             cudaStream_t st) {
   using Cfg = te::GemmKCfg<BN, EPI>;
   const int tiles = p.num_m_blk * p.num_n_blk;
   lc.coop = p.splits > 1;  // the groups spin on each other: all CTAs resident at once, or the launch waits
-  return launch_k(lc, te::te_gemmk_kernel<BN, EPI, DH>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS), Cfg::SMEM_BYTES, st,
-                  tmA, tmB, p);
+  return launch_k(lc, te::te_gemmk_kernel<BN, EPI, DH, VAR>, dim3(tiles * p.splits), dim3(te::GEMMK_THREADS), Cfg::SMEM_BYTES,
+                  st, tmA, tmB, p);
+}
+// split-K kernel: `p.splits` CTAs per 128 x bn tile (small batches; te_gemm_splitk.cuh); one instantiation per epilogue
+// variant (te::gemmk_variant)
+template <int BN, int EPI, int DH>
+cudaError_t launch_gemmk(const LaunchCtx& lc, const CUtensorMap& tmA, const CUtensorMap& tmB, const te::GemmParams& p,
+                         cudaStream_t st) {
+  switch (p.splits == 1 ? 0 : te::gemmk_variant(EPI, p.splits * (BN / 128))) {
+    case 0: return launch_gemmk_var<BN, EPI, DH, 0>(lc, tmA, tmB, p, st);
+    case 1: return launch_gemmk_var<BN, EPI, DH, 1>(lc, tmA, tmB, p, st);
+    case 2: return launch_gemmk_var<BN, EPI, DH, 2>(lc, tmA, tmB, p, st);
+    case 3: return launch_gemmk_var<BN, EPI, DH, 3>(lc, tmA, tmB, p, st);
+    case 4: return launch_gemmk_var<BN, EPI, DH, 4>(lc, tmA, tmB, p, st);
+    case 5: return launch_gemmk_var<BN, EPI, DH, 5>(lc, tmA, tmB, p, st);
+    default: return launch_gemmk_var<BN, EPI, DH, 6>(lc, tmA, tmB, p, st);
+  }
 }
 template <int EPI>
 cudaError_t launch_gemmk_bn(const LaunchCtx& lc, int bn, int dh, const CUtensorMap& a, const CUtensorMap& b,
@@ -454,9 +469,12 @@ cudaError_t set_gemm_attr() {
                                        te::GemmCfg<BN>::SMEM_BYTES);
   if (e != cudaSuccess) return e;
   if constexpr (EPI != te::EPI_QKV || BN == 128) {
-    e = cudaFuncSetAttribute(te::te_gemmk_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             te::GemmKCfg<BN, EPI>::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
+#define TE_KATTR(V)                                                                                              \
+  e = cudaFuncSetAttribute(te::te_gemmk_kernel<BN, EPI, DH, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
+                           te::GemmKCfg<BN, EPI>::SMEM_BYTES);                                                      \
+  if (e != cudaSuccess) return e
+    TE_KATTR(0); TE_KATTR(1); TE_KATTR(2); TE_KATTR(3); TE_KATTR(4); TE_KATTR(5); TE_KATTR(6);
+#undef TE_KATTR
   }
   return cudaFuncSetAttribute(te::te_gemm2_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               te::Gemm2Cfg<BN, EPI>::SMEM_BYTES);
