@@ -32,7 +32,7 @@ enum {
   TE_OPT_CHAIN = 13,       /* 1: at small batches consecutive GEMMs that are all one wave of 128 x 128 split-K tiles
                               run as phases of ONE cooperative launch with grid-wide barriers between them
                               (te_gemm_chain.cuh): O-proj -> gate/up -> down -> next QKV at T <= 128, down -> next QKV at
-                              T = 512.  0 (default): one launch per GEMM.  Bitwise the same results; measured SLOWER than the
+                              T = 512.  0 (default): one launch per GEMM.  Compiled only with -DTE_WITH_CHAIN (else 1 is refused).  Bitwise the same results; measured SLOWER than the
                               PDL-chained separate launches                                          */
   TE_OPT_RESID_WIDE = 9    /* O-proj / down on CTA pairs: 1 (default) = when their 128-wide tiles would need two or
                               more waves, ONE wave of wide tiles (width = hidden / n rounded up to 32, <= 512

@@ -348,29 +348,6 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const int lane = threadIdx.x & 31;
   if (threadIdx.x == 0) trace_stamp(p, 0);
 
-  if (warp == 0 && elect_one()) {
-    tma_prefetch_desc(&tmA);
-    tma_prefetch_desc(&tmB);
-  }
-  if (warp == 1) {
-    if (elect_one()) {
-      for (int i = 0; i < STAGES; ++i) {
-        mbar_init(&full[i], 1);
-        mbar_init(&empty[i], 1);
-      }
-      mbar_init(tfull, 1);
-      fence_mbar_init();
-    }
-    __syncwarp();
-    tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
-  }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
-  pdl_launch_dependents();
-  if (threadIdx.x == 0) trace_stamp(p, 1);
-
   const int M = gemm_rows(p);
   const int S = p.splits;
   const int tile = blockIdx.x / S;
@@ -381,26 +358,47 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const int kb0 = (s * num_kb) / S;
   const int kb1 = ((s + 1) * num_kb) / S;
   const int nkb = kb1 - kb0;
+  // B tile of one k-block: BN weight rows in one box, or (gu_half: 128-wide SwiGLU tile over weights
+  // interleaved per 256 rows; tmB then has 64-row boxes) the 64 gate rows and the 64 matching up rows
+  auto load_b = [&](uint8_t* dst, uint64_t* bar, int kb) {
+    if (p.gu_half) {
+      const int g_row = (n_blk >> 1) * 256 + (n_blk & 1) * 64;
+      tma_load_2d(dst, &tmB, bar, kb * GEMM_BK, g_row);
+      tma_load_2d(dst + 64 * GEMM_BK * 2, &tmB, bar, kb * GEMM_BK, g_row + 128);
+    } else {
+      tma_load_2d(dst, &tmB, bar, kb * GEMM_BK, n_blk * BN);
+    }
+  };
+  const int pre = nkb < STAGES ? nkb : STAGES;
+
+  // The producer thread initialises the barriers itself and requests its first ring of WEIGHT tiles at once — they depend
+  // on nothing, and at small batches their DRAM round trip (~1 us) is what the first MMA waits for — while warp 1
+  // allocates tensor memory; the other warps see the barriers after the block barrier below.
+  if (warp == 0 && elect_one()) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB);
+    for (int i = 0; i < STAGES; ++i) {
+      mbar_init(&full[i], 1);
+      mbar_init(&empty[i], 1);
+    }
+    mbar_init(tfull, 1);
+    fence_mbar_init();
+    for (int i = 0; i < pre; ++i) {
+      mbar_arrive_expect_tx(&full[i], Cfg::STAGE_BYTES);
+      load_b(sB + i * Cfg::B_BYTES, &full[i], kb0 + i);
+    }
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  pdl_launch_dependents();
+  if (threadIdx.x == 0) trace_stamp(p, 1);
 
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (elect_one()) {
-      // B tile of one k-block: BN weight rows in one box, or (gu_half: 128-wide SwiGLU tile over weights
-      // interleaved per 256 rows; tmB then has 64-row boxes) the 64 gate rows and the 64 matching up rows
-      auto load_b = [&](uint8_t* dst, uint64_t* bar, int kb) {
-        if (p.gu_half) {
-          const int g_row = (n_blk >> 1) * 256 + (n_blk & 1) * 64;
-          tma_load_2d(dst, &tmB, bar, kb * GEMM_BK, g_row);
-          tma_load_2d(dst + 64 * GEMM_BK * 2, &tmB, bar, kb * GEMM_BK, g_row + 128);
-        } else {
-          tma_load_2d(dst, &tmB, bar, kb * GEMM_BK, n_blk * BN);
-        }
-      };
-      const int pre = nkb < STAGES ? nkb : STAGES;
-      for (int i = 0; i < pre; ++i) {  // weights first: independent of the predecessor kernel
-        mbar_arrive_expect_tx(&full[i], Cfg::STAGE_BYTES);
-        load_b(sB + i * Cfg::B_BYTES, &full[i], kb0 + i);
-      }
       pdl_wait();
       trace_stamp(p, 2);
       int stage = 0;

@@ -18,7 +18,9 @@
 #include "te_gemm.cuh"
 #include "te_gemm8.cuh"
 #include "te_gemm_splitk.cuh"
+#ifdef TE_WITH_CHAIN  // experiment: build with TE_NVCC_EXTRA=-DTE_WITH_CHAIN
 #include "te_gemm_chain.cuh"
+#endif
 #include "te_gemm_wide.cuh"
 #include "te_prep.cuh"
 #include "te_vision.cuh"
@@ -493,6 +495,7 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
   TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
+#ifdef TE_WITH_CHAIN
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -501,6 +504,7 @@ cudaError_t init_kernel_attrs() {
                                 te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+#endif
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -821,6 +825,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
   // chain2: down -> next layer's QKV (e.g. T = 512, where gate/up runs on the wide CTA-pair kernel).
   const bool chain_ok = pl.chain != 0 && !prefix_pass;
   const bool chain4 = chain_ok && pl.chain == 4;
+#ifdef TE_WITH_CHAIN
   auto launch_chain = [&](int n_ph, const te::GemmParams* ps, const int* epis, const CUtensorMap* const* ma,
                           const CUtensorMap* const* mb) -> cudaError_t {
     te::ChainParams cp{};
@@ -844,6 +849,11 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
                     *fb[0], *fa[1], *fb[1], *fa[2], *fb[2], *fa[3], *fb[3], cp);
   };
 
+#else
+  auto launch_chain = [&](int, const te::GemmParams*, const int*, const CUtensorMap* const*, const CUtensorMap* const*) -> cudaError_t {
+    return cudaErrorNotSupported;
+  };
+#endif
   bool qkv_done = false;  // this layer's QKV was the last phase of the previous layer's chain
   for (int l = lb; l < le; ++l) {
     const LayerOff& o = h->off[l];
@@ -1559,7 +1569,14 @@ int te_set_option(te_handle* h, int option, int value) {
       if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
       h->resid_wide = value;
       break;
-    case TE_OPT_CHAIN: h->chain = value ? 1 : 0; break;
+    case TE_OPT_CHAIN:
+#ifdef TE_WITH_CHAIN
+      h->chain = value ? 1 : 0;
+      break;
+#else
+      if (value) return TE_ERR_UNSUPPORTED;  // the chained-launch experiment is not in this build (TE_WITH_CHAIN)
+      break;
+#endif
     case TE_OPT_RESID_HALVES:
       if (value < 0 || value > 3) return TE_ERR_INVALID_ARG;
       h->resid_halves = value;

@@ -377,12 +377,6 @@ def test_encode_is_async_no_sync_and_counts_launches(H):
     st.synchronize()
     assert not done_at_return
     assert te.te_kernel_launches(g.enc.h) - n0 == 2 + 5 * w.model.n_layers   # refresh + prep + 5 per layer
-    te.te_set_option(g.enc.h, te.TE_OPT_CHAIN, 1)
-    g.encode(emb, tl, 4, 4)
-    n1 = te.te_kernel_launches(g.enc.h)
-    g.encode(emb, tl, 4, 4)
-    # chained: refresh + prep + first QKV + per layer [attention, one launch of O-proj / gate-up / down / next QKV]
-    assert te.te_kernel_launches(g.enc.h) - n1 == 3 + 2 * w.model.n_layers
     g.close()
 
 
@@ -926,7 +920,9 @@ def test_chained_launches_equal_separate_launches_bitwise(H, cfg_id):
     (the grid-barrier counters are re-armed by every launch)."""
     w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
     g = H.GpuTE(w.model, w.n_frames, T, blob)
-    g.te.te_set_option(g.enc.h, g.te.TE_OPT_CHAIN, 1)
+    if g.te.lib().te_set_option(g.enc.h, g.te.TE_OPT_CHAIN, 1) == g.te.TE_ERR_UNSUPPORTED:
+        g.close()
+        pytest.skip("the chained-launch experiment is not in this build (TE_NVCC_EXTRA=-DTE_WITH_CHAIN)")
     out = g.encode(emb, tl, w.grid_h, w.grid_w)
     assert "chain" in g.te.te_dispatch_info(g.enc.h), g.te.te_dispatch_info(g.enc.h)
     for _ in range(5):
