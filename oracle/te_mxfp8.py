@@ -256,10 +256,22 @@ def dequantise_fp4(codes: np.ndarray, scales: np.ndarray) -> np.ndarray:
     return (blk * X[..., None]).reshape(c.shape)
 
 
+def e2m1_round(v: np.ndarray) -> np.ndarray:
+    """float -> the nearest E2M1 VALUE (ties to even), |v| <= 6 (larger clamps): the grid step is 0.5 below 2, 1 in [2, 4)
+    and 2 in [4, 6], and np.rint rounds half to even.  Same function as e2m1_decode(e2m1_encode_rne(v)) (pinned on every
+    midpoint and a dense sweep), without the table search — the 28-layer oracle quantises 1.4 G weights."""
+    v = np.asarray(v, dtype=np.float64)
+    a = np.minimum(np.abs(v), E2M1_MAX)
+    r = np.where(a < 2.0, np.rint(a * 2.0) / 2.0, np.where(a < 4.0, np.rint(a), np.rint(a / 2.0) * 2.0))
+    return np.copysign(r, v)
+
+
 def fake_quant_fp4(x: np.ndarray) -> np.ndarray:
-    """dequantise_fp4(quantise_fp4(x)) -> float64."""
-    c, s = quantise_fp4(x)
-    return dequantise_fp4(c, s)
+    """dequantise_fp4(quantise_fp4(x)) -> float64, evaluated on values (e2m1_round); identical by construction, pinned."""
+    x32 = np.asarray(x, dtype=np.float32)
+    blk = x32.reshape(x32.shape[:-1] + (x32.shape[-1] // BLOCK, BLOCK))
+    X = np.float64(2.0) ** (scale_code_fp4(np.max(np.abs(blk), axis=-1)).astype(np.float64) - 127.0)
+    return (e2m1_round(blk.astype(np.float64) / X[..., None]) * X[..., None]).reshape(x32.shape)
 
 
 def quantise_layer_weights_fp4(W: dict) -> dict:

@@ -160,6 +160,19 @@ def test_e2m1_rounding_hand_worked():
     assert np.max(np.abs(once - x)) <= 1.0                              # half of the widest grid step (4 -> 6)
 
 
+def test_e2m1_round_equals_decode_of_encode():
+    """The value-domain rounding used by fake_quant_fp4 is the table-search quantiser: on every midpoint, every grid
+    value, both signs, a dense sweep, and beyond the clamp."""
+    pts = np.concatenate([[0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5.0], Q._GRID4, np.linspace(0, 7.5, 6001),
+                          np.nextafter([0.25, 0.75, 1.25, 1.75, 2.0, 2.5, 3.5, 4.0, 5.0], 0),
+                          np.nextafter([0.25, 0.75, 1.25, 1.75, 2.0, 2.5, 3.5, 4.0, 5.0], 10)])
+    pts = np.concatenate([pts, -pts])
+    assert np.array_equal(Q.e2m1_round(pts), Q.e2m1_decode(Q.e2m1_encode_rne(pts)))
+    x = np.random.default_rng(1).standard_normal((64, 256)).astype(np.float32) * 3
+    c, s = Q.quantise_fp4(x)
+    assert np.array_equal(Q.fake_quant_fp4(x), Q.dequantise_fp4(c, s))
+
+
 def test_fp4_scale_codes_worked():
     """Smallest power of two X with amax / X <= 6 (= 1.5 * 2^2): worked from the float32 fields."""
     amax = np.asarray([6.0, 6.0001, 1.0, 1.5, 1.51, 0.0, 12.0, 0.02, 3.0e-3], dtype=np.float32)
