@@ -79,8 +79,6 @@ def _check_stages(v, V, blob, px, taps, tag):
         assert np.isfinite(got).all(), (tag, name)
         assert PM.rel_l2(got, want) <= PM.GATE_LAYER_REL_L2, (tag, name, PM.rel_l2(got, want))
         assert PM.max_row_rel_l2(got, want) <= PM.GATE_ROW_UPDATE_REL_L2, (tag, name, PM.max_row_rel_l2(got, want))
-    # the tower's own contribution (what a wrong mask / wrong ids would move): update = tower_out is normalised, so
-    # compare the pre-norm direction through the merged output AND the tower update relative to x0's scale
     return ref
 
 
