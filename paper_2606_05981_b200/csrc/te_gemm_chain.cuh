@@ -23,6 +23,8 @@
 namespace te {
 
 constexpr int CHAIN_MAX_PHASES = 4;
+constexpr int CHAIN_STAGES = 5;
+constexpr int CHAIN_SMEM_BYTES = CHAIN_STAGES * (GEMM_BM * GEMM_BK * 2 + 128 * GEMM_BK * 2) + 256 + GEMMK_EPI_WARPS * 2 * 32 * 32 * 4 + 1024;
 
 struct ChainParams {
   GemmParams p[CHAIN_MAX_PHASES];
@@ -94,7 +96,7 @@ te_gemmk_chain_kernel(const __grid_constant__ CUtensorMap tmA0, const __grid_con
                       const __grid_constant__ ChainParams cp) {
   using Cfg = GemmKCfg<128, EPI_QKV>;  // the largest staging area of the three epilogues
   constexpr int BN = 128;
-  constexpr int STAGES = Cfg::STAGES;
+  constexpr int STAGES = CHAIN_STAGES;  // (private staging here: the next phase's weights land in the ring during an epilogue)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sA = smem;

@@ -34,9 +34,14 @@ struct GemmKCfg {
   static constexpr int STG_WARP_BYTES = (EPI == EPI_QKV ? 2 : 1) * 32 * 32 * 4;
   static constexpr int STG_BYTES = GEMMK_EPI_WARPS * STG_WARP_BYTES;
   static constexpr int SMEM_LIMIT = 232448;  // 227 KB
-  static constexpr int STAGES_FIT = (SMEM_LIMIT - 1024 - BAR_BYTES - STG_BYTES) / STAGE_BYTES;
+  // The epilogue's staging buffers ALIAS the TMA ring: they are first written after the accumulator barrier, i.e. when
+  // every MMA has read its stage and no TMA write is outstanding (a CTA computes one tile).  All of shared memory is
+  // therefore ring: a small-batch main loop is bound by bytes in flight per SM (5 stages x 32 KB / ~1.1 us of DRAM
+  // latency = the 140 GB/s per SM of the pipeline trace), so two more stages are worth more than a private staging area.
+  static constexpr int STAGES_FIT = (SMEM_LIMIT - 1024 - BAR_BYTES) / STAGE_BYTES;
   static constexpr int STAGES = STAGES_FIT > 8 ? 8 : STAGES_FIT;
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STG_BYTES + 1024;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;
+  static_assert(STAGES * STAGE_BYTES >= STG_BYTES, "staging must fit inside the ring it aliases");
   static constexpr int TMEM_COLS = BN;  // one accumulator: a CTA computes a single (partial) tile
   static_assert(STAGES >= 3 && 2 * STAGES + 2 <= BAR_BYTES / 8, "pipeline configuration");
 };
@@ -342,7 +347,7 @@ te_gemmk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   uint64_t* empty = bars + STAGES;
   uint64_t* tfull = bars + 2 * STAGES;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tfull + 1);
-  float* stg_all = reinterpret_cast<float*>(smem + STAGES * Cfg::STAGE_BYTES + Cfg::BAR_BYTES);
+  float* stg_all = reinterpret_cast<float*>(smem);  // aliases the ring (see GemmKCfg)
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;

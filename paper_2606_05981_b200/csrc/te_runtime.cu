@@ -497,13 +497,13 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
 #ifdef TE_WITH_CHAIN
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+                                te::CHAIN_SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+                                te::CHAIN_SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+                                te::CHAIN_SMEM_BYTES)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES)));
+                                te::CHAIN_SMEM_BYTES)));
 #endif
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
@@ -845,7 +845,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
     for (int i = 0; i < te::CHAIN_MAX_PHASES; ++i) { fa[i] = ma[i < n_ph ? i : 0]; fb[i] = mb[i < n_ph ? i : 0]; }
     auto kern = n_ph >= 3 ? (dh == 128 ? te::te_gemmk_chain_kernel<128, true> : te::te_gemmk_chain_kernel<64, true>)
                           : (dh == 128 ? te::te_gemmk_chain_kernel<128, false> : te::te_gemmk_chain_kernel<64, false>);
-    return launch_k(lcc, kern, dim3(grid), dim3(te::GEMMK_THREADS), te::GemmKCfg<128, te::EPI_QKV>::SMEM_BYTES, st, *fa[0],
+    return launch_k(lcc, kern, dim3(grid), dim3(te::GEMMK_THREADS), te::CHAIN_SMEM_BYTES, st, *fa[0],
                     *fb[0], *fa[1], *fb[1], *fa[2], *fb[2], *fa[3], *fb[3], cp);
   };
 
