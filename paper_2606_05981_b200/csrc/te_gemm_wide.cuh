@@ -37,12 +37,16 @@ struct GemmWideCfg {
     return ((halves ? sub_w0(bn) : bn) / 2) * GEMM_BK * 2;
   }
   __host__ __device__ static constexpr int stage_bytes(int bn, int halves = 0) { return A_BYTES + b_bytes(bn, halves); }
+  // halves = 0: one tile per CTA pair and ONE accumulator barrier, so the epilogue staging ALIASES the ring (first
+  // written when every MMA has read its stage and no TMA write is outstanding in either CTA): one more stage in flight
+  // at the SwiGLU widths.  halves = 1 keeps a private staging area (sub-tile 1's loads land during sub-tile 0's epilogue).
   __host__ __device__ static constexpr int stages(int bn, int halves = 0) {
-    const int fit = (SMEM_LIMIT - 1024 - BAR_BYTES - STG_BYTES) / stage_bytes(bn, halves);
+    const int fit = (SMEM_LIMIT - 1024 - BAR_BYTES - (halves ? STG_BYTES : 0)) / stage_bytes(bn, halves);
     return fit > MAX_STAGES ? MAX_STAGES : fit;
   }
   __host__ __device__ static constexpr int smem_bytes(int bn, int halves = 0) {
-    return stages(bn, halves) * stage_bytes(bn, halves) + BAR_BYTES + STG_BYTES + 1024;
+    const int ring = stages(bn, halves) * stage_bytes(bn, halves);
+    return (halves ? ring + STG_BYTES : (ring > STG_BYTES ? ring : STG_BYTES)) + BAR_BYTES + 1024;
   }
 };
 
@@ -67,7 +71,7 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
   uint64_t* empty = bars + Cfg::MAX_STAGES;       // one set per CTA
   uint64_t* tfull = bars + 2 * Cfg::MAX_STAGES;   // one per CTA
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tfull + 1);
-  float* stg_all = reinterpret_cast<float*>(smem + STAGES * Cfg::stage_bytes(bn) + Cfg::BAR_BYTES);
+  float* stg_all = reinterpret_cast<float*>(smem);  // aliases the ring (see GemmWideCfg::stages)
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
