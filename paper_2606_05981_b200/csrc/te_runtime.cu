@@ -668,8 +668,15 @@ std::string describe_plan(const te_handle* h, const Plan& pl) {
   const te_config& c = h->cfg;
   char b[320];
   std::string s;
+  const int d_ = c.hidden, F_ = c.ffn;
   auto gemm = [&](const char* cls, int epi, bool k, bool pair2, int bn, int dh) {
-    if (k) snprintf(b, sizeof(b), "%s=te_gemmk_kernel<%d, %d, %d>;", cls, bn, epi, dh);
+    if (k) {  // the split-K kernel's 4th template argument = its epilogue variant, decided by the K split (as in enqueue_stack)
+      const int n_cols = epi == te::EPI_QKV ? (c.n_q_heads + 2 * c.n_kv_heads) * c.head_dim : (epi == te::EPI_SWIGLU ? 2 * F_ : d_);
+      const int k_dim = (cls[0] == 'd') ? F_ : ((cls[0] == 'o') ? c.n_q_heads * c.head_dim : d_);
+      int S = choose_splits(h->split_target, pl.num_m * (n_cols / bn), k_dim / te::GEMM_BK, h->sm_count);
+      if (epi == te::EPI_QKV && S == 2 && h->split_target == 0) S = 1;
+      snprintf(b, sizeof(b), "%s=te_gemmk_kernel<%d, %d, %d, %d>;", cls, bn, epi, dh, S == 1 ? 0 : te::gemmk_variant(epi, S * (bn / 128)));
+    }
     else if (pair2) snprintf(b, sizeof(b), "%s=te_gemm2_kernel<%d, %d, %d>;", cls, bn, epi, dh);
     else snprintf(b, sizeof(b), "%s=te_gemm_kernel<%d, %d, %d>;", cls, bn, epi, dh);
     s += b;
