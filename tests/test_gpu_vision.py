@@ -64,7 +64,20 @@ def _run_gpu(v, blob, px, text_lens=None, d_text_fill=None):
         te.te_vision_debug_tap(enc.v, what, buf)
         taps[name] = buf
     launches = te.te_vision_kernel_launches(enc.v)
-    assert te.te_query_async_error(te.te_vision_debug_tower(enc.v)) == te.TE_OK
+    tower = te.te_vision_debug_tower(enc.v)
+    assert te.te_query_async_error(tower) == te.TE_OK
+    # the tower's rotary ids (0, py, px) bit-exact and its cos/sin table (what an h / w swap would show in; the outputs
+    # barely move under it, tests/test_vision_pins.py)
+    from oracle import te_oracle as O_
+    pos = np.empty((3, n_patch), dtype=np.int32)
+    te.te_debug_tap(tower, te.TE_TAP_POS, pos)
+    want = O_.position_ids([0] * B, v.grid_h, v.grid_w)
+    assert np.array_equal(pos, want)
+    hd2 = v.tower.head_dim // 2
+    cos_t = np.empty((n_patch, hd2), dtype=np.float32)
+    te.te_debug_tap(tower, te.TE_TAP_COS, cos_t)
+    phi = O_.mrope_angles(want, v.tower.head_dim, v.tower.rope_sections, v.tower.rope_theta)
+    assert np.max(np.abs(cos_t - np.cos(phi))) <= PM.GATE_COSSIN_ABS
     out = emb.cpu().numpy()
     enc.close()
     return out, taps, launches

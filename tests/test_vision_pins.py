@@ -135,3 +135,53 @@ def test_front_end_dense_restatement_and_invariants():
     out2 = V.encode_image(w_pe, tower, lay, mv, w_m, px2, v.patch)
     assert not np.allclose(out2[:v.tokens_per_frame], out[:v.tokens_per_frame])
     assert np.max(np.abs(out2[v.tokens_per_frame:] - out[v.tokens_per_frame:])) <= 1e-12
+
+
+def test_vision_mutants_exceed_the_gpu_gates():
+    """Test power of the GPU parity gates of the front end (tests/test_gpu_vision.py: rel-L2 <= 1e-2 per stage): every
+    plausible mistake — transposed patch flattening, swapped merge order, swapped rotary axes, a causal mask in the tower,
+    a dropped final norm — must move the oracle's output by MORE than the gate, or the gate could not see it."""
+    import parity_metrics as PM
+    v, w_pe, tower, w_m, px = _tiny_inputs(2)
+    mv = v.tower
+    lay = W.blob_layout(mv)
+    ref = V.encode_image(w_pe, tower, lay, mv, w_m, px, v.patch)
+    f64 = O.bf16_bits_to_f64
+    B, gh, gw = 2, v.grid_h, v.grid_w
+
+    def front(patches_fn=V.patchify, merge_fn=V.merge2x2, attention=V.attention_full_gqa, final_norm=1, swap_hw=False):
+        x0 = patches_fn(px, v.patch) @ f64(w_pe).reshape(w_pe.shape).T
+        if swap_hw:      # ids (0, px, py) instead of (0, py, px): on a square grid = the tower run over the TRANSPOSED patch order
+            perm = np.concatenate([b * gh * gw + np.arange(gh * gw).reshape(gh, gw).T.reshape(-1) for b in range(B)])
+            hid_t = O.encode(tower, lay, mv, x0[perm], [0] * B, gh, gw, final_norm=final_norm, attention=attention)
+            hid = np.empty_like(hid_t)
+            hid[perm] = hid_t
+        else:
+            hid = O.encode(tower, lay, mv, x0, [0] * B, gh, gw, final_norm=final_norm, attention=attention)
+        return merge_fn(hid, B, gh, gw) @ f64(w_m).reshape(w_m.shape).T
+
+    def patchify_channel_major(pixels, P):      # (channel, dy, dx) instead of (dy, dx, channel)
+        p = V.patchify(pixels, P)
+        return p.reshape(p.shape[0], P, P, 3).transpose(0, 3, 1, 2).reshape(p.shape[0], -1)
+
+    def merge_dx_dy(h, n_frames, gh_, gw_):     # (dx, dy) instead of (dy, dx) inside a 2x2 cell
+        m = V.merge2x2(h, n_frames, gh_, gw_)
+        d = h.shape[1]
+        return np.concatenate([m[:, 0:d], m[:, 2 * d:3 * d], m[:, d:2 * d], m[:, 3 * d:4 * d]], axis=1)
+
+    assert PM.rel_l2(front(), ref) <= 1e-12                                  # the harness reproduces the oracle
+    mutants = {
+        "patch flattening (c, dy, dx)": front(patches_fn=patchify_channel_major),
+        "merge order (dx, dy)": front(merge_fn=merge_dx_dy),
+        "causal mask in the tower": front(attention=O.attention_causal_gqa),
+        "final norm dropped": front(final_norm=0),
+    }
+    for name, out in mutants.items():
+        assert PM.rel_l2(out, ref) > 3 * PM.GATE_LAYER_REL_L2, (name, PM.rel_l2(out, ref))
+    # ... except swapped rotary axes (ids (0, px, py)): with theta = 1e6 the h / w pairs rotate by < 0.1 rad on a 4 x 4 grid and
+    # the output moves by less than the gate (SURVEY §8c "Test power": the same holds for the decoder).  That mistake is
+    # caught where it is made: the GPU test compares the tower's position ids bit-exactly and its cos/sin table to 1e-5.
+    swapped = front(swap_hw=True)
+    assert 0 < PM.rel_l2(swapped, ref) < PM.GATE_LAYER_REL_L2
+    ids = O.position_ids([0] * B, gh, gw)
+    assert not np.array_equal(ids[1], ids[2])                                # ... which do differ between the two axes
