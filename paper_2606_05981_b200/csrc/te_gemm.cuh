@@ -81,6 +81,17 @@ struct GemmParams {
   // rows (n'>>1)*256 + (n'&1)*64 .. +64 and the matching up rows 128 further on, as two 64-row halves
   int gu_half;
 };
+// Loads of data that an EARLIER PHASE of the same launch may have rewritten (te_gemm_chain.cuh, built only with
+// -DTE_WITH_CHAIN) must not be served from a stale L1 line; in the default build a kernel boundary separates writer and
+// reader and the ordinary (L1-cached) load is what the epilogue-bound kernels want.
+template <typename T>
+__device__ __forceinline__ T ld_phase(const T* ptr) {
+#ifdef TE_WITH_CHAIN
+  return __ldcg(ptr);
+#else
+  return *ptr;
+#endif
+}
 __device__ __forceinline__ int gemm_rows(const GemmParams& p) { return p.dyn != nullptr ? p.dyn->total_tokens : p.M; }
 __device__ __forceinline__ float* resid_dst(const GemmParams& p) { return p.x_to_out ? p.dyn->out : p.x; }
 constexpr int TRACE_SLOTS = 96;  // [0,48): globaltimer ns, [48,96): SM clock of the same stamp
@@ -166,7 +177,7 @@ __device__ __forceinline__ void resid_issue(const GemmParams& p, int M, ResidPre
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const int row = row_base + sub + 4 * i;
-    if (row < M) pf.xv[i] = __ldcg(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col));  // (L2: see te_gemm_chain.cuh)
+    if (row < M) pf.xv[i] = ld_phase(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col));
   }
 }
 template <int BN>
@@ -246,10 +257,10 @@ __device__ __forceinline__ float row_rstd(const GemmParams& p, int row, bool val
     const float* q = p.ssq_in + (size_t)row * p.ssq_stride;
     int i = 0;
     for (; i + 4 <= p.ssq_parts; i += 4) {  // sequential sum, fixed order
-      const float4 v = __ldcg(reinterpret_cast<const float4*>(q + i));  // (L2: rewritten between phases of a chain launch)
+      const float4 v = ld_phase(reinterpret_cast<const float4*>(q + i));
       s += v.x; s += v.y; s += v.z; s += v.w;
     }
-    for (; i < p.ssq_parts; ++i) s += __ldcg(q + i);
+    for (; i < p.ssq_parts; ++i) s += ld_phase(q + i);
   }
   return 1.0f / sqrtf(s * p.inv_d + p.eps);
 }

@@ -16,7 +16,7 @@
 //     scales straight from the fp32 values (a 32-column chunk of a row is exactly one MX block), so the block-scaled
 //     path needs no extra pass over the activations.
 // TMEM budget (512 columns): ACC accumulator stages x BN columns + 2 x (4 + 4 * ceil(BN / 128)) scale columns:
-//   BN = 128 / 192 -> two accumulator stages (epilogue overlaps the next tile), BN = 256 -> one.
+//   BN = 128 -> three accumulator stages, BN = 192 -> two (the epilogue overlaps the next tiles), BN = 256 -> one.
 #pragma once
 #include "te_gemm.cuh"
 
@@ -202,7 +202,12 @@ constexpr uint32_t UMMA_F8F6F4_E2M1 = 5u;  // element format code of kind::mxf8f
 
 template <int BN, int EPI>
 struct Gemm8Cfg {
-  static constexpr int ACC = (BN <= 192) ? 2 : 1;               // accumulator stages
+  // accumulator stages: three for 128-wide tiles (3 x 128 + scale columns <= 512): main loop (16-48 k-blocks of K = 128)
+  // and epilogue take about as long as each other there, and a third stage keeps either from waiting on the other's jitter
+#ifndef TE_ACC128
+#define TE_ACC128 3
+#endif
+  static constexpr int ACC = (BN <= 128) ? TE_ACC128 : ((BN <= 192) ? 2 : 1);
   static constexpr int SFB_TILES = (BN + 127) / 128;
   static constexpr int A_BYTES = GEMM_BM * GEMM8_BK;
   static constexpr int B_BYTES = (BN / 2) * GEMM8_BK;

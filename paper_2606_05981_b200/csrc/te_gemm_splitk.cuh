@@ -105,7 +105,7 @@ __device__ __forceinline__ void slice_aux_load(const GemmParams& p, int M, Slice
     if constexpr (EPI == EPI_RESID) {
 #pragma unroll
       for (int v = 0; v < NV; ++v)
-        if (ok) ax.xv[b][v] = __ldcg(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + n_blk * BN + v * 128) + lane);
+        if (ok) ax.xv[b][v] = ld_phase(reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + n_blk * BN + v * 128) + lane);
     }
     if constexpr (EPI == EPI_QKV) {
       if (ok) {
@@ -119,9 +119,9 @@ __device__ __forceinline__ void slice_aux_load(const GemmParams& p, int M, Slice
       float sq = 0.f;
       if (ok) {
         const float* q = p.ssq_in + (size_t)row * p.ssq_stride;
-        sq = (lane < p.ssq_parts) ? __ldcg(q + lane) : 0.f;
-        sq += (lane + 32 < p.ssq_parts) ? __ldcg(q + lane + 32) : 0.f;
-        for (int i = lane + 64; i < p.ssq_parts; i += 32) sq += __ldcg(q + i);
+        sq = (lane < p.ssq_parts) ? ld_phase(q + lane) : 0.f;
+        sq += (lane + 32 < p.ssq_parts) ? ld_phase(q + lane + 32) : 0.f;
+        for (int i = lane + 64; i < p.ssq_parts; i += 32) sq += ld_phase(q + i);
       }
       ax.rstd[b] = sq;
     }
