@@ -932,3 +932,38 @@ def test_chained_launches_equal_separate_launches_bitwise(H, cfg_id):
     assert "chain" not in g.te.te_dispatch_info(g.enc.h)
     assert np.array_equal(out, plain)
     g.close()
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_shape_sweep_all_dtypes(H, O, seed):
+    """Seeded random calls on ONE handle per operand type (bf16 / MXFP8 / MXFP4 weights): 1-40 frames, grids 1x1 .. 8x8,
+    text lengths 0 .. 256 - grid (token counts on both sides of the CTA-pair threshold, many graph shape classes,
+    shrinking and growing), each against its oracle with the per-row gates; ids bit-exact."""
+    from oracle import te_mxfp8 as Q
+    import paper_2606_05981_b200 as te
+    m = W.TINY
+    blob = H.cached_blob(m, 1)
+    lay = W.blob_layout(m)
+    rng = np.random.default_rng(seed)
+    encs = {dt: H.GpuTE(m, 40, 4096, blob, weight_dtype=dt) for dt in (0, 1, 2)}
+    for case in range(10):
+        dt = int(rng.integers(0, 3))
+        B = int(rng.integers(1, 41))
+        gh, gw = int(rng.integers(1, 9)), int(rng.integers(1, 9))
+        tl = rng.integers(0, 257 - gh * gw, size=B).astype(np.int32)
+        while B * gh * gw + int(tl.sum()) > 4000:
+            tl = (tl // 2).astype(np.int32)
+        T = B * gh * gw + int(tl.sum())
+        emb = rng.standard_normal((T, m.hidden)).astype(np.float32)
+        g = encs[dt]
+        out = g.encode(emb, tl, gh, gw)
+        if dt == 0:
+            mm = PM.stack_metrics(out, O.encode(blob, lay, m, emb, tl, gh, gw), emb)
+            assert PM.passes_final_gates(mm), (case, B, gh, gw, T, mm)
+        else:
+            mm = PM.stack_metrics(out, Q.encode_mxfp8(blob, lay, m, emb, tl, gh, gw, fp4_weights=(dt == 2)), emb)
+            assert PM.passes_mx_gates(mm), (case, dt, B, gh, gw, T, mm)
+        assert np.array_equal(g.tap(te.TE_TAP_POS, (3, T), np.int32), O.position_ids(tl, gh, gw))
+        assert te.te_query_async_error(g.enc.h) == te.TE_OK
+    for g in encs.values():
+        g.close()
