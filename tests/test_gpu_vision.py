@@ -417,3 +417,20 @@ def test_per_frame_grids_full_width_ragged(O, H):
     assert np.array_equal(pos, want_pos)
     mm = PM.stack_metrics(got, ref, emb, outlier_ch=[5, 1500])
     assert PM.passes_final_gates(mm), mm
+
+
+def test_vision_non_square_image(V):
+    """A 32 x 64 image (4 x 8 patches -> 2 x 4 visual tokens): row-major patch order, (dy, dx) merge order and the (0, py, px)
+    ids on a non-square grid (a transposed layout anywhere would pass on the square configs)."""
+    import dataclasses
+    v = dataclasses.replace(W.VISION_TINY, image_h=32, image_w=64)
+    blob = W.make_vision_blob(v)
+    px = W.make_pixels(v, 3)
+    out, taps, _ = _run_gpu(v, blob, px)
+    ref = _check_stages(v, V, blob, px, taps, "non-square")
+    assert out.shape == (3 * 8, v.out_hidden)
+    assert PM.rel_l2(out, ref) <= PM.GATE_LAYER_REL_L2
+    v2 = dataclasses.replace(W.VISION_TINY, image_h=64, image_w=16)
+    px2 = W.make_pixels(v2, 2)
+    out2, taps2, _ = _run_gpu(v2, W.make_vision_blob(v2), px2)
+    _check_stages(v2, V, W.make_vision_blob(v2), px2, taps2, "tall")
