@@ -40,7 +40,9 @@ typedef enum te_status {
   TE_ERR_BLOB_SIZE = -3,   /* n_bytes != te_blob_bytes(cfg)                                      */
   TE_ERR_CUDA = -4,        /* a CUDA call failed; text via te_last_error                         */
   TE_ERR_UNSUPPORTED = -5, /* head_dim not in {64,128}, dims not tileable, device not sm_100     */
-  TE_ERR_DEVICE_CHECK = -6 /* te_query_async_error: device-side validation flag was raised       */
+  TE_ERR_DEVICE_CHECK = -6, /* te_query_async_error: device-side validation flag was raised      */
+  TE_ERR_TOO_LARGE = -7    /* te_matmul_noalloc: the problem needs more scratch than the library's
+                              built-in array holds (TE_NOALLOC_SCRATCH_BYTES)                     */
 } te_status;
 
 /* Decoder-stack shape + capacities (POD, copied at te_create).
@@ -252,6 +254,49 @@ int te_encode_image(te_vision* v, int32_t n_frames, const float* pixels, const i
 int64_t te_vision_kernel_launches(te_vision* v);
 const char* te_vision_last_error(te_vision* v);
 void te_vision_destroy(te_vision* v);
+
+/* ---------------------------------------------------------------------------------------------------------------
+ * A matrix product for callers that must not allocate device memory.
+ *
+ * Who this is for.  Two kinds of caller cannot afford cudaMalloc / cudaFree around a kernel.  (1) A frame loop that
+ * shares the GPU with a denoiser on another stream (the paper's side-stream / main-stream pipeline, PAPER.md:114,
+ * Algorithm 1 :118-137): both calls may block the host until the whole device is idle, which stalls the other stream
+ * and shows up as a dropped frame.  (2) A process in which some other component — an inference server's memory pool,
+ * a framework's caching allocator — has claimed all of HBM at start-up: cudaMalloc then fails with out-of-memory
+ * although the pool's owner could hand out a buffer.  Every other entry point of this library allocates (te_create
+ * builds the workspace, the stand-alone products of te_debug.h allocate and free their scratch on every call).
+ *
+ * What it computes.  C[m, n] (DEVICE fp32, row-major) = A[m, k] * B[n, k]^T, A and B DEVICE bf16 row-major, fp32
+ * accumulation — the same small-batch split-K kernel the stack runs for T <= 512: `splits` CTAs share
+ * one 128 x block_n output tile, each multiplies its own slice of k, and the partial tiles meet in scratch memory and
+ * are summed in a fixed order, so the result is bitwise repeatable.  The caller owns a, b and c and still passes
+ * them; the only memory the call does not get from the caller is that scratch.
+ *
+ * Where the scratch lives.  In a fixed array inside the library's device image, TE_NOALLOC_SCRATCH_BYTES of partial
+ * tiles plus 2 KiB of group counters.  Every GPU that loads libte_b200.so carries this array from module load until
+ * the process exits, whether or not this function is ever called.  The call runs no cudaMalloc, cudaFree,
+ * cudaMallocAsync or other allocating routine; it enqueues one 2 KiB memset of the counters and one kernel on
+ * `cuda_stream` and returns without synchronising.
+ *
+ * Limits.  k % 64 == 0; block_n in {128, 256}; n % block_n == 0; 1 <= splits <= 8 and splits <= k / 64;
+ * tiles = ceil(m / 128) * (n / block_n) must satisfy tiles * splits <= number of SMs (the CTAs of a group wait for each
+ * other, so all must be resident; TE_ERR_UNSUPPORTED otherwise) and
+ *     tiles * splits * 128 * block_n * 4 bytes <= TE_NOALLOC_SCRATCH_BYTES,
+ * else the call launches nothing and returns TE_ERR_TOO_LARGE.  (128 partial tiles of 128 x 128, e.g. m <= 128,
+ * n = 2048, splits = 8, fill it exactly.)
+ *
+ * First call on a device.  It looks up the array's device address and opts the kernels into their shared-memory size;
+ * this set-up happens once per device, inside the first call made for that device, and is not something to do in the
+ * middle of a stream capture — make one call per device at start-up, outside any capture.
+ *
+ * Sharing.  There is ONE array per GPU and every call uses it from offset 0, and it keeps whatever the previous call
+ * left there.  The partial tiles are fully overwritten before they are read and the counters are cleared on the
+ * stream before each kernel, so successive calls on one stream are independent of each other.  Two calls whose kernels
+ * can run at the same time on one GPU (different streams, different host threads, different handles of any kind) race
+ * on the array and produce garbage or hang: the caller must order them (same stream, or an event between them). */
+#define TE_NOALLOC_SCRATCH_BYTES (8u << 20)
+int te_matmul_noalloc(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m, int32_t n, int32_t k,
+                      int32_t block_n, int32_t splits, void* cuda_stream);
 
 void te_destroy(te_handle* h);
 const char* te_strerror(int code);

@@ -19,6 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libte_b200.so")
 TE_OK = 0
 TE_ERR_INVALID_ARG, TE_ERR_NOT_LOADED, TE_ERR_BLOB_SIZE = -1, -2, -3
 TE_ERR_CUDA, TE_ERR_UNSUPPORTED, TE_ERR_DEVICE_CHECK = -4, -5, -6
+TE_ERR_TOO_LARGE = -7
+TE_NOALLOC_SCRATCH_BYTES = 8 << 20   # include/te.h: partial-tile capacity of te_matmul_noalloc's built-in array
 TE_OPT_USE_GRAPH = 0
 TE_OPT_KERNEL_TIMING = 1
 TE_OPT_CTA_PAIR = 2
@@ -41,7 +43,7 @@ EXPORTS = [
     "te_encode_host_submit", "te_encode_host_wait", "te_query_async_error", "te_set_option", "te_kernel_launches",
     "te_graph_captures", "te_dispatch_info", "te_kernel_times", "te_destroy", "te_strerror", "te_last_error",
     "te_vision_blob_bytes", "te_vision_create", "te_vision_load_weights", "te_encode_image", "te_vision_kernel_launches",
-    "te_vision_last_error", "te_vision_destroy",
+    "te_vision_last_error", "te_vision_destroy", "te_matmul_noalloc",
 ]
 DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide", "te_debug_gemm_wide2",
                  "te_debug_mx_quantise", "te_debug_gemm_mxfp8", "te_debug_mx_quantise_fp4", "te_debug_gemm_mxfp4", "te_vision_debug_tap", "te_vision_debug_tower"]
@@ -128,6 +130,8 @@ def lib() -> ctypes.CDLL:
     L.te_debug_gemm.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
     L.te_debug_gemm_splitk.restype = c_int
     L.te_debug_gemm_splitk.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32]
+    L.te_matmul_noalloc.restype = c_int
+    L.te_matmul_noalloc.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32, c_void_p]
     L.te_debug_gemm_wide.restype = c_int
     L.te_debug_gemm_wide.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
     L.te_debug_gemm_wide2.restype = c_int
@@ -307,6 +311,16 @@ def te_debug_gemm(device, a_bf16, b_bf16, c, m, n, k, block_n=256, cta_pair=0):
 
 def te_debug_gemm_splitk(device, a_bf16, b_bf16, c, m, n, k, block_n=128, splits=2):
     _check(lib().te_debug_gemm_splitk(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, splits))
+
+
+def te_matmul_noalloc(device, a_bf16, b_bf16, c, m, n, k, block_n=128, splits=2, stream=None):
+    """c[m, n] (DEVICE fp32) = a[m, k] @ b[n, k]^T (DEVICE bf16) through the split-K kernel, with the kernel's scratch in
+    the library's built-in device array: for callers that cannot call cudaMalloc (a frame loop that must not stall the
+    GPU's other streams; a process whose memory pool already owns all of HBM).  Enqueues on `stream` (cudaStream_t as
+    int, None = default stream) and returns without synchronising.  Raises TEError(TE_ERR_TOO_LARGE) when
+    ceil(m/128) * (n/block_n) * splits * 128 * block_n * 4 bytes exceeds TE_NOALLOC_SCRATCH_BYTES.  All calls on one GPU
+    share that array: do not let two of them overlap.  See include/te.h."""
+    _check(lib().te_matmul_noalloc(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n, splits, _ptr(stream)))
 
 
 def te_debug_mx_quantise(device, src_bf16, rows, k, codes, scales_tiled):

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -2048,6 +2049,86 @@ void te_destroy(te_handle* h) {
   delete h;
 }
 
+}  // extern "C" (reopened below: the scratch array and its bookkeeping have C++ linkage)
+
+// ------------------------------------------------------------------------------------------------- te_matmul_noalloc
+// The split-K scratch for callers that cannot allocate (include/te.h): a fixed array in the device image instead of a
+// cudaMalloc'd buffer.  Layout: [0, TE_NOALLOC_SCRATCH_BYTES) fp32 partial tiles [tile][split][128][block_n], then
+// NOALLOC_SEM_BYTES of int counters (two per tile: arrivals, departures).  Zero at module load; each GPU has its own copy.
+// In HOST code the name `te_noalloc_pool` is only a handle for the runtime's symbol table — passing it (or its host
+// address) to a kernel would hand the kernel a host pointer.  The device address comes from cudaGetSymbolAddress, asked
+// once per device with that device current (noalloc_pool_of below).
+namespace {
+constexpr size_t NOALLOC_MAX_TILES = 256;  // >= any SM count: tiles <= tiles * splits <= SMs
+constexpr size_t NOALLOC_SEM_BYTES = 2 * NOALLOC_MAX_TILES * sizeof(int);
+constexpr int NOALLOC_MAX_DEVICES = 64;
+}  // namespace
+static __device__ __align__(256) unsigned char te_noalloc_pool[TE_NOALLOC_SCRATCH_BYTES + NOALLOC_SEM_BYTES];
+
+namespace {
+struct NoAllocDevice {
+  bool ready = false;
+  unsigned char* pool = nullptr;  // DEVICE address of te_noalloc_pool on this GPU
+  int sm_count = 0;
+};
+NoAllocDevice g_noalloc_dev[NOALLOC_MAX_DEVICES];
+std::mutex g_noalloc_mu;
+
+// Per-device set-up, done by the first call for `device` (which is current): checks the architecture, opts the kernels
+// into their dynamic shared-memory size and resolves the array's device address.  Nothing here allocates.
+int noalloc_pool_of(int device, NoAllocDevice* out) {
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  NoAllocDevice& d = g_noalloc_dev[device];
+  if (!d.ready) {
+    int major = 0, sms = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
+      return TE_ERR_CUDA;
+    if (major != 10) return TE_ERR_UNSUPPORTED;  // tcgen05 / TMEM kernel: sm_100 only, no fallback
+    if (!get_encode_fn() || init_kernel_attrs() != cudaSuccess) return TE_ERR_CUDA;
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, te_noalloc_pool) != cudaSuccess || !p) return TE_ERR_CUDA;
+    d.pool = static_cast<unsigned char*>(p);
+    d.sm_count = sms;
+    d.ready = true;
+  }
+  *out = d;
+  return TE_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int te_matmul_noalloc(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
+                      int32_t block_n, int32_t splits, void* cuda_stream) {
+  if (!a || !b || !cmat || m < 1 || n < 1 || k < 1 || device < 0 || device >= NOALLOC_MAX_DEVICES) return TE_ERR_INVALID_ARG;
+  if (k % 64 != 0 || (block_n != 128 && block_n != 256) || n % block_n != 0) return TE_ERR_UNSUPPORTED;
+  if (splits < 1 || splits > te::GEMMK_MAX_SPLITS || splits > k / 64) return TE_ERR_INVALID_ARG;
+  const size_t num_m = ((size_t)m + te::GEMM_BM - 1) / te::GEMM_BM, num_n = (size_t)n / block_n;
+  const size_t tiles = num_m * num_n;
+  // size check first: it needs no device and must hold whatever the GPU is
+  if (tiles > NOALLOC_MAX_TILES || tiles * splits * te::GEMM_BM * block_n * sizeof(float) > (size_t)TE_NOALLOC_SCRATCH_BYTES)
+    return TE_ERR_TOO_LARGE;
+  if (cudaSetDevice(device) != cudaSuccess) return TE_ERR_CUDA;
+  NoAllocDevice dev;
+  const int rc = noalloc_pool_of(device, &dev);
+  if (rc != TE_OK) return rc;
+  if (tiles * splits > (size_t)dev.sm_count) return TE_ERR_UNSUPPORTED;  // a group's CTAs wait for each other
+  CUtensorMap ta, tb;
+  if (!make_tmap(&ta, a, m, k, te::GEMM_BM) || !make_tmap(&tb, b, n, k, block_n)) return TE_ERR_CUDA;
+  te::GemmParams p{};
+  p.M = m; p.N = n; p.K = k; p.num_m_blk = (int)num_m; p.num_n_blk = (int)num_n;
+  p.c = cmat; p.ld_c = n; p.splits = splits;
+  p.sk_scratch = reinterpret_cast<float*>(dev.pool);
+  p.sk_sem = reinterpret_cast<int*>(dev.pool + TE_NOALLOC_SCRATCH_BYTES);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  // The counters must start at zero.  A finished launch re-arms them itself, but the array outlives every call and an
+  // aborted one (device fault, cooperative launch refused half-way) would leave them counting: clear them every time.
+  if (cudaMemsetAsync(p.sk_sem, 0, NOALLOC_SEM_BYTES, st) != cudaSuccess) return TE_ERR_CUDA;
+  const LaunchCtx lc;  // plain stream order (no programmatic overlap with the memset); cooperative when splits > 1
+  return launch_gemmk_bn<te::EPI_PLAIN>(lc, block_n, 128, ta, tb, p, st) == cudaSuccess ? TE_OK : TE_ERR_CUDA;
+}
+
 const char* te_strerror(int code) {
   switch (code) {
     case TE_OK: return "ok";
@@ -2057,6 +2138,7 @@ const char* te_strerror(int code) {
     case TE_ERR_CUDA: return "CUDA error";
     case TE_ERR_UNSUPPORTED: return "unsupported configuration or device";
     case TE_ERR_DEVICE_CHECK: return "device-side validation failed";
+    case TE_ERR_TOO_LARGE: return "problem needs more scratch memory than the library's built-in no-allocation array holds";
     default: return "unknown error";
   }
 }

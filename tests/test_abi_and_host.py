@@ -52,6 +52,25 @@ def test_vision_blob_bytes_without_gpu(te):
     assert te.te_vision_blob_bytes(bad) == 0
 
 
+def test_matmul_noalloc_size_limit_without_gpu(te):
+    """te_matmul_noalloc (te.h) checks its arguments and the capacity of the built-in scratch array before it touches
+    the device: an over-size problem is refused with TE_ERR_TOO_LARGE and bad shapes with their own codes, GPU or not."""
+    L = te.lib()
+    dummy = 256                                            # non-null, never dereferenced on these paths
+    assert te.TE_NOALLOC_SCRATCH_BYTES == 8 << 20
+    hdr = open(os.path.join(ROOT, "include", "te.h")).read()
+    assert "#define TE_NOALLOC_SCRATCH_BYTES (8u << 20)" in hdr and "TE_ERR_TOO_LARGE = -7" in hdr
+    # 17 tiles x 8 splits x 128 x 128 x 4 B = 8.5 MiB
+    assert L.te_matmul_noalloc(0, dummy, dummy, dummy, 128, 2176, 2048, 128, 8, None) == te.TE_ERR_TOO_LARGE
+    # 1 x 4 tiles x 5 splits x 128 KiB = 2.5 MiB fits, but m = 3000 makes it 24 x 4 x 5
+    assert L.te_matmul_noalloc(0, dummy, dummy, dummy, 3000, 1024, 2048, 256, 5, None) == te.TE_ERR_TOO_LARGE
+    assert "scratch" in L.te_strerror(te.TE_ERR_TOO_LARGE).decode()
+    assert L.te_matmul_noalloc(0, None, dummy, dummy, 128, 128, 64, 128, 1, None) == te.TE_ERR_INVALID_ARG
+    assert L.te_matmul_noalloc(0, dummy, dummy, dummy, 128, 128, 64, 128, 2, None) == te.TE_ERR_INVALID_ARG    # splits > k/64
+    assert L.te_matmul_noalloc(0, dummy, dummy, dummy, 128, 128, 96, 128, 1, None) == te.TE_ERR_UNSUPPORTED    # k % 64
+    assert L.te_matmul_noalloc(0, dummy, dummy, dummy, 128, 192, 64, 128, 1, None) == te.TE_ERR_UNSUPPORTED    # n % block_n
+
+
 def test_blob_bytes_and_strerror_without_gpu(te):
     import workloads as W
     for m in (W.TINY, W.FULL1, W.FULL28):
