@@ -244,12 +244,20 @@ int te_vision_load_weights(te_vision* v, const void* bf16_blob, size_t n_bytes);
 /* Encode the frames' images into the decoder's visual-token embeddings, IN PLACE in the decoder's input:
  *   pixels     DEVICE fp32 [n_frames, image_h, image_w, 3]
  *   text_lens  DEVICE int32 [n_frames] (the decoder call's text_lens) or NULL (= all zero)
- *   embeds     DEVICE fp32 [T, out_hidden], the packed input of te_encode: the n_vis = (image_h/2P)*(image_w/2P)
+ *   embeds     DEVICE fp32 [total_tokens, out_hidden], the packed input of te_encode: the n_vis = (image_h/2P)*(image_w/2P)
  *              merged tokens of frame b are written to rows cu[b] .. cu[b] + n_vis, cu[b] = b*n_vis + sum of
  *              text_lens[0..b) — computed on the device; the text rows are not touched
+ *   total_tokens  HOST value: the number of rows of `embeds` (the same value the following te_encode call gets);
+ *              >= n_frames * n_vis, else TE_ERR_INVALID_ARG
+ * Containment: text_lens is read on the device, unvalidated.  No row at or past total_tokens is ever written, whatever
+ * text_lens holds; a negative length (counted as 0) or lengths whose packed sum differs from total_tokens raise the
+ * sticky device flag that te_vision_query_async_error reports (bits as in te_query_async_error).
  * Enqueues on cuda_stream and returns (no synchronisation, no device->host copy). */
 int te_encode_image(te_vision* v, int32_t n_frames, const float* pixels, const int32_t* text_lens, float* embeds,
-                    void* cuda_stream);
+                    int32_t total_tokens, void* cuda_stream);
+/* Synchronises the device; TE_ERR_DEVICE_CHECK (and clears the flag) if te_encode_image — or the tower's own
+ * validation — raised the device-side flag since the last query, TE_ERR_CUDA on a CUDA error, else TE_OK. */
+int te_vision_query_async_error(te_vision* v);
 /* Kernels launched so far on behalf of te_encode_image (the tower's graph nodes included). */
 int64_t te_vision_kernel_launches(te_vision* v);
 const char* te_vision_last_error(te_vision* v);

@@ -43,7 +43,7 @@ EXPORTS = [
     "te_encode_host_submit", "te_encode_host_wait", "te_query_async_error", "te_set_option", "te_kernel_launches",
     "te_graph_captures", "te_dispatch_info", "te_kernel_times", "te_destroy", "te_strerror", "te_last_error",
     "te_vision_blob_bytes", "te_vision_create", "te_vision_load_weights", "te_encode_image", "te_vision_kernel_launches",
-    "te_vision_last_error", "te_vision_destroy", "te_matmul_noalloc",
+    "te_vision_last_error", "te_vision_destroy", "te_matmul_noalloc", "te_vision_query_async_error",
 ]
 DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide", "te_debug_gemm_wide2",
                  "te_debug_mx_quantise", "te_debug_gemm_mxfp8", "te_debug_mx_quantise_fp4", "te_debug_gemm_mxfp4", "te_vision_debug_tap", "te_vision_debug_tower"]
@@ -151,7 +151,9 @@ def lib() -> ctypes.CDLL:
     L.te_vision_load_weights.restype = c_int
     L.te_vision_load_weights.argtypes = [c_void_p, c_void_p, c_size_t]
     L.te_encode_image.restype = c_int
-    L.te_encode_image.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p]
+    L.te_encode_image.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_int32, c_void_p]
+    L.te_vision_query_async_error.restype = c_int
+    L.te_vision_query_async_error.argtypes = [c_void_p]
     L.te_vision_kernel_launches.restype = c_int64
     L.te_vision_kernel_launches.argtypes = [c_void_p]
     L.te_vision_last_error.restype = c_char_p
@@ -375,9 +377,17 @@ def te_vision_load_weights(v, blob, n_bytes: int | None = None):
     _vcheck(lib().te_vision_load_weights(v, _ptr(blob), n_bytes), v)
 
 
-def te_encode_image(v, n_frames, pixels, text_lens, embeds, stream=None):
-    """pixels: DEVICE fp32 [B, H, W, 3]; text_lens: DEVICE int32 [B] or None; embeds: DEVICE fp32 [T, out_hidden]."""
-    _vcheck(lib().te_encode_image(v, n_frames, _ptr(pixels), _ptr(text_lens), _ptr(embeds), _ptr(stream)), v)
+def te_encode_image(v, n_frames, pixels, text_lens, embeds, stream=None, total_tokens: int | None = None):
+    """pixels: DEVICE fp32 [B, H, W, 3]; text_lens: DEVICE int32 [B] or None; embeds: DEVICE fp32 [T, out_hidden];
+    total_tokens: rows of `embeds` (default: embeds.shape[0]) — no row past it is written whatever text_lens holds."""
+    if total_tokens is None:
+        total_tokens = int(embeds.shape[0])
+    _vcheck(lib().te_encode_image(v, n_frames, _ptr(pixels), _ptr(text_lens), _ptr(embeds), total_tokens, _ptr(stream)), v)
+
+
+def te_vision_query_async_error(v) -> int:
+    """Synchronises; returns TE_OK or TE_ERR_DEVICE_CHECK (no raise: the caller decides)."""
+    return int(lib().te_vision_query_async_error(v))
 
 
 def te_vision_kernel_launches(v) -> int:
@@ -463,8 +473,11 @@ class VisionEncoder:
     def load_weights(self, blob):
         te_vision_load_weights(self.v, blob)
 
-    def encode_image(self, n_frames, pixels, text_lens, embeds, stream=None):
-        te_encode_image(self.v, n_frames, pixels, text_lens, embeds, stream)
+    def encode_image(self, n_frames, pixels, text_lens, embeds, stream=None, total_tokens=None):
+        te_encode_image(self.v, n_frames, pixels, text_lens, embeds, stream, total_tokens)
+
+    def query_async_error(self) -> int:
+        return te_vision_query_async_error(self.v)
 
     def close(self):
         if self.v:

@@ -29,6 +29,9 @@ enum { EPI_PLAIN = 0, EPI_QKV = 1, EPI_RESID = 2, EPI_SWIGLU = 3 };
 // Per-call values that a cached graph must not bake in: written on the stream ahead of the stack's kernels
 // (te_set_dyn_kernel), read by every kernel.  A graph is therefore reusable for any caller buffers and for any
 // token count of the same row-block bucket (te_runtime.cu, graph cache).
+// Ordering: the GEMM kernels read total_tokens / out BEFORE their griddepcontrol.wait (gemm_rows, resid_dst).  That is
+// safe because the kernel that follows te_set_dyn_kernel in the stream (te_prep_kernel) is launched WITHOUT programmatic
+// overlap: by the time any later kernel of the call can start, set_dyn has completed and flushed.
 struct DynParams {
   const void* embeds;        // DEVICE [T, d]: fp32, or bf16 when embeds_bf16 (te_encode_ex)
   const int32_t* text_lens;  // DEVICE int32 [B]

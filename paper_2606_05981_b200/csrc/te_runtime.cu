@@ -161,9 +161,9 @@ struct te_handle {
   int resid_halves = 0; // wide residual tiles as two column halves (te_gemm_wide2_kernel): 1 = O-proj and down, 2 = O-proj, 0 = one pass
   int l2_resid = 1;          // 1: the residual stream is an L2-persisting access window of every kernel
   size_t l2_limit_bytes = 0; // persisting-L2 carve-out requested for it (0 until the first te_encode sets the limit)
-  size_t l2_prev_limit = 0;  // the device limit found before it was raised (restored by te_destroy / option 0)
-  bool l2_limit_raised = false;
+  bool l2_ref_held = false;  // this handle holds one reference on the device's shared persisting-L2 record (l2_acquire)
   size_t l2_max_persist = 0; // device property persistingL2CacheMaxSize
+  size_t l2_max_window = 0;  // device property accessPolicyMaxWindowSize: an access-policy window may not be larger
   int splitk = 1;     // 1: small batches (no CTA pairs) use the split-K kernel when a GEMM has <= one tile per SM
   int split_target = 0;  // experiments: target CTA count of a split-K launch (0 = one per SM)
   float* sk_scratch = nullptr;  // [sm_count][128 x 256] fp32 partial tiles
@@ -750,8 +750,10 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
   lc.pdl = h->pdl && !h->timing;
   // The fp32 residual stream (read and rewritten by both residual GEMMs of every layer) is marked persisting in L2
   // for every kernel of the stack, so that its 2 x 2 passes per layer stay out of DRAM (TE_OPT_L2_RESIDUAL).
-  if (h->l2_resid && h->l2_limit_bytes > 0) {
-    const size_t bytes = (size_t)Tb * d * sizeof(float);
+  if (h->l2_resid && h->l2_limit_bytes > 0 && h->l2_max_window > 0) {
+    // a window larger than the device allows makes every launch fail: cover the first accessPolicyMaxWindowSize bytes only
+    size_t bytes = (size_t)Tb * d * sizeof(float);
+    if (bytes > h->l2_max_window) bytes = h->l2_max_window;
     lc.l2.base_ptr = h->resid;
     lc.l2.num_bytes = bytes;
     lc.l2.hitRatio = bytes <= h->l2_limit_bytes ? 1.0f : (float)h->l2_limit_bytes / (float)bytes;
@@ -770,7 +772,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
     tick();
     pp.qkv_rows = reinterpret_cast<uint4*>(h->qkv); pp.qkv_row_vec16 = n_qkv / 8;
     pp.xg8 = pl.mx ? h->xg8 : nullptr; pp.sf_xg = h->sf_xg;
-    TE_CUDA(h, launch_k(lc, te::te_prep_kernel, dim3(Tb + te::PREP_PAD_ROWS), dim3(256), 0, st, pp));
+    // te_set_dyn_kernel -> prep is a FULL stream dependency (no programmatic overlap): the GEMM kernels read DynParams
+    // (total_tokens, out) before their griddepcontrol.wait, which is only ordered behind set_dyn if the kernel between
+    // them started after set_dyn had completed.  Inside a replayed graph prep is the first node, so nothing is lost.
+    LaunchCtx lc_first = lc;
+    lc_first.pdl = false;
+    TE_CUDA(h, launch_k(lc_first, te::te_prep_kernel, dim3(Tb + te::PREP_PAD_ROWS), dim3(256), 0, st, pp));
     tock(TE_KCLASS_PREP);
     ++nk;
   }
@@ -1054,12 +1061,49 @@ cudaError_t set_dyn(te_handle* h, const void* embeds, const int32_t* lens, float
   return cudaGetLastError();
 }
 
-void release_l2_limit(te_handle* h) {
-  if (h->l2_limit_raised) {
+// cudaLimitPersistingL2CacheSize is ONE value per device, shared by every handle of the process (a decoder handle and a
+// vision tower's handle is the normal pairing) and possibly touched from several host threads: one mutex-protected
+// record per device keeps the value found before the first handle asked, the largest request, and how many handles
+// hold it.  The limit is raised to the largest request and put back (persisting lines reset) by the LAST release.
+struct L2Record {
+  size_t orig = 0, cur = 0;
+  int refs = 0;
+};
+constexpr int L2_MAX_DEVICES = 64;
+L2Record g_l2[L2_MAX_DEVICES];
+std::mutex g_l2_mu;
+
+// Device `device` is current.  True if a carve-out of at least `want` bytes is now in force (one reference taken).
+bool l2_acquire(int device, size_t want) {
+  if (device < 0 || device >= L2_MAX_DEVICES || want == 0) return false;
+  std::lock_guard<std::mutex> lock(g_l2_mu);
+  L2Record& r = g_l2[device];
+  if (r.refs == 0) {
+    if (cudaDeviceGetLimit(&r.orig, cudaLimitPersistingL2CacheSize) != cudaSuccess) { cudaGetLastError(); return false; }
+    r.cur = r.orig;
+  }
+  if (want > r.cur) {
+    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) { cudaGetLastError(); return false; }
+    r.cur = want;
+  }
+  ++r.refs;
+  return true;
+}
+void l2_release(int device) {
+  std::lock_guard<std::mutex> lock(g_l2_mu);
+  L2Record& r = g_l2[device];
+  if (r.refs > 0 && --r.refs == 0) {
     cudaCtxResetPersistingL2Cache();
-    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, h->l2_prev_limit);
+    if (r.cur != r.orig) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, r.orig);
     cudaGetLastError();
-    h->l2_limit_raised = false;
+    r.cur = r.orig;
+  }
+}
+
+void release_l2_limit(te_handle* h) {
+  if (h->l2_ref_held) {
+    l2_release(h->device);
+    h->l2_ref_held = false;
   }
   h->l2_limit_bytes = 0;
 }
@@ -1092,6 +1136,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   h->device = device;
   h->sm_count = prop.multiProcessorCount;
   h->l2_max_persist = (size_t)prop.persistingL2CacheMaxSize;
+  h->l2_max_window = prop.accessPolicyMaxWindowSize > 0 ? (size_t)prop.accessPolicyMaxWindowSize : 0;
   h->dbg_lb = 0;
   h->dbg_le = cfg->n_layers;
   const te_config& c = h->cfg;
@@ -1345,22 +1390,17 @@ static int encode_impl(te_handle* h, int32_t n_frames, const int32_t* grids, int
   if (h->timing && cap != cudaStreamCaptureStatusNone) return TE_ERR_INVALID_ARG;
   if (h->l2_resid && h->l2_limit_bytes == 0 && cap == cudaStreamCaptureStatusNone) {
     // once per handle, outside any capture: reserve persisting L2 for the residual stream.  This is a DEVICE-WIDE
-    // limit; the previous value is restored by te_destroy and by TE_OPT_L2_RESIDUAL = 0.
+    // limit shared by all handles (l2_acquire); the value found before the first handle is restored when the last one
+    // lets go (te_destroy, TE_OPT_L2_RESIDUAL = 0).
     size_t want = (size_t)h->cap_rows * c.hidden * sizeof(float);
     if (want > (64u << 20)) want = 64u << 20;
     if (want > h->l2_max_persist) want = h->l2_max_persist;
-    size_t prev = 0;
-    cudaDeviceGetLimit(&prev, cudaLimitPersistingL2CacheSize);
-    if (want > 0 && prev >= want) {
-      h->l2_limit_bytes = want;  // someone already reserved enough
-    } else if (want > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
+    if (l2_acquire(h->device, want)) {
       h->l2_limit_bytes = want;
-      h->l2_prev_limit = prev;
-      h->l2_limit_raised = true;
+      h->l2_ref_held = true;
     } else {
       h->l2_resid = 0;
     }
-    cudaGetLastError();
   }
   // per-call pointers and token count: one tiny kernel ahead of the stack (stream-ordered, also under capture)
   TE_CUDA(h, set_dyn(h, embeds, text_lens, out, total_tokens, st, grids, embeds_bf16));
@@ -1965,10 +2005,11 @@ int te_vision_load_weights(te_vision* v, const void* blob, size_t n_bytes) {
 }
 
 int te_encode_image(te_vision* v, int32_t n_frames, const float* pixels, const int32_t* text_lens, float* embeds,
-                    void* cuda_stream) {
+                    int32_t total_tokens, void* cuda_stream) {
   if (!v || !pixels || !embeds) return TE_ERR_INVALID_ARG;
   if (!v->loaded) return TE_ERR_NOT_LOADED;
   if (n_frames < 1 || n_frames > v->cfg.max_frames) return TE_ERR_INVALID_ARG;
+  if ((long long)total_tokens < (long long)n_frames * v->n_vis) return TE_ERR_INVALID_ARG;  // the visual rows alone do not fit
   TE_CUDA(v, cudaSetDevice(v->device));
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const int gh = v->gh, gw = v->gw, d_v = v->d_v;
@@ -1989,10 +2030,18 @@ int te_encode_image(te_vision* v, int32_t n_frames, const float* pixels, const i
   te::te_merge2x2_kernel<<<n_merged, 256, 0, st>>>(v->tower_out, v->a_m, gh, gw, d_v);
   TE_CUDA(v, cudaGetLastError());
   TE_CUDA(v, vision_gemm(v->tmA_m, v->tmB_m, v->vis, n_merged, v->cfg.out_hidden, 4 * d_v, v->bn_m, v->pair_m, v->sm_count, st));
-  te::te_scatter_visual_kernel<<<n_merged, 256, 0, st>>>(v->vis, embeds, text_lens, v->n_vis, v->cfg.out_hidden);
+  te::te_scatter_visual_kernel<<<n_merged, 256, 0, st>>>(v->vis, embeds, text_lens, v->n_vis, v->cfg.out_hidden, n_frames,
+                                                         total_tokens, v->tower->flag);
   TE_CUDA(v, cudaGetLastError());
   v->launches += 5 + (v->tower->launches - before);
   return TE_OK;
+}
+
+int te_vision_query_async_error(te_vision* v) {
+  if (!v) return TE_ERR_INVALID_ARG;
+  const int rc = te_query_async_error(v->tower);  // the scatter raises the tower handle's flag
+  if (rc != TE_OK) v->err = v->tower->err;
+  return rc;
 }
 
 int64_t te_vision_kernel_launches(te_vision* v) { return v ? v->launches : 0; }

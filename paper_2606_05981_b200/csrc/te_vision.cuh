@@ -52,17 +52,31 @@ __global__ void __launch_bounds__(256) te_merge2x2_kernel(const float* __restric
 
 // One block per merged token: row b*n_vis + m of `vis` -> row cu[b] + m of `embeds`, cu[b] = b*n_vis + sum of the
 // text lengths of the frames before b (negative lengths count as 0, as in te_prep_kernel).  text_lens == nullptr:
-// the frames are packed without text (embeds = [B*n_vis, d]).
+// the frames are packed without text (embeds = [B*n_vis, d]).  `embeds` has total_tokens rows and text_lens is
+// unvalidated device data: a row at or past total_tokens is NOT written, and the sticky validation flag (the tower
+// handle's; same bits as te_prep_kernel) gets 1 for a negative length, 2 when the packed frames do not fit in (or, seen
+// from the last frame, do not add up to) total_tokens.
 __global__ void __launch_bounds__(256) te_scatter_visual_kernel(const float* __restrict__ vis, float* __restrict__ embeds,
-                                                                const int32_t* __restrict__ text_lens, int n_vis, int d) {
+                                                                const int32_t* __restrict__ text_lens, int n_vis, int d,
+                                                                int n_frames, int total_tokens, int32_t* __restrict__ flag) {
   const int mt = blockIdx.x;
   const int b = mt / n_vis, m = mt - b * n_vis;
   long long row = (long long)b * n_vis + m;
+  int bad = 0;
   if (text_lens != nullptr)
     for (int i = 0; i < b; ++i) {
       const int tl = text_lens[i];
+      if (tl < 0) bad |= 1;
       row += tl > 0 ? tl : 0;
     }
+  if (m == n_vis - 1 && b == n_frames - 1) {  // the last visual row of the call: the whole sum is known here
+    const int tl = text_lens != nullptr ? text_lens[b] : 0;
+    if (tl < 0) bad |= 1;
+    if (row + 1 + (tl > 0 ? tl : 0) != (long long)total_tokens) bad |= 2;
+  }
+  if (row >= (long long)total_tokens) bad |= 2;
+  if (bad && threadIdx.x == 0) atomicOr(flag, bad);
+  if (row >= (long long)total_tokens) return;
   const float4* src = reinterpret_cast<const float4*>(vis + (size_t)mt * d);
   float4* dst = reinterpret_cast<float4*>(embeds + (size_t)row * d);
   for (int i = threadIdx.x; i < d / 4; i += blockDim.x) dst[i] = src[i];

@@ -967,3 +967,80 @@ def test_random_shape_sweep_all_dtypes(H, O, seed):
         assert te.te_query_async_error(g.enc.h) == te.TE_OK
     for g in encs.values():
         g.close()
+
+
+# ------------------------------------------------------------------- device-wide L2 settings
+def _persisting_l2_limit():
+    """cudaDeviceGetLimit(cudaLimitPersistingL2CacheSize) of the current device, through the runtime torch loaded (the
+    limit belongs to the device's primary context, which the library shares)."""
+    import ctypes
+    import glob
+    import os
+    import torch
+    cands = glob.glob(os.path.join(os.path.dirname(torch.__file__), "..", "nvidia", "cuda_runtime", "lib", "libcudart.so*"))
+    cands += ["libcudart.so.12", "libcudart.so"]
+    for c in cands:
+        try:
+            rt = ctypes.CDLL(c)
+            break
+        except OSError:
+            continue
+    else:
+        pytest.skip("no libcudart to query the limit with")
+    v = ctypes.c_size_t(0)
+    assert rt.cudaDeviceGetLimit(ctypes.byref(v), 6) == 0        # cudaLimitPersistingL2CacheSize = 0x06
+    return v.value
+
+
+def test_persisting_l2_limit_is_shared_by_handles_and_restored_by_the_last(H):
+    """Two live handles (the decoder + vision-tower pairing): the device-wide persisting-L2 limit is raised once, stays
+    up when the handle that raised it is destroyed FIRST, still serves the survivor (same bits), and returns to the
+    value found before the first handle only when the last one goes — whatever the destruction order."""
+    import torch
+    w, blob, tl, T, emb, ch = H.workload_inputs(2)
+    torch.cuda.synchronize()
+    before = _persisting_l2_limit()
+    a = H.GpuTE(w.model, len(tl), T, blob)
+    ref = a.encode(emb, tl, w.grid_h, w.grid_w)
+    raised = _persisting_l2_limit()
+    assert raised >= min(T, 128) * w.model.hidden * 4 and raised >= before
+    b = H.GpuTE(w.model, len(tl), T, blob)
+    assert np.array_equal(b.encode(emb, tl, w.grid_h, w.grid_w), ref)
+    assert _persisting_l2_limit() == raised
+    a.close()                                                    # the one that raised it goes first
+    assert _persisting_l2_limit() == raised
+    assert np.array_equal(b.encode(emb, tl, w.grid_h, w.grid_w), ref)
+    b.close()
+    assert _persisting_l2_limit() == before
+    c = H.GpuTE(w.model, len(tl), T, blob)                       # and the cycle starts clean again
+    assert np.array_equal(c.encode(emb, tl, w.grid_h, w.grid_w), ref)
+    c.close()
+    assert _persisting_l2_limit() == before
+
+
+def test_residual_larger_than_the_access_policy_window(H):
+    """72 frames x 256 tokens x 2048 x 4 B = 151 MB of fp32 residual: more than accessPolicyMaxWindowSize.  The L2 window
+    must shrink to what the device allows instead of making every launch fail; results equal the no-window run bitwise."""
+    import torch
+    import paper_2606_05981_b200 as te
+    w = W.get_workload(2)
+    m = w.model
+    B, text = 72, 192
+    T = B * (w.grid_h * w.grid_w + text)
+    assert T * m.hidden * 4 > torch.cuda.get_device_properties(0).L2_cache_size
+    blob = H.cached_blob(m, w.seed_weights)
+    emb = np.random.default_rng(5).standard_normal((T, m.hidden)).astype(np.float32)
+    tl = np.full(B, text, dtype=np.int32)
+    g = H.GpuTE(m, B, T, blob)
+    got = g.encode(emb, tl, w.grid_h, w.grid_w)                  # default options: window on
+    assert te.te_query_async_error(g.enc.h) == te.TE_OK
+    te.te_set_option(g.enc.h, te.TE_OPT_L2_RESIDUAL, 0)
+    plain = g.encode(emb, tl, w.grid_h, w.grid_w)
+    g.close()
+    assert np.isfinite(got).all() and np.array_equal(got, plain)
+    # frames are independent and identical in shape: frame 0 of this batch == the same frame encoded alone
+    S = w.grid_h * w.grid_w + text
+    g1 = H.GpuTE(m, 1, S, blob)
+    alone = g1.encode(emb[:S], tl[:1], w.grid_h, w.grid_w)
+    g1.close()
+    assert PM.rel_l2(got[:S], alone) < 1e-3

@@ -239,6 +239,55 @@ def test_image_to_hidden_states_end_to_end(O, V, H):
     assert mm["max_row_update_rel_l2"] <= PM.GATE_ROW_UPDATE_REL_L2, mm
 
 
+def test_encode_image_never_writes_past_total_tokens():
+    """te_encode_image reads text_lens on the device, unvalidated: whatever it holds, no row at or past total_tokens may
+    be written (te.h containment promise, same as te_encode), and the sticky flag must say what was wrong.  A guard band
+    behind `embeds` shows any stray write."""
+    import torch
+    import paper_2606_05981_b200 as te
+    v = W.VISION_TINY
+    B, n_vis, d, guard = 3, v.tokens_per_frame, v.out_hidden, 64
+    good = [5, 0, 7]
+    T = B * n_vis + sum(good)
+    enc = te.VisionEncoder(v, B)
+    enc.load_weights(W.make_vision_blob(v))
+    pd = torch.from_numpy(np.ascontiguousarray(W.make_pixels(v, B), dtype=np.float32)).cuda()
+
+    def run(lens):
+        buf = torch.full((T + guard, d), -7.0, dtype=torch.float32, device="cuda")
+        tl = torch.tensor(lens, dtype=torch.int32, device="cuda")
+        enc.encode_image(B, pd, tl, buf, total_tokens=T)
+        rc = enc.query_async_error()
+        return buf.cpu().numpy(), rc, te.lib().te_vision_last_error(enc.v).decode()
+
+    ref, rc, _ = run(good)
+    assert rc == te.TE_OK
+    cu = np.concatenate([[0], np.cumsum([n_vis + t for t in good])])
+    vis_rows = np.concatenate([np.arange(cu[b], cu[b] + n_vis) for b in range(B)])
+    text_rows = np.setdiff1d(np.arange(T + guard), vis_rows)
+    assert np.all(ref[text_rows] == -7.0) and not np.any(ref[vis_rows] == -7.0)
+
+    # frame 1 claims 1000 text tokens: frame 2's visual rows would land ~1000 rows past the buffer
+    got, rc, msg = run([5, 1000, 7])
+    assert rc == te.TE_ERR_DEVICE_CHECK and "0x2" in msg, msg
+    assert np.all(got[T:] == -7.0)                                         # guard band intact
+    assert np.array_equal(got[:cu[2]], ref[:cu[2]])                        # frames 0 and 1 as before
+    assert np.all(got[cu[2]:T] == -7.0)                                    # frame 2: skipped, not misplaced
+    # partly out of range: frame 2 starts 10 rows late, so its last 3 visual rows fall off the end (7 text rows absorb the rest)
+    got, rc, msg = run([5, 10, 7])
+    assert rc == te.TE_ERR_DEVICE_CHECK and "0x2" in msg, msg
+    assert np.all(got[T:] == -7.0)
+    assert np.array_equal(got[cu[2] + 10:T], ref[cu[2]:cu[2] + n_vis][:T - cu[2] - 10])
+    # negative length: counted as 0 and flagged as such (9 + 0 + 3 still adds up to the 12 text rows: bit 1 alone)
+    got, rc, msg = run([9, -4, 3])
+    assert rc == te.TE_ERR_DEVICE_CHECK and "0x1 " in msg, msg
+    assert np.all(got[T:] == -7.0)
+    # the flag is cleared by the query: a good call afterwards is clean and identical to the first one
+    again, rc, _ = run(good)
+    assert rc == te.TE_OK and np.array_equal(again, ref)
+    enc.close()
+
+
 def test_vision_boundary_errors():
     import ctypes
     import paper_2606_05981_b200 as te
@@ -255,11 +304,12 @@ def test_vision_boundary_errors():
     assert L.te_vision_create(ctypes.byref(big), 0, ctypes.byref(h)) == te.TE_ERR_UNSUPPORTED
     vh = te.te_vision_create(cfg)
     blob = W.make_vision_blob(v)
-    assert L.te_encode_image(vh, 1, 1, 0, 1, 0) == te.TE_ERR_NOT_LOADED
+    assert L.te_encode_image(vh, 1, 1, 0, 1, 64, 0) == te.TE_ERR_NOT_LOADED
     assert L.te_vision_load_weights(vh, blob.ctypes.data, blob.nbytes - 2) == te.TE_ERR_BLOB_SIZE
     te.te_vision_load_weights(vh, blob)
-    assert L.te_encode_image(vh, 3, 1, 0, 1, 0) == te.TE_ERR_INVALID_ARG      # n_frames > max_frames
-    assert L.te_encode_image(vh, 1, 0, 0, 1, 0) == te.TE_ERR_INVALID_ARG      # null pixels
+    assert L.te_encode_image(vh, 3, 1, 0, 1, 4096, 0) == te.TE_ERR_INVALID_ARG      # n_frames > max_frames
+    assert L.te_encode_image(vh, 1, 0, 0, 1, 4096, 0) == te.TE_ERR_INVALID_ARG      # null pixels
+    assert L.te_encode_image(vh, 1, 1, 0, 1, 0, 0) == te.TE_ERR_INVALID_ARG         # total_tokens < n_frames * n_vis
     te.te_vision_destroy(vh)
     # non_causal and a cached prefix exclude each other
     c = te.make_config(W.get_workload(1).model, 2, 80, max_prefix_tokens=8, non_causal=1)
