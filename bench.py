@@ -92,12 +92,30 @@ def weights_fit_l2(m) -> bool:
 
 
 # ncu --set full captures of the dominant kernel, per launch (dram__bytes_read.sum + dram__bytes_write.sum), keyed by
-# (workload, kernel name as te_dispatch_info reports it).  NOT measured in the bench run: the value is quoted only when
-# the kernel that ran is the one that was profiled, with its source; otherwise `traffic` is null.
+# (workload, kernel name as te_dispatch_info reports it).  NOT measured in the bench run: each entry carries the hash of
+# the device code (csrc/*.cuh, kernel_source_hash) the capture was taken on, and `traffic` is quoted only when the kernel
+# that ran has that name AND the library's device code still hashes to that value; otherwise `traffic` is null.
 PROFILED_TRAFFIC = {
-    ("cfg4_28L_B16", "te_gemm2_kernel<256, 3, 128>"): (63.342336e6 + 15.066368e6, "profiles/r02a_cfg4.md"),
-    ("cfg4_28L_B16", "te_gemm8_kernel<192, 3, 128>"): (33.131520e6 + 0.233728e6, "profiles/r02a_cfg4.md"),
 }
+
+
+def kernel_source_hash() -> str:
+    """sha256 (first 16 hex digits) over the device-code headers of the library, in name order."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2606_05981_b200", "csrc")
+    hsh = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith(".cuh"):
+            hsh.update(f.encode())
+            hsh.update(open(os.path.join(d, f), "rb").read())
+    return hsh.hexdigest()[:16]
+
+
+def profiled_traffic(workload: str, kernel: str):
+    ent = PROFILED_TRAFFIC.get((workload, kernel))
+    if ent is None or ent[2] != kernel_source_hash():
+        return None, None
+    return ent[0], ent[1]
 
 
 # ------------------------------------------------------------------------- N>1 helpers (gloo-tested)
@@ -251,6 +269,94 @@ def measure_overlap(torch, te_step, side, te_ms, reps: int = 20):
             "main_ms": t_main, "side_te_ms": t_side, "both_ms": t_both, "max_ms": max(t_main, t_side),
             "sum_ms": t_main + t_side, "hidden_fraction_of_shorter_stream": hidden,
             "wall_over_max": t_both / max(t_main, t_side), "reps": reps}
+
+
+def time_encode(torch, enc, w, tl, T, emb, stream, warm: int, steps: int, flush_buf=None):
+    """Device time of `steps` te_encode calls of workload w on `stream` (CUDA events on that stream; optional L2 flush
+    before each timed call).  Returns (mean ms, min ms)."""
+    e = torch.from_numpy(emb).cuda()
+    ln = torch.from_numpy(np.asarray(tl, dtype=np.int32)).cuda()
+    o = torch.empty_like(e)
+    with torch.cuda.stream(stream):
+        for _ in range(warm):
+            enc.encode(len(tl), w.grid_h, w.grid_w, e, ln, T, o, stream.cuda_stream)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            if flush_buf is not None:
+                flush_buf.zero_()
+            a.record(stream)
+            enc.encode(len(tl), w.grid_h, w.grid_w, e, ln, T, o, stream.cuda_stream)
+            b.record(stream)
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, b in evs]
+    return sum(ms) / len(ms), min(ms)
+
+
+def stack_roofline_block(m, seq_lens, t_s, tc_ratio=1.0, wscale=1.0):
+    f, wb, ab = stack_work(m, seq_lens)
+    wb *= wscale
+    pk = load_peaks()
+    roof = max(f / (pk["tf_burst"] * tc_ratio * 1e12), (wb + ab) / (pk["hbm_gbs"] * 1e9))
+    roof_s = max(f / (pk["tf_sustained"] * tc_ratio * 1e12), (wb + ab) / (pk["hbm_gbs"] * 1e9))
+    return {"flops": f, "weight_bytes": wb, "act_bytes": ab, "roofline_ms_burst": 1000 * roof,
+            "bound": "tensor" if f / (pk["tf_burst"] * tc_ratio * 1e12) >= (wb + ab) / (pk["hbm_gbs"] * 1e9) else "hbm",
+            "frac_of_burst": roof / t_s, "frac_of_sustained": roof_s / t_s}
+
+
+def measure_sm_budget_overlap(torch, te, enc_side, enc_main, shapes, n_sms: int, reps: int = 10):
+    """Spatial sharing (TE_OPT_SM_BUDGET): the encoder on a side stream sized for n SMs while a second handle of the same
+    library — the stand-in for the denoiser, sized for the other n_sms - n — works on the main stream, one event joining
+    them as in the paper's Algorithm 1 (PAPER.md:118-137; :184 reports wall = max(side, main)).  For each split: each
+    stream alone, both together, wall / max(alone) and wall / (the two full-GPU runs back to back)."""
+    main = torch.cuda.current_stream()
+    side = torch.cuda.Stream()
+    out = {}
+    for name, (w, tl, T, emb) in shapes.items():
+        bufs = []
+        for _ in range(2):
+            e = torch.from_numpy(emb).cuda()
+            bufs.append((e, torch.from_numpy(np.asarray(tl, dtype=np.int32)).cuda(), torch.empty_like(e)))
+
+        def run(enc, buf, stream):
+            enc.encode(len(tl), w.grid_h, w.grid_w, buf[0], buf[1], T, buf[2], stream.cuda_stream)
+
+        def timed(do_main, do_side):
+            ts = []
+            for i in range(reps + 3):
+                e0, e1, es = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+                torch.cuda.synchronize()
+                e0.record(main)
+                side.wait_event(e0)
+                if do_side:
+                    run(enc_side, bufs[0], side)
+                es.record(side)
+                if do_main:
+                    run(enc_main, bufs[1], main)
+                main.wait_event(es)
+                e1.record(main)
+                torch.cuda.synchronize()
+                if i >= 3:
+                    ts.append(e0.elapsed_time(e1))
+            return statistics.median(ts)
+
+        rows = []
+        serial_full = None
+        for n in (n_sms, 112, 96, 74):
+            if n > n_sms:
+                continue
+            te.te_set_option(enc_side.h, te.TE_OPT_SM_BUDGET, 0 if n == n_sms else n)
+            te.te_set_option(enc_main.h, te.TE_OPT_SM_BUDGET, 0 if n == n_sms else n_sms - n)
+            t_side, t_main, t_both = timed(False, True), timed(True, False), timed(True, True)
+            if n == n_sms:
+                serial_full = t_side + t_main
+            rows.append({"side_sms": n, "main_sms": n_sms if n == n_sms else n_sms - n, "side_ms": t_side, "main_ms": t_main,
+                         "both_ms": t_both, "wall_over_max": t_both / max(t_side, t_main),
+                         "wall_over_serial_full_gpu": t_both / serial_full})
+        te.te_set_option(enc_side.h, te.TE_OPT_SM_BUDGET, 0)
+        te.te_set_option(enc_main.h, te.TE_OPT_SM_BUDGET, 0)
+        out[name] = rows
+    return {"main_load": "a second handle of this library running the same batch (stand-in for the denoiser)",
+            "reps": reps, "splits": out}
 
 
 # ------------------------------------------------------------- vision-tower front end (SURVEY 8f NEXT-4)
@@ -440,7 +546,7 @@ def main():
     opt_ids = {"pdl": te.TE_OPT_PDL, "cta_pair": te.TE_OPT_CTA_PAIR, "resid_bn": te.TE_OPT_RESID_BLOCK_N,
                "graph": te.TE_OPT_USE_GRAPH, "attn_impl": te.TE_OPT_ATTN_IMPL, "split_k": te.TE_OPT_SPLIT_K,
                "resid_wide": te.TE_OPT_RESID_WIDE, "l2_residual": te.TE_OPT_L2_RESIDUAL,
-               "resid_halves": te.TE_OPT_RESID_HALVES, "chain": te.TE_OPT_CHAIN}
+               "sm_budget": te.TE_OPT_SM_BUDGET}
     for kv in filter(None, args.opt.split(",")):
         k, v = kv.split("=")
         te.te_set_option(enc.h, opt_ids[k], int(v))
@@ -597,6 +703,50 @@ def main():
         }
         # the same frames' visual tokens from pixels: te_encode_image, B = this config's frames
         secondary[f"vision_front_end_B{w.n_frames}"] = measure_vision(torch, te, stream, w.n_frames)
+        # B = 1 on the same 28-layer handle (the paper's Table V starts at B = 1)
+        import dataclasses as _dc
+        w1 = _dc.replace(w3, n_frames=1, name="cfg3_28L_B1")
+        tl1 = W.make_text_lens(w1)
+        T1 = W.total_tokens(w1, tl1)
+        t1, t1min = time_encode(torch, enc, w1, tl1, T1, W.make_embeddings(w1, T1), stream, 20, 100)
+        secondary[w1.name] = {"metric": METRIC, "value": 1000.0 / t1, "unit": UNIT, "ms_per_step": t1, "ms_per_step_min": t1min,
+                              "steps": 100, "config": config_dict(w1, T1, world), "dispatch": te.te_dispatch_info(enc.h),
+                              "stack_roofline": stack_roofline_block(w1.model, [w1.grid_h * w1.grid_w + int(t) for t in tl1],
+                                                                     t1 / 1000.0, tc_ratio, wscale * ((1 + 1 / 16 if fp4 else 1 + 1 / 32) if mx else 1))}
+        # cfg 2: ONE full-width layer, one frame, weights (100 MB) evicted from L2 before every timed call
+        w2 = W.get_workload(2)
+        tl2 = W.make_text_lens(w2)
+        T2 = W.total_tokens(w2, tl2)
+        enc2 = te.TextEncoder(w2.model, w2.n_frames, T2, device=local_rank, weight_dtype=(2 if fp4 else 1) if mx else 0)
+        enc2.load_weights(W.make_weight_blob(w2.model, w2.seed_weights))
+        fb = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+        t2, t2min = time_encode(torch, enc2, w2, tl2, T2, W.make_embeddings(w2, T2), stream, 20, 100, flush_buf=fb)
+        secondary[w2.name] = {"metric": METRIC, "value": w2.n_frames * 1000.0 / t2, "unit": UNIT, "ms_per_step": t2,
+                              "ms_per_step_min": t2min, "steps": 100, "config": config_dict(w2, T2, world, flush_l2=True),
+                              "dispatch": te.te_dispatch_info(enc2.h),
+                              "stack_roofline": stack_roofline_block(w2.model, [w2.grid_h * w2.grid_w + int(t) for t in tl2],
+                                                                     t2 / 1000.0, tc_ratio, wscale * ((1 + 1 / 16 if fp4 else 1 + 1 / 32) if mx else 1))}
+        enc2.close()
+        del fb
+        if not mx:
+            # the block-scaled FP8 variant of the headline config, so that the driver's record has it
+            enc8 = te.TextEncoder(m, w.n_frames, T, device=local_rank, weight_dtype=1)
+            enc8.load_weights(blob)
+            t8a, _ = time_encode(torch, enc8, w, tl, T, emb, stream, 5, 20)
+            t8b, t8min = time_encode(torch, enc8, w, tl, T, emb, stream, 0, 50)
+            secondary[w.name + "_mxfp8"] = {
+                "metric": METRIC, "value": w.n_frames * 1000.0 / t8b, "unit": UNIT, "dtype": "mxfp8 (E4M3 x E4M3, E8M0 block scales, fp32 accumulate)",
+                "ms_per_step": t8b, "ms_per_step_first_20": t8a, "ms_per_step_min": t8min, "steps": 50,
+                "config": config_dict(w, T, world), "dispatch": te.te_dispatch_info(enc8.h),
+                "stack_roofline": stack_roofline_block(m, seq_lens, t8b / 1000.0, 2.0, 0.5 * (1 + 1 / 32))}
+            enc8.close()
+            # spatial sharing under an SM budget
+            encm = te.TextEncoder(m, w.n_frames, T, device=local_rank)
+            encm.load_weights(blob)
+            n_sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+            secondary["sm_budget_overlap"] = measure_sm_budget_overlap(
+                torch, te, enc, encm, {w.name: (w, tl, T, emb), w3.name: (w3, tl3, T3, W.make_embeddings(w3, T3))}, n_sms)
+            encm.close()
 
     if rank != 0:
         if dist is not None:
@@ -631,7 +781,7 @@ def main():
     gu_bytes = ((0.5 + 1 / 32 if fp4 else 1.0 + 1 / 32) * (2 * m.ffn * m.hidden) + (1.0 + 1 / 32) * T * m.hidden + (1.0 + 1 / 32) * T * m.ffn) if mx \
         else 2.0 * (2 * m.ffn * m.hidden) + 2.0 * T * m.hidden + 2.0 * T * m.ffn
     gu_name = dispatch.get("gateup", "?")
-    traffic, traffic_src = PROFILED_TRAFFIC.get((w.name, gu_name.split(" (")[0]), (None, None))
+    traffic, traffic_src = profiled_traffic(w.name, gu_name.split(" (")[0])
     region = f"{args.steps} steps = {t_dev:.2f} s timed region; per-kernel pass {args.kernel_timing_steps} steps"
     if t_compute >= t_hbm:
         achieved = gu_flops / (gu_ms_launch / 1000.0) / 1e12

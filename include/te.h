@@ -177,12 +177,21 @@ enum {
   TE_OPT_KERNEL_TIMING = 1,/* 1: direct launches bracketed by CUDA events per kernel (implies no
                               graph); read with te_kernel_times.  Measurement aid, default 0.     */
   TE_OPT_PDL = 4,          /* 1 (default): kernels are chained with programmatic dependent launch   */
-  TE_OPT_L2_RESIDUAL = 10  /* 1 (default): the library's fp32 residual stream is an L2-persisting access-policy window
+  TE_OPT_L2_RESIDUAL = 10, /* 1 (default): the library's fp32 residual stream is an L2-persisting access-policy window
                               of every kernel, so that the residual GEMMs' read-add-write passes stay out of DRAM.
                               The first te_encode raises the DEVICE-WIDE limit cudaLimitPersistingL2CacheSize to
                               min(max_tokens * hidden * 4, 64 MiB, device maximum) if it is lower; te_destroy and
                               setting this option to 0 reset the persisting lines and restore the previous limit.
                               0: no window                                                                        */
+  TE_OPT_SM_BUDGET = 14    /* n in [16, SMs of the device]: size every GEMM grid and every dispatch decision (tile
+                              shapes, split-K groups, one-wave wide tiles) for n SMs instead of all of them, so that a
+                              caller who runs a denoiser next to the encoder (the paper's side-stream pipeline,
+                              PAPER.md:114, Algorithm 1 :118-137) can leave the other SMs to it: the stack's kernels hold
+                              one CTA per SM with most of its shared memory, so without a budget nothing else fits
+                              beside them.  The budget bounds how many SMs the GEMMs occupy, it does not pin which;
+                              attention keeps one CTA per (frame, kv head) and the tiny prep kernel one block per
+                              token.  Results under a budget are correct to the same gates but not bitwise equal to
+                              the full-GPU run (other K splits, other summation order).  0 (default): all SMs         */
 };
 int te_set_option(te_handle* h, int option, int value);
 

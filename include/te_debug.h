@@ -25,15 +25,6 @@ enum {
                               CTA pairs) run the split-K kernel: several CTAs per output tile, each
                               streaming its own K-slice of the weights; partial tiles are summed in a
                               fixed order (deterministic).  0: one CTA per tile; n > 1: target CTA count */
-  TE_OPT_RESID_HALVES = 11,/* wide residual tiles as TWO column halves accumulated one after the other, so that the first
-                              half's read-add-write epilogue overlaps the second half's MMAs (te_gemm_wide2_kernel):
-                              1 = O-proj and down, 2 = O-proj only, 0 (default) = one pass (te_gemm_wide_kernel).
-                              Measured slower at cfg 4 (the A rows are fetched twice)                     */
-  TE_OPT_CHAIN = 13,       /* 1: at small batches consecutive GEMMs that are all one wave of 128 x 128 split-K tiles
-                              run as phases of ONE cooperative launch with grid-wide barriers between them
-                              (te_gemm_chain.cuh): O-proj -> gate/up -> down -> next QKV at T <= 128, down -> next QKV at
-                              T = 512.  0 (default): one launch per GEMM.  Compiled only with -DTE_WITH_CHAIN (else 1 is refused).  Bitwise the same results; measured SLOWER than the
-                              PDL-chained separate launches                                          */
   TE_OPT_RESID_WIDE = 9    /* O-proj / down on CTA pairs: 1 (default) = when their 128-wide tiles would need two or
                               more waves, ONE wave of wide tiles (width = hidden / n rounded up to 32, <= 512
                               columns, two MMAs per k-step; te_gemm_wide.cuh); 0 = never; n in 2..16 = always,
@@ -82,10 +73,6 @@ int te_debug_gemm_splitk(int device, const void* a_bf16, const void* b_bf16, flo
  * wholly out of range.  N % 32 == 0, width <= 512, ceil(M/256) * n_tiles <= SM pairs.  Synchronous. */
 int te_debug_gemm_wide(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
                        int32_t n, int32_t k, int32_t n_tiles);
-
-/* The same through the two-half variant (te_gemm_wide2_kernel: the tile's columns as two sub-tiles one after the other). */
-int te_debug_gemm_wide2(int device, const void* a_bf16, const void* b_bf16, float* c, int32_t m,
-                        int32_t n, int32_t k, int32_t n_tiles);
 
 /* MXFP8 quantiser alone (te_config.weight_dtype = 1; DESIGN.md §3 Q24-Q25): src DEVICE bf16 [rows, k] ->
  * codes DEVICE uint8 [rows, k] (E4M3) and scales_tiled DEVICE uint8 [rows/128 (rounded up), k/128, 512] (E8M0): the

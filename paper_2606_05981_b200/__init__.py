@@ -31,8 +31,7 @@ TE_OPT_ATTN_IMPL = 6
 TE_OPT_SPLIT_K = 7
 TE_OPT_RESID_WIDE = 9
 TE_OPT_L2_RESIDUAL = 10
-TE_OPT_RESID_HALVES = 11
-TE_OPT_CHAIN = 13
+TE_OPT_SM_BUDGET = 14
 TE_KCLASS_NAMES = ["scan", "prep", "qkv", "attn", "oproj", "gateup", "down", "final_norm"]
 TE_TAP_POS, TE_TAP_CU_SEQLENS, TE_TAP_COS, TE_TAP_SIN, TE_TAP_QKV, TE_TAP_ATTN, TE_TAP_ACT, TE_TAP_TRACE = range(8)
 TE_TAP_ATTN8, TE_TAP_ACT8, TE_TAP_SF_ATTN, TE_TAP_SF_ACT = 8, 9, 10, 11
@@ -45,7 +44,7 @@ EXPORTS = [
     "te_vision_blob_bytes", "te_vision_create", "te_vision_load_weights", "te_encode_image", "te_vision_kernel_launches",
     "te_vision_last_error", "te_vision_destroy", "te_matmul_noalloc", "te_vision_query_async_error",
 ]
-DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide", "te_debug_gemm_wide2",
+DEBUG_EXPORTS = ["te_debug_set_range", "te_debug_tap", "te_debug_gemm", "te_debug_gemm_splitk", "te_debug_gemm_wide",
                  "te_debug_mx_quantise", "te_debug_gemm_mxfp8", "te_debug_mx_quantise_fp4", "te_debug_gemm_mxfp4", "te_vision_debug_tap", "te_vision_debug_tower"]
 TE_VTAP_PATCH_EMBEDS, TE_VTAP_TOWER_OUT, TE_VTAP_MERGED = 0, 1, 2
 TE_DTYPE_BF16, TE_DTYPE_MXFP8, TE_DTYPE_MXFP4 = 0, 1, 2
@@ -134,8 +133,6 @@ def lib() -> ctypes.CDLL:
     L.te_matmul_noalloc.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32, c_int32, c_void_p]
     L.te_debug_gemm_wide.restype = c_int
     L.te_debug_gemm_wide.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
-    L.te_debug_gemm_wide2.restype = c_int
-    L.te_debug_gemm_wide2.argtypes = [c_int, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_int32, c_int32]
     L.te_debug_mx_quantise.restype = c_int
     L.te_debug_mx_quantise.argtypes = [c_int, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
     L.te_debug_gemm_mxfp8.restype = c_int
@@ -341,9 +338,8 @@ def te_debug_gemm_mxfp4(device, a_bf16, b_bf16, c, m, n, k, block_n=256):
     _check(lib().te_debug_gemm_mxfp4(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, block_n))
 
 
-def te_debug_gemm_wide(device, a_bf16, b_bf16, c, m, n, k, n_tiles, halves=0):
-    fn = lib().te_debug_gemm_wide2 if halves else lib().te_debug_gemm_wide
-    _check(fn(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, n_tiles))
+def te_debug_gemm_wide(device, a_bf16, b_bf16, c, m, n, k, n_tiles):
+    _check(lib().te_debug_gemm_wide(device, _ptr(a_bf16), _ptr(b_bf16), _ptr(c), m, n, k, n_tiles))
 
 
 def te_destroy(h):

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libte_b200.so")
 SOURCES = ["te_runtime.cu"]
-HEADERS = ["te_ptx.cuh", "te_gemm.cuh", "te_gemm8.cuh", "te_gemm_splitk.cuh", "te_gemm_chain.cuh", "te_gemm_wide.cuh", "te_vision.cuh", "te_attn.cuh", "te_attn_tc.cuh", "te_prep.cuh"]
+HEADERS = ["te_ptx.cuh", "te_gemm.cuh", "te_gemm8.cuh", "te_gemm_splitk.cuh", "te_gemm_wide.cuh", "te_vision.cuh", "te_attn.cuh", "te_attn_tc.cuh", "te_prep.cuh"]
 
 
 def _stale() -> bool:

@@ -84,16 +84,11 @@ struct GemmParams {
   // rows (n'>>1)*256 + (n'&1)*64 .. +64 and the matching up rows 128 further on, as two 64-row halves
   int gu_half;
 };
-// Loads of data that an EARLIER PHASE of the same launch may have rewritten (te_gemm_chain.cuh, built only with
-// -DTE_WITH_CHAIN) must not be served from a stale L1 line; in the default build a kernel boundary separates writer and
-// reader and the ordinary (L1-cached) load is what the epilogue-bound kernels want.
+// Epilogue loads of data written by an earlier KERNEL (gains, RMSNorm statistics, rotary table): a kernel boundary
+// separates writer and reader, so the ordinary L1-cached load is right.
 template <typename T>
 __device__ __forceinline__ T ld_phase(const T* ptr) {
-#ifdef TE_WITH_CHAIN
-  return __ldcg(ptr);
-#else
   return *ptr;
-#endif
 }
 __device__ __forceinline__ int gemm_rows(const GemmParams& p) { return p.dyn != nullptr ? p.dyn->total_tokens : p.M; }
 __device__ __forceinline__ float* resid_dst(const GemmParams& p) { return p.x_to_out ? p.dyn->out : p.x; }

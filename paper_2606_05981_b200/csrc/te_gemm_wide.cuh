@@ -29,24 +29,18 @@ struct GemmWideCfg {
   static constexpr int SMEM_LIMIT = 232448;  // 227 KB
   static constexpr int TMEM_COLS = 512;
   static constexpr int MAX_STAGES = 8;
-  // halves = 1 (EPI_RESID / EPI_PLAIN): the tile's columns are accumulated as TWO sub-tiles one after the other
-  // (widths w0 = ceil(bn / 64) * 32 and bn - w0, one MMA of that width per k-step), so a stage holds only w0 / 2
-  // weight rows per CTA
-  __host__ __device__ static constexpr int sub_w0(int bn) { return ((bn / 32 + 1) / 2) * 32; }
-  __host__ __device__ static constexpr int b_bytes(int bn, int halves = 0) {  // per CTA and stage
-    return ((halves ? sub_w0(bn) : bn) / 2) * GEMM_BK * 2;
-  }
-  __host__ __device__ static constexpr int stage_bytes(int bn, int halves = 0) { return A_BYTES + b_bytes(bn, halves); }
-  // halves = 0: one tile per CTA pair and ONE accumulator barrier, so the epilogue staging ALIASES the ring (first
-  // written when every MMA has read its stage and no TMA write is outstanding in either CTA): one more stage in flight
-  // at the SwiGLU widths.  halves = 1 keeps a private staging area (sub-tile 1's loads land during sub-tile 0's epilogue).
-  __host__ __device__ static constexpr int stages(int bn, int halves = 0) {
-    const int fit = (SMEM_LIMIT - 1024 - BAR_BYTES - (halves ? STG_BYTES : 0)) / stage_bytes(bn, halves);
+  __host__ __device__ static constexpr int b_bytes(int bn) { return (bn / 2) * GEMM_BK * 2; }  // per CTA and stage
+  __host__ __device__ static constexpr int stage_bytes(int bn) { return A_BYTES + b_bytes(bn); }
+  // One tile per CTA pair and ONE accumulator barrier, so the epilogue staging ALIASES the ring (first written when
+  // every MMA has read its stage and no TMA write is outstanding in either CTA): one more stage in flight at the SwiGLU
+  // widths.
+  __host__ __device__ static constexpr int stages(int bn) {
+    const int fit = (SMEM_LIMIT - 1024 - BAR_BYTES) / stage_bytes(bn);
     return fit > MAX_STAGES ? MAX_STAGES : fit;
   }
-  __host__ __device__ static constexpr int smem_bytes(int bn, int halves = 0) {
-    const int ring = stages(bn, halves) * stage_bytes(bn, halves);
-    return (halves ? ring + STG_BYTES : (ring > STG_BYTES ? ring : STG_BYTES)) + BAR_BYTES + 1024;
+  __host__ __device__ static constexpr int smem_bytes(int bn) {
+    const int ring = stages(bn) * stage_bytes(bn);
+    return (ring > STG_BYTES ? ring : STG_BYTES) + BAR_BYTES + 1024;
   }
 };
 
@@ -325,279 +319,6 @@ te_gemm_wide_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_consta
   __syncwarp();  // the elected producer / MMA lanes rejoin their warps before the block barrier
   __syncthreads();
   if (threadIdx.x == 0) trace_stamp(p, 36);
-  cluster_sync_all();  // the peer may still be signalling our barriers / reading our smem until here
-  if (threadIdx.x == 0) trace_stamp(p, 37);
-  if (warp == 1) {
-    __syncwarp();
-    tc_fence_after();
-    tmem_dealloc_cg2(tmem_base, Cfg::TMEM_COLS);
-  }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// Two column halves per tile (EPI_RESID, EPI_PLAIN).  What the one-pass kernel above cannot hide is its epilogue:
-// every CTA read-add-writes its 128 x bn fp32 slice of the residual with no main loop left (pipeline trace at cfg 4:
-// O-proj 15.3 us main loop + 9.8 us epilogue, down 45.3 + 7.7).  Here the tile's columns are accumulated as two
-// sub-tiles one after the other — sub-tile 0 = the first w0 = ceil(bn / 64) * 32 columns over ALL k-blocks, then
-// sub-tile 1 = the remaining bn - w0 — each by one tcgen05.mma.cta_group::2 of that width per k-step into its own TMEM
-// columns, so the epilogue warps work on sub-tile 0 while the tensor core contracts sub-tile 1; only the (smaller)
-// second epilogue stays exposed.  Price: the A rows are fetched twice (per k-block 16 KB of A + w/4 weight rows per
-// CTA: 73 / 81 B/clk per SM at bn = 352 instead of 54).  tmB0 / tmB1: the weight matrix in boxes of w0/2 and w1/2 rows.
-template <int EPI>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM2_THREADS, 1)
-te_gemm_wide2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
-                     const __grid_constant__ CUtensorMap tmB1, const GemmParams p, const int bn) {
-  static_assert(EPI == EPI_RESID || EPI == EPI_PLAIN, "two-half wide tiles: residual / plain epilogues");
-  using Cfg = GemmWideCfg;
-  const int STAGES = Cfg::stages(bn, 1);
-  const int b_bytes = Cfg::b_bytes(bn, 1);
-  const int wsub[2] = {Cfg::sub_w0(bn), bn - Cfg::sub_w0(bn)};
-  const int osub[2] = {0, Cfg::sub_w0(bn)};
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint8_t* sA = smem;
-  uint8_t* sB = smem + STAGES * Cfg::A_BYTES;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * Cfg::stage_bytes(bn, 1));
-  uint64_t* full = bars;                          // used in the leader CTA only
-  uint64_t* empty = bars + Cfg::MAX_STAGES;       // one set per CTA
-  uint64_t* tfull = bars + 2 * Cfg::MAX_STAGES;   // [2] one per sub-tile and CTA
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tfull + 2);
-  float* stg_all = reinterpret_cast<float*>(smem + STAGES * Cfg::stage_bytes(bn, 1) + Cfg::BAR_BYTES);
-
-  const int warp = threadIdx.x >> 5;
-  const int lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();
-  const bool leader = rank == 0;
-  if (threadIdx.x == 0) trace_stamp(p, 0);
-
-  if (warp == 0 && elect_one()) {
-    tma_prefetch_desc(&tmA);
-    tma_prefetch_desc(&tmB0);
-    tma_prefetch_desc(&tmB1);
-  }
-  if (warp == 1) {
-    if (elect_one()) {
-      for (int i = 0; i < STAGES; ++i) {
-        mbar_init(&full[i], 1);
-        mbar_init(&empty[i], 1);
-      }
-      mbar_init(&tfull[0], 1);
-      mbar_init(&tfull[1], 1);
-      fence_mbar_init();
-    }
-    __syncwarp();
-    tmem_alloc_cg2(tmem_slot, Cfg::TMEM_COLS);
-  }
-  tc_fence_before();
-  __syncthreads();
-  cluster_sync_all();
-  tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
-  pdl_launch_dependents();
-  if (threadIdx.x == 0) trace_stamp(p, 1);
-
-  const int M = gemm_rows(p);
-  const int num_kb = p.K / GEMM_BK;
-  const int num_mp = (p.num_m_blk + 1) >> 1;  // 256-row blocks
-  const int tile = blockIdx.x >> 1;           // one tile per CTA pair
-  const int mp = tile % num_mp;
-  const int n_blk = tile / num_mp;
-  const int col_base = n_blk * bn;
-  const int n_sub = wsub[1] > 0 ? 2 : 1;
-
-  if (warp == 0) {
-    // ===================== TMA producer (both CTAs) =====================
-    if (elect_one()) {
-      const int a_row = mp * 2 * GEMM_BM + rank * GEMM_BM;
-      const int pre = num_kb < STAGES ? num_kb : STAGES;
-      {  // sub-tile 0's first ring of weights: independent of the predecessor kernel
-        const int b_row = col_base + rank * (wsub[0] / 2);
-        for (int kb = 0; kb < pre; ++kb) {
-          if (leader) mbar_arrive_expect_tx(&full[kb], 2 * (Cfg::A_BYTES + wsub[0] * GEMM_BK));
-          tma_load_2d_cg2(sB + kb * b_bytes, &tmB0, mapa_u32(smem_u32(&full[kb]), 0), kb * GEMM_BK, b_row);
-        }
-      }
-      pdl_wait();
-      trace_stamp(p, 2);
-      int stage = 0;
-      uint32_t phase = 0;
-      for (int sub = 0; sub < n_sub; ++sub) {
-        const int b_row = col_base + osub[sub] + rank * (wsub[sub] / 2);
-        const CUtensorMap* tmB = sub == 0 ? &tmB0 : &tmB1;
-        for (int kb = 0; kb < num_kb; ++kb) {
-          const uint32_t bar = mapa_u32(smem_u32(&full[stage]), 0);
-          if (sub != 0 || kb >= pre) {
-            mbar_wait(&empty[stage], phase ^ 1);
-            if (leader) mbar_arrive_expect_tx(&full[stage], 2 * (Cfg::A_BYTES + wsub[sub] * GEMM_BK));
-            tma_load_2d_cg2(sB + stage * b_bytes, tmB, bar, kb * GEMM_BK, b_row);
-          }
-          tma_load_2d_cg2(sA + stage * Cfg::A_BYTES, &tmA, bar, kb * GEMM_BK, a_row);
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ===================== MMA issuer (leader CTA only) =====================
-    if (leader && elect_one()) {
-      int stage = 0;
-      uint32_t phase = 0;
-      for (int sub = 0; sub < n_sub; ++sub) {
-        const uint32_t idesc = umma_idesc_bf16(2 * GEMM_BM, static_cast<uint32_t>(wsub[sub]));
-        const uint32_t d_tmem = tmem_base + osub[sub];
-        for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(&full[stage], phase);
-          if (kb == 0) trace_stamp(p, 3 + sub);
-          tc_fence_after();
-          const uint64_t a_desc = umma_smem_desc_sw128(smem_u32(sA + stage * Cfg::A_BYTES));
-          const uint64_t b_desc = umma_smem_desc_sw128(smem_u32(sB + stage * b_bytes));
-#pragma unroll
-          for (int k = 0; k < GEMM_BK / 16; ++k)
-            umma_bf16_cg2(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
-          umma_commit_cg2(&empty[stage], 0x3);  // frees this stage in BOTH CTAs
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-        umma_commit_cg2(&tfull[sub], 0x3);  // this sub-tile's accumulator is ready in BOTH CTAs
-      }
-    }
-  } else {
-    // ===================== epilogue warps (both CTAs, own 128 rows) =====================
-    const int quad = warp & 3;
-    const int part = (warp - 2) >> 2;
-    const int sub_l = lane >> 3, cq = lane & 7;
-    const int row_base = mp * 2 * GEMM_BM + rank * GEMM_BM + quad * 32;
-    const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quad * 32) << 16);
-    float* stg = stg_all + (warp - 2) * (Cfg::STG_WARP_BYTES / 4);
-    int n_valid = p.N - col_base;
-    n_valid = n_valid < 0 ? 0 : (n_valid > bn ? bn : n_valid);
-    // the valid 32-column chunks of each sub-tile are split between the two warps of a quadrant
-    int c_begin[2], c_end[2];
-#pragma unroll
-    for (int sub = 0; sub < 2; ++sub) {
-      int v = n_valid - osub[sub];
-      v = v < 0 ? 0 : (v > wsub[sub] ? wsub[sub] : v);
-      const int chunks = v / 32;
-      c_begin[sub] = osub[sub] + (part == 0 ? 0 : ((chunks + 1) / 2) * 32);
-      c_end[sub] = osub[sub] + (part == 0 ? ((chunks + 1) / 2) * 32 : chunks * 32);
-    }
-    pdl_wait();
-    if constexpr (EPI == EPI_PLAIN) {
-      const int row = row_base + lane;
-#pragma unroll 1
-      for (int sub = 0; sub < 2; ++sub) {
-        if (c_begin[sub] >= c_end[sub]) continue;
-        mbar_wait(&tfull[sub], 0);
-        tc_fence_after();
-#pragma unroll 1
-        for (int c0 = c_begin[sub]; c0 < c_end[sub]; c0 += 32) {
-          uint32_t r[32];
-          tmem_ld32(t_row + c0, r);
-          tmem_ld_wait();
-          if (row < M) {
-            float4* dst = reinterpret_cast<float4*>(p.c + (size_t)row * p.ld_c + col_base + c0);
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-              dst[j] = make_float4(__uint_as_float(r[4 * j]), __uint_as_float(r[4 * j + 1]), __uint_as_float(r[4 * j + 2]),
-                                   __uint_as_float(r[4 * j + 3]));
-          }
-        }
-      }
-    } else {
-      const bool has_g = p.g_next != nullptr;
-      float* const x_dst = resid_dst(p);
-      auto issue_x = [&](float4 (&xv)[8], int c0) {
-        const int col = col_base + c0 + cq * 4;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const int row = row_base + sub_l + 4 * i;
-          if (row < M) xv[i] = *reinterpret_cast<const float4*>(p.x + (size_t)row * p.ld_x + col);
-        }
-      };
-      // next chunk after c0 in this warp's order (sub-tile 0's range, then sub-tile 1's); -1: none
-      auto next_chunk = [&](int c0) {
-        if (c0 < osub[1]) {
-          if (c0 + 32 < c_end[0]) return c0 + 32;
-          return c_begin[1] < c_end[1] ? c_begin[1] : -1;
-        }
-        return c0 + 32 < c_end[1] ? c0 + 32 : -1;
-      };
-      float4 xn[8];
-      const int c_first = c_begin[0] < c_end[0] ? c_begin[0] : (c_begin[1] < c_end[1] ? c_begin[1] : -1);
-      if (c_first >= 0) issue_x(xn, c_first);  // first chunk's x while the main loop runs
-      float ss[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) ss[i] = 0.f;
-#pragma unroll 1
-      for (int sub = 0; sub < 2; ++sub) {
-        if (c_begin[sub] >= c_end[sub]) continue;
-        mbar_wait(&tfull[sub], 0);
-        if (warp == 2 && lane == 0) trace_stamp(p, 14 + sub);
-        tc_fence_after();
-#pragma unroll 1
-        for (int c0 = c_begin[sub]; c0 < c_end[sub]; c0 += 32) {
-          {
-            uint32_t r[32];
-            tmem_ld32(t_row + c0, r);
-            tmem_ld_wait();
-            float v[32];
-#pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
-            stg_put_row(stg, lane, v);
-          }
-          __syncwarp();
-          const int col = col_base + c0 + cq * 4;
-          float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f;
-          if (has_g) {
-            const uint2 g = __ldg(reinterpret_cast<const uint2*>(p.g_next + col));
-            g0 = bf16_lo(g.x); g1 = bf16_hi(g.x); g2 = bf16_lo(g.y); g3 = bf16_hi(g.y);
-          }
-          float4 xv[8];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) xv[i] = xn[i];
-          const int cn = next_chunk(c0);
-          if (cn >= 0) issue_x(xn, cn);  // next chunk's x in flight
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const int rr = sub_l + 4 * i;
-            const int row = row_base + rr;
-            if (row < M) {
-              const float4 a = stg_get(stg, rr, cq);
-              float4 v = xv[i];
-              v.x += a.x; v.y += a.y; v.z += a.z; v.w += a.w;
-              *reinterpret_cast<float4*>(x_dst + (size_t)row * p.ld_x + col) = v;
-              ss[i] = fmaf(v.x, v.x, ss[i]); ss[i] = fmaf(v.y, v.y, ss[i]);
-              ss[i] = fmaf(v.z, v.z, ss[i]); ss[i] = fmaf(v.w, v.w, ss[i]);
-              if (has_g) {
-                uint2 o;
-                o.x = pack_bf16(v.x * g0, v.y * g1);
-                o.y = pack_bf16(v.z * g2, v.w * g3);
-                *reinterpret_cast<uint2*>(p.xg + (size_t)row * p.ld_x + col) = o;
-              }
-            }
-          }
-          __syncwarp();
-        }
-        if (warp == 2 && lane == 0) trace_stamp(p, 25 + sub);
-      }
-      // per-row sum of squares over this warp's columns of BOTH sub-tiles (fixed-order reduction over the row's 8
-      // lanes); a warp without valid columns still writes its zero
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 1);
-        ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 2);
-        ss[i] += __shfl_xor_sync(0xffffffffu, ss[i], 4);
-      }
-      if (cq == 0 && p.ssq_out != nullptr) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const int row = row_base + sub_l + 4 * i;
-          if (row < M) p.ssq_out[(size_t)row * p.ssq_stride + (n_blk * 2 + part)] = ss[i];
-        }
-      }
-    }
-  }
-  tc_fence_before();
-  __syncwarp();  // the elected producer / MMA lanes rejoin their warps before the block barrier
-  __syncthreads();
   cluster_sync_all();  // the peer may still be signalling our barriers / reading our smem until here
   if (threadIdx.x == 0) trace_stamp(p, 37);
   if (warp == 1) {

@@ -19,9 +19,6 @@
 #include "te_gemm.cuh"
 #include "te_gemm8.cuh"
 #include "te_gemm_splitk.cuh"
-#ifdef TE_WITH_CHAIN  // experiment: build with TE_NVCC_EXTRA=-DTE_WITH_CHAIN
-#include "te_gemm_chain.cuh"
-#endif
 #include "te_gemm_wide.cuh"
 #include "te_prep.cuh"
 #include "te_vision.cuh"
@@ -139,7 +136,6 @@ struct Plan {
   int bn_res = 128, k_res = 0, bx_res = 0, n_blk_res = 0, wide_tiles = 0, wide_bn = 0;
   int parts = 1;       // RMSNorm partial sums per row written by the residual GEMMs
   int attn_tc = 0, attn_split = 1, q_blocks = 1, g_shift = 0, s_bound = 0;
-  int chain = 0;       // small batches: 4 = O-proj -> gate/up -> down -> next QKV in one launch, 2 = down -> next QKV, 0 = none
   int mx = 0;          // MXFP8 variant: every GEMM on te_gemm8_kernel (CTA pairs, block-scaled tcgen05)
 };
 
@@ -148,7 +144,8 @@ struct Plan {
 struct te_handle {
   te_config cfg{};
   int device = 0;
-  int sm_count = 0;
+  int sm_count = 0;  // SMs every grid and dispatch decision is sized for: sm_dev, or the caller's budget (TE_OPT_SM_BUDGET)
+  int sm_dev = 0;    // SMs of the device
   bool loaded = false;
   // tile choices
   int bn_qkv = 256, bn_gu = 256, bn_res = 128;
@@ -156,9 +153,6 @@ struct te_handle {
   int pair_mode = 2;  // 0: always 1-CTA tiles, 1: always CTA pairs (cta_group::2), 2: auto (by token count)
   int resid_wide = 1; // residual GEMMs on CTA pairs: 1 = auto (one wave of wide tiles when 128-wide tiles need >= 2
                       // waves), 0 = never, n >= 2 = always with n tiles across N (tests)
-  int chain = 0;        // small batches: consecutive split-K GEMMs as phases of one launch (te_gemm_chain.cuh; measured slower)
-  int* chain_bar = nullptr;  // [2] its grid-barrier arrival / departure counters
-  int resid_halves = 0; // wide residual tiles as two column halves (te_gemm_wide2_kernel): 1 = O-proj and down, 2 = O-proj, 0 = one pass
   int l2_resid = 1;          // 1: the residual stream is an L2-persisting access window of every kernel
   size_t l2_limit_bytes = 0; // persisting-L2 carve-out requested for it (0 until the first te_encode sets the limit)
   bool l2_ref_held = false;  // this handle holds one reference on the device's shared persisting-L2 record (l2_acquire)
@@ -496,25 +490,11 @@ cudaError_t init_kernel_attrs() {
   TE_ATTR((set_gemm_attr<128, te::EPI_SWIGLU, 128>()));
   TE_ATTR((set_gemm_attr<256, te::EPI_PLAIN, 128>()));
   TE_ATTR((set_gemm_attr<128, te::EPI_PLAIN, 128>()));
-#ifdef TE_WITH_CHAIN
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::CHAIN_SMEM_BYTES)));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::CHAIN_SMEM_BYTES)));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::CHAIN_SMEM_BYTES)));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemmk_chain_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::CHAIN_SMEM_BYTES)));
-#endif
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide_kernel<te::EPI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::GemmWideCfg::SMEM_LIMIT)));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide2_kernel<te::EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                te::GemmWideCfg::SMEM_LIMIT)));
-  TE_ATTR((cudaFuncSetAttribute(te::te_gemm_wide2_kernel<te::EPI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 te::GemmWideCfg::SMEM_LIMIT)));
   TE_ATTR((set_gemm8_attr<128, te::EPI_QKV, 128>()));
   TE_ATTR((set_gemm8_attr<128, te::EPI_QKV, 64>()));
@@ -547,20 +527,6 @@ cudaError_t launch_wide(const LaunchCtx& lc, const CUtensorMap& tmA, const CUten
   const int num_mp = (p.num_m_blk + 1) / 2;
   return launch_k(lc, te::te_gemm_wide_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
                   te::GemmWideCfg::smem_bytes(bn), st, tmA, tmB, p, bn);
-}
-
-// The same tiles as two column halves accumulated one after the other (te_gemm_wide2_kernel): the first half's
-// epilogue overlaps the second half's main loop.  `w`: the weight matrix [N, K].
-template <int EPI>
-cudaError_t launch_wide2(const LaunchCtx& lc, const CUtensorMap& tmA, const void* w, int n_rows, int k, const te::GemmParams& p,
-                         int n_tiles, int bn, cudaStream_t st) {
-  const int w0 = te::GemmWideCfg::sub_w0(bn), w1 = bn - w0;
-  CUtensorMap tb0, tb1;
-  if (!make_tmap(&tb0, w, n_rows, k, w0 / 2) || !make_tmap(&tb1, w, n_rows, k, w1 > 0 ? w1 / 2 : w0 / 2))
-    return cudaErrorInvalidValue;
-  const int num_mp = (p.num_m_blk + 1) / 2;
-  return launch_k(lc, te::te_gemm_wide2_kernel<EPI>, dim3(2 * num_mp * n_tiles), dim3(te::GEMM2_THREADS),
-                  te::GemmWideCfg::smem_bytes(bn, 1), st, tmA, tb0, tb1, p, bn);
 }
 
 // Token-count bucket: the row-block count that every grid and every dispatch decision is derived from.
@@ -641,9 +607,6 @@ Plan make_plan(const te_handle* h, int Tb, int n_frames, int n_vis) {
     pl.n_blk_res = d / 128;
     pl.parts = pl.n_blk_res * 2;
   }
-  // chained launches (te_gemm_chain.cuh): consecutive GEMMs that are all one wave of 128 x 128 split-K tiles
-  if (h->chain && !h->timing && !pl.mx && pl.k_qkv && pl.bn_qkv == 128 && pl.k_res && pl.bn_res == 128)
-    pl.chain = (pl.k_gu && pl.bn_gu == 128) ? 4 : 2;
   // attention: host-side upper bound of S_b for the grid (exact lengths stay on the device)
   int s_bound = Tb - (n_frames - 1) * n_vis;
   if (s_bound > c.max_tokens_per_frame) s_bound = c.max_tokens_per_frame;
@@ -693,9 +656,8 @@ std::string describe_plan(const te_handle* h, const Plan& pl) {
                                                 : "te_attn_kernel");
   s += b;
   if (pl.wide_tiles) {
-    const bool h_o = h->resid_halves != 0, h_d = (h->resid_halves & 1) && !(h->resid_halves & 2);
-    snprintf(b, sizeof(b), "oproj=te_gemm_wide%s_kernel<2> (%d tiles x %d cols);down=te_gemm_wide%s_kernel<2> (%d tiles x %d cols);",
-             h_o ? "2" : "", pl.wide_tiles, pl.wide_bn, h_d ? "2" : "", pl.wide_tiles, pl.wide_bn);
+    snprintf(b, sizeof(b), "oproj=te_gemm_wide_kernel<2> (%d tiles x %d cols);down=te_gemm_wide_kernel<2> (%d tiles x %d cols);",
+             pl.wide_tiles, pl.wide_bn, pl.wide_tiles, pl.wide_bn);
     s += b;
   } else {
     gemm("oproj", te::EPI_RESID, pl.k_res, pl.pair, pl.bn_res, 128);
@@ -707,8 +669,6 @@ std::string describe_plan(const te_handle* h, const Plan& pl) {
   } else {
     gemm("gateup", te::EPI_SWIGLU, pl.k_gu, pl.pair_gu, pl.bn_gu, 128);
   }
-  if (pl.chain == 4) s += "chain=te_gemmk_chain_kernel (oproj, gateup, down and the next layer's qkv as phases of one launch);";
-  if (pl.chain == 2) s += "chain=te_gemmk_chain_kernel (down and the next layer's qkv as phases of one launch);";
   snprintf(b, sizeof(b), "bucket_tokens=%d", pl.Tb);
   s += b;
   return s;
@@ -786,12 +746,12 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
   base.splits = 1; base.sk_scratch = h->sk_scratch; base.sk_sem = h->sk_sem;
   base.M = Tb; base.num_m_blk = num_m; base.ssq_in = h->ssq; base.ssq_parts = pl.parts; base.ssq_stride = h->ssq_parts_cap;
   base.inv_d = 1.0f / static_cast<float>(d); base.eps = c.rms_eps;
-  const size_t trace_stride = (size_t)h->sm_count * te::TRACE_SLOTS;
+  const size_t trace_stride = (size_t)h->sm_dev * te::TRACE_SLOTS;
   auto trace_ptr = [&](int cls) { return h->trace_on ? h->trace + cls * trace_stride : nullptr; };
   // the last residual GEMM of the stack hands the stream over to the caller's buffer
   const bool norm_tail = c.final_norm && le == c.n_layers && !dbg_stop;
 
-  // ---- per-GEMM parameters of layer l (shared by the stand-alone launches and by the chained phases)
+  // ---- per-GEMM parameters of layer l
   auto qkv_params = [&](int l) {
     const LayerOff& o = h->off[l];
     te::GemmParams p = base;
@@ -835,45 +795,10 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
     if (pl.k_res) p.splits = choose_splits(h->split_target, num_m * p.num_n_blk, p.K / te::GEMM_BK, h->sm_count);
     return p;
   };
-  // Chained launches (te_gemm_chain.cuh): consecutive GEMMs that are all one wave of 128 x 128 split-K tiles run as
-  // phases of ONE cooperative grid.  chain4: O-proj -> gate/up -> down -> next layer's QKV (T <= 128);
-  // chain2: down -> next layer's QKV (e.g. T = 512, where gate/up runs on the wide CTA-pair kernel).
-  const bool chain_ok = pl.chain != 0 && !prefix_pass;
-  const bool chain4 = chain_ok && pl.chain == 4;
-#ifdef TE_WITH_CHAIN
-  auto launch_chain = [&](int n_ph, const te::GemmParams* ps, const int* epis, const CUtensorMap* const* ma,
-                          const CUtensorMap* const* mb) -> cudaError_t {
-    te::ChainParams cp{};
-    int grid = 1;
-    for (int i = 0; i < n_ph; ++i) {
-      cp.p[i] = ps[i];
-      cp.epi[i] = epis[i];
-      const int ctas = ps[i].num_m_blk * ps[i].num_n_blk * ps[i].splits;
-      if (ctas > grid) grid = ctas;
-    }
-    cp.n_phases = n_ph;
-    cp.gbar = h->chain_bar;
-    LaunchCtx lcc = lc;
-    lcc.coop = true;  // the phases meet at a grid-wide counter: every CTA resident at once
-    const CUtensorMap* fa[te::CHAIN_MAX_PHASES];
-    const CUtensorMap* fb[te::CHAIN_MAX_PHASES];
-    for (int i = 0; i < te::CHAIN_MAX_PHASES; ++i) { fa[i] = ma[i < n_ph ? i : 0]; fb[i] = mb[i < n_ph ? i : 0]; }
-    auto kern = n_ph >= 3 ? (dh == 128 ? te::te_gemmk_chain_kernel<128, true> : te::te_gemmk_chain_kernel<64, true>)
-                          : (dh == 128 ? te::te_gemmk_chain_kernel<128, false> : te::te_gemmk_chain_kernel<64, false>);
-    return launch_k(lcc, kern, dim3(grid), dim3(te::GEMMK_THREADS), te::CHAIN_SMEM_BYTES, st, *fa[0],
-                    *fb[0], *fa[1], *fb[1], *fa[2], *fb[2], *fa[3], *fb[3], cp);
-  };
-
-#else
-  auto launch_chain = [&](int, const te::GemmParams*, const int*, const CUtensorMap* const*, const CUtensorMap* const*) -> cudaError_t {
-    return cudaErrorNotSupported;
-  };
-#endif
-  bool qkv_done = false;  // this layer's QKV was the last phase of the previous layer's chain
   for (int l = lb; l < le; ++l) {
     const LayerOff& o = h->off[l];
     const bool last_layer = l == le - 1;
-    if (!qkv_done) {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
+    {  // a1: RMSNorm -> QKV GEMM -> QK-norm + M-RoPE
       te::GemmParams p = qkv_params(l);
       tick();
       if (pl.mx) {
@@ -894,7 +819,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tock(TE_KCLASS_QKV);
       ++nk;
     }
-    qkv_done = false;
     if (prefix_pass) {  // keep this layer's keys | values of the prefix tokens
       TE_CUDA(h, cudaMemcpy2DAsync(h->kv_prefix + (size_t)l * c.max_prefix_tokens * n_kv, (size_t)n_kv * sizeof(bf16),
                                    h->qkv + n_q, (size_t)n_qkv * sizeof(bf16), (size_t)n_kv * sizeof(bf16),
@@ -909,7 +833,7 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         tp.g_shift = pl.g_shift; tp.scale_log2 = scale_log2; tp.non_causal = c.non_causal;
         tp.stats = P > 0 ? h->attn_stats : nullptr; tp.o32 = P > 0 ? h->attn_o32 : nullptr; tp.prefix_mode = 0; tp.prefix_len = 0;
         tp.out8 = pl.mx ? h->attn8 : nullptr; tp.sf_out = h->sf_attn;
-        tp.trace = trace_ptr(4); tp.trace_ctas = h->sm_count;
+        tp.trace = trace_ptr(4); tp.trace_ctas = h->sm_dev;
         TE_CUDA(h, dh == 128 ? launch_attn_tc<128>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st)
                              : launch_attn_tc<64>(lc, h->tmQ, h->tmKV, tp, pl.attn_split, n_frames, st));
         if (P > 0) {  // second pass: the P cached prefix keys of this layer, merged in place
@@ -929,24 +853,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tock(TE_KCLASS_ATTN);
       ++nk;
     }
-    const bool next_qkv = l + 1 < le;  // a following layer whose QKV can ride along
-    if (chain4 && !(dbg_stop && last_layer)) {
-      // a3 + a4 + a5 (+ the next layer's a1) as phases of one launch
-      te::GemmParams ps[4] = {oproj_params(l, last_layer), gu_params(l), down_params(l, last_layer), te::GemmParams{}};
-      int epis[4] = {te::EPI_RESID, te::EPI_SWIGLU, te::EPI_RESID, te::EPI_QKV};
-      const CUtensorMap* ma[4] = {&h->tmA_attn, &h->tmA_xg, &h->tmA_act, &h->tmA_xg};
-      const CUtensorMap* mb[4] = {&h->tm[l].o[pl.bx_res], &h->tm[l].gu[pl.bx_gu], &h->tm[l].d[pl.bx_res], nullptr};
-      int n_ph = 3;
-      if (next_qkv) {
-        ps[3] = qkv_params(l + 1);
-        mb[3] = &h->tm[l + 1].qkv[pl.bx_qkv];
-        n_ph = 4;
-      }
-      TE_CUDA(h, launch_chain(n_ph, ps, epis, ma, mb));
-      ++nk;
-      qkv_done = next_qkv;
-      continue;
-    }
     {  // a3: O projection + residual add (+ next norm's gain / statistics)
       te::GemmParams p = oproj_params(l, last_layer);
       tick();
@@ -956,8 +862,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
         TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_attn8, h->tm8[l].o[0], h->tmSF_attn, h->tm8[l].sf_o, p, x8,
                                                         h->sm_count, st)));
-      } else if (pl.wide_tiles && h->resid_halves) {
-        TE_CUDA(h, launch_wide2<te::EPI_RESID>(lc, h->tmA_attn, h->w + o.wo, d, n_q, p, pl.wide_tiles, pl.wide_bn, st));
       } else if (pl.wide_tiles) {
         CUtensorMap tmB;
         if (!make_tmap(&tmB, h->w + o.wo, d, n_q, pl.wide_bn / 4)) { h->err = "tensor map (wide O-proj)"; return TE_ERR_CUDA; }
@@ -997,16 +901,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
       tock(TE_KCLASS_GATEUP);
       ++nk;
     }
-    if (chain_ok && next_qkv) {  // a5 + the next layer's a1 in one launch
-      te::GemmParams ps[2] = {down_params(l, last_layer), qkv_params(l + 1)};
-      int epis[2] = {te::EPI_RESID, te::EPI_QKV};
-      const CUtensorMap* ma[2] = {&h->tmA_act, &h->tmA_xg};
-      const CUtensorMap* mb[2] = {&h->tm[l].d[pl.bx_res], &h->tm[l + 1].qkv[pl.bx_qkv]};
-      TE_CUDA(h, launch_chain(2, ps, epis, ma, mb));
-      ++nk;
-      qkv_done = true;
-      continue;
-    }
     {  // a5: down projection + residual add
       te::GemmParams p = down_params(l, last_layer);
       tick();
@@ -1016,8 +910,6 @@ int enqueue_stack(te_handle* h, int n_frames, int grid_h, int grid_w, int Tb, cu
         x8.q_out = h->xg8; x8.q_sf = h->sf_xg; x8.q_kchunks = d / 128; x8.q_ld = d;
         TE_CUDA(h, (launch_gemm8<128, te::EPI_RESID, 128>(lc, h->tmA_act8, h->tm8[l].d[0], h->tmSF_act, h->tm8[l].sf_d, p, x8,
                                                         h->sm_count, st)));
-      } else if (pl.wide_tiles && (h->resid_halves & 1) && !(h->resid_halves & 2)) {
-        TE_CUDA(h, launch_wide2<te::EPI_RESID>(lc, h->tmA_act, h->w + o.wd, d, F, p, pl.wide_tiles, pl.wide_bn, st));
       } else if (pl.wide_tiles) {
         CUtensorMap tmB;
         if (!make_tmap(&tmB, h->w + o.wd, d, F, pl.wide_bn / 4)) { h->err = "tensor map (wide down)"; return TE_ERR_CUDA; }
@@ -1134,7 +1026,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   te_handle* h = new te_handle();
   h->cfg = *cfg;
   h->device = device;
-  h->sm_count = prop.multiProcessorCount;
+  h->sm_count = h->sm_dev = prop.multiProcessorCount;
   h->l2_max_persist = (size_t)prop.persistingL2CacheMaxSize;
   h->l2_max_window = prop.accessPolicyMaxWindowSize > 0 ? (size_t)prop.accessPolicyMaxWindowSize : 0;
   h->dbg_lb = 0;
@@ -1170,7 +1062,6 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
   TE_ALLOC(h->act, T * c.ffn * sizeof(bf16));
   TE_ALLOC(h->sk_scratch, (size_t)h->sm_count * te::GEMM_BM * 256 * sizeof(float));
   TE_ALLOC(h->sk_sem, 2 * (size_t)h->sm_count * sizeof(int));
-  TE_ALLOC(h->chain_bar, 2 * sizeof(int));
 #undef TE_ALLOC
   // rows past a call's tokens are read (never stored) by the tile-granular kernels: start them finite
   if (cudaMemset(h->xg, 0, T * c.hidden * sizeof(bf16)) != cudaSuccess ||
@@ -1178,8 +1069,7 @@ int te_create(const te_config* cfg, int device, te_handle** out) {
       cudaMemset(h->attn, 0, T * (size_t)n_q * sizeof(bf16)) != cudaSuccess ||
       cudaMemset(h->act, 0, T * c.ffn * sizeof(bf16)) != cudaSuccess ||
       cudaMemset(h->dyn, 0, sizeof(te::DynParams)) != cudaSuccess ||
-      cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess ||
-      cudaMemset(h->chain_bar, 0, 2 * sizeof(int)) != cudaSuccess)
+      cudaMemset(h->sk_sem, 0, 2 * (size_t)h->sm_count * sizeof(int)) != cudaSuccess)
     return fail(TE_ERR_CUDA);
   if (c.weight_dtype >= 1) {  // MXFP8 activations (A operands) + tiled block scales (one byte per 32 elements)
     const size_t rb = (T + 127) / 128;  // 128-row scale tiles
@@ -1590,7 +1480,7 @@ int te_set_option(te_handle* h, int option, int value) {
     case TE_OPT_KERNEL_TIMING: h->timing = value ? 1 : 0; return TE_OK;
     case TE_OPT_TRACE:
       if (value && !h->trace) {
-        const size_t bytes = 5 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+        const size_t bytes = 5 * (size_t)h->sm_dev * te::TRACE_SLOTS * sizeof(unsigned long long);
         TE_CUDA(h, cudaMalloc(reinterpret_cast<void**>(&h->trace), bytes));
         TE_CUDA(h, cudaMemset(h->trace, 0, bytes));
       }
@@ -1617,21 +1507,13 @@ int te_set_option(te_handle* h, int option, int value) {
       if (value < 0 || value > 16) return TE_ERR_INVALID_ARG;
       h->resid_wide = value;
       break;
-    case TE_OPT_CHAIN:
-#ifdef TE_WITH_CHAIN
-      h->chain = value ? 1 : 0;
-      break;
-#else
-      if (value) return TE_ERR_UNSUPPORTED;  // the chained-launch experiment is not in this build (TE_WITH_CHAIN)
-      break;
-#endif
-    case TE_OPT_RESID_HALVES:
-      if (value < 0 || value > 3) return TE_ERR_INVALID_ARG;
-      h->resid_halves = value;
-      break;
     case TE_OPT_SPLIT_K:
       h->splitk = value ? 1 : 0;
       h->split_target = value > 1 ? value : 0;
+      break;
+    case TE_OPT_SM_BUDGET:
+      if (value != 0 && (value < 16 || value > h->sm_dev)) return TE_ERR_INVALID_ARG;
+      h->sm_count = value ? value : h->sm_dev;
       break;
     case TE_OPT_RESID_BLOCK_N:
       if ((value != 128 && value != 256) || h->cfg.hidden % value != 0) return TE_ERR_INVALID_ARG;
@@ -1701,7 +1583,7 @@ int te_debug_tap(te_handle* h, int what, void* dst, size_t n_bytes) {
     case TE_TAP_SF_ACT: src = h->sf_act; need = (T + 127) / 128 * ((size_t)c.ffn / 128) * 512; break;
     case TE_TAP_TRACE:
       src = h->trace;
-      need = 5 * (size_t)h->sm_count * te::TRACE_SLOTS * sizeof(unsigned long long);
+      need = 5 * (size_t)h->sm_dev * te::TRACE_SLOTS * sizeof(unsigned long long);
       if (!src) return TE_ERR_INVALID_ARG;
       break;
     default: return TE_ERR_INVALID_ARG;
@@ -1790,26 +1672,6 @@ int te_debug_gemm_wide(int device, const void* a, const void* b, float* cmat, in
   p.c = cmat; p.ld_c = n;
   const LaunchCtx lc;
   cudaError_t e = launch_wide<te::EPI_PLAIN>(lc, ta, tb, p, n_tiles, bn, nullptr);
-  if (e == cudaSuccess) e = cudaDeviceSynchronize();
-  return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
-}
-
-int te_debug_gemm_wide2(int device, const void* a, const void* b, float* cmat, int32_t m, int32_t n, int32_t k,
-                        int32_t n_tiles) {
-  int sms = 0;
-  int rc = debug_gemm_prologue(device, a, b, cmat, m, n, k, &sms);
-  if (rc != TE_OK) return rc;
-  if (n_tiles < 1 || n % 32 != 0) return TE_ERR_UNSUPPORTED;
-  const int bn = (((n + n_tiles - 1) / n_tiles) + 31) / 32 * 32;
-  const int num_m = (m + te::GEMM_BM - 1) / te::GEMM_BM;
-  if (bn > 512 || ((num_m + 1) / 2) * n_tiles > sms / 2) return TE_ERR_UNSUPPORTED;  // one wave only
-  CUtensorMap ta;
-  if (!make_tmap(&ta, a, m, k, te::GEMM_BM)) return TE_ERR_CUDA;
-  te::GemmParams p{};
-  p.M = m; p.N = n; p.K = k; p.num_m_blk = num_m; p.num_n_blk = n_tiles;
-  p.c = cmat; p.ld_c = n;
-  const LaunchCtx lc;
-  cudaError_t e = launch_wide2<te::EPI_PLAIN>(lc, ta, b, n, k, p, n_tiles, bn, nullptr);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   return e == cudaSuccess ? TE_OK : TE_ERR_CUDA;
 }
@@ -2086,7 +1948,7 @@ void te_destroy(te_handle* h) {
   for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
   void* ptrs[] = {h->w, h->dyn, h->resid, h->cu, h->pos, h->flag, h->cos_t, h->sin_t, h->ssq, h->inv_freq, h->xg, h->qkv,
                   h->attn, h->act, h->slot[0].embeds, h->slot[0].out, h->slot[0].lens, h->slot[1].embeds, h->slot[1].out,
-                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->chain_bar, h->kv_prefix, h->prefix_buf, h->prefix_lens,
+                  h->slot[1].lens, h->trace, h->sk_scratch, h->sk_sem, h->kv_prefix, h->prefix_buf, h->prefix_lens,
                   h->attn_stats, h->attn_o32, h->w8, h->sfw, h->xg8, h->attn8, h->act8, h->sf_xg, h->sf_attn, h->sf_act};
   for (void* p : ptrs)
     if (p) cudaFree(p);

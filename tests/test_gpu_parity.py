@@ -88,13 +88,11 @@ def test_gemm_splitk_vs_fp64_matmul(H, M, N, K, bn, splits):
 @pytest.mark.parametrize("M,N,K,n_tiles", [(3072, 2048, 2048, 6), (3072, 2048, 6144, 6), (3733, 2048, 2048, 4),
                                            (2048, 2048, 6144, 9), (1500, 2048, 2048, 7), (593, 256, 768, 5),
                                            (300, 256, 256, 3), (256, 2048, 2048, 16)])
-@pytest.mark.parametrize("halves", [0, 1])
-def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles, halves):
+def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles):
     """One-wave wide-tile kernel alone (te_gemm_wide.cuh, plain epilogue), elementwise against an fp64 matmul: the
     widths the stack's dispatch picks at cfg 4 (6 x 352) and cfg 5 (4 x 512), a partly out-of-range last tile
     (7 x 320 > 2048), a wholly out-of-range one (5 x 64 > 256), a ragged last row-pair block, one MMA narrower than
-    the other tile widths (16 x 128).  halves = 1: te_gemm_wide2_kernel — the tile's columns as two sub-tiles accumulated
-    one after the other (352 -> 192 + 160, 64 -> 32 + 32, 512 -> 256 + 256, 128 -> 64 + 64, 32 -> 32 + 0 ...)."""
+    the other tile widths (16 x 128)."""
     import torch
     import paper_2606_05981_b200 as te
     rng = np.random.default_rng(M * 3 + N + n_tiles)
@@ -104,7 +102,7 @@ def test_gemm_wide_vs_fp64_matmul(H, M, N, K, n_tiles, halves):
     ad = torch.from_numpy(a.view(np.int16)).cuda()
     bd = torch.from_numpy(b.view(np.int16)).cuda()
     c = torch.full((M, N), float("nan"), dtype=torch.float32, device="cuda")
-    te.te_debug_gemm_wide(0, ad, bd, c, M, N, K, n_tiles, halves)
+    te.te_debug_gemm_wide(0, ad, bd, c, M, N, K, n_tiles)
     out = c.cpu().numpy()
     assert np.isfinite(out).all()
     assert PM.rel_l2(out, ref) < 1e-5
@@ -604,12 +602,10 @@ def test_many_small_frames(H, O):
     g.close()
 
 
-@pytest.mark.parametrize("halves", [1, 0, 2])
 @pytest.mark.parametrize("n_tiles", [2, 3, 5, 8])
-def test_wide_residual_tiles(H, O, n_tiles, halves):
+def test_wide_residual_tiles(H, O, n_tiles):
     """O-proj / down as one wave of wide CTA-pair tiles: forced tile counts whose widths do and do not divide the hidden
-    size (a partly and a completely out-of-range last tile), ragged last row-pair block.  halves: 1 = both GEMMs as two
-    column halves (te_gemm_wide2_kernel), 0 = one pass with two MMAs per k-step (the default), 2 = O-proj only."""
+    size (a partly and a completely out-of-range last tile), ragged last row-pair block."""
     m = W.TINY
     blob = H.cached_blob(m, 1)
     tl = [5, 0, 190, 33, 240, 65]
@@ -618,9 +614,8 @@ def test_wide_residual_tiles(H, O, n_tiles, halves):
     emb = np.random.default_rng(4).standard_normal((T, m.hidden)).astype(np.float32)
     ref = O.encode(blob, W.blob_layout(m), m, emb, tl, gh, gw)
     g = H.GpuTE(m, len(tl), T, blob, cta_pair=1, resid_wide=n_tiles)
-    g.te.te_set_option(g.enc.h, g.te.TE_OPT_RESID_HALVES, halves)
     out = g.encode(emb, tl, gh, gw)
-    _assert_final(PM.stack_metrics(out, ref, emb), f"wide residual tiles n={n_tiles} halves={halves}")
+    _assert_final(PM.stack_metrics(out, ref, emb), f"wide residual tiles n={n_tiles}")
     assert np.array_equal(out, g.encode(emb, tl, gh, gw))
     g.close()
 
@@ -796,11 +791,14 @@ def test_stale_rows_of_a_larger_call_do_not_leak(H, O):
 
 
 # --------------------------------------------- side stream against a foreign load
+@pytest.mark.parametrize("budget", [0, 74])
 @pytest.mark.parametrize("case", ["cfg2_split_k", "pairs_T1024"])
-def test_side_stream_under_foreign_load_is_bitwise_identical(H, case):
+def test_side_stream_under_foreign_load_is_bitwise_identical(H, case, budget):
     """The paper's mechanism 1 (Algorithm 1 :118-137): te_encode on a SIDE stream while the main stream
     runs a denoiser-shaped load (library bf16 matmuls), joined by one event.  The result must be bitwise the solo
-    result — the cooperative split-K groups (cfg 2) and the CTA-pair kernels (T = 1024) only get delayed."""
+    result — the cooperative split-K groups (cfg 2) and the CTA-pair kernels (T = 1024) only get delayed.
+    budget = 74: the same with the encoder sized for half the SMs (TE_OPT_SM_BUDGET), the arrangement that lets the
+    foreign load actually run beside it."""
     import torch
     import paper_2606_05981_b200 as te
     w, blob, tl, T, emb, ch = H.workload_inputs(2)
@@ -811,6 +809,7 @@ def test_side_stream_under_foreign_load_is_bitwise_identical(H, case):
         emb = np.random.default_rng(17).standard_normal((T, m.hidden)).astype(np.float32)
     B = len(tl)
     g = H.GpuTE(m, B, T, blob)
+    te.te_set_option(g.enc.h, te.TE_OPT_SM_BUDGET, budget)
     solo = g.encode(emb, tl, w.grid_h, w.grid_w)
     e, lens, out = g._keep
     a = torch.randn(4096, 4096, device="cuda", dtype=torch.bfloat16)
@@ -833,6 +832,52 @@ def test_side_stream_under_foreign_load_is_bitwise_identical(H, case):
         torch.cuda.synchronize()
         assert np.array_equal(out.cpu().numpy(), solo)
     assert te.te_query_async_error(g.enc.h) == te.TE_OK
+    g.close()
+
+
+@pytest.mark.parametrize("budget", [74, 112, 16])
+def test_sm_budget_changes_the_grids_not_the_results(H, O, budget):
+    """TE_OPT_SM_BUDGET (te.h): every GEMM grid and dispatch decision sized for `budget` SMs.  One full-width layer
+    against the fp64 oracle in the split-K regime (T = 128), the CTA-pair regime (T = 1024) against the full-GPU run of
+    the same handle, both bitwise repeatable; out-of-range budgets are refused."""
+    import paper_2606_05981_b200 as te
+    w, blob, tl, T, emb, ch = H.workload_inputs(2)
+    m = w.model
+    ref = O.encode(blob, W.blob_layout(m), m, emb, tl, w.grid_h, w.grid_w)
+    g = H.GpuTE(m, 8, 1024, blob)
+    full_info = None
+    tl8 = np.full(8, 64, dtype=np.int32)
+    emb8 = np.random.default_rng(17).standard_normal((1024, m.hidden)).astype(np.float32)
+    full8 = g.encode(emb8, tl8, w.grid_h, w.grid_w)
+    full_info = te.te_dispatch_info(g.enc.h)
+    te.te_set_option(g.enc.h, te.TE_OPT_SM_BUDGET, budget)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    _assert_final(PM.stack_metrics(out, ref, emb), f"sm budget {budget}, T=128")
+    assert np.array_equal(out, g.encode(emb, tl, w.grid_h, w.grid_w))
+    out8 = g.encode(emb8, tl8, w.grid_h, w.grid_w)
+    mm = PM.stack_metrics(out8, full8, emb8)
+    assert mm["update_rel_l2"] <= PM.GATE_UPDATE_REL_L2 and mm["max_row_update_rel_l2"] <= PM.GATE_ROW_UPDATE_REL_L2, mm
+    assert np.array_equal(out8, g.encode(emb8, tl8, w.grid_h, w.grid_w))
+    if budget == 74:   # 37 CTA pairs: the residual GEMMs' 128-wide tiles would need two waves -> one wave of wide tiles
+        assert te.te_dispatch_info(g.enc.h) != full_info         # (at 16 or 112 SMs only the grids shrink, not the kernels)
+    assert te.te_query_async_error(g.enc.h) == te.TE_OK
+    for bad in (1, 15, 100000, -3):
+        assert te.lib().te_set_option(g.enc.h, te.TE_OPT_SM_BUDGET, bad) == te.TE_ERR_INVALID_ARG
+    te.te_set_option(g.enc.h, te.TE_OPT_SM_BUDGET, 0)             # back to the whole GPU: bitwise the first result
+    assert np.array_equal(g.encode(emb8, tl8, w.grid_h, w.grid_w), full8)
+    g.close()
+
+
+def test_sm_budget_28_layers(H):
+    """The 28-layer stack at B = 4 under a 74-SM budget: close to the full-GPU run at the stack gates, and repeatable."""
+    import paper_2606_05981_b200 as te
+    w, blob, tl, T, emb, ch = H.workload_inputs(3)
+    g = H.GpuTE(w.model, w.n_frames, T, blob)
+    full = g.encode(emb, tl, w.grid_h, w.grid_w)
+    te.te_set_option(g.enc.h, te.TE_OPT_SM_BUDGET, 74)
+    out = g.encode(emb, tl, w.grid_h, w.grid_w)
+    assert np.array_equal(out, g.encode(emb, tl, w.grid_h, w.grid_w))
+    _assert_final(PM.stack_metrics(out, full, emb), "sm budget 74, cfg 3")
     g.close()
 
 
@@ -909,28 +954,6 @@ def test_host_path_refuses_a_frame_longer_than_the_capacity(H):
     with pytest.raises(te.TEError) as ei:
         g.enc.encode_host(2, 4, 4, emb, np.asarray([250, 10], dtype=np.int32), out)     # 16 + 250 > 256
     assert ei.value.code == te.TE_ERR_INVALID_ARG
-    g.close()
-
-
-@pytest.mark.parametrize("cfg_id", [1, 2, 3])
-def test_chained_launches_equal_separate_launches_bitwise(H, cfg_id):
-    """te_gemm_chain.cuh: the same tiles, K slices, reduction order and epilogue arithmetic as one launch per GEMM, so
-    the chained stack (O-proj -> gate/up -> down -> next QKV at T <= 128 and on the tiny stack, down -> next QKV at
-    T = 512) must reproduce the unchained one BITWISE — at cfg 3 over all 28 layers — and stay so over repeated replays
-    (the grid-barrier counters are re-armed by every launch)."""
-    w, blob, tl, T, emb, ch = H.workload_inputs(cfg_id)
-    g = H.GpuTE(w.model, w.n_frames, T, blob)
-    if g.te.lib().te_set_option(g.enc.h, g.te.TE_OPT_CHAIN, 1) == g.te.TE_ERR_UNSUPPORTED:
-        g.close()
-        pytest.skip("the chained-launch experiment is not in this build (TE_NVCC_EXTRA=-DTE_WITH_CHAIN)")
-    out = g.encode(emb, tl, w.grid_h, w.grid_w)
-    assert "chain" in g.te.te_dispatch_info(g.enc.h), g.te.te_dispatch_info(g.enc.h)
-    for _ in range(5):
-        assert np.array_equal(out, g.encode(emb, tl, w.grid_h, w.grid_w))
-    g.te.te_set_option(g.enc.h, g.te.TE_OPT_CHAIN, 0)
-    plain = g.encode(emb, tl, w.grid_h, w.grid_w)
-    assert "chain" not in g.te.te_dispatch_info(g.enc.h)
-    assert np.array_equal(out, plain)
     g.close()
 
 
