@@ -15,7 +15,10 @@
  * Conventions.  Plain C, no torch types.  Every pointer argument says HOST or DEVICE.  All
  * functions return 0 (TE_OK) or a negative te_status; none throws, aborts or prints.
  * The library is single-GPU; a handle must not be used from two host threads at once, different handles may be
- * (all launch state is per handle).  The small-batch (split-K) kernels
+ * (all launch state is per handle).  One handle serves ONE stream at a time: every call works in the handle's single
+ * workspace (residual, q/k/v, activations) and refreshes its single block of per-call parameters on the stream it is
+ * given, so a call enqueued on stream B while an earlier call of the same handle may still be running on stream A
+ * races with it — order them with an event, or use one handle per stream.  The small-batch (split-K) kernels
  * synchronise the CTAs of a group through device memory; they are launched as cooperative grids
  * (all CTAs resident at once, at most one CTA per SM), so other work on the GPU — another handle
  * on another stream, a denoiser (bench.py --overlap) — can delay them but not deadlock them.  There is NO CPU fallback:

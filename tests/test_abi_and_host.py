@@ -126,8 +126,6 @@ dist.destroy_process_group()
 ''' % ROOT
     env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29533")
     r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
-                        "--master-addr", "127.0.0.1", "--master-port", "29533", "-c", code] if False else
-                       [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
                         "--master-addr", "127.0.0.1", "--master-port", "29533", "--no-python",
                         sys.executable, "-c", code],
                        capture_output=True, text=True, env=env, timeout=240)
