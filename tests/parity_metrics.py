@@ -42,13 +42,17 @@ GATE_TAP_REL_L2 = 1e-2
 # cfg-3 shape, after 1 / 2 / 4 / 8 / 14 / 28 layers: update 0.9 / 1.1 / 1.4 / 1.7 / 2.1 / 2.5 e-2, max row 2.4 / 3.2 /
 # 6.2 / 6.2 / 8.3 / 9.7 e-2 over 256 rows, max |err| / rms 0.10 / 0.11 / 0.21 / 0.25 / 0.33 / 0.37).  Shallow gates
 # (one or two layers, teacher-forced layers at any depth) keep >= 3x over the 1-2 layer floor; the full-depth gates
-# keep >= 2x over the 28-layer floor.  What certifies the deep stack layer by layer is the teacher-forced test.
+# are 2x the 28-layer floor of that emulation (2.5e-2 / 9.7e-2 / 0.37 -> 5e-2 / 0.2 / 0.75; round 3, was 6e-2 / 0.3 / 1.2).
+# Measured on the B200 at full depth (cfg 3 / 4 / 5 MXFP8, cfg 4 MXFP4; deterministic): update 2.5 - 2.6e-2, max row
+# 0.10 - 0.15, max |err| / rms 0.32 - 0.55.  A full-depth gate can only say "no gross defect": depth is certified
+# LAYER BY LAYER by the teacher-forced all-rows tests (test_one_layer_every_row_full_size_mxfp8 / _mxfp4: every row of
+# one layer at full size against the oracle on the same input, shallow gates) and by the bit-exact quantiser tests.
 GATE_MX_UPDATE_REL_L2 = 5e-2
 GATE_MX_ROW_UPDATE_REL_L2 = 9e-2
 GATE_MX_MAXABS_UPDATE_OVER_RMS = 4e-1
-GATE_MX_DEEP_UPDATE_REL_L2 = 6e-2
-GATE_MX_DEEP_ROW_UPDATE_REL_L2 = 3e-1
-GATE_MX_DEEP_MAXABS_UPDATE_OVER_RMS = 1.2
+GATE_MX_DEEP_UPDATE_REL_L2 = 5e-2
+GATE_MX_DEEP_ROW_UPDATE_REL_L2 = 2e-1
+GATE_MX_DEEP_MAXABS_UPDATE_OVER_RMS = 0.75
 GATE_MX_TAP_REL_L2 = 4e-2          # dequantised attn / act taps (code flips); q/k/v of layer 0 use GATE_TAP_REL_L2
 
 
