@@ -409,8 +409,14 @@ cudaError_t launch_gemmk(const LaunchCtx& lc, const CUtensorMap& tmA, const CUte
                          cudaStream_t st) {
   switch (p.splits == 1 ? 0 : te::gemmk_variant(EPI, p.splits * (BN / 128))) {
     case 0: return launch_gemmk_var<BN, EPI, DH, 0>(lc, tmA, tmB, p, st);
-    case 1: return launch_gemmk_var<BN, EPI, DH, 1>(lc, tmA, tmB, p, st);
-    case 2: return launch_gemmk_var<BN, EPI, DH, 2>(lc, tmA, tmB, p, st);
+    // variants 1 and 2 (two / three partial tiles per row batch) exist for the residual, SwiGLU and plain epilogues only:
+    // gemmk_variant never selects them for EPI_QKV, so they are not instantiated for it
+    case 1:
+      if constexpr (EPI != te::EPI_QKV) return launch_gemmk_var<BN, EPI, DH, 1>(lc, tmA, tmB, p, st);
+      else return cudaErrorInvalidValue;
+    case 2:
+      if constexpr (EPI != te::EPI_QKV) return launch_gemmk_var<BN, EPI, DH, 2>(lc, tmA, tmB, p, st);
+      else return cudaErrorInvalidValue;
     case 3: return launch_gemmk_var<BN, EPI, DH, 3>(lc, tmA, tmB, p, st);
     case 4: return launch_gemmk_var<BN, EPI, DH, 4>(lc, tmA, tmB, p, st);
     case 5: return launch_gemmk_var<BN, EPI, DH, 5>(lc, tmA, tmB, p, st);
@@ -470,7 +476,8 @@ cudaError_t set_gemm_attr() {
   e = cudaFuncSetAttribute(te::te_gemmk_kernel<BN, EPI, DH, V>, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
                            te::GemmKCfg<BN, EPI>::SMEM_BYTES);                                                      \
   if (e != cudaSuccess) return e
-    TE_KATTR(0); TE_KATTR(1); TE_KATTR(2); TE_KATTR(3); TE_KATTR(4); TE_KATTR(5); TE_KATTR(6);
+    TE_KATTR(0); TE_KATTR(3); TE_KATTR(4); TE_KATTR(5); TE_KATTR(6);
+    if constexpr (EPI != te::EPI_QKV) { TE_KATTR(1); TE_KATTR(2); }  // (launch_gemmk: never selected for EPI_QKV)
 #undef TE_KATTR
   }
   return cudaFuncSetAttribute(te::te_gemm2_kernel<BN, EPI, DH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
